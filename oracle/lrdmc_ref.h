@@ -1,0 +1,87 @@
+/* oracle/lrdmc_ref.h -- interface of the CPU FP64 ORACLE for load-balanced LRDMC.
+ *
+ * TEST INFRASTRUCTURE, NOT PRODUCT.  Only tests/, __graft_entry__.smoke() and bench.py's
+ * cpu_baseline / --impl reference legs may build, load or call this.  It shares no code, header,
+ * table or constant generator with the CUDA path (paper_2508_12033_b200/csrc, include/lrdmc.h).
+ *
+ * Everything is host memory, plain C, FP64.  Citations are PAPER.md line numbers (L...) plus the
+ * equation / algorithm; "Qn" are the readings of silent or garbled passages listed in DESIGN.md.
+ */
+#ifndef LRDMC_REF_H
+#define LRDMC_REF_H
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct lrdmc_ref_ctx lrdmc_ref_ctx;
+
+enum { LRDMC_REF_OK = 0, LRDMC_REF_EINVAL = -1, LRDMC_REF_ESINGULAR = -2, LRDMC_REF_ESTATE = -3 };
+enum { LRDMC_REF_BALANCED = 0, LRDMC_REF_CONVENTIONAL = 1 };
+
+/* per-cycle record: Eq.34 (L227) / Eq.20 (L135) numerator and denominator, Eq.16 (L115) wbar */
+typedef struct {
+    double wbar, num, den;
+    int64_t moves_min, moves_max, moves_sum;
+    int64_t n_node_flag, n_nonpos_diag, n_nonfinite;
+    double lockstep_idle_frac; /* 1 - sum_k n_k / (N_w max_k n_k): what a lock-step batch would idle */
+} lrdmc_ref_stats;
+
+/* System description (all arrays copied).  pp == NULL: all-electron; else [n_nuc][4] local
+ * pseudopotential parameters (alpha, beta, gamma, delta), alpha <= 0 meaning a bare Coulomb nucleus.
+ * shell type: 0/1/2 = cartesian s/p/d Gaussian primitive, 10 = Slater-type s.  C_up [n_ao][n_up],
+ * C_dn [n_ao][n_dn], row-major.  c1/b1 == NULL: no one-body Jastrow.  a2 == 0: single mesh. */
+int lrdmc_ref_create(lrdmc_ref_ctx **out, int n_nuc, const double *Z, const double *Rnuc, const double *pp,
+                     int n_up, int n_dn, int n_shell, const int *center, const int *type, const double *zeta,
+                     int n_ao, const double *C_up, const double *C_dn, double a_par, double a_anti, double b2,
+                     const double *c1, const double *b1, double a, double a2, uint64_t seed);
+void lrdmc_ref_destroy(lrdmc_ref_ctx *);
+int lrdmc_ref_n_candidates(const lrdmc_ref_ctx *); /* P = 6 N n_mesh */
+
+/* walkers */
+int lrdmc_ref_set_positions(lrdmc_ref_ctx *, int n_w, const double *r /*[n_w][N][3]*/);
+int lrdmc_ref_get_state(const lrdmc_ref_ctx *, double *r, double *dinv_up, double *dinv_dn, double *w);
+int lrdmc_ref_set_state(lrdmc_ref_ctx *, int n_w, const double *r, const double *dinv_up, const double *dinv_dn,
+                        const double *w);
+int lrdmc_ref_get_obs(const lrdmc_ref_ctx *, double *eL, double *W, double *omega, int64_t *n_moves);
+
+/* the path: Alg.2 (L389-L423) / Alg.1 (L311-L387) inner loops, Eq.15-17 branching, Eq.20/34 sums */
+int lrdmc_ref_propagate(lrdmc_ref_ctx *, int mode, int n_moves, double tau, double E0, uint64_t cycle);
+int lrdmc_ref_reconfigure(lrdmc_ref_ctx *, uint64_t cycle, int32_t *parents_out /*nullable*/);
+int lrdmc_ref_estimators(const lrdmc_ref_ctx *, lrdmc_ref_stats *out);
+int lrdmc_ref_set_threads(int n); /* OpenMP threads over walkers; returns the count in effect */
+
+/* one evaluation + selection for every walker at (cycle, step), no state change.
+ * scal[k][8] = { bbar, V_sf, W, e_L, b_x = bbar/(W-E0), tau_xi = -log1p(-u_tau)/bbar (unclipped),
+ *                node flag (0/1), selection margin min_j |t - C_j| / C_{P-1} } */
+int lrdmc_ref_step_debug(const lrdmc_ref_ctx *, double E0, uint64_t cycle, uint64_t step, double *R /*[n_w][P]*/,
+                         double *scal /*[n_w][8]*/, int32_t *jstar /*[n_w]*/);
+
+/* ---- primitives exported so the pins can reach every part on its own ---- */
+void lrdmc_ref_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);
+double lrdmc_ref_uniform53(uint32_t lo, uint32_t hi);
+void lrdmc_ref_draws(const lrdmc_ref_ctx *, uint32_t slot, uint64_t cycle, uint64_t step,
+                     double u[5] /*u1,u2,u3,u_sel,u_tau*/);
+void lrdmc_ref_frame(double u1, double u2, double u3, double U[9] /*row-major, columns = versors*/);
+uint32_t lrdmc_ref_comb_r32(const lrdmc_ref_ctx *, uint64_t cycle);
+int lrdmc_ref_comb(int n_w, const double *w, uint32_t r32, int32_t *parents, double *wbar, uint64_t *u_out /*nullable [n_w]*/,
+                   uint64_t *T_out /*nullable*/, int *sh_out /*nullable*/);
+int lrdmc_ref_ao(const lrdmc_ref_ctx *, const double r[3], double *val, double *grad /*[n_ao][3]*/, double *lap);
+int lrdmc_ref_mo(const lrdmc_ref_ctx *, int spin, const double r[3], double *val, double *grad /*[O][3]*/, double *lap);
+/* log|Psi_G| and sign from scratch (pivoted LU of the Slater matrices + full Jastrow double sum) */
+int lrdmc_ref_logpsi(const lrdmc_ref_ctx *, const double *x /*[N][3]*/, double *logabs, int *sign);
+/* Slater inverses from positions (a13); returns LRDMC_REF_ESINGULAR on a zero pivot */
+int lrdmc_ref_build_inverse(const lrdmc_ref_ctx *, const double *x, double *dinv_up, double *dinv_dn);
+/* one evaluation C2 at x with given inverses (NULL: built from x) and frame U.
+ * scal[10] = { bbar, V_sf, W, e_L, node, V_ee, V_ii, K_diag = sum_j kappa_j, n_vmax_fired, e_L_continuum (D7 rhs) }
+ * per-electron per[N][5] = { T_i, lap_i = nabla_i^2 Psi/Psi, v_ei(r_i), v_zv_i, v^a_ei_i } */
+int lrdmc_ref_evaluate(const lrdmc_ref_ctx *, const double *x, const double *dinv_up, const double *dinv_dn,
+                       const double U[9], double *R /*[P]*/, double *scal /*[10]*/, double *per /*[N][5]*/,
+                       double *cand /*nullable [P][3] candidate positions*/);
+/* heat-bath selection C4 on q_j = kappa_j max(R_j, 0) */
+int lrdmc_ref_select(const lrdmc_ref_ctx *, const double *R, double u_sel, double *margin /*nullable*/);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

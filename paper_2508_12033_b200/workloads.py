@@ -1,0 +1,217 @@
+"""Seeded synthetic input generators shared by the oracle, the CUDA path, the tests and bench.py.
+
+This module holds NONE of the method's arithmetic: it only draws the arrays that describe a
+system (nuclei, shells, MO coefficients, Jastrow / pseudopotential parameters, lattice spacing) and
+the initial walker positions, with numpy only.  Both `oracle/` and the CUDA binding consume the
+plain dict it returns; neither imports the other.
+
+The five configurations are the ones listed in BASELINE.json `configs` (SURVEY.md section 8, table
+"Config shorthand", and section 8(d) "Inputs").  The paper's own workloads (water-methane with ccECP /
+cc-pVTZ and PySCF trial wavefunctions; benzene, L279-L285) are not available; these
+synthetic systems take their shapes (electron count, nuclei count, basis size, N_w, a, moves per
+branching) and nothing else.
+"""
+from __future__ import annotations
+
+import numpy as np
+
+# shell type codes (the C-ABI and the oracle use the same integers; PAPER.md names the basis only,
+# L242/L285 -- the functional forms are DESIGN.md reading Q14)
+SHELL_S, SHELL_P, SHELL_D, SHELL_SLATER_S = 0, 1, 2, 10
+_AO_PER_SHELL = {SHELL_S: 1, SHELL_P: 3, SHELL_D: 6, SHELL_SLATER_S: 1}
+
+PHILOX_RUN_SEED = 12345
+
+
+def n_ao_of(types) -> int:
+    return int(sum(_AO_PER_SHELL[int(t)] for t in types))
+
+
+def _system(name, Z, R, n_up, n_dn, center, stype, zeta, C_up, C_dn, jastrow, a, a2=0.0, pp=None,
+            n_walkers=0, cycles=0, moves=0, seed=PHILOX_RUN_SEED):
+    Z = np.ascontiguousarray(Z, dtype=np.float64)
+    R = np.ascontiguousarray(R, dtype=np.float64).reshape(-1, 3)
+    d = dict(
+        name=name,
+        Z=Z, R=R, n_nuc=int(Z.shape[0]), n_up=int(n_up), n_dn=int(n_dn),
+        pp=None if pp is None else np.ascontiguousarray(pp, dtype=np.float64).reshape(-1, 4),
+        shell_center=np.ascontiguousarray(center, dtype=np.int32),
+        shell_type=np.ascontiguousarray(stype, dtype=np.int32),
+        shell_zeta=np.ascontiguousarray(zeta, dtype=np.float64),
+        n_shell=int(len(center)), n_ao=n_ao_of(stype),
+        C_up=np.ascontiguousarray(C_up, dtype=np.float64),
+        C_dn=np.ascontiguousarray(C_dn, dtype=np.float64),
+        a_par=float(jastrow.get("a_par", 0.0)), a_anti=float(jastrow.get("a_anti", 0.0)),
+        b2=float(jastrow.get("b2", 1.0)),
+        c1=None if jastrow.get("c1") is None else np.ascontiguousarray(jastrow["c1"], dtype=np.float64),
+        b1=None if jastrow.get("b1") is None else np.ascontiguousarray(jastrow["b1"], dtype=np.float64),
+        a=float(a), a2=float(a2), seed=int(seed),
+        n_walkers=int(n_walkers), cycles=int(cycles), moves=int(moves),
+    )
+    assert d["C_up"].shape == (d["n_ao"], d["n_up"])
+    assert d["C_dn"].shape == (d["n_ao"], d["n_dn"])
+    return d
+
+
+def _round_robin_shells(rng, n_nuc, n_shell):
+    center = np.arange(n_shell) % n_nuc
+    stype = np.array([(SHELL_S, SHELL_P, SHELL_D)[k % 3] for k in range(n_shell)])
+    zeta = np.exp(rng.uniform(np.log(0.1), np.log(20.0), size=n_shell))
+    return center, stype, zeta
+
+
+def _orthonormal_mos(rng, n_ao, n_occ):
+    q, _ = np.linalg.qr(rng.standard_normal((n_ao, n_occ)))
+    return np.ascontiguousarray(q[:, :n_occ])
+
+
+def _separated_points(rng, n, draw, min_sep):
+    pts = []
+    while len(pts) < n:
+        p = draw()
+        if all(np.linalg.norm(p - q) >= min_sep for q in pts):
+            pts.append(p)
+    return np.array(pts)
+
+
+def initial_walkers(sysd, n_walkers, seed):
+    """Q18: each electron starts at a nucleus chosen with probability ~ Z plus a
+    N(0, 1 bohr) offset.  Config C1 overrides this (uniform cube).  Returns [n_w][N][3] float64."""
+    rng = np.random.default_rng(seed)
+    N = sysd["n_up"] + sysd["n_dn"]
+    p = sysd["Z"] / sysd["Z"].sum()
+    which = rng.choice(sysd["n_nuc"], size=(n_walkers, N), p=p)
+    return np.ascontiguousarray(sysd["R"][which] + rng.standard_normal((n_walkers, N, 3)))
+
+
+def hydrogen(alpha=0.9, a=0.2, n_walkers=256, cycles=200, moves=40, seed=PHILOX_RUN_SEED):
+    """C1: H atom, one electron, Z=1 at the origin, psi = exp(-alpha r), no Jastrow."""
+    return _system("C1-hydrogen", [1.0], [[0.0, 0.0, 0.0]], 1, 0, [0], [SHELL_SLATER_S], [alpha],
+                   np.ones((1, 1)), np.zeros((1, 0)), {}, a,
+                   n_walkers=n_walkers, cycles=cycles, moves=moves, seed=seed)
+
+
+def hydrogen_walkers(n_walkers=256, seed=1):
+    """C1 start: uniform in the 2-bohr cube [-1, 1]^3 (BASELINE.json configs[0])."""
+    rng = np.random.default_rng(seed)
+    return np.ascontiguousarray(rng.uniform(-1.0, 1.0, size=(n_walkers, 1, 3)))
+
+
+def slater_atom(Z, zetas, n_up, n_dn, C_up, C_dn, a, jastrow=None, name="slater-atom"):
+    """Small all-electron atom on Slater-type s orbitals at the origin (pins P7/P8: He singlet and
+    He 2^3S).  Not one of the BASELINE configs; used by the oracle's physics pins and GPU parity."""
+    ns = len(zetas)
+    return _system(name, [float(Z)], [[0.0, 0.0, 0.0]], n_up, n_dn, [0] * ns, [SHELL_SLATER_S] * ns,
+                   zetas, C_up, C_dn, jastrow or {}, a)
+
+
+def slater_molecule(Z, R, zetas, centers, n_up, n_dn, C_up, C_dn, a, jastrow=None, name="slater-mol"):
+    """Small all-electron molecule on Slater-type s orbitals (pin P7: H2)."""
+    return _system(name, Z, R, n_up, n_dn, centers, [SHELL_SLATER_S] * len(zetas), zetas, C_up, C_dn,
+                   jastrow or {}, a)
+
+
+def synthetic10(a=0.2, n_walkers=1024, cycles=100, moves=50, seed=PHILOX_RUN_SEED):
+    """C2: 10 electrons (5/5), nuclei Z = 6, 2, 2 inside a 3-bohr ball, 60 s/p/d GTOs (18 shells),
+    random orthonormal MOs, one- and two-body Pade Jastrow with b = 1."""
+    rng = np.random.default_rng(2)
+
+    def draw():
+        while True:
+            p = rng.uniform(-3.0, 3.0, size=3)
+            if np.linalg.norm(p) <= 3.0:
+                return p
+    R = _separated_points(rng, 3, draw, 1.0)
+    Z = np.array([6.0, 2.0, 2.0])
+    center, stype, zeta = _round_robin_shells(rng, 3, 18)
+    C = _orthonormal_mos(rng, n_ao_of(stype), 5)
+    jas = dict(a_par=0.25, a_anti=0.5, b2=1.0, c1=Z.copy(), b1=np.ones(3))
+    return _system("C2-synthetic10", Z, R, 5, 5, center, stype, zeta, C, C.copy(), jas, a,
+                   n_walkers=n_walkers, cycles=cycles, moves=moves, seed=seed)
+
+
+def _water_methane_geometry(rng):
+    # equilibrium-LIKE template (generic bond lengths/angles), jittered; not a published geometry
+    oh, hoh = 1.81, np.deg2rad(104.5)
+    O = np.zeros(3)
+    H1 = oh * np.array([np.sin(hoh / 2), 0.0, np.cos(hoh / 2)])
+    H2 = oh * np.array([-np.sin(hoh / 2), 0.0, np.cos(hoh / 2)])
+    Cc = np.array([0.0, 0.0, -6.5])
+    ch = 2.05
+    t = np.array([[1, 1, 1], [1, -1, -1], [-1, 1, -1], [-1, -1, 1]], dtype=float) / np.sqrt(3.0)
+    Hc = Cc + ch * t
+    R = np.vstack([O, Cc, H1, H2, Hc])
+    return R + rng.normal(0.0, 0.05, size=R.shape)
+
+
+def water_methane(a=0.2, n_walkers=400, cycles=200, moves=100, seed=PHILOX_RUN_SEED, name=None):
+    """C3/C4: water-methane-SHAPED complex: 16 valence electrons (8/8); O, C, 6 H with effective
+    charges 6, 4, 1 and a local Gaussian pseudopotential per nucleus; 200 s/p/d GTOs (60 shells)."""
+    rng = np.random.default_rng(3)
+    R = _water_methane_geometry(rng)
+    Z = np.array([6.0, 4.0] + [1.0] * 6)
+    center, stype, zeta = _round_robin_shells(rng, 8, 60)
+    C = _orthonormal_mos(rng, n_ao_of(stype), 8)
+    # local PP parameters (alpha, beta, gamma, delta) per nucleus, reading Q14
+    alpha = np.exp(rng.uniform(0.0, np.log(10.0), size=8))
+    beta = np.exp(rng.uniform(0.0, np.log(10.0), size=8))
+    delta = np.exp(rng.uniform(0.0, np.log(10.0), size=8))
+    gamma = rng.uniform(0.0, 2.0 * Z)
+    pp = np.stack([alpha, beta, gamma, delta], axis=1)
+    jas = dict(a_par=0.25, a_anti=0.5, b2=1.0, c1=np.full(8, 0.5), b1=np.ones(8))
+    return _system(name or f"C3-water-methane-shaped-Nw{n_walkers}", Z, R, 8, 8, center, stype, zeta,
+                   C, C.copy(), jas, a, pp=pp, n_walkers=n_walkers, cycles=cycles, moves=moves, seed=seed)
+
+
+def water_methane_full(a=0.2, seed=PHILOX_RUN_SEED):
+    """C4: the C3 system scaled to fill one B200: N_w = 25600, 500 cycles x 100 moves."""
+    return water_methane(a=a, n_walkers=25600, cycles=500, moves=100, seed=seed,
+                         name="C4-water-methane-shaped-Nw25600")
+
+
+def cluster64(a=0.2, a2=0.4, n_walkers=4096, cycles=200, moves=200, seed=PHILOX_RUN_SEED):
+    """C5: 64 electrons (32/32), 24 all-electron nuclei with Z in {1, 4, 6} (sum 64) in a 12-bohr
+    box, 600 s/p/d GTOs (180 shells), double lattice spacing a / a'."""
+    rng = np.random.default_rng(5)
+    R = _separated_points(rng, 24, lambda: rng.uniform(0.0, 12.0, size=3), 1.5)
+    while True:
+        Z = rng.choice([1.0, 4.0, 6.0], size=24)
+        if Z.sum() == 64.0:
+            break
+    center, stype, zeta = _round_robin_shells(rng, 24, 180)
+    C = _orthonormal_mos(rng, n_ao_of(stype), 32)
+    jas = dict(a_par=0.25, a_anti=0.5, b2=1.0, c1=Z.copy(), b1=np.ones(24))
+    return _system("C5-cluster64", Z, R, 32, 32, center, stype, zeta, C, C.copy(), jas, a, a2=a2,
+                   n_walkers=n_walkers, cycles=cycles, moves=moves, seed=seed)
+
+
+def tiny_molecule(n_up=2, n_dn=1, n_nuc=2, n_shell=6, seed=7, a=0.2, a2=0.0, with_pp=False):
+    """A few-electron s/p/d system for brute-force pins (P3) and ragged-shape parity cases."""
+    rng = np.random.default_rng(seed)
+    R = _separated_points(rng, n_nuc, lambda: rng.uniform(-1.5, 1.5, size=3), 1.0)
+    Z = rng.choice([1.0, 2.0, 3.0], size=n_nuc)
+    center, stype, zeta = _round_robin_shells(rng, n_nuc, n_shell)
+    zeta = np.exp(rng.uniform(np.log(0.2), np.log(3.0), size=n_shell))
+    n_ao = n_ao_of(stype)
+    C_up = _orthonormal_mos(rng, n_ao, n_up)
+    C_dn = _orthonormal_mos(rng, n_ao, n_dn) if n_dn else np.zeros((n_ao, 0))
+    pp = None
+    c1 = Z.copy()
+    if with_pp:
+        pp = np.stack([np.exp(rng.uniform(0.0, np.log(10.0), size=n_nuc)),
+                       np.exp(rng.uniform(0.0, np.log(10.0), size=n_nuc)),
+                       rng.uniform(0.0, 2.0 * Z),
+                       np.exp(rng.uniform(0.0, np.log(10.0), size=n_nuc))], axis=1)
+        c1 = np.full(n_nuc, 0.5)
+    jas = dict(a_par=0.25, a_anti=0.5, b2=0.8, c1=c1, b1=rng.uniform(0.5, 1.5, size=n_nuc))
+    return _system(f"tiny-{n_up}u{n_dn}d", Z, R, n_up, n_dn, center, stype, zeta, C_up, C_dn, jas, a,
+                   a2=a2, pp=pp)
+
+
+CONFIGS = {
+    "C1": hydrogen,
+    "C2": synthetic10,
+    "C3": water_methane,
+    "C4": water_methane_full,
+    "C5": cluster64,
+}
