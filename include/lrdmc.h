@@ -1,0 +1,151 @@
+/* include/lrdmc.h -- C-ABI of liblrdmc.so: the data-parallel hot path of load-balanced LRDMC
+ * (arxiv 2508.12033, Nakano / Sorella / Casula) on one NVIDIA B200 (sm_100a), FP64.
+ *
+ * Citations "L<n>" are line numbers of the paper text with the equation / algorithm they
+ * fall in; "Qn" are the readings of silent or garbled passages listed in DESIGN.md.
+ *
+ * Conventions
+ *   - Every function returns int: 0 = LRDMC_OK, < 0 = hard error (nothing modified unless stated).
+ *   - "host"   pointer: ordinary CPU memory, read or written synchronously inside the call.
+ *   - "device" pointer: CUDA device memory of the current device; used asynchronously on `stream`
+ *     (a cudaStream_t passed as void*, NULL = legacy default stream).  The caller keeps such buffers alive
+ *     until the stream has passed the call.
+ *   - The library owns only the ctx (and small device tables inside it).  Walker storage is CALLER-owned
+ *     device memory handed over with lrdmc_bind_walkers (e.g. a torch tensor).
+ *   - No CPU fallback exists: without a CUDA device every call that needs one returns LRDMC_ECUDA.
+ *   - Soft numerical events (W(x)-E_0 <= 0, node flags, non-finite weights) are counted in
+ *     lrdmc_cycle_stats, never returned as errors.
+ *   - Electron order: the n_up spin-up electrons first, then the n_dn spin-down ones.
+ *   - Candidate (off-diagonal move) order: j = mesh*6N + 6*i + d, d = 0..5 <-> (+e1,-e1,+e2,-e2,+e3,-e3),
+ *     e_k = k-th column of the step's random frame U (Eq.D3-D4).
+ */
+#ifndef LRDMC_H
+#define LRDMC_H
+#include <stddef.h>
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct lrdmc_ctx lrdmc_ctx; /* opaque; created by lrdmc_init, destroyed by lrdmc_free */
+
+enum { LRDMC_OK = 0, LRDMC_EINVAL = -1, LRDMC_ESINGULAR = -2, LRDMC_ESTATE = -3, LRDMC_ECUDA = -4, LRDMC_ENOMEM = -5 };
+enum { LRDMC_BALANCED = 0, LRDMC_CONVENTIONAL = 1 };
+enum { LRDMC_SHELL_S = 0, LRDMC_SHELL_P = 1, LRDMC_SHELL_D = 2, LRDMC_SHELL_SLATER_S = 10 };
+#define LRDMC_MAX_OCC 32 /* occupied MOs per spin supported by the kernels */
+
+/* ---- problem statement (all arrays are HOST pointers and are COPIED by lrdmc_init) -------------------- */
+typedef struct {
+    int n_nuc;
+    const double *Z;  /* [n_nuc] charge (Z, or Z_eff for a pseudo-atom) */
+    const double *R;  /* [n_nuc][3] bohr */
+    int n_up, n_dn;   /* n_up >= 1, n_dn >= 0, each <= LRDMC_MAX_OCC */
+    const double *pp; /* NULL = all bare nuclei; else [n_nuc][4] = (alpha,beta,gamma,delta) of the local
+                         pseudopotential v(r) = -(Z/r)(1-e^{-alpha r^2}) + Z alpha r e^{-beta r^2} + gamma e^{-delta r^2}
+                         (reading Q14); alpha <= 0 marks a bare -Z/r nucleus */
+} lrdmc_system;
+typedef struct {
+    int n_shell;
+    const int *center;  /* [n_shell] nucleus index */
+    const int *type;    /* [n_shell] LRDMC_SHELL_*: cartesian Gaussian primitives s (1 AO), p (x,y,z),
+                           d (xx,xy,xz,yy,yz,zz), each normalised to unit self-overlap; or Slater s exp(-zeta r) */
+    const double *zeta; /* [n_shell] > 0 */
+} lrdmc_basis;
+typedef struct {
+    int n_ao;                 /* must equal the AO count implied by the shells */
+    const double *C_up, *C_dn; /* [n_ao][n_up], [n_ao][n_dn] row-major: phi_m = sum_mu chi_mu C[mu][m] */
+} lrdmc_mo;
+typedef struct {
+    double a_par, a_anti, b2; /* two-body Pade u2 = a r/(1+b2 r), a by spin pair; a = 0 disables */
+    const double *c1, *b1;    /* [n_nuc] one-body Pade u1_I = -c1_I r/(1+b1_I r); c1 == NULL disables */
+} lrdmc_jastrow;
+typedef struct {
+    double a;      /* lattice spacing (Eq.D3) */
+    double a2;     /* 0 = single mesh; > 0 = second spacing a' of the double mesh (reading Q13, g = 1/2) */
+    uint64_t seed; /* Philox4x32-10 key; counter = (walker slot, cycle, step, purpose) (readings Q7, Q12) */
+} lrdmc_lattice;
+
+/* Psi_G = D_up D_dn exp(J) and the lattice-regularised fixed-node Hamiltonian of Appendix D (L554-L628).
+ * Builds the device tables (sorted/padded shell list, MO coefficients pre-swizzled into FP64 tensor-core
+ * B fragments with the AO norms folded in).  Errors: EINVAL (sizes, non-positive zeta/a, AO count), ECUDA, ENOMEM. */
+int lrdmc_init(lrdmc_ctx **out, const lrdmc_system *, const lrdmc_basis *, const lrdmc_mo *, const lrdmc_jastrow *,
+               const lrdmc_lattice *);
+void lrdmc_free(lrdmc_ctx *);
+const char *lrdmc_strerror(int code);
+int lrdmc_n_candidates(const lrdmc_ctx *); /* P = 6 N n_mesh */
+
+/* ---- walker storage: structure of arrays in ONE caller-owned device buffer ---------------------------
+ * positions (double-buffered for the branching gather), inverse Slater matrices per spin, cached MO
+ * value/gradient/Laplacian rows, weights, per-walker observables, reconfiguration workspace.  256-byte aligned. */
+size_t lrdmc_walker_bytes(const lrdmc_ctx *, int n_walkers);
+int lrdmc_bind_walkers(lrdmc_ctx *, void *dev_buf /*device*/, size_t bytes, int n_walkers); /* EINVAL if too small */
+
+/* Upload positions r [n_w][N][3] (device), build Dinv_sigma = D_sigma^{-1} by pivoted elimination and the MO
+ * caches (row a13), weights <- 1.  Synchronises `stream`; returns ESINGULAR if any Slater matrix had a zero pivot. */
+int lrdmc_set_positions(lrdmc_ctx *, const double *r_dev, void *stream);
+
+/* One branching interval for every walker (weights reset to 1 on entry, Alg.2 line 4 L401 / Alg.1 line 4 L350):
+ *  BALANCED     (Alg.2, Eq.28-30): exactly n_moves times { evaluate; w *= bbar/(W-E0); heat-bath hop },
+ *               then one measurement evaluation storing e_L, W and omega = w/(W-E0) (Eq.34, reading Q10).
+ *  CONVENTIONAL (Alg.1, Eq.24-25): while tau_left > 0 { evaluate; tau_xi = min(-ln(1-xi)/bbar, tau_left);
+ *               w *= exp(-tau_xi (e_L - E0)); tau_left -= tau_xi; hop unless the time ran out }, omega = w.
+ *               Here E0 is the constant reference shift (Q8b); n_moves > 0 caps the evaluations, 0 = no cap.
+ * `cycle` < 2^32 labels the random streams.  Asynchronous on `stream`. */
+int lrdmc_propagate(lrdmc_ctx *, int mode, int n_moves, double tau, double E0, uint64_t cycle, void *stream);
+
+/* Branching at fixed N_w (Eq.15-17) on the raw weights w: integer comb (prefix sum + search, indices
+ * bit-exact by construction, reading Q21), gather of the surviving walkers, weights <- 1, wbar recorded (Eq.16),
+ * inverses and caches rebuilt from the positions (reading Q15).  parents_dev (device, nullable) receives parent[k].
+ * Asynchronous on `stream`. */
+int lrdmc_reconfigure(lrdmc_ctx *, uint64_t cycle, int32_t *parents_dev, void *stream);
+
+typedef struct {
+    double wbar;     /* Eq.16: mean raw weight of the last reconfigure */
+    double num, den; /* sum_k omega_k e_L,k and sum_k omega_k of the last propagate (Eq.20 L135 / Eq.34) */
+    int64_t moves_min, moves_max, moves_sum; /* hops per walker in the last propagate */
+    int64_t n_node_flag;    /* evaluations that saw at least one R_j < 0 */
+    int64_t n_nonpos_diag;  /* evaluations with W(x)-E0 <= 0 (balanced; walker weight set to 0, reading Q16) */
+    int64_t n_nonfinite;    /* walkers whose weight left the finite range (set to 0) */
+    double lockstep_idle_frac; /* 1 - sum n_k/(N_w max n_k): idle share of a lock-step batch (L168, App. C) */
+    double barrier_idle_frac;  /* measured: 1 - sum_warps busy time / (resident warps x kernel span) */
+    float propagate_ms, reconfigure_ms; /* CUDA-event durations of the last calls on their stream */
+} lrdmc_cycle_stats;
+/* Synchronises the stream of the last propagate/reconfigure and fills *out_host (host). */
+int lrdmc_estimators(lrdmc_ctx *, lrdmc_cycle_stats *out_host);
+
+/* Host-side estimators over generations (Eq.18-19): G_n^p = prod_{j=1..p} wbar_{n-j},
+ * E = sum_n G_n^p e_n / sum_n G_n^p over n >= n_therm, e_n = num_n/den_n; sigma from a delete-one-block
+ * jackknife over n_blocks blocks of generations (reading Q9).  All pointers host. */
+int lrdmc_energy(const lrdmc_cycle_stats *recs, int n, int p, int n_therm, int n_blocks, double *E, double *sigma);
+
+/* Parity hook: one evaluation + selection for every walker at (cycle, step) with NO state change.  Device outputs:
+ * R [n_w][P]; scal [n_w][8] = { bbar, V_sf, W, e_L, b_x = bbar/(W-E0), tau_xi = -log1p(-u_tau)/bbar, node flag, u_sel };
+ * jstar [n_w] (-1: no allowed move).  Runs the same device code as lrdmc_propagate. */
+int lrdmc_step_debug(lrdmc_ctx *, double E0, uint64_t cycle, uint64_t step, double *R_dev, double *scal_dev,
+                     int32_t *jstar_dev, void *stream);
+
+/* State access (device arrays, any may be NULL): r [n_w][N][3], dinv_up [n_w][n_up][n_up], dinv_dn [n_w][n_dn][n_dn]
+ * with Dinv[m][i] (sum_m D[i][m] Dinv[m][k] = delta_ik), w [n_w]. set_state with dinv == NULL rebuilds the inverses. */
+int lrdmc_get_walkers(lrdmc_ctx *, double *r_dev, double *dinv_up_dev, double *dinv_dn_dev, double *w_dev, void *stream);
+int lrdmc_set_state(lrdmc_ctx *, const double *r_dev, const double *dinv_up_dev, const double *dinv_dn_dev,
+                    const double *w_dev, void *stream);
+/* Per-walker observables of the last propagate (device, nullable): e_L, W, omega [n_w] doubles; n_moves [n_w] int64 */
+int lrdmc_get_obs(lrdmc_ctx *, double *eL_dev, double *W_dev, double *omega_dev, int64_t *n_moves_dev, void *stream);
+
+/* End-to-end convenience with HOST buffers: H2D of r_in [n_w][N][3], set_positions, n_cycles x (propagate,
+ * reconfigure, estimators -> stats_out[c], E0 feedback as running mean of e_n when mode is balanced), D2H of the
+ * final positions into r_out (nullable).  Walkers must be bound.  Synchronous. */
+int lrdmc_run_host(lrdmc_ctx *, const double *r_in_host, double *r_out_host, int mode, int n_moves, double tau, double E0,
+                   uint64_t first_cycle, int n_cycles, lrdmc_cycle_stats *stats_out_host, void *stream);
+
+/* Roofline denominators measured on this device ("measure DFMA and DMMA peaks on the box"):
+ * TFLOP/s of independent FP64 FMA chains, of mma.sync m8n8k4 f64 chains, and of both issued together. Host outputs. */
+int lrdmc_measure_fp64_peaks(double *dfma_tflops, double *dmma_tflops, double *mixed_tflops);
+
+/* Test hook for pin P11: fills out_dev [n][4] (uint32) with Philox4x32-10 blocks for counters ctr_dev [n][4], key[2]. */
+int lrdmc_debug_philox(const uint32_t *ctr_dev, uint32_t key0, uint32_t key1, uint32_t *out_dev, int n, void *stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

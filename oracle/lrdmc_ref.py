@@ -119,8 +119,12 @@ class Ref:
         self.n_w = 0
 
     def __del__(self):
-        if getattr(self, "h", None):
-            lib().lrdmc_ref_destroy(self.h); self.h = None
+        if getattr(self, "h", None) and _lib is not None:
+            try:
+                _lib.lrdmc_ref_destroy(self.h)
+            except Exception:       # interpreter shutdown
+                pass
+            self.h = None
 
     # ---- walkers ----
     def set_positions(self, r):

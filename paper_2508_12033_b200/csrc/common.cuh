@@ -1,0 +1,66 @@
+// common.cuh -- shared device/host declarations of liblrdmc (CUDA path; shares nothing with oracle/).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "../../include/lrdmc.h"
+
+#define LRDMC_NUC_STRIDE 12   // doubles per nucleus row: Rx Ry Rz Z c1 b1 alpha beta gamma delta is_pp pad
+#define LRDMC_EL_ARRAYS 6     // per-electron scratch arrays in shared memory: Jold vei vb lap T spare
+
+// Everything a kernel needs to know about the system; passed by value (fits the 4 KB parameter space).
+struct DevSys {
+    int N, n_up, n_dn, n_nuc, P, n_mesh;
+    int n_it[4];          // DMMA k-iterations (4 shells each) per shell group: 0 Slater-s, 1 s, 2 p, 3 d
+    int n_slots;          // 4 * sum n_it  (sorted + padded shell list)
+    int n_ksteps;         // n_it[0] + n_it[1] + 3 n_it[2] + 6 n_it[3]  = (padded AO count)/4
+    int NT[2];            // 8-wide MO tiles per spin
+    int OS;               // MO stride of the cache rows, 8*max(NT)
+    int same_C;           // C_dn == C_up: one fragment table
+    int has_j1, has_pp;
+    double amesh[2], gmesh[2], kappa[2], g_over_a2[2];
+    double a_par, a_anti, b2, V_ii, Kdiag, a;
+    uint32_t key0, key1;
+    // device tables (global memory copies; staged into shared memory when they fit)
+    const double *shells;      // [n_slots][4] = cx cy cz zeta
+    const double *bfrag[2];    // [n_ksteps][NT][32] FP64 mma B fragments, AO norms folded in
+    const double *nuc;         // [n_nuc][LRDMC_NUC_STRIDE]
+    // shared-memory plan (units: doubles)
+    int bf_in_smem, moc_in_smem;
+    int off_shells, off_nuc, off_bf[2], tables_doubles;
+    int o_r, o_dinv[2], o_moc, o_R, o_cum, o_el, per_warp_doubles;
+    int dinv_rows[2];     // padded row count 8*NT
+};
+
+// Walker storage (views into the caller's buffer)
+struct DevWalk {
+    int n_w;
+    double *r;            // current positions [n_w][3N]
+    double *r_alt;        // gather target
+    double *dinv[2];      // [n_w][n_s*n_s]
+    double *moc;          // [n_w][N][5][OS] cached MO value/grad/lap rows at each electron
+    double *w, *eL, *W, *omega;
+    long long *nmoves;
+    int *flags;           // [n_w][3] node / nonpos / nonfinite counts of the last propagate
+    unsigned long long *wq, *prefix; // comb workspace
+    int *parents;
+    unsigned long long *timing;      // [max_warps][2] globaltimer start/end per resident warp
+    double *stats;        // device copy of the reduced numbers (see k_reduce_obs)
+    int *counter;         // dynamic walker queue head; [1] = singular flag
+};
+
+__device__ __forceinline__ double warp_sum(double v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+__device__ __forceinline__ double quad_sum(double v)
+{
+    v += __shfl_xor_sync(0xffffffffu, v, 1);
+    v += __shfl_xor_sync(0xffffffffu, v, 2);
+    return v;
+}
+__device__ __forceinline__ unsigned long long globaltimer_ns()
+{
+    unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t;
+}

@@ -1,0 +1,389 @@
+// lrdmc.cu -- C-ABI of liblrdmc.so (see include/lrdmc.h).  Host logic only: table construction, the shared-memory
+// plan, kernel launches, CUDA-event timing.  Every step of the path runs in the kernels of the *.cuh files.
+#include <climits>
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <vector>
+
+#include "common.cuh"
+#include "philox.cuh"
+#include "wavefunction.cuh"
+#include "evaluate.cuh"
+#include "propagate.cuh"
+#include "reconfigure.cuh"
+#include "peaks.cuh"
+#include "api_internal.h"
+
+#define CK(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) { snprintf(g_cuda_msg, sizeof g_cuda_msg, "%s at %s:%d", cudaGetErrorString(e_), __FILE__, __LINE__); return LRDMC_ECUDA; } } while (0)
+static char g_cuda_msg[256] = "";
+
+struct lrdmc_ctx {
+    DevSys S; DevWalk W;
+    void *d_tables; DevStats *d_stats;
+    int NT, wpb, ctas_per_sm, sm_count, smem_bytes, grid_max;
+    int bound, have_prop, have_reconf, state_ok;
+    cudaEvent_t ev[4]; cudaStream_t last_stream;
+    int launches;   // kernels launched so far (bench.py reports it)
+};
+
+extern "C" const char *lrdmc_strerror(int code)
+{
+    switch (code) {
+    case LRDMC_OK: return "ok";
+    case LRDMC_EINVAL: return "invalid argument";
+    case LRDMC_ESINGULAR: return "singular Slater matrix";
+    case LRDMC_ESTATE: return "call order: walkers not bound / positions not set / nothing propagated";
+    case LRDMC_ECUDA: return g_cuda_msg[0] ? g_cuda_msg : "CUDA error";
+    case LRDMC_ENOMEM: return "system does not fit the shared-memory plan";
+    default: return "unknown error";
+    }
+}
+
+static double odd_dfact(int k) { double f = 1.0; for (int j = 1; j <= k; ++j) f *= (2 * j - 1); return f; }
+static double gto_norm(double z, int l, int m, int n)
+{
+    return pow(2.0 * z / M_PI, 0.75) * pow(4.0 * z, 0.5 * (l + m + n)) / sqrt(odd_dfact(l) * odd_dfact(m) * odd_dfact(n));
+}
+static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+extern "C" int lrdmc_init(lrdmc_ctx **out, const lrdmc_system *sys, const lrdmc_basis *bas, const lrdmc_mo *mo, const lrdmc_jastrow *jas,
+                          const lrdmc_lattice *lat)
+{
+    if (!out || !sys || !bas || !mo || !jas || !lat) return LRDMC_EINVAL;
+    if (sys->n_nuc < 1 || sys->n_up < 1 || sys->n_dn < 0 || sys->n_up > LRDMC_MAX_OCC || sys->n_dn > LRDMC_MAX_OCC) return LRDMC_EINVAL;
+    if (bas->n_shell < 1 || !(lat->a > 0.0) || lat->a2 < 0.0 || !sys->Z || !sys->R || !mo->C_up || (sys->n_dn && !mo->C_dn)) return LRDMC_EINVAL;
+    int ndev = 0; CK(cudaGetDeviceCount(&ndev));
+    // ---- shells: sort by group (Slater s, s, p, d), pad each group to a multiple of 4
+    static const int ncomp[4] = { 1, 1, 3, 6 };
+    static const int lmn[4][6][3] = { { {0,0,0} }, { {0,0,0} }, { {1,0,0}, {0,1,0}, {0,0,1} }, { {2,0,0}, {1,1,0}, {1,0,1}, {0,2,0}, {0,1,1}, {0,0,2} } };
+    std::vector<int> ao0(bas->n_shell), group(bas->n_shell);
+    int n_ao = 0;
+    for (int s = 0; s < bas->n_shell; ++s) {
+        int t = bas->type[s], g = t == LRDMC_SHELL_SLATER_S ? 0 : (t == LRDMC_SHELL_S ? 1 : (t == LRDMC_SHELL_P ? 2 : (t == LRDMC_SHELL_D ? 3 : -1)));
+        if (g < 0 || bas->center[s] < 0 || bas->center[s] >= sys->n_nuc || !(bas->zeta[s] > 0.0)) return LRDMC_EINVAL;
+        group[s] = g; ao0[s] = n_ao; n_ao += ncomp[g];
+    }
+    if (n_ao != mo->n_ao) return LRDMC_EINVAL;
+    lrdmc_ctx *c = (lrdmc_ctx *)calloc(1, sizeof(lrdmc_ctx));
+    DevSys &S = c->S;
+    S.N = sys->n_up + sys->n_dn; S.n_up = sys->n_up; S.n_dn = sys->n_dn; S.n_nuc = sys->n_nuc;
+    S.n_mesh = lat->a2 > 0.0 ? 2 : 1; S.P = 6 * S.N * S.n_mesh; S.a = lat->a;
+    S.amesh[0] = lat->a; S.amesh[1] = lat->a2; S.gmesh[0] = S.n_mesh == 2 ? 0.5 : 1.0; S.gmesh[1] = S.n_mesh == 2 ? 0.5 : 0.0;
+    S.Kdiag = 0.0;
+    for (int m = 0; m < S.n_mesh; ++m) {
+        S.kappa[m] = S.gmesh[m] / (2.0 * S.amesh[m] * S.amesh[m]); S.g_over_a2[m] = S.gmesh[m] / (S.amesh[m] * S.amesh[m]);
+    }
+    for (int j = 0; j < S.P; ++j) S.Kdiag += S.kappa[j / (6 * S.N)];      // K^a_{x,x} = sum_j kappa_j = 3N/a^2 (Eq.D5)
+    S.a_par = jas->a_par; S.a_anti = jas->a_anti; S.b2 = jas->b2; S.has_j1 = jas->c1 != NULL; S.has_pp = sys->pp != NULL;
+    S.key0 = (uint32_t)lat->seed; S.key1 = (uint32_t)(lat->seed >> 32);
+    S.V_ii = 0.0;
+    for (int I = 0; I < sys->n_nuc; ++I) for (int J = I + 1; J < sys->n_nuc; ++J) {
+        double dx = sys->R[3 * I] - sys->R[3 * J], dy = sys->R[3 * I + 1] - sys->R[3 * J + 1], dz = sys->R[3 * I + 2] - sys->R[3 * J + 2];
+        S.V_ii += sys->Z[I] * sys->Z[J] / sqrt(dx * dx + dy * dy + dz * dz);
+    }
+    std::vector<int> slot_shell; int base[4];
+    for (int g = 0; g < 4; ++g) {
+        base[g] = (int)slot_shell.size();
+        for (int s = 0; s < bas->n_shell; ++s) if (group[s] == g) slot_shell.push_back(s);
+        while ((slot_shell.size() - base[g]) % 4) slot_shell.push_back(-1);
+        S.n_it[g] = ((int)slot_shell.size() - base[g]) / 4;
+    }
+    S.n_slots = (int)slot_shell.size();
+    S.n_ksteps = S.n_it[0] + S.n_it[1] + 3 * S.n_it[2] + 6 * S.n_it[3];
+    int omax = sys->n_up > sys->n_dn ? sys->n_up : sys->n_dn, nt = (omax + 7) / 8;
+    c->NT = nt <= 1 ? 1 : (nt == 2 ? 2 : 4);
+    S.NT[0] = S.NT[1] = c->NT; S.OS = 8 * c->NT; S.dinv_rows[0] = S.dinv_rows[1] = 8 * c->NT;
+    S.same_C = (sys->n_dn == 0) || (sys->n_dn == sys->n_up && (mo->C_dn == mo->C_up || !memcmp(mo->C_up, mo->C_dn, sizeof(double) * (size_t)n_ao * sys->n_up)));
+    // ---- host images of the tables
+    std::vector<double> h_sh((size_t)S.n_slots * 4), h_nuc((size_t)S.n_nuc * LRDMC_NUC_STRIDE, 0.0);
+    for (int q = 0; q < S.n_slots; ++q) {
+        int s = slot_shell[q];
+        if (s < 0) { h_sh[4 * q] = h_sh[4 * q + 1] = h_sh[4 * q + 2] = 0.0; h_sh[4 * q + 3] = 1.0; continue; }
+        const double *Rc = sys->R + 3 * bas->center[s];
+        h_sh[4 * q] = Rc[0]; h_sh[4 * q + 1] = Rc[1]; h_sh[4 * q + 2] = Rc[2]; h_sh[4 * q + 3] = bas->zeta[s];
+    }
+    for (int I = 0; I < S.n_nuc; ++I) {
+        double *nu = &h_nuc[(size_t)I * LRDMC_NUC_STRIDE];
+        nu[0] = sys->R[3 * I]; nu[1] = sys->R[3 * I + 1]; nu[2] = sys->R[3 * I + 2]; nu[3] = sys->Z[I];
+        nu[4] = jas->c1 ? jas->c1[I] : 0.0; nu[5] = jas->c1 ? (jas->b1 ? jas->b1[I] : 1.0) : 1.0;
+        if (sys->pp && sys->pp[4 * I] > 0.0) { nu[6] = sys->pp[4 * I]; nu[7] = sys->pp[4 * I + 1]; nu[8] = sys->pp[4 * I + 2]; nu[9] = sys->pp[4 * I + 3]; nu[10] = 1.0; }
+    }
+    const size_t bf_n = (size_t)S.n_ksteps * c->NT * 32;
+    std::vector<double> h_bf[2];
+    for (int sp = 0; sp < (S.same_C ? 1 : 2); ++sp) {
+        const int ns = sp ? sys->n_dn : sys->n_up; const double *C = sp ? mo->C_dn : mo->C_up;
+        h_bf[sp].assign(bf_n, 0.0);
+        int kstep = 0;
+        for (int g = 0; g < 4; ++g) for (int it = 0; it < S.n_it[g]; ++it) for (int comp = 0; comp < ncomp[g]; ++comp, ++kstep)
+            for (int t = 0; t < c->NT; ++t) for (int lane = 0; lane < 32; ++lane) {
+                int gp = lane >> 2, tp = lane & 3, s = slot_shell[base[g] + 4 * it + tp], m = 8 * t + gp;
+                if (s < 0 || m >= ns) continue;
+                double nrm = g == 0 ? 1.0 : gto_norm(bas->zeta[s], lmn[g][comp][0], lmn[g][comp][1], lmn[g][comp][2]);
+                h_bf[sp][((size_t)kstep * c->NT + t) * 32 + lane] = nrm * C[(size_t)(ao0[s] + comp) * ns + m];
+            }
+    }
+    // ---- device copies
+    size_t bytes = (h_sh.size() + h_nuc.size() + bf_n * (S.same_C ? 1 : 2)) * sizeof(double);
+    cudaError_t ce = cudaMalloc(&c->d_tables, bytes);
+    if (ce != cudaSuccess) { snprintf(g_cuda_msg, sizeof g_cuda_msg, "%s (cudaMalloc tables)", cudaGetErrorString(ce)); free(c); return LRDMC_ECUDA; }
+    double *d = (double *)c->d_tables;
+    cudaMemcpy(d, h_sh.data(), h_sh.size() * 8, cudaMemcpyHostToDevice); S.shells = d; d += h_sh.size();
+    cudaMemcpy(d, h_nuc.data(), h_nuc.size() * 8, cudaMemcpyHostToDevice); S.nuc = d; d += h_nuc.size();
+    cudaMemcpy(d, h_bf[0].data(), bf_n * 8, cudaMemcpyHostToDevice); S.bfrag[0] = d; d += bf_n;
+    if (!S.same_C) { cudaMemcpy(d, h_bf[1].data(), bf_n * 8, cudaMemcpyHostToDevice); S.bfrag[1] = d; } else S.bfrag[1] = S.bfrag[0];
+    if (cudaMalloc((void **)&c->d_stats, sizeof(DevStats)) != cudaSuccess) { cudaFree(c->d_tables); free(c); return LRDMC_ECUDA; }
+    cudaMemset(c->d_stats, 0, sizeof(DevStats));
+    // ---- shared-memory plan
+    cudaDeviceProp prop; int dev = 0; cudaGetDevice(&dev); cudaGetDeviceProperties(&prop, dev);
+    c->sm_count = prop.multiProcessorCount;
+    const size_t bf_doubles = bf_n * (S.same_C ? 1 : 2);
+    S.bf_in_smem = bf_doubles * 8 <= 64 * 1024;
+    const size_t moc_doubles = (size_t)S.N * 5 * S.OS;
+    S.moc_in_smem = moc_doubles * 8 <= 12 * 1024;
+    size_t o = 0;
+    S.off_shells = (int)o; o += align_up(h_sh.size(), 2);
+    S.off_nuc = (int)o; o += align_up(h_nuc.size(), 2);
+    S.off_bf[0] = (int)o; if (S.bf_in_smem) o += bf_n;
+    S.off_bf[1] = (int)o; if (S.bf_in_smem && !S.same_C) o += bf_n;
+    S.tables_doubles = (int)align_up(o, 2);
+    size_t w = 0;
+    S.o_r = (int)w; w += align_up(3 * (size_t)S.N, 2);
+    S.o_dinv[0] = (int)w; w += align_up((size_t)S.dinv_rows[0] * S.n_up, 2);
+    S.o_dinv[1] = (int)w; w += align_up((size_t)S.dinv_rows[1] * S.n_dn, 2);
+    S.o_moc = (int)w; if (S.moc_in_smem) w += align_up(moc_doubles, 2);
+    S.o_R = (int)w; w += align_up((size_t)S.P, 2);
+    S.o_cum = (int)w; w += align_up((size_t)S.P, 2);
+    S.o_el = (int)w; w += align_up((size_t)LRDMC_EL_ARRAYS * S.N, 2);
+    S.per_warp_doubles = (int)w;
+    const size_t per_sm = prop.sharedMemPerMultiprocessor, per_blk_max = prop.sharedMemPerBlockOptin, reserve = 1024;
+    c->wpb = 8;
+    for (;;) {
+        size_t need = ((size_t)S.tables_doubles + (size_t)c->wpb * S.per_warp_doubles) * 8;
+        if ((need + reserve) * 2 <= per_sm || c->wpb == 1) { c->smem_bytes = (int)need; break; }
+        c->wpb >>= 1;
+    }
+    if ((size_t)c->smem_bytes > per_blk_max) { lrdmc_free(c); return LRDMC_ENOMEM; }
+    for (int i = 0; i < 4; ++i) cudaEventCreate(&c->ev[i]);
+#define SET_SMEM(K) cudaFuncSetAttribute(K, cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem_bytes)
+    SET_SMEM(k_propagate<1>); SET_SMEM(k_propagate<2>); SET_SMEM(k_propagate<4>);
+    SET_SMEM(k_step_debug<1>); SET_SMEM(k_step_debug<2>); SET_SMEM(k_step_debug<4>);
+    SET_SMEM(k_rebuild<1>); SET_SMEM(k_rebuild<2>); SET_SMEM(k_rebuild<4>);
+#undef SET_SMEM
+    int occ = 0;
+    if (c->NT == 1) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_propagate<1>, c->wpb * 32, c->smem_bytes);
+    else if (c->NT == 2) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_propagate<2>, c->wpb * 32, c->smem_bytes);
+    else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_propagate<4>, c->wpb * 32, c->smem_bytes);
+    c->ctas_per_sm = occ > 0 ? occ : 1;
+    c->grid_max = c->sm_count * c->ctas_per_sm;
+    if (cudaGetLastError() != cudaSuccess) { /* attribute errors surface at launch */ }
+    *out = c;
+    return LRDMC_OK;
+}
+
+extern "C" void lrdmc_free(lrdmc_ctx *c)
+{
+    if (!c) return;
+    if (c->d_tables) cudaFree(c->d_tables);
+    if (c->d_stats) cudaFree(c->d_stats);
+    for (int i = 0; i < 4; ++i) if (c->ev[i]) cudaEventDestroy(c->ev[i]);
+    free(c);
+}
+
+extern "C" int lrdmc_n_candidates(const lrdmc_ctx *c) { return c ? c->S.P : LRDMC_EINVAL; }
+
+// ---- walker buffer carving -------------------------------------------------------------------------------------
+static size_t carve(const lrdmc_ctx *c, int n_w, char *base, DevWalk *W)
+{
+    const DevSys &S = c->S; size_t o = 0; const size_t nw = (size_t)n_w;
+#define TAKE(field, type, count) do { if (W) W->field = (type *)(base + o); o = align_up(o + sizeof(type) * (count), 256); } while (0)
+    TAKE(r, double, nw * 3 * S.N); TAKE(r_alt, double, nw * 3 * S.N);
+    TAKE(dinv[0], double, nw * S.n_up * S.n_up); TAKE(dinv[1], double, nw * S.n_dn * S.n_dn + 1);
+    TAKE(moc, double, nw * S.N * 5 * S.OS);
+    TAKE(w, double, nw); TAKE(eL, double, nw); TAKE(W, double, nw); TAKE(omega, double, nw);
+    TAKE(nmoves, long long, nw); TAKE(flags, int, nw * 3);
+    TAKE(wq, unsigned long long, nw); TAKE(prefix, unsigned long long, nw); TAKE(parents, int, nw);
+    TAKE(timing, unsigned long long, 2 * (size_t)c->grid_max * c->wpb); TAKE(counter, int, 64);
+#undef TAKE
+    return o;
+}
+
+extern "C" size_t lrdmc_walker_bytes(const lrdmc_ctx *c, int n_walkers)
+{
+    if (!c || n_walkers < 1) return 0;
+    return carve(c, n_walkers, NULL, NULL) + 256;
+}
+
+extern "C" int lrdmc_bind_walkers(lrdmc_ctx *c, void *dev_buf, size_t bytes, int n_walkers)
+{
+    if (!c || !dev_buf || n_walkers < 1 || n_walkers > (1 << 20)) return LRDMC_EINVAL;
+    char *base = (char *)align_up((size_t)dev_buf, 256);
+    if (carve(c, n_walkers, NULL, NULL) + (size_t)(base - (char *)dev_buf) > bytes) return LRDMC_EINVAL;
+    carve(c, n_walkers, base, &c->W);
+    c->W.n_w = n_walkers; c->bound = 1; c->state_ok = 0; c->have_prop = c->have_reconf = 0;
+    return LRDMC_OK;
+}
+
+// ---- launch helpers -----------------------------------------------------------------------------------------------
+static int grid_for(const lrdmc_ctx *c) { int g = (c->W.n_w + c->wpb - 1) / c->wpb; return g < c->grid_max ? g : c->grid_max; }
+#define DISPATCH_NT(KERNEL, grid, stream, ...)                                                                   \
+    do {                                                                                                         \
+        if (c->NT == 1) KERNEL<1><<<grid, c->wpb * 32, c->smem_bytes, stream>>>(__VA_ARGS__);                    \
+        else if (c->NT == 2) KERNEL<2><<<grid, c->wpb * 32, c->smem_bytes, stream>>>(__VA_ARGS__);               \
+        else KERNEL<4><<<grid, c->wpb * 32, c->smem_bytes, stream>>>(__VA_ARGS__);                               \
+        ++c->launches;                                                                                           \
+    } while (0)
+
+static int rebuild(lrdmc_ctx *c, int do_invert, cudaStream_t st)
+{
+    CK(cudaMemsetAsync(c->W.counter, 0, 64 * sizeof(int), st));
+    DISPATCH_NT(k_rebuild, grid_for(c), st, c->S, c->W, do_invert);
+    CK(cudaGetLastError());
+    return LRDMC_OK;
+}
+
+static void fill_ones(lrdmc_ctx *c, cudaStream_t st);
+__global__ void k_fill(double *p, double v, int n) { for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) p[i] = v; }
+static void fill_ones(lrdmc_ctx *c, cudaStream_t st) { k_fill<<<(c->W.n_w + 255) / 256, 256, 0, st>>>(c->W.w, 1.0, c->W.n_w); ++c->launches; }
+
+extern "C" int lrdmc_set_positions(lrdmc_ctx *c, const double *r_dev, void *stream)
+{
+    if (!c || !r_dev) return LRDMC_EINVAL;
+    if (!c->bound) return LRDMC_ESTATE;
+    cudaStream_t st = (cudaStream_t)stream;
+    CK(cudaMemcpyAsync(c->W.r, r_dev, sizeof(double) * (size_t)c->W.n_w * 3 * c->S.N, cudaMemcpyDeviceToDevice, st));
+    fill_ones(c, st);
+    int rc = rebuild(c, 1, st); if (rc) return rc;
+    int flag[2] = { 0, 0 };
+    CK(cudaMemcpyAsync(flag, c->W.counter, sizeof flag, cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    c->state_ok = 1; c->have_prop = c->have_reconf = 0; c->last_stream = st;
+    return flag[1] ? LRDMC_ESINGULAR : LRDMC_OK;
+}
+
+extern "C" int lrdmc_set_state(lrdmc_ctx *c, const double *r_dev, const double *du, const double *dd, const double *w_dev, void *stream)
+{
+    if (!c || !r_dev) return LRDMC_EINVAL;
+    if (!c->bound) return LRDMC_ESTATE;
+    cudaStream_t st = (cudaStream_t)stream; const DevSys &S = c->S; const size_t nw = (size_t)c->W.n_w;
+    CK(cudaMemcpyAsync(c->W.r, r_dev, sizeof(double) * nw * 3 * S.N, cudaMemcpyDeviceToDevice, st));
+    if (du) {
+        CK(cudaMemcpyAsync(c->W.dinv[0], du, sizeof(double) * nw * S.n_up * S.n_up, cudaMemcpyDeviceToDevice, st));
+        if (S.n_dn) { if (!dd) return LRDMC_EINVAL; CK(cudaMemcpyAsync(c->W.dinv[1], dd, sizeof(double) * nw * S.n_dn * S.n_dn, cudaMemcpyDeviceToDevice, st)); }
+    }
+    if (w_dev) CK(cudaMemcpyAsync(c->W.w, w_dev, sizeof(double) * nw, cudaMemcpyDeviceToDevice, st)); else fill_ones(c, st);
+    int rc = rebuild(c, du ? 0 : 1, st); if (rc) return rc;
+    c->state_ok = 1; c->have_prop = c->have_reconf = 0; c->last_stream = st;
+    return LRDMC_OK;
+}
+
+extern "C" int lrdmc_get_walkers(lrdmc_ctx *c, double *r_dev, double *du, double *dd, double *w_dev, void *stream)
+{
+    if (!c) return LRDMC_EINVAL;
+    if (!c->bound || !c->state_ok) return LRDMC_ESTATE;
+    cudaStream_t st = (cudaStream_t)stream; const DevSys &S = c->S; const size_t nw = (size_t)c->W.n_w;
+    if (r_dev) CK(cudaMemcpyAsync(r_dev, c->W.r, sizeof(double) * nw * 3 * S.N, cudaMemcpyDeviceToDevice, st));
+    if (du) CK(cudaMemcpyAsync(du, c->W.dinv[0], sizeof(double) * nw * S.n_up * S.n_up, cudaMemcpyDeviceToDevice, st));
+    if (dd && S.n_dn) CK(cudaMemcpyAsync(dd, c->W.dinv[1], sizeof(double) * nw * S.n_dn * S.n_dn, cudaMemcpyDeviceToDevice, st));
+    if (w_dev) CK(cudaMemcpyAsync(w_dev, c->W.w, sizeof(double) * nw, cudaMemcpyDeviceToDevice, st));
+    return LRDMC_OK;
+}
+
+extern "C" int lrdmc_get_obs(lrdmc_ctx *c, double *eL, double *Wd, double *om, int64_t *nm, void *stream)
+{
+    if (!c) return LRDMC_EINVAL;
+    if (!c->have_prop) return LRDMC_ESTATE;
+    cudaStream_t st = (cudaStream_t)stream; const size_t nw = (size_t)c->W.n_w;
+    if (eL) CK(cudaMemcpyAsync(eL, c->W.eL, 8 * nw, cudaMemcpyDeviceToDevice, st));
+    if (Wd) CK(cudaMemcpyAsync(Wd, c->W.W, 8 * nw, cudaMemcpyDeviceToDevice, st));
+    if (om) CK(cudaMemcpyAsync(om, c->W.omega, 8 * nw, cudaMemcpyDeviceToDevice, st));
+    if (nm) CK(cudaMemcpyAsync(nm, c->W.nmoves, 8 * nw, cudaMemcpyDeviceToDevice, st));
+    return LRDMC_OK;
+}
+
+extern "C" int lrdmc_propagate(lrdmc_ctx *c, int mode, int n_moves, double tau, double E0, uint64_t cycle, void *stream)
+{
+    if (!c) return LRDMC_EINVAL;
+    if (!c->bound || !c->state_ok) return LRDMC_ESTATE;
+    if ((mode != LRDMC_BALANCED && mode != LRDMC_CONVENTIONAL) || n_moves < 0 || (mode == LRDMC_CONVENTIONAL && !(tau > 0.0)) || cycle > 0xFFFFFFFFull
+        || !std::isfinite(E0)) return LRDMC_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    CK(cudaMemsetAsync(c->W.counter, 0, 64 * sizeof(int), st));
+    const int grid = grid_for(c);
+    CK(cudaEventRecord(c->ev[0], st));
+    DISPATCH_NT(k_propagate, grid, st, c->S, c->W, mode, n_moves, tau, E0, (uint32_t)cycle);
+    CK(cudaEventRecord(c->ev[1], st));
+    CK(cudaGetLastError());
+    k_reduce_obs<<<1, 1024, 0, st>>>(c->W, c->d_stats, grid * c->wpb); ++c->launches;
+    CK(cudaGetLastError());
+    c->have_prop = 1; c->last_stream = st;
+    return LRDMC_OK;
+}
+
+extern "C" int lrdmc_reconfigure(lrdmc_ctx *c, uint64_t cycle, int32_t *parents_dev, void *stream)
+{
+    if (!c) return LRDMC_EINVAL;
+    if (!c->bound || !c->state_ok) return LRDMC_ESTATE;
+    if (cycle > 0xFFFFFFFFull) return LRDMC_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    // comb random number: counter (0xFFFFFFFF, cycle, 0, 3), word 0 -- same block function as the device generator, run on the host
+    uint32_t ctr[4] = { 0xFFFFFFFFu, (uint32_t)cycle, 0u, 3u }, k0 = c->S.key0, k1 = c->S.key1;
+    for (int r = 0; r < 10; ++r) {
+        uint64_t p0 = (uint64_t)0xD2511F53u * ctr[0], p1 = (uint64_t)0xCD9E8D57u * ctr[2];
+        uint32_t n0 = (uint32_t)(p1 >> 32) ^ ctr[1] ^ k0, n1 = (uint32_t)p1, n2 = (uint32_t)(p0 >> 32) ^ ctr[3] ^ k1, n3 = (uint32_t)p0;
+        ctr[0] = n0; ctr[1] = n1; ctr[2] = n2; ctr[3] = n3; k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+    }
+    CK(cudaEventRecord(c->ev[2], st));
+    k_comb<<<1, COMB_THREADS, 0, st>>>(c->W, ctr[0], c->d_stats, parents_dev); ++c->launches;
+    CK(cudaGetLastError());
+    const int rec = 3 * c->S.N;
+    size_t total = (size_t)c->W.n_w * rec; int gb = (int)((total + 255) / 256); if (gb > 148 * 16) gb = 148 * 16;
+    k_gather<<<gb, 256, 0, st>>>(c->W, rec); ++c->launches;
+    CK(cudaGetLastError());
+    double *tmp = c->W.r; c->W.r = c->W.r_alt; c->W.r_alt = tmp;
+    int rc = rebuild(c, 1, st); if (rc) return rc;
+    CK(cudaEventRecord(c->ev[3], st));
+    c->have_reconf = 1; c->last_stream = st;
+    return LRDMC_OK;
+}
+
+extern "C" int lrdmc_estimators(lrdmc_ctx *c, lrdmc_cycle_stats *out)
+{
+    if (!c || !out) return LRDMC_EINVAL;
+    if (!c->have_prop) return LRDMC_ESTATE;
+    CK(cudaStreamSynchronize(c->last_stream));
+    DevStats h; CK(cudaMemcpy(&h, c->d_stats, sizeof h, cudaMemcpyDeviceToHost));
+    memset(out, 0, sizeof *out);
+    out->wbar = c->have_reconf ? h.wbar : 0.0; out->num = h.num; out->den = h.den;
+    out->moves_min = h.moves_min; out->moves_max = h.moves_max; out->moves_sum = h.moves_sum;
+    out->n_node_flag = h.n_node; out->n_nonpos_diag = h.n_nonpos; out->n_nonfinite = h.n_nonfinite;
+    out->lockstep_idle_frac = h.moves_max > 0 ? 1.0 - (double)h.moves_sum / ((double)c->W.n_w * (double)h.moves_max) : 0.0;
+    out->barrier_idle_frac = (h.span_ns > 0.0 && h.n_warps > 0) ? 1.0 - h.busy_ns / (h.span_ns * h.n_warps) : 0.0;
+    cudaEventElapsedTime(&out->propagate_ms, c->ev[0], c->ev[1]);
+    if (c->have_reconf) cudaEventElapsedTime(&out->reconfigure_ms, c->ev[2], c->ev[3]);
+    cudaGetLastError();
+    return LRDMC_OK;
+}
+
+extern "C" int lrdmc_step_debug(lrdmc_ctx *c, double E0, uint64_t cycle, uint64_t step, double *R_dev, double *scal_dev, int32_t *jstar_dev, void *stream)
+{
+    if (!c || !R_dev || !scal_dev || !jstar_dev || cycle > 0xFFFFFFFFull || step > 0xFFFFFFFFull) return LRDMC_EINVAL;
+    if (!c->bound || !c->state_ok) return LRDMC_ESTATE;
+    cudaStream_t st = (cudaStream_t)stream;
+    DISPATCH_NT(k_step_debug, grid_for(c), st, c->S, c->W, E0, (uint32_t)cycle, (uint32_t)step, R_dev, scal_dev, jstar_dev);
+    CK(cudaGetLastError());
+    return LRDMC_OK;
+}
+
+extern "C" int lrdmc_launch_count(const lrdmc_ctx *c) { return c ? c->launches : 0; }
+extern "C" int lrdmc_bound_walkers(const lrdmc_ctx *c) { return (c && c->bound) ? c->W.n_w : 0; }
+extern "C" int lrdmc_n_electrons(const lrdmc_ctx *c) { return c ? c->S.N : 0; }
+extern "C" const DevSys *lrdmc_devsys(const lrdmc_ctx *c) { return &c->S; }
+extern "C" int lrdmc_launch_config(const lrdmc_ctx *c, int *grid, int *block, int *smem_bytes, int *ctas_per_sm)
+{
+    if (!c) return LRDMC_EINVAL;
+    if (grid) *grid = c->bound ? grid_for(c) : c->grid_max; if (block) *block = c->wpb * 32; if (smem_bytes) *smem_bytes = c->smem_bytes;
+    if (ctas_per_sm) *ctas_per_sm = c->ctas_per_sm;
+    return LRDMC_OK;
+}

@@ -1,0 +1,25 @@
+// peaks.cuh -- FP64 roofline denominators measured on the device itself (MEASURED_PEAKS.json has no FP64 number).
+// DFMA: 8 independent FMA chains per thread.  DMMA: 8 independent mma.sync.m8n8k4.f64 accumulator chains per warp.
+// MIXED: both interleaved, to see whether the FP64 tensor path and the FP64 ALUs overlap on sm_100a.
+#pragma once
+#include "wavefunction.cuh"
+
+template <int MODE>   // 0 DFMA, 1 DMMA, 2 both
+__global__ void __launch_bounds__(256) k_fp64_peak(double *out, int iters, double seed)
+{
+    double f[8], c[8][2];
+    const double a = seed + threadIdx.x * 1e-9, b = 1.0 - 1e-7;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) { f[i] = seed * (i + 1); c[i][0] = seed * i; c[i][1] = -seed * i; }
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            if (MODE != 1) f[i] = fma(f[i], b, a);
+            if (MODE != 0) dmma884(c[i][0], c[i][1], a, b);
+        }
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) s += f[i] + c[i][0] + c[i][1];
+    if (s == 123.456) out[blockIdx.x * blockDim.x + threadIdx.x] = s;   // keep the work alive
+}

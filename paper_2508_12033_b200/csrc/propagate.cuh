@@ -1,0 +1,181 @@
+// propagate.cuh -- the persistent walker kernels: one warp = one walker, state resident in shared memory for the
+// whole branching interval (HBM is touched once per walker per cycle); walkers are pulled from a device-side queue
+// so that the stochastic trip counts of the conventional mode (L168) do not leave SMs idle.
+#pragma once
+#include "evaluate.cuh"
+
+// ---- shared-memory staging -------------------------------------------------------------------------------------
+__device__ __forceinline__ void stage_tables(const DevSys &S, double *smem)
+{
+    for (int i = threadIdx.x; i < S.n_slots * 4; i += blockDim.x) smem[S.off_shells + i] = S.shells[i];
+    for (int i = threadIdx.x; i < S.n_nuc * LRDMC_NUC_STRIDE; i += blockDim.x) smem[S.off_nuc + i] = S.nuc[i];
+    if (S.bf_in_smem) {
+        const int nb = S.n_ksteps * S.NT[0] * 32;
+        for (int i = threadIdx.x; i < nb; i += blockDim.x) smem[S.off_bf[0] + i] = S.bfrag[0][i];
+        if (!S.same_C && S.n_dn > 0) for (int i = threadIdx.x; i < nb; i += blockDim.x) smem[S.off_bf[1] + i] = S.bfrag[1][i];
+    }
+    __syncthreads();
+}
+
+__device__ __forceinline__ void table_pointers(const DevSys &S, const double *smem, const double *&shells, const double *&nuc, const double *bf[2])
+{
+    shells = smem + S.off_shells; nuc = smem + S.off_nuc;
+    if (S.bf_in_smem) { bf[0] = smem + S.off_bf[0]; bf[1] = S.same_C ? bf[0] : smem + S.off_bf[1]; }
+    else { bf[0] = S.bfrag[0]; bf[1] = S.same_C ? S.bfrag[0] : S.bfrag[1]; }
+}
+
+__device__ __forceinline__ WarpState warp_views(const DevSys &S, double *smem, int warp)
+{
+    double *base = smem + S.tables_doubles + (size_t)warp * S.per_warp_doubles;
+    WarpState ws;
+    ws.r = base + S.o_r; ws.dinv[0] = base + S.o_dinv[0]; ws.dinv[1] = base + S.o_dinv[1];
+    ws.moc = base + S.o_moc; ws.R = base + S.o_R; ws.cum = base + S.o_cum; ws.el = base + S.o_el;
+    return ws;
+}
+
+__device__ __forceinline__ void load_walker(const DevSys &S, const DevWalk &W, WarpState &ws, int k, int lane, bool with_dinv)
+{
+    const int N = S.N;
+    for (int i = lane; i < 3 * N; i += 32) ws.r[i] = W.r[(size_t)k * 3 * N + i];
+    for (int sp = 0; sp < 2; ++sp) {
+        const int ns = sp ? S.n_dn : S.n_up, tot = S.dinv_rows[sp] * ns;
+        const double *src = W.dinv[sp] + (size_t)k * ns * ns;
+        for (int i = lane; i < tot; i += 32) ws.dinv[sp][i] = (with_dinv && i < ns * ns) ? src[i] : 0.0;
+    }
+    const size_t mocn = (size_t)N * 5 * S.OS;
+    if (S.moc_in_smem) { for (int i = lane; i < (int)mocn; i += 32) ws.moc[i] = W.moc[(size_t)k * mocn + i]; }
+    else ws.moc = W.moc + (size_t)k * mocn;
+    __syncwarp();
+}
+
+__device__ __forceinline__ void store_walker(const DevSys &S, const DevWalk &W, const WarpState &ws, int k, int lane)
+{
+    const int N = S.N;
+    __syncwarp();
+    for (int i = lane; i < 3 * N; i += 32) W.r[(size_t)k * 3 * N + i] = ws.r[i];
+    for (int sp = 0; sp < 2; ++sp) {
+        const int ns = sp ? S.n_dn : S.n_up;
+        double *dst = W.dinv[sp] + (size_t)k * ns * ns;
+        for (int i = lane; i < ns * ns; i += 32) dst[i] = ws.dinv[sp][i];
+    }
+    const size_t mocn = (size_t)N * 5 * S.OS;
+    if (S.moc_in_smem) for (int i = lane; i < (int)mocn; i += 32) W.moc[(size_t)k * mocn + i] = ws.moc[i];
+    __syncwarp();
+}
+
+// ---- the projection kernel (Alg.2 lines 4-8 L401-L410 / Alg.1 lines 4-16 L350-L374) ----------------------------
+template <int NT>
+__global__ void __launch_bounds__(256) k_propagate(DevSys S, DevWalk W, int mode, int n_moves, double tau, double E0, uint32_t cycle)
+{
+    extern __shared__ __align__(16) double smem[];
+    stage_tables(S, smem);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, gwarp = blockIdx.x * (blockDim.x >> 5) + warp;
+    const double *shells, *nuc, *bf[2];
+    table_pointers(S, smem, shells, nuc, bf);
+    WarpState ws = warp_views(S, smem, warp);
+    const unsigned long long t_start = globaltimer_ns();
+    for (;;) {
+        int k = 0;
+        if (lane == 0) k = atomicAdd(W.counter, 1);
+        k = __shfl_sync(0xffffffffu, k, 0);
+        if (k >= W.n_w) break;
+        load_walker(S, W, ws, k, lane, true);
+        double w = 1.0, tau_left = tau, omega = 0.0, eL_out = 0.0, W_out = 0.0;
+        long long moves = 0; int n_node = 0, n_nonpos = 0;
+        for (uint32_t s = 0;; ++s) {
+            const StepDraws d = step_draws(S, (uint32_t)k, cycle, s, mode == LRDMC_CONVENTIONAL);
+            double U[9]; lattice_frame(d.u1, d.u2, d.u3, U);
+            const EvalOut e = evaluate_walker<NT>(S, ws, shells, bf, nuc, U, lane);
+            n_node += e.node;
+            bool last = false;
+            if (mode == LRDMC_BALANCED) {
+                const double den = e.W - E0;                       // b_x = bbar/(W - E0)   (Eq.29)
+                if ((int)s == n_moves) {                           // measurement evaluation (reading Q10; Eq.34)
+                    if (!(den > 0.0)) { ++n_nonpos; w = 0.0; omega = 0.0; } else omega = w / den;
+                    last = true;
+                } else if (!(den > 0.0)) { ++n_nonpos; w = 0.0; }  // reading Q16
+                else w *= e.bbar / den;                            // Alg.2 line 6 (L406)
+            } else {
+                double tx = -log1p(-d.u_tau) / e.bbar;             // Eq.24 (L160)
+                if (!(tx < tau_left) || (n_moves > 0 && (int)s >= n_moves)) { tx = tau_left; last = true; }   // min[., tau_left] (L362)
+                w *= exp(-tx * (e.eL - E0));                       // Eq.25 (L164), constant shift of reading Q8b
+                tau_left -= tx;
+                if (last) omega = w;
+            }
+            if (last) { eL_out = e.eL; W_out = e.W; break; }
+            const int j = select_move(S, ws, d.u_sel, lane);       // Alg.2 line 7 (L408)
+            if (j >= 0) { apply_move<NT>(S, ws, shells, bf, U, j, lane); ++moves; }
+        }
+        int nonfinite = 0;
+        if (!isfinite(w) || !isfinite(omega)) { nonfinite = 1; w = 0.0; omega = 0.0; }
+        store_walker(S, W, ws, k, lane);
+        if (lane == 0) {
+            W.w[k] = w; W.eL[k] = eL_out; W.W[k] = W_out; W.omega[k] = omega; W.nmoves[k] = moves;
+            W.flags[3 * k] = n_node; W.flags[3 * k + 1] = n_nonpos; W.flags[3 * k + 2] = nonfinite;
+        }
+    }
+    if (lane == 0) { W.timing[2 * gwarp] = t_start; W.timing[2 * gwarp + 1] = globaltimer_ns(); }
+}
+
+// ---- parity hook: one evaluation + selection, no state change ---------------------------------------------------
+template <int NT>
+__global__ void __launch_bounds__(256) k_step_debug(DevSys S, DevWalk W, double E0, uint32_t cycle, uint32_t step, double *R_out,
+                                                    double *scal_out, int *jstar_out)
+{
+    extern __shared__ __align__(16) double smem[];
+    stage_tables(S, smem);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, wpb = blockDim.x >> 5;
+    const double *shells, *nuc, *bf[2];
+    table_pointers(S, smem, shells, nuc, bf);
+    WarpState ws = warp_views(S, smem, warp);
+    for (int k = blockIdx.x * wpb + warp; k < W.n_w; k += gridDim.x * wpb) {
+        load_walker(S, W, ws, k, lane, true);
+        const StepDraws d = step_draws(S, (uint32_t)k, cycle, step, true);
+        double U[9]; lattice_frame(d.u1, d.u2, d.u3, U);
+        const EvalOut e = evaluate_walker<NT>(S, ws, shells, bf, nuc, U, lane);
+        const int j = select_move(S, ws, d.u_sel, lane);
+        for (int p = lane; p < S.P; p += 32) R_out[(size_t)k * S.P + p] = ws.R[p];
+        if (lane == 0) {
+            double *o = scal_out + 8 * (size_t)k;
+            o[0] = e.bbar; o[1] = e.Vsf; o[2] = e.W; o[3] = e.eL; o[4] = e.bbar / (e.W - E0);
+            o[5] = -log1p(-d.u_tau) / e.bbar; o[6] = (double)e.node; o[7] = d.u_sel;
+            jstar_out[k] = j;
+        }
+        if (!S.moc_in_smem) ws = warp_views(S, smem, warp);
+        __syncwarp();
+    }
+}
+
+// ---- (re)build of the inverses and MO caches from the positions (row a13) ---------------------------------------
+template <int NT>
+__global__ void __launch_bounds__(256) k_rebuild(DevSys S, DevWalk W, int do_invert)
+{
+    extern __shared__ __align__(16) double smem[];
+    stage_tables(S, smem);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, wpb = blockDim.x >> 5;
+    const double *shells, *nuc, *bf[2];
+    table_pointers(S, smem, shells, nuc, bf);
+    WarpState ws = warp_views(S, smem, warp);
+    const int N = S.N;
+    for (int k = blockIdx.x * wpb + warp; k < W.n_w; k += gridDim.x * wpb) {
+        load_walker(S, W, ws, k, lane, !do_invert);
+        for (int i = 0; i < N; ++i) {
+            const int sp = spin_of(S, i);
+            refresh_mo_cache<NT>(S, shells, bf[sp], ws.moc + (size_t)i * 5 * S.OS, ws.r[3 * i], ws.r[3 * i + 1], ws.r[3 * i + 2], lane);
+        }
+        __syncwarp();
+        if (do_invert) {
+            for (int sp = 0; sp < 2; ++sp) {
+                const int ns = sp ? S.n_dn : S.n_up, off = sp ? S.n_up : 0;
+                if (!ns) continue;
+                double *A = ws.dinv[sp];
+                for (int idx = lane; idx < ns * ns; idx += 32) { int i = idx / ns, m = idx - i * ns; A[idx] = ws.moc[(size_t)(off + i) * 5 * S.OS + m]; }
+                __syncwarp();
+                if (!warp_invert(A, ns, ns, reinterpret_cast<int *>(ws.cum), lane) && lane == 0) atomicOr(W.counter + 1, 1);
+                __syncwarp();
+            }
+        }
+        store_walker(S, W, ws, k, lane);
+        if (!S.moc_in_smem) ws = warp_views(S, smem, warp);
+    }
+}

@@ -1,0 +1,162 @@
+// wavefunction.cuh -- AO evaluation fused with the AO->MO contraction on the FP64 tensor pipe.
+//
+// Rows a2/a3 of the scope table.  One warp evaluates 8 points at a time:
+//   lane = 4*g + t :  g = point (mma row), t = which of 4 concurrently processed shells (mma k slot).
+// Each lane computes exp(-zeta |r_g - R_c|^2) of ITS shell at ITS point once (no redundant exponentials) and feeds the
+// AO values of that shell straight into mma.sync.m8n8k4.f64 as the A fragment (A[g][t]); the B fragment
+// B[t][n] = norm * C[ao(shell t, component)][n] comes pre-swizzled from the table built at init (conflict-free, 256 B per
+// warp load).  The contraction index k of the mma is just "which (shell, component)", so shells are sorted by type and
+// padded to multiples of 4 -- all four k slots always run the same code.  Accumulator: lane holds MO (2t, 2t+1) of point g.
+#pragma once
+#include "common.cuh"
+
+__device__ __forceinline__ void dmma884(double &c0, double &c1, double a, double b)
+{
+    asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
+}
+
+// per-axis monomial v^k and its first / second derivative including the Gaussian factor's contribution:
+//   d/dv [v^k e^{-z v^2}] = (k v^{k-1} - 2 z v^{k+1}) e ,  d2/dv2 = (k(k-1) v^{k-2} - 2 z (2k+1) v^k + 4 z^2 v^{k+2}) e
+struct AxisPoly { double f[3], f1[3], f2[3]; };
+__device__ __forceinline__ AxisPoly axis_poly(double v, double z)
+{
+    AxisPoly p; double v2 = v * v, tz = 2.0 * z, fz2 = 4.0 * z * z;
+    p.f[0] = 1.0; p.f[1] = v; p.f[2] = v2;
+    p.f1[0] = -tz * v;            p.f1[1] = 1.0 - tz * v2;              p.f1[2] = 2.0 * v - tz * v2 * v;
+    p.f2[0] = -tz + fz2 * v2;     p.f2[1] = (-3.0 * tz + fz2 * v2) * v; p.f2[2] = 2.0 - 5.0 * tz * v2 + fz2 * v2 * v2;
+    return p;
+}
+// component g of the cartesian primitive x^l y^m z^n e:  g = 0 value, 1..3 gradient, 4 Laplacian, >4 zero
+template <int L, int M, int N>
+__device__ __forceinline__ double gto_component(int g, const AxisPoly &X, const AxisPoly &Y, const AxisPoly &Z, double e)
+{
+    double fx = (g == 1) ? X.f1[L] : X.f[L], fy = (g == 2) ? Y.f1[M] : Y.f[M], fz = (g == 3) ? Z.f1[N] : Z.f[N];
+    double v = fx * fy * fz;
+    double lap = X.f2[L] * Y.f[M] * Z.f[N] + X.f[L] * Y.f2[M] * Z.f[N] + X.f[L] * Y.f[M] * Z.f2[N];
+    v = (g == 4) ? lap : v;
+    return (g > 4) ? 0.0 : v * e;
+}
+
+// One pass over the whole (sorted, padded) shell list for the 8 points held by the warp.
+// DERIV = false: A fragment = AO value (candidate evaluation, row a2/a3).
+// DERIV = true : the 8 mma rows are 8 COMPONENTS (value, d/dx, d/dy, d/dz, Laplacian, 0,0,0) of ONE point, selector g = lane/4.
+template <int NT, bool DERIV>
+__device__ __forceinline__ void mo_pass(const DevSys &S, const double *__restrict__ shells, const double *__restrict__ bf,
+                                        double px, double py, double pz, int lane, double (&acc)[NT][2])
+{
+    const int t = lane & 3, g = lane >> 2;
+    const double4 *sh4 = reinterpret_cast<const double4 *>(shells) + t;
+    const double *b = bf + lane;
+#pragma unroll
+    for (int nt = 0; nt < NT; ++nt) { acc[nt][0] = 0.0; acc[nt][1] = 0.0; }
+#define LRDMC_FEED(aval)                                                                        \
+    {                                                                                           \
+        double a_ = (aval);                                                                     \
+        _Pragma("unroll") for (int nt = 0; nt < NT; ++nt) dmma884(acc[nt][0], acc[nt][1], a_, b[nt * 32]); \
+        b += NT * 32;                                                                           \
+    }
+    // ---- group 0: Slater-type s, chi = exp(-z r); grad = -z chi rhat; lap = chi (z^2 - 2 z / r)
+    for (int it = 0; it < S.n_it[0]; ++it, sh4 += 4) {
+        double4 s = *sh4; double dx = px - s.x, dy = py - s.y, dz = pz - s.z, z = s.w;
+        double r = sqrt(dx * dx + dy * dy + dz * dz), e = exp(-z * r);
+        if (!DERIV) { LRDMC_FEED(e); }
+        else {
+            double ir = 1.0 / r, d = (g == 1) ? dx : ((g == 2) ? dy : dz);
+            double v = (g == 0) ? e : ((g == 4) ? e * (z * z - 2.0 * z * ir) : -z * e * d * ir);
+            LRDMC_FEED((g > 4) ? 0.0 : v);
+        }
+    }
+    // ---- group 1: s Gaussians
+    for (int it = 0; it < S.n_it[1]; ++it, sh4 += 4) {
+        double4 s = *sh4; double dx = px - s.x, dy = py - s.y, dz = pz - s.z, z = s.w;
+        double e = exp(-z * (dx * dx + dy * dy + dz * dz));
+        if (!DERIV) { LRDMC_FEED(e); }
+        else { AxisPoly X = axis_poly(dx, z), Y = axis_poly(dy, z), Z = axis_poly(dz, z); LRDMC_FEED((gto_component<0, 0, 0>(g, X, Y, Z, e))); }
+    }
+    // ---- group 2: p Gaussians (x, y, z)
+    for (int it = 0; it < S.n_it[2]; ++it, sh4 += 4) {
+        double4 s = *sh4; double dx = px - s.x, dy = py - s.y, dz = pz - s.z, z = s.w;
+        double e = exp(-z * (dx * dx + dy * dy + dz * dz));
+        if (!DERIV) { LRDMC_FEED(dx * e); LRDMC_FEED(dy * e); LRDMC_FEED(dz * e); }
+        else {
+            AxisPoly X = axis_poly(dx, z), Y = axis_poly(dy, z), Z = axis_poly(dz, z);
+            LRDMC_FEED((gto_component<1, 0, 0>(g, X, Y, Z, e))); LRDMC_FEED((gto_component<0, 1, 0>(g, X, Y, Z, e)));
+            LRDMC_FEED((gto_component<0, 0, 1>(g, X, Y, Z, e)));
+        }
+    }
+    // ---- group 3: d Gaussians (xx, xy, xz, yy, yz, zz)
+    for (int it = 0; it < S.n_it[3]; ++it, sh4 += 4) {
+        double4 s = *sh4; double dx = px - s.x, dy = py - s.y, dz = pz - s.z, z = s.w;
+        double e = exp(-z * (dx * dx + dy * dy + dz * dz));
+        if (!DERIV) {
+            double xe = dx * e, ye = dy * e, ze = dz * e;
+            LRDMC_FEED(dx * xe); LRDMC_FEED(dx * ye); LRDMC_FEED(dx * ze); LRDMC_FEED(dy * ye); LRDMC_FEED(dy * ze); LRDMC_FEED(dz * ze);
+        } else {
+            AxisPoly X = axis_poly(dx, z), Y = axis_poly(dy, z), Z = axis_poly(dz, z);
+            LRDMC_FEED((gto_component<2, 0, 0>(g, X, Y, Z, e))); LRDMC_FEED((gto_component<1, 1, 0>(g, X, Y, Z, e)));
+            LRDMC_FEED((gto_component<1, 0, 1>(g, X, Y, Z, e))); LRDMC_FEED((gto_component<0, 2, 0>(g, X, Y, Z, e)));
+            LRDMC_FEED((gto_component<0, 1, 1>(g, X, Y, Z, e))); LRDMC_FEED((gto_component<0, 0, 2>(g, X, Y, Z, e)));
+        }
+    }
+#undef LRDMC_FEED
+}
+
+// Refresh the cached MO rows (value, gradient, Laplacian) of electron i at position (px,py,pz): moc[i][comp][m].
+template <int NT>
+__device__ __forceinline__ void refresh_mo_cache(const DevSys &S, const double *shells, const double *bf, double *moc_i,
+                                                 double px, double py, double pz, int lane)
+{
+    double acc[NT][2];
+    mo_pass<NT, true>(S, shells, bf, px, py, pz, lane, acc);
+    const int t = lane & 3, g = lane >> 2;
+    if (g < 5) {
+#pragma unroll
+        for (int nt = 0; nt < NT; ++nt) {
+            moc_i[g * S.OS + 8 * nt + 2 * t] = acc[nt][0];
+            moc_i[g * S.OS + 8 * nt + 2 * t + 1] = acc[nt][1];
+        }
+    }
+}
+
+// In-place Gauss-Jordan inversion with partial (row) pivoting of the n x n matrix A (row stride ld) by one warp.
+// On entry A[i][m] = D[i][m]; on exit A[m][i] = Dinv[m][i] (sum_m D[i][m] Dinv[m][k] = delta_ik).  Returns false on a zero pivot.
+__device__ __forceinline__ bool warp_invert(double *A, int n, int ld, int *perm, int lane)
+{
+    bool ok = true;
+    for (int c = 0; c < n; ++c) {
+        // pivot search over rows i >= c
+        double best = -1.0; int bi = c;
+        for (int i = c + lane; i < n; i += 32) { double v = fabs(A[i * ld + c]); if (v > best) { best = v; bi = i; } }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            double ob = __shfl_xor_sync(0xffffffffu, best, o); int oi = __shfl_xor_sync(0xffffffffu, bi, o);
+            if (ob > best || (ob == best && oi < bi)) { best = ob; bi = oi; }
+        }
+        if (!(best > 0.0) || isinf(best)) { ok = false; break; }
+        if (lane == 0) perm[c] = bi;
+        if (bi != c) for (int j = lane; j < n; j += 32) { double tmp = A[c * ld + j]; A[c * ld + j] = A[bi * ld + j]; A[bi * ld + j] = tmp; }
+        __syncwarp();
+        double ip = 1.0 / A[c * ld + c];
+        __syncwarp();
+        for (int j = lane; j < n; j += 32) A[c * ld + j] = (j == c) ? ip : A[c * ld + j] * ip;
+        __syncwarp();
+        for (int idx = lane; idx < n * n; idx += 32) {
+            int i = idx / n, j = idx - i * n;
+            if (i == c) continue;
+            double f = A[i * ld + c];
+            // column c of row i must be read by every lane of that row before it is overwritten: do it in two sweeps
+            if (j != c) A[i * ld + j] -= f * A[c * ld + j];
+        }
+        __syncwarp();
+        for (int i = lane; i < n; i += 32) if (i != c) A[i * ld + c] = -A[i * ld + c] * A[c * ld + c];
+        __syncwarp();
+    }
+    if (ok) {
+        for (int c = n - 1; c >= 0; --c) {
+            int p = perm[c];
+            if (p != c) for (int i = lane; i < n; i += 32) { double tmp = A[i * ld + c]; A[i * ld + c] = A[i * ld + p]; A[i * ld + p] = tmp; }
+            __syncwarp();
+        }
+    }
+    return ok;
+}

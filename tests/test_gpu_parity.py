@@ -1,0 +1,249 @@
+"""Parity of the CUDA path (through the C-ABI binding) with the CPU oracle on identical seeded inputs.  -m gpu.
+
+Tolerances: FP64 quantities within 1e-10 relative to max(|value|, natural scale) where
+the natural scale is the size of the summands the value is assembled from (1 for a wavefunction ratio, K_diag = 3N/a^2
+for W and e_L, max|Dinv| for an inverse); selected moves, trip counts and reconfiguration indices bit-exact.
+"""
+import numpy as np
+import pytest
+
+from oracle import lrdmc_ref as ref, ref_driver as rdrv
+from paper_2508_12033_b200 import workloads as wl
+from conftest import read_golden
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-10
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2508_12033_b200 import binding
+    binding.load_library()
+    return binding
+
+
+def np_(t):
+    return t.cpu().numpy()
+
+
+def relerr(a, b, scale=0.0):
+    a = np.asarray(a, float); b = np.asarray(b, float)
+    return float(np.max(np.abs(a - b) / np.maximum(np.maximum(np.abs(a), np.abs(b)), max(scale, 1e-300)))) if a.size else 0.0
+
+
+SYSTEMS = {
+    "C1-hydrogen": lambda: (wl.hydrogen(), wl.hydrogen_walkers(256, 1)),
+    "tiny-2u1d": lambda: _with_walkers(wl.tiny_molecule(2, 1, 2, 6, seed=7), 37),
+    "tiny-3u3d-pp": lambda: _with_walkers(wl.tiny_molecule(3, 3, 3, 9, seed=8, with_pp=True), 37),
+    "tiny-2u2d-doublemesh": lambda: _with_walkers(wl.tiny_molecule(2, 2, 2, 7, seed=9, a=0.15, a2=0.3), 41),
+    "ragged-5u2d": lambda: _with_walkers(wl.tiny_molecule(5, 2, 3, 11, seed=10), 19),
+    "ragged-9u4d-NT2": lambda: _with_walkers(wl.tiny_molecule(9, 4, 4, 20, seed=11), 13),
+    "ragged-17u3d-NT4": lambda: _with_walkers(wl.tiny_molecule(17, 3, 5, 30, seed=12), 9),
+    "he-triplet-slater": lambda: _with_walkers(wl.slater_atom(2.0, [2.0, 0.6], 2, 0, np.eye(2), np.zeros((2, 0)), 0.2, jastrow=dict(a_par=0.25, a_anti=0.5, b2=0.5)), 64),
+    "C2-synthetic10": lambda: _with_walkers(wl.synthetic10(), 300),
+    "C3-water-methane-shaped": lambda: _with_walkers(wl.water_methane(n_walkers=100), 100),
+}
+
+
+def _with_walkers(s, n):
+    return s, wl.initial_walkers(s, n, 5)
+
+
+def _pair(B, name):
+    s, x0 = SYSTEMS[name]()
+    o = ref.Ref(s); rc = o.set_positions(x0); assert rc == 0, rc
+    g = B.Lrdmc(s); g.lrdmc_set_positions(x0)
+    return s, x0, o, g
+
+
+# ------------------------------------------------------------------------------------------ a0: RNG + frame
+def test_philox_device_matches_oracle_and_known_answers(B):
+    g = B.Lrdmc(wl.hydrogen())
+    kat = read_golden("philox4x32_10_kat.txt")
+    for name, v in kat.items():
+        x = [int(t, 16) for t in v]
+        out = g.debug_philox(np.array([x[0:4]], dtype=np.uint32), (x[4], x[5]))
+        assert [int(t) for t in out[0]] == x[6:10], name
+    rng = np.random.default_rng(0)
+    ctr = rng.integers(0, 2**32, size=(1000, 4), dtype=np.uint64).astype(np.uint32)
+    out = g.debug_philox(ctr, (0xDEADBEEF, 0x12345678))
+    for i in range(0, 1000, 7):
+        assert tuple(int(t) for t in out[i]) == ref.philox4x32_10([int(t) for t in ctr[i]], (0xDEADBEEF, 0x12345678))
+
+
+def test_draws_and_frames_match_oracle(B):
+    s = wl.synthetic10(); g = B.Lrdmc(s); o = ref.Ref(s)
+    out = np_(g.debug_draws(9, 4, 500))
+    for k in range(0, 500, 3):
+        u = o.draws(k, 9, 4)
+        assert np.array_equal(out[k, :5], u)                      # uniforms are integer arithmetic: bit-exact
+        assert np.abs(out[k, 5:].reshape(3, 3) - ref.frame(u[0], u[1], u[2])).max() < 4e-16
+
+
+# ------------------------------------------------------------------------------------------ a13: inverse build
+@pytest.mark.parametrize("name", list(SYSTEMS))
+def test_set_positions_builds_the_same_inverse(B, name):
+    s, x0, o, g = _pair(B, name)
+    r, du, dd, w = o.get_state(); gr, gdu, gdd, gw = [np_(t) for t in g.lrdmc_get_walkers()]
+    assert np.array_equal(gr, r) and np.all(gw == 1.0)
+    for a, b in ((gdu, du), (gdd, dd)):
+        if b.size:
+            sc = np.abs(b).max(axis=(1, 2), keepdims=True)
+            assert np.max(np.abs(a - b) / sc) < 1e-8          # conditioning of random Slater matrices, not arithmetic
+
+
+# ------------------------------------------------------------------------------------------ a1-a9: one step
+@pytest.mark.parametrize("name", list(SYSTEMS))
+def test_one_evaluation_and_selection_from_the_oracle_state(B, name):
+    s, x0, o, g = _pair(B, name)
+    N = s["n_up"] + s["n_dn"]
+    r, du, dd, w = o.get_state(); g.lrdmc_set_state(r, du, dd, w)
+    for (E0, cycle, step) in ((-3.0, 0, 0), (0.5, 7, 3)):
+        R, scal, js = o.step_debug(E0, cycle, step)
+        gR, gscal, gjs = [np_(t) for t in g.lrdmc_step_debug(E0, cycle, step)]
+        assert gR.shape == R.shape == (len(x0), 6 * N * (2 if s["a2"] > 0 else 1))
+        Kdiag = scal[:, 2:3] * 0 + 3 * N * ((1 / s["a"]**2) if s["a2"] == 0 else (0.5 / s["a"]**2 + 0.5 / s["a2"]**2))
+        assert relerr(gR, R, 1.0) < TOL                                                  # ratios
+        for col, nm in ((0, "bbar"), (1, "V_sf"), (2, "W"), (3, "e_L")):
+            assert np.max(np.abs(gscal[:, col] - scal[:, col]) / np.maximum(np.abs(scal[:, col]), Kdiag[:, 0])) < TOL, nm
+        ok = np.abs(scal[:, 2] - E0) > 1e-6 * Kdiag[:, 0]
+        assert relerr(gscal[ok, 4], scal[ok, 4]) < 1e-9                                   # b_x = bbar/(W-E0)
+        assert relerr(gscal[:, 5], scal[:, 5]) < TOL and np.array_equal(gscal[:, 6], scal[:, 6])   # tau_xi, node flag
+        near_tie = scal[:, 7] < 1e-9
+        assert np.array_equal(gjs[~near_tie], js[~near_tie]) and near_tie.sum() == 0      # selected moves: bit-exact
+    g.close()
+
+
+# ------------------------------------------------------------------------------------------ whole cycles
+@pytest.mark.parametrize("name", list(SYSTEMS))
+@pytest.mark.parametrize("mode", ["balanced", "conventional"])
+def test_whole_cycle_trajectories_weights_and_branching(B, name, mode):
+    s, x0, o, g = _pair(B, name)
+    N = s["n_up"] + s["n_dn"]; n_moves = 30
+    for cycle in (0, 1):
+        if mode == "balanced":
+            assert o.propagate(ref.BALANCED, n_moves, 0.0, -5.0, cycle) == 0
+            g.lrdmc_propagate(B.BALANCED, n_moves, 0.0, -5.0, cycle)
+        else:
+            tau = n_moves * s["a"]**2 / (3 * N)
+            assert o.propagate(ref.CONVENTIONAL, 0, tau, -1.0, cycle) == 0
+            g.lrdmc_propagate(B.CONVENTIONAL, 0, tau, -1.0, cycle)
+        r, du, dd, w = o.get_state(); gr, gdu, gdd, gw = [np_(t) for t in g.lrdmc_get_walkers()]
+        eL, W, om, nm = o.get_obs(); geL, gW, gom, gnm = [np_(t) for t in g.lrdmc_get_obs()]
+        assert np.array_equal(gnm, nm)                                                    # trip counts bit-exact
+        assert np.abs(gr - r).max() < 1e-11                                               # same trajectory
+        assert relerr(gw, w) < 1e-9 and relerr(gom, om) < 1e-9                            # products of ~30 factors
+        Kd = 3 * N / s["a"]**2
+        assert np.max(np.abs(geL - eL) / np.maximum(np.abs(eL), Kd)) < TOL and relerr(gW, W) < TOL
+        rc, par = o.reconfigure(cycle); gpar = np_(g.lrdmc_reconfigure(cycle, want_parents=True))
+        so, sg = o.estimators(), g.lrdmc_estimators()
+        assert np.array_equal(gpar, par)                                                  # reconfiguration indices bit-exact
+        assert abs(sg.wbar - so["wbar"]) <= 1e-9 * so["wbar"]
+        assert abs(sg.num - so["num"]) <= 1e-9 * max(abs(so["num"]), Kd * so["den"]) and abs(sg.den - so["den"]) <= 1e-9 * so["den"]
+        assert (sg.moves_min, sg.moves_max, sg.moves_sum) == (so["moves_min"], so["moves_max"], so["moves_sum"])
+        assert (sg.n_node_flag, sg.n_nonpos_diag, sg.n_nonfinite) == (so["n_node_flag"], so["n_nonpos_diag"], so["n_nonfinite"])
+        assert abs(sg.lockstep_idle_frac - so["lockstep_idle_frac"]) < 1e-12
+        r2, *_ = o.get_state(); gr2 = np_(g.lrdmc_get_walkers()[0])
+        assert np.abs(gr2 - r2).max() < 1e-11 and np.all(np_(g.lrdmc_get_walkers()[3]) == 1.0)
+    g.close()
+
+
+# ------------------------------------------------------------------------------------------ a12: reconfiguration alone
+@pytest.mark.parametrize("n_w", [1, 2, 5, 33, 1024, 1025, 4099])
+def test_reconfigure_indices_bit_exact_for_adversarial_weights(B, n_w):
+    s = wl.hydrogen(); g = B.Lrdmc(s); o = ref.Ref(s); rng = np.random.default_rng(n_w)
+    x0 = wl.hydrogen_walkers(n_w, 2)
+    cases = [rng.random(n_w), rng.random(n_w) ** 8 * 1e-200, np.exp(rng.normal(size=n_w) * 20), np.ones(n_w)]
+    sparse = np.zeros(n_w); sparse[rng.integers(0, n_w, size=max(1, n_w // 50))] = rng.random(max(1, n_w // 50)) + 0.1; cases.append(sparse)
+    for ci, w in enumerate(cases):
+        g.lrdmc_set_state(x0, None, None, w)
+        gpar = np_(g.lrdmc_reconfigure(100 + ci, want_parents=True))
+        rc, par, wbar, *_ = ref.comb(w, o.comb_r32(100 + ci))
+        assert np.array_equal(gpar, par), ci
+        gr = np_(g.lrdmc_get_walkers()[0]); assert np.array_equal(gr, x0[par])
+    # degenerate: all weights zero -> identity, wbar = 0
+    g.lrdmc_set_state(x0, None, None, np.zeros(n_w))
+    assert np.array_equal(np_(g.lrdmc_reconfigure(3, want_parents=True)), np.arange(n_w))
+    g.close()
+
+
+def test_reconfigure_worked_example(B):
+    gold = read_golden("comb_worked_example.txt"); w = np.array([float(v) for v in gold["w"]])
+    s = wl.hydrogen(); g = B.Lrdmc(s); o = ref.Ref(s); x0 = wl.hydrogen_walkers(5, 2)
+    for cycle in range(6):
+        g.lrdmc_set_state(x0, None, None, w)
+        gpar = np_(g.lrdmc_reconfigure(cycle, want_parents=True))
+        assert list(gpar) == list(ref.comb(w, o.comb_r32(cycle))[1])
+
+
+# ------------------------------------------------------------------------------------------ full size, bench launch configuration
+def test_full_size_c4_sampled_walkers_match_oracle(B):
+    """N_w = 25600 (BASELINE configs[3]) in the launch configuration bench.py times; the oracle recomputes sampled walkers one by one."""
+    n_w = 25600
+    s = wl.water_methane(n_walkers=n_w); x0 = wl.initial_walkers(s, n_w, 5)
+    g = B.Lrdmc(s); g.lrdmc_set_positions(x0, allow_singular=True)
+    g.lrdmc_propagate(B.BALANCED, 5, 0.0, 0.0, 0)
+    gr, gdu, gdd, gw = [np_(t) for t in g.lrdmc_get_walkers()]
+    gR, gscal, gjs = [np_(t) for t in g.lrdmc_step_debug(0.0, 1, 0)]
+    o = ref.Ref(s); rng = np.random.default_rng(1); pick = np.sort(rng.choice(n_w, 24, replace=False))
+    for k in pick:
+        u = o.draws(int(k), 1, 0)
+        R, sc, per, _ = o.evaluate(gr[k], ref.frame(u[0], u[1], u[2]), gdu[k], gdd[k])
+        assert relerr(gR[k], R, 1.0) < TOL
+        assert abs(gscal[k, 2] - sc["W"]) < TOL * 1200 and abs(gscal[k, 3] - sc["e_L"]) < TOL * 1200 and abs(gscal[k, 0] - sc["bbar"]) < TOL * 1200
+        assert gjs[k] == o.select(R, u[3])[0]
+    # properties that hold at any size: parents sorted, copies within floor/ceil of N_w w/sum(w), weights reset
+    g.lrdmc_propagate(B.BALANCED, 3, 0.0, 0.0, 2)
+    w = np_(g.lrdmc_get_walkers()[3]); par = np_(g.lrdmc_reconfigure(2, want_parents=True))
+    assert np.array_equal(par, ref.comb(w, o.comb_r32(2))[1])
+    assert np.all(np.diff(par) >= 0)
+    st = g.lrdmc_estimators(); assert abs(st.wbar - w.mean()) < 1e-9 * w.mean() and st.moves_sum == 3 * n_w
+    g.close()
+
+
+# ------------------------------------------------------------------------------------------ runs: energies within 3 sigma
+def test_hydrogen_run_energy_matches_oracle_and_exact(B):
+    from paper_2508_12033_b200 import driver as drv
+    s = wl.hydrogen(alpha=0.9, a=0.2); x0 = wl.hydrogen_walkers(256, 1)
+    g = B.Lrdmc(s); g.lrdmc_set_positions(x0)
+    recs = drv.run(g, B.BALANCED, 200, n_moves=40, E0=-0.495)
+    Eg, sg = B.lrdmc_energy(recs, p=10, n_therm=40, n_blocks=10)
+    o = ref.Ref(s); o.set_positions(x0)
+    out = rdrv.run(o, ref.BALANCED, 200, n_moves=40, E0=-0.495)
+    Eo, so = rdrv.energy(out["wbar"], out["num"], out["den"], p=10, n_therm=40, n_blocks=10)
+    assert abs(Eg - Eo) < 3 * np.hypot(sg, so) and abs(Eg + 0.5) < 3 * sg + 2e-3
+    # same seed, same RNG stream: the first generations are identical to rounding
+    for n in range(5):
+        assert abs(recs[n].num / recs[n].den - out["e"][n]) < 1e-9 and abs(recs[n].wbar - out["wbar"][n]) < 1e-9
+    recs_c = drv.run(g, B.CONVENTIONAL, 200, tau=40 * 0.04 / 3, E0=-0.5, first_cycle=1000)
+    Ec, sc = B.lrdmc_energy(recs_c, p=10, n_therm=40, n_blocks=10)
+    assert abs(Ec - Eg) < 3 * np.hypot(sc, sg) + 1e-3                                     # balanced == conventional (L244)
+    g.close()
+
+
+# ------------------------------------------------------------------------------------------ edge cases and error behaviour
+def test_edge_cases_and_errors(B):
+    s = wl.tiny_molecule(2, 1, 2, 6, seed=7); g = B.Lrdmc(s)
+    with pytest.raises(B.LrdmcError) as e:
+        g.lrdmc_propagate(B.BALANCED, 5, 0.0, 0.0, 0)                                    # nothing bound
+    assert e.value.code == B.ESTATE
+    x0 = wl.initial_walkers(s, 1, 3); g.lrdmc_set_positions(x0)                          # a single walker
+    o = ref.Ref(s); o.set_positions(x0)
+    g.lrdmc_propagate(B.BALANCED, 0, 0.0, -5.0, 0); o.propagate(ref.BALANCED, 0, 0.0, -5.0, 0)   # zero moves: measurement only
+    assert np_(g.lrdmc_get_obs()[3])[0] == 0 and relerr(np_(g.lrdmc_get_obs()[0]), o.get_obs()[0], 100.0) < TOL
+    for bad in (dict(mode=7, n_moves=1, tau=0.0), dict(mode=B.CONVENTIONAL, n_moves=0, tau=0.0), dict(mode=B.BALANCED, n_moves=-1, tau=0.0)):
+        with pytest.raises(B.LrdmcError) as e:
+            g.lrdmc_propagate(bad["mode"], bad["n_moves"], bad["tau"], 0.0, 0)
+        assert e.value.code == B.EINVAL
+    xs = wl.initial_walkers(s, 4, 3); xs[2, 1] = xs[2, 0]                                 # coincident same-spin electrons
+    rc = g.lrdmc_set_positions(xs, allow_singular=True)
+    assert rc in (0, B.ESINGULAR)
+    # W - E0 <= 0 is counted and kills the weight (reading Q16)
+    g.lrdmc_set_positions(wl.initial_walkers(s, 8, 3)); o.set_positions(wl.initial_walkers(s, 8, 3))
+    g.lrdmc_propagate(B.BALANCED, 3, 0.0, 1e6, 0); o.propagate(ref.BALANCED, 3, 0.0, 1e6, 0)
+    g.lrdmc_reconfigure(0); o.reconfigure(0)
+    st = g.lrdmc_estimators(); so = o.estimators()
+    assert st.n_nonpos_diag == so["n_nonpos_diag"] == 8 * 4 and st.wbar == 0.0 == so["wbar"]
+    g.close()
