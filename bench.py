@@ -71,7 +71,7 @@ class ClockSampler:
                 "reasons": reasons, "samples": len(self.rows)}
 
 
-def oracle_sample(sysd, n_w, cycles, moves, seed=5):
+def oracle_sample(sysd, n_w, cycles, moves, seed=5, min_seconds=0.0):
     """The oracle as it stands, timed on the host cores on a bounded sample of the same workload."""
     from oracle import lrdmc_ref as ref
     o = ref.Ref(sysd)
@@ -80,9 +80,9 @@ def oracle_sample(sysd, n_w, cycles, moves, seed=5):
     rc = o.set_positions(x0)
     if rc not in (0, -2):
         raise RuntimeError(f"oracle set_positions failed: {rc}")
-    t0 = time.perf_counter(); n = 0
-    for c in range(cycles):
-        o.propagate(ref.BALANCED, moves, 0.0, -1000.0, c); o.reconfigure(c); n += int(o.estimators()["moves_sum"])
+    t0 = time.perf_counter(); n = 0; c = 0
+    while c < cycles or (min_seconds > 0 and time.perf_counter() - t0 < min_seconds and c < 50 * cycles):
+        o.propagate(ref.BALANCED, moves, 0.0, 0.0, c); o.reconfigure(c); n += int(o.estimators()["moves_sum"]); c += 1
     dt = time.perf_counter() - t0
     return n / dt, cores, dt, n
 
@@ -222,9 +222,9 @@ def main():
     line["clocks"] = clk.summary()
 
     if rank == 0 and not args.no_cpu_baseline and world == 1:
-        v, cores, dt, n = oracle_sample(wl.water_methane(n_walkers=args.ref_nw), args.ref_nw, 4, args.moves)
+        v, cores, dt, n = oracle_sample(wl.water_methane(n_walkers=args.ref_nw), args.ref_nw, 2, args.moves, min_seconds=12.0)
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
-                                "sample": f"same C4 system, N_w={args.ref_nw} walkers x 4 cycles x {args.moves} moves ({n} walker-moves, {dt:.1f} s), balanced, incl. reconfiguration"}
+                                "sample": f"same C4 system, N_w={args.ref_nw} walkers x {n // (args.ref_nw * args.moves)} cycles x {args.moves} moves ({n} walker-moves, {dt:.1f} s), balanced, incl. reconfiguration"}
     if rank == 0:
         print(json.dumps(line), flush=True)
     g.close()

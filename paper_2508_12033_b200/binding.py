@@ -236,7 +236,11 @@ class Lrdmc:
         n_w = int(r_in.shape[0])
         if self.n_w != n_w:
             self.lrdmc_bind_walkers(n_w)
-        r_out = (self.torch.empty((n_w, self.N, 3), dtype=self.torch.float64).pin_memory() if want_positions else None)
+        r_out = None
+        if want_positions:      # pinned result buffer, allocated once per walker count
+            if getattr(self, "_pinned_out", None) is None or self._pinned_out.shape[0] != n_w:
+                self._pinned_out = self.torch.empty((n_w, self.N, 3), dtype=self.torch.float64).pin_memory()
+            r_out = self._pinned_out
         stats = (CycleStats * max(1, n_cycles))()
         pin = r_in.data_ptr() if isinstance(r_in, self.torch.Tensor) else r_in.ctypes.data
         _check(self.L.lrdmc_run_host(self.h, pin, None if r_out is None else r_out.data_ptr(), mode, n_moves, tau, E0, first_cycle, n_cycles,

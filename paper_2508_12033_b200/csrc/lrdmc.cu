@@ -380,6 +380,7 @@ extern "C" int lrdmc_launch_count(const lrdmc_ctx *c) { return c ? c->launches :
 extern "C" int lrdmc_bound_walkers(const lrdmc_ctx *c) { return (c && c->bound) ? c->W.n_w : 0; }
 extern "C" int lrdmc_n_electrons(const lrdmc_ctx *c) { return c ? c->S.N : 0; }
 extern "C" const DevSys *lrdmc_devsys(const lrdmc_ctx *c) { return &c->S; }
+extern "C" double *lrdmc_positions_ptr(const lrdmc_ctx *c, int which) { return which ? c->W.r_alt : c->W.r; }
 extern "C" int lrdmc_launch_config(const lrdmc_ctx *c, int *grid, int *block, int *smem_bytes, int *ctas_per_sm)
 {
     if (!c) return LRDMC_EINVAL;

@@ -54,8 +54,7 @@ extern "C" int lrdmc_run_host(lrdmc_ctx *c, const double *r_in, double *r_out, i
     cudaStream_t st = (cudaStream_t)stream;
     const int n_w = lrdmc_bound_walkers(c); if (n_w <= 0) return LRDMC_ESTATE;
     const size_t bytes = sizeof(double) * (size_t)n_w * 3 * lrdmc_n_electrons(c);
-    double *d_r = NULL;
-    if (cudaMalloc((void **)&d_r, bytes) != cudaSuccess) return LRDMC_ECUDA;
+    double *d_r = lrdmc_positions_ptr(c, 1);      // the gather target doubles as the H2D staging area (no allocation here)
     int rc = LRDMC_OK;
     if (cudaMemcpyAsync(d_r, r_in, bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) rc = LRDMC_ECUDA;
     if (!rc) rc = lrdmc_set_positions(c, d_r, st);
@@ -71,11 +70,9 @@ extern "C" int lrdmc_run_host(lrdmc_ctx *c, const double *r_in, double *r_out, i
         if (mode == LRDMC_BALANCED) E0 = esum / (i + 1);          // "Update E_0" (Alg.2 line 12 L418; reading Q8a)
     }
     if (!rc && r_out) {
-        rc = lrdmc_get_walkers(c, d_r, NULL, NULL, NULL, st);
-        if (!rc && cudaMemcpyAsync(r_out, d_r, bytes, cudaMemcpyDeviceToHost, st) != cudaSuccess) rc = LRDMC_ECUDA;
+        if (cudaMemcpyAsync(r_out, lrdmc_positions_ptr(c, 0), bytes, cudaMemcpyDeviceToHost, st) != cudaSuccess) rc = LRDMC_ECUDA;
     }
     cudaStreamSynchronize(st);
-    cudaFree(d_r);
     return rc;
 }
 

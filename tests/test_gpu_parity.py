@@ -79,7 +79,7 @@ def test_draws_and_frames_match_oracle(B):
     for k in range(0, 500, 3):
         u = o.draws(k, 9, 4)
         assert np.array_equal(out[k, :5], u)                      # uniforms are integer arithmetic: bit-exact
-        assert np.abs(out[k, 5:].reshape(3, 3) - ref.frame(u[0], u[1], u[2])).max() < 4e-16
+        assert np.abs(out[k, 5:].reshape(3, 3) - ref.frame(u[0], u[1], u[2])).max() < 2e-15   # sincospi vs sin(2 pi u): a few ulp
 
 
 # ------------------------------------------------------------------------------------------ a13: inverse build
