@@ -172,8 +172,10 @@ def main():
     achieved = flop["total"] * (moves / len(recs)) / (prop_ms * 1e-3) / 1e12
     traffic = None
     try:
-        with open(os.path.join(ROOT, "profiles", "ncu_propagate_summary.json")) as f:
-            traffic = json.load(f).get("dram_bytes_per_launch")
+        with open(os.path.join(ROOT, "profiles", "ncu_propagate_traffic.txt")) as f:     # last ncu --set full capture (text)
+            for ln in f:
+                if ln.startswith("dram_bytes_per_launch"):
+                    traffic = float(ln.split()[1])
     except Exception:
         pass
     roofline = {"bound": "alu", "kernel": "k_propagate", "achieved": achieved, "peak": peaks["dfma_tflops"], "unit": "TFLOP/s", "frac": achieved / peaks["dfma_tflops"],
