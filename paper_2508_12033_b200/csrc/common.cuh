@@ -4,8 +4,11 @@
 #include <stdint.h>
 #include "../../include/lrdmc.h"
 
-#define LRDMC_NUC_STRIDE 12   // doubles per nucleus row: Rx Ry Rz Z c1 b1 alpha beta gamma delta is_pp pad
-#define LRDMC_EL_ARRAYS 6     // per-electron scratch arrays in shared memory: Jold vei vb lap T spare
+// __builtin_assume(__isShared(p)) made nvcc 12.9 delete the hop (apply_move) from k_propagate: measured, reverted.
+// Address spaces are inferred instead: with TS every per-warp pointer is "shared base + offset" with no global alternative.
+#define LRDMC_ASSUME_SHARED(p) ((void)0)
+#define LRDMC_NUC_STRIDE 12  // doubles per nucleus row: Rx Ry Rz Z c1 b1 alpha beta gamma delta is_pp pad
+#define LRDMC_EL_ARRAYS 4     // per-electron scratch arrays in shared memory: Jold, lap, s_k, old column
 
 // Everything a kernel needs to know about the system; passed by value (fits the 4 KB parameter space).
 struct DevSys {
@@ -27,7 +30,7 @@ struct DevSys {
     // shared-memory plan (units: doubles)
     int bf_in_smem, moc_in_smem;
     int off_shells, off_nuc, off_bf[2], tables_doubles;
-    int o_r, o_dinv[2], o_moc, o_R, o_cum, o_el, per_warp_doubles;
+    int o_r, o_dinv[2], o_moc, o_R, o_cum, o_el, o_ob, per_warp_doubles;
     int dinv_rows[2];     // padded row count 8*NT
 };
 

@@ -2,68 +2,102 @@
 // (Appendix D; rows a1, a4-a10 of the scope table), by ONE WARP on shared-memory state.
 #pragma once
 #include "common.cuh"
+#include "fastmath.cuh"
 #include "philox.cuh"
 #include "wavefunction.cuh"
 
 struct WarpState {            // per-warp views (shared memory; moc may live in global memory for large systems)
-    double *r, *dinv[2], *moc, *R, *cum, *el;
+    double *r, *dinv[2], *moc, *R, *cum, *el, *ob;
 };
 struct EvalOut { double bbar, Vsf, W, eL; int node; };
 
 __device__ __forceinline__ int spin_of(const DevSys &S, int i) { return i < S.n_up ? 0 : 1; }
 
-// Pade pair terms (reading Q14): u = c r/(1+b r), u' = c/(1+br)^2, lap u = 2c/(r (1+br)^3)
-__device__ __forceinline__ double pade_u(double c, double b, double r) { return c * r / (1.0 + b * r); }
-
-// electron-ion potential of one nucleus and its lower bound (Eq.D10 L620; ECP rule L623)
-__device__ __forceinline__ void nuc_potential(const DevSys &S, const double *nu, double r, double &v, double &vb)
+// Address-space hints: all per-warp state and the small tables are shared memory (LDS/STS instead of generic LD/ST);
+// TS = the MO fragment table and the MO cache are in shared memory too (every config except the 64-electron one).
+template <bool TS>
+__device__ __forceinline__ void assume_shared(const WarpState &ws, const double *shells, const double *nuc, const double *const bf[2])
 {
-    double Z = nu[3];
-    if (nu[10] != 0.0) {
-        double r2 = r * r;
-        v = Z * expm1(-nu[6] * r2) / r + Z * nu[6] * r * exp(-nu[7] * r2) + nu[8] * exp(-nu[9] * r2);
-        vb = -Z / r;
-    } else { v = -Z / r; vb = -Z / fmax(r, S.a); }
+    LRDMC_ASSUME_SHARED(ws.r); LRDMC_ASSUME_SHARED(ws.dinv[0]); LRDMC_ASSUME_SHARED(ws.dinv[1]);
+    LRDMC_ASSUME_SHARED(ws.R); LRDMC_ASSUME_SHARED(ws.cum); LRDMC_ASSUME_SHARED(ws.el);
+    LRDMC_ASSUME_SHARED(ws.ob); LRDMC_ASSUME_SHARED(shells); LRDMC_ASSUME_SHARED(nuc);
+    if (TS) { LRDMC_ASSUME_SHARED(ws.moc); LRDMC_ASSUME_SHARED(bf[0]); LRDMC_ASSUME_SHARED(bf[1]); }
 }
 
-template <int NT>
+// electron-ion potential of one nucleus and its lower bound (Eq.D10 L620; ECP rule L623)
+__device__ __forceinline__ void nuc_potential(double a_cut, const double *nu, double r, double ir, double &v, double &vb)
+{
+    const double Z = nu[3];
+    if (nu[10] != 0.0) {
+        const double r2 = r * r;
+        v = Z * expm1(-nu[6] * r2) * ir + Z * nu[6] * r * exp_nonpos(-nu[7] * r2) + nu[8] * exp_nonpos(-nu[9] * r2);
+        vb = -Z * ir;
+    } else { v = -Z * ir; vb = (r > a_cut) ? -Z * ir : -Z / a_cut; }
+}
+
+// One-body cache of electron i (depends on its own position only): ob[i][0..6] = J1_i, grad J1 (3), lap J1, v_ei, v^a_ei.
+// Nuclei are spread over the lanes; called for every electron when a walker is loaded and for the mover after a hop.
+__device__ __forceinline__ void refresh_onebody(int n_nuc, int has_j1, double a_cut, const double *nuc, double *ob_i, double xi, double yi, double zi, int lane)
+{
+    LRDMC_ASSUME_SHARED(nuc); LRDMC_ASSUME_SHARED(ob_i);
+    double J = 0.0, gx = 0.0, gy = 0.0, gz = 0.0, lJ = 0.0, vei = 0.0, vb = 0.0;
+    for (int I = lane; I < n_nuc; I += 32) {
+        const double *nu = nuc + I * LRDMC_NUC_STRIDE;
+        const double dx = xi - nu[0], dy = yi - nu[1], dz = zi - nu[2], r2 = dx * dx + dy * dy + dz * dz;
+        const double ir = fast_rsqrt(r2), r = r2 * ir;
+        if (has_j1) {                                              // u1 = -c1 r/(1+b1 r): u' = c/(1+br)^2, lap u = 2c/(r (1+br)^3)
+            const double c = -nu[4], iq = fast_rcp(1.0 + nu[5] * r), du = c * iq * iq * ir;
+            J += c * r * iq; gx += du * dx; gy += du * dy; gz += du * dz; lJ += 2.0 * du * iq;
+        }
+        double v, b; nuc_potential(a_cut, nu, r, ir, v, b); vei += v; vb += b;
+    }
+    J = warp_sum(J); gx = warp_sum(gx); gy = warp_sum(gy); gz = warp_sum(gz); lJ = warp_sum(lJ); vei = warp_sum(vei); vb = warp_sum(vb);
+    if (lane == 0) { ob_i[0] = J; ob_i[1] = gx; ob_i[2] = gy; ob_i[3] = gz; ob_i[4] = lJ; ob_i[5] = vei; ob_i[6] = vb; }
+}
+
+template <int NT, bool TS>
 __device__ __forceinline__ EvalOut evaluate_walker(const DevSys &S, const WarpState &ws, const double *shells, const double *const bf[2],
                                                    const double *nuc, const double U[9], int lane)
 {
+    assume_shared<TS>(ws, shells, nuc, bf);
     const int N = S.N, n_nuc = S.n_nuc;
     const int t = lane & 3, g = lane >> 2;
-    double *Jold = ws.el, *vei_s = ws.el + N, *vb_s = ws.el + 2 * N, *lap_s = ws.el + 3 * N;
+    double *Jold = ws.el, *lap_s = ws.el + N;
 
-    // ---- phase A (row a6): per-electron continuum pieces.  lane <-> electron.
+    // ---- phase A (row a6): per-electron continuum pieces.  Two lanes per electron split the e-e partners; the
+    //      one-body parts come from the cache.
     double vee_part = 0.0;
-    for (int i = lane; i < N; i += 32) {
-        const int sp = spin_of(S, i), il = sp ? i - S.n_up : i, ns = sp ? S.n_dn : S.n_up;
-        const double xi = ws.r[3 * i], yi = ws.r[3 * i + 1], zi = ws.r[3 * i + 2];
-        double J = 0.0, gx = 0.0, gy = 0.0, gz = 0.0, lJ = 0.0, vei = 0.0, vb = 0.0;
-        for (int I = 0; I < n_nuc; ++I) {
-            const double *nu = nuc + I * LRDMC_NUC_STRIDE;
-            double dx = xi - nu[0], dy = yi - nu[1], dz = zi - nu[2], r = sqrt(dx * dx + dy * dy + dz * dz);
-            if (S.has_j1) {
-                double c = -nu[4], q = 1.0 + nu[5] * r, iq = 1.0 / q, du = c * iq * iq / r;
-                J += c * r * iq; gx += du * dx; gy += du * dy; gz += du * dz; lJ += 2.0 * du * iq;
-            }
-            double v, b; nuc_potential(S, nu, r, v, b); vei += v; vb += b;
-        }
-        for (int j = 0; j < N; ++j) if (j != i) {
-            double dx = xi - ws.r[3 * j], dy = yi - ws.r[3 * j + 1], dz = zi - ws.r[3 * j + 2], r = sqrt(dx * dx + dy * dy + dz * dz);
-            double c = (spin_of(S, j) == sp) ? S.a_par : S.a_anti, q = 1.0 + S.b2 * r, iq = 1.0 / q, du = c * iq * iq / r;
+    for (int i0 = 0; i0 < N; i0 += 16) {
+        const int i = i0 + (lane >> 1), sub = lane & 1;
+        const bool act = i < N;
+        const int ii = act ? i : 0;
+        const int sp = spin_of(S, ii), il = sp ? ii - S.n_up : ii, ns = sp ? S.n_dn : S.n_up;
+        const double xi = ws.r[3 * ii], yi = ws.r[3 * ii + 1], zi = ws.r[3 * ii + 2];
+        double J = 0.0, gx = 0.0, gy = 0.0, gz = 0.0, lJ = 0.0, ve = 0.0;
+        for (int j = sub; j < N; j += 2) if (j != ii) {
+            const double dx = xi - ws.r[3 * j], dy = yi - ws.r[3 * j + 1], dz = zi - ws.r[3 * j + 2], r2 = dx * dx + dy * dy + dz * dz;
+            const double ir = fast_rsqrt(r2), r = r2 * ir;
+            const double c = (spin_of(S, j) == sp) ? S.a_par : S.a_anti, iq = fast_rcp(1.0 + S.b2 * r), du = c * iq * iq * ir;
             J += c * r * iq; gx += du * dx; gy += du * dy; gz += du * dz; lJ += 2.0 * du * iq;
-            if (j > i) vee_part += 1.0 / r;
+            if (j > ii) ve += ir;
         }
-        // grad D / D and lap D / D through the stored inverse and the cached MO rows
-        const double *mc = ws.moc + (size_t)i * 5 * S.OS, *di = ws.dinv[sp] + il;
+        // grad D / D and lap D / D through the stored inverse and the cached MO rows: the two lanes split the MOs
+        const double *mc = ws.moc + (size_t)ii * 5 * S.OS, *di = ws.dinv[sp] + il;
         double Gx = 0.0, Gy = 0.0, Gz = 0.0, Ld = 0.0;
-        for (int m = 0; m < ns; ++m) {
-            double d = di[m * ns];
+        for (int m = sub; m < ns; m += 2) {
+            const double d = di[m * ns];
             Gx += mc[S.OS + m] * d; Gy += mc[2 * S.OS + m] * d; Gz += mc[3 * S.OS + m] * d; Ld += mc[4 * S.OS + m] * d;
         }
-        Jold[i] = J; vei_s[i] = vei; vb_s[i] = vb;
-        lap_s[i] = Ld + 2.0 * (Gx * gx + Gy * gy + Gz * gz) + lJ + (gx * gx + gy * gy + gz * gz);
+#define PAIR_SUM(v) v += __shfl_xor_sync(0xffffffffu, v, 1)
+        PAIR_SUM(J); PAIR_SUM(gx); PAIR_SUM(gy); PAIR_SUM(gz); PAIR_SUM(lJ); PAIR_SUM(Gx); PAIR_SUM(Gy); PAIR_SUM(Gz); PAIR_SUM(Ld);
+#undef PAIR_SUM
+        if (act) vee_part += ve;
+        if (act && sub == 0) {
+            const double *ob = ws.ob + 8 * ii;
+            gx += ob[1]; gy += ob[2]; gz += ob[3];
+            Jold[ii] = J + ob[0];
+            lap_s[ii] = Ld + 2.0 * (Gx * gx + Gy * gy + Gz * gz) + (lJ + ob[4]) + (gx * gx + gy * gy + gz * gz);
+        }
     }
     const double Vee = warp_sum(vee_part);
     __syncwarp();
@@ -86,21 +120,23 @@ __device__ __forceinline__ EvalOut evaluate_walker(const DevSys &S, const WarpSt
                 double part = 0.0;
 #pragma unroll
                 for (int nt = 0; nt < NT; ++nt) {
-                    int m = 8 * nt + 2 * t;
+                    const int m = 8 * nt + 2 * t;
                     part += acc[nt][0] * dinv[m * ns + il] + acc[nt][1] * dinv[(m + 1) * ns + il];
                 }
-                const double dr = quad_sum(part);
-                // Jastrow ratio (row a5): partners split over the 4 lanes of the quad
+                // Jastrow ratio (row a5): partners split over the 4 lanes of the quad; quad-reduce both partial sums together
                 double Jn = 0.0;
                 if (S.has_j1) for (int I = t; I < n_nuc; I += 4) {
                     const double *nu = nuc + I * LRDMC_NUC_STRIDE;
-                    double dx = px - nu[0], dy = py - nu[1], dz = pz - nu[2];
-                    Jn -= pade_u(nu[4], nu[5], sqrt(dx * dx + dy * dy + dz * dz));
+                    const double dx = px - nu[0], dy = py - nu[1], dz = pz - nu[2], r2 = dx * dx + dy * dy + dz * dz;
+                    const double r = r2 * fast_rsqrt(r2);
+                    Jn -= nu[4] * r * fast_rcp(1.0 + nu[5] * r);
                 }
                 for (int j = t; j < N; j += 4) if (j != i) {
-                    double dx = px - ws.r[3 * j], dy = py - ws.r[3 * j + 1], dz = pz - ws.r[3 * j + 2];
-                    Jn += pade_u((spin_of(S, j) == sp) ? S.a_par : S.a_anti, S.b2, sqrt(dx * dx + dy * dy + dz * dz));
+                    const double dx = px - ws.r[3 * j], dy = py - ws.r[3 * j + 1], dz = pz - ws.r[3 * j + 2], r2 = dx * dx + dy * dy + dz * dz;
+                    const double r = r2 * fast_rsqrt(r2);
+                    Jn += ((spin_of(S, j) == sp) ? S.a_par : S.a_anti) * r * fast_rcp(1.0 + S.b2 * r);
                 }
+                const double dr = quad_sum(part);
                 Jn = quad_sum(Jn);
                 if (valid && t == 0) ws.R[mesh * 6 * N + 6 * i + d] = dr * exp(Jn - Jold[i]);
             }
@@ -108,22 +144,29 @@ __device__ __forceinline__ EvalOut evaluate_walker(const DevSys &S, const WarpSt
     }
     __syncwarp();
 
-    // ---- phase C (row a7): fixed-node split (Eq.D1), sequential cumulative sums in candidate order (row a9 needs them)
-    double bbar = 0.0, Vsf = 0.0; int node = 0;
-    if (lane == 0) {
-        const int P = S.P, sixN = 6 * N;
-        for (int mesh = 0, j = 0; mesh < S.n_mesh; ++mesh) {
-            const double kap = S.kappa[mesh];
-            for (int jj = 0; jj < sixN; ++jj, ++j) {
-                double Rj = ws.R[j];
-                if (Rj > 0.0) bbar = __dadd_rn(bbar, __dmul_rn(kap, Rj));
-                else if (Rj < 0.0) { Vsf -= kap * Rj; node = 1; }
-                ws.cum[j] = bbar;
-            }
+    // ---- phase C (row a7): fixed-node split (Eq.D1) and the cumulative sums C_j of the allowed amplitudes, strictly in
+    //      candidate order (row a9 needs them; products rounded before each add, reading Q12).  Each lane owns a contiguous
+    //      chunk of candidates; the running sum is handed from lane to lane, so the association is exactly sequential.
+    const int P = S.P, chunk = (P + 31) >> 5, j0 = lane * chunk;
+    double vsf_part = 0.0; int node = 0;
+    for (int e = 0; e < chunk; ++e) {
+        const int j = j0 + e;
+        double qj = 0.0;
+        if (j < P) {
+            const double Rj = ws.R[j], kap = S.kappa[j >= 6 * N ? 1 : 0];
+            if (Rj > 0.0) qj = __dmul_rn(kap, Rj);
+            else if (Rj < 0.0) { vsf_part -= kap * Rj; node = 1; }
+            ws.cum[j] = qj;                                            // staged amplitude, overwritten by the prefix below
         }
-        (void)P;
     }
-    bbar = __shfl_sync(0xffffffffu, bbar, 0); Vsf = __shfl_sync(0xffffffffu, Vsf, 0); node = __shfl_sync(0xffffffffu, node, 0);
+    double run = 0.0;
+    for (int src = 0; src < 32; ++src) {
+        if (lane == src) for (int e = 0; e < chunk; ++e) { const int j = j0 + e; if (j < P) { run = __dadd_rn(run, ws.cum[j]); ws.cum[j] = run; } }
+        run = __shfl_sync(0xffffffffu, run, src);
+    }
+    const double bbar = run;
+    const double Vsf = warp_sum(vsf_part);
+    node = __any_sync(0xffffffffu, node);
     double vsum = 0.0;
     for (int i = lane; i < N; i += 32) {
         double T = 0.0;
@@ -132,9 +175,9 @@ __device__ __forceinline__ EvalOut evaluate_walker(const DevSys &S, const WarpSt
             double s = Rm[0]; s += Rm[1]; s += Rm[2]; s += Rm[3]; s += Rm[4]; s += Rm[5];
             T += S.g_over_a2[mesh] * (s - 6.0);                      // discretised Laplacian of Eq.D3 over Psi_G
         }
-        double vzv = vei_s[i] + 0.5 * (T - lap_s[i]);                 // Eq.D8
-        double vopt = node ? fmax(vzv, vb_s[i]) : vzv;                // Eq.D9 / D11 (reading Q5: global node flag)
-        vsum += vopt;
+        const double *ob = ws.ob + 8 * i;
+        const double vzv = ob[5] + 0.5 * (T - lap_s[i]);              // Eq.D8
+        vsum += node ? fmax(vzv, ob[6]) : vzv;                        // Eq.D9 / D11 (reading Q5: global node flag)
     }
     vsum = warp_sum(vsum);
     EvalOut o;
@@ -149,6 +192,7 @@ __device__ __forceinline__ EvalOut evaluate_walker(const DevSys &S, const WarpSt
 // fallback = last allowed move; -1 if none is allowed.  All lanes return the same j*.
 __device__ __forceinline__ int select_move(const DevSys &S, const WarpState &ws, double u_sel, int lane)
 {
+    LRDMC_ASSUME_SHARED(ws.cum); LRDMC_ASSUME_SHARED(ws.R);
     const int P = S.P;
     const double tot = ws.cum[P - 1];
     if (!(tot > 0.0)) return -1;
@@ -165,11 +209,12 @@ __device__ __forceinline__ int select_move(const DevSys &S, const WarpState &ws,
     return last;
 }
 
-// Apply move j (row a10): r_i <- r'_j, refresh the cached MO rows of electron i, Sherman-Morrison on Dinv_sigma.
-template <int NT>
-__device__ __forceinline__ void apply_move(const DevSys &S, const WarpState &ws, const double *shells, const double *const bf[2],
+// Apply move j (row a10): r_i <- r'_j, refresh the cached MO rows and the one-body cache of electron i, Sherman-Morrison on Dinv_sigma.
+template <int NT, bool TS>
+__device__ __forceinline__ void apply_move(const DevSys &S, const WarpState &ws, const double *shells, const double *const bf[2], const double *nuc,
                                            const double U[9], int j, int lane)
 {
+    assume_shared<TS>(ws, shells, nuc, bf);
     const int N = S.N, mesh = j / (6 * N), jj = j - mesh * 6 * N, i = jj / 6, d = jj - 6 * i, k = d >> 1;
     const int sp = spin_of(S, i), il = sp ? i - S.n_up : i, ns = sp ? S.n_dn : S.n_up;
     const double step = (d & 1) ? -S.amesh[mesh] : S.amesh[mesh];
@@ -177,20 +222,22 @@ __device__ __forceinline__ void apply_move(const DevSys &S, const WarpState &ws,
     double *mc = ws.moc + (size_t)i * 5 * S.OS;
     __syncwarp();
     refresh_mo_cache<NT>(S, shells, bf[sp], mc, px, py, pz, lane);
+    refresh_onebody(S.n_nuc, S.has_j1, S.a, nuc, ws.ob + 8 * i, px, py, pz, lane);
     if (lane == 0) { ws.r[3 * i] = px; ws.r[3 * i + 1] = py; ws.r[3 * i + 2] = pz; }
     __syncwarp();
     // s_k = sum_m phi_m Dinv[m][k];  rho = s_il;  Dinv'[m][il] = Dinv[m][il]/rho;  Dinv'[m][k] = Dinv[m][k] - Dinv[m][il] s_k / rho
-    double *dinv = ws.dinv[sp], *sk = ws.el + 4 * N, *col = ws.el + 5 * N;   // scratch: s_k and the old column il (n_s <= N each)
+    double *dinv = ws.dinv[sp], *sk = ws.el + 2 * N, *col = ws.el + 3 * N;   // scratch: s_k and the old column il (n_s <= N each)
     for (int kk = lane; kk < ns; kk += 32) {
         double s = 0.0;
         for (int m = 0; m < ns; ++m) s += mc[m] * dinv[m * ns + kk];
         sk[kk] = s; col[kk] = dinv[kk * ns + il];
     }
     __syncwarp();
-    const double rho = sk[il];
+    const double irho = 1.0 / sk[il];
     for (int idx = lane; idx < ns * ns; idx += 32) {
-        int m = idx / ns, kk = idx - m * ns;
-        dinv[idx] = (kk == il) ? col[m] / rho : dinv[idx] - col[m] * sk[kk] / rho;
+        const int m = idx / ns, kk = idx - m * ns;
+        const double ci = col[m] * irho;
+        dinv[idx] = (kk == il) ? ci : dinv[idx] - ci * sk[kk];
     }
     __syncwarp();
 }

@@ -22,7 +22,7 @@ static char g_cuda_msg[256] = "";
 struct lrdmc_ctx {
     DevSys S; DevWalk W;
     void *d_tables; DevStats *d_stats;
-    int NT, wpb, ctas_per_sm, sm_count, smem_bytes, grid_max;
+    int NT, ts, wpb, ctas_per_sm, sm_count, smem_bytes, grid_max;
     int bound, have_prop, have_reconf, state_ok;
     cudaEvent_t ev[4]; cudaStream_t last_stream;
     int launches;   // kernels launched so far (bench.py reports it)
@@ -156,6 +156,7 @@ extern "C" int lrdmc_init(lrdmc_ctx **out, const lrdmc_system *sys, const lrdmc_
     S.o_R = (int)w; w += align_up((size_t)S.P, 2);
     S.o_cum = (int)w; w += align_up((size_t)S.P, 2);
     S.o_el = (int)w; w += align_up((size_t)LRDMC_EL_ARRAYS * S.N, 2);
+    S.o_ob = (int)w; w += 8 * (size_t)S.N;      // one-body cache: J1, grad J1, lap J1, v_ei, v^a_ei per electron
     S.per_warp_doubles = (int)w;
     const size_t per_sm = prop.sharedMemPerMultiprocessor, per_blk_max = prop.sharedMemPerBlockOptin, reserve = 1024;
     c->wpb = 8;
@@ -167,14 +168,16 @@ extern "C" int lrdmc_init(lrdmc_ctx **out, const lrdmc_system *sys, const lrdmc_
     if ((size_t)c->smem_bytes > per_blk_max) { lrdmc_free(c); return LRDMC_ENOMEM; }
     for (int i = 0; i < 4; ++i) cudaEventCreate(&c->ev[i]);
 #define SET_SMEM(K) cudaFuncSetAttribute(K, cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem_bytes)
-    SET_SMEM(k_propagate<1>); SET_SMEM(k_propagate<2>); SET_SMEM(k_propagate<4>);
-    SET_SMEM(k_step_debug<1>); SET_SMEM(k_step_debug<2>); SET_SMEM(k_step_debug<4>);
-    SET_SMEM(k_rebuild<1>); SET_SMEM(k_rebuild<2>); SET_SMEM(k_rebuild<4>);
+#define SET_ALL(NTV, TSV) SET_SMEM((k_propagate<NTV, TSV>)); SET_SMEM((k_step_debug<NTV, TSV>)); SET_SMEM((k_rebuild<NTV, TSV>))
+    SET_ALL(1, true); SET_ALL(2, true); SET_ALL(4, true); SET_ALL(1, false); SET_ALL(2, false); SET_ALL(4, false);
+#undef SET_ALL
 #undef SET_SMEM
+    c->ts = S.bf_in_smem && S.moc_in_smem;
     int occ = 0;
-    if (c->NT == 1) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_propagate<1>, c->wpb * 32, c->smem_bytes);
-    else if (c->NT == 2) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_propagate<2>, c->wpb * 32, c->smem_bytes);
-    else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_propagate<4>, c->wpb * 32, c->smem_bytes);
+#define OCC(NTV, TSV) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_propagate<NTV, TSV>, c->wpb * 32, c->smem_bytes)
+    if (c->ts) { if (c->NT == 1) OCC(1, true); else if (c->NT == 2) OCC(2, true); else OCC(4, true); }
+    else { if (c->NT == 1) OCC(1, false); else if (c->NT == 2) OCC(2, false); else OCC(4, false); }
+#undef OCC
     c->ctas_per_sm = occ > 0 ? occ : 1;
     c->grid_max = c->sm_count * c->ctas_per_sm;
     if (cudaGetLastError() != cudaSuccess) { /* attribute errors surface at launch */ }
@@ -227,11 +230,18 @@ extern "C" int lrdmc_bind_walkers(lrdmc_ctx *c, void *dev_buf, size_t bytes, int
 
 // ---- launch helpers -----------------------------------------------------------------------------------------------
 static int grid_for(const lrdmc_ctx *c) { int g = (c->W.n_w + c->wpb - 1) / c->wpb; return g < c->grid_max ? g : c->grid_max; }
+#define LAUNCH_(KERNEL, NTV, TSV, grid, stream, ...) KERNEL<NTV, TSV><<<grid, c->wpb * 32, c->smem_bytes, stream>>>(__VA_ARGS__)
 #define DISPATCH_NT(KERNEL, grid, stream, ...)                                                                   \
     do {                                                                                                         \
-        if (c->NT == 1) KERNEL<1><<<grid, c->wpb * 32, c->smem_bytes, stream>>>(__VA_ARGS__);                    \
-        else if (c->NT == 2) KERNEL<2><<<grid, c->wpb * 32, c->smem_bytes, stream>>>(__VA_ARGS__);               \
-        else KERNEL<4><<<grid, c->wpb * 32, c->smem_bytes, stream>>>(__VA_ARGS__);                               \
+        if (c->ts) {                                                                                             \
+            if (c->NT == 1) LAUNCH_(KERNEL, 1, true, grid, stream, __VA_ARGS__);                                 \
+            else if (c->NT == 2) LAUNCH_(KERNEL, 2, true, grid, stream, __VA_ARGS__);                            \
+            else LAUNCH_(KERNEL, 4, true, grid, stream, __VA_ARGS__);                                            \
+        } else {                                                                                                 \
+            if (c->NT == 1) LAUNCH_(KERNEL, 1, false, grid, stream, __VA_ARGS__);                                \
+            else if (c->NT == 2) LAUNCH_(KERNEL, 2, false, grid, stream, __VA_ARGS__);                           \
+            else LAUNCH_(KERNEL, 4, false, grid, stream, __VA_ARGS__);                                           \
+        }                                                                                                        \
         ++c->launches;                                                                                           \
     } while (0)
 

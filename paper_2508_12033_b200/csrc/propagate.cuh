@@ -17,10 +17,14 @@ __device__ __forceinline__ void stage_tables(const DevSys &S, double *smem)
     __syncthreads();
 }
 
+// TS (tables + MO cache in shared memory): every pointer below is "shared base + offset" with no global alternative, so the
+// compiler's address-space inference emits LDS/STS.  !TS (64-electron config): fragments / cache stay in global memory.
+template <bool TS>
 __device__ __forceinline__ void table_pointers(const DevSys &S, const double *smem, const double *&shells, const double *&nuc, const double *bf[2])
 {
     shells = smem + S.off_shells; nuc = smem + S.off_nuc;
-    if (S.bf_in_smem) { bf[0] = smem + S.off_bf[0]; bf[1] = S.same_C ? bf[0] : smem + S.off_bf[1]; }
+    if (TS) { bf[0] = smem + S.off_bf[0]; bf[1] = smem + (S.same_C ? S.off_bf[0] : S.off_bf[1]); }
+    else if (S.bf_in_smem) { bf[0] = smem + S.off_bf[0]; bf[1] = S.same_C ? bf[0] : smem + S.off_bf[1]; }
     else { bf[0] = S.bfrag[0]; bf[1] = S.same_C ? S.bfrag[0] : S.bfrag[1]; }
 }
 
@@ -29,11 +33,12 @@ __device__ __forceinline__ WarpState warp_views(const DevSys &S, double *smem, i
     double *base = smem + S.tables_doubles + (size_t)warp * S.per_warp_doubles;
     WarpState ws;
     ws.r = base + S.o_r; ws.dinv[0] = base + S.o_dinv[0]; ws.dinv[1] = base + S.o_dinv[1];
-    ws.moc = base + S.o_moc; ws.R = base + S.o_R; ws.cum = base + S.o_cum; ws.el = base + S.o_el;
+    ws.moc = base + S.o_moc; ws.R = base + S.o_R; ws.cum = base + S.o_cum; ws.el = base + S.o_el; ws.ob = base + S.o_ob;
     return ws;
 }
 
-__device__ __forceinline__ void load_walker(const DevSys &S, const DevWalk &W, WarpState &ws, int k, int lane, bool with_dinv)
+template <bool TS>
+__device__ __forceinline__ void load_walker(const DevSys &S, const DevWalk &W, WarpState &ws, const double *nuc, int k, int lane, bool with_dinv)
 {
     const int N = S.N;
     for (int i = lane; i < 3 * N; i += 32) ws.r[i] = W.r[(size_t)k * 3 * N + i];
@@ -43,8 +48,10 @@ __device__ __forceinline__ void load_walker(const DevSys &S, const DevWalk &W, W
         for (int i = lane; i < tot; i += 32) ws.dinv[sp][i] = (with_dinv && i < ns * ns) ? src[i] : 0.0;
     }
     const size_t mocn = (size_t)N * 5 * S.OS;
-    if (S.moc_in_smem) { for (int i = lane; i < (int)mocn; i += 32) ws.moc[i] = W.moc[(size_t)k * mocn + i]; }
+    if (TS || S.moc_in_smem) { for (int i = lane; i < (int)mocn; i += 32) ws.moc[i] = W.moc[(size_t)k * mocn + i]; }
     else ws.moc = W.moc + (size_t)k * mocn;
+    __syncwarp();
+    for (int i = 0; i < N; ++i) refresh_onebody(S.n_nuc, S.has_j1, S.a, nuc, ws.ob + 8 * i, ws.r[3 * i], ws.r[3 * i + 1], ws.r[3 * i + 2], lane);
     __syncwarp();
 }
 
@@ -64,14 +71,14 @@ __device__ __forceinline__ void store_walker(const DevSys &S, const DevWalk &W, 
 }
 
 // ---- the projection kernel (Alg.2 lines 4-8 L401-L410 / Alg.1 lines 4-16 L350-L374) ----------------------------
-template <int NT>
+template <int NT, bool TS>
 __global__ void __launch_bounds__(256) k_propagate(DevSys S, DevWalk W, int mode, int n_moves, double tau, double E0, uint32_t cycle)
 {
     extern __shared__ __align__(16) double smem[];
     stage_tables(S, smem);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, gwarp = blockIdx.x * (blockDim.x >> 5) + warp;
     const double *shells, *nuc, *bf[2];
-    table_pointers(S, smem, shells, nuc, bf);
+    table_pointers<TS>(S, smem, shells, nuc, bf);
     WarpState ws = warp_views(S, smem, warp);
     const unsigned long long t_start = globaltimer_ns();
     for (;;) {
@@ -79,13 +86,13 @@ __global__ void __launch_bounds__(256) k_propagate(DevSys S, DevWalk W, int mode
         if (lane == 0) k = atomicAdd(W.counter, 1);
         k = __shfl_sync(0xffffffffu, k, 0);
         if (k >= W.n_w) break;
-        load_walker(S, W, ws, k, lane, true);
+        load_walker<TS>(S, W, ws, nuc, k, lane, true);
         double w = 1.0, tau_left = tau, omega = 0.0, eL_out = 0.0, W_out = 0.0;
         long long moves = 0; int n_node = 0, n_nonpos = 0;
         for (uint32_t s = 0;; ++s) {
             const StepDraws d = step_draws(S, (uint32_t)k, cycle, s, mode == LRDMC_CONVENTIONAL);
             double U[9]; lattice_frame(d.u1, d.u2, d.u3, U);
-            const EvalOut e = evaluate_walker<NT>(S, ws, shells, bf, nuc, U, lane);
+            const EvalOut e = evaluate_walker<NT, TS>(S, ws, shells, bf, nuc, U, lane);
             n_node += e.node;
             bool last = false;
             if (mode == LRDMC_BALANCED) {
@@ -104,7 +111,7 @@ __global__ void __launch_bounds__(256) k_propagate(DevSys S, DevWalk W, int mode
             }
             if (last) { eL_out = e.eL; W_out = e.W; break; }
             const int j = select_move(S, ws, d.u_sel, lane);       // Alg.2 line 7 (L408)
-            if (j >= 0) { apply_move<NT>(S, ws, shells, bf, U, j, lane); ++moves; }
+            if (j >= 0) { apply_move<NT, TS>(S, ws, shells, bf, nuc, U, j, lane); ++moves; }
         }
         int nonfinite = 0;
         if (!isfinite(w) || !isfinite(omega)) { nonfinite = 1; w = 0.0; omega = 0.0; }
@@ -118,7 +125,7 @@ __global__ void __launch_bounds__(256) k_propagate(DevSys S, DevWalk W, int mode
 }
 
 // ---- parity hook: one evaluation + selection, no state change ---------------------------------------------------
-template <int NT>
+template <int NT, bool TS>
 __global__ void __launch_bounds__(256) k_step_debug(DevSys S, DevWalk W, double E0, uint32_t cycle, uint32_t step, double *R_out,
                                                     double *scal_out, int *jstar_out)
 {
@@ -126,13 +133,13 @@ __global__ void __launch_bounds__(256) k_step_debug(DevSys S, DevWalk W, double 
     stage_tables(S, smem);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, wpb = blockDim.x >> 5;
     const double *shells, *nuc, *bf[2];
-    table_pointers(S, smem, shells, nuc, bf);
+    table_pointers<TS>(S, smem, shells, nuc, bf);
     WarpState ws = warp_views(S, smem, warp);
     for (int k = blockIdx.x * wpb + warp; k < W.n_w; k += gridDim.x * wpb) {
-        load_walker(S, W, ws, k, lane, true);
+        load_walker<TS>(S, W, ws, nuc, k, lane, true);
         const StepDraws d = step_draws(S, (uint32_t)k, cycle, step, true);
         double U[9]; lattice_frame(d.u1, d.u2, d.u3, U);
-        const EvalOut e = evaluate_walker<NT>(S, ws, shells, bf, nuc, U, lane);
+        const EvalOut e = evaluate_walker<NT, TS>(S, ws, shells, bf, nuc, U, lane);
         const int j = select_move(S, ws, d.u_sel, lane);
         for (int p = lane; p < S.P; p += 32) R_out[(size_t)k * S.P + p] = ws.R[p];
         if (lane == 0) {
@@ -147,18 +154,18 @@ __global__ void __launch_bounds__(256) k_step_debug(DevSys S, DevWalk W, double 
 }
 
 // ---- (re)build of the inverses and MO caches from the positions (row a13) ---------------------------------------
-template <int NT>
+template <int NT, bool TS>
 __global__ void __launch_bounds__(256) k_rebuild(DevSys S, DevWalk W, int do_invert)
 {
     extern __shared__ __align__(16) double smem[];
     stage_tables(S, smem);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, wpb = blockDim.x >> 5;
     const double *shells, *nuc, *bf[2];
-    table_pointers(S, smem, shells, nuc, bf);
+    table_pointers<TS>(S, smem, shells, nuc, bf);
     WarpState ws = warp_views(S, smem, warp);
     const int N = S.N;
     for (int k = blockIdx.x * wpb + warp; k < W.n_w; k += gridDim.x * wpb) {
-        load_walker(S, W, ws, k, lane, !do_invert);
+        load_walker<TS>(S, W, ws, nuc, k, lane, !do_invert);
         for (int i = 0; i < N; ++i) {
             const int sp = spin_of(S, i);
             refresh_mo_cache<NT>(S, shells, bf[sp], ws.moc + (size_t)i * 5 * S.OS, ws.r[3 * i], ws.r[3 * i + 1], ws.r[3 * i + 2], lane);

@@ -9,6 +9,7 @@
 // padded to multiples of 4 -- all four k slots always run the same code.  Accumulator: lane holds MO (2t, 2t+1) of point g.
 #pragma once
 #include "common.cuh"
+#include "fastmath.cuh"
 
 __device__ __forceinline__ void dmma884(double &c0, double &c1, double a, double b)
 {
@@ -58,7 +59,7 @@ __device__ __forceinline__ void mo_pass(const DevSys &S, const double *__restric
     // ---- group 0: Slater-type s, chi = exp(-z r); grad = -z chi rhat; lap = chi (z^2 - 2 z / r)
     for (int it = 0; it < S.n_it[0]; ++it, sh4 += 4) {
         double4 s = *sh4; double dx = px - s.x, dy = py - s.y, dz = pz - s.z, z = s.w;
-        double r = sqrt(dx * dx + dy * dy + dz * dz), e = exp(-z * r);
+        double r = sqrt(dx * dx + dy * dy + dz * dz), e = exp_nonpos(-z * r);
         if (!DERIV) { LRDMC_FEED(e); }
         else {
             double ir = 1.0 / r, d = (g == 1) ? dx : ((g == 2) ? dy : dz);
@@ -69,14 +70,14 @@ __device__ __forceinline__ void mo_pass(const DevSys &S, const double *__restric
     // ---- group 1: s Gaussians
     for (int it = 0; it < S.n_it[1]; ++it, sh4 += 4) {
         double4 s = *sh4; double dx = px - s.x, dy = py - s.y, dz = pz - s.z, z = s.w;
-        double e = exp(-z * (dx * dx + dy * dy + dz * dz));
+        double e = exp_nonpos(-z * (dx * dx + dy * dy + dz * dz));
         if (!DERIV) { LRDMC_FEED(e); }
         else { AxisPoly X = axis_poly(dx, z), Y = axis_poly(dy, z), Z = axis_poly(dz, z); LRDMC_FEED((gto_component<0, 0, 0>(g, X, Y, Z, e))); }
     }
     // ---- group 2: p Gaussians (x, y, z)
     for (int it = 0; it < S.n_it[2]; ++it, sh4 += 4) {
         double4 s = *sh4; double dx = px - s.x, dy = py - s.y, dz = pz - s.z, z = s.w;
-        double e = exp(-z * (dx * dx + dy * dy + dz * dz));
+        double e = exp_nonpos(-z * (dx * dx + dy * dy + dz * dz));
         if (!DERIV) { LRDMC_FEED(dx * e); LRDMC_FEED(dy * e); LRDMC_FEED(dz * e); }
         else {
             AxisPoly X = axis_poly(dx, z), Y = axis_poly(dy, z), Z = axis_poly(dz, z);
@@ -87,7 +88,7 @@ __device__ __forceinline__ void mo_pass(const DevSys &S, const double *__restric
     // ---- group 3: d Gaussians (xx, xy, xz, yy, yz, zz)
     for (int it = 0; it < S.n_it[3]; ++it, sh4 += 4) {
         double4 s = *sh4; double dx = px - s.x, dy = py - s.y, dz = pz - s.z, z = s.w;
-        double e = exp(-z * (dx * dx + dy * dy + dz * dz));
+        double e = exp_nonpos(-z * (dx * dx + dy * dy + dz * dz));
         if (!DERIV) {
             double xe = dx * e, ye = dy * e, ze = dz * e;
             LRDMC_FEED(dx * xe); LRDMC_FEED(dx * ye); LRDMC_FEED(dx * ze); LRDMC_FEED(dy * ye); LRDMC_FEED(dy * ze); LRDMC_FEED(dz * ze);
