@@ -30,7 +30,7 @@ struct DevSys {
     // shared-memory plan (units: doubles)
     int bf_in_smem, moc_in_smem;
     int off_shells, off_nuc, off_bf[2], tables_doubles;
-    int o_r, o_dinv[2], o_moc, o_R, o_cum, o_el, o_ob, per_warp_doubles;
+    int o_r, o_dinv[2], o_moc, o_R, o_cum, o_el, o_ob, o_U, per_warp_doubles;
     int dinv_rows[2];     // padded row count 8*NT
 };
 

@@ -7,7 +7,7 @@
 #include "wavefunction.cuh"
 
 struct WarpState {            // per-warp views (shared memory; moc may live in global memory for large systems)
-    double *r, *dinv[2], *moc, *R, *cum, *el, *ob;
+    double *r, *dinv[2], *moc, *R, *cum, *el, *ob, *U;
 };
 struct EvalOut { double bbar, Vsf, W, eL; int node; };
 
@@ -57,9 +57,8 @@ __device__ __forceinline__ void refresh_onebody(int n_nuc, int has_j1, double a_
 
 template <int NT, bool TS>
 __device__ __forceinline__ EvalOut evaluate_walker(const DevSys &S, const WarpState &ws, const double *shells, const double *const bf[2],
-                                                   const double *nuc, const double U[9], int lane)
+                                                   const double *nuc, int lane)
 {
-    assume_shared<TS>(ws, shells, nuc, bf);
     const int N = S.N, n_nuc = S.n_nuc;
     const int t = lane & 3, g = lane >> 2;
     double *Jold = ws.el, *lap_s = ws.el + N;
@@ -102,69 +101,86 @@ __device__ __forceinline__ EvalOut evaluate_walker(const DevSys &S, const WarpSt
     const double Vee = warp_sum(vee_part);
     __syncwarp();
 
-    // ---- phase B (rows a1-a5): candidates in batches of 8 points through the tensor-core MO pass
+    // ---- phase B (rows a1-a5): candidates, 16 points (two mma batches of 8) per warp pass through the tensor-core MO pass
     for (int mesh = 0; mesh < S.n_mesh; ++mesh) {
         const double am = S.amesh[mesh];
         for (int sp = 0; sp < 2; ++sp) {
             const int ns = sp ? S.n_dn : S.n_up, off = sp ? S.n_up : 0, npts = 6 * ns;
             if (ns == 0) continue;
             const double *dinv = ws.dinv[sp];
-            for (int q0 = 0; q0 < npts; q0 += 8) {
-                const bool valid = q0 + g < npts;
-                const int q = valid ? q0 + g : 0, il = q / 6, d = q - 6 * il, i = off + il, k = d >> 1;
-                const double step = (d & 1) ? -am : am;
-                const double px = ws.r[3 * i] + step * U[k], py = ws.r[3 * i + 1] + step * U[3 + k], pz = ws.r[3 * i + 2] + step * U[6 + k];
-                double acc[NT][2];
-                mo_pass<NT, false>(S, shells, bf[sp], px, py, pz, lane, acc);
-                // determinant ratio (row a4): sum_m phi_m(r') Dinv[m][il]; this lane holds m = 8 nt + 2t, +1 (rows beyond n_s are zero-padded)
-                double part = 0.0;
+            for (int q0 = 0; q0 < npts; q0 += 16) {
+                bool valid[2]; int ci[2], cd[2], cil[2]; double pt[2][3];
 #pragma unroll
-                for (int nt = 0; nt < NT; ++nt) {
-                    const int m = 8 * nt + 2 * t;
-                    part += acc[nt][0] * dinv[m * ns + il] + acc[nt][1] * dinv[(m + 1) * ns + il];
+                for (int h = 0; h < 2; ++h) {
+                    valid[h] = q0 + 8 * h + g < npts;
+                    const int q = valid[h] ? q0 + 8 * h + g : 0, il = q / 6, d = q - 6 * il, i = off + il, k = d >> 1;
+                    const double step = (d & 1) ? -am : am;
+                    ci[h] = i; cd[h] = d; cil[h] = il;
+                    pt[h][0] = ws.r[3 * i] + step * ws.U[k]; pt[h][1] = ws.r[3 * i + 1] + step * ws.U[3 + k]; pt[h][2] = ws.r[3 * i + 2] + step * ws.U[6 + k];
                 }
-                // Jastrow ratio (row a5): partners split over the 4 lanes of the quad; quad-reduce both partial sums together
-                double Jn = 0.0;
+                double acc[2][NT][2];
+                mo_values2<NT>(S, shells, bf[sp], pt[0], pt[1], lane, acc);
+                // determinant ratio (row a4): sum_m phi_m(r') Dinv[m][il]; this lane holds m = 8 nt + 2t, +1 (rows beyond n_s are zero-padded)
+                double part[2] = { 0.0, 0.0 }, Jn[2] = { 0.0, 0.0 };
+#pragma unroll
+                for (int h = 0; h < 2; ++h)
+#pragma unroll
+                    for (int nt = 0; nt < NT; ++nt) {
+                        const int m = 8 * nt + 2 * t;
+                        part[h] += acc[h][nt][0] * dinv[m * ns + cil[h]] + acc[h][nt][1] * dinv[(m + 1) * ns + cil[h]];
+                    }
+                // Jastrow ratio (row a5): partners split over the 4 lanes of the quad; both points share each partner load
                 if (S.has_j1) for (int I = t; I < n_nuc; I += 4) {
                     const double *nu = nuc + I * LRDMC_NUC_STRIDE;
-                    const double dx = px - nu[0], dy = py - nu[1], dz = pz - nu[2], r2 = dx * dx + dy * dy + dz * dz;
-                    const double r = r2 * fast_rsqrt(r2);
-                    Jn -= nu[4] * r * fast_rcp(1.0 + nu[5] * r);
+                    const double nx = nu[0], ny = nu[1], nz = nu[2], c1 = nu[4], b1 = nu[5];
+#pragma unroll
+                    for (int h = 0; h < 2; ++h) {
+                        const double dx = pt[h][0] - nx, dy = pt[h][1] - ny, dz = pt[h][2] - nz, r2 = dx * dx + dy * dy + dz * dz;
+                        const double r = r2 * fast_rsqrt(r2);
+                        Jn[h] -= c1 * r * fast_rcp(1.0 + b1 * r);
+                    }
                 }
-                for (int j = t; j < N; j += 4) if (j != i) {
-                    const double dx = px - ws.r[3 * j], dy = py - ws.r[3 * j + 1], dz = pz - ws.r[3 * j + 2], r2 = dx * dx + dy * dy + dz * dz;
-                    const double r = r2 * fast_rsqrt(r2);
-                    Jn += ((spin_of(S, j) == sp) ? S.a_par : S.a_anti) * r * fast_rcp(1.0 + S.b2 * r);
+                for (int j = t; j < N; j += 4) {
+                    const double jx = ws.r[3 * j], jy = ws.r[3 * j + 1], jz = ws.r[3 * j + 2];
+                    const double cpar = (spin_of(S, j) == sp) ? S.a_par : S.a_anti;
+#pragma unroll
+                    for (int h = 0; h < 2; ++h) {
+                        const double dx = pt[h][0] - jx, dy = pt[h][1] - jy, dz = pt[h][2] - jz, r2 = dx * dx + dy * dy + dz * dz;
+                        const double r = r2 * fast_rsqrt(r2);
+                        const double u = cpar * r * fast_rcp(1.0 + S.b2 * r);
+                        if (j != ci[h]) Jn[h] += u;
+                    }
                 }
-                const double dr = quad_sum(part);
-                Jn = quad_sum(Jn);
-                if (valid && t == 0) ws.R[mesh * 6 * N + 6 * i + d] = dr * exp(Jn - Jold[i]);
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    const double dr = quad_sum(part[h]), dJ = quad_sum(Jn[h]) - Jold[ci[h]];
+                    if (valid[h] && t == 0) ws.R[mesh * 6 * N + 6 * ci[h] + cd[h]] = dr * exp(dJ);
+                }
             }
         }
     }
     __syncwarp();
 
-    // ---- phase C (row a7): fixed-node split (Eq.D1) and the cumulative sums C_j of the allowed amplitudes, strictly in
-    //      candidate order (row a9 needs them; products rounded before each add, reading Q12).  Each lane owns a contiguous
-    //      chunk of candidates; the running sum is handed from lane to lane, so the association is exactly sequential.
+    // ---- phase C (row a7): fixed-node split (Eq.D1) and the cumulative sums C_j of the allowed amplitudes in candidate
+    //      order (row a9 searches them).  Each lane owns a contiguous chunk; chunk totals are scanned across the warp
+    //      (reading Q12: the summation order is free, a draw closer than 1e-9 to a bin edge is a reported near-tie).
     const int P = S.P, chunk = (P + 31) >> 5, j0 = lane * chunk;
-    double vsf_part = 0.0; int node = 0;
+    double vsf_part = 0.0, loc = 0.0; int node = 0;
     for (int e = 0; e < chunk; ++e) {
         const int j = j0 + e;
-        double qj = 0.0;
         if (j < P) {
             const double Rj = ws.R[j], kap = S.kappa[j >= 6 * N ? 1 : 0];
-            if (Rj > 0.0) qj = __dmul_rn(kap, Rj);
+            if (Rj > 0.0) loc += kap * Rj;
             else if (Rj < 0.0) { vsf_part -= kap * Rj; node = 1; }
-            ws.cum[j] = qj;                                            // staged amplitude, overwritten by the prefix below
+            ws.cum[j] = loc;
         }
     }
-    double run = 0.0;
-    for (int src = 0; src < 32; ++src) {
-        if (lane == src) for (int e = 0; e < chunk; ++e) { const int j = j0 + e; if (j < P) { run = __dadd_rn(run, ws.cum[j]); ws.cum[j] = run; } }
-        run = __shfl_sync(0xffffffffu, run, src);
-    }
-    const double bbar = run;
+    double inc = loc;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const double v = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += v; }
+    double excl = __shfl_up_sync(0xffffffffu, inc, 1); if (lane == 0) excl = 0.0;
+    for (int e = 0; e < chunk; ++e) { const int j = j0 + e; if (j < P) ws.cum[j] += excl; }
+    const double bbar = __shfl_sync(0xffffffffu, inc, 31);
     const double Vsf = warp_sum(vsf_part);
     node = __any_sync(0xffffffffu, node);
     double vsum = 0.0;
@@ -212,13 +228,12 @@ __device__ __forceinline__ int select_move(const DevSys &S, const WarpState &ws,
 // Apply move j (row a10): r_i <- r'_j, refresh the cached MO rows and the one-body cache of electron i, Sherman-Morrison on Dinv_sigma.
 template <int NT, bool TS>
 __device__ __forceinline__ void apply_move(const DevSys &S, const WarpState &ws, const double *shells, const double *const bf[2], const double *nuc,
-                                           const double U[9], int j, int lane)
+                                           int j, int lane)
 {
-    assume_shared<TS>(ws, shells, nuc, bf);
     const int N = S.N, mesh = j / (6 * N), jj = j - mesh * 6 * N, i = jj / 6, d = jj - 6 * i, k = d >> 1;
     const int sp = spin_of(S, i), il = sp ? i - S.n_up : i, ns = sp ? S.n_dn : S.n_up;
     const double step = (d & 1) ? -S.amesh[mesh] : S.amesh[mesh];
-    const double px = ws.r[3 * i] + step * U[k], py = ws.r[3 * i + 1] + step * U[3 + k], pz = ws.r[3 * i + 2] + step * U[6 + k];
+    const double px = ws.r[3 * i] + step * ws.U[k], py = ws.r[3 * i + 1] + step * ws.U[3 + k], pz = ws.r[3 * i + 2] + step * ws.U[6 + k];
     double *mc = ws.moc + (size_t)i * 5 * S.OS;
     __syncwarp();
     refresh_mo_cache<NT>(S, shells, bf[sp], mc, px, py, pz, lane);

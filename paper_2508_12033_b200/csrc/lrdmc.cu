@@ -156,6 +156,7 @@ extern "C" int lrdmc_init(lrdmc_ctx **out, const lrdmc_system *sys, const lrdmc_
     S.o_R = (int)w; w += align_up((size_t)S.P, 2);
     S.o_cum = (int)w; w += align_up((size_t)S.P, 2);
     S.o_el = (int)w; w += align_up((size_t)LRDMC_EL_ARRAYS * S.N, 2);
+    S.o_U = (int)w; w += 10;                    // the step's lattice frame (9 doubles)
     S.o_ob = (int)w; w += 8 * (size_t)S.N;      // one-body cache: J1, grad J1, lap J1, v_ei, v^a_ei per electron
     S.per_warp_doubles = (int)w;
     const size_t per_sm = prop.sharedMemPerMultiprocessor, per_blk_max = prop.sharedMemPerBlockOptin, reserve = 1024;

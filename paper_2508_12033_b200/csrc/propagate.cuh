@@ -33,8 +33,18 @@ __device__ __forceinline__ WarpState warp_views(const DevSys &S, double *smem, i
     double *base = smem + S.tables_doubles + (size_t)warp * S.per_warp_doubles;
     WarpState ws;
     ws.r = base + S.o_r; ws.dinv[0] = base + S.o_dinv[0]; ws.dinv[1] = base + S.o_dinv[1];
-    ws.moc = base + S.o_moc; ws.R = base + S.o_R; ws.cum = base + S.o_cum; ws.el = base + S.o_el; ws.ob = base + S.o_ob;
+    ws.moc = base + S.o_moc; ws.R = base + S.o_R; ws.cum = base + S.o_cum; ws.el = base + S.o_el; ws.ob = base + S.o_ob; ws.U = base + S.o_U;
     return ws;
+}
+
+// the step's lattice frame, computed by lane 0 and published in shared memory (the versors are indexed by direction)
+__device__ __forceinline__ void publish_frame(const WarpState &ws, const StepDraws &d, int lane)
+{
+    __syncwarp();
+    if (lane == 0) { double U[9]; lattice_frame(d.u1, d.u2, d.u3, U);
+#pragma unroll
+        for (int i = 0; i < 9; ++i) ws.U[i] = U[i]; }
+    __syncwarp();
 }
 
 template <bool TS>
@@ -91,8 +101,8 @@ __global__ void __launch_bounds__(256) k_propagate(DevSys S, DevWalk W, int mode
         long long moves = 0; int n_node = 0, n_nonpos = 0;
         for (uint32_t s = 0;; ++s) {
             const StepDraws d = step_draws(S, (uint32_t)k, cycle, s, mode == LRDMC_CONVENTIONAL);
-            double U[9]; lattice_frame(d.u1, d.u2, d.u3, U);
-            const EvalOut e = evaluate_walker<NT, TS>(S, ws, shells, bf, nuc, U, lane);
+            publish_frame(ws, d, lane);
+            const EvalOut e = evaluate_walker<NT, TS>(S, ws, shells, bf, nuc, lane);
             n_node += e.node;
             bool last = false;
             if (mode == LRDMC_BALANCED) {
@@ -111,7 +121,7 @@ __global__ void __launch_bounds__(256) k_propagate(DevSys S, DevWalk W, int mode
             }
             if (last) { eL_out = e.eL; W_out = e.W; break; }
             const int j = select_move(S, ws, d.u_sel, lane);       // Alg.2 line 7 (L408)
-            if (j >= 0) { apply_move<NT, TS>(S, ws, shells, bf, nuc, U, j, lane); ++moves; }
+            if (j >= 0) { apply_move<NT, TS>(S, ws, shells, bf, nuc, j, lane); ++moves; }
         }
         int nonfinite = 0;
         if (!isfinite(w) || !isfinite(omega)) { nonfinite = 1; w = 0.0; omega = 0.0; }
@@ -138,8 +148,8 @@ __global__ void __launch_bounds__(256) k_step_debug(DevSys S, DevWalk W, double 
     for (int k = blockIdx.x * wpb + warp; k < W.n_w; k += gridDim.x * wpb) {
         load_walker<TS>(S, W, ws, nuc, k, lane, true);
         const StepDraws d = step_draws(S, (uint32_t)k, cycle, step, true);
-        double U[9]; lattice_frame(d.u1, d.u2, d.u3, U);
-        const EvalOut e = evaluate_walker<NT, TS>(S, ws, shells, bf, nuc, U, lane);
+        publish_frame(ws, d, lane);
+        const EvalOut e = evaluate_walker<NT, TS>(S, ws, shells, bf, nuc, lane);
         const int j = select_move(S, ws, d.u_sel, lane);
         for (int p = lane; p < S.P; p += 32) R_out[(size_t)k * S.P + p] = ws.R[p];
         if (lane == 0) {

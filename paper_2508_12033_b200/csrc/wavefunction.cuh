@@ -102,6 +102,59 @@ __device__ __forceinline__ void mo_pass(const DevSys &S, const double *__restric
 #undef LRDMC_FEED
 }
 
+// Value-only pass over TWO batches of 8 points at once (16 candidate points per warp pass): every shell row and every
+// B fragment is loaded once and used twice, and the two exponential chains of a lane are independent (ILP 2), which is
+// what the FP64 pipe needs with 4 warps per scheduler.  acc[b] = accumulators of batch b.
+template <int NT>
+__device__ __forceinline__ void mo_values2(const DevSys &S, const double *__restrict__ shells, const double *__restrict__ bf,
+                                           const double (&p0)[3], const double (&p1)[3], int lane, double (&acc)[2][NT][2])
+{
+    const int t = lane & 3;
+    const double4 *sh4 = reinterpret_cast<const double4 *>(shells) + t;
+    const double *b = bf + lane;
+#pragma unroll
+    for (int nt = 0; nt < NT; ++nt) { acc[0][nt][0] = 0.0; acc[0][nt][1] = 0.0; acc[1][nt][0] = 0.0; acc[1][nt][1] = 0.0; }
+#define LRDMC_FEED2(a0val, a1val)                                                               \
+    {                                                                                           \
+        const double a0_ = (a0val), a1_ = (a1val);                                              \
+        _Pragma("unroll") for (int nt = 0; nt < NT; ++nt) {                                     \
+            const double bv_ = b[nt * 32];                                                      \
+            dmma884(acc[0][nt][0], acc[0][nt][1], a0_, bv_);                                    \
+            dmma884(acc[1][nt][0], acc[1][nt][1], a1_, bv_);                                    \
+        }                                                                                       \
+        b += NT * 32;                                                                           \
+    }
+#define LRDMC_DISP2                                                                             \
+        const double4 s = *sh4; const double z = s.w;                                           \
+        const double x0 = p0[0] - s.x, y0 = p0[1] - s.y, z0 = p0[2] - s.z;                      \
+        const double x1 = p1[0] - s.x, y1 = p1[1] - s.y, z1 = p1[2] - s.z;                      \
+        const double q0 = x0 * x0 + y0 * y0 + z0 * z0, q1 = x1 * x1 + y1 * y1 + z1 * z1;
+    for (int it = 0; it < S.n_it[0]; ++it, sh4 += 4) {            // Slater s
+        LRDMC_DISP2
+        const double e0 = exp_nonpos(-z * (q0 * fast_rsqrt(q0))), e1 = exp_nonpos(-z * (q1 * fast_rsqrt(q1)));
+        LRDMC_FEED2(e0, e1);
+    }
+    for (int it = 0; it < S.n_it[1]; ++it, sh4 += 4) {            // s
+        LRDMC_DISP2
+        const double e0 = exp_nonpos(-z * q0), e1 = exp_nonpos(-z * q1);
+        LRDMC_FEED2(e0, e1);
+    }
+    for (int it = 0; it < S.n_it[2]; ++it, sh4 += 4) {            // p: x y z
+        LRDMC_DISP2
+        const double e0 = exp_nonpos(-z * q0), e1 = exp_nonpos(-z * q1);
+        LRDMC_FEED2(x0 * e0, x1 * e1); LRDMC_FEED2(y0 * e0, y1 * e1); LRDMC_FEED2(z0 * e0, z1 * e1);
+    }
+    for (int it = 0; it < S.n_it[3]; ++it, sh4 += 4) {            // d: xx xy xz yy yz zz
+        LRDMC_DISP2
+        const double e0 = exp_nonpos(-z * q0), e1 = exp_nonpos(-z * q1);
+        const double xe0 = x0 * e0, ye0 = y0 * e0, ze0 = z0 * e0, xe1 = x1 * e1, ye1 = y1 * e1, ze1 = z1 * e1;
+        LRDMC_FEED2(x0 * xe0, x1 * xe1); LRDMC_FEED2(x0 * ye0, x1 * ye1); LRDMC_FEED2(x0 * ze0, x1 * ze1);
+        LRDMC_FEED2(y0 * ye0, y1 * ye1); LRDMC_FEED2(y0 * ze0, y1 * ze1); LRDMC_FEED2(z0 * ze0, z1 * ze1);
+    }
+#undef LRDMC_DISP2
+#undef LRDMC_FEED2
+}
+
 // Refresh the cached MO rows (value, gradient, Laplacian) of electron i at position (px,py,pz): moc[i][comp][m].
 template <int NT>
 __device__ __forceinline__ void refresh_mo_cache(const DevSys &S, const double *shells, const double *bf, double *moc_i,
