@@ -11,7 +11,7 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "liblrdmc.so")
+LIB_PATH = os.environ.get("LRDMC_LIB", os.path.join(_HERE, "liblrdmc.so"))    # override: kernel experiments only
 BALANCED, CONVENTIONAL = 0, 1
 OK, EINVAL, ESINGULAR, ESTATE, ECUDA, ENOMEM = 0, -1, -2, -3, -4, -5
 

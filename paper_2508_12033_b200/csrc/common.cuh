@@ -7,6 +7,15 @@
 // __builtin_assume(__isShared(p)) made nvcc 12.9 delete the hop (apply_move) from k_propagate: measured, reverted.
 // Address spaces are inferred instead: with TS every per-warp pointer is "shared base + offset" with no global alternative.
 #define LRDMC_ASSUME_SHARED(p) ((void)0)
+#ifndef LRDMC_NB
+#define LRDMC_NB 2             // mma batches (of 8 candidate points) per warp pass
+#endif
+#ifndef LRDMC_WPB
+#define LRDMC_WPB 8            // warps (= walkers in flight) per CTA
+#endif
+#ifndef LRDMC_MINB
+#define LRDMC_MINB 2           // CTAs per SM the register allocation must allow
+#endif
 #define LRDMC_NUC_STRIDE 12  // doubles per nucleus row: Rx Ry Rz Z c1 b1 alpha beta gamma delta is_pp pad
 #define LRDMC_EL_ARRAYS 4     // per-electron scratch arrays in shared memory: Jold, lap, s_k, old column
 

@@ -55,7 +55,7 @@ __device__ __forceinline__ void refresh_onebody(int n_nuc, int has_j1, double a_
     if (lane == 0) { ob_i[0] = J; ob_i[1] = gx; ob_i[2] = gy; ob_i[3] = gz; ob_i[4] = lJ; ob_i[5] = vei; ob_i[6] = vb; }
 }
 
-template <int NT, bool TS>
+template <int NT, bool TS, int NB>
 __device__ __forceinline__ EvalOut evaluate_walker(const DevSys &S, const WarpState &ws, const double *shells, const double *const bf[2],
                                                    const double *nuc, int lane)
 {
@@ -101,29 +101,31 @@ __device__ __forceinline__ EvalOut evaluate_walker(const DevSys &S, const WarpSt
     const double Vee = warp_sum(vee_part);
     __syncwarp();
 
-    // ---- phase B (rows a1-a5): candidates, 16 points (two mma batches of 8) per warp pass through the tensor-core MO pass
+    // ---- phase B (rows a1-a5): candidates, 8*NB points (NB mma batches of 8) per warp pass through the tensor-core MO pass
     for (int mesh = 0; mesh < S.n_mesh; ++mesh) {
         const double am = S.amesh[mesh];
         for (int sp = 0; sp < 2; ++sp) {
             const int ns = sp ? S.n_dn : S.n_up, off = sp ? S.n_up : 0, npts = 6 * ns;
             if (ns == 0) continue;
             const double *dinv = ws.dinv[sp];
-            for (int q0 = 0; q0 < npts; q0 += 16) {
-                bool valid[2]; int ci[2], cd[2], cil[2]; double pt[2][3];
+            for (int q0 = 0; q0 < npts; q0 += 8 * NB) {
+                bool valid[NB]; int ci[NB], cd[NB], cil[NB]; double pt[NB][3];
 #pragma unroll
-                for (int h = 0; h < 2; ++h) {
+                for (int h = 0; h < NB; ++h) {
                     valid[h] = q0 + 8 * h + g < npts;
                     const int q = valid[h] ? q0 + 8 * h + g : 0, il = q / 6, d = q - 6 * il, i = off + il, k = d >> 1;
                     const double step = (d & 1) ? -am : am;
                     ci[h] = i; cd[h] = d; cil[h] = il;
                     pt[h][0] = ws.r[3 * i] + step * ws.U[k]; pt[h][1] = ws.r[3 * i + 1] + step * ws.U[3 + k]; pt[h][2] = ws.r[3 * i + 2] + step * ws.U[6 + k];
                 }
-                double acc[2][NT][2];
-                mo_values2<NT>(S, shells, bf[sp], pt[0], pt[1], lane, acc);
+                double acc[NB][NT][2];
+                mo_values<NT, NB>(S, shells, bf[sp], pt, lane, acc);
                 // determinant ratio (row a4): sum_m phi_m(r') Dinv[m][il]; this lane holds m = 8 nt + 2t, +1 (rows beyond n_s are zero-padded)
-                double part[2] = { 0.0, 0.0 }, Jn[2] = { 0.0, 0.0 };
+                double part[NB], Jn[NB];
 #pragma unroll
-                for (int h = 0; h < 2; ++h)
+                for (int h = 0; h < NB; ++h) { part[h] = 0.0; Jn[h] = 0.0; }
+#pragma unroll
+                for (int h = 0; h < NB; ++h)
 #pragma unroll
                     for (int nt = 0; nt < NT; ++nt) {
                         const int m = 8 * nt + 2 * t;
@@ -134,7 +136,7 @@ __device__ __forceinline__ EvalOut evaluate_walker(const DevSys &S, const WarpSt
                     const double *nu = nuc + I * LRDMC_NUC_STRIDE;
                     const double nx = nu[0], ny = nu[1], nz = nu[2], c1 = nu[4], b1 = nu[5];
 #pragma unroll
-                    for (int h = 0; h < 2; ++h) {
+                    for (int h = 0; h < NB; ++h) {
                         const double dx = pt[h][0] - nx, dy = pt[h][1] - ny, dz = pt[h][2] - nz, r2 = dx * dx + dy * dy + dz * dz;
                         const double r = r2 * fast_rsqrt(r2);
                         Jn[h] -= c1 * r * fast_rcp(1.0 + b1 * r);
@@ -144,7 +146,7 @@ __device__ __forceinline__ EvalOut evaluate_walker(const DevSys &S, const WarpSt
                     const double jx = ws.r[3 * j], jy = ws.r[3 * j + 1], jz = ws.r[3 * j + 2];
                     const double cpar = (spin_of(S, j) == sp) ? S.a_par : S.a_anti;
 #pragma unroll
-                    for (int h = 0; h < 2; ++h) {
+                    for (int h = 0; h < NB; ++h) {
                         const double dx = pt[h][0] - jx, dy = pt[h][1] - jy, dz = pt[h][2] - jz, r2 = dx * dx + dy * dy + dz * dz;
                         const double r = r2 * fast_rsqrt(r2);
                         const double u = cpar * r * fast_rcp(1.0 + S.b2 * r);
@@ -152,7 +154,7 @@ __device__ __forceinline__ EvalOut evaluate_walker(const DevSys &S, const WarpSt
                     }
                 }
 #pragma unroll
-                for (int h = 0; h < 2; ++h) {
+                for (int h = 0; h < NB; ++h) {
                     const double dr = quad_sum(part[h]), dJ = quad_sum(Jn[h]) - Jold[ci[h]];
                     if (valid[h] && t == 0) ws.R[mesh * 6 * N + 6 * ci[h] + cd[h]] = dr * exp(dJ);
                 }

@@ -160,7 +160,7 @@ extern "C" int lrdmc_init(lrdmc_ctx **out, const lrdmc_system *sys, const lrdmc_
     S.o_ob = (int)w; w += 8 * (size_t)S.N;      // one-body cache: J1, grad J1, lap J1, v_ei, v^a_ei per electron
     S.per_warp_doubles = (int)w;
     const size_t per_sm = prop.sharedMemPerMultiprocessor, per_blk_max = prop.sharedMemPerBlockOptin, reserve = 1024;
-    c->wpb = 8;
+    c->wpb = LRDMC_WPB;
     for (;;) {
         size_t need = ((size_t)S.tables_doubles + (size_t)c->wpb * S.per_warp_doubles) * 8;
         if ((need + reserve) * 2 <= per_sm || c->wpb == 1) { c->smem_bytes = (int)need; break; }

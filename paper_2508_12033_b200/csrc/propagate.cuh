@@ -82,7 +82,7 @@ __device__ __forceinline__ void store_walker(const DevSys &S, const DevWalk &W, 
 
 // ---- the projection kernel (Alg.2 lines 4-8 L401-L410 / Alg.1 lines 4-16 L350-L374) ----------------------------
 template <int NT, bool TS>
-__global__ void __launch_bounds__(256) k_propagate(DevSys S, DevWalk W, int mode, int n_moves, double tau, double E0, uint32_t cycle)
+__global__ void __launch_bounds__(LRDMC_WPB * 32, LRDMC_MINB) k_propagate(DevSys S, DevWalk W, int mode, int n_moves, double tau, double E0, uint32_t cycle)
 {
     extern __shared__ __align__(16) double smem[];
     stage_tables(S, smem);
@@ -102,7 +102,7 @@ __global__ void __launch_bounds__(256) k_propagate(DevSys S, DevWalk W, int mode
         for (uint32_t s = 0;; ++s) {
             const StepDraws d = step_draws(S, (uint32_t)k, cycle, s, mode == LRDMC_CONVENTIONAL);
             publish_frame(ws, d, lane);
-            const EvalOut e = evaluate_walker<NT, TS>(S, ws, shells, bf, nuc, lane);
+            const EvalOut e = evaluate_walker<NT, TS, LRDMC_NB>(S, ws, shells, bf, nuc, lane);
             n_node += e.node;
             bool last = false;
             if (mode == LRDMC_BALANCED) {
@@ -136,7 +136,7 @@ __global__ void __launch_bounds__(256) k_propagate(DevSys S, DevWalk W, int mode
 
 // ---- parity hook: one evaluation + selection, no state change ---------------------------------------------------
 template <int NT, bool TS>
-__global__ void __launch_bounds__(256) k_step_debug(DevSys S, DevWalk W, double E0, uint32_t cycle, uint32_t step, double *R_out,
+__global__ void __launch_bounds__(LRDMC_WPB * 32, LRDMC_MINB) k_step_debug(DevSys S, DevWalk W, double E0, uint32_t cycle, uint32_t step, double *R_out,
                                                     double *scal_out, int *jstar_out)
 {
     extern __shared__ __align__(16) double smem[];
@@ -149,7 +149,7 @@ __global__ void __launch_bounds__(256) k_step_debug(DevSys S, DevWalk W, double 
         load_walker<TS>(S, W, ws, nuc, k, lane, true);
         const StepDraws d = step_draws(S, (uint32_t)k, cycle, step, true);
         publish_frame(ws, d, lane);
-        const EvalOut e = evaluate_walker<NT, TS>(S, ws, shells, bf, nuc, lane);
+        const EvalOut e = evaluate_walker<NT, TS, LRDMC_NB>(S, ws, shells, bf, nuc, lane);
         const int j = select_move(S, ws, d.u_sel, lane);
         for (int p = lane; p < S.P; p += 32) R_out[(size_t)k * S.P + p] = ws.R[p];
         if (lane == 0) {

@@ -102,57 +102,75 @@ __device__ __forceinline__ void mo_pass(const DevSys &S, const double *__restric
 #undef LRDMC_FEED
 }
 
-// Value-only pass over TWO batches of 8 points at once (16 candidate points per warp pass): every shell row and every
-// B fragment is loaded once and used twice, and the two exponential chains of a lane are independent (ILP 2), which is
-// what the FP64 pipe needs with 4 warps per scheduler.  acc[b] = accumulators of batch b.
-template <int NT>
-__device__ __forceinline__ void mo_values2(const DevSys &S, const double *__restrict__ shells, const double *__restrict__ bf,
-                                           const double (&p0)[3], const double (&p1)[3], int lane, double (&acc)[2][NT][2])
+// Value-only pass over NB batches of 8 points at once (8*NB candidate points per warp pass): every shell row and every
+// B fragment is loaded once and used NB times, and the NB exponential chains of a lane are independent (ILP NB), which is
+// what the FP64 pipe needs with 4 warps per scheduler.  acc[h] = accumulators of batch h.
+template <int NT, int NB>
+__device__ __forceinline__ void mo_values(const DevSys &S, const double *__restrict__ shells, const double *__restrict__ bf,
+                                          const double (&pt)[NB][3], int lane, double (&acc)[NB][NT][2])
 {
     const int t = lane & 3;
     const double4 *sh4 = reinterpret_cast<const double4 *>(shells) + t;
     const double *b = bf + lane;
 #pragma unroll
-    for (int nt = 0; nt < NT; ++nt) { acc[0][nt][0] = 0.0; acc[0][nt][1] = 0.0; acc[1][nt][0] = 0.0; acc[1][nt][1] = 0.0; }
-#define LRDMC_FEED2(a0val, a1val)                                                               \
+    for (int h = 0; h < NB; ++h)
+#pragma unroll
+        for (int nt = 0; nt < NT; ++nt) { acc[h][nt][0] = 0.0; acc[h][nt][1] = 0.0; }
+    double dx[NB], dy[NB], dz[NB], e[NB], a[NB];
+#ifdef LRDMC_SPLIT_ACC
+    double acc2[NB][NT][2];       // second accumulator set: consecutive k-steps of one batch do not wait for each other
+#pragma unroll
+    for (int h = 0; h < NB; ++h)
+#pragma unroll
+        for (int nt = 0; nt < NT; ++nt) { acc2[h][nt][0] = 0.0; acc2[h][nt][1] = 0.0; }
+#define LRDMC_ACC2 acc2
+#else
+#define LRDMC_ACC2 acc
+#endif
+#define LRDMC_FEED_(ACC)                                                                        \
     {                                                                                           \
-        const double a0_ = (a0val), a1_ = (a1val);                                              \
         _Pragma("unroll") for (int nt = 0; nt < NT; ++nt) {                                     \
             const double bv_ = b[nt * 32];                                                      \
-            dmma884(acc[0][nt][0], acc[0][nt][1], a0_, bv_);                                    \
-            dmma884(acc[1][nt][0], acc[1][nt][1], a1_, bv_);                                    \
+            _Pragma("unroll") for (int h = 0; h < NB; ++h) dmma884(ACC[h][nt][0], ACC[h][nt][1], a[h], bv_); \
         }                                                                                       \
         b += NT * 32;                                                                           \
     }
-#define LRDMC_DISP2                                                                             \
+#define LRDMC_FEEDN LRDMC_FEED_(acc)
+#define LRDMC_FEEDM LRDMC_FEED_(LRDMC_ACC2)
+#define LRDMC_DISPN(SLATER)                                                                     \
         const double4 s = *sh4; const double z = s.w;                                           \
-        const double x0 = p0[0] - s.x, y0 = p0[1] - s.y, z0 = p0[2] - s.z;                      \
-        const double x1 = p1[0] - s.x, y1 = p1[1] - s.y, z1 = p1[2] - s.z;                      \
-        const double q0 = x0 * x0 + y0 * y0 + z0 * z0, q1 = x1 * x1 + y1 * y1 + z1 * z1;
-    for (int it = 0; it < S.n_it[0]; ++it, sh4 += 4) {            // Slater s
-        LRDMC_DISP2
-        const double e0 = exp_nonpos(-z * (q0 * fast_rsqrt(q0))), e1 = exp_nonpos(-z * (q1 * fast_rsqrt(q1)));
-        LRDMC_FEED2(e0, e1);
+        _Pragma("unroll") for (int h = 0; h < NB; ++h) {                                        \
+            dx[h] = pt[h][0] - s.x; dy[h] = pt[h][1] - s.y; dz[h] = pt[h][2] - s.z;              \
+            const double q = dx[h] * dx[h] + dy[h] * dy[h] + dz[h] * dz[h];                      \
+            e[h] = exp_nonpos(-z * (SLATER ? q * fast_rsqrt(q) : q));                           \
+        }
+#define LRDMC_SETA(expr) _Pragma("unroll") for (int h = 0; h < NB; ++h) a[h] = (expr);
+    for (int it = 0; it < S.n_it[0]; ++it, sh4 += 4) { LRDMC_DISPN(true) LRDMC_SETA(e[h]) LRDMC_FEEDN }      // Slater s
+    for (int it = 0; it < S.n_it[1]; ++it, sh4 += 4) { LRDMC_DISPN(false) LRDMC_SETA(e[h]) LRDMC_FEEDN }     // s
+    for (int it = 0; it < S.n_it[2]; ++it, sh4 += 4) {                                                        // p: x y z
+        LRDMC_DISPN(false)
+        LRDMC_SETA(dx[h] * e[h]) LRDMC_FEEDN LRDMC_SETA(dy[h] * e[h]) LRDMC_FEEDM LRDMC_SETA(dz[h] * e[h]) LRDMC_FEEDN
     }
-    for (int it = 0; it < S.n_it[1]; ++it, sh4 += 4) {            // s
-        LRDMC_DISP2
-        const double e0 = exp_nonpos(-z * q0), e1 = exp_nonpos(-z * q1);
-        LRDMC_FEED2(e0, e1);
+    for (int it = 0; it < S.n_it[3]; ++it, sh4 += 4) {                                                        // d: xx xy xz yy yz zz
+        LRDMC_DISPN(false)
+        double xe[NB], ye[NB], ze[NB];
+#pragma unroll
+        for (int h = 0; h < NB; ++h) { xe[h] = dx[h] * e[h]; ye[h] = dy[h] * e[h]; ze[h] = dz[h] * e[h]; }
+        LRDMC_SETA(dx[h] * xe[h]) LRDMC_FEEDN LRDMC_SETA(dx[h] * ye[h]) LRDMC_FEEDM LRDMC_SETA(dx[h] * ze[h]) LRDMC_FEEDN
+        LRDMC_SETA(dy[h] * ye[h]) LRDMC_FEEDM LRDMC_SETA(dy[h] * ze[h]) LRDMC_FEEDN LRDMC_SETA(dz[h] * ze[h]) LRDMC_FEEDM
     }
-    for (int it = 0; it < S.n_it[2]; ++it, sh4 += 4) {            // p: x y z
-        LRDMC_DISP2
-        const double e0 = exp_nonpos(-z * q0), e1 = exp_nonpos(-z * q1);
-        LRDMC_FEED2(x0 * e0, x1 * e1); LRDMC_FEED2(y0 * e0, y1 * e1); LRDMC_FEED2(z0 * e0, z1 * e1);
-    }
-    for (int it = 0; it < S.n_it[3]; ++it, sh4 += 4) {            // d: xx xy xz yy yz zz
-        LRDMC_DISP2
-        const double e0 = exp_nonpos(-z * q0), e1 = exp_nonpos(-z * q1);
-        const double xe0 = x0 * e0, ye0 = y0 * e0, ze0 = z0 * e0, xe1 = x1 * e1, ye1 = y1 * e1, ze1 = z1 * e1;
-        LRDMC_FEED2(x0 * xe0, x1 * xe1); LRDMC_FEED2(x0 * ye0, x1 * ye1); LRDMC_FEED2(x0 * ze0, x1 * ze1);
-        LRDMC_FEED2(y0 * ye0, y1 * ye1); LRDMC_FEED2(y0 * ze0, y1 * ze1); LRDMC_FEED2(z0 * ze0, z1 * ze1);
-    }
-#undef LRDMC_DISP2
-#undef LRDMC_FEED2
+#ifdef LRDMC_SPLIT_ACC
+#pragma unroll
+    for (int h = 0; h < NB; ++h)
+#pragma unroll
+        for (int nt = 0; nt < NT; ++nt) { acc[h][nt][0] += acc2[h][nt][0]; acc[h][nt][1] += acc2[h][nt][1]; }
+#endif
+#undef LRDMC_SETA
+#undef LRDMC_DISPN
+#undef LRDMC_FEEDN
+#undef LRDMC_FEEDM
+#undef LRDMC_FEED_
+#undef LRDMC_ACC2
 }
 
 // Refresh the cached MO rows (value, gradient, Laplacian) of electron i at position (px,py,pz): moc[i][comp][m].
