@@ -36,12 +36,16 @@ struct DevSys {
     const double *shells;      // [n_slots][4] = cx cy cz zeta
     const double *bfrag[2];    // [n_ksteps][NT][32] FP64 mma B fragments, AO norms folded in
     const double *nuc;         // [n_nuc][LRDMC_NUC_STRIDE]
+    const double *etab;        // [256] 2^(j/256) for exp_tab
     // shared-memory plan (units: doubles)
     int bf_in_smem, moc_in_smem;
-    int off_shells, off_nuc, off_bf[2], tables_doubles;
+    int off_shells, off_nuc, off_bf[2], off_etab, tables_doubles;
     int o_r, o_dinv[2], o_moc, o_R, o_cum, o_el, o_ob, o_U, per_warp_doubles;
     int dinv_rows[2];     // padded row count 8*NT
 };
+
+// Table pointers as a kernel sees them (shared memory, or global memory for the fragments of the largest systems)
+struct Tables { const double *shells, *nuc, *bf[2], *etab; };
 
 // Walker storage (views into the caller's buffer)
 struct DevWalk {

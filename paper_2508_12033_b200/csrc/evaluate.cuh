@@ -13,17 +13,6 @@ struct EvalOut { double bbar, Vsf, W, eL; int node; };
 
 __device__ __forceinline__ int spin_of(const DevSys &S, int i) { return i < S.n_up ? 0 : 1; }
 
-// Address-space hints: all per-warp state and the small tables are shared memory (LDS/STS instead of generic LD/ST);
-// TS = the MO fragment table and the MO cache are in shared memory too (every config except the 64-electron one).
-template <bool TS>
-__device__ __forceinline__ void assume_shared(const WarpState &ws, const double *shells, const double *nuc, const double *const bf[2])
-{
-    LRDMC_ASSUME_SHARED(ws.r); LRDMC_ASSUME_SHARED(ws.dinv[0]); LRDMC_ASSUME_SHARED(ws.dinv[1]);
-    LRDMC_ASSUME_SHARED(ws.R); LRDMC_ASSUME_SHARED(ws.cum); LRDMC_ASSUME_SHARED(ws.el);
-    LRDMC_ASSUME_SHARED(ws.ob); LRDMC_ASSUME_SHARED(shells); LRDMC_ASSUME_SHARED(nuc);
-    if (TS) { LRDMC_ASSUME_SHARED(ws.moc); LRDMC_ASSUME_SHARED(bf[0]); LRDMC_ASSUME_SHARED(bf[1]); }
-}
-
 // electron-ion potential of one nucleus and its lower bound (Eq.D10; ECP rule L623)
 __device__ __forceinline__ void nuc_potential(double a_cut, const double *nu, double r, double ir, double &v, double &vb)
 {
@@ -55,9 +44,21 @@ __device__ __forceinline__ void refresh_onebody(int n_nuc, int has_j1, double a_
     if (lane == 0) { ob_i[0] = J; ob_i[1] = gx; ob_i[2] = gy; ob_i[3] = gz; ob_i[4] = lJ; ob_i[5] = vei; ob_i[6] = vb; }
 }
 
+// Pade term c r/(1 + b r) = c/(b + 1/r) of one partner at the six displaced points of an electron:
+// |d0 +- a e_k|^2 = |d0|^2 + a^2 +- 2 a e_k.d0 (d0 = electron - partner), one reciprocal square root and one reciprocal each.
+__device__ __forceinline__ void pade_six(double dx, double dy, double dz, const double (&av)[3][3], double a2, double c, double b, double (&J)[6])
+{
+    const double q0 = fma(dx, dx, fma(dy, dy, fma(dz, dz, a2)));
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        const double sk = fma(av[k][0], dx, fma(av[k][1], dy, av[k][2] * dz));
+        J[2 * k] = fma(c, fast_rcp(b + fast_rsqrt(fma(2.0, sk, q0))), J[2 * k]);
+        J[2 * k + 1] = fma(c, fast_rcp(b + fast_rsqrt(fma(-2.0, sk, q0))), J[2 * k + 1]);
+    }
+}
+
 template <int NT, bool TS, int NB>
-__device__ __forceinline__ EvalOut evaluate_walker(const DevSys &S, const WarpState &ws, const double *shells, const double *const bf[2],
-                                                   const double *nuc, int lane)
+__device__ __forceinline__ EvalOut evaluate_walker(const DevSys &S, const WarpState &ws, const Tables &T, int lane)
 {
     const int N = S.N, n_nuc = S.n_nuc;
     const int t = lane & 3, g = lane >> 2;
@@ -101,7 +102,46 @@ __device__ __forceinline__ EvalOut evaluate_walker(const DevSys &S, const WarpSt
     const double Vee = warp_sum(vee_part);
     __syncwarp();
 
-    // ---- phase B (rows a1-a5): candidates, 8*NB points (NB mma batches of 8) per warp pass through the tensor-core MO pass
+    // ---- phase B (rows a1-a5): the 6 n_s candidates of each spin, 8 electrons (48 points) per warp pass in column form
+#ifndef LRDMC_CONTRACTION_MO
+    for (int mesh = 0; mesh < S.n_mesh; ++mesh) {
+        const double am = S.amesh[mesh], a2 = am * am;
+        double av[3][3];                                             // av[k] = a e_k, e_k = k-th column of U (Eq.D3-D4)
+#pragma unroll
+        for (int k = 0; k < 3; ++k) { av[k][0] = am * ws.U[k]; av[k][1] = am * ws.U[3 + k]; av[k][2] = am * ws.U[6 + k]; }
+        for (int sp = 0; sp < 2; ++sp) {
+            const int ns = sp ? S.n_dn : S.n_up, off = sp ? S.n_up : 0;
+            for (int il0 = 0; il0 < ns; il0 += 8) {
+                const bool valid = il0 + g < ns;
+                const int il = valid ? il0 + g : 0, i = off + il;
+                const double x0 = ws.r[3 * i], y0 = ws.r[3 * i + 1], z0 = ws.r[3 * i + 2];
+                double acc[6], Jn[6];
+                ao_columns<NT>(S, T.shells, T.bf[sp], T.etab, ws.dinv[sp], ns, il, x0, y0, z0, av, a2, lane, acc);
+                // Jastrow ratio (row a5): the 4 lanes of the quad split the partners; u = c r/(1 + b r) = c/(b + 1/r)
+#pragma unroll
+                for (int d = 0; d < 6; ++d) Jn[d] = 0.0;
+                if (S.has_j1) for (int I = t; I < n_nuc; I += 4) {
+                    const double *nu = T.nuc + I * LRDMC_NUC_STRIDE;
+                    pade_six(x0 - nu[0], y0 - nu[1], z0 - nu[2], av, a2, -nu[4], nu[5], Jn);
+                }
+                for (int j = t; j < N; j += 4) {
+                    const double c = (j == i) ? 0.0 : ((spin_of(S, j) == sp) ? S.a_par : S.a_anti);
+                    pade_six(x0 - ws.r[3 * j], y0 - ws.r[3 * j + 1], z0 - ws.r[3 * j + 2], av, a2, c, S.b2, Jn);
+                }
+                const double Jo = Jold[i];
+                double Rv[6];
+#pragma unroll
+                for (int d = 0; d < 6; ++d) Rv[d] = quad_sum(acc[d]) * exp_tab(quad_sum(Jn[d]) - Jo, T.etab);
+                if (valid && t == 0) {
+                    double *Ro = ws.R + mesh * 6 * N + 6 * i;
+#pragma unroll
+                    for (int d = 0; d < 6; ++d) Ro[d] = Rv[d];
+                }
+            }
+        }
+    }
+#else
+    // MO form: candidates, 8*NB points (NB mma batches of 8) per warp pass through the tensor-core MO pass
     for (int mesh = 0; mesh < S.n_mesh; ++mesh) {
         const double am = S.amesh[mesh];
         for (int sp = 0; sp < 2; ++sp) {
@@ -119,7 +159,7 @@ __device__ __forceinline__ EvalOut evaluate_walker(const DevSys &S, const WarpSt
                     pt[h][0] = ws.r[3 * i] + step * ws.U[k]; pt[h][1] = ws.r[3 * i + 1] + step * ws.U[3 + k]; pt[h][2] = ws.r[3 * i + 2] + step * ws.U[6 + k];
                 }
                 double acc[NB][NT][2];
-                mo_values<NT, NB>(S, shells, bf[sp], pt, lane, acc);
+                mo_values<NT, NB>(S, T.shells, T.bf[sp], T.etab, pt, lane, acc);
                 // determinant ratio (row a4): sum_m phi_m(r') Dinv[m][il]; this lane holds m = 8 nt + 2t, +1 (rows beyond n_s are zero-padded)
                 double part[NB], Jn[NB];
 #pragma unroll
@@ -133,7 +173,7 @@ __device__ __forceinline__ EvalOut evaluate_walker(const DevSys &S, const WarpSt
                     }
                 // Jastrow ratio (row a5): partners split over the 4 lanes of the quad; both points share each partner load
                 if (S.has_j1) for (int I = t; I < n_nuc; I += 4) {
-                    const double *nu = nuc + I * LRDMC_NUC_STRIDE;
+                    const double *nu = T.nuc + I * LRDMC_NUC_STRIDE;
                     const double nx = nu[0], ny = nu[1], nz = nu[2], c1 = nu[4], b1 = nu[5];
 #pragma unroll
                     for (int h = 0; h < NB; ++h) {
@@ -161,6 +201,7 @@ __device__ __forceinline__ EvalOut evaluate_walker(const DevSys &S, const WarpSt
             }
         }
     }
+#endif
     __syncwarp();
 
     // ---- phase C (row a7): fixed-node split (Eq.D1) and the cumulative sums C_j of the allowed amplitudes in candidate
@@ -229,8 +270,7 @@ __device__ __forceinline__ int select_move(const DevSys &S, const WarpState &ws,
 
 // Apply move j (row a10): r_i <- r'_j, refresh the cached MO rows and the one-body cache of electron i, Sherman-Morrison on Dinv_sigma.
 template <int NT, bool TS>
-__device__ __forceinline__ void apply_move(const DevSys &S, const WarpState &ws, const double *shells, const double *const bf[2], const double *nuc,
-                                           int j, int lane)
+__device__ __forceinline__ void apply_move(const DevSys &S, const WarpState &ws, const Tables &T, int j, int lane)
 {
     const int N = S.N, mesh = j / (6 * N), jj = j - mesh * 6 * N, i = jj / 6, d = jj - 6 * i, k = d >> 1;
     const int sp = spin_of(S, i), il = sp ? i - S.n_up : i, ns = sp ? S.n_dn : S.n_up;
@@ -238,8 +278,8 @@ __device__ __forceinline__ void apply_move(const DevSys &S, const WarpState &ws,
     const double px = ws.r[3 * i] + step * ws.U[k], py = ws.r[3 * i + 1] + step * ws.U[3 + k], pz = ws.r[3 * i + 2] + step * ws.U[6 + k];
     double *mc = ws.moc + (size_t)i * 5 * S.OS;
     __syncwarp();
-    refresh_mo_cache<NT>(S, shells, bf[sp], mc, px, py, pz, lane);
-    refresh_onebody(S.n_nuc, S.has_j1, S.a, nuc, ws.ob + 8 * i, px, py, pz, lane);
+    refresh_mo_cache<NT>(S, T.shells, T.bf[sp], T.etab, mc, px, py, pz, lane);
+    refresh_onebody(S.n_nuc, S.has_j1, S.a, T.nuc, ws.ob + 8 * i, px, py, pz, lane);
     if (lane == 0) { ws.r[3 * i] = px; ws.r[3 * i + 1] = py; ws.r[3 * i + 2] = pz; }
     __syncwarp();
     // s_k = sum_m phi_m Dinv[m][k];  rho = s_il;  Dinv'[m][il] = Dinv[m][il]/rho;  Dinv'[m][k] = Dinv[m][k] - Dinv[m][il] s_k / rho

@@ -38,6 +38,26 @@ __device__ __forceinline__ double exp_nonpos(double x)
     return (x < -708.0) ? 0.0 : res;
 }
 
+// exp(x) for -708 < x < 708 through a 256-entry table of 2^(j/256) (shared memory, built at init):
+//   x = (256 e + j) ln2/256 + r, |r| <= ln2/512 = 1.36e-3;  e^r by the degree-4 Taylor polynomial (truncation r^5/120 < 4e-17);
+//   exp(x) = 2^e * tab[j] * e^r.  8 FP64 instructions + one LDS instead of 16: the AO exponentials are 1/3 of the FP64 work.
+// The reduction uses ln2/256 as one double: |error of r| <= |k| 2^-53 ln2/256, i.e. < 5e-15 relative for results above 1e-20.
+__device__ __forceinline__ double exp_tab(double x, const double *__restrict__ etab)
+{
+    const double magic = 6755399441055744.0;                       // 1.5 * 2^52
+    const double t = fma(x, 369.32993046757463228, magic);         // 256 / ln2
+    const int k = __double2loint(t);
+    const double kd = t - magic;
+    const double r = fma(kd, -2.7076061740622863649e-03, x);       // ln2 / 256
+    double p = fma(r, 4.16666666666666666667e-02, 1.66666666666666666667e-01);
+    p = fma(p, r, 0.5);
+    p = fma(p, r, 1.0);
+    p = fma(p, r, 1.0);
+    const double v = etab[k & 255] * p;                            // in (0.99, 2.01): adding to the exponent stays normal for e >= -1021
+    const double res = __hiloint2double(__double2hiint(v) + ((k >> 8) << 20), __double2loint(v));
+    return (k < -1021 * 256) ? 0.0 : res;
+}
+
 // 1/a for ordinary positive a (no denormal / inf handling): hardware seed (about 2^-22) + one cubic step.
 __device__ __forceinline__ double fast_rcp(double a)
 {

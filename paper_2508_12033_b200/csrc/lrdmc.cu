@@ -111,7 +111,8 @@ extern "C" int lrdmc_init(lrdmc_ctx **out, const lrdmc_system *sys, const lrdmc_
         if (sys->pp && sys->pp[4 * I] > 0.0) { nu[6] = sys->pp[4 * I]; nu[7] = sys->pp[4 * I + 1]; nu[8] = sys->pp[4 * I + 2]; nu[9] = sys->pp[4 * I + 3]; nu[10] = 1.0; }
     }
     const size_t bf_n = (size_t)S.n_ksteps * c->NT * 32;
-    std::vector<double> h_bf[2];
+    std::vector<double> h_bf[2], h_et(256);
+    for (int j = 0; j < 256; ++j) h_et[j] = exp2((double)j / 256.0);       // table of exp_tab
     for (int sp = 0; sp < (S.same_C ? 1 : 2); ++sp) {
         const int ns = sp ? sys->n_dn : sys->n_up; const double *C = sp ? mo->C_dn : mo->C_up;
         h_bf[sp].assign(bf_n, 0.0);
@@ -125,12 +126,13 @@ extern "C" int lrdmc_init(lrdmc_ctx **out, const lrdmc_system *sys, const lrdmc_
             }
     }
     // ---- device copies
-    size_t bytes = (h_sh.size() + h_nuc.size() + bf_n * (S.same_C ? 1 : 2)) * sizeof(double);
+    size_t bytes = (h_sh.size() + h_nuc.size() + h_et.size() + bf_n * (S.same_C ? 1 : 2)) * sizeof(double);
     cudaError_t ce = cudaMalloc(&c->d_tables, bytes);
     if (ce != cudaSuccess) { snprintf(g_cuda_msg, sizeof g_cuda_msg, "%s (cudaMalloc tables)", cudaGetErrorString(ce)); free(c); return LRDMC_ECUDA; }
     double *d = (double *)c->d_tables;
     cudaMemcpy(d, h_sh.data(), h_sh.size() * 8, cudaMemcpyHostToDevice); S.shells = d; d += h_sh.size();
     cudaMemcpy(d, h_nuc.data(), h_nuc.size() * 8, cudaMemcpyHostToDevice); S.nuc = d; d += h_nuc.size();
+    cudaMemcpy(d, h_et.data(), h_et.size() * 8, cudaMemcpyHostToDevice); S.etab = d; d += h_et.size();
     cudaMemcpy(d, h_bf[0].data(), bf_n * 8, cudaMemcpyHostToDevice); S.bfrag[0] = d; d += bf_n;
     if (!S.same_C) { cudaMemcpy(d, h_bf[1].data(), bf_n * 8, cudaMemcpyHostToDevice); S.bfrag[1] = d; } else S.bfrag[1] = S.bfrag[0];
     if (cudaMalloc((void **)&c->d_stats, sizeof(DevStats)) != cudaSuccess) { cudaFree(c->d_tables); free(c); return LRDMC_ECUDA; }
@@ -145,6 +147,7 @@ extern "C" int lrdmc_init(lrdmc_ctx **out, const lrdmc_system *sys, const lrdmc_
     size_t o = 0;
     S.off_shells = (int)o; o += align_up(h_sh.size(), 2);
     S.off_nuc = (int)o; o += align_up(h_nuc.size(), 2);
+    S.off_etab = (int)o; o += 256;
     S.off_bf[0] = (int)o; if (S.bf_in_smem) o += bf_n;
     S.off_bf[1] = (int)o; if (S.bf_in_smem && !S.same_C) o += bf_n;
     S.tables_doubles = (int)align_up(o, 2);

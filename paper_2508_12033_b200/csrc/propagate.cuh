@@ -14,18 +14,21 @@ __device__ __forceinline__ void stage_tables(const DevSys &S, double *smem)
         for (int i = threadIdx.x; i < nb; i += blockDim.x) smem[S.off_bf[0] + i] = S.bfrag[0][i];
         if (!S.same_C && S.n_dn > 0) for (int i = threadIdx.x; i < nb; i += blockDim.x) smem[S.off_bf[1] + i] = S.bfrag[1][i];
     }
+    for (int i = threadIdx.x; i < 256; i += blockDim.x) smem[S.off_etab + i] = S.etab[i];
     __syncthreads();
 }
 
 // TS (tables + MO cache in shared memory): every pointer below is "shared base + offset" with no global alternative, so the
 // compiler's address-space inference emits LDS/STS.  !TS (64-electron config): fragments / cache stay in global memory.
 template <bool TS>
-__device__ __forceinline__ void table_pointers(const DevSys &S, const double *smem, const double *&shells, const double *&nuc, const double *bf[2])
+__device__ __forceinline__ Tables table_pointers(const DevSys &S, const double *smem)
 {
-    shells = smem + S.off_shells; nuc = smem + S.off_nuc;
-    if (TS) { bf[0] = smem + S.off_bf[0]; bf[1] = smem + (S.same_C ? S.off_bf[0] : S.off_bf[1]); }
-    else if (S.bf_in_smem) { bf[0] = smem + S.off_bf[0]; bf[1] = S.same_C ? bf[0] : smem + S.off_bf[1]; }
-    else { bf[0] = S.bfrag[0]; bf[1] = S.same_C ? S.bfrag[0] : S.bfrag[1]; }
+    Tables T;
+    T.shells = smem + S.off_shells; T.nuc = smem + S.off_nuc; T.etab = smem + S.off_etab;
+    if (TS) { T.bf[0] = smem + S.off_bf[0]; T.bf[1] = smem + (S.same_C ? S.off_bf[0] : S.off_bf[1]); }
+    else if (S.bf_in_smem) { T.bf[0] = smem + S.off_bf[0]; T.bf[1] = S.same_C ? T.bf[0] : smem + S.off_bf[1]; }
+    else { T.bf[0] = S.bfrag[0]; T.bf[1] = S.same_C ? S.bfrag[0] : S.bfrag[1]; }
+    return T;
 }
 
 __device__ __forceinline__ WarpState warp_views(const DevSys &S, double *smem, int warp)
@@ -87,8 +90,7 @@ __global__ void __launch_bounds__(LRDMC_WPB * 32, LRDMC_MINB) k_propagate(DevSys
     extern __shared__ __align__(16) double smem[];
     stage_tables(S, smem);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, gwarp = blockIdx.x * (blockDim.x >> 5) + warp;
-    const double *shells, *nuc, *bf[2];
-    table_pointers<TS>(S, smem, shells, nuc, bf);
+    const Tables T = table_pointers<TS>(S, smem);
     WarpState ws = warp_views(S, smem, warp);
     const unsigned long long t_start = globaltimer_ns();
     for (;;) {
@@ -96,13 +98,13 @@ __global__ void __launch_bounds__(LRDMC_WPB * 32, LRDMC_MINB) k_propagate(DevSys
         if (lane == 0) k = atomicAdd(W.counter, 1);
         k = __shfl_sync(0xffffffffu, k, 0);
         if (k >= W.n_w) break;
-        load_walker<TS>(S, W, ws, nuc, k, lane, true);
+        load_walker<TS>(S, W, ws, T.nuc, k, lane, true);
         double w = 1.0, tau_left = tau, omega = 0.0, eL_out = 0.0, W_out = 0.0;
         long long moves = 0; int n_node = 0, n_nonpos = 0;
         for (uint32_t s = 0;; ++s) {
             const StepDraws d = step_draws(S, (uint32_t)k, cycle, s, mode == LRDMC_CONVENTIONAL);
             publish_frame(ws, d, lane);
-            const EvalOut e = evaluate_walker<NT, TS, LRDMC_NB>(S, ws, shells, bf, nuc, lane);
+            const EvalOut e = evaluate_walker<NT, TS, LRDMC_NB>(S, ws, T, lane);
             n_node += e.node;
             bool last = false;
             if (mode == LRDMC_BALANCED) {
@@ -121,7 +123,7 @@ __global__ void __launch_bounds__(LRDMC_WPB * 32, LRDMC_MINB) k_propagate(DevSys
             }
             if (last) { eL_out = e.eL; W_out = e.W; break; }
             const int j = select_move(S, ws, d.u_sel, lane);       // Alg.2 line 7 (L408)
-            if (j >= 0) { apply_move<NT, TS>(S, ws, shells, bf, nuc, j, lane); ++moves; }
+            if (j >= 0) { apply_move<NT, TS>(S, ws, T, j, lane); ++moves; }
         }
         int nonfinite = 0;
         if (!isfinite(w) || !isfinite(omega)) { nonfinite = 1; w = 0.0; omega = 0.0; }
@@ -142,14 +144,13 @@ __global__ void __launch_bounds__(LRDMC_WPB * 32, LRDMC_MINB) k_step_debug(DevSy
     extern __shared__ __align__(16) double smem[];
     stage_tables(S, smem);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, wpb = blockDim.x >> 5;
-    const double *shells, *nuc, *bf[2];
-    table_pointers<TS>(S, smem, shells, nuc, bf);
+    const Tables T = table_pointers<TS>(S, smem);
     WarpState ws = warp_views(S, smem, warp);
     for (int k = blockIdx.x * wpb + warp; k < W.n_w; k += gridDim.x * wpb) {
-        load_walker<TS>(S, W, ws, nuc, k, lane, true);
+        load_walker<TS>(S, W, ws, T.nuc, k, lane, true);
         const StepDraws d = step_draws(S, (uint32_t)k, cycle, step, true);
         publish_frame(ws, d, lane);
-        const EvalOut e = evaluate_walker<NT, TS, LRDMC_NB>(S, ws, shells, bf, nuc, lane);
+        const EvalOut e = evaluate_walker<NT, TS, LRDMC_NB>(S, ws, T, lane);
         const int j = select_move(S, ws, d.u_sel, lane);
         for (int p = lane; p < S.P; p += 32) R_out[(size_t)k * S.P + p] = ws.R[p];
         if (lane == 0) {
@@ -170,15 +171,14 @@ __global__ void __launch_bounds__(256) k_rebuild(DevSys S, DevWalk W, int do_inv
     extern __shared__ __align__(16) double smem[];
     stage_tables(S, smem);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, wpb = blockDim.x >> 5;
-    const double *shells, *nuc, *bf[2];
-    table_pointers<TS>(S, smem, shells, nuc, bf);
+    const Tables T = table_pointers<TS>(S, smem);
     WarpState ws = warp_views(S, smem, warp);
     const int N = S.N;
     for (int k = blockIdx.x * wpb + warp; k < W.n_w; k += gridDim.x * wpb) {
-        load_walker<TS>(S, W, ws, nuc, k, lane, !do_invert);
+        load_walker<TS>(S, W, ws, T.nuc, k, lane, !do_invert);
         for (int i = 0; i < N; ++i) {
             const int sp = spin_of(S, i);
-            refresh_mo_cache<NT>(S, shells, bf[sp], ws.moc + (size_t)i * 5 * S.OS, ws.r[3 * i], ws.r[3 * i + 1], ws.r[3 * i + 2], lane);
+            refresh_mo_cache<NT>(S, T.shells, T.bf[sp], T.etab, ws.moc + (size_t)i * 5 * S.OS, ws.r[3 * i], ws.r[3 * i + 1], ws.r[3 * i + 2], lane);
         }
         __syncwarp();
         if (do_invert) {

@@ -42,7 +42,7 @@ __device__ __forceinline__ double gto_component(int g, const AxisPoly &X, const 
 // DERIV = false: A fragment = AO value (candidate evaluation, row a2/a3).
 // DERIV = true : the 8 mma rows are 8 COMPONENTS (value, d/dx, d/dy, d/dz, Laplacian, 0,0,0) of ONE point, selector g = lane/4.
 template <int NT, bool DERIV>
-__device__ __forceinline__ void mo_pass(const DevSys &S, const double *__restrict__ shells, const double *__restrict__ bf,
+__device__ __forceinline__ void mo_pass(const DevSys &S, const double *__restrict__ shells, const double *__restrict__ bf, const double *__restrict__ etab,
                                         double px, double py, double pz, int lane, double (&acc)[NT][2])
 {
     const int t = lane & 3, g = lane >> 2;
@@ -59,7 +59,7 @@ __device__ __forceinline__ void mo_pass(const DevSys &S, const double *__restric
     // ---- group 0: Slater-type s, chi = exp(-z r); grad = -z chi rhat; lap = chi (z^2 - 2 z / r)
     for (int it = 0; it < S.n_it[0]; ++it, sh4 += 4) {
         double4 s = *sh4; double dx = px - s.x, dy = py - s.y, dz = pz - s.z, z = s.w;
-        double r = sqrt(dx * dx + dy * dy + dz * dz), e = exp_nonpos(-z * r);
+        double r = sqrt(dx * dx + dy * dy + dz * dz), e = exp_tab(-z * r, etab);
         if (!DERIV) { LRDMC_FEED(e); }
         else {
             double ir = 1.0 / r, d = (g == 1) ? dx : ((g == 2) ? dy : dz);
@@ -70,14 +70,14 @@ __device__ __forceinline__ void mo_pass(const DevSys &S, const double *__restric
     // ---- group 1: s Gaussians
     for (int it = 0; it < S.n_it[1]; ++it, sh4 += 4) {
         double4 s = *sh4; double dx = px - s.x, dy = py - s.y, dz = pz - s.z, z = s.w;
-        double e = exp_nonpos(-z * (dx * dx + dy * dy + dz * dz));
+        double e = exp_tab(-z * (dx * dx + dy * dy + dz * dz), etab);
         if (!DERIV) { LRDMC_FEED(e); }
         else { AxisPoly X = axis_poly(dx, z), Y = axis_poly(dy, z), Z = axis_poly(dz, z); LRDMC_FEED((gto_component<0, 0, 0>(g, X, Y, Z, e))); }
     }
     // ---- group 2: p Gaussians (x, y, z)
     for (int it = 0; it < S.n_it[2]; ++it, sh4 += 4) {
         double4 s = *sh4; double dx = px - s.x, dy = py - s.y, dz = pz - s.z, z = s.w;
-        double e = exp_nonpos(-z * (dx * dx + dy * dy + dz * dz));
+        double e = exp_tab(-z * (dx * dx + dy * dy + dz * dz), etab);
         if (!DERIV) { LRDMC_FEED(dx * e); LRDMC_FEED(dy * e); LRDMC_FEED(dz * e); }
         else {
             AxisPoly X = axis_poly(dx, z), Y = axis_poly(dy, z), Z = axis_poly(dz, z);
@@ -88,7 +88,7 @@ __device__ __forceinline__ void mo_pass(const DevSys &S, const double *__restric
     // ---- group 3: d Gaussians (xx, xy, xz, yy, yz, zz)
     for (int it = 0; it < S.n_it[3]; ++it, sh4 += 4) {
         double4 s = *sh4; double dx = px - s.x, dy = py - s.y, dz = pz - s.z, z = s.w;
-        double e = exp_nonpos(-z * (dx * dx + dy * dy + dz * dz));
+        double e = exp_tab(-z * (dx * dx + dy * dy + dz * dz), etab);
         if (!DERIV) {
             double xe = dx * e, ye = dy * e, ze = dz * e;
             LRDMC_FEED(dx * xe); LRDMC_FEED(dx * ye); LRDMC_FEED(dx * ze); LRDMC_FEED(dy * ye); LRDMC_FEED(dy * ze); LRDMC_FEED(dz * ze);
@@ -106,7 +106,7 @@ __device__ __forceinline__ void mo_pass(const DevSys &S, const double *__restric
 // B fragment is loaded once and used NB times, and the NB exponential chains of a lane are independent (ILP NB), which is
 // what the FP64 pipe needs with 4 warps per scheduler.  acc[h] = accumulators of batch h.
 template <int NT, int NB>
-__device__ __forceinline__ void mo_values(const DevSys &S, const double *__restrict__ shells, const double *__restrict__ bf,
+__device__ __forceinline__ void mo_values(const DevSys &S, const double *__restrict__ shells, const double *__restrict__ bf, const double *__restrict__ etab,
                                           const double (&pt)[NB][3], int lane, double (&acc)[NB][NT][2])
 {
     const int t = lane & 3;
@@ -142,7 +142,7 @@ __device__ __forceinline__ void mo_values(const DevSys &S, const double *__restr
         _Pragma("unroll") for (int h = 0; h < NB; ++h) {                                        \
             dx[h] = pt[h][0] - s.x; dy[h] = pt[h][1] - s.y; dz[h] = pt[h][2] - s.z;              \
             const double q = dx[h] * dx[h] + dy[h] * dy[h] + dz[h] * dz[h];                      \
-            e[h] = exp_nonpos(-z * (SLATER ? q * fast_rsqrt(q) : q));                           \
+            e[h] = exp_tab(-z * (SLATER ? q * fast_rsqrt(q) : q), etab);                         \
         }
 #define LRDMC_SETA(expr) _Pragma("unroll") for (int h = 0; h < NB; ++h) a[h] = (expr);
     for (int it = 0; it < S.n_it[0]; ++it, sh4 += 4) { LRDMC_DISPN(true) LRDMC_SETA(e[h]) LRDMC_FEEDN }      // Slater s
@@ -173,13 +173,111 @@ __device__ __forceinline__ void mo_values(const DevSys &S, const double *__restr
 #undef LRDMC_ACC2
 }
 
+// ---- candidate ratios in column form (rows a2-a4 fused) -----------------------------------------------------------
+// The determinant ratio of candidate p (electron i moved to r'_p) needs ONE linear combination of the MOs at r'_p:
+//     sum_m phi_m(r'_p) Dinv[m][i]  =  sum_mu chi_mu(r'_p) Bc[mu][i],      Bc = C Dinv   (A x n_s),
+// so the warp forms the entries of Bc it needs once per evaluation (2 A n_s^2 flop per spin) and contracts every AO value
+// with one number (2 P A flop) instead of with n_s MO coefficients (2 P A n_s flop through the MOs).
+// Lane = 4 g + t: row g = electron il of the current block of 8 same-spin electrons, t = shell slot of the current
+// 4-shell group.  The lane builds Bc[ao(shell t, component c)][electron g] from the same fragment table the tensor-core
+// pass uses -- exactly the entries it consumes, nothing is exchanged between lanes -- and handles all six displaced
+// points r_i +- a e_k of its electron:  |r_i +- a e_k - R|^2 = |d0|^2 + a^2 +- 2 a e_k.d0  (d0 = r_i - R) shares the
+// centre distance and three dot products between the six exponent arguments.
+//   av[k] = a e_k (displacement of direction +k), a2 = a^2;  acc[d], d = 2k (+), 2k+1 (-): this lane's share (its
+//   shells) of the determinant ratio of candidate (i, d); the caller adds the four lanes of a quad.
+template <int NT>
+__device__ __forceinline__ void ao_columns(const DevSys &S, const double *__restrict__ shells, const double *__restrict__ bf, const double *__restrict__ etab,
+                                           const double *__restrict__ dinv, int ns, int il, double x0, double y0, double z0,
+                                           const double (&av)[3][3], double a2, int lane, double (&acc)[6])
+{
+    const int t = lane & 3;
+    const double4 *sh4 = reinterpret_cast<const double4 *>(shells) + t;
+    const double *b = bf + t;                        // entry (k-step, MO m, shell slot t) sits at b[(kstep NT + m/8) 32 + (m%8) 4]
+    constexpr int NM = 8 * NT;
+    double dcol[NT <= 2 ? NM : 1];                   // column il of Dinv (rows >= n_s are zero padded)
+    if (NT <= 2) {
+#pragma unroll
+        for (int m = 0; m < (NT <= 2 ? NM : 1); ++m) dcol[m] = dinv[m * ns + il];
+    }
+#pragma unroll
+    for (int d = 0; d < 6; ++d) acc[d] = 0.0;
+#define LRDMC_DC(m) (NT <= 2 ? dcol[NT <= 2 ? (m) : 0] : dinv[(m) * ns + il])
+#define LRDMC_BCOL(dst)                                                                         \
+    {                                                                                           \
+        double s_ = 0.0;                                                                        \
+        _Pragma("unroll") for (int m = 0; m < NM; ++m) s_ = fma(b[(m >> 3) * 32 + (m & 7) * 4], LRDMC_DC(m), s_); \
+        dst = s_; b += NT * 32;                                                                 \
+    }
+    // exponent arguments of the six displaced points: -z (q0 +- 2 sk[k]),  q0 = |d0|^2 + a^2,  sk[k] = a e_k . d0
+#define LRDMC_GEOM                                                                              \
+        const double4 s = *sh4; const double z = s.w;                                           \
+        const double dx0 = x0 - s.x, dy0 = y0 - s.y, dz0 = z0 - s.z;                            \
+        const double q0 = fma(dx0, dx0, fma(dy0, dy0, fma(dz0, dz0, a2)));                      \
+        double sk[3];                                                                           \
+        _Pragma("unroll") for (int k = 0; k < 3; ++k) sk[k] = fma(av[k][0], dx0, fma(av[k][1], dy0, av[k][2] * dz0));
+#define LRDMC_EXPS                                                                              \
+        const double zq = -z * q0, tz = -2.0 * z;                                               \
+        double e[6];                                                                            \
+        _Pragma("unroll") for (int k = 0; k < 3; ++k) { e[2 * k] = exp_tab(fma(tz, sk[k], zq), etab); e[2 * k + 1] = exp_tab(fma(-tz, sk[k], zq), etab); }
+    for (int it = 0; it < S.n_it[0]; ++it, sh4 += 4) {            // Slater s: exp(-z r)
+        LRDMC_GEOM
+        double bc; LRDMC_BCOL(bc)
+#pragma unroll
+        for (int d = 0; d < 6; ++d) {
+            const double q = fma((d & 1) ? -2.0 : 2.0, sk[d >> 1], q0);
+            acc[d] = fma(exp_tab(-z * (q * fast_rsqrt(q)), etab), bc, acc[d]);
+        }
+    }
+    for (int it = 0; it < S.n_it[1]; ++it, sh4 += 4) {            // s
+        LRDMC_GEOM
+        double bc; LRDMC_BCOL(bc)
+        LRDMC_EXPS
+#pragma unroll
+        for (int d = 0; d < 6; ++d) acc[d] = fma(e[d], bc, acc[d]);
+    }
+    for (int it = 0; it < S.n_it[2]; ++it, sh4 += 4) {            // p: x y z  ->  e (bc . d)
+        LRDMC_GEOM
+        double bc[3]; LRDMC_BCOL(bc[0]) LRDMC_BCOL(bc[1]) LRDMC_BCOL(bc[2])
+        LRDMC_EXPS
+        const double l0 = fma(bc[0], dx0, fma(bc[1], dy0, bc[2] * dz0));        // linear form at d0; the shift adds bc . (a e_k)
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            const double lk = fma(bc[0], av[k][0], fma(bc[1], av[k][1], bc[2] * av[k][2]));
+            acc[2 * k] = fma(e[2 * k], l0 + lk, acc[2 * k]);
+            acc[2 * k + 1] = fma(e[2 * k + 1], l0 - lk, acc[2 * k + 1]);
+        }
+    }
+    for (int it = 0; it < S.n_it[3]; ++it, sh4 += 4) {            // d: xx xy xz yy yz zz  ->  e Q(d),  Q(d0 +- v) = Q(d0) +- v.grad Q(d0) + Q(v)
+        LRDMC_GEOM
+        double bc[6]; LRDMC_BCOL(bc[0]) LRDMC_BCOL(bc[1]) LRDMC_BCOL(bc[2]) LRDMC_BCOL(bc[3]) LRDMC_BCOL(bc[4]) LRDMC_BCOL(bc[5])
+        LRDMC_EXPS
+        const double gx = fma(2.0 * bc[0], dx0, fma(bc[1], dy0, bc[2] * dz0));
+        const double gy = fma(bc[1], dx0, fma(2.0 * bc[3], dy0, bc[4] * dz0));
+        const double gz = fma(bc[2], dx0, fma(bc[4], dy0, 2.0 * bc[5] * dz0));
+        const double Q0 = 0.5 * fma(gx, dx0, fma(gy, dy0, gz * dz0));
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            const double vx = av[k][0], vy = av[k][1], vz = av[k][2];
+            const double lin = fma(gx, vx, fma(gy, vy, gz * vz));
+            const double Qv = fma(vx, fma(bc[0], vx, fma(bc[1], vy, bc[2] * vz)), fma(vy, fma(bc[3], vy, bc[4] * vz), bc[5] * vz * vz));
+            const double Qs = Q0 + Qv;
+            acc[2 * k] = fma(e[2 * k], Qs + lin, acc[2 * k]);
+            acc[2 * k + 1] = fma(e[2 * k + 1], Qs - lin, acc[2 * k + 1]);
+        }
+    }
+#undef LRDMC_EXPS
+#undef LRDMC_GEOM
+#undef LRDMC_BCOL
+#undef LRDMC_DC
+}
+
 // Refresh the cached MO rows (value, gradient, Laplacian) of electron i at position (px,py,pz): moc[i][comp][m].
 template <int NT>
-__device__ __forceinline__ void refresh_mo_cache(const DevSys &S, const double *shells, const double *bf, double *moc_i,
+__device__ __forceinline__ void refresh_mo_cache(const DevSys &S, const double *shells, const double *bf, const double *etab, double *moc_i,
                                                  double px, double py, double pz, int lane)
 {
     double acc[NT][2];
-    mo_pass<NT, true>(S, shells, bf, px, py, pz, lane, acc);
+    mo_pass<NT, true>(S, shells, bf, etab, px, py, pz, lane, acc);
     const int t = lane & 3, g = lane >> 2;
     if (g < 5) {
 #pragma unroll
