@@ -82,7 +82,7 @@ __device__ __forceinline__ EvalOut evaluate_walker(const DevSys &S, const WarpSt
             if (j > ii) ve += ir;
         }
         // grad D / D and lap D / D through the stored inverse and the cached MO rows: the two lanes split the MOs
-        const double *mc = ws.moc + (size_t)ii * 5 * S.OS, *di = ws.dinv[sp] + il;
+        const double *mc = ws.moc + (size_t)ii * 5 * S.OS, *di = (sp ? ws.dinv[1] : ws.dinv[0]) + il;
         double Gx = 0.0, Gy = 0.0, Gz = 0.0, Ld = 0.0;
         for (int m = sub; m < ns; m += 2) {
             const double d = di[m * ns];
@@ -116,7 +116,7 @@ __device__ __forceinline__ EvalOut evaluate_walker(const DevSys &S, const WarpSt
                 const int il = valid ? il0 + g : 0, i = off + il;
                 const double x0 = ws.r[3 * i], y0 = ws.r[3 * i + 1], z0 = ws.r[3 * i + 2];
                 double acc[6], Jn[6];
-                ao_columns<NT>(S, T.shells, T.bf[sp], T.etab, ws.dinv[sp], ns, il, x0, y0, z0, av, a2, lane, acc);
+                ao_columns<NT>(S, T.shells, sp ? T.bf[1] : T.bf[0], T.etab, sp ? ws.dinv[1] : ws.dinv[0], ns, il, x0, y0, z0, av, a2, lane, acc);
                 // Jastrow ratio (row a5): the 4 lanes of the quad split the partners; u = c r/(1 + b r) = c/(b + 1/r)
 #pragma unroll
                 for (int d = 0; d < 6; ++d) Jn[d] = 0.0;
@@ -278,12 +278,12 @@ __device__ __forceinline__ void apply_move(const DevSys &S, const WarpState &ws,
     const double px = ws.r[3 * i] + step * ws.U[k], py = ws.r[3 * i + 1] + step * ws.U[3 + k], pz = ws.r[3 * i + 2] + step * ws.U[6 + k];
     double *mc = ws.moc + (size_t)i * 5 * S.OS;
     __syncwarp();
-    refresh_mo_cache<NT>(S, T.shells, T.bf[sp], T.etab, mc, px, py, pz, lane);
+    refresh_mo_cache<NT>(S, T.shells, sp ? T.bf[1] : T.bf[0], T.etab, mc, px, py, pz, lane);
     refresh_onebody(S.n_nuc, S.has_j1, S.a, T.nuc, ws.ob + 8 * i, px, py, pz, lane);
     if (lane == 0) { ws.r[3 * i] = px; ws.r[3 * i + 1] = py; ws.r[3 * i + 2] = pz; }
     __syncwarp();
     // s_k = sum_m phi_m Dinv[m][k];  rho = s_il;  Dinv'[m][il] = Dinv[m][il]/rho;  Dinv'[m][k] = Dinv[m][k] - Dinv[m][il] s_k / rho
-    double *dinv = ws.dinv[sp], *sk = ws.el + 2 * N, *col = ws.el + 3 * N;   // scratch: s_k and the old column il (n_s <= N each)
+    double *dinv = sp ? ws.dinv[1] : ws.dinv[0], *sk = ws.el + 2 * N, *col = ws.el + 3 * N;   // scratch: s_k and the old column il (n_s <= N each)
     for (int kk = lane; kk < ns; kk += 32) {
         double s = 0.0;
         for (int m = 0; m < ns; ++m) s += mc[m] * dinv[m * ns + kk];

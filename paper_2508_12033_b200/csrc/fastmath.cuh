@@ -38,10 +38,15 @@ __device__ __forceinline__ double exp_nonpos(double x)
     return (x < -708.0) ? 0.0 : res;
 }
 
-// exp(x) for -708 < x < 708 through a 256-entry table of 2^(j/256) (shared memory, built at init):
-//   x = (256 e + j) ln2/256 + r, |r| <= ln2/512 = 1.36e-3;  e^r by the degree-4 Taylor polynomial (truncation r^5/120 < 4e-17);
-//   exp(x) = 2^e * tab[j] * e^r.  8 FP64 instructions + one LDS instead of 16: the AO exponentials are 1/3 of the FP64 work.
+// exp(x) for -5e6 < x < 708 through a 256-entry table of 2^(j/256) (shared memory, built at init):
+//   x = (256 e + j) ln2/256 + r, |r| <= h = ln2/512 = 1.36e-3;  e^r by a cubic: the Taylor cubic with its r^4/24 term
+//   economised onto [-h, h] (r^4 ~ h^2 r^2 - h^4/8), |error| < 1.8e-14 relative;  exp(x) = 2^e * tab[j] * e^r.
+//   7 FP64 instructions + 6 integer/LDS ones: the AO exponentials are 1/3 of the FP64 work of the path.
 // The reduction uses ln2/256 as one double: |error of r| <= |k| 2^-53 ln2/256, i.e. < 5e-15 relative for results above 1e-20.
+// Below x = -707.7 the exponent is clamped: the result is then a correct mantissa times 2^-1021 (1e-308, i.e. zero for
+// every sum of the path).  The caller keeps x above -5e6 (the integer conversion of x 256/ln2 must not wrap).
+#define LRDMC_EXP_XMIN (-4.0e6)
+__device__ __forceinline__ double exp_arg_floor(double x) { return (x < LRDMC_EXP_XMIN) ? LRDMC_EXP_XMIN : x; }   // no NaN handling: 3 instructions
 __device__ __forceinline__ double exp_tab(double x, const double *__restrict__ etab)
 {
     const double magic = 6755399441055744.0;                       // 1.5 * 2^52
@@ -49,13 +54,15 @@ __device__ __forceinline__ double exp_tab(double x, const double *__restrict__ e
     const int k = __double2loint(t);
     const double kd = t - magic;
     const double r = fma(kd, -2.7076061740622863649e-03, x);       // ln2 / 256
-    double p = fma(r, 4.16666666666666666667e-02, 1.66666666666666666667e-01);
-    p = fma(p, r, 0.5);
+    double p = fma(r, 1.66666666666666666667e-01, 0.5000000763659499);
     p = fma(p, r, 1.0);
-    p = fma(p, r, 1.0);
-    const double v = etab[k & 255] * p;                            // in (0.99, 2.01): adding to the exponent stays normal for e >= -1021
-    const double res = __hiloint2double(__double2hiint(v) + ((k >> 8) << 20), __double2loint(v));
-    return (k < -1021 * 256) ? 0.0 : res;
+    p = fma(p, r, 0.9999999999999825);
+    int j; asm("and.b32 %0, %1, 255;" : "=r"(j) : "r"(k));         // opaque to the optimiser, or it re-derives the address from k (2 more instructions)
+    double tv;                                                     // explicit shared-space load: one LOP3 (j) serves the address and the exponent
+    asm("ld.shared.f64 %0, [%1];" : "=d"(tv) : "r"((unsigned)__cvta_generic_to_shared(etab) + 8u * (unsigned)j));
+    const double v = tv * p;                                       // in (0.99, 2.01)
+    const int kc = max(k, -1021 * 256);                            // clamped: kc - j is no multiple of 256 then, the value is ~1e-308 anyway
+    return __hiloint2double(__double2hiint(v) + ((kc - j) << 12), __double2loint(v));
 }
 
 // 1/a for ordinary positive a (no denormal / inf handling): hardware seed (about 2^-22) + one cubic step.

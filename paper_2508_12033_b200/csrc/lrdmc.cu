@@ -145,9 +145,9 @@ extern "C" int lrdmc_init(lrdmc_ctx **out, const lrdmc_system *sys, const lrdmc_
     const size_t moc_doubles = (size_t)S.N * 5 * S.OS;
     S.moc_in_smem = moc_doubles * 8 <= 12 * 1024;
     size_t o = 0;
+    S.off_etab = (int)o; o += 256;              // always first: exp_tab addresses it as (dynamic smem base) + 8 j
     S.off_shells = (int)o; o += align_up(h_sh.size(), 2);
     S.off_nuc = (int)o; o += align_up(h_nuc.size(), 2);
-    S.off_etab = (int)o; o += 256;
     S.off_bf[0] = (int)o; if (S.bf_in_smem) o += bf_n;
     S.off_bf[1] = (int)o; if (S.bf_in_smem && !S.same_C) o += bf_n;
     S.tables_doubles = (int)align_up(o, 2);

@@ -14,7 +14,7 @@ __device__ __forceinline__ void stage_tables(const DevSys &S, double *smem)
         for (int i = threadIdx.x; i < nb; i += blockDim.x) smem[S.off_bf[0] + i] = S.bfrag[0][i];
         if (!S.same_C && S.n_dn > 0) for (int i = threadIdx.x; i < nb; i += blockDim.x) smem[S.off_bf[1] + i] = S.bfrag[1][i];
     }
-    for (int i = threadIdx.x; i < 256; i += blockDim.x) smem[S.off_etab + i] = S.etab[i];
+    for (int i = threadIdx.x; i < 256; i += blockDim.x) smem[i] = S.etab[i];        // off_etab == 0 by construction
     __syncthreads();
 }
 
@@ -24,7 +24,7 @@ template <bool TS>
 __device__ __forceinline__ Tables table_pointers(const DevSys &S, const double *smem)
 {
     Tables T;
-    T.shells = smem + S.off_shells; T.nuc = smem + S.off_nuc; T.etab = smem + S.off_etab;
+    T.shells = smem + S.off_shells; T.nuc = smem + S.off_nuc; T.etab = smem;
     if (TS) { T.bf[0] = smem + S.off_bf[0]; T.bf[1] = smem + (S.same_C ? S.off_bf[0] : S.off_bf[1]); }
     else if (S.bf_in_smem) { T.bf[0] = smem + S.off_bf[0]; T.bf[1] = S.same_C ? T.bf[0] : smem + S.off_bf[1]; }
     else { T.bf[0] = S.bfrag[0]; T.bf[1] = S.same_C ? S.bfrag[0] : S.bfrag[1]; }

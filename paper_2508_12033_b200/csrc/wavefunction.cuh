@@ -59,7 +59,7 @@ __device__ __forceinline__ void mo_pass(const DevSys &S, const double *__restric
     // ---- group 0: Slater-type s, chi = exp(-z r); grad = -z chi rhat; lap = chi (z^2 - 2 z / r)
     for (int it = 0; it < S.n_it[0]; ++it, sh4 += 4) {
         double4 s = *sh4; double dx = px - s.x, dy = py - s.y, dz = pz - s.z, z = s.w;
-        double r = sqrt(dx * dx + dy * dy + dz * dz), e = exp_tab(-z * r, etab);
+        double r = sqrt(dx * dx + dy * dy + dz * dz), e = exp_tab(exp_arg_floor(-z * r), etab);
         if (!DERIV) { LRDMC_FEED(e); }
         else {
             double ir = 1.0 / r, d = (g == 1) ? dx : ((g == 2) ? dy : dz);
@@ -70,14 +70,14 @@ __device__ __forceinline__ void mo_pass(const DevSys &S, const double *__restric
     // ---- group 1: s Gaussians
     for (int it = 0; it < S.n_it[1]; ++it, sh4 += 4) {
         double4 s = *sh4; double dx = px - s.x, dy = py - s.y, dz = pz - s.z, z = s.w;
-        double e = exp_tab(-z * (dx * dx + dy * dy + dz * dz), etab);
+        double e = exp_tab(exp_arg_floor(-z * (dx * dx + dy * dy + dz * dz)), etab);
         if (!DERIV) { LRDMC_FEED(e); }
         else { AxisPoly X = axis_poly(dx, z), Y = axis_poly(dy, z), Z = axis_poly(dz, z); LRDMC_FEED((gto_component<0, 0, 0>(g, X, Y, Z, e))); }
     }
     // ---- group 2: p Gaussians (x, y, z)
     for (int it = 0; it < S.n_it[2]; ++it, sh4 += 4) {
         double4 s = *sh4; double dx = px - s.x, dy = py - s.y, dz = pz - s.z, z = s.w;
-        double e = exp_tab(-z * (dx * dx + dy * dy + dz * dz), etab);
+        double e = exp_tab(exp_arg_floor(-z * (dx * dx + dy * dy + dz * dz)), etab);
         if (!DERIV) { LRDMC_FEED(dx * e); LRDMC_FEED(dy * e); LRDMC_FEED(dz * e); }
         else {
             AxisPoly X = axis_poly(dx, z), Y = axis_poly(dy, z), Z = axis_poly(dz, z);
@@ -88,7 +88,7 @@ __device__ __forceinline__ void mo_pass(const DevSys &S, const double *__restric
     // ---- group 3: d Gaussians (xx, xy, xz, yy, yz, zz)
     for (int it = 0; it < S.n_it[3]; ++it, sh4 += 4) {
         double4 s = *sh4; double dx = px - s.x, dy = py - s.y, dz = pz - s.z, z = s.w;
-        double e = exp_tab(-z * (dx * dx + dy * dy + dz * dz), etab);
+        double e = exp_tab(exp_arg_floor(-z * (dx * dx + dy * dy + dz * dz)), etab);
         if (!DERIV) {
             double xe = dx * e, ye = dy * e, ze = dz * e;
             LRDMC_FEED(dx * xe); LRDMC_FEED(dx * ye); LRDMC_FEED(dx * ze); LRDMC_FEED(dy * ye); LRDMC_FEED(dy * ze); LRDMC_FEED(dz * ze);
@@ -142,7 +142,7 @@ __device__ __forceinline__ void mo_values(const DevSys &S, const double *__restr
         _Pragma("unroll") for (int h = 0; h < NB; ++h) {                                        \
             dx[h] = pt[h][0] - s.x; dy[h] = pt[h][1] - s.y; dz[h] = pt[h][2] - s.z;              \
             const double q = dx[h] * dx[h] + dy[h] * dy[h] + dz[h] * dz[h];                      \
-            e[h] = exp_tab(-z * (SLATER ? q * fast_rsqrt(q) : q), etab);                         \
+            e[h] = exp_tab(exp_arg_floor(-z * (SLATER ? q * fast_rsqrt(q) : q)), etab);                         \
         }
 #define LRDMC_SETA(expr) _Pragma("unroll") for (int h = 0; h < NB; ++h) a[h] = (expr);
     for (int it = 0; it < S.n_it[0]; ++it, sh4 += 4) { LRDMC_DISPN(true) LRDMC_SETA(e[h]) LRDMC_FEEDN }      // Slater s
@@ -216,7 +216,8 @@ __device__ __forceinline__ void ao_columns(const DevSys &S, const double *__rest
         double sk[3];                                                                           \
         _Pragma("unroll") for (int k = 0; k < 3; ++k) sk[k] = fma(av[k][0], dx0, fma(av[k][1], dy0, av[k][2] * dz0));
 #define LRDMC_EXPS                                                                              \
-        const double zq = -z * q0, tz = -2.0 * z;                                               \
+        const double zq0 = -z * q0; const bool far_ = zq0 < 0.5 * LRDMC_EXP_XMIN;   /* |2 z sk| <= z q0: the six arguments lie in [2 zq, 0] */ \
+        const double zq = far_ ? 0.5 * LRDMC_EXP_XMIN : zq0, tz = far_ ? 0.0 : -2.0 * z;        \
         double e[6];                                                                            \
         _Pragma("unroll") for (int k = 0; k < 3; ++k) { e[2 * k] = exp_tab(fma(tz, sk[k], zq), etab); e[2 * k + 1] = exp_tab(fma(-tz, sk[k], zq), etab); }
     for (int it = 0; it < S.n_it[0]; ++it, sh4 += 4) {            // Slater s: exp(-z r)
@@ -225,7 +226,7 @@ __device__ __forceinline__ void ao_columns(const DevSys &S, const double *__rest
 #pragma unroll
         for (int d = 0; d < 6; ++d) {
             const double q = fma((d & 1) ? -2.0 : 2.0, sk[d >> 1], q0);
-            acc[d] = fma(exp_tab(-z * (q * fast_rsqrt(q)), etab), bc, acc[d]);
+            acc[d] = fma(exp_tab(exp_arg_floor(-z * (q * fast_rsqrt(q))), etab), bc, acc[d]);
         }
     }
     for (int it = 0; it < S.n_it[1]; ++it, sh4 += 4) {            // s
