@@ -16,6 +16,9 @@
 #ifndef LRDMC_MINB
 #define LRDMC_MINB 2           // CTAs per SM the register allocation must allow
 #endif
+#ifndef LRDMC_LOCKSTEP
+#define LRDMC_LOCKSTEP 1        // balanced mode: the warps of a CTA step together (one barrier per step)
+#endif
 #define LRDMC_NUC_STRIDE 12  // doubles per nucleus row: Rx Ry Rz Z c1 b1 alpha beta gamma delta is_pp pad
 #define LRDMC_EL_ARRAYS 4     // per-electron scratch arrays in shared memory: Jold, lap, s_k, old column
 

@@ -166,7 +166,7 @@ extern "C" int lrdmc_init(lrdmc_ctx **out, const lrdmc_system *sys, const lrdmc_
     c->wpb = LRDMC_WPB;
     for (;;) {
         size_t need = ((size_t)S.tables_doubles + (size_t)c->wpb * S.per_warp_doubles) * 8;
-        if ((need + reserve) * 2 <= per_sm || c->wpb == 1) { c->smem_bytes = (int)need; break; }
+        if ((need + reserve) * LRDMC_MINB <= per_sm || c->wpb == 1) { c->smem_bytes = (int)need; break; }
         c->wpb >>= 1;
     }
     if ((size_t)c->smem_bytes > per_blk_max) { lrdmc_free(c); return LRDMC_ENOMEM; }

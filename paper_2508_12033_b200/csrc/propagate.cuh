@@ -93,15 +93,31 @@ __global__ void __launch_bounds__(LRDMC_WPB * 32, LRDMC_MINB) k_propagate(DevSys
     const Tables T = table_pointers<TS>(S, smem);
     WarpState ws = warp_views(S, smem, warp);
     const unsigned long long t_start = globaltimer_ns();
+    // Balanced mode: every walker takes the same number of steps, so the warps of a CTA pull their walkers together and
+    // meet at a barrier once per step -- they then run the same code region at the same time and share the small
+    // instruction caches (L0 6 KB, L1.5 32 KB against 140 KB of kernel).  Conventional mode: stochastic trip counts
+    // (L168), every warp pulls for itself and never waits.
+    const bool lockstep = LRDMC_LOCKSTEP && mode == LRDMC_BALANCED;
+    __shared__ int s_base;
     for (;;) {
         int k = 0;
-        if (lane == 0) k = atomicAdd(W.counter, 1);
-        k = __shfl_sync(0xffffffffu, k, 0);
-        if (k >= W.n_w) break;
-        load_walker<TS>(S, W, ws, T.nuc, k, lane, true);
+        if (lockstep) {
+            __syncthreads();
+            if (threadIdx.x == 0) s_base = atomicAdd(W.counter, (int)(blockDim.x >> 5));
+            __syncthreads();
+            if (s_base >= W.n_w) break;
+            k = s_base + warp;
+        } else {
+            if (lane == 0) k = atomicAdd(W.counter, 1);
+            k = __shfl_sync(0xffffffffu, k, 0);
+            if (k >= W.n_w) break;
+        }
+        const bool act = k < W.n_w;
+        if (act) load_walker<TS>(S, W, ws, T.nuc, k, lane, true);
         double w = 1.0, tau_left = tau, omega = 0.0, eL_out = 0.0, W_out = 0.0;
         long long moves = 0; int n_node = 0, n_nonpos = 0;
         for (uint32_t s = 0;; ++s) {
+            if (lockstep) { __syncthreads(); if (!act) { if ((int)s == n_moves) break; continue; } }
             const StepDraws d = step_draws(S, (uint32_t)k, cycle, s, mode == LRDMC_CONVENTIONAL);
             publish_frame(ws, d, lane);
             const EvalOut e = evaluate_walker<NT, TS, LRDMC_NB>(S, ws, T, lane);
@@ -125,6 +141,7 @@ __global__ void __launch_bounds__(LRDMC_WPB * 32, LRDMC_MINB) k_propagate(DevSys
             const int j = select_move(S, ws, d.u_sel, lane);       // Alg.2 line 7 (L408)
             if (j >= 0) { apply_move<NT, TS>(S, ws, T, j, lane); ++moves; }
         }
+        if (!act) continue;
         int nonfinite = 0;
         if (!isfinite(w) || !isfinite(omega)) { nonfinite = 1; w = 0.0; omega = 0.0; }
         store_walker(S, W, ws, k, lane);
@@ -166,7 +183,7 @@ __global__ void __launch_bounds__(LRDMC_WPB * 32, LRDMC_MINB) k_step_debug(DevSy
 
 // ---- (re)build of the inverses and MO caches from the positions (row a13) ---------------------------------------
 template <int NT, bool TS>
-__global__ void __launch_bounds__(256) k_rebuild(DevSys S, DevWalk W, int do_invert)
+__global__ void __launch_bounds__(LRDMC_WPB * 32) k_rebuild(DevSys S, DevWalk W, int do_invert)
 {
     extern __shared__ __align__(16) double smem[];
     stage_tables(S, smem);
