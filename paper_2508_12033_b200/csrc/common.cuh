@@ -19,6 +19,9 @@
 #ifndef LRDMC_LOCKSTEP
 #define LRDMC_LOCKSTEP 1        // balanced mode: the warps of a CTA step together (one barrier per step)
 #endif
+#ifndef LRDMC_BC_DMMA
+#define LRDMC_BC_DMMA 1         // Bc = C Dinv of the column form on the FP64 tensor pipe (0: DFMA chains over the mo_pass fragments)
+#endif
 #define LRDMC_NUC_STRIDE 12  // doubles per nucleus row: Rx Ry Rz Z c1 b1 alpha beta gamma delta is_pp pad
 #define LRDMC_EL_ARRAYS 4     // per-electron scratch arrays in shared memory: Jold, lap, s_k, old column
 
@@ -40,6 +43,8 @@ struct DevSys {
     const double *bfrag[2];    // [n_ksteps][NT][32] FP64 mma B fragments, AO norms folded in
     const double *nuc;         // [n_nuc][LRDMC_NUC_STRIDE]
     const double *etab;        // [256] 2^(j/256) for exp_tab
+    const double *cfrag[2];    // [n_kpairs][2 NT][32] FP64 mma B fragments of the Bc = C Dinv product (ao_columns), norms folded in
+    int n_kpairs, off_cf[2];   // pairs of k-steps (each shell group padded to an even number of k-steps)
     // shared-memory plan (units: doubles)
     int bf_in_smem, moc_in_smem;
     int off_shells, off_nuc, off_bf[2], off_etab, tables_doubles;
@@ -48,7 +53,7 @@ struct DevSys {
 };
 
 // Table pointers as a kernel sees them (shared memory, or global memory for the fragments of the largest systems)
-struct Tables { const double *shells, *nuc, *bf[2], *etab; };
+struct Tables { const double *shells, *nuc, *bf[2], *cf[2], *etab; };
 
 // Walker storage (views into the caller's buffer)
 struct DevWalk {

@@ -116,7 +116,7 @@ __device__ __forceinline__ EvalOut evaluate_walker(const DevSys &S, const WarpSt
                 const int il = valid ? il0 + g : 0, i = off + il;
                 const double x0 = ws.r[3 * i], y0 = ws.r[3 * i + 1], z0 = ws.r[3 * i + 2];
                 double acc[6], Jn[6];
-                ao_columns<NT>(S, T.shells, sp ? T.bf[1] : T.bf[0], T.etab, sp ? ws.dinv[1] : ws.dinv[0], ns, il, x0, y0, z0, av, a2, lane, acc);
+                ao_columns<NT, TS>(S, T.shells, LRDMC_BC_DMMA ? (sp ? T.cf[1] : T.cf[0]) : (sp ? T.bf[1] : T.bf[0]), T.etab, sp ? ws.dinv[1] : ws.dinv[0], ns, il, x0, y0, z0, av, a2, lane, acc);
                 // Jastrow ratio (row a5): the 4 lanes of the quad split the partners; u = c r/(1 + b r) = c/(b + 1/r)
 #pragma unroll
                 for (int d = 0; d < 6; ++d) Jn[d] = 0.0;
@@ -159,7 +159,7 @@ __device__ __forceinline__ EvalOut evaluate_walker(const DevSys &S, const WarpSt
                     pt[h][0] = ws.r[3 * i] + step * ws.U[k]; pt[h][1] = ws.r[3 * i + 1] + step * ws.U[3 + k]; pt[h][2] = ws.r[3 * i + 2] + step * ws.U[6 + k];
                 }
                 double acc[NB][NT][2];
-                mo_values<NT, NB>(S, T.shells, T.bf[sp], T.etab, pt, lane, acc);
+                mo_values<NT, NB, TS>(S, T.shells, T.bf[sp], T.etab, pt, lane, acc);
                 // determinant ratio (row a4): sum_m phi_m(r') Dinv[m][il]; this lane holds m = 8 nt + 2t, +1 (rows beyond n_s are zero-padded)
                 double part[NB], Jn[NB];
 #pragma unroll
@@ -278,7 +278,7 @@ __device__ __forceinline__ void apply_move(const DevSys &S, const WarpState &ws,
     const double px = ws.r[3 * i] + step * ws.U[k], py = ws.r[3 * i + 1] + step * ws.U[3 + k], pz = ws.r[3 * i + 2] + step * ws.U[6 + k];
     double *mc = ws.moc + (size_t)i * 5 * S.OS;
     __syncwarp();
-    refresh_mo_cache<NT>(S, T.shells, sp ? T.bf[1] : T.bf[0], T.etab, mc, px, py, pz, lane);
+    refresh_mo_cache<NT, TS>(S, T.shells, sp ? T.bf[1] : T.bf[0], T.etab, mc, px, py, pz, lane);
     refresh_onebody(S.n_nuc, S.has_j1, S.a, T.nuc, ws.ob + 8 * i, px, py, pz, lane);
     if (lane == 0) { ws.r[3 * i] = px; ws.r[3 * i + 1] = py; ws.r[3 * i + 2] = pz; }
     __syncwarp();

@@ -125,8 +125,32 @@ extern "C" int lrdmc_init(lrdmc_ctx **out, const lrdmc_system *sys, const lrdmc_
                 h_bf[sp][((size_t)kstep * c->NT + t) * 32 + lane] = nrm * C[(size_t)(ao0[s] + comp) * ns + m];
             }
     }
+    // ---- pair table of ao_columns: B fragments of Bc[ao][el] = sum_m C[ao][m] Dinv[m][el], two k-steps per mma column set.
+    //      mma column n = 2 slot + parity (k-step 2 pair + parity of the group's own sequence), mma k = MO 4 j + k.
+    int pair_base[5]; pair_base[0] = 0;
+    for (int g = 0; g < 4; ++g) pair_base[g + 1] = pair_base[g] + (ncomp[g] * S.n_it[g] + 1) / 2;
+    S.n_kpairs = pair_base[4];
+    const int NA = 2 * c->NT;
+    const size_t cf_n = LRDMC_BC_DMMA ? (size_t)S.n_kpairs * NA * 32 : 0;
+    std::vector<double> h_cf[2];
+    for (int sp = 0; sp < (S.same_C ? 1 : 2) && cf_n; ++sp) {
+        const int ns = sp ? sys->n_dn : sys->n_up; const double *C = sp ? mo->C_dn : mo->C_up;
+        h_cf[sp].assign(cf_n, 0.0);
+        for (int g = 0; g < 4; ++g) for (int it = 0; it < S.n_it[g]; ++it) for (int comp = 0; comp < ncomp[g]; ++comp) {
+            const int q = it * ncomp[g] + comp, pair = pair_base[g] + q / 2, par = q & 1;
+            for (int slot = 0; slot < 4; ++slot) {
+                const int s = slot_shell[base[g] + 4 * it + slot];
+                if (s < 0) continue;
+                const double nrm = g == 0 ? 1.0 : gto_norm(bas->zeta[s], lmn[g][comp][0], lmn[g][comp][1], lmn[g][comp][2]);
+                for (int j = 0; j < NA; ++j) for (int k = 0; k < 4; ++k) {
+                    const int m = 4 * j + k; if (m >= ns) continue;
+                    h_cf[sp][((size_t)pair * NA + j) * 32 + 4 * (2 * slot + par) + k] = nrm * C[(size_t)(ao0[s] + comp) * ns + m];
+                }
+            }
+        }
+    }
     // ---- device copies
-    size_t bytes = (h_sh.size() + h_nuc.size() + h_et.size() + bf_n * (S.same_C ? 1 : 2)) * sizeof(double);
+    size_t bytes = (h_sh.size() + h_nuc.size() + h_et.size() + (bf_n + cf_n) * (S.same_C ? 1 : 2)) * sizeof(double);
     cudaError_t ce = cudaMalloc(&c->d_tables, bytes);
     if (ce != cudaSuccess) { snprintf(g_cuda_msg, sizeof g_cuda_msg, "%s (cudaMalloc tables)", cudaGetErrorString(ce)); free(c); return LRDMC_ECUDA; }
     double *d = (double *)c->d_tables;
@@ -134,22 +158,32 @@ extern "C" int lrdmc_init(lrdmc_ctx **out, const lrdmc_system *sys, const lrdmc_
     cudaMemcpy(d, h_nuc.data(), h_nuc.size() * 8, cudaMemcpyHostToDevice); S.nuc = d; d += h_nuc.size();
     cudaMemcpy(d, h_et.data(), h_et.size() * 8, cudaMemcpyHostToDevice); S.etab = d; d += h_et.size();
     cudaMemcpy(d, h_bf[0].data(), bf_n * 8, cudaMemcpyHostToDevice); S.bfrag[0] = d; d += bf_n;
-    if (!S.same_C) { cudaMemcpy(d, h_bf[1].data(), bf_n * 8, cudaMemcpyHostToDevice); S.bfrag[1] = d; } else S.bfrag[1] = S.bfrag[0];
+    if (!S.same_C) { cudaMemcpy(d, h_bf[1].data(), bf_n * 8, cudaMemcpyHostToDevice); S.bfrag[1] = d; d += bf_n; } else S.bfrag[1] = S.bfrag[0];
+    S.cfrag[0] = S.cfrag[1] = d;
+    if (cf_n) {
+        cudaMemcpy(d, h_cf[0].data(), cf_n * 8, cudaMemcpyHostToDevice); d += cf_n;
+        if (!S.same_C) { cudaMemcpy(d, h_cf[1].data(), cf_n * 8, cudaMemcpyHostToDevice); S.cfrag[1] = d; }
+    }
     if (cudaMalloc((void **)&c->d_stats, sizeof(DevStats)) != cudaSuccess) { cudaFree(c->d_tables); free(c); return LRDMC_ECUDA; }
     cudaMemset(c->d_stats, 0, sizeof(DevStats));
     // ---- shared-memory plan
     cudaDeviceProp prop; int dev = 0; cudaGetDevice(&dev); cudaGetDeviceProperties(&prop, dev);
     c->sm_count = prop.multiProcessorCount;
-    const size_t bf_doubles = bf_n * (S.same_C ? 1 : 2);
-    S.bf_in_smem = bf_doubles * 8 <= 64 * 1024;
+    const size_t bf_doubles = (bf_n + cf_n) * (S.same_C ? 1 : 2);
     const size_t moc_doubles = (size_t)S.N * 5 * S.OS;
-    S.moc_in_smem = moc_doubles * 8 <= 12 * 1024;
+    // Either every table and the MO cache sit in shared memory (TS kernels), or the fragment tables and the cache are read
+    // from global memory (large systems; LRDMC_GLOBAL_TABLES forces this path for tests).  No mixed case: a fragment pointer
+    // that may be shared OR global makes nvcc 12.9 infer "shared" for it (cvta.to.shared + ld.shared on a global address).
+    const bool fits = bf_doubles * 8 <= 64 * 1024 && moc_doubles * 8 <= 12 * 1024 && !getenv("LRDMC_GLOBAL_TABLES");
+    S.bf_in_smem = fits; S.moc_in_smem = fits;
     size_t o = 0;
     S.off_etab = (int)o; o += 256;              // always first: exp_tab addresses it as (dynamic smem base) + 8 j
     S.off_shells = (int)o; o += align_up(h_sh.size(), 2);
     S.off_nuc = (int)o; o += align_up(h_nuc.size(), 2);
     S.off_bf[0] = (int)o; if (S.bf_in_smem) o += bf_n;
     S.off_bf[1] = (int)o; if (S.bf_in_smem && !S.same_C) o += bf_n;
+    S.off_cf[0] = (int)o; if (S.bf_in_smem) o += cf_n;
+    S.off_cf[1] = (int)o; if (S.bf_in_smem && !S.same_C) o += cf_n;
     S.tables_doubles = (int)align_up(o, 2);
     size_t w = 0;
     S.o_r = (int)w; w += align_up(3 * (size_t)S.N, 2);

@@ -13,6 +13,9 @@ __device__ __forceinline__ void stage_tables(const DevSys &S, double *smem)
         const int nb = S.n_ksteps * S.NT[0] * 32;
         for (int i = threadIdx.x; i < nb; i += blockDim.x) smem[S.off_bf[0] + i] = S.bfrag[0][i];
         if (!S.same_C && S.n_dn > 0) for (int i = threadIdx.x; i < nb; i += blockDim.x) smem[S.off_bf[1] + i] = S.bfrag[1][i];
+        const int nc = LRDMC_BC_DMMA ? S.n_kpairs * 2 * S.NT[0] * 32 : 0;
+        for (int i = threadIdx.x; i < nc; i += blockDim.x) smem[S.off_cf[0] + i] = S.cfrag[0][i];
+        if (!S.same_C && S.n_dn > 0) for (int i = threadIdx.x; i < nc; i += blockDim.x) smem[S.off_cf[1] + i] = S.cfrag[1][i];
     }
     for (int i = threadIdx.x; i < 256; i += blockDim.x) smem[i] = S.etab[i];        // off_etab == 0 by construction
     __syncthreads();
@@ -25,9 +28,13 @@ __device__ __forceinline__ Tables table_pointers(const DevSys &S, const double *
 {
     Tables T;
     T.shells = smem + S.off_shells; T.nuc = smem + S.off_nuc; T.etab = smem;
-    if (TS) { T.bf[0] = smem + S.off_bf[0]; T.bf[1] = smem + (S.same_C ? S.off_bf[0] : S.off_bf[1]); }
-    else if (S.bf_in_smem) { T.bf[0] = smem + S.off_bf[0]; T.bf[1] = S.same_C ? T.bf[0] : smem + S.off_bf[1]; }
-    else { T.bf[0] = S.bfrag[0]; T.bf[1] = S.same_C ? S.bfrag[0] : S.bfrag[1]; }
+    if (TS) {
+        T.bf[0] = smem + S.off_bf[0]; T.bf[1] = smem + (S.same_C ? S.off_bf[0] : S.off_bf[1]);
+        T.cf[0] = smem + S.off_cf[0]; T.cf[1] = smem + (S.same_C ? S.off_cf[0] : S.off_cf[1]);
+    } else {                                       // global memory only: a single provenance per pointer (see lrdmc_init)
+        T.bf[0] = S.bfrag[0]; T.bf[1] = S.bfrag[1];
+        T.cf[0] = S.cfrag[0]; T.cf[1] = S.cfrag[1];
+    }
     return T;
 }
 
@@ -61,7 +68,7 @@ __device__ __forceinline__ void load_walker(const DevSys &S, const DevWalk &W, W
         for (int i = lane; i < tot; i += 32) ws.dinv[sp][i] = (with_dinv && i < ns * ns) ? src[i] : 0.0;
     }
     const size_t mocn = (size_t)N * 5 * S.OS;
-    if (TS || S.moc_in_smem) { for (int i = lane; i < (int)mocn; i += 32) ws.moc[i] = W.moc[(size_t)k * mocn + i]; }
+    if (TS) { for (int i = lane; i < (int)mocn; i += 32) ws.moc[i] = W.moc[(size_t)k * mocn + i]; }
     else ws.moc = W.moc + (size_t)k * mocn;
     __syncwarp();
     for (int i = 0; i < N; ++i) refresh_onebody(S.n_nuc, S.has_j1, S.a, nuc, ws.ob + 8 * i, ws.r[3 * i], ws.r[3 * i + 1], ws.r[3 * i + 2], lane);
@@ -195,7 +202,7 @@ __global__ void __launch_bounds__(LRDMC_WPB * 32) k_rebuild(DevSys S, DevWalk W,
         load_walker<TS>(S, W, ws, T.nuc, k, lane, !do_invert);
         for (int i = 0; i < N; ++i) {
             const int sp = spin_of(S, i);
-            refresh_mo_cache<NT>(S, T.shells, T.bf[sp], T.etab, ws.moc + (size_t)i * 5 * S.OS, ws.r[3 * i], ws.r[3 * i + 1], ws.r[3 * i + 2], lane);
+            refresh_mo_cache<NT, TS>(S, T.shells, T.bf[sp], T.etab, ws.moc + (size_t)i * 5 * S.OS, ws.r[3 * i], ws.r[3 * i + 1], ws.r[3 * i + 2], lane);
         }
         __syncwarp();
         if (do_invert) {

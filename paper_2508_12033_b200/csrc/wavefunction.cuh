@@ -11,6 +11,11 @@
 #include "common.cuh"
 #include "fastmath.cuh"
 
+// Table element load with an explicit address space.  TS: the tables sit in shared memory (plain load, inferred LDS).
+// !TS: global memory -- spelled as ld.global.nc, because nvcc 12.9 otherwise infers "shared" for the fragment pointer of the
+// inlined passes (cvta.to.shared + ld.shared on a global address: illegal access; seen in PTX, found by the C5 parity test).
+template <bool TS> __device__ __forceinline__ double ldt(const double *p) { return TS ? *p : __ldg(p); }
+
 __device__ __forceinline__ void dmma884(double &c0, double &c1, double a, double b)
 {
     asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
@@ -41,7 +46,7 @@ __device__ __forceinline__ double gto_component(int g, const AxisPoly &X, const 
 // One pass over the whole (sorted, padded) shell list for the 8 points held by the warp.
 // DERIV = false: A fragment = AO value (candidate evaluation, row a2/a3).
 // DERIV = true : the 8 mma rows are 8 COMPONENTS (value, d/dx, d/dy, d/dz, Laplacian, 0,0,0) of ONE point, selector g = lane/4.
-template <int NT, bool DERIV>
+template <int NT, bool DERIV, bool TS>
 __device__ __forceinline__ void mo_pass(const DevSys &S, const double *__restrict__ shells, const double *__restrict__ bf, const double *__restrict__ etab,
                                         double px, double py, double pz, int lane, double (&acc)[NT][2])
 {
@@ -53,7 +58,7 @@ __device__ __forceinline__ void mo_pass(const DevSys &S, const double *__restric
 #define LRDMC_FEED(aval)                                                                        \
     {                                                                                           \
         double a_ = (aval);                                                                     \
-        _Pragma("unroll") for (int nt = 0; nt < NT; ++nt) dmma884(acc[nt][0], acc[nt][1], a_, b[nt * 32]); \
+        _Pragma("unroll") for (int nt = 0; nt < NT; ++nt) dmma884(acc[nt][0], acc[nt][1], a_, ldt<TS>(b + nt * 32)); \
         b += NT * 32;                                                                           \
     }
     // ---- group 0: Slater-type s, chi = exp(-z r); grad = -z chi rhat; lap = chi (z^2 - 2 z / r)
@@ -105,7 +110,7 @@ __device__ __forceinline__ void mo_pass(const DevSys &S, const double *__restric
 // Value-only pass over NB batches of 8 points at once (8*NB candidate points per warp pass): every shell row and every
 // B fragment is loaded once and used NB times, and the NB exponential chains of a lane are independent (ILP NB), which is
 // what the FP64 pipe needs with 4 warps per scheduler.  acc[h] = accumulators of batch h.
-template <int NT, int NB>
+template <int NT, int NB, bool TS>
 __device__ __forceinline__ void mo_values(const DevSys &S, const double *__restrict__ shells, const double *__restrict__ bf, const double *__restrict__ etab,
                                           const double (&pt)[NB][3], int lane, double (&acc)[NB][NT][2])
 {
@@ -130,7 +135,7 @@ __device__ __forceinline__ void mo_values(const DevSys &S, const double *__restr
 #define LRDMC_FEED_(ACC)                                                                        \
     {                                                                                           \
         _Pragma("unroll") for (int nt = 0; nt < NT; ++nt) {                                     \
-            const double bv_ = b[nt * 32];                                                      \
+            const double bv_ = ldt<TS>(b + nt * 32);                                                      \
             _Pragma("unroll") for (int h = 0; h < NB; ++h) dmma884(ACC[h][nt][0], ACC[h][nt][1], a[h], bv_); \
         }                                                                                       \
         b += NT * 32;                                                                           \
@@ -185,7 +190,8 @@ __device__ __forceinline__ void mo_values(const DevSys &S, const double *__restr
 // centre distance and three dot products between the six exponent arguments.
 //   av[k] = a e_k (displacement of direction +k), a2 = a^2;  acc[d], d = 2k (+), 2k+1 (-): this lane's share (its
 //   shells) of the determinant ratio of candidate (i, d); the caller adds the four lanes of a quad.
-template <int NT>
+#if !LRDMC_BC_DMMA
+template <int NT, bool TS>
 __device__ __forceinline__ void ao_columns(const DevSys &S, const double *__restrict__ shells, const double *__restrict__ bf, const double *__restrict__ etab,
                                            const double *__restrict__ dinv, int ns, int il, double x0, double y0, double z0,
                                            const double (&av)[3][3], double a2, int lane, double (&acc)[6])
@@ -205,7 +211,7 @@ __device__ __forceinline__ void ao_columns(const DevSys &S, const double *__rest
 #define LRDMC_BCOL(dst)                                                                         \
     {                                                                                           \
         double s_ = 0.0;                                                                        \
-        _Pragma("unroll") for (int m = 0; m < NM; ++m) s_ = fma(b[(m >> 3) * 32 + (m & 7) * 4], LRDMC_DC(m), s_); \
+        _Pragma("unroll") for (int m = 0; m < NM; ++m) s_ = fma(ldt<TS>(b + (m >> 3) * 32 + (m & 7) * 4), LRDMC_DC(m), s_); \
         dst = s_; b += NT * 32;                                                                 \
     }
     // exponent arguments of the six displaced points: -z (q0 +- 2 sk[k]),  q0 = |d0|^2 + a^2,  sk[k] = a e_k . d0
@@ -271,14 +277,117 @@ __device__ __forceinline__ void ao_columns(const DevSys &S, const double *__rest
 #undef LRDMC_BCOL
 #undef LRDMC_DC
 }
+#else
+// Bc on the FP64 tensor pipe: one mma.m8n8k4 row = electron g, k = 4 MOs, columns = (k-step parity, shell slot), so the
+// lane's two accumulators are exactly its own entries Bc[ao(slot t)][electron g] of two consecutive k-steps:
+// 2 NT DMMA + 2 NT LDS per pair of entries instead of 16 NT DFMA + 16 NT LDS (same FP64-pipe time, 1/8 of the issue slots).
+// A operand = column il of Dinv (2 NT registers per lane); B operand = the pair table `cf` built at init.  Each shell
+// group is padded to an even number of k-steps; s and p iterations are taken two at a time with a one-iteration tail.
+template <int NT, bool TS>
+__device__ __forceinline__ void ao_columns(const DevSys &S, const double *__restrict__ shells, const double *__restrict__ cf, const double *__restrict__ etab,
+                                           const double *__restrict__ dinv, int ns, int il, double x0, double y0, double z0,
+                                           const double (&av)[3][3], double a2, int lane, double (&acc)[6])
+{
+    const int t = lane & 3;
+    const double4 *sh4 = reinterpret_cast<const double4 *>(shells) + t;
+    const double *b = cf + lane;
+    constexpr int NA = 2 * NT;
+    double aop[NA];                                  // A fragments: Dinv[4 j + t][il] (rows >= n_s are zero padded)
+#pragma unroll
+    for (int j = 0; j < NA; ++j) aop[j] = dinv[(4 * j + t) * ns + il];
+#pragma unroll
+    for (int d = 0; d < 6; ++d) acc[d] = 0.0;
+#define LRDMC_BPAIR(v0, v1)                                                                     \
+    {                                                                                           \
+        v0 = 0.0; v1 = 0.0;                                                                     \
+        _Pragma("unroll") for (int j = 0; j < NA; ++j) dmma884(v0, v1, aop[j], ldt<TS>(b + j * 32));      \
+        b += NA * 32;                                                                           \
+    }
+#define LRDMC_GEOM                                                                              \
+        const double4 s = *sh4; const double z = s.w;                                           \
+        const double dx0 = x0 - s.x, dy0 = y0 - s.y, dz0 = z0 - s.z;                            \
+        const double q0 = fma(dx0, dx0, fma(dy0, dy0, fma(dz0, dz0, a2)));                      \
+        double sk[3];                                                                           \
+        _Pragma("unroll") for (int k = 0; k < 3; ++k) sk[k] = fma(av[k][0], dx0, fma(av[k][1], dy0, av[k][2] * dz0));
+#define LRDMC_EXPS                                                                              \
+        const double zq0 = -z * q0; const bool far_ = zq0 < 0.5 * LRDMC_EXP_XMIN;   /* |2 z sk| <= z q0: the six arguments lie in [2 zq, 0] */ \
+        const double zq = far_ ? 0.5 * LRDMC_EXP_XMIN : zq0, tz = far_ ? 0.0 : -2.0 * z;        \
+        double e[6];                                                                            \
+        _Pragma("unroll") for (int k = 0; k < 3; ++k) { e[2 * k] = exp_tab(fma(tz, sk[k], zq), etab); e[2 * k + 1] = exp_tab(fma(-tz, sk[k], zq), etab); }
+    auto slater_body = [&](double bc) {              // Slater s: exp(-z r)
+        LRDMC_GEOM
+#pragma unroll
+        for (int d = 0; d < 6; ++d) {
+            const double q = fma((d & 1) ? -2.0 : 2.0, sk[d >> 1], q0);
+            acc[d] = fma(exp_tab(exp_arg_floor(-z * (q * fast_rsqrt(q))), etab), bc, acc[d]);
+        }
+        sh4 += 4;
+    };
+    auto s_body = [&](double bc) {
+        LRDMC_GEOM
+        LRDMC_EXPS
+#pragma unroll
+        for (int d = 0; d < 6; ++d) acc[d] = fma(e[d], bc, acc[d]);
+        sh4 += 4;
+    };
+    auto p_body = [&](double bcx, double bcy, double bcz) {       // x y z  ->  e (bc . d); the shift adds bc . (a e_k)
+        LRDMC_GEOM
+        LRDMC_EXPS
+        const double l0 = fma(bcx, dx0, fma(bcy, dy0, bcz * dz0));
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            const double lk = fma(bcx, av[k][0], fma(bcy, av[k][1], bcz * av[k][2]));
+            acc[2 * k] = fma(e[2 * k], l0 + lk, acc[2 * k]);
+            acc[2 * k + 1] = fma(e[2 * k + 1], l0 - lk, acc[2 * k + 1]);
+        }
+        sh4 += 4;
+    };
+    {
+        const int n = S.n_it[0]; int it = 0; double b0, b1;
+        for (; it + 1 < n; it += 2) { LRDMC_BPAIR(b0, b1) slater_body(b0); slater_body(b1); }
+        if (it < n) { LRDMC_BPAIR(b0, b1) slater_body(b0); }
+    }
+    {
+        const int n = S.n_it[1]; int it = 0; double b0, b1;
+        for (; it + 1 < n; it += 2) { LRDMC_BPAIR(b0, b1) s_body(b0); s_body(b1); }
+        if (it < n) { LRDMC_BPAIR(b0, b1) s_body(b0); }
+    }
+    {
+        const int n = S.n_it[2]; int it = 0; double b0, b1, b2, b3, b4, b5;
+        for (; it + 1 < n; it += 2) { LRDMC_BPAIR(b0, b1) LRDMC_BPAIR(b2, b3) LRDMC_BPAIR(b4, b5) p_body(b0, b1, b2); p_body(b3, b4, b5); }
+        if (it < n) { LRDMC_BPAIR(b0, b1) LRDMC_BPAIR(b2, b3) p_body(b0, b1, b2); }
+    }
+    for (int it = 0; it < S.n_it[3]; ++it, sh4 += 4) {            // d: xx xy xz yy yz zz  ->  e Q(d),  Q(d0 +- v) = Q(d0) +- v.grad Q(d0) + Q(v)
+        double bc[6]; LRDMC_BPAIR(bc[0], bc[1]) LRDMC_BPAIR(bc[2], bc[3]) LRDMC_BPAIR(bc[4], bc[5])
+        LRDMC_GEOM
+        LRDMC_EXPS
+        const double gx = fma(2.0 * bc[0], dx0, fma(bc[1], dy0, bc[2] * dz0));
+        const double gy = fma(bc[1], dx0, fma(2.0 * bc[3], dy0, bc[4] * dz0));
+        const double gz = fma(bc[2], dx0, fma(bc[4], dy0, 2.0 * bc[5] * dz0));
+        const double Q0 = 0.5 * fma(gx, dx0, fma(gy, dy0, gz * dz0));
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            const double vx = av[k][0], vy = av[k][1], vz = av[k][2];
+            const double lin = fma(gx, vx, fma(gy, vy, gz * vz));
+            const double Qv = fma(vx, fma(bc[0], vx, fma(bc[1], vy, bc[2] * vz)), fma(vy, fma(bc[3], vy, bc[4] * vz), bc[5] * vz * vz));
+            const double Qs = Q0 + Qv;
+            acc[2 * k] = fma(e[2 * k], Qs + lin, acc[2 * k]);
+            acc[2 * k + 1] = fma(e[2 * k + 1], Qs - lin, acc[2 * k + 1]);
+        }
+    }
+#undef LRDMC_EXPS
+#undef LRDMC_GEOM
+#undef LRDMC_BPAIR
+}
+#endif
 
 // Refresh the cached MO rows (value, gradient, Laplacian) of electron i at position (px,py,pz): moc[i][comp][m].
-template <int NT>
+template <int NT, bool TS>
 __device__ __forceinline__ void refresh_mo_cache(const DevSys &S, const double *shells, const double *bf, const double *etab, double *moc_i,
                                                  double px, double py, double pz, int lane)
 {
     double acc[NT][2];
-    mo_pass<NT, true>(S, shells, bf, etab, px, py, pz, lane, acc);
+    mo_pass<NT, true, TS>(S, shells, bf, etab, px, py, pz, lane, acc);
     const int t = lane & 3, g = lane >> 2;
     if (g < 5) {
 #pragma unroll

@@ -42,8 +42,9 @@ SYSTEMS = {
     "ragged-9u4d-NT2": lambda: _with_walkers(wl.tiny_molecule(9, 4, 4, 20, seed=11), 13),
     "ragged-17u3d-NT4": lambda: _with_walkers(wl.tiny_molecule(17, 3, 5, 30, seed=12), 9),
     "he-triplet-slater": lambda: _with_walkers(wl.slater_atom(2.0, [2.0, 0.6], 2, 0, np.eye(2), np.zeros((2, 0)), 0.2, jastrow=dict(a_par=0.25, a_anti=0.5, b2=0.5)), 64),
-    "C2-synthetic10": lambda: _with_walkers(wl.synthetic10(), 300),
+    "C2-synthetic10": lambda: _with_walkers(wl.synthetic10(), 1024),          # BASELINE configs[1] at its full N_w
     "C3-water-methane-shaped": lambda: _with_walkers(wl.water_methane(n_walkers=100), 100),
+    "C5-cluster64-doublemesh": lambda: _with_walkers(wl.cluster64(n_walkers=10), 10),   # 64 e, 600 AOs, a/a' (NT = 4, tables in global memory)
 }
 
 
@@ -147,6 +148,27 @@ def test_whole_cycle_trajectories_weights_and_branching(B, name, mode):
         assert abs(sg.lockstep_idle_frac - so["lockstep_idle_frac"]) < 1e-12
         r2, *_ = o.get_state(); gr2 = np_(g.lrdmc_get_walkers()[0])
         assert np.abs(gr2 - r2).max() < 1e-11 and np.all(np_(g.lrdmc_get_walkers()[3]) == 1.0)
+    g.close()
+
+
+@pytest.mark.parametrize("name", ["C1-hydrogen", "tiny-3u3d-pp", "C3-water-methane-shaped"])
+def test_large_system_path_tables_in_global_memory(B, name, monkeypatch):
+    """The kernels of systems whose tables do not fit shared memory (C5) read fragments and MO cache from global memory;
+    LRDMC_GLOBAL_TABLES forces that path on small systems so that it is compared with the oracle on every run."""
+    monkeypatch.setenv("LRDMC_GLOBAL_TABLES", "1")
+    s, x0, o, g = _pair(B, name)
+    N = s["n_up"] + s["n_dn"]; Kd = 3 * N / s["a"]**2
+    r, du, dd, w = o.get_state(); g.lrdmc_set_state(r, du, dd, w)
+    R, scal, js = o.step_debug(-3.0, 2, 1)
+    gR, gscal, gjs = [np_(t) for t in g.lrdmc_step_debug(-3.0, 2, 1)]
+    assert relerr(gR, R, 1.0) < TOL and np.array_equal(gjs, js)
+    assert np.max(np.abs(gscal[:, :4] - scal[:, :4]) / np.maximum(np.abs(scal[:, :4]), Kd)) < TOL
+    assert o.propagate(ref.BALANCED, 12, 0.0, -5.0, 4) == 0
+    g.lrdmc_propagate(B.BALANCED, 12, 0.0, -5.0, 4)
+    assert np.abs(np_(g.lrdmc_get_walkers()[0]) - o.get_state()[0]).max() < 1e-11
+    assert relerr(np_(g.lrdmc_get_walkers()[3]), o.get_state()[3]) < 1e-9
+    rc, par = o.reconfigure(4)
+    assert np.array_equal(np_(g.lrdmc_reconfigure(4, want_parents=True)), par)
     g.close()
 
 
