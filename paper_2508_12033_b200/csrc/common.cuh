@@ -62,6 +62,7 @@ struct DevWalk {
     double *r_alt;        // gather target
     double *dinv[2];      // [n_w][n_s*n_s]
     double *moc;          // [n_w][N][5][OS] cached MO value/grad/lap rows at each electron
+    double *moc_alt;      // gather target of the cache rows (they depend on the positions only: copies of the parent's are exact)
     double *w, *eL, *W, *omega;
     long long *nmoves;
     int *flags;           // [n_w][3] node / nonpos / nonfinite counts of the last propagate

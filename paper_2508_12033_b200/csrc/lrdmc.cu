@@ -241,7 +241,7 @@ static size_t carve(const lrdmc_ctx *c, int n_w, char *base, DevWalk *W)
 #define TAKE(field, type, count) do { if (W) W->field = (type *)(base + o); o = align_up(o + sizeof(type) * (count), 256); } while (0)
     TAKE(r, double, nw * 3 * S.N); TAKE(r_alt, double, nw * 3 * S.N);
     TAKE(dinv[0], double, nw * S.n_up * S.n_up); TAKE(dinv[1], double, nw * S.n_dn * S.n_dn + 1);
-    TAKE(moc, double, nw * S.N * 5 * S.OS);
+    TAKE(moc, double, nw * S.N * 5 * S.OS); TAKE(moc_alt, double, nw * S.N * 5 * S.OS);
     TAKE(w, double, nw); TAKE(eL, double, nw); TAKE(W, double, nw); TAKE(omega, double, nw);
     TAKE(nmoves, long long, nw); TAKE(flags, int, nw * 3);
     TAKE(wq, unsigned long long, nw); TAKE(prefix, unsigned long long, nw); TAKE(parents, int, nw);
@@ -283,7 +283,7 @@ static int grid_for(const lrdmc_ctx *c) { int g = (c->W.n_w + c->wpb - 1) / c->w
         ++c->launches;                                                                                           \
     } while (0)
 
-static int rebuild(lrdmc_ctx *c, int do_invert, cudaStream_t st)
+static int rebuild(lrdmc_ctx *c, int do_invert /* bit 0: invert, bit 1: the MO cache is valid */, cudaStream_t st)
 {
     CK(cudaMemsetAsync(c->W.counter, 0, 64 * sizeof(int), st));
     DISPATCH_NT(k_rebuild, grid_for(c), st, c->S, c->W, do_invert);
@@ -386,11 +386,12 @@ extern "C" int lrdmc_reconfigure(lrdmc_ctx *c, uint64_t cycle, int32_t *parents_
     k_comb<<<1, COMB_THREADS, 0, st>>>(c->W, ctr[0], c->d_stats, parents_dev); ++c->launches;
     CK(cudaGetLastError());
     const int rec = 3 * c->S.N;
-    size_t total = (size_t)c->W.n_w * rec; int gb = (int)((total + 255) / 256); if (gb > 148 * 16) gb = 148 * 16;
-    k_gather<<<gb, 256, 0, st>>>(c->W, rec); ++c->launches;
+    size_t total = (size_t)c->W.n_w * (rec + c->S.N * 5 * c->S.OS / 2); int gb = (int)((total + 255) / 256); if (gb > 148 * 16) gb = 148 * 16;
+    k_gather<<<gb, 256, 0, st>>>(c->W, rec, c->S.N * 5 * c->S.OS); ++c->launches;
     CK(cudaGetLastError());
     double *tmp = c->W.r; c->W.r = c->W.r_alt; c->W.r_alt = tmp;
-    int rc = rebuild(c, 1, st); if (rc) return rc;
+    tmp = c->W.moc; c->W.moc = c->W.moc_alt; c->W.moc_alt = tmp;
+    int rc = rebuild(c, 1 | 2, st); if (rc) return rc;          // invert from the gathered cache rows (reading Q15)
     CK(cudaEventRecord(c->ev[3], st));
     c->have_reconf = 1; c->last_stream = st;
     return LRDMC_OK;

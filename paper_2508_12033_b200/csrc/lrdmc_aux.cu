@@ -106,6 +106,27 @@ extern "C" int lrdmc_measure_fp64_peaks(double *dfma, double *dmma, double *mixe
     return LRDMC_OK;
 }
 
+extern "C" int lrdmc_measure_fp64_operand_peak(double *dfma3)
+{
+    int dev = 0; cudaDeviceProp prop;
+    if (!dfma3 || cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return LRDMC_ECUDA;
+    const int blocks = prop.multiProcessorCount * 8, threads = 256, iters = 8192;
+    double *d_out = NULL; if (cudaMalloc((void **)&d_out, sizeof(double) * blocks * threads) != cudaSuccess) return LRDMC_ECUDA;
+    cudaEvent_t e0, e1; cudaEventCreate(&e0); cudaEventCreate(&e1);
+    float best = 1e30f;
+    for (int rep = 0; rep < 5; ++rep) {
+        cudaEventRecord(e0);
+        k_fp64_peak_3reg<<<blocks, threads>>>(d_out, iters, 1.000001);
+        cudaEventRecord(e1); cudaEventSynchronize(e1);
+        float ms = 0; cudaEventElapsedTime(&ms, e0, e1);
+        if (rep > 0 && ms < best) best = ms;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d_out);
+    if (cudaGetLastError() != cudaSuccess) return LRDMC_ECUDA;
+    *dfma3 = (double)blocks * threads * iters * 8.0 * 2.0 / (best * 1e-3) / 1e12;
+    return LRDMC_OK;
+}
+
 __global__ void k_philox_debug(const uint32_t *ctr, uint32_t k0, uint32_t k1, uint32_t *out, int n)
 {
     int i = blockIdx.x * blockDim.x + threadIdx.x;

@@ -58,7 +58,7 @@ __device__ __forceinline__ void publish_frame(const WarpState &ws, const StepDra
 }
 
 template <bool TS>
-__device__ __forceinline__ void load_walker(const DevSys &S, const DevWalk &W, WarpState &ws, const double *nuc, int k, int lane, bool with_dinv)
+__device__ __forceinline__ void load_walker(const DevSys &S, const DevWalk &W, WarpState &ws, const double *nuc, int k, int lane, bool with_dinv, bool with_onebody = true)
 {
     const int N = S.N;
     for (int i = lane; i < 3 * N; i += 32) ws.r[i] = W.r[(size_t)k * 3 * N + i];
@@ -71,7 +71,7 @@ __device__ __forceinline__ void load_walker(const DevSys &S, const DevWalk &W, W
     if (TS) { for (int i = lane; i < (int)mocn; i += 32) ws.moc[i] = W.moc[(size_t)k * mocn + i]; }
     else ws.moc = W.moc + (size_t)k * mocn;
     __syncwarp();
-    for (int i = 0; i < N; ++i) refresh_onebody(S.n_nuc, S.has_j1, S.a, nuc, ws.ob + 8 * i, ws.r[3 * i], ws.r[3 * i + 1], ws.r[3 * i + 2], lane);
+    if (with_onebody) for (int i = 0; i < N; ++i) refresh_onebody(S.n_nuc, S.has_j1, S.a, nuc, ws.ob + 8 * i, ws.r[3 * i], ws.r[3 * i + 1], ws.r[3 * i + 2], lane);
     __syncwarp();
 }
 
@@ -199,13 +199,13 @@ __global__ void __launch_bounds__(LRDMC_WPB * 32) k_rebuild(DevSys S, DevWalk W,
     WarpState ws = warp_views(S, smem, warp);
     const int N = S.N;
     for (int k = blockIdx.x * wpb + warp; k < W.n_w; k += gridDim.x * wpb) {
-        load_walker<TS>(S, W, ws, T.nuc, k, lane, !do_invert);
-        for (int i = 0; i < N; ++i) {
+        load_walker<TS>(S, W, ws, T.nuc, k, lane, !(do_invert & 1), false);
+        if (!(do_invert & 2)) for (int i = 0; i < N; ++i) {
             const int sp = spin_of(S, i);
             refresh_mo_cache<NT, TS>(S, T.shells, T.bf[sp], T.etab, ws.moc + (size_t)i * 5 * S.OS, ws.r[3 * i], ws.r[3 * i + 1], ws.r[3 * i + 2], lane);
         }
         __syncwarp();
-        if (do_invert) {
+        if (do_invert & 1) {
             for (int sp = 0; sp < 2; ++sp) {
                 const int ns = sp ? S.n_dn : S.n_up, off = sp ? S.n_up : 0;
                 if (!ns) continue;

@@ -73,13 +73,21 @@ __global__ void __launch_bounds__(COMB_THREADS) k_comb(DevWalk W, uint32_t r32, 
 
 // new slot k <- positions of parent[k]; weights <- 1 (L129).  Inverses and caches are rebuilt afterwards (reading Q15),
 // so the positions are the whole walker record that has to move.
-__global__ void k_gather(DevWalk W, int rec)
+__global__ void k_gather(DevWalk W, int rec, int mocn)
 {
     const size_t total = (size_t)W.n_w * rec;
     for (size_t idx = blockIdx.x * (size_t)blockDim.x + threadIdx.x; idx < total; idx += (size_t)gridDim.x * blockDim.x) {
         int k = (int)(idx / rec), c = (int)(idx - (size_t)k * rec);
         W.r_alt[idx] = W.r[(size_t)W.parents[k] * rec + c];
         if (c == 0) W.w[k] = 1.0;
+    }
+    // cached MO rows: functions of the electron positions alone, so the parent's rows are the child's, bit for bit (HBM-bound copy)
+    const int m2 = mocn >> 1;                                       // mocn = 5 N OS is even; rows are 16-byte aligned
+    const size_t total2 = (size_t)W.n_w * m2;
+    const double2 *src = reinterpret_cast<const double2 *>(W.moc); double2 *dst = reinterpret_cast<double2 *>(W.moc_alt);
+    for (size_t idx = blockIdx.x * (size_t)blockDim.x + threadIdx.x; idx < total2; idx += (size_t)gridDim.x * blockDim.x) {
+        int k = (int)(idx / m2), c = (int)(idx - (size_t)k * m2);
+        dst[idx] = src[(size_t)W.parents[k] * m2 + c];
     }
 }
 

@@ -224,8 +224,9 @@ __device__ __forceinline__ void ao_columns(const DevSys &S, const double *__rest
 #define LRDMC_EXPS                                                                              \
         const double zq0 = -z * q0; const bool far_ = zq0 < 0.5 * LRDMC_EXP_XMIN;   /* |2 z sk| <= z q0: the six arguments lie in [2 zq, 0] */ \
         const double zq = far_ ? 0.5 * LRDMC_EXP_XMIN : zq0, tz = far_ ? 0.0 : -2.0 * z;        \
-        double e[6];                                                                            \
-        _Pragma("unroll") for (int k = 0; k < 3; ++k) { e[2 * k] = exp_tab(fma(tz, sk[k], zq), etab); e[2 * k + 1] = exp_tab(fma(-tz, sk[k], zq), etab); }
+        double ex_[6], e[6];                                                                    \
+        _Pragma("unroll") for (int k = 0; k < 3; ++k) { ex_[2 * k] = fma(tz, sk[k], zq); ex_[2 * k + 1] = fma(-tz, sk[k], zq); } \
+        exp_tab_n<6>(ex_, e, etab);
     for (int it = 0; it < S.n_it[0]; ++it, sh4 += 4) {            // Slater s: exp(-z r)
         LRDMC_GEOM
         double bc; LRDMC_BCOL(bc)
@@ -312,8 +313,9 @@ __device__ __forceinline__ void ao_columns(const DevSys &S, const double *__rest
 #define LRDMC_EXPS                                                                              \
         const double zq0 = -z * q0; const bool far_ = zq0 < 0.5 * LRDMC_EXP_XMIN;   /* |2 z sk| <= z q0: the six arguments lie in [2 zq, 0] */ \
         const double zq = far_ ? 0.5 * LRDMC_EXP_XMIN : zq0, tz = far_ ? 0.0 : -2.0 * z;        \
-        double e[6];                                                                            \
-        _Pragma("unroll") for (int k = 0; k < 3; ++k) { e[2 * k] = exp_tab(fma(tz, sk[k], zq), etab); e[2 * k + 1] = exp_tab(fma(-tz, sk[k], zq), etab); }
+        double ex_[6], e[6];                                                                    \
+        _Pragma("unroll") for (int k = 0; k < 3; ++k) { ex_[2 * k] = fma(tz, sk[k], zq); ex_[2 * k + 1] = fma(-tz, sk[k], zq); } \
+        exp_tab_n<6>(ex_, e, etab);
     auto slater_body = [&](double bc) {              // Slater s: exp(-z r)
         LRDMC_GEOM
 #pragma unroll
