@@ -180,7 +180,7 @@ def main():
         pass
     roofline = {"bound": "alu", "kernel": "k_propagate", "achieved": achieved, "peak": peaks["dfma_tflops"], "unit": "TFLOP/s", "frac": achieved / peaks["dfma_tflops"],
                 "traffic": traffic, "peak_source": "measured live: lrdmc_measure_fp64_peaks (independent DFMA chains, all SMs)",
-                "dmma_peak": peaks["dmma_tflops"], "dfma_dmma_mixed": peaks["mixed_tflops"], "dfma_3reg_peak": peaks["dfma_3reg_tflops"], "flop_per_walker_move": flop["total"],
+                "dmma_peak": peaks["dmma_tflops"], "dfma_dmma_mixed": peaks["mixed_tflops"], "dfma_3reg_peak": peaks["dfma_3reg_tflops"], "dfma_with_2_alu_peak": peaks["dfma_alu_tflops"], "flop_per_walker_move": flop["total"],
                 "kernel_ms": prop_ms, "kernel_share_of_step": prop_ms * len(recs) / (secs * 1e3),
                 "hbm_bytes_per_launch_algorithmic": 2 * drv.state_bytes_per_walker(sysd) * args.nw}
 

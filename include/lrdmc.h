@@ -141,9 +141,11 @@ int lrdmc_run_host(lrdmc_ctx *, const double *r_in_host, double *r_out_host, int
 /* Roofline denominators measured on this device ("measure DFMA and DMMA peaks on the box"):
  * TFLOP/s of independent FP64 FMA chains, of mma.sync m8n8k4 f64 chains, and of both issued together. Host outputs. */
 int lrdmc_measure_fp64_peaks(double *dfma_tflops, double *dmma_tflops, double *mixed_tflops);
-/* Same, for FMAs whose three source operands are three different registers (no reuse-cache hit, no constant operand):
- * the register-file-bound rate, 2/3 of dfma_tflops on B200.  Host output. */
-int lrdmc_measure_fp64_operand_peak(double *dfma_3reg_tflops);
+/* Same, for the two instruction forms that set the real ceiling of the path (dispatch model):
+ * dfma_3reg_tflops -- FMAs whose three source operands are three different registers (3 dispatch cycles instead of 2);
+ * dfma_alu_tflops  -- two-register FMAs each followed by two independent integer ALU instructions of the same warp
+ *                     (FP64 flop only; 1/2 of dfma_tflops when nothing overlaps).  Host outputs; the second may be NULL. */
+int lrdmc_measure_fp64_operand_peak(double *dfma_3reg_tflops, double *dfma_alu_tflops);
 
 /* Test hook for pin P11: fills out_dev [n][4] (uint32) with Philox4x32-10 blocks for counters ctr_dev [n][4], key[2]. */
 int lrdmc_debug_philox(const uint32_t *ctr_dev, uint32_t key0, uint32_t key1, uint32_t *out_dev, int n, void *stream);

@@ -80,7 +80,7 @@ def load_library():
         L.lrdmc_get_obs.argtypes = [vp, vp, vp, vp, vp, vp]
         L.lrdmc_run_host.argtypes = [vp, vp, vp, i32, i32, dbl, dbl, u64, i32, C.POINTER(CycleStats), vp]
         L.lrdmc_measure_fp64_peaks.argtypes = [C.POINTER(dbl), C.POINTER(dbl), C.POINTER(dbl)]
-        L.lrdmc_measure_fp64_operand_peak.argtypes = [C.POINTER(dbl)]
+        L.lrdmc_measure_fp64_operand_peak.argtypes = [C.POINTER(dbl), C.POINTER(dbl)]
         L.lrdmc_debug_philox.argtypes = [vp, C.c_uint32, C.c_uint32, vp, i32, vp]
         L.lrdmc_debug_draws.argtypes = [vp, u64, u64, vp, i32, vp]
         L.lrdmc_launch_count.argtypes = [vp]
@@ -116,9 +116,9 @@ def lrdmc_energy(records, p=10, n_therm=0, n_blocks=20):
 def lrdmc_measure_fp64_peaks():
     a, b, m = C.c_double(), C.c_double(), C.c_double()
     _check(load_library().lrdmc_measure_fp64_peaks(C.byref(a), C.byref(b), C.byref(m)), "lrdmc_measure_fp64_peaks")
-    t = C.c_double()
-    _check(load_library().lrdmc_measure_fp64_operand_peak(C.byref(t)), "lrdmc_measure_fp64_operand_peak")
-    return dict(dfma_tflops=a.value, dmma_tflops=b.value, mixed_tflops=m.value, dfma_3reg_tflops=t.value)
+    t, u = C.c_double(), C.c_double()
+    _check(load_library().lrdmc_measure_fp64_operand_peak(C.byref(t), C.byref(u)), "lrdmc_measure_fp64_operand_peak")
+    return dict(dfma_tflops=a.value, dmma_tflops=b.value, mixed_tflops=m.value, dfma_3reg_tflops=t.value, dfma_alu_tflops=u.value)
 
 
 class Lrdmc:

@@ -79,7 +79,10 @@ __device__ __forceinline__ void exp_tab_n(const double (&x)[NX], double (&out)[N
 #pragma unroll
     for (int i = 0; i < NX; ++i) { k[i] = __double2loint(t[i]); asm("and.b32 %0, %1, 255;" : "=r"(j[i]) : "r"(k[i])); }
 #pragma unroll
-    for (int i = 0; i < NX; ++i) asm("ld.shared.f64 %0, [%1];" : "=d"(tv[i]) : "r"(base + 8u * (unsigned)j[i]));
+    for (int i = 0; i < NX; ++i) asm volatile("ld.shared.f64 %0, [%1];" : "=d"(tv[i]) : "r"(base + 8u * (unsigned)j[i]) : "memory");
+#ifndef LRDMC_NO_EXP_FENCE
+    __syncwarp();            // scheduling fence: ptxas otherwise sinks each table load to just before its use (29-cycle LDS latency exposed per exponential)
+#endif
 #pragma unroll
     for (int i = 0; i < NX; ++i) t[i] -= magic;
 #pragma unroll

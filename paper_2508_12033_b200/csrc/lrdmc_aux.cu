@@ -106,24 +106,29 @@ extern "C" int lrdmc_measure_fp64_peaks(double *dfma, double *dmma, double *mixe
     return LRDMC_OK;
 }
 
-extern "C" int lrdmc_measure_fp64_operand_peak(double *dfma3)
+extern "C" int lrdmc_measure_fp64_operand_peak(double *dfma3, double *dfma_alu)
 {
     int dev = 0; cudaDeviceProp prop;
     if (!dfma3 || cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return LRDMC_ECUDA;
     const int blocks = prop.multiProcessorCount * 8, threads = 256, iters = 8192;
     double *d_out = NULL; if (cudaMalloc((void **)&d_out, sizeof(double) * blocks * threads) != cudaSuccess) return LRDMC_ECUDA;
     cudaEvent_t e0, e1; cudaEventCreate(&e0); cudaEventCreate(&e1);
-    float best = 1e30f;
-    for (int rep = 0; rep < 5; ++rep) {
-        cudaEventRecord(e0);
-        k_fp64_peak_3reg<<<blocks, threads>>>(d_out, iters, 1.000001);
-        cudaEventRecord(e1); cudaEventSynchronize(e1);
-        float ms = 0; cudaEventElapsedTime(&ms, e0, e1);
-        if (rep > 0 && ms < best) best = ms;
+    double res[2] = { 0, 0 };
+    for (int mode = 0; mode < 2; ++mode) {
+        float best = 1e30f;
+        for (int rep = 0; rep < 5; ++rep) {
+            cudaEventRecord(e0);
+            if (mode == 0) k_fp64_peak_3reg<<<blocks, threads>>>(d_out, iters, 1.000001);
+            else k_fp64_peak_alu<<<blocks, threads>>>(d_out, iters, 1.000001);
+            cudaEventRecord(e1); cudaEventSynchronize(e1);
+            float ms = 0; cudaEventElapsedTime(&ms, e0, e1);
+            if (rep > 0 && ms < best) best = ms;
+        }
+        res[mode] = (double)blocks * threads * iters * 8.0 * 2.0 / (best * 1e-3) / 1e12;      // FP64 flop only
     }
     cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d_out);
     if (cudaGetLastError() != cudaSuccess) return LRDMC_ECUDA;
-    *dfma3 = (double)blocks * threads * iters * 8.0 * 2.0 / (best * 1e-3) / 1e12;
+    *dfma3 = res[0]; if (dfma_alu) *dfma_alu = res[1];
     return LRDMC_OK;
 }
 

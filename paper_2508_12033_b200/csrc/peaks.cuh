@@ -41,3 +41,22 @@ static __global__ void __launch_bounds__(256) k_fp64_peak_3reg(double *out, int 
     for (int i = 0; i < 8; ++i) s += f[i];
     if (s == 123.456) out[blockIdx.x * blockDim.x + threadIdx.x] = s;
 }
+
+// DFMA (two register operands + a constant: 2 dispatch cycles) interleaved with independent integer ALU work of the same
+// warp (an and and an add per DFMA with run-time operands, which the compiler cannot fold): does the other work hide in the FP64 instruction's
+// second cycle?  On B200 it does not: the time is the SUM of the dispatch cycles (2 + 1 + 1), see DESIGN.md section 4.
+static __global__ void __launch_bounds__(256) k_fp64_peak_alu(double *out, int iters, double seed)
+{
+    double f[8]; unsigned y[8]; const unsigned m = 0xfff0ff0fu ^ (unsigned)iters, c = 0x9e3779b9u + (unsigned)iters;
+    const double a = seed + threadIdx.x * 1e-9, b = 1.0 - 1e-7;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) { f[i] = seed * (i + 1); y[i] = threadIdx.x * 2654435761u + i; }
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int i = 0; i < 8; ++i) { f[i] = fma(f[i], b, a); y[i] = (y[i] & m) + c; }
+    }
+    double s = 0.0; unsigned t = 0;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) { s += f[i]; t += y[i]; }
+    if (s == 123.456 || t == 77u) out[blockIdx.x * blockDim.x + threadIdx.x] = s + t;
+}
