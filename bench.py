@@ -113,6 +113,8 @@ def main():
     ap.add_argument("--impl", default="ours"); ap.add_argument("--nw", type=int, default=25600); ap.add_argument("--moves", type=int, default=100)
     ap.add_argument("--ref-nw", type=int, default=64); ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-conventional", action="store_true"); ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--workload", default="C4", choices=["C2", "C4", "C5"],
+                    help="C4 (default) is the configuration the metric is quoted on; C2 / C5 are the other BASELINE.json systems (use with --nw/--moves)")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1")); local = int(os.environ.get("LOCAL_RANK", "0"))
     if args.impl == "reference":
@@ -129,7 +131,15 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
     dev = f"cuda:{local}"; torch.cuda.set_device(dev)
 
-    sysd = wl.water_methane(n_walkers=args.nw, moves=args.moves, seed=wl.PHILOX_RUN_SEED + rank, name="C4-water-methane-shaped")
+    if args.workload == "C4":
+        sysd = wl.water_methane(n_walkers=args.nw, moves=args.moves, seed=wl.PHILOX_RUN_SEED + rank, name="C4-water-methane-shaped")
+        wname = "C4 water-methane-shaped: 16 e (8/8), 8 nuclei, 200 s/p/d GTOs, local PP, 1b+2b Jastrow, a=0.2 (BASELINE.json configs[3])"
+    elif args.workload == "C2":
+        sysd = wl.synthetic10(n_walkers=args.nw, moves=args.moves, seed=wl.PHILOX_RUN_SEED + rank)
+        wname = "C2 synthetic 10-electron molecule: 5/5, 3 nuclei, 60 s/p/d GTOs, 1b+2b Jastrow, a=0.2 (BASELINE.json configs[1])"
+    else:
+        sysd = wl.cluster64(n_walkers=args.nw, moves=args.moves, seed=wl.PHILOX_RUN_SEED + rank)
+        wname = "C5 64-electron cluster: 32/32, 24 nuclei, 600 s/p/d GTOs, 1b+2b Jastrow, double mesh a=0.2/a'=0.4 (BASELINE.json configs[4])"
     x0 = wl.initial_walkers(sysd, args.nw, 5 + rank)
     g = B.Lrdmc(sysd, device=dev)
     g.lrdmc_set_positions(x0, allow_singular=True)
@@ -186,7 +196,7 @@ def main():
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tmax / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": "C4 water-methane-shaped: 16 e (8/8), 8 nuclei, 200 s/p/d GTOs, local PP, 1b+2b Jastrow, a=0.2 (BASELINE.json configs[3])",
+            "config": {"workload": wname,
                        "n_walkers": args.nw, "moves_per_cycle": args.moves, "mode": "balanced", "parallelism": f"replicas x{world}",
                        "l2": "inputs larger than L2: walker state %.0f MB per replica" % (drv.state_bytes_per_walker(sysd) * args.nw / 1e6),
                        "launch": g.launch_config()},
@@ -224,9 +234,10 @@ def main():
     line["clocks"] = clk.summary()
 
     if rank == 0 and not args.no_cpu_baseline and world == 1:
-        v, cores, dt, n = oracle_sample(wl.water_methane(n_walkers=args.ref_nw), args.ref_nw, 2, args.moves, min_seconds=12.0)
+        ref_sys = sysd if args.workload != "C4" else wl.water_methane(n_walkers=args.ref_nw)
+        v, cores, dt, n = oracle_sample(ref_sys, args.ref_nw, 2, args.moves, min_seconds=12.0)
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
-                                "sample": f"same C4 system, N_w={args.ref_nw} walkers x {n // (args.ref_nw * args.moves)} cycles x {args.moves} moves ({n} walker-moves, {dt:.1f} s), balanced, incl. reconfiguration"}
+                                "sample": f"same {args.workload} system, N_w={args.ref_nw} walkers x {n // (args.ref_nw * args.moves)} cycles x {args.moves} moves ({n} walker-moves, {dt:.1f} s), balanced, incl. reconfiguration"}
     if rank == 0:
         print(json.dumps(line), flush=True)
     g.close()

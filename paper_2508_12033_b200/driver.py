@@ -39,3 +39,43 @@ def run(g: "B.Lrdmc", mode, cycles, n_moves=0, tau=0.0, E0=0.0, first_cycle=0, f
         if mode == B.BALANCED and feedback:
             E0 = esum / len(recs)
     return recs
+
+
+# ---- a -> 0 driver ("extrapolated to a -> 0", Table I L254-L265 shape) -----------------
+def fit_a_to_zero(a_list, energies, sigmas, n_terms=2):
+    """Weighted least squares of E(a) = E_0 + c_2 a^2 (+ c_4 a^4 for n_terms = 3): the lattice bias is even in a (L23, L140).
+    Returns (E_0, sigma(E_0), coefficients, chi2).  Host arithmetic on a handful of numbers; no device work."""
+    import numpy as np
+    a = np.asarray(a_list, float); E = np.asarray(energies, float); s = np.asarray(sigmas, float)
+    if not (len(a) == len(E) == len(s)) or len(a) < n_terms or np.any(s <= 0):
+        raise ValueError("need at least n_terms points with positive error bars")
+    X = np.stack([a ** (2 * k) for k in range(n_terms)], axis=1) / s[:, None]
+    cov = np.linalg.inv(X.T @ X)
+    coef = cov @ (X.T @ (E / s))
+    chi2 = float(np.sum((X @ coef - E / s) ** 2))
+    return float(coef[0]), float(np.sqrt(cov[0, 0])), coef, chi2
+
+
+def a_scan(make_system, make_walkers, a_list, n_walkers, cycles, moves, modes=("balanced", "conventional"), E0=0.0, n_therm=None,
+           p=10, n_blocks=10, device="cuda:0"):
+    """One LRDMC run per lattice spacing and mode on the CUDA path; rows shaped like Table I (a, E_balanced, E_conventional).
+    make_system(a) -> system dict; make_walkers(system, n_walkers) -> positions.  Conventional mode uses the projection time with
+    the same mean move count, tau = moves a^2 / (3N) (reading Q19)."""
+    rows = []
+    for a in a_list:
+        sysd = make_system(a); N = sysd["n_up"] + sysd["n_dn"]
+        row = {"a": a}
+        for mode in modes:
+            g = B.Lrdmc(sysd, device=device)
+            g.lrdmc_set_positions(make_walkers(sysd, n_walkers))
+            if mode == "balanced":
+                recs = run(g, B.BALANCED, cycles, n_moves=moves, E0=E0)
+            else:
+                recs = run(g, B.CONVENTIONAL, cycles, tau=moves * a * a / (3 * N), E0=E0)
+            row[mode] = B.lrdmc_energy(recs, p=p, n_therm=cycles // 5 if n_therm is None else n_therm, n_blocks=n_blocks)
+            g.close()
+        rows.append(row)
+    out = {"rows": rows}
+    for mode in modes:
+        out[mode] = fit_a_to_zero([r["a"] for r in rows], [r[mode][0] for r in rows], [r[mode][1] for r in rows])
+    return out

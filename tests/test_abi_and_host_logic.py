@@ -79,6 +79,22 @@ def test_algorithmic_work_count_matches_survey_table():
     assert drv.state_bytes_per_walker(wl.water_methane()) == 8 * (48 + 128 + 640)
 
 
+def test_a_to_zero_fit_closed_forms():
+    """f3 host logic: two points reduce to the textbook Richardson formula with its error propagation; exact data are recovered."""
+    from paper_2508_12033_b200 import driver as drv
+    a1, a2, E1, E2, s1, s2 = 0.2, 0.4, -0.49, -0.46, 1e-3, 2e-3
+    E0, sg, coef, chi2 = drv.fit_a_to_zero([a1, a2], [E1, E2], [s1, s2])
+    d = a2**2 - a1**2
+    assert abs(E0 - (E1 * a2**2 - E2 * a1**2) / d) < 1e-14 and abs(sg - np.hypot(s1 * a2**2, s2 * a1**2) / d) < 1e-14 and chi2 < 1e-20
+    a = np.array([0.1, 0.2, 0.3, 0.4]); E = -0.5 + 0.07 * a**2 - 0.3 * a**4
+    E0, sg, coef, chi2 = drv.fit_a_to_zero(a, E, np.full(4, 1e-4), n_terms=3)
+    assert abs(E0 + 0.5) < 1e-12 and abs(coef[1] - 0.07) < 1e-10 and abs(coef[2] + 0.3) < 1e-9
+    E0, sg, *_ = drv.fit_a_to_zero(a, E, np.full(4, 1e-4), n_terms=2)      # a^4 term left out: biased, and chi2 says so
+    assert abs(E0 + 0.5) > 3 * sg
+    with pytest.raises(ValueError):
+        drv.fit_a_to_zero([0.1], [0.0], [1.0])
+
+
 def test_workload_generators_are_seeded_and_shaped():
     a, b = wl.water_methane(), wl.water_methane()
     assert np.array_equal(a["C_up"], b["C_up"]) and np.array_equal(a["R"], b["R"]) and a["n_ao"] == 200 and a["n_shell"] == 60

@@ -245,6 +245,63 @@ def test_hydrogen_run_energy_matches_oracle_and_exact(B):
     g.close()
 
 
+def test_a_to_zero_scan_balanced_vs_conventional_table_shape(B):
+    """SURVEY 8(f) f3, the shape of Table I (L254-L265): at every a the two modes agree within 3 combined sigma, and both
+    E(a) extrapolate to the exact -1/2 Ha of the hydrogen atom (L23, L140) -- on the CUDA path, 2048 walkers."""
+    from paper_2508_12033_b200 import driver as drv
+    out = drv.a_scan(lambda a: wl.hydrogen(alpha=0.9, a=a), lambda s, n: wl.hydrogen_walkers(n, 1), [0.15, 0.25, 0.35, 0.45],
+                     n_walkers=2048, cycles=150, moves=30, E0=-0.5)
+    for r in out["rows"]:
+        (Eb, sb), (Ec, sc) = r["balanced"], r["conventional"]
+        assert abs(Eb - Ec) < 3 * np.hypot(sb, sc) + 2e-4, r
+        assert Eb < -0.495 + 3 * sb                                                       # below the variational energy
+    for mode in ("balanced", "conventional"):
+        E0, s0, coef, chi2 = out[mode]
+        assert abs(E0 + 0.5) < 3 * s0 + 2e-4 and s0 < 1e-3, (mode, E0, s0)
+
+
+def test_helium_energies_on_the_cuda_path(B):
+    """Pins P7/P8 through the CUDA path: nodeless He 1S -> -2.903724 Ha as a -> 0; He 2 3S with its exact node -> -2.175229 Ha."""
+    from paper_2508_12033_b200 import driver as drv
+    rng = np.random.default_rng(0); a = [0.15, 0.25, 0.35]; E = []; sg = []
+    for ai in a:
+        s = wl.slater_atom(2.0, [1.85], 1, 1, np.ones((1, 1)), np.ones((1, 1)), ai, jastrow=dict(a_anti=0.5, a_par=0.25, b2=0.5))
+        g = B.Lrdmc(s); g.lrdmc_set_positions(rng.normal(size=(4096, 2, 3)) * 0.7)
+        recs = drv.run(g, B.BALANCED, 300, n_moves=int(round(20 * (0.2 / ai) ** 2)), E0=-2.9)
+        e, sd = B.lrdmc_energy(recs, p=10, n_therm=60, n_blocks=10); E.append(e); sg.append(sd); g.close()
+    E0, s0, *_ = drv.fit_a_to_zero(a, E, sg)
+    assert abs(E0 + 2.903724) < 3 * s0 + 3e-4 and s0 < 2e-3, (E0, s0)
+    s = wl.slater_atom(2.0, [2.0, 0.6], 2, 0, np.eye(2), np.zeros((2, 0)), 0.2, jastrow=dict(a_par=0.25, a_anti=0.5, b2=0.5))
+    x = rng.normal(size=(4096, 2, 3)); x[:, 0] *= 0.4; x[:, 1] *= 2.0
+    g = B.Lrdmc(s); g.lrdmc_set_positions(x)
+    recs = drv.run(g, B.BALANCED, 400, n_moves=30, E0=-2.17)
+    Et, st = B.lrdmc_energy(recs, p=10, n_therm=80, n_blocks=10)
+    assert sum(r.n_node_flag for r in recs) > 0 and sum(r.n_nonpos_diag for r in recs) == 0
+    assert abs(Et + 2.175229) < 3 * st + 5e-4 and st < 1e-3, (Et, st)
+    g.close()
+
+
+def test_balanced_equals_conventional_on_the_synthetic_molecule(B):
+    """Pin P12 on config C2 (10 electrons, s/p/d GTOs, Jastrow, nodes): the two modes sample the same fixed-node state (L234, L244)."""
+    from paper_2508_12033_b200 import driver as drv
+    s = wl.synthetic10(); x0 = wl.initial_walkers(s, 4096, 5); N = 10
+    g = B.Lrdmc(s); g.lrdmc_set_positions(x0, allow_singular=True)
+    pilot = drv.run(g, B.BALANCED, 30, n_moves=50, E0=0.0, feedback=False)
+    Eref = float(np.mean([r.num / r.den for r in pilot[10:]]))
+    # the balanced Green's function projects onto the ground state only for E_0 = E (Eq.28 L190, "E_0 is updated after each
+    # branching step" L232): run it with the feedback of Alg.2 line 12, first a thermalising leg, then the measured one
+    rt = drv.run(g, B.BALANCED, 60, n_moves=50, E0=Eref, first_cycle=100)
+    rb = drv.run(g, B.BALANCED, 200, n_moves=50, E0=float(np.mean([r.num / r.den for r in rt[20:]])), first_cycle=200)
+    Eb, sb = B.lrdmc_energy(rb, p=5, n_therm=30, n_blocks=10)
+    rc = drv.run(g, B.CONVENTIONAL, 260, tau=50 * s["a"]**2 / (3 * N), E0=Eref, first_cycle=1000)
+    Ec, sc = B.lrdmc_energy(rc, p=5, n_therm=90, n_blocks=10)
+    mean_moves = np.mean([r.moves_sum for r in rc]) / 4096
+    assert 35 < mean_moves < 65
+    assert sum(r.n_nonfinite for r in rb + rc) == 0
+    assert abs(Eb - Ec) < 3 * np.hypot(sb, sc), (Eb, sb, Ec, sc)
+    g.close()
+
+
 # ------------------------------------------------------------------------------------------ edge cases and error behaviour
 def test_edge_cases_and_errors(B):
     s = wl.tiny_molecule(2, 1, 2, 6, seed=7); g = B.Lrdmc(s)
