@@ -52,6 +52,25 @@ struct DevSys {
     int dinv_rows[2];     // padded row count 8*NT
 };
 
+// ---- team mode (team.cuh): one CTA of TW warps works on ONE walker --------------------------------------------------
+// A shell part = per shell group [lo, hi) ranges of 4-shell iterations of the sorted, padded shell list.
+struct ShellPart { int lo[4], hi[4]; };
+#define LRDMC_TEAM_MAX_WARPS 16
+#define LRDMC_TEAM_MAX_PARTS 8
+struct TeamPlan {
+    int TW;               // warps per walker (= blockDim.x / 32)
+    int NP;               // shell parts of the candidate pass (work units = electron blocks x NP)
+    int lpe;              // lanes per electron in phase A (power of two, 2..32)
+    int nblk[2];          // 8-electron blocks per spin
+    int n_units;          // n_mesh (nblk[0] + nblk[1]) NP
+    int it_base[4];       // first 4-shell iteration of each shell group
+    int kstep_base[4];    // first mma k-step of each group in the `bf` fragment table
+    int pair_base[4];     // first k-step pair of each group in the `cf` fragment table
+    int o_scr, scr_doubles; // scratch (partial sums) behind the walker state, in doubles from the state base
+    ShellPart col[LRDMC_TEAM_MAX_PARTS];     // parts of ao_columns (groups 0-2 start on even iterations: k-step pairs)
+    ShellPart mo[LRDMC_TEAM_MAX_WARPS];      // parts of the derivative pass of the mover (one per warp)
+};
+
 // Table pointers as a kernel sees them (shared memory, or global memory for the fragments of the largest systems)
 struct Tables { const double *shells, *nuc, *bf[2], *cf[2], *etab; };
 

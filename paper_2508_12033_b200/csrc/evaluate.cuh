@@ -57,6 +57,52 @@ __device__ __forceinline__ void pade_six(double dx, double dy, double dz, const 
     }
 }
 
+// Phase C (row a7) of one evaluation, by one warp on the candidate ratios R[P] left in shared memory.
+__device__ __forceinline__ EvalOut phase_c(const DevSys &S, const WarpState &ws, const double *lap_s, double Vee, int lane)
+{
+    const int N = S.N;
+    // ---- phase C (row a7): fixed-node split (Eq.D1) and the cumulative sums C_j of the allowed amplitudes in candidate
+    //      order (row a9 searches them).  Each lane owns a contiguous chunk; chunk totals are scanned across the warp
+    //      (reading Q12: the summation order is free, a draw closer than 1e-9 to a bin edge is a reported near-tie).
+    const int P = S.P, chunk = (P + 31) >> 5, j0 = lane * chunk;
+    double vsf_part = 0.0, loc = 0.0; int node = 0;
+    for (int e = 0; e < chunk; ++e) {
+        const int j = j0 + e;
+        if (j < P) {
+            const double Rj = ws.R[j], kap = S.kappa[j >= 6 * N ? 1 : 0];
+            if (Rj > 0.0) loc += kap * Rj;
+            else if (Rj < 0.0) { vsf_part -= kap * Rj; node = 1; }
+            ws.cum[j] = loc;
+        }
+    }
+    double inc = loc;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const double v = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += v; }
+    double excl = __shfl_up_sync(0xffffffffu, inc, 1); if (lane == 0) excl = 0.0;
+    for (int e = 0; e < chunk; ++e) { const int j = j0 + e; if (j < P) ws.cum[j] += excl; }
+    const double bbar = __shfl_sync(0xffffffffu, inc, 31);
+    const double Vsf = warp_sum(vsf_part);
+    node = __any_sync(0xffffffffu, node);
+    double vsum = 0.0;
+    for (int i = lane; i < N; i += 32) {
+        double T = 0.0;
+        for (int mesh = 0; mesh < S.n_mesh; ++mesh) {
+            const double *Rm = ws.R + mesh * 6 * N + 6 * i;
+            double s = Rm[0]; s += Rm[1]; s += Rm[2]; s += Rm[3]; s += Rm[4]; s += Rm[5];
+            T += S.g_over_a2[mesh] * (s - 6.0);                      // discretised Laplacian of Eq.D3 over Psi_G
+        }
+        const double *ob = ws.ob + 8 * i;
+        const double vzv = ob[5] + 0.5 * (T - lap_s[i]);              // Eq.D8
+        vsum += node ? fmax(vzv, ob[6]) : vzv;                        // Eq.D9 / D11 (reading Q5: global node flag)
+    }
+    vsum = warp_sum(vsum);
+    EvalOut o;
+    o.bbar = bbar; o.Vsf = Vsf; o.node = node;
+    o.W = S.Kdiag + vsum + Vee + S.V_ii + Vsf;                        // L628 + kinetic diagonal of Eq.D5 (reading Q3)
+    o.eL = o.W - bbar;                                                // L223
+    return o;
+}
+
 template <int NT, bool TS, int NB>
 __device__ __forceinline__ EvalOut evaluate_walker(const DevSys &S, const WarpState &ws, const Tables &T, int lane)
 {
@@ -204,45 +250,7 @@ __device__ __forceinline__ EvalOut evaluate_walker(const DevSys &S, const WarpSt
 #endif
     __syncwarp();
 
-    // ---- phase C (row a7): fixed-node split (Eq.D1) and the cumulative sums C_j of the allowed amplitudes in candidate
-    //      order (row a9 searches them).  Each lane owns a contiguous chunk; chunk totals are scanned across the warp
-    //      (reading Q12: the summation order is free, a draw closer than 1e-9 to a bin edge is a reported near-tie).
-    const int P = S.P, chunk = (P + 31) >> 5, j0 = lane * chunk;
-    double vsf_part = 0.0, loc = 0.0; int node = 0;
-    for (int e = 0; e < chunk; ++e) {
-        const int j = j0 + e;
-        if (j < P) {
-            const double Rj = ws.R[j], kap = S.kappa[j >= 6 * N ? 1 : 0];
-            if (Rj > 0.0) loc += kap * Rj;
-            else if (Rj < 0.0) { vsf_part -= kap * Rj; node = 1; }
-            ws.cum[j] = loc;
-        }
-    }
-    double inc = loc;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) { const double v = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += v; }
-    double excl = __shfl_up_sync(0xffffffffu, inc, 1); if (lane == 0) excl = 0.0;
-    for (int e = 0; e < chunk; ++e) { const int j = j0 + e; if (j < P) ws.cum[j] += excl; }
-    const double bbar = __shfl_sync(0xffffffffu, inc, 31);
-    const double Vsf = warp_sum(vsf_part);
-    node = __any_sync(0xffffffffu, node);
-    double vsum = 0.0;
-    for (int i = lane; i < N; i += 32) {
-        double T = 0.0;
-        for (int mesh = 0; mesh < S.n_mesh; ++mesh) {
-            const double *Rm = ws.R + mesh * 6 * N + 6 * i;
-            double s = Rm[0]; s += Rm[1]; s += Rm[2]; s += Rm[3]; s += Rm[4]; s += Rm[5];
-            T += S.g_over_a2[mesh] * (s - 6.0);                      // discretised Laplacian of Eq.D3 over Psi_G
-        }
-        const double *ob = ws.ob + 8 * i;
-        const double vzv = ob[5] + 0.5 * (T - lap_s[i]);              // Eq.D8
-        vsum += node ? fmax(vzv, ob[6]) : vzv;                        // Eq.D9 / D11 (reading Q5: global node flag)
-    }
-    vsum = warp_sum(vsum);
-    EvalOut o;
-    o.bbar = bbar; o.Vsf = Vsf; o.node = node;
-    o.W = S.Kdiag + vsum + Vee + S.V_ii + Vsf;                        // L628 + kinetic diagonal of Eq.D5 (reading Q3)
-    o.eL = o.W - bbar;                                                // L223
+    const EvalOut o = phase_c(S, ws, lap_s, Vee, lane);
     __syncwarp();
     return o;
 }

@@ -12,6 +12,7 @@
 #include "wavefunction.cuh"
 #include "evaluate.cuh"
 #include "propagate.cuh"
+#include "team.cuh"
 #include "reconfigure.cuh"
 #include "peaks.cuh"
 #include "api_internal.h"
@@ -26,6 +27,8 @@ struct lrdmc_ctx {
     int bound, have_prop, have_reconf, state_ok;
     cudaEvent_t ev[4]; cudaStream_t last_stream;
     int launches;   // kernels launched so far (bench.py reports it)
+    // team mode (team.cuh): chosen at lrdmc_bind_walkers from N_w and the footprint; team_tw == 1 -> warp-per-walker kernel
+    TeamPlan team; int team_tw, team_smem, team_ctas_per_sm, team_grid_max, pair_base[5];
 };
 
 extern "C" const char *lrdmc_strerror(int code)
@@ -130,6 +133,7 @@ extern "C" int lrdmc_init(lrdmc_ctx **out, const lrdmc_system *sys, const lrdmc_
     int pair_base[5]; pair_base[0] = 0;
     for (int g = 0; g < 4; ++g) pair_base[g + 1] = pair_base[g] + (ncomp[g] * S.n_it[g] + 1) / 2;
     S.n_kpairs = pair_base[4];
+    for (int g = 0; g < 5; ++g) c->pair_base[g] = pair_base[g];
     const int NA = 2 * c->NT;
     const size_t cf_n = LRDMC_BC_DMMA ? (size_t)S.n_kpairs * NA * 32 : 0;
     std::vector<double> h_cf[2];
@@ -245,7 +249,7 @@ static size_t carve(const lrdmc_ctx *c, int n_w, char *base, DevWalk *W)
     TAKE(w, double, nw); TAKE(eL, double, nw); TAKE(W, double, nw); TAKE(omega, double, nw);
     TAKE(nmoves, long long, nw); TAKE(flags, int, nw * 3);
     TAKE(wq, unsigned long long, nw); TAKE(prefix, unsigned long long, nw); TAKE(parents, int, nw);
-    TAKE(timing, unsigned long long, 2 * (size_t)c->grid_max * c->wpb); TAKE(counter, int, 64);
+    TAKE(timing, unsigned long long, 2 * (size_t)(c->grid_max * c->wpb > c->sm_count * 32 ? c->grid_max * c->wpb : c->sm_count * 32)); TAKE(counter, int, 64);
 #undef TAKE
     return o;
 }
@@ -256,12 +260,90 @@ extern "C" size_t lrdmc_walker_bytes(const lrdmc_ctx *c, int n_walkers)
     return carve(c, n_walkers, NULL, NULL) + 256;
 }
 
+// ---- team mode planning (team.cuh) ----------------------------------------------------------------------------------
+// Cut the sorted shell list into K parts of about equal cost.  Unit = two 4-shell iterations in groups 0-2 when `pairs`
+// (a part of ao_columns must start on a k-step pair), else one iteration; units go to parts by their cumulative cost.
+static void partition_shells(const int n_it[4], const double cost[4], bool pairs, int K, ShellPart *out)
+{
+    struct Unit { int g, lo, hi; double c; };
+    std::vector<Unit> units; double total = 0.0;
+    for (int g = 0; g < 4; ++g) {
+        const int stepu = (pairs && g < 3) ? 2 : 1;
+        for (int it = 0; it < n_it[g]; it += stepu) {
+            const int hi = it + stepu < n_it[g] ? it + stepu : n_it[g];
+            units.push_back({ g, it, hi, cost[g] * (hi - it) }); total += cost[g] * (hi - it);
+        }
+    }
+    for (int k = 0; k < K; ++k) for (int g = 0; g < 4; ++g) out[k].lo[g] = out[k].hi[g] = 0;
+    double cum = 0.0;
+    for (const Unit &u : units) {
+        int k = total > 0.0 ? (int)((cum + 0.5 * u.c) / total * K) : 0;
+        if (k > K - 1) k = K - 1;
+        if (out[k].hi[u.g] == out[k].lo[u.g]) out[k].lo[u.g] = u.lo;
+        out[k].hi[u.g] = u.hi; cum += u.c;
+    }
+}
+
+template <int NT, bool TS> static int team_occupancy(int threads, int smem)
+{
+    int occ = 0;
+    cudaFuncSetAttribute(k_propagate_team<NT, TS>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_propagate_team<NT, TS>, threads, smem);
+    return occ;
+}
+
+// Choose the team size for n_w walkers.  Warp-per-walker (team_tw = 1) when the walkers alone fill the resident warp slots;
+// otherwise the largest power of two 4 <= TW <= 16 with n_w TW <= slots (few walkers), or 4 for the large systems whose 36 KB
+// state leaves one warp per scheduler.  LRDMC_TEAM=<tw> forces a size (0/1: never).
+static void plan_team(lrdmc_ctx *c, int n_w)
+{
+    const DevSys &S = c->S; TeamPlan &P = c->team;
+    c->team_tw = 1;
+#if LRDMC_BC_DMMA
+    int tw = 1;
+    const long slots = (long)c->grid_max * c->wpb;
+    if (!c->ts) tw = 4;
+    else for (int cand = 4; cand <= LRDMC_TEAM_MAX_WARPS; cand *= 2) if ((long)n_w * cand <= slots) tw = cand;   // measured: 2 warps per walker do not pay
+    if (const char *e = getenv("LRDMC_TEAM")) { int v = atoi(e); tw = v < 1 ? 1 : v; }
+    int p2 = 1; while (p2 * 2 <= tw && p2 * 2 <= LRDMC_TEAM_MAX_WARPS) p2 *= 2;
+    tw = p2;
+    if (tw <= 1) return;
+    memset(&P, 0, sizeof P);
+    static const int ncomp[4] = { 1, 1, 3, 6 };
+    P.TW = tw;
+    P.nblk[0] = (S.n_up + 7) / 8; P.nblk[1] = (S.n_dn + 7) / 8;
+    const int nblk = S.n_mesh * (P.nblk[0] + P.nblk[1]);
+    int it_total = 0;
+    for (int g = 0; g < 4; ++g) {
+        P.it_base[g] = it_total; it_total += S.n_it[g];
+        P.kstep_base[g] = g ? P.kstep_base[g - 1] + ncomp[g - 1] * S.n_it[g - 1] : 0;
+        P.pair_base[g] = c->pair_base[g];
+    }
+    int np = 1; while (nblk * np < tw && np < LRDMC_TEAM_MAX_PARTS && 2 * np <= (it_total + 1) / 2) np *= 2;
+    P.NP = np; P.n_units = nblk * np;
+    int lpe = 32; while (lpe > 1 && (tw * 32) / lpe < S.N) lpe >>= 1;     // largest power of two with one pass over the electrons
+    P.lpe = lpe;
+    const double cost_col[4] = { 2.0, 1.0, 1.7, 2.9 }, cost_mo[4] = { 1.5, 1.0, 3.0, 6.0 };
+    partition_shells(S.n_it, cost_col, true, np, P.col);
+    partition_shells(S.n_it, cost_mo, false, tw, P.mo);
+    const size_t scr_col = np > 1 ? (size_t)S.n_mesh * S.N * np * 12 : 0, scr_mo = (size_t)tw * 5 * S.OS;
+    P.o_scr = S.per_warp_doubles; P.scr_doubles = (int)align_up(scr_col > scr_mo ? scr_col : scr_mo, 2);
+    const int smem = (int)(((size_t)S.tables_doubles + S.per_warp_doubles + P.scr_doubles) * 8);
+    int occ = 0;
+    if (c->ts) occ = c->NT == 1 ? team_occupancy<1, true>(tw * 32, smem) : (c->NT == 2 ? team_occupancy<2, true>(tw * 32, smem) : team_occupancy<4, true>(tw * 32, smem));
+    else occ = c->NT == 1 ? team_occupancy<1, false>(tw * 32, smem) : (c->NT == 2 ? team_occupancy<2, false>(tw * 32, smem) : team_occupancy<4, false>(tw * 32, smem));
+    if (cudaGetLastError() != cudaSuccess || occ < 1) return;             // does not fit: stay with warp-per-walker
+    c->team_tw = tw; c->team_smem = smem; c->team_ctas_per_sm = occ; c->team_grid_max = c->sm_count * occ;
+#endif
+}
+
 extern "C" int lrdmc_bind_walkers(lrdmc_ctx *c, void *dev_buf, size_t bytes, int n_walkers)
 {
     if (!c || !dev_buf || n_walkers < 1 || n_walkers > (1 << 20)) return LRDMC_EINVAL;
     char *base = (char *)align_up((size_t)dev_buf, 256);
     if (carve(c, n_walkers, NULL, NULL) + (size_t)(base - (char *)dev_buf) > bytes) return LRDMC_EINVAL;
     carve(c, n_walkers, base, &c->W);
+    plan_team(c, n_walkers);
     c->W.n_w = n_walkers; c->bound = 1; c->state_ok = 0; c->have_prop = c->have_reconf = 0;
     return LRDMC_OK;
 }
@@ -358,12 +440,21 @@ extern "C" int lrdmc_propagate(lrdmc_ctx *c, int mode, int n_moves, double tau, 
         || !std::isfinite(E0)) return LRDMC_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
     CK(cudaMemsetAsync(c->W.counter, 0, 64 * sizeof(int), st));
-    const int grid = grid_for(c);
+    const bool team = c->team_tw > 1;
+    const int grid = team ? (c->W.n_w < c->team_grid_max ? c->W.n_w : c->team_grid_max) : grid_for(c);
     CK(cudaEventRecord(c->ev[0], st));
-    DISPATCH_NT(k_propagate, grid, st, c->S, c->W, mode, n_moves, tau, E0, (uint32_t)cycle);
+    if (team) {
+#if LRDMC_BC_DMMA
+#define TEAM_(NTV, TSV) k_propagate_team<NTV, TSV><<<grid, c->team_tw * 32, c->team_smem, st>>>(c->S, c->W, c->team, mode, n_moves, tau, E0, (uint32_t)cycle)
+        if (c->ts) { if (c->NT == 1) TEAM_(1, true); else if (c->NT == 2) TEAM_(2, true); else TEAM_(4, true); }
+        else { if (c->NT == 1) TEAM_(1, false); else if (c->NT == 2) TEAM_(2, false); else TEAM_(4, false); }
+#undef TEAM_
+        ++c->launches;
+#endif
+    } else DISPATCH_NT(k_propagate, grid, st, c->S, c->W, mode, n_moves, tau, E0, (uint32_t)cycle);
     CK(cudaEventRecord(c->ev[1], st));
     CK(cudaGetLastError());
-    k_reduce_obs<<<1, 1024, 0, st>>>(c->W, c->d_stats, grid * c->wpb); ++c->launches;
+    k_reduce_obs<<<1, 1024, 0, st>>>(c->W, c->d_stats, team ? grid : grid * c->wpb); ++c->launches;
     CK(cudaGetLastError());
     c->have_prop = 1; c->last_stream = st;
     return LRDMC_OK;
@@ -433,6 +524,11 @@ extern "C" double *lrdmc_positions_ptr(const lrdmc_ctx *c, int which) { return w
 extern "C" int lrdmc_launch_config(const lrdmc_ctx *c, int *grid, int *block, int *smem_bytes, int *ctas_per_sm)
 {
     if (!c) return LRDMC_EINVAL;
+    if (c->bound && c->team_tw > 1) {            // team mode: one CTA of team_tw warps per walker
+        if (grid) *grid = c->W.n_w < c->team_grid_max ? c->W.n_w : c->team_grid_max;
+        if (block) *block = c->team_tw * 32; if (smem_bytes) *smem_bytes = c->team_smem; if (ctas_per_sm) *ctas_per_sm = c->team_ctas_per_sm;
+        return LRDMC_OK;
+    }
     if (grid) *grid = c->bound ? grid_for(c) : c->grid_max; if (block) *block = c->wpb * 32; if (smem_bytes) *smem_bytes = c->smem_bytes;
     if (ctas_per_sm) *ctas_per_sm = c->ctas_per_sm;
     return LRDMC_OK;

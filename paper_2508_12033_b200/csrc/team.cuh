@@ -1,0 +1,276 @@
+// team.cuh -- the projection kernel in TEAM form: one CTA of TW warps works on ONE walker (north_star: "one CTA or warp
+// group per walker").  Same arithmetic per candidate as the warp-per-walker kernel of propagate.cuh; what changes is who
+// does it:
+//   * few walkers (the paper runs 100 walkers per GPU, L289): with one warp per walker 100 warps would sit on 148 SMs.
+//     The candidate pass of an evaluation is cut into work units (8-electron block) x (shell part) that the TW warps take
+//     in turn; partial determinant ratios and partial Jastrow sums meet in shared memory.
+//   * large systems (64 electrons, 600 AOs): one walker's state is 36 KB of shared memory, so warp-per-walker leaves one warp
+//     per scheduler (ncu: 6 % warps active, FP64 pipe 21 %).  Here TW warps share that one state.
+// The walker queue, the weight rules (Alg.2 lines 4-8 L401-L410 / Alg.1) and the HBM layout are those of k_propagate.
+#pragma once
+#include "propagate.cuh"
+
+#if LRDMC_BC_DMMA
+
+__device__ __forceinline__ void load_walker_team(const DevSys &S, const DevWalk &W, WarpState &ws, const double *nuc, int k, int TW)
+{
+    const int N = S.N, tid = threadIdx.x, nthr = blockDim.x, lane = tid & 31, wt = tid >> 5;
+    for (int i = tid; i < 3 * N; i += nthr) ws.r[i] = W.r[(size_t)k * 3 * N + i];
+    for (int sp = 0; sp < 2; ++sp) {
+        const int ns = sp ? S.n_dn : S.n_up, tot = S.dinv_rows[sp] * ns;
+        const double *src = W.dinv[sp] + (size_t)k * ns * ns;
+        for (int i = tid; i < tot; i += nthr) ws.dinv[sp][i] = (i < ns * ns) ? src[i] : 0.0;
+    }
+    const size_t mocn = (size_t)N * 5 * S.OS;
+    if (S.moc_in_smem) { for (int i = tid; i < (int)mocn; i += nthr) ws.moc[i] = W.moc[(size_t)k * mocn + i]; }
+    else ws.moc = W.moc + (size_t)k * mocn;
+    __syncthreads();
+    for (int i = wt; i < N; i += TW) refresh_onebody(S.n_nuc, S.has_j1, S.a, nuc, ws.ob + 8 * i, ws.r[3 * i], ws.r[3 * i + 1], ws.r[3 * i + 2], lane);
+    __syncthreads();
+}
+
+__device__ __forceinline__ void store_walker_team(const DevSys &S, const DevWalk &W, const WarpState &ws, int k)
+{
+    const int N = S.N, tid = threadIdx.x, nthr = blockDim.x;
+    for (int i = tid; i < 3 * N; i += nthr) W.r[(size_t)k * 3 * N + i] = ws.r[i];
+    for (int sp = 0; sp < 2; ++sp) {
+        const int ns = sp ? S.n_dn : S.n_up;
+        double *dst = W.dinv[sp] + (size_t)k * ns * ns;
+        for (int i = tid; i < ns * ns; i += nthr) dst[i] = ws.dinv[sp][i];
+    }
+    const size_t mocn = (size_t)N * 5 * S.OS;
+    if (S.moc_in_smem) for (int i = tid; i < (int)mocn; i += nthr) W.moc[(size_t)k * mocn + i] = ws.moc[i];
+}
+
+// One evaluation by the team.  The result is valid in warp 0 only (it runs phase C); ws.R / ws.cum are complete for everyone
+// after the caller's next barrier.  s_vee: TW doubles of static shared memory.
+template <int NT, bool TS>
+__device__ __forceinline__ EvalOut evaluate_team(const DevSys &S, const TeamPlan &P, const WarpState &ws, const Tables &T, double *scr, double *s_vee)
+{
+    const int N = S.N, n_nuc = S.n_nuc, TW = P.TW, NP = P.NP, tid = threadIdx.x, nthr = blockDim.x, lane = tid & 31, wt = tid >> 5;
+    const int t = lane & 3, g = lane >> 2;
+    double *Jold = ws.el, *lap_s = ws.el + N;
+
+    // ---- phase A (row a6): per-electron continuum pieces; P.lpe lanes of one warp per electron split the partners and the MOs
+    {
+        const int LPE = P.lpe, epp = nthr / LPE;
+        double vee_part = 0.0;
+        for (int i0 = 0; i0 < N; i0 += epp) {
+            const int i = i0 + tid / LPE, sub = tid & (LPE - 1);
+            const bool act = i < N;
+            const int ii = act ? i : 0;
+            const int sp = spin_of(S, ii), il = sp ? ii - S.n_up : ii, ns = sp ? S.n_dn : S.n_up;
+            const double xi = ws.r[3 * ii], yi = ws.r[3 * ii + 1], zi = ws.r[3 * ii + 2];
+            double J = 0.0, gx = 0.0, gy = 0.0, gz = 0.0, lJ = 0.0, ve = 0.0;
+            for (int j = sub; j < N; j += LPE) if (j != ii) {
+                const double dx = xi - ws.r[3 * j], dy = yi - ws.r[3 * j + 1], dz = zi - ws.r[3 * j + 2], r2 = dx * dx + dy * dy + dz * dz;
+                const double ir = fast_rsqrt(r2), r = r2 * ir;
+                const double c = (spin_of(S, j) == sp) ? S.a_par : S.a_anti, iq = fast_rcp(1.0 + S.b2 * r), du = c * iq * iq * ir;
+                J += c * r * iq; gx += du * dx; gy += du * dy; gz += du * dz; lJ += 2.0 * du * iq;
+                if (j > ii) ve += ir;
+            }
+            const double *mc = ws.moc + (size_t)ii * 5 * S.OS, *di = (sp ? ws.dinv[1] : ws.dinv[0]) + il;
+            double Gx = 0.0, Gy = 0.0, Gz = 0.0, Ld = 0.0;
+            for (int m = sub; m < ns; m += LPE) {
+                const double d = di[m * ns];
+                Gx += mc[S.OS + m] * d; Gy += mc[2 * S.OS + m] * d; Gz += mc[3 * S.OS + m] * d; Ld += mc[4 * S.OS + m] * d;
+            }
+            for (int o = 1; o < LPE; o <<= 1) {
+#define GRP_SUM(v) v += __shfl_xor_sync(0xffffffffu, v, o)
+                GRP_SUM(J); GRP_SUM(gx); GRP_SUM(gy); GRP_SUM(gz); GRP_SUM(lJ); GRP_SUM(Gx); GRP_SUM(Gy); GRP_SUM(Gz); GRP_SUM(Ld);
+#undef GRP_SUM
+            }
+            if (act) vee_part += ve;
+            if (act && sub == 0) {
+                const double *ob = ws.ob + 8 * ii;
+                gx += ob[1]; gy += ob[2]; gz += ob[3];
+                Jold[ii] = J + ob[0];
+                lap_s[ii] = Ld + 2.0 * (Gx * gx + Gy * gy + Gz * gz) + (lJ + ob[4]) + (gx * gx + gy * gy + gz * gz);
+            }
+        }
+        vee_part = warp_sum(vee_part);
+        if (lane == 0) s_vee[wt] = vee_part;
+    }
+    __syncthreads();
+
+    // ---- phase B (rows a1-a5): work units (mesh, spin, 8-electron block, shell part); unit u -> warp u mod TW
+    const int nb_mesh = P.nblk[0] + P.nblk[1];
+    for (int u = wt; u < P.n_units; u += TW) {
+        const int part = u % NP, blk = u / NP, mesh = blk / nb_mesh, rem = blk - mesh * nb_mesh;
+        const int sp = rem >= P.nblk[0] ? 1 : 0, il0 = 8 * (sp ? rem - P.nblk[0] : rem);
+        const int ns = sp ? S.n_dn : S.n_up, off = sp ? S.n_up : 0;
+        const double am = S.amesh[mesh], a2 = am * am;
+        double av[3][3];
+#pragma unroll
+        for (int k = 0; k < 3; ++k) { av[k][0] = am * ws.U[k]; av[k][1] = am * ws.U[3 + k]; av[k][2] = am * ws.U[6 + k]; }
+        const bool valid = il0 + g < ns;
+        const int il = valid ? il0 + g : 0, i = off + il;
+        const double x0 = ws.r[3 * i], y0 = ws.r[3 * i + 1], z0 = ws.r[3 * i + 2];
+        double acc[6], Jn[6];
+        ao_columns<NT, TS, true>(S, T.shells, sp ? T.cf[1] : T.cf[0], T.etab, sp ? ws.dinv[1] : ws.dinv[0], ns, il, x0, y0, z0, av, a2, lane, acc, &P, &P.col[part]);
+#pragma unroll
+        for (int d = 0; d < 6; ++d) Jn[d] = 0.0;
+        if (S.has_j1) for (int I = t + 4 * part; I < n_nuc; I += 4 * NP) {
+            const double *nu = T.nuc + I * LRDMC_NUC_STRIDE;
+            pade_six(x0 - nu[0], y0 - nu[1], z0 - nu[2], av, a2, -nu[4], nu[5], Jn);
+        }
+        for (int j = t + 4 * part; j < N; j += 4 * NP) {
+            const double c = (j == i) ? 0.0 : ((spin_of(S, j) == sp) ? S.a_par : S.a_anti);
+            pade_six(x0 - ws.r[3 * j], y0 - ws.r[3 * j + 1], z0 - ws.r[3 * j + 2], av, a2, c, S.b2, Jn);
+        }
+        if (NP == 1) {
+            const double Jo = Jold[i];
+            double Rv[6];
+#pragma unroll
+            for (int d = 0; d < 6; ++d) Rv[d] = quad_sum(acc[d]) * exp_tab(quad_sum(Jn[d]) - Jo, T.etab);
+            if (valid && t == 0) {
+                double *Ro = ws.R + mesh * 6 * N + 6 * i;
+#pragma unroll
+                for (int d = 0; d < 6; ++d) Ro[d] = Rv[d];
+            }
+        } else {
+            double *q = scr + ((size_t)(mesh * N + i) * NP + part) * 12;
+#pragma unroll
+            for (int d = 0; d < 6; ++d) {
+                const double A = quad_sum(acc[d]), J = quad_sum(Jn[d]);
+                if (valid && t == 0) { q[d] = A; q[6 + d] = J; }
+            }
+        }
+    }
+    __syncthreads();
+    if (NP > 1) {                      // the parts of a candidate meet: R = (sum of determinant shares) exp(sum of Jastrow shares - J_old)
+        for (int p = tid; p < S.P; p += nthr) {
+            const int mesh = p / (6 * N), rem = p - mesh * 6 * N, i = rem / 6, d = rem - 6 * i;
+            const double *q = scr + (size_t)(mesh * N + i) * NP * 12;
+            double A = 0.0, J = 0.0;
+            for (int part = 0; part < NP; ++part) { A += q[part * 12 + d]; J += q[part * 12 + 6 + d]; }
+            ws.R[p] = A * exp_tab(J - Jold[i], T.etab);
+        }
+        __syncthreads();
+    }
+    EvalOut o; o.bbar = 0.0; o.Vsf = 0.0; o.W = 0.0; o.eL = 0.0; o.node = 0;
+    if (wt == 0) {
+        double Vee = 0.0;
+        for (int w = 0; w < TW; ++w) Vee += s_vee[w];
+        o = phase_c(S, ws, lap_s, Vee, lane);
+    }
+    return o;
+}
+
+// Apply move j (row a10) by the team: warp w takes part P.mo[w] of the derivative pass of the mover (value, gradient, Laplacian
+// rows by DMMA), the partial rows meet in scr; Sherman-Morrison on Dinv_sigma over all threads.
+template <int NT, bool TS>
+__device__ __forceinline__ void apply_move_team(const DevSys &S, const TeamPlan &P, const WarpState &ws, const Tables &T, double *scr, int j)
+{
+    const int N = S.N, TW = P.TW, tid = threadIdx.x, nthr = blockDim.x, lane = tid & 31, wt = tid >> 5;
+    const int mesh = j / (6 * N), jj = j - mesh * 6 * N, i = jj / 6, d = jj - 6 * i, k = d >> 1;
+    const int sp = spin_of(S, i), il = sp ? i - S.n_up : i, ns = sp ? S.n_dn : S.n_up;
+    const double step = (d & 1) ? -S.amesh[mesh] : S.amesh[mesh];
+    const double px = ws.r[3 * i] + step * ws.U[k], py = ws.r[3 * i + 1] + step * ws.U[3 + k], pz = ws.r[3 * i + 2] + step * ws.U[6 + k];
+    double *mc = ws.moc + (size_t)i * 5 * S.OS;
+    const int rows = 5 * S.OS;
+    {
+        double acc[NT][2];
+        mo_pass<NT, true, TS, true>(S, T.shells, sp ? T.bf[1] : T.bf[0], T.etab, px, py, pz, lane, acc, &P, &P.mo[wt]);
+        const int t = lane & 3, g = lane >> 2;
+        if (g < 5) {
+            double *q = scr + (size_t)wt * rows + g * S.OS;
+#pragma unroll
+            for (int nt = 0; nt < NT; ++nt) { q[8 * nt + 2 * t] = acc[nt][0]; q[8 * nt + 2 * t + 1] = acc[nt][1]; }
+        }
+    }
+    if (wt == TW - 1) refresh_onebody(S.n_nuc, S.has_j1, S.a, T.nuc, ws.ob + 8 * i, px, py, pz, lane);
+    __syncthreads();                                   // every thread has read the old position
+    for (int idx = tid; idx < rows; idx += nthr) {
+        double s = 0.0;
+        for (int w = 0; w < TW; ++w) s += scr[(size_t)w * rows + idx];
+        mc[idx] = s;
+    }
+    if (tid == 0) { ws.r[3 * i] = px; ws.r[3 * i + 1] = py; ws.r[3 * i + 2] = pz; }
+    __syncthreads();
+    // s_k = sum_m phi_m Dinv[m][k];  rho = s_il;  Dinv'[m][il] = Dinv[m][il]/rho;  Dinv'[m][k] = Dinv[m][k] - Dinv[m][il] s_k / rho
+    double *dinv = sp ? ws.dinv[1] : ws.dinv[0], *sk = ws.el + 2 * N, *col = ws.el + 3 * N;
+    for (int kk = tid; kk < ns; kk += nthr) {
+        double s = 0.0;
+        for (int m = 0; m < ns; ++m) s += mc[m] * dinv[m * ns + kk];
+        sk[kk] = s; col[kk] = dinv[kk * ns + il];
+    }
+    __syncthreads();
+    const double irho = 1.0 / sk[il];
+    for (int idx = tid; idx < ns * ns; idx += nthr) {
+        const int m = idx / ns, kk = idx - m * ns;
+        const double ci = col[m] * irho;
+        dinv[idx] = (kk == il) ? ci : dinv[idx] - ci * sk[kk];
+    }
+    __syncthreads();
+}
+
+template <int NT, bool TS>
+__global__ void __launch_bounds__(LRDMC_TEAM_MAX_WARPS * 32, 1) k_propagate_team(DevSys S, DevWalk W, TeamPlan P, int mode, int n_moves, double tau, double E0, uint32_t cycle)
+{
+    extern __shared__ __align__(16) double smem[];
+    __shared__ double s_vee[LRDMC_TEAM_MAX_WARPS];
+    __shared__ int s_ctrl[4];
+    stage_tables(S, smem);
+    const int tid = threadIdx.x, lane = tid & 31, wt = tid >> 5;
+    const Tables T = table_pointers<TS>(S, smem);
+    WarpState ws = warp_views(S, smem, 0);
+    double *scr = smem + S.tables_doubles + P.o_scr;
+    const unsigned long long t_start = globaltimer_ns();
+    for (;;) {
+        if (tid == 0) s_ctrl[0] = atomicAdd(W.counter, 1);
+        __syncthreads();
+        const int k = s_ctrl[0];
+        if (k >= W.n_w) break;
+        load_walker_team(S, W, ws, T.nuc, k, P.TW);
+        uint32_t s = 0;
+        double w = 1.0, tau_left = tau, omega = 0.0, eL_last = 0.0, W_last = 0.0; long long moves = 0; int n_node = 0, n_nonpos = 0;
+        for (;;) {
+            const StepDraws d = step_draws(S, (uint32_t)k, cycle, s, mode == LRDMC_CONVENTIONAL);
+            if (tid == 0) { double U[9]; lattice_frame(d.u1, d.u2, d.u3, U);
+#pragma unroll
+                for (int i = 0; i < 9; ++i) ws.U[i] = U[i]; }
+            __syncthreads();
+            const EvalOut e = evaluate_team<NT, TS>(S, P, ws, T, scr, s_vee);
+            if (wt == 0) {                                       // the leader warp keeps the weight (same rules as k_propagate)
+                n_node += e.node;
+                bool last = false;
+                if (mode == LRDMC_BALANCED) {
+                    const double den = e.W - E0;                       // b_x = bbar/(W - E0)   (Eq.29)
+                    if ((int)s == n_moves) {                           // measurement evaluation (reading Q10; Eq.34)
+                        if (!(den > 0.0)) { ++n_nonpos; w = 0.0; omega = 0.0; } else omega = w / den;
+                        last = true;
+                    } else if (!(den > 0.0)) { ++n_nonpos; w = 0.0; }  // reading Q16
+                    else w *= e.bbar / den;                            // Alg.2 line 6 (L406)
+                } else {
+                    double tx = -log1p(-d.u_tau) / e.bbar;             // Eq.24 (L160)
+                    if (!(tx < tau_left) || (n_moves > 0 && (int)s >= n_moves)) { tx = tau_left; last = true; }   // min[., tau_left] (L362)
+                    w *= exp(-tx * (e.eL - E0));                       // Eq.25 (L164), constant shift of reading Q8b
+                    tau_left -= tx;
+                    if (last) omega = w;
+                }
+                int j = -1;
+                if (!last) j = select_move(S, ws, d.u_sel, lane);      // Alg.2 line 7 (L408)
+                else { eL_last = e.eL; W_last = e.W; }
+                if (lane == 0) { s_ctrl[1] = last ? 1 : 0; s_ctrl[2] = j; }
+            }
+            __syncthreads();
+            const bool last = s_ctrl[1] != 0; const int j = s_ctrl[2];
+            if (last) break;
+            if (j >= 0) { apply_move_team<NT, TS>(S, P, ws, T, scr, j); ++moves; }
+            ++s;
+        }
+        store_walker_team(S, W, ws, k);
+        if (tid == 0) {
+            int nonfinite = 0;
+            if (!isfinite(w) || !isfinite(omega)) { nonfinite = 1; w = 0.0; omega = 0.0; }
+            W.w[k] = w; W.eL[k] = eL_last; W.W[k] = W_last; W.omega[k] = omega; W.nmoves[k] = moves;
+            W.flags[3 * k] = n_node; W.flags[3 * k + 1] = n_nonpos; W.flags[3 * k + 2] = nonfinite;
+        }
+        if (!S.moc_in_smem) ws = warp_views(S, smem, 0);
+        __syncthreads();                                        // the state and s_ctrl are free for the next walker
+    }
+    if (tid == 0) { W.timing[2 * blockIdx.x] = t_start; W.timing[2 * blockIdx.x + 1] = globaltimer_ns(); }
+}
+
+#endif  // LRDMC_BC_DMMA

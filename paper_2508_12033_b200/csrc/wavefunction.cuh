@@ -46,10 +46,15 @@ __device__ __forceinline__ double gto_component(int g, const AxisPoly &X, const 
 // One pass over the whole (sorted, padded) shell list for the 8 points held by the warp.
 // DERIV = false: A fragment = AO value (candidate evaluation, row a2/a3).
 // DERIV = true : the 8 mma rows are 8 COMPONENTS (value, d/dx, d/dy, d/dz, Laplacian, 0,0,0) of ONE point, selector g = lane/4.
-template <int NT, bool DERIV, bool TS>
+// PART (team mode): only the 4-shell iterations [part->lo[g], part->hi[g]) of each group g; the partial sums of the parts add up.
+template <int NT, bool DERIV, bool TS, bool PART = false>
 __device__ __forceinline__ void mo_pass(const DevSys &S, const double *__restrict__ shells, const double *__restrict__ bf, const double *__restrict__ etab,
-                                        double px, double py, double pz, int lane, double (&acc)[NT][2])
+                                        double px, double py, double pz, int lane, double (&acc)[NT][2],
+                                        const TeamPlan *tp = nullptr, const ShellPart *part = nullptr)
 {
+#define LRDMC_MO_RANGE(G, NC)                                                                   \
+    const int n_ = PART ? part->hi[G] : S.n_it[G]; int it = PART ? part->lo[G] : 0;             \
+    if (PART) { sh4 = reinterpret_cast<const double4 *>(shells) + t + 4 * (tp->it_base[G] + it); b = bf + lane + (size_t)(tp->kstep_base[G] + NC * it) * NT * 32; }
     const int t = lane & 3, g = lane >> 2;
     const double4 *sh4 = reinterpret_cast<const double4 *>(shells) + t;
     const double *b = bf + lane;
@@ -62,7 +67,7 @@ __device__ __forceinline__ void mo_pass(const DevSys &S, const double *__restric
         b += NT * 32;                                                                           \
     }
     // ---- group 0: Slater-type s, chi = exp(-z r); grad = -z chi rhat; lap = chi (z^2 - 2 z / r)
-    for (int it = 0; it < S.n_it[0]; ++it, sh4 += 4) {
+    { LRDMC_MO_RANGE(0, 1) for (; it < n_; ++it, sh4 += 4) {
         double4 s = *sh4; double dx = px - s.x, dy = py - s.y, dz = pz - s.z, z = s.w;
         double r = sqrt(dx * dx + dy * dy + dz * dz), e = exp_tab(exp_arg_floor(-z * r), etab);
         if (!DERIV) { LRDMC_FEED(e); }
@@ -71,16 +76,16 @@ __device__ __forceinline__ void mo_pass(const DevSys &S, const double *__restric
             double v = (g == 0) ? e : ((g == 4) ? e * (z * z - 2.0 * z * ir) : -z * e * d * ir);
             LRDMC_FEED((g > 4) ? 0.0 : v);
         }
-    }
+    } }
     // ---- group 1: s Gaussians
-    for (int it = 0; it < S.n_it[1]; ++it, sh4 += 4) {
+    { LRDMC_MO_RANGE(1, 1) for (; it < n_; ++it, sh4 += 4) {
         double4 s = *sh4; double dx = px - s.x, dy = py - s.y, dz = pz - s.z, z = s.w;
         double e = exp_tab(exp_arg_floor(-z * (dx * dx + dy * dy + dz * dz)), etab);
         if (!DERIV) { LRDMC_FEED(e); }
         else { AxisPoly X = axis_poly(dx, z), Y = axis_poly(dy, z), Z = axis_poly(dz, z); LRDMC_FEED((gto_component<0, 0, 0>(g, X, Y, Z, e))); }
-    }
+    } }
     // ---- group 2: p Gaussians (x, y, z)
-    for (int it = 0; it < S.n_it[2]; ++it, sh4 += 4) {
+    { LRDMC_MO_RANGE(2, 3) for (; it < n_; ++it, sh4 += 4) {
         double4 s = *sh4; double dx = px - s.x, dy = py - s.y, dz = pz - s.z, z = s.w;
         double e = exp_tab(exp_arg_floor(-z * (dx * dx + dy * dy + dz * dz)), etab);
         if (!DERIV) { LRDMC_FEED(dx * e); LRDMC_FEED(dy * e); LRDMC_FEED(dz * e); }
@@ -89,9 +94,9 @@ __device__ __forceinline__ void mo_pass(const DevSys &S, const double *__restric
             LRDMC_FEED((gto_component<1, 0, 0>(g, X, Y, Z, e))); LRDMC_FEED((gto_component<0, 1, 0>(g, X, Y, Z, e)));
             LRDMC_FEED((gto_component<0, 0, 1>(g, X, Y, Z, e)));
         }
-    }
+    } }
     // ---- group 3: d Gaussians (xx, xy, xz, yy, yz, zz)
-    for (int it = 0; it < S.n_it[3]; ++it, sh4 += 4) {
+    { LRDMC_MO_RANGE(3, 6) for (; it < n_; ++it, sh4 += 4) {
         double4 s = *sh4; double dx = px - s.x, dy = py - s.y, dz = pz - s.z, z = s.w;
         double e = exp_tab(exp_arg_floor(-z * (dx * dx + dy * dy + dz * dz)), etab);
         if (!DERIV) {
@@ -103,7 +108,8 @@ __device__ __forceinline__ void mo_pass(const DevSys &S, const double *__restric
             LRDMC_FEED((gto_component<1, 0, 1>(g, X, Y, Z, e))); LRDMC_FEED((gto_component<0, 2, 0>(g, X, Y, Z, e)));
             LRDMC_FEED((gto_component<0, 1, 1>(g, X, Y, Z, e))); LRDMC_FEED((gto_component<0, 0, 2>(g, X, Y, Z, e)));
         }
-    }
+    } }
+#undef LRDMC_MO_RANGE
 #undef LRDMC_FEED
 }
 
@@ -284,11 +290,17 @@ __device__ __forceinline__ void ao_columns(const DevSys &S, const double *__rest
 // 2 NT DMMA + 2 NT LDS per pair of entries instead of 16 NT DFMA + 16 NT LDS (same FP64-pipe time, 1/8 of the issue slots).
 // A operand = column il of Dinv (2 NT registers per lane); B operand = the pair table `cf` built at init.  Each shell
 // group is padded to an even number of k-steps; s and p iterations are taken two at a time with a one-iteration tail.
-template <int NT, bool TS>
+// PART (team mode): only the iterations [part->lo[g], part->hi[g]) of each shell group (lo even in groups 0-2, so that a part
+// starts on a k-step pair); acc is then the part's share of the ratio.
+template <int NT, bool TS, bool PART = false>
 __device__ __forceinline__ void ao_columns(const DevSys &S, const double *__restrict__ shells, const double *__restrict__ cf, const double *__restrict__ etab,
                                            const double *__restrict__ dinv, int ns, int il, double x0, double y0, double z0,
-                                           const double (&av)[3][3], double a2, int lane, double (&acc)[6])
+                                           const double (&av)[3][3], double a2, int lane, double (&acc)[6],
+                                           const TeamPlan *tp = nullptr, const ShellPart *part = nullptr)
 {
+#define LRDMC_COL_RANGE(G, PAIRS)                                                               \
+    const int n = PART ? part->hi[G] : S.n_it[G]; int it = PART ? part->lo[G] : 0;              \
+    if (PART) { sh4 = reinterpret_cast<const double4 *>(shells) + t + 4 * (tp->it_base[G] + it); b = cf + lane + (size_t)(tp->pair_base[G] + (PAIRS)) * NA * 32; }
     const int t = lane & 3;
     const double4 *sh4 = reinterpret_cast<const double4 *>(shells) + t;
     const double *b = cf + lane;
@@ -345,21 +357,21 @@ __device__ __forceinline__ void ao_columns(const DevSys &S, const double *__rest
         sh4 += 4;
     };
     {
-        const int n = S.n_it[0]; int it = 0; double b0, b1;
+        LRDMC_COL_RANGE(0, it / 2) double b0, b1;
         for (; it + 1 < n; it += 2) { LRDMC_BPAIR(b0, b1) slater_body(b0); slater_body(b1); }
         if (it < n) { LRDMC_BPAIR(b0, b1) slater_body(b0); }
     }
     {
-        const int n = S.n_it[1]; int it = 0; double b0, b1;
+        LRDMC_COL_RANGE(1, it / 2) double b0, b1;
         for (; it + 1 < n; it += 2) { LRDMC_BPAIR(b0, b1) s_body(b0); s_body(b1); }
         if (it < n) { LRDMC_BPAIR(b0, b1) s_body(b0); }
     }
     {
-        const int n = S.n_it[2]; int it = 0; double b0, b1, b2, b3, b4, b5;
+        LRDMC_COL_RANGE(2, 3 * it / 2) double b0, b1, b2, b3, b4, b5;
         for (; it + 1 < n; it += 2) { LRDMC_BPAIR(b0, b1) LRDMC_BPAIR(b2, b3) LRDMC_BPAIR(b4, b5) p_body(b0, b1, b2); p_body(b3, b4, b5); }
         if (it < n) { LRDMC_BPAIR(b0, b1) LRDMC_BPAIR(b2, b3) p_body(b0, b1, b2); }
     }
-    for (int it = 0; it < S.n_it[3]; ++it, sh4 += 4) {            // d: xx xy xz yy yz zz  ->  e Q(d),  Q(d0 +- v) = Q(d0) +- v.grad Q(d0) + Q(v)
+    { LRDMC_COL_RANGE(3, 3 * it) for (; it < n; ++it, sh4 += 4) {   // d: xx xy xz yy yz zz  ->  e Q(d),  Q(d0 +- v) = Q(d0) +- v.grad Q(d0) + Q(v)
         double bc[6]; LRDMC_BPAIR(bc[0], bc[1]) LRDMC_BPAIR(bc[2], bc[3]) LRDMC_BPAIR(bc[4], bc[5])
         LRDMC_GEOM
         LRDMC_EXPS
@@ -376,10 +388,11 @@ __device__ __forceinline__ void ao_columns(const DevSys &S, const double *__rest
             acc[2 * k] = fma(e[2 * k], Qs + lin, acc[2 * k]);
             acc[2 * k + 1] = fma(e[2 * k + 1], Qs - lin, acc[2 * k + 1]);
         }
-    }
+    } }
 #undef LRDMC_EXPS
 #undef LRDMC_GEOM
 #undef LRDMC_BPAIR
+#undef LRDMC_COL_RANGE
 }
 #endif
 

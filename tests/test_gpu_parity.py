@@ -120,10 +120,32 @@ def test_one_evaluation_and_selection_from_the_oracle_state(B, name):
 # ------------------------------------------------------------------------------------------ whole cycles
 @pytest.mark.parametrize("name", list(SYSTEMS))
 @pytest.mark.parametrize("mode", ["balanced", "conventional"])
-def test_whole_cycle_trajectories_weights_and_branching(B, name, mode):
+@pytest.mark.parametrize("kernel", ["warp-per-walker", "auto"])
+def test_whole_cycle_trajectories_weights_and_branching(B, name, mode, kernel, monkeypatch):
+    """kernel = warp-per-walker forces k_propagate; auto lets lrdmc_bind_walkers pick the team size (k_propagate_team for
+    these small ensembles and for the 64-electron system), as bench.py and a user get it."""
+    if kernel == "warp-per-walker":
+        monkeypatch.setenv("LRDMC_TEAM", "1")
+    _whole_cycles(B, name, mode)
+
+
+@pytest.mark.parametrize("tw", [2, 4, 8, 16])
+@pytest.mark.parametrize("name,mode", [("tiny-3u3d-pp", "balanced"), ("tiny-2u2d-doublemesh", "conventional"), ("ragged-9u4d-NT2", "balanced"),
+                                       ("ragged-17u3d-NT4", "conventional"), ("he-triplet-slater", "balanced"), ("C3-water-methane-shaped", "balanced"),
+                                       ("C3-water-methane-shaped", "conventional"), ("C5-cluster64-doublemesh", "balanced")])
+def test_team_kernel_every_team_size(B, name, mode, tw, monkeypatch):
+    """k_propagate_team with TW = 2, 4, 8, 16 warps per walker (work units = electron blocks x shell parts, partial sums
+    in shared memory): same trajectories, weights and indices as the oracle."""
+    monkeypatch.setenv("LRDMC_TEAM", str(tw))
+    g = _whole_cycles(B, name, mode, n_cycles=1, keep=True)
+    assert g.launch_config()["block"] == 32 * tw
+    g.close()
+
+
+def _whole_cycles(B, name, mode, n_cycles=2, keep=False):
     s, x0, o, g = _pair(B, name)
     N = s["n_up"] + s["n_dn"]; n_moves = 30
-    for cycle in (0, 1):
+    for cycle in range(n_cycles):
         if mode == "balanced":
             assert o.propagate(ref.BALANCED, n_moves, 0.0, -5.0, cycle) == 0
             g.lrdmc_propagate(B.BALANCED, n_moves, 0.0, -5.0, cycle)
@@ -148,6 +170,8 @@ def test_whole_cycle_trajectories_weights_and_branching(B, name, mode):
         assert abs(sg.lockstep_idle_frac - so["lockstep_idle_frac"]) < 1e-12
         r2, *_ = o.get_state(); gr2 = np_(g.lrdmc_get_walkers()[0])
         assert np.abs(gr2 - r2).max() < 1e-11 and np.all(np_(g.lrdmc_get_walkers()[3]) == 1.0)
+    if keep:
+        return g
     g.close()
 
 
