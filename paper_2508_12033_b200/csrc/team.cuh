@@ -162,7 +162,7 @@ __device__ __forceinline__ EvalOut evaluate_team(const DevSys &S, const TeamPlan
 template <int NT, bool TS>
 __device__ __forceinline__ void apply_move_team(const DevSys &S, const TeamPlan &P, const WarpState &ws, const Tables &T, double *scr, int j)
 {
-    const int N = S.N, TW = P.TW, tid = threadIdx.x, nthr = blockDim.x, lane = tid & 31, wt = tid >> 5;
+    const int N = S.N, TW = P.TW, tid = threadIdx.x, nthr = blockDim.x, lane = tid & 31, wt = tid >> 5;   // warp 0 holds the lightest shell part (s shells): it also refreshes the one-body cache
     const int mesh = j / (6 * N), jj = j - mesh * 6 * N, i = jj / 6, d = jj - 6 * i, k = d >> 1;
     const int sp = spin_of(S, i), il = sp ? i - S.n_up : i, ns = sp ? S.n_dn : S.n_up;
     const double step = (d & 1) ? -S.amesh[mesh] : S.amesh[mesh];
@@ -179,7 +179,7 @@ __device__ __forceinline__ void apply_move_team(const DevSys &S, const TeamPlan 
             for (int nt = 0; nt < NT; ++nt) { q[8 * nt + 2 * t] = acc[nt][0]; q[8 * nt + 2 * t + 1] = acc[nt][1]; }
         }
     }
-    if (wt == TW - 1) refresh_onebody(S.n_nuc, S.has_j1, S.a, T.nuc, ws.ob + 8 * i, px, py, pz, lane);
+    if (wt == 0) refresh_onebody(S.n_nuc, S.has_j1, S.a, T.nuc, ws.ob + 8 * i, px, py, pz, lane);
     __syncthreads();                                   // every thread has read the old position
     for (int idx = tid; idx < rows; idx += nthr) {
         double s = 0.0;
