@@ -36,7 +36,24 @@ int lrdmc_ref_create(lrdmc_ref_ctx **out, int n_nuc, const double *Z, const doub
                      int n_ao, const double *C_up, const double *C_dn, double a_par, double a_anti, double b2,
                      const double *c1, const double *b1, double a, double a2, uint64_t seed);
 void lrdmc_ref_destroy(lrdmc_ref_ctx *);
-int lrdmc_ref_n_candidates(const lrdmc_ref_ctx *); /* P = 6 N n_mesh */
+int lrdmc_ref_n_candidates(const lrdmc_ref_ctx *); /* P = 6 N n_mesh (+ 6 N K non-local slots) */
+
+/* Non-local (semi-local) pseudopotential, scope row f1 (L242 "DLA", L567 D1 "non-local pseudopotentials", L576 "DTM").
+ * nl [n_nuc][7] = { r_c, A_0, B_0, A_1, B_1, A_2, B_2 }: channel l of nucleus I is v_l(r) = A_l exp(-B_l r^2) inside r < r_c
+ * (synthetic Gaussian channels: the ccECP tables are not in the container); r_c <= 0: no non-local part on that nucleus.
+ *   V_nl Psi(x)/Psi(x) = sum_i sum_I sum_l v_l(r_iI) (2l+1)/(4 pi) int P_l(cos th') Psi(.. R_I + r_iI Omega' ..)/Psi(x) dOmega'
+ * with the integral on the 6-point octahedral rule (weights 1/6, exact to degree 3) along +-e_k of the step's random frame
+ * ("and the discretized ECP mesh", L625-L628).  Each (electron i, centre I in range) gives 6 more candidates x_q with
+ * H_{x_q,x} = nu_q = (1/6) sum_l (2l+1) v_l(r_iI) P_l(cos th_q) and ratio rho_q = D(x_q)/D(x) (dla = 1: determinant
+ * locality, L576) or Psi_G(x_q)/Psi_G(x) (dla = 0: T-move form).  Fixed node (Eq.D1): nu_q rho_q < 0 -> allowed hop with
+ * Green's function -nu_q rho_q; nu_q rho_q > 0 -> added to V_sf.  Slots: j = 6 N n_mesh + 6 (i K + kk) + q, kk = rank of
+ * centre I among the centres in range of electron i (ascending I), q = 2k (+e_k) / 2k+1 (-e_k); R[j] holds the signed
+ * Green's-function amplitude -nu_q rho_q (0 for an empty slot), i.e. the slot has "kappa = 1".  K = max centres in range of
+ * one point (a property of the geometry; evaluation fails with EINVAL if exceeded).  Call before set_positions. */
+int lrdmc_ref_set_nonlocal(lrdmc_ref_ctx *, int K, int dla, const double *nl);
+/* nu_q and rho_q of every non-local slot at x in frame U (for the pins): nu, rho [6 N K], cand [6 N K][3] (nullable) */
+int lrdmc_ref_nl_info(const lrdmc_ref_ctx *, const double *x, const double *dinv_up, const double *dinv_dn, const double U[9],
+                      double *nu, double *rho, double *cand);
 
 /* walkers */
 int lrdmc_ref_set_positions(lrdmc_ref_ctx *, int n_w, const double *r /*[n_w][N][3]*/);

@@ -63,6 +63,9 @@ def lib():
                                           C.c_double, C.c_double, C.c_double, C.c_void_p, C.c_void_p, C.c_double, C.c_double,
                                           C.c_uint64]
         _lib.lrdmc_ref_destroy.argtypes = [C.c_void_p]
+        _lib.lrdmc_ref_set_nonlocal.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p]
+        _lib.lrdmc_ref_nl_info.argtypes = [C.c_void_p] + [C.c_void_p] * 7
+        _lib.lrdmc_ref_n_candidates.argtypes = [C.c_void_p]
         _lib.lrdmc_ref_propagate.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_double, C.c_double, C.c_uint64]
         _lib.lrdmc_ref_reconfigure.argtypes = [C.c_void_p, C.c_uint64, C.c_void_p]
         _lib.lrdmc_ref_step_debug.argtypes = [C.c_void_p, C.c_double, C.c_uint64, C.c_uint64, C.c_void_p, C.c_void_p, C.c_void_p]
@@ -115,6 +118,13 @@ class Ref:
         if rc:
             raise ValueError(f"lrdmc_ref_create failed: {rc}")
         self.h = h
+        self.nl_slots = 0
+        if sysd.get("nl") is not None and sysd.get("nl_K", 0) > 0:      # non-local pseudopotential channels (scope row f1)
+            nl = np.ascontiguousarray(sysd["nl"], dtype=np.float64)
+            rc = L.lrdmc_ref_set_nonlocal(h, int(sysd["nl_K"]), int(sysd["nl_dla"]), nl.ctypes.data)
+            if rc:
+                raise ValueError(f"lrdmc_ref_set_nonlocal failed: {rc}")
+            self.nl_slots = 6 * self.N * int(sysd["nl_K"])
         self.P = L.lrdmc_ref_n_candidates(h)
         self.n_w = 0
 
@@ -209,6 +219,15 @@ class Ref:
             raise FloatingPointError(f"evaluate failed: {rc}")
         keys = ("bbar", "V_sf", "W", "e_L", "node", "V_ee", "V_ii", "K_diag", "n_vmax", "e_L_continuum")
         return R, dict(zip(keys, scal)), per, cand
+
+    def nl_info(self, x, U, du, dd):
+        """nu_q = V^nl_{x_q,x}, rho_q (determinant or wavefunction ratio) and the quadrature points of every non-local slot"""
+        x = np.ascontiguousarray(x, dtype=np.float64); U = np.ascontiguousarray(U, dtype=np.float64)
+        du = np.ascontiguousarray(du); dd = np.ascontiguousarray(dd) if dd is not None and dd.size else np.zeros(1)
+        n = self.nl_slots; nu = np.zeros(n); rho = np.zeros(n); cand = np.zeros((n, 3))
+        rc = lib().lrdmc_ref_nl_info(self.h, x.ctypes.data, du.ctypes.data, dd.ctypes.data, U.ctypes.data, nu.ctypes.data, rho.ctypes.data, cand.ctypes.data)
+        assert rc == 0
+        return nu, rho, cand
 
     def select(self, R, u_sel):
         R = np.ascontiguousarray(R, dtype=np.float64); mg = C.c_double()

@@ -46,10 +46,63 @@ static double jastrow_of_electron(const lrdmc_ref_ctx *c, const double *x, int i
     return J;
 }
 
+/* ---- non-local pseudopotential candidates (scope row f1; definition in lrdmc_ref.h) ------------------------------- */
+/* centres in range of a point: nuclei with r_c > 0 and |ri - R_I| < r_c, ascending I; returns their number */
+static int nl_in_range(const lrdmc_ref_ctx *c, const double ri[3], int *list)
+{
+    int n = 0;
+    if (c->nl) for (int I = 0; I < c->n_nuc; ++I) if (c->nl[7 * I] > 0.0 && dist(ri, c->Rn + 3 * I) < c->nl[7 * I]) list[n++] = I;
+    return n;
+}
+
+int ref_nl_slot(const lrdmc_ref_ctx *c, const double *x, const double U[9], int j, int *i_out, double rp[3], double *nu)
+{
+    int s = (j - c->P_lat) / 6, q = (j - c->P_lat) % 6, i = s / c->nl_K, kk = s % c->nl_K;
+    int *list = (int *)malloc(sizeof(int) * (size_t)c->n_nuc);
+    int n = nl_in_range(c, x + 3 * i, list), I = kk < n ? list[kk] : -1;
+    free(list);
+    *i_out = i;
+    if (I < 0) return 0;
+    const double *ri = x + 3 * i, *RI = c->Rn + 3 * I, *par = c->nl + 7 * I;
+    double r = dist(ri, RI);
+    int k = q / 2; double sgn = (q % 2 == 0) ? 1.0 : -1.0;
+    double e[3] = { U[k], U[3 + k], U[6 + k] };                       /* versor k = column k of the frame */
+    for (int ax = 0; ax < 3; ++ax) rp[ax] = RI[ax] + sgn * r * e[ax];  /* quadrature point on the sphere |r' - R_I| = r_iI */
+    double ct = sgn * (e[0] * (ri[0] - RI[0]) + e[1] * (ri[1] - RI[1]) + e[2] * (ri[2] - RI[2])) / r;   /* cos(theta_q) */
+    double P[3] = { 1.0, ct, 0.5 * (3.0 * ct * ct - 1.0) }, v = 0.0;   /* Legendre P_0, P_1, P_2 */
+    for (int l = 0; l < 3; ++l) v += (2 * l + 1) * par[1 + 2 * l] * exp(-par[2 + 2 * l] * r * r) * P[l];
+    *nu = v / 6.0;                                                     /* octahedral rule: six points, weight 1/6 each */
+    return 1;
+}
+
+/* rho_q: determinant ratio (dla) or full wavefunction ratio of moving electron i to rp */
+static double nl_ratio(const lrdmc_ref_ctx *c, const double *x, const double *const dinv[2], int i, const double rp[3])
+{
+    int spin = ref_spin(c, i), il = ref_local(c, i), O = ref_nocc(c, spin);
+    double phi[REF_MAX_OCC];
+    lrdmc_ref_mo(c, spin, rp, phi, NULL, NULL);
+    double dr = 0.0; for (int m = 0; m < O; ++m) dr += phi[m] * dinv[spin][m * O + il];
+    if (c->nl_dla) return dr;                                          /* D_G(x')/D_G(x), L576 */
+    return dr * exp(jastrow_of_electron(c, x, i, rp) - jastrow_of_electron(c, x, i, x + 3 * i));
+}
+
+int lrdmc_ref_nl_info(const lrdmc_ref_ctx *c, const double *x, const double *dinv_up, const double *dinv_dn, const double U[9],
+                      double *nu, double *rho, double *cand)
+{
+    const double *dinv[2] = { dinv_up, dinv_dn };
+    for (int j = c->P_lat; j < c->P; ++j) {
+        int i, o = j - c->P_lat; double rp[3] = { 0, 0, 0 }, v = 0.0;
+        int act = ref_nl_slot(c, x, U, j, &i, rp, &v);
+        nu[o] = act ? v : 0.0; rho[o] = act ? nl_ratio(c, x, dinv, i, rp) : 0.0;
+        if (cand) { cand[3 * o] = rp[0]; cand[3 * o + 1] = rp[1]; cand[3 * o + 2] = rp[2]; }
+    }
+    return LRDMC_REF_OK;
+}
+
 int lrdmc_ref_evaluate(const lrdmc_ref_ctx *c, const double *x, const double *dinv_up_in, const double *dinv_dn_in,
                        const double U[9], double *R, double *scal, double *per, double *cand)
 {
-    int N = c->N, P = c->P;
+    int N = c->N, P = c->P_lat;
     double *own = NULL; const double *dinv[2] = { dinv_up_in, dinv_dn_in };
     if (!dinv_up_in) {
         own = (double *)calloc((size_t)(c->n_up * c->n_up + c->n_dn * c->n_dn + 1), sizeof(double));
@@ -79,6 +132,28 @@ int lrdmc_ref_evaluate(const lrdmc_ref_ctx *c, const double *x, const double *di
         Kdiag += kap;                                   /* K^a_{x,x} = sum_j kappa_j = 3N/a^2 (Eq.D5) */
         if (R[j] > 0.0) bbar += kap * R[j];             /* bbar_x of Eq.29 (L199), summed in index order */
         else if (R[j] < 0.0) { Vsf -= kap * R[j]; node = 1; }
+    }
+    /* --- non-local pseudopotential candidates (f1): amplitude -nu_q rho_q; fixed node by the sign of H_{x',x} Psi'/Psi
+     *     (Eq.D1 "for the non-local pseudopotentials ... chosen simply to guarantee the non-negativity");
+     *     the D11 trigger looks at the wavefunction sign, rho_q < 0 ("(and ECP)", L625-L628) */
+    double enl = 0.0;
+    if (c->P > c->P_lat) {
+        int *list = (int *)malloc(sizeof(int) * (size_t)c->n_nuc);
+        for (int i = 0; i < N; ++i) if (nl_in_range(c, x + 3 * i, list) > c->nl_K) { free(list); free(own); return LRDMC_REF_EINVAL; }
+        free(list);
+        for (int j = c->P_lat; j < c->P; ++j) {
+            int i; double rp[3] = { 0, 0, 0 }, nu = 0.0;
+            R[j] = 0.0;
+            if (cand) { cand[3 * j] = cand[3 * j + 1] = cand[3 * j + 2] = 0.0; }
+            if (!ref_nl_slot(c, x, U, j, &i, rp, &nu)) continue;
+            if (cand) { cand[3 * j] = rp[0]; cand[3 * j + 1] = rp[1]; cand[3 * j + 2] = rp[2]; }
+            double rho = nl_ratio(c, x, dinv, i, rp);
+            R[j] = -nu * rho;
+            enl += nu * rho;                            /* V_nl Psi / Psi on the quadrature (its share of e_L, Eq.D7) */
+            if (R[j] > 0.0) bbar += R[j];               /* allowed non-local hop: G = -H_{x',x} rho */
+            else if (R[j] < 0.0) Vsf -= R[j];           /* s_{x',x} > 0: localised into V_sf (Eq.D1) */
+            if (rho < 0.0) node = 1;
+        }
     }
     /* --- step 4: per electron, continuum pieces and the regularised electron-ion potential (D6-D11) */
     double Vee = 0.0, sum_vopt = 0.0, eL_cont = 0.0; int n_vmax = 0;
@@ -129,7 +204,7 @@ int lrdmc_ref_evaluate(const lrdmc_ref_ctx *c, const double *x, const double *di
      *     and local energy e_L = -bbar + W (L223) */
     double W = Kdiag + sum_vopt + Vee + c->V_ii + Vsf;
     scal[0] = bbar; scal[1] = Vsf; scal[2] = W; scal[3] = -bbar + W; scal[4] = node; scal[5] = Vee; scal[6] = c->V_ii;
-    scal[7] = Kdiag; scal[8] = n_vmax; scal[9] = eL_cont + Vee + c->V_ii;   /* right-hand side of Eq.D7 (L604) */
+    scal[7] = Kdiag; scal[8] = n_vmax; scal[9] = eL_cont + Vee + c->V_ii + enl;   /* right-hand side of Eq.D7 (L604) */
     free(own);
     return LRDMC_REF_OK;
 }
@@ -140,14 +215,14 @@ int lrdmc_ref_evaluate(const lrdmc_ref_ctx *c, const double *x, const double *di
  * margin = min_j |t - C_j| / C_{P-1}: how close the draw came to a bin edge (near-tie report, Q12). */
 int lrdmc_ref_select(const lrdmc_ref_ctx *c, const double *R, double u_sel, double *margin)
 {
-    int P = c->P, N = c->N, jstar = -1, last = -1;
+    int P = c->P, jstar = -1, last = -1;
     double tot = 0.0;
-    for (int j = 0; j < P; ++j) if (R[j] > 0.0) { tot += c->kappa[j / (6 * N)] * R[j]; last = j; }
+    for (int j = 0; j < P; ++j) if (R[j] > 0.0) { tot += ref_kappa(c, j) * R[j]; last = j; }
     if (margin) *margin = 1.0;
     if (last < 0) return -1;
     double t = u_sel * tot, C = 0.0, mg = 1.0;
     for (int j = 0; j < P; ++j) {
-        if (R[j] > 0.0) C += c->kappa[j / (6 * N)] * R[j];
+        if (R[j] > 0.0) C += ref_kappa(c, j) * R[j];
         if (jstar < 0 && C > t) jstar = j;
         double dm = fabs(t - C) / tot; if (dm < mg) mg = dm;
     }

@@ -20,7 +20,11 @@ struct lrdmc_ref_ctx {
     double a_par, a_anti, b2; double *c1, *b1; /* c1 NULL: no one-body term */
     /* lattice */
     double a, a2; int n_mesh; double amesh[2], gmesh[2], kappa[2]; /* kappa_m = g_m / (2 a_m^2) */
-    int P;                           /* 6 N n_mesh candidates */
+    int P;                           /* all candidates: P_lat lattice hops + 6 N nl_K non-local slots */
+    int P_lat;                       /* 6 N n_mesh lattice hops (Eq.D4) */
+    /* non-local (semi-local) pseudopotential channels, section 8(f) f1 (L242, L567, L576): per nucleus
+     * nl[I][7] = { r_c, A_0, B_0, A_1, B_1, A_2, B_2 }: v_l(r) = A_l exp(-B_l r^2) for r < r_c; r_c <= 0: none */
+    int nl_K, nl_dla; double *nl;
     uint64_t seed;
     double V_ii;
     /* walkers */
@@ -36,12 +40,16 @@ static inline int ref_spin(const lrdmc_ref_ctx *c, int i) { return i < c->n_up ?
 static inline int ref_local(const lrdmc_ref_ctx *c, int i) { return i < c->n_up ? i : i - c->n_up; }
 
 /* candidate j -> (mesh block, electron, direction d in 0..5); displacement sign and versor index */
+static inline double ref_kappa(const lrdmc_ref_ctx *c, int j) { return j < c->P_lat ? c->kappa[j / (6 * c->N)] : 1.0; }
 static inline void ref_cand(const lrdmc_ref_ctx *c, int j, int *mesh, int *i, int *d)
 {
     *mesh = j / (6 * c->N); j -= *mesh * 6 * c->N; *i = j / 6; *d = j % 6;
 }
 
 int ref_invert(int n, const double *A /*[n][n] row-major*/, double *Ainv, double *logabs, int *sign);
+/* non-local slot j >= P_lat of configuration x in frame U: electron, target point, amplitude nu_q = V^nl_{x',x};
+ * returns 0 if the slot is inactive (fewer than kk+1 centres in range) */
+int ref_nl_slot(const lrdmc_ref_ctx *c, const double *x, const double U[9], int j, int *i_out, double rp[3], double *nu);
 void ref_apply_move(const lrdmc_ref_ctx *c, double *x, double *dinv_up, double *dinv_dn, int i, const double rnew[3]);
 
 #endif

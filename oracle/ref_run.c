@@ -35,7 +35,7 @@ int lrdmc_ref_create(lrdmc_ref_ctx **out, int n_nuc, const double *Z, const doub
     c->a = a; c->a2 = a2; c->n_mesh = a2 > 0.0 ? 2 : 1;
     c->amesh[0] = a; c->amesh[1] = a2; c->gmesh[0] = a2 > 0.0 ? 0.5 : 1.0; c->gmesh[1] = a2 > 0.0 ? 0.5 : 0.0;
     for (int m = 0; m < c->n_mesh; ++m) c->kappa[m] = c->gmesh[m] / (2.0 * c->amesh[m] * c->amesh[m]);
-    c->P = 6 * c->N * c->n_mesh; c->seed = seed;
+    c->P_lat = 6 * c->N * c->n_mesh; c->P = c->P_lat; c->seed = seed;
     c->V_ii = 0.0;
     for (int I = 0; I < n_nuc; ++I) for (int J = I + 1; J < n_nuc; ++J) {
         double dx = Rnuc[3 * I] - Rnuc[3 * J], dy = Rnuc[3 * I + 1] - Rnuc[3 * J + 1], dz = Rnuc[3 * I + 2] - Rnuc[3 * J + 2];
@@ -58,10 +58,20 @@ void lrdmc_ref_destroy(lrdmc_ref_ctx *c)
     if (!c) return;
     free_walkers(c);
     free(c->Z); free(c->Rn); free(c->pp); free(c->center); free(c->type); free(c->zeta); free(c->ao0);
-    free(c->C_up); free(c->C_dn); free(c->c1); free(c->b1); free(c);
+    free(c->C_up); free(c->C_dn); free(c->c1); free(c->b1); free(c->nl); free(c);
 }
 
 int lrdmc_ref_n_candidates(const lrdmc_ref_ctx *c) { return c->P; }
+
+int lrdmc_ref_set_nonlocal(lrdmc_ref_ctx *c, int K, int dla, const double *nl)
+{
+    if (!c || K < 0 || (K > 0 && !nl) || c->n_w) return LRDMC_REF_EINVAL;
+    free(c->nl); c->nl = NULL; c->nl_K = 0; c->P = c->P_lat;
+    if (K == 0) return LRDMC_REF_OK;
+    c->nl = dupd(nl, 7 * (size_t)c->n_nuc); c->nl_K = K; c->nl_dla = dla ? 1 : 0;
+    c->P = c->P_lat + 6 * c->N * K;
+    return LRDMC_REF_OK;
+}
 
 int lrdmc_ref_set_threads(int n)
 {
@@ -141,6 +151,7 @@ int lrdmc_ref_get_obs(const lrdmc_ref_ctx *c, double *eL, double *W, double *ome
 /* candidate j of walker position x in frame U -> new position of its electron */
 static void cand_pos(const lrdmc_ref_ctx *c, const double *x, const double U[9], int j, int *i_out, double rp[3])
 {
+    if (j >= c->P_lat) { double nu; ref_nl_slot(c, x, U, j, i_out, rp, &nu); return; }   /* non-local hop onto the quadrature point */
     int mesh, i, d; ref_cand(c, j, &mesh, &i, &d);
     int k = d / 2; double step = ((d % 2 == 0) ? 1.0 : -1.0) * c->amesh[mesh];
     rp[0] = x[3 * i] + step * U[k]; rp[1] = x[3 * i + 1] + step * U[3 + k]; rp[2] = x[3 * i + 2] + step * U[6 + k];

@@ -47,6 +47,7 @@ def _system(name, Z, R, n_up, n_dn, center, stype, zeta, C_up, C_dn, jastrow, a,
         b1=None if jastrow.get("b1") is None else np.ascontiguousarray(jastrow["b1"], dtype=np.float64),
         a=float(a), a2=float(a2), seed=int(seed),
         n_walkers=int(n_walkers), cycles=int(cycles), moves=int(moves),
+        nl=None, nl_K=0, nl_dla=1,      # non-local pseudopotential channels (scope row f1): see with_nonlocal
     )
     assert d["C_up"].shape == (d["n_ao"], d["n_up"])
     assert d["C_dn"].shape == (d["n_ao"], d["n_dn"])
@@ -206,6 +207,40 @@ def tiny_molecule(n_up=2, n_dn=1, n_nuc=2, n_shell=6, seed=7, a=0.2, a2=0.0, wit
     jas = dict(a_par=0.25, a_anti=0.5, b2=0.8, c1=c1, b1=rng.uniform(0.5, 1.5, size=n_nuc))
     return _system(f"tiny-{n_up}u{n_dn}d", Z, R, n_up, n_dn, center, stype, zeta, C_up, C_dn, jas, a,
                    a2=a2, pp=pp)
+
+
+def with_nonlocal(sysd, nl, dla=True):
+    """Attach non-local (semi-local) pseudopotential channels to a system (scope row f1).
+    nl [n_nuc][7] = (r_c, A_0, B_0, A_1, B_1, A_2, B_2): v_l(r) = A_l exp(-B_l r^2) inside r < r_c, r_c <= 0 = none.
+    nl_K = how many cutoff spheres can contain one point: the largest number of centres J (itself included) whose sphere
+    overlaps that of a centre I -- a property of the geometry, counted here, used as the slot count per electron."""
+    d = dict(sysd)
+    nl = np.ascontiguousarray(nl, dtype=np.float64).reshape(sysd["n_nuc"], 7)
+    rc = np.maximum(nl[:, 0], 0.0); R = sysd["R"]
+    K = 0
+    for I in range(sysd["n_nuc"]):
+        if rc[I] > 0.0:
+            K = max(K, int(sum(1 for J in range(sysd["n_nuc"]) if rc[J] > 0.0 and np.linalg.norm(R[I] - R[J]) < rc[I] + rc[J])))
+    d.update(nl=nl, nl_K=K, nl_dla=1 if dla else 0, name=sysd["name"] + ("-nlDLA" if dla else "-nlTM"))
+    return d
+
+
+def random_nonlocal(sysd, seed, r_c, l_max=2, dla=True, nuclei=None):
+    """Seeded synthetic channels: A_l uniform in [-Z, Z], B_l log-uniform in [2, 8], cutoff r_c on the chosen nuclei (default all)."""
+    rng = np.random.default_rng(seed)
+    n = sysd["n_nuc"]; nl = np.zeros((n, 7))
+    for I in (range(n) if nuclei is None else nuclei):
+        nl[I, 0] = r_c
+        for l in range(l_max + 1):
+            nl[I, 1 + 2 * l] = rng.uniform(-1.0, 1.0) * sysd["Z"][I]
+            nl[I, 2 + 2 * l] = np.exp(rng.uniform(np.log(2.0), np.log(8.0)))
+    return with_nonlocal(sysd, nl, dla)
+
+
+def water_methane_nonlocal(n_walkers=400, moves=100, dla=True, seed=PHILOX_RUN_SEED, a=0.2):
+    """C3 with s/p/d non-local channels of range 0.8 bohr on every nucleus (spheres disjoint: one slot per electron) -- the
+    shape of the paper's ccECP + DLA runs (L242); the channels themselves are synthetic."""
+    return random_nonlocal(water_methane(a=a, n_walkers=n_walkers, moves=moves, seed=seed), 33, 0.8, 2, dla)
 
 
 CONFIGS = {
