@@ -43,6 +43,18 @@ typedef struct {
     const double *pp; /* NULL = all bare nuclei; else [n_nuc][4] = (alpha,beta,gamma,delta) of the local
                          pseudopotential v(r) = -(Z/r)(1-e^{-alpha r^2}) + Z alpha r e^{-beta r^2} + gamma e^{-delta r^2}
                          (reading Q14); alpha <= 0 marks a bare -Z/r nucleus */
+    /* Non-local (semi-local) pseudopotential channels ("DLA", Eq.D1 "DTM", L625-L628):
+     * nl == NULL or nl_K == 0: none.  Else nl [n_nuc][7] = (r_c, A_0, B_0, A_1, B_1, A_2, B_2): channel l of nucleus I is
+     * v_l(r) = A_l exp(-B_l r^2) for r < r_c (r_c <= 0: no channels on that nucleus).  Each (electron i, centre I with
+     * r_iI < r_c) adds the six candidates x_q = "electron i at R_I +- r_iI e_k" (octahedral rule in the step's frame) with
+     * H_{x_q,x} = nu_q = (1/6) sum_l (2l+1) v_l(r_iI) P_l(cos theta_q) and rho_q = D(x_q)/D(x) (nl_dla != 0) or
+     * Psi_G(x_q)/Psi_G(x) (nl_dla == 0); nu_q rho_q < 0: hop with Green's function -nu_q rho_q, > 0: into V_sf (Eq.D1).
+     * nl_K = slots per electron = the largest number of cutoff spheres containing one point (1 <= nl_K <= 4; centres in range beyond the
+     * nl_K-th are ignored -- a wrong nl_K is a caller error).  Candidate order: after the
+     * 6 N n_mesh lattice hops, j = 6 N n_mesh + 6 (i nl_K + kk) + q, kk = rank of I among the centres in range (ascending),
+     * q = 2k (+e_k), 2k+1 (-e_k); R[j] of lrdmc_step_debug holds -nu_q rho_q there (0: empty slot). */
+    const double *nl;
+    int nl_K, nl_dla;
 } lrdmc_system;
 typedef struct {
     int n_shell;
@@ -72,7 +84,7 @@ int lrdmc_init(lrdmc_ctx **out, const lrdmc_system *, const lrdmc_basis *, const
                const lrdmc_lattice *);
 void lrdmc_free(lrdmc_ctx *);
 const char *lrdmc_strerror(int code);
-int lrdmc_n_candidates(const lrdmc_ctx *); /* P = 6 N n_mesh */
+int lrdmc_n_candidates(const lrdmc_ctx *); /* P = 6 N n_mesh + 6 N nl_K */
 
 /* ---- walker storage: structure of arrays in ONE caller-owned device buffer ---------------------------
  * positions (double-buffered for the branching gather), inverse Slater matrices per spin, cached MO

@@ -21,7 +21,8 @@ EXPORTS = ["lrdmc_init", "lrdmc_free", "lrdmc_strerror", "lrdmc_n_candidates", "
 
 
 class System(C.Structure):
-    _fields_ = [("n_nuc", C.c_int), ("Z", C.c_void_p), ("R", C.c_void_p), ("n_up", C.c_int), ("n_dn", C.c_int), ("pp", C.c_void_p)]
+    _fields_ = [("n_nuc", C.c_int), ("Z", C.c_void_p), ("R", C.c_void_p), ("n_up", C.c_int), ("n_dn", C.c_int), ("pp", C.c_void_p),
+                ("nl", C.c_void_p), ("nl_K", C.c_int), ("nl_dla", C.c_int)]
 
 
 class Basis(C.Structure):
@@ -136,10 +137,11 @@ class Lrdmc:
         self.sysd = sysd
         self.N = sysd["n_up"] + sysd["n_dn"]; self.n_up = sysd["n_up"]; self.n_dn = sysd["n_dn"]
         k = {n: (None if sysd.get(n) is None else np.ascontiguousarray(sysd[n])) for n in
-             ("Z", "R", "pp", "shell_center", "shell_type", "shell_zeta", "C_up", "C_dn", "c1", "b1")}
+             ("Z", "R", "pp", "shell_center", "shell_type", "shell_zeta", "C_up", "C_dn", "c1", "b1", "nl")}
         self._keep = k
         p = lambda a: None if a is None else a.ctypes.data
-        s = System(sysd["n_nuc"], p(k["Z"]), p(k["R"]), sysd["n_up"], sysd["n_dn"], p(k["pp"]))
+        s = System(sysd["n_nuc"], p(k["Z"]), p(k["R"]), sysd["n_up"], sysd["n_dn"], p(k["pp"]),
+                   p(k["nl"]), int(sysd.get("nl_K", 0) or 0), int(sysd.get("nl_dla", 1)))
         b = Basis(sysd["n_shell"], p(k["shell_center"]), p(k["shell_type"]), p(k["shell_zeta"]))
         m = Mo(sysd["n_ao"], p(k["C_up"]), p(k["C_dn"]))
         j = Jastrow(sysd["a_par"], sysd["a_anti"], sysd["b2"], p(k["c1"]), p(k["b1"]))

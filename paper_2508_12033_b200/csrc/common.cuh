@@ -22,12 +22,15 @@
 #ifndef LRDMC_BC_DMMA
 #define LRDMC_BC_DMMA 1         // Bc = C Dinv of the column form on the FP64 tensor pipe (0: DFMA chains over the mo_pass fragments)
 #endif
-#define LRDMC_NUC_STRIDE 12  // doubles per nucleus row: Rx Ry Rz Z c1 b1 alpha beta gamma delta is_pp pad
+#define LRDMC_NUC_STRIDE 20  // doubles per nucleus row: Rx Ry Rz Z c1 b1 alpha beta gamma delta is_pp pad | r_c A0 B0 A1 B1 A2 B2 pad (non-local channels)
+#define LRDMC_NL_OFF 12      // first non-local entry of a nucleus row
+#define LRDMC_NL_MAX_K 4
 #define LRDMC_EL_ARRAYS 4     // per-electron scratch arrays in shared memory: Jold, lap, s_k, old column
 
 // Everything a kernel needs to know about the system; passed by value (fits the 4 KB parameter space).
 struct DevSys {
-    int N, n_up, n_dn, n_nuc, P, n_mesh;
+    int N, n_up, n_dn, n_nuc, P, n_mesh;   // P = all candidates = P_lat + 6 N nl_K
+    int P_lat, nl_K, nl_dla;               // 6 N n_mesh lattice hops; non-local pseudopotential slots per electron (0: none); determinant-locality flag
     int n_it[4];          // DMMA k-iterations (4 shells each) per shell group: 0 Slater-s, 1 s, 2 p, 3 d
     int n_slots;          // 4 * sum n_it  (sorted + padded shell list)
     int n_ksteps;         // n_it[0] + n_it[1] + 3 n_it[2] + 6 n_it[3]  = (padded AO count)/4
@@ -63,6 +66,7 @@ struct TeamPlan {
     int lpe;              // lanes per electron in phase A (power of two, 2..32)
     int nblk[2];          // 8-electron blocks per spin
     int n_units;          // n_mesh (nblk[0] + nblk[1]) NP
+    int nblk_nl[2], n_units_nl, o_nl, o_nu;   // non-local slot blocks (8 slots) per spin, their units, scratch offsets (partials, nu_q)
     int it_base[4];       // first 4-shell iteration of each shell group
     int kstep_base[4];    // first mma k-step of each group in the `bf` fragment table
     int pair_base[4];     // first k-step pair of each group in the `cf` fragment table

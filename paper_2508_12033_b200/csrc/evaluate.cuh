@@ -57,21 +57,111 @@ __device__ __forceinline__ void pade_six(double dx, double dy, double dz, const 
     }
 }
 
+// ---- non-local pseudopotential candidates (scope row f1; include/lrdmc.h lrdmc_system.nl) ------------------------------
+// The kk-th centre in range of the point (x,y,z): nuclei with r_c > 0 and |r - R_I| < r_c in ascending order.  Returns its index
+// (-1: fewer than kk+1 in range) and the distance.  Every lane runs the same loop on the same data (uniform result).
+__device__ __forceinline__ int nl_centre(const DevSys &S, const double *nuc, double x, double y, double z, int kk, double &r_out)
+{
+    int seen = 0;
+    for (int I = 0; I < S.n_nuc; ++I) {
+        const double *nu = nuc + I * LRDMC_NUC_STRIDE, rc = nu[LRDMC_NL_OFF];
+        if (!(rc > 0.0)) continue;
+        const double dx = x - nu[0], dy = y - nu[1], dz = z - nu[2], r = sqrt(dx * dx + dy * dy + dz * dz);
+        if (r < rc) { if (seen == kk) { r_out = r; return I; } ++seen; }
+    }
+    r_out = 0.0;
+    return -1;
+}
+
+// One pass over 8 non-local slots of spin sp (slot = (electron il, rank kk), lane = 4 g + t handles slot s0 + g): the six
+// quadrature points R_I +- r_iI e_k have exactly the +-(a e_k) structure of the lattice hops about the CENTRE R_I with step
+// r_iI, so the determinant ratios come from the same ao_columns (per-lane x0 = R_I, av = r_iI e_k, a2 = r_iI^2), and the
+// Jastrow ratios (nl_dla == 0) from the same pade_six.  nu_q = (1/6) sum_l (2l+1) v_l(r) P_l(+-e_k . rhat).
+// Output (lanes t == 0 of valid slots): acc6 = determinant-ratio share of this shell part, jn6 = Jastrow share, nu6.
+// Returns false (nothing computed) when no slot of the pass is active.
+template <int NT, bool TS, bool PART>
+__device__ __forceinline__ bool nl_pass(const DevSys &S, const WarpState &ws, const Tables &T, int sp, int s0, int lane,
+                                        double (&acc)[6], double (&Jn)[6], double (&nuq)[6], bool &valid, bool &active, int &i_out, int &slot_out,
+                                        const TeamPlan *tp = nullptr, const ShellPart *part = nullptr, int jpart = 0, int jparts = 1)
+{
+    const int t = lane & 3, g = lane >> 2, K = S.nl_K;
+    const int ns = sp ? S.n_dn : S.n_up, off = sp ? S.n_up : 0;
+    valid = s0 + g < ns * K;
+    const int sidx = valid ? s0 + g : 0, il = sidx / K, kk = sidx - il * K, i = off + il;
+    i_out = i; slot_out = i * K + kk;
+    const double xi = ws.r[3 * i], yi = ws.r[3 * i + 1], zi = ws.r[3 * i + 2];
+    double r;
+    const int I = valid ? nl_centre(S, T.nuc, xi, yi, zi, kk, r) : -1;
+    active = I >= 0;
+    if (!__any_sync(0xffffffffu, active)) return false;
+    const double *nu = T.nuc + (active ? I : 0) * LRDMC_NUC_STRIDE;
+    const double x0 = active ? nu[0] : xi, y0 = active ? nu[1] : yi, z0 = active ? nu[2] : zi;
+    const double rr = active ? r : 0.0, a2 = rr * rr;
+    double av[3][3];                                             // av[k] = r_iI e_k
+#pragma unroll
+    for (int k = 0; k < 3; ++k) { av[k][0] = rr * ws.U[k]; av[k][1] = rr * ws.U[3 + k]; av[k][2] = rr * ws.U[6 + k]; }
+    ao_columns<NT, TS, PART>(S, T.shells, sp ? T.cf[1] : T.cf[0], T.etab, sp ? ws.dinv[1] : ws.dinv[0], ns, il, x0, y0, z0, av, a2, lane, acc, tp, part);
+#pragma unroll
+    for (int d = 0; d < 6; ++d) { Jn[d] = 0.0; nuq[d] = 0.0; }
+    if (!S.nl_dla) {                                             // full ratio: Jastrow part at the quadrature points
+        if (S.has_j1) for (int Ip = t + 4 * jpart; Ip < S.n_nuc; Ip += 4 * jparts) {
+            const double *np_ = T.nuc + Ip * LRDMC_NUC_STRIDE;
+            pade_six(x0 - np_[0], y0 - np_[1], z0 - np_[2], av, a2, -np_[4], np_[5], Jn);
+        }
+        for (int j = t + 4 * jpart; j < S.N; j += 4 * jparts) {
+            const double c = (j == i) ? 0.0 : ((spin_of(S, j) == sp) ? S.a_par : S.a_anti);
+            pade_six(x0 - ws.r[3 * j], y0 - ws.r[3 * j + 1], z0 - ws.r[3 * j + 2], av, a2, c, S.b2, Jn);
+        }
+    }
+    if (active) {
+        const double ir = 1.0 / r, hx = (xi - nu[0]) * ir, hy = (yi - nu[1]) * ir, hz = (zi - nu[2]) * ir;   // rhat of the electron about the centre
+        const double r2 = r * r, *ch = nu + LRDMC_NL_OFF;
+        const double v0 = ch[1] * exp_nonpos(-ch[2] * r2), v1 = 3.0 * ch[3] * exp_nonpos(-ch[4] * r2), v2 = 5.0 * ch[5] * exp_nonpos(-ch[6] * r2);
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            const double ct = ws.U[k] * hx + ws.U[3 + k] * hy + ws.U[6 + k] * hz, p2 = 0.5 * (3.0 * ct * ct - 1.0);
+            nuq[2 * k] = (v0 + v1 * ct + v2 * p2) * (1.0 / 6.0);
+            nuq[2 * k + 1] = (v0 - v1 * ct + v2 * p2) * (1.0 / 6.0);
+        }
+    }
+    return true;
+}
+
+// Position an accepted move j puts its electron at: lattice hop r_i +- a e_k, or the quadrature point of a non-local slot.
+__device__ __forceinline__ void move_target(const DevSys &S, const WarpState &ws, const double *nuc, int j, int &i, double &px, double &py, double &pz)
+{
+    const int N = S.N;
+    if (j < S.P_lat) {
+        const int mesh = j / (6 * N), jj = j - mesh * 6 * N, d = jj - 6 * (jj / 6), k = d >> 1;
+        i = jj / 6;
+        const double step = (d & 1) ? -S.amesh[mesh] : S.amesh[mesh];
+        px = ws.r[3 * i] + step * ws.U[k]; py = ws.r[3 * i + 1] + step * ws.U[3 + k]; pz = ws.r[3 * i + 2] + step * ws.U[6 + k];
+    } else {
+        const int o = j - S.P_lat, slot = o / 6, q = o - 6 * slot, k = q >> 1, kk = slot % S.nl_K;
+        i = slot / S.nl_K;
+        double r;
+        const int I = nl_centre(S, nuc, ws.r[3 * i], ws.r[3 * i + 1], ws.r[3 * i + 2], kk, r);
+        const double *nu = nuc + (I < 0 ? 0 : I) * LRDMC_NUC_STRIDE, step = (q & 1) ? -r : r;
+        px = nu[0] + step * ws.U[k]; py = nu[1] + step * ws.U[3 + k]; pz = nu[2] + step * ws.U[6 + k];
+    }
+}
+
 // Phase C (row a7) of one evaluation, by one warp on the candidate ratios R[P] left in shared memory.
-__device__ __forceinline__ EvalOut phase_c(const DevSys &S, const WarpState &ws, const double *lap_s, double Vee, int lane)
+// node0: node flag already raised by the non-local candidates (rho_q < 0), any lane.
+__device__ __forceinline__ EvalOut phase_c(const DevSys &S, const WarpState &ws, const double *lap_s, double Vee, int lane, int node0 = 0)
 {
     const int N = S.N;
     // ---- phase C (row a7): fixed-node split (Eq.D1) and the cumulative sums C_j of the allowed amplitudes in candidate
     //      order (row a9 searches them).  Each lane owns a contiguous chunk; chunk totals are scanned across the warp
     //      (reading Q12: the summation order is free, a draw closer than 1e-9 to a bin edge is a reported near-tie).
     const int P = S.P, chunk = (P + 31) >> 5, j0 = lane * chunk;
-    double vsf_part = 0.0, loc = 0.0; int node = 0;
+    double vsf_part = 0.0, loc = 0.0; int node = node0;
     for (int e = 0; e < chunk; ++e) {
         const int j = j0 + e;
         if (j < P) {
-            const double Rj = ws.R[j], kap = S.kappa[j >= 6 * N ? 1 : 0];
+            const double Rj = ws.R[j], kap = j < 6 * N ? S.kappa[0] : (j < S.P_lat ? S.kappa[1] : 1.0);   // non-local slots hold -nu_q rho_q itself
             if (Rj > 0.0) loc += kap * Rj;
-            else if (Rj < 0.0) { vsf_part -= kap * Rj; node = 1; }
+            else if (Rj < 0.0) { vsf_part -= kap * Rj; if (j < S.P_lat) node = 1; }
             ws.cum[j] = loc;
         }
     }
@@ -248,9 +338,32 @@ __device__ __forceinline__ EvalOut evaluate_walker(const DevSys &S, const WarpSt
         }
     }
 #endif
+    // ---- non-local pseudopotential slots (row f1): 8 slots per warp pass, whole shell list
+    int node_nl = 0;
+    if (S.nl_K) {
+        for (int sp = 0; sp < 2; ++sp) {
+            const int nslot = (sp ? S.n_dn : S.n_up) * S.nl_K;
+            for (int s0 = 0; s0 < nslot; s0 += 8) {
+                double acc[6], Jn[6], nuq[6]; bool valid, active; int i, slot;
+                const bool any = nl_pass<NT, TS, false>(S, ws, T, sp, s0, lane, acc, Jn, nuq, valid, active, i, slot);
+                double *Ro = ws.R + S.P_lat + 6 * slot;
+                if (!any) { if (valid && t == 0) {
+#pragma unroll
+                        for (int d = 0; d < 6; ++d) Ro[d] = 0.0; }
+                    continue; }
+                const double Jo = Jold[i];
+#pragma unroll
+                for (int d = 0; d < 6; ++d) {
+                    double rho = quad_sum(acc[d]);
+                    if (!S.nl_dla) rho *= exp_tab(quad_sum(Jn[d]) - Jo, T.etab);
+                    if (valid && t == 0) { Ro[d] = active ? -nuq[d] * rho : 0.0; if (active && rho < 0.0) node_nl = 1; }
+                }
+            }
+        }
+    }
     __syncwarp();
 
-    const EvalOut o = phase_c(S, ws, lap_s, Vee, lane);
+    const EvalOut o = phase_c(S, ws, lap_s, Vee, lane, node_nl);
     __syncwarp();
     return o;
 }
@@ -280,10 +393,9 @@ __device__ __forceinline__ int select_move(const DevSys &S, const WarpState &ws,
 template <int NT, bool TS>
 __device__ __forceinline__ void apply_move(const DevSys &S, const WarpState &ws, const Tables &T, int j, int lane)
 {
-    const int N = S.N, mesh = j / (6 * N), jj = j - mesh * 6 * N, i = jj / 6, d = jj - 6 * i, k = d >> 1;
+    const int N = S.N; int i; double px, py, pz;
+    move_target(S, ws, T.nuc, j, i, px, py, pz);
     const int sp = spin_of(S, i), il = sp ? i - S.n_up : i, ns = sp ? S.n_dn : S.n_up;
-    const double step = (d & 1) ? -S.amesh[mesh] : S.amesh[mesh];
-    const double px = ws.r[3 * i] + step * ws.U[k], py = ws.r[3 * i + 1] + step * ws.U[3 + k], pz = ws.r[3 * i + 2] + step * ws.U[6 + k];
     double *mc = ws.moc + (size_t)i * 5 * S.OS;
     __syncwarp();
     refresh_mo_cache<NT, TS>(S, T.shells, sp ? T.bf[1] : T.bf[0], T.etab, mc, px, py, pz, lane);

@@ -72,13 +72,16 @@ extern "C" int lrdmc_init(lrdmc_ctx **out, const lrdmc_system *sys, const lrdmc_
     lrdmc_ctx *c = (lrdmc_ctx *)calloc(1, sizeof(lrdmc_ctx));
     DevSys &S = c->S;
     S.N = sys->n_up + sys->n_dn; S.n_up = sys->n_up; S.n_dn = sys->n_dn; S.n_nuc = sys->n_nuc;
-    S.n_mesh = lat->a2 > 0.0 ? 2 : 1; S.P = 6 * S.N * S.n_mesh; S.a = lat->a;
+    S.n_mesh = lat->a2 > 0.0 ? 2 : 1; S.P_lat = 6 * S.N * S.n_mesh; S.a = lat->a;
+    S.nl_K = (sys->nl && sys->nl_K > 0) ? sys->nl_K : 0; S.nl_dla = sys->nl_dla ? 1 : 0;
+    if (S.nl_K > LRDMC_NL_MAX_K) { free(c); return LRDMC_EINVAL; }
+    S.P = S.P_lat + 6 * S.N * S.nl_K;
     S.amesh[0] = lat->a; S.amesh[1] = lat->a2; S.gmesh[0] = S.n_mesh == 2 ? 0.5 : 1.0; S.gmesh[1] = S.n_mesh == 2 ? 0.5 : 0.0;
     S.Kdiag = 0.0;
     for (int m = 0; m < S.n_mesh; ++m) {
         S.kappa[m] = S.gmesh[m] / (2.0 * S.amesh[m] * S.amesh[m]); S.g_over_a2[m] = S.gmesh[m] / (S.amesh[m] * S.amesh[m]);
     }
-    for (int j = 0; j < S.P; ++j) S.Kdiag += S.kappa[j / (6 * S.N)];      // K^a_{x,x} = sum_j kappa_j = 3N/a^2 (Eq.D5)
+    for (int j = 0; j < S.P_lat; ++j) S.Kdiag += S.kappa[j / (6 * S.N)];      // K^a_{x,x} = sum_j kappa_j = 3N/a^2 (Eq.D5)
     S.a_par = jas->a_par; S.a_anti = jas->a_anti; S.b2 = jas->b2; S.has_j1 = jas->c1 != NULL; S.has_pp = sys->pp != NULL;
     S.key0 = (uint32_t)lat->seed; S.key1 = (uint32_t)(lat->seed >> 32);
     S.V_ii = 0.0;
@@ -111,6 +114,7 @@ extern "C" int lrdmc_init(lrdmc_ctx **out, const lrdmc_system *sys, const lrdmc_
         double *nu = &h_nuc[(size_t)I * LRDMC_NUC_STRIDE];
         nu[0] = sys->R[3 * I]; nu[1] = sys->R[3 * I + 1]; nu[2] = sys->R[3 * I + 2]; nu[3] = sys->Z[I];
         nu[4] = jas->c1 ? jas->c1[I] : 0.0; nu[5] = jas->c1 ? (jas->b1 ? jas->b1[I] : 1.0) : 1.0;
+        if (S.nl_K) for (int q = 0; q < 7; ++q) nu[LRDMC_NL_OFF + q] = sys->nl[7 * I + q];
         if (sys->pp && sys->pp[4 * I] > 0.0) { nu[6] = sys->pp[4 * I]; nu[7] = sys->pp[4 * I + 1]; nu[8] = sys->pp[4 * I + 2]; nu[9] = sys->pp[4 * I + 3]; nu[10] = 1.0; }
     }
     const size_t bf_n = (size_t)S.n_ksteps * c->NT * 32;
@@ -205,7 +209,7 @@ extern "C" int lrdmc_init(lrdmc_ctx **out, const lrdmc_system *sys, const lrdmc_
     for (;;) {
         size_t need = ((size_t)S.tables_doubles + (size_t)c->wpb * S.per_warp_doubles) * 8;
         if ((need + reserve) * LRDMC_MINB <= per_sm || c->wpb == 1) { c->smem_bytes = (int)need; break; }
-        c->wpb >>= 1;
+        --c->wpb;
     }
     if ((size_t)c->smem_bytes > per_blk_max) { lrdmc_free(c); return LRDMC_ENOMEM; }
     for (int i = 0; i < 4; ++i) cudaEventCreate(&c->ev[i]);
@@ -326,7 +330,10 @@ static void plan_team(lrdmc_ctx *c, int n_w)
     const double cost_col[4] = { 2.0, 1.0, 1.7, 2.9 }, cost_mo[4] = { 1.5, 1.0, 3.0, 6.0 };
     partition_shells(S.n_it, cost_col, true, np, P.col);
     partition_shells(S.n_it, cost_mo, false, tw, P.mo);
-    const size_t scr_col = np > 1 ? (size_t)S.n_mesh * S.N * np * 12 : 0, scr_mo = (size_t)tw * 5 * S.OS;
+    P.nblk_nl[0] = (S.n_up * S.nl_K + 7) / 8; P.nblk_nl[1] = (S.n_dn * S.nl_K + 7) / 8; P.n_units_nl = (P.nblk_nl[0] + P.nblk_nl[1]) * np;
+    const size_t scr_lat = np > 1 ? (size_t)S.n_mesh * S.N * np * 12 : 0, scr_nl = np > 1 ? (size_t)S.N * S.nl_K * np * 12 : 0,
+                 scr_nu = np > 1 ? (size_t)S.N * S.nl_K * 7 : 0, scr_col = scr_lat + scr_nl + scr_nu, scr_mo = (size_t)tw * 5 * S.OS;
+    P.o_nl = (int)scr_lat; P.o_nu = (int)(scr_lat + scr_nl);
     P.o_scr = S.per_warp_doubles; P.scr_doubles = (int)align_up(scr_col > scr_mo ? scr_col : scr_mo, 2);
     const int smem = (int)(((size_t)S.tables_doubles + S.per_warp_doubles + P.scr_doubles) * 8);
     int occ = 0;

@@ -45,7 +45,7 @@ __device__ __forceinline__ void store_walker_team(const DevSys &S, const DevWalk
 // One evaluation by the team.  The result is valid in warp 0 only (it runs phase C); ws.R / ws.cum are complete for everyone
 // after the caller's next barrier.  s_vee: TW doubles of static shared memory.
 template <int NT, bool TS>
-__device__ __forceinline__ EvalOut evaluate_team(const DevSys &S, const TeamPlan &P, const WarpState &ws, const Tables &T, double *scr, double *s_vee)
+__device__ __forceinline__ EvalOut evaluate_team(const DevSys &S, const TeamPlan &P, const WarpState &ws, const Tables &T, double *scr, double *s_vee, int *s_node)
 {
     const int N = S.N, n_nuc = S.n_nuc, TW = P.TW, NP = P.NP, tid = threadIdx.x, nthr = blockDim.x, lane = tid & 31, wt = tid >> 5;
     const int t = lane & 3, g = lane >> 2;
@@ -95,7 +95,32 @@ __device__ __forceinline__ EvalOut evaluate_team(const DevSys &S, const TeamPlan
 
     // ---- phase B (rows a1-a5): work units (mesh, spin, 8-electron block, shell part); unit u -> warp u mod TW
     const int nb_mesh = P.nblk[0] + P.nblk[1];
-    for (int u = wt; u < P.n_units; u += TW) {
+    for (int v = wt; v < P.n_units + P.n_units_nl; v += TW) {
+        if (v >= P.n_units) {            // non-local pseudopotential slots (row f1): unit = (spin, 8-slot block, shell part)
+            const int u = v - P.n_units, part = u % NP, blk = u / NP, sp = blk >= P.nblk_nl[0] ? 1 : 0, s0 = 8 * (sp ? blk - P.nblk_nl[0] : blk);
+            double acc[6], Jn[6], nuq[6]; bool valid, active; int i, slot;
+            const bool any = nl_pass<NT, TS, true>(S, ws, T, sp, s0, lane, acc, Jn, nuq, valid, active, i, slot, &P, &P.col[part], part, NP);
+            if (NP == 1) {
+                double *Ro = ws.R + S.P_lat + 6 * slot;
+                const double Jo = Jold[i];
+#pragma unroll
+                for (int d = 0; d < 6; ++d) {
+                    double rho = any ? quad_sum(acc[d]) : 0.0;
+                    if (any && !S.nl_dla) rho *= exp_tab(quad_sum(Jn[d]) - Jo, T.etab);
+                    if (valid && t == 0) { Ro[d] = (any && active) ? -nuq[d] * rho : 0.0; if (any && active && rho < 0.0) atomicOr(s_node, 1); }
+                }
+            } else {
+                double *q = scr + P.o_nl + ((size_t)slot * NP + part) * 12, *qn = scr + P.o_nu + (size_t)slot * 7;
+#pragma unroll
+                for (int d = 0; d < 6; ++d) {
+                    const double A = any ? quad_sum(acc[d]) : 0.0, J = any ? quad_sum(Jn[d]) : 0.0;
+                    if (valid && t == 0) { q[d] = A; q[6 + d] = J; if (part == 0) qn[d] = (any && active) ? nuq[d] : 0.0; }
+                }
+                if (valid && t == 0 && part == 0) qn[6] = (any && active) ? 1.0 : 0.0;
+            }
+            continue;
+        }
+        const int u = v;
         const int part = u % NP, blk = u / NP, mesh = blk / nb_mesh, rem = blk - mesh * nb_mesh;
         const int sp = rem >= P.nblk[0] ? 1 : 0, il0 = 8 * (sp ? rem - P.nblk[0] : rem);
         const int ns = sp ? S.n_dn : S.n_up, off = sp ? S.n_up : 0;
@@ -139,12 +164,22 @@ __device__ __forceinline__ EvalOut evaluate_team(const DevSys &S, const TeamPlan
     }
     __syncthreads();
     if (NP > 1) {                      // the parts of a candidate meet: R = (sum of determinant shares) exp(sum of Jastrow shares - J_old)
-        for (int p = tid; p < S.P; p += nthr) {
+        for (int p = tid; p < S.P_lat; p += nthr) {
             const int mesh = p / (6 * N), rem = p - mesh * 6 * N, i = rem / 6, d = rem - 6 * i;
             const double *q = scr + (size_t)(mesh * N + i) * NP * 12;
             double A = 0.0, J = 0.0;
             for (int part = 0; part < NP; ++part) { A += q[part * 12 + d]; J += q[part * 12 + 6 + d]; }
             ws.R[p] = A * exp_tab(J - Jold[i], T.etab);
+        }
+        for (int p = S.P_lat + tid; p < S.P; p += nthr) {          // non-local slots: R = -nu_q rho_q
+            const int o = p - S.P_lat, slot = o / 6, d = o - 6 * slot, i = slot / S.nl_K;
+            const double *q = scr + P.o_nl + (size_t)slot * NP * 12, *qn = scr + P.o_nu + (size_t)slot * 7;
+            double A = 0.0, J = 0.0;
+            for (int part = 0; part < NP; ++part) { A += q[part * 12 + d]; J += q[part * 12 + 6 + d]; }
+            const bool active = qn[6] != 0.0;
+            const double rho = S.nl_dla ? A : A * exp_tab(J - Jold[i], T.etab);
+            ws.R[p] = active ? -qn[d] * rho : 0.0;
+            if (active && rho < 0.0) atomicOr(s_node, 1);
         }
         __syncthreads();
     }
@@ -152,7 +187,7 @@ __device__ __forceinline__ EvalOut evaluate_team(const DevSys &S, const TeamPlan
     if (wt == 0) {
         double Vee = 0.0;
         for (int w = 0; w < TW; ++w) Vee += s_vee[w];
-        o = phase_c(S, ws, lap_s, Vee, lane);
+        o = phase_c(S, ws, lap_s, Vee, lane, *s_node);
     }
     return o;
 }
@@ -163,10 +198,9 @@ template <int NT, bool TS>
 __device__ __forceinline__ void apply_move_team(const DevSys &S, const TeamPlan &P, const WarpState &ws, const Tables &T, double *scr, int j)
 {
     const int N = S.N, TW = P.TW, tid = threadIdx.x, nthr = blockDim.x, lane = tid & 31, wt = tid >> 5;   // warp 0 holds the lightest shell part (s shells): it also refreshes the one-body cache
-    const int mesh = j / (6 * N), jj = j - mesh * 6 * N, i = jj / 6, d = jj - 6 * i, k = d >> 1;
+    int i; double px, py, pz;
+    move_target(S, ws, T.nuc, j, i, px, py, pz);
     const int sp = spin_of(S, i), il = sp ? i - S.n_up : i, ns = sp ? S.n_dn : S.n_up;
-    const double step = (d & 1) ? -S.amesh[mesh] : S.amesh[mesh];
-    const double px = ws.r[3 * i] + step * ws.U[k], py = ws.r[3 * i + 1] + step * ws.U[3 + k], pz = ws.r[3 * i + 2] + step * ws.U[6 + k];
     double *mc = ws.moc + (size_t)i * 5 * S.OS;
     const int rows = 5 * S.OS;
     {
@@ -227,11 +261,11 @@ __global__ void __launch_bounds__(LRDMC_TEAM_MAX_WARPS * 32, 1) k_propagate_team
         double w = 1.0, tau_left = tau, omega = 0.0, eL_last = 0.0, W_last = 0.0; long long moves = 0; int n_node = 0, n_nonpos = 0;
         for (;;) {
             const StepDraws d = step_draws(S, (uint32_t)k, cycle, s, mode == LRDMC_CONVENTIONAL);
-            if (tid == 0) { double U[9]; lattice_frame(d.u1, d.u2, d.u3, U);
+            if (tid == 0) { s_ctrl[3] = 0; double U[9]; lattice_frame(d.u1, d.u2, d.u3, U);
 #pragma unroll
                 for (int i = 0; i < 9; ++i) ws.U[i] = U[i]; }
             __syncthreads();
-            const EvalOut e = evaluate_team<NT, TS>(S, P, ws, T, scr, s_vee);
+            const EvalOut e = evaluate_team<NT, TS>(S, P, ws, T, scr, s_vee, &s_ctrl[3]);
             if (wt == 0) {                                       // the leader warp keeps the weight (same rules as k_propagate)
                 n_node += e.node;
                 bool last = false;

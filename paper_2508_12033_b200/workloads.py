@@ -225,14 +225,15 @@ def with_nonlocal(sysd, nl, dla=True):
     return d
 
 
-def random_nonlocal(sysd, seed, r_c, l_max=2, dla=True, nuclei=None):
-    """Seeded synthetic channels: A_l uniform in [-Z, Z], B_l log-uniform in [2, 8], cutoff r_c on the chosen nuclei (default all)."""
+def random_nonlocal(sysd, seed, r_c, l_max=2, dla=True, nuclei=None, scale=1.0):
+    """Seeded synthetic channels: A_l uniform in [-Z, Z] x scale, B_l log-uniform in [2, 8], cutoff r_c on the chosen nuclei
+    (default all).  scale >> 1 makes the non-local hops as likely as the lattice ones (kappa = 1/2a^2): test systems only."""
     rng = np.random.default_rng(seed)
     n = sysd["n_nuc"]; nl = np.zeros((n, 7))
     for I in (range(n) if nuclei is None else nuclei):
         nl[I, 0] = r_c
         for l in range(l_max + 1):
-            nl[I, 1 + 2 * l] = rng.uniform(-1.0, 1.0) * sysd["Z"][I]
+            nl[I, 1 + 2 * l] = rng.uniform(-1.0, 1.0) * sysd["Z"][I] * scale
             nl[I, 2 + 2 * l] = np.exp(rng.uniform(np.log(2.0), np.log(8.0)))
     return with_nonlocal(sysd, nl, dla)
 

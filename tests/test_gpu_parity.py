@@ -45,6 +45,15 @@ SYSTEMS = {
     "C2-synthetic10": lambda: _with_walkers(wl.synthetic10(), 1024),          # BASELINE configs[1] at its full N_w
     "C3-water-methane-shaped": lambda: _with_walkers(wl.water_methane(n_walkers=100), 100),
     "C5-cluster64-doublemesh": lambda: _with_walkers(wl.cluster64(n_walkers=10), 10),   # 64 e, 600 AOs, a/a' (NT = 4, tables in global memory)
+    # scope row f1: non-local pseudopotential channels (synthetic), determinant locality (DLA) and full-ratio (T-move) forms
+    "hydrogen-nl-s-channel": lambda: (wl.with_nonlocal(wl.hydrogen(alpha=1.1), [[2.2, -0.8, 1.5, 0, 1, 0, 1]]), wl.hydrogen_walkers(100, 3)),
+    "tiny-3u2d-nlDLA-K2": lambda: _with_walkers(wl.random_nonlocal(wl.tiny_molecule(3, 2, 3, 9, seed=21, with_pp=True), 5, 1.6, 2, True), 37),
+    "tiny-3u2d-nlTM-K2": lambda: _with_walkers(wl.random_nonlocal(wl.tiny_molecule(3, 2, 3, 9, seed=21, with_pp=True), 5, 1.6, 2, False), 37),
+    "tiny-3u2d-nlDLA-strong": lambda: _with_walkers(wl.random_nonlocal(wl.tiny_molecule(3, 2, 3, 9, seed=21, with_pp=True), 5, 1.6, 2, True, scale=200.0), 37),
+    "tiny-2u1d-nlTM-strong": lambda: _with_walkers(wl.random_nonlocal(wl.tiny_molecule(2, 1, 2, 6, seed=7), 8, 1.4, 1, False, scale=600.0), 41),
+    "ragged-9u4d-nlDLA": lambda: _with_walkers(wl.random_nonlocal(wl.tiny_molecule(9, 4, 4, 20, seed=11), 6, 1.2, 2, True), 13),
+    "C3-water-methane-nlDLA": lambda: _with_walkers(wl.water_methane_nonlocal(n_walkers=100), 100),
+    "C3-water-methane-nlTM": lambda: _with_walkers(wl.water_methane_nonlocal(n_walkers=50, dla=False), 50),
 }
 
 
@@ -104,7 +113,9 @@ def test_one_evaluation_and_selection_from_the_oracle_state(B, name):
     for (E0, cycle, step) in ((-3.0, 0, 0), (0.5, 7, 3)):
         R, scal, js = o.step_debug(E0, cycle, step)
         gR, gscal, gjs = [np_(t) for t in g.lrdmc_step_debug(E0, cycle, step)]
-        assert gR.shape == R.shape == (len(x0), 6 * N * (2 if s["a2"] > 0 else 1))
+        assert gR.shape == R.shape == (len(x0), 6 * N * ((2 if s["a2"] > 0 else 1) + s["nl_K"]))
+        if s["nl_K"]:
+            assert np.count_nonzero(R[:, 6 * N * (2 if s["a2"] > 0 else 1):]) > 0        # the non-local slots are exercised
         Kdiag = scal[:, 2:3] * 0 + 3 * N * ((1 / s["a"]**2) if s["a2"] == 0 else (0.5 / s["a"]**2 + 0.5 / s["a2"]**2))
         assert relerr(gR, R, 1.0) < TOL                                                  # ratios
         for col, nm in ((0, "bbar"), (1, "V_sf"), (2, "W"), (3, "e_L")):
@@ -132,7 +143,9 @@ def test_whole_cycle_trajectories_weights_and_branching(B, name, mode, kernel, m
 @pytest.mark.parametrize("tw", [2, 4, 8, 16])
 @pytest.mark.parametrize("name,mode", [("tiny-3u3d-pp", "balanced"), ("tiny-2u2d-doublemesh", "conventional"), ("ragged-9u4d-NT2", "balanced"),
                                        ("ragged-17u3d-NT4", "conventional"), ("he-triplet-slater", "balanced"), ("C3-water-methane-shaped", "balanced"),
-                                       ("C3-water-methane-shaped", "conventional"), ("C5-cluster64-doublemesh", "balanced")])
+                                       ("C3-water-methane-shaped", "conventional"), ("C5-cluster64-doublemesh", "balanced"),
+                                       ("tiny-3u2d-nlDLA-strong", "balanced"), ("tiny-2u1d-nlTM-strong", "conventional"), ("C3-water-methane-nlDLA", "balanced"),
+                                       ("C3-water-methane-nlTM", "balanced")])
 def test_team_kernel_every_team_size(B, name, mode, tw, monkeypatch):
     """k_propagate_team with TW = 2, 4, 8, 16 warps per walker (work units = electron blocks x shell parts, partial sums
     in shared memory): same trajectories, weights and indices as the oracle."""
