@@ -1,6 +1,10 @@
 """Build liblrdmc.so in-tree with nvcc for sm_100a (cross-compiles without a GPU).
 
-    python -m paper_2508_12033_b200.build [--force]
+    python -m paper_2508_12033_b200.build [--force] [-v]
+
+Translation units (compiled in parallel, then linked): lrdmc.cu (C-ABI, host logic, rebuild / reconfigure / reduction kernels),
+lrdmc_aux.cu (estimators over generations, host-buffer driver, peak probes) and kernels.cu four times -- the walker kernels
+{lattice-only, with non-local pseudopotential slots} x {warp-per-walker, team}.
 """
 from __future__ import annotations
 
@@ -11,12 +15,18 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "liblrdmc.so")
-SOURCES = ["lrdmc.cu", "lrdmc_aux.cu"]
-NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC", "-shared"]
+OBJDIR = os.path.join(HERE, "build")
+# (source, object name, extra defines)
+UNITS = [("lrdmc.cu", "lrdmc.o", []), ("lrdmc_aux.cu", "lrdmc_aux.o", []),
+         ("kernels.cu", "kernels_lat_warp.o", ["-DLRDMC_NL=0", "-DLRDMC_TEAM_TU=0"]),
+         ("kernels.cu", "kernels_lat_team.o", ["-DLRDMC_NL=0", "-DLRDMC_TEAM_TU=1"]),
+         ("kernels.cu", "kernels_nl_warp.o", ["-DLRDMC_NL=1", "-DLRDMC_TEAM_TU=0"]),
+         ("kernels.cu", "kernels_nl_team.o", ["-DLRDMC_NL=1", "-DLRDMC_TEAM_TU=1"])]
+NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC"]
 
 
 def _deps():
-    out = [os.path.join(HERE, "..", "include", "lrdmc.h")]
+    out = [os.path.join(HERE, "..", "include", "lrdmc.h"), os.path.abspath(__file__)]
     for f in os.listdir(CSRC):
         if f.endswith((".cu", ".cuh", ".h")):
             out.append(os.path.join(CSRC, f))
@@ -28,8 +38,15 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if stale:
         nvcc = os.environ.get("NVCC", "nvcc")
         extra = os.environ.get("LRDMC_NVCC_EXTRA", "").split()       # tuning knobs, e.g. "-DLRDMC_WPB=16 -DLRDMC_MINB=1"
-        cmd = [nvcc] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + [os.path.join(CSRC, s) for s in SOURCES]
-        subprocess.run(cmd, check=True)
+        os.makedirs(OBJDIR, exist_ok=True)
+        procs = []
+        for src, obj, defs in UNITS:
+            cmd = [nvcc] + NVCC_FLAGS + extra + defs + (["-Xptxas", "-v"] if verbose else []) + ["-c", "-o", os.path.join(OBJDIR, obj), os.path.join(CSRC, src)]
+            procs.append((cmd, subprocess.Popen(cmd)))
+        failed = [cmd for cmd, p in procs if p.wait() != 0]
+        if failed:
+            raise subprocess.CalledProcessError(1, failed[0])
+        subprocess.run([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", LIB] + [os.path.join(OBJDIR, o) for _, o, _ in UNITS], check=True)
     return LIB
 
 

@@ -128,10 +128,11 @@ __device__ __forceinline__ bool nl_pass(const DevSys &S, const WarpState &ws, co
 }
 
 // Position an accepted move j puts its electron at: lattice hop r_i +- a e_k, or the quadrature point of a non-local slot.
+template <bool NL>
 __device__ __forceinline__ void move_target(const DevSys &S, const WarpState &ws, const double *nuc, int j, int &i, double &px, double &py, double &pz)
 {
     const int N = S.N;
-    if (j < S.P_lat) {
+    if (!NL || j < S.P_lat) {
         const int mesh = j / (6 * N), jj = j - mesh * 6 * N, d = jj - 6 * (jj / 6), k = d >> 1;
         i = jj / 6;
         const double step = (d & 1) ? -S.amesh[mesh] : S.amesh[mesh];
@@ -148,6 +149,7 @@ __device__ __forceinline__ void move_target(const DevSys &S, const WarpState &ws
 
 // Phase C (row a7) of one evaluation, by one warp on the candidate ratios R[P] left in shared memory.
 // node0: node flag already raised by the non-local candidates (rho_q < 0), any lane.
+template <bool NL = false>
 __device__ __forceinline__ EvalOut phase_c(const DevSys &S, const WarpState &ws, const double *lap_s, double Vee, int lane, int node0 = 0)
 {
     const int N = S.N;
@@ -159,9 +161,11 @@ __device__ __forceinline__ EvalOut phase_c(const DevSys &S, const WarpState &ws,
     for (int e = 0; e < chunk; ++e) {
         const int j = j0 + e;
         if (j < P) {
-            const double Rj = ws.R[j], kap = j < 6 * N ? S.kappa[0] : (j < S.P_lat ? S.kappa[1] : 1.0);   // non-local slots hold -nu_q rho_q itself
+            const double Rj = ws.R[j];
+            const double kap = NL ? (j < 6 * N ? S.kappa[0] : (j < S.P_lat ? S.kappa[1] : 1.0))   // non-local slots hold -nu_q rho_q itself
+                                  : S.kappa[j >= 6 * N ? 1 : 0];
             if (Rj > 0.0) loc += kap * Rj;
-            else if (Rj < 0.0) { vsf_part -= kap * Rj; if (j < S.P_lat) node = 1; }
+            else if (Rj < 0.0) { vsf_part -= kap * Rj; if (!NL || j < S.P_lat) node = 1; }
             ws.cum[j] = loc;
         }
     }
@@ -193,7 +197,7 @@ __device__ __forceinline__ EvalOut phase_c(const DevSys &S, const WarpState &ws,
     return o;
 }
 
-template <int NT, bool TS, int NB>
+template <int NT, bool TS, int NB, bool NL = false>
 __device__ __forceinline__ EvalOut evaluate_walker(const DevSys &S, const WarpState &ws, const Tables &T, int lane)
 {
     const int N = S.N, n_nuc = S.n_nuc;
@@ -340,7 +344,7 @@ __device__ __forceinline__ EvalOut evaluate_walker(const DevSys &S, const WarpSt
 #endif
     // ---- non-local pseudopotential slots (row f1): 8 slots per warp pass, whole shell list
     int node_nl = 0;
-    if (S.nl_K) {
+    if (NL) {
         for (int sp = 0; sp < 2; ++sp) {
             const int nslot = (sp ? S.n_dn : S.n_up) * S.nl_K;
             for (int s0 = 0; s0 < nslot; s0 += 8) {
@@ -363,7 +367,7 @@ __device__ __forceinline__ EvalOut evaluate_walker(const DevSys &S, const WarpSt
     }
     __syncwarp();
 
-    const EvalOut o = phase_c(S, ws, lap_s, Vee, lane, node_nl);
+    const EvalOut o = phase_c<NL>(S, ws, lap_s, Vee, lane, node_nl);
     __syncwarp();
     return o;
 }
@@ -390,11 +394,11 @@ __device__ __forceinline__ int select_move(const DevSys &S, const WarpState &ws,
 }
 
 // Apply move j (row a10): r_i <- r'_j, refresh the cached MO rows and the one-body cache of electron i, Sherman-Morrison on Dinv_sigma.
-template <int NT, bool TS>
+template <int NT, bool TS, bool NL = false>
 __device__ __forceinline__ void apply_move(const DevSys &S, const WarpState &ws, const Tables &T, int j, int lane)
 {
     const int N = S.N; int i; double px, py, pz;
-    move_target(S, ws, T.nuc, j, i, px, py, pz);
+    move_target<NL>(S, ws, T.nuc, j, i, px, py, pz);
     const int sp = spin_of(S, i), il = sp ? i - S.n_up : i, ns = sp ? S.n_dn : S.n_up;
     double *mc = ws.moc + (size_t)i * 5 * S.OS;
     __syncwarp();

@@ -5,7 +5,7 @@
 #include <cuda_runtime.h>
 
 // Taylor coefficients 1/k! (k = 2..11) in constant memory: DFMA takes them as c[bank][offset] operands directly.
-__constant__ double c_exp_poly[10] = {
+static __constant__ double c_exp_poly[10] = {
     2.50521083854417187751e-08,  // 1/11!
     2.75573192239858906526e-07,  // 1/10!
     2.75573192239858906526e-06,  // 1/9!

@@ -1,0 +1,81 @@
+// kernels.cu -- the walker kernels' launchers.  This one source is compiled FOUR times (build.py: -DLRDMC_NL=0|1 x
+// -DLRDMC_TEAM_TU=0|1, in parallel): NL = with / without the non-local pseudopotential slots (separate code, so that lattice-only
+// systems keep their register allocation: inlined into one kernel the slots cost 284 B of spills and 9 % of the C4 throughput),
+// TEAM_TU = the team kernel / the warp-per-walker kernels.  lrdmc.cu (host logic) calls them through kernels.h.
+#include "common.cuh"
+#include "philox.cuh"
+#include "wavefunction.cuh"
+#include "evaluate.cuh"
+#include "propagate.cuh"
+#include "team.cuh"
+#include "kernels.h"
+
+#ifndef LRDMC_NL
+#error "compile with -DLRDMC_NL=0 or 1"
+#endif
+#if LRDMC_NL
+#define KFN(name) name##_nl
+#else
+#define KFN(name) name##_lat
+#endif
+static constexpr bool kNL = LRDMC_NL != 0;
+
+#define FOR_EACH_NT_TS(X) X(1, true) X(2, true) X(4, true) X(1, false) X(2, false) X(4, false)
+#define PICK(NT_, TS_, STMT)                                                                   \
+    do {                                                                                       \
+        if (TS_) { if (NT_ == 1) { STMT(1, true); } else if (NT_ == 2) { STMT(2, true); } else { STMT(4, true); } } \
+        else { if (NT_ == 1) { STMT(1, false); } else if (NT_ == 2) { STMT(2, false); } else { STMT(4, false); } }   \
+    } while (0)
+
+#if !LRDMC_TEAM_TU
+void KFN(lrdmc_k_set_smem)(int smem)
+{
+#define X(NTV, TSV) cudaFuncSetAttribute(k_propagate<NTV, TSV, kNL>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); \
+                    cudaFuncSetAttribute(k_step_debug<NTV, TSV, kNL>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    FOR_EACH_NT_TS(X)
+#undef X
+}
+int KFN(lrdmc_k_occupancy)(int NT, int ts, int threads, int smem)
+{
+    int occ = 0;
+#define STMT(NTV, TSV) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_propagate<NTV, TSV, kNL>, threads, smem)
+    PICK(NT, ts, STMT);
+#undef STMT
+    return occ;
+}
+void KFN(lrdmc_k_propagate)(int NT, int ts, int grid, int threads, int smem, cudaStream_t st, const DevSys &S, const DevWalk &W, int mode, int n_moves,
+                            double tau, double E0, uint32_t cycle)
+{
+#define STMT(NTV, TSV) k_propagate<NTV, TSV, kNL><<<grid, threads, smem, st>>>(S, W, mode, n_moves, tau, E0, cycle)
+    PICK(NT, ts, STMT);
+#undef STMT
+}
+void KFN(lrdmc_k_step_debug)(int NT, int ts, int grid, int threads, int smem, cudaStream_t st, const DevSys &S, const DevWalk &W, double E0, uint32_t cycle,
+                             uint32_t step, double *R_out, double *scal_out, int *jstar_out)
+{
+#define STMT(NTV, TSV) k_step_debug<NTV, TSV, kNL><<<grid, threads, smem, st>>>(S, W, E0, cycle, step, R_out, scal_out, jstar_out)
+    PICK(NT, ts, STMT);
+#undef STMT
+}
+#else
+int KFN(lrdmc_k_team_occupancy)(int NT, int ts, int threads, int smem)
+{
+    int occ = 0;
+#if LRDMC_BC_DMMA
+#define STMT(NTV, TSV) cudaFuncSetAttribute(k_propagate_team<NTV, TSV, kNL>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); \
+                       cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_propagate_team<NTV, TSV, kNL>, threads, smem)
+    PICK(NT, ts, STMT);
+#undef STMT
+#endif
+    return occ;
+}
+void KFN(lrdmc_k_team)(int NT, int ts, int grid, int threads, int smem, cudaStream_t st, const DevSys &S, const DevWalk &W, const TeamPlan &P, int mode,
+                       int n_moves, double tau, double E0, uint32_t cycle)
+{
+#if LRDMC_BC_DMMA
+#define STMT(NTV, TSV) k_propagate_team<NTV, TSV, kNL><<<grid, threads, smem, st>>>(S, W, P, mode, n_moves, tau, E0, cycle)
+    PICK(NT, ts, STMT);
+#undef STMT
+#endif
+}
+#endif

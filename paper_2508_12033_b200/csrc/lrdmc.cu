@@ -12,7 +12,7 @@
 #include "wavefunction.cuh"
 #include "evaluate.cuh"
 #include "propagate.cuh"
-#include "team.cuh"
+#include "kernels.h"
 #include "reconfigure.cuh"
 #include "peaks.cuh"
 #include "api_internal.h"
@@ -214,16 +214,13 @@ extern "C" int lrdmc_init(lrdmc_ctx **out, const lrdmc_system *sys, const lrdmc_
     if ((size_t)c->smem_bytes > per_blk_max) { lrdmc_free(c); return LRDMC_ENOMEM; }
     for (int i = 0; i < 4; ++i) cudaEventCreate(&c->ev[i]);
 #define SET_SMEM(K) cudaFuncSetAttribute(K, cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem_bytes)
-#define SET_ALL(NTV, TSV) SET_SMEM((k_propagate<NTV, TSV>)); SET_SMEM((k_step_debug<NTV, TSV>)); SET_SMEM((k_rebuild<NTV, TSV>))
+#define SET_ALL(NTV, TSV) SET_SMEM((k_rebuild<NTV, TSV, false>))
     SET_ALL(1, true); SET_ALL(2, true); SET_ALL(4, true); SET_ALL(1, false); SET_ALL(2, false); SET_ALL(4, false);
 #undef SET_ALL
 #undef SET_SMEM
     c->ts = S.bf_in_smem && S.moc_in_smem;
-    int occ = 0;
-#define OCC(NTV, TSV) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_propagate<NTV, TSV>, c->wpb * 32, c->smem_bytes)
-    if (c->ts) { if (c->NT == 1) OCC(1, true); else if (c->NT == 2) OCC(2, true); else OCC(4, true); }
-    else { if (c->NT == 1) OCC(1, false); else if (c->NT == 2) OCC(2, false); else OCC(4, false); }
-#undef OCC
+    if (S.nl_K) lrdmc_k_set_smem_nl(c->smem_bytes); else lrdmc_k_set_smem_lat(c->smem_bytes);
+    const int occ = S.nl_K ? lrdmc_k_occupancy_nl(c->NT, c->ts, c->wpb * 32, c->smem_bytes) : lrdmc_k_occupancy_lat(c->NT, c->ts, c->wpb * 32, c->smem_bytes);
     c->ctas_per_sm = occ > 0 ? occ : 1;
     c->grid_max = c->sm_count * c->ctas_per_sm;
     if (cudaGetLastError() != cudaSuccess) { /* attribute errors surface at launch */ }
@@ -288,14 +285,6 @@ static void partition_shells(const int n_it[4], const double cost[4], bool pairs
     }
 }
 
-template <int NT, bool TS> static int team_occupancy(int threads, int smem)
-{
-    int occ = 0;
-    cudaFuncSetAttribute(k_propagate_team<NT, TS>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_propagate_team<NT, TS>, threads, smem);
-    return occ;
-}
-
 // Choose the team size for n_w walkers.  Warp-per-walker (team_tw = 1) when the walkers alone fill the resident warp slots;
 // otherwise the largest power of two 4 <= TW <= 16 with n_w TW <= slots (few walkers), or 4 for the large systems whose 36 KB
 // state leaves one warp per scheduler.  LRDMC_TEAM=<tw> forces a size (0/1: never).
@@ -336,9 +325,7 @@ static void plan_team(lrdmc_ctx *c, int n_w)
     P.o_nl = (int)scr_lat; P.o_nu = (int)(scr_lat + scr_nl);
     P.o_scr = S.per_warp_doubles; P.scr_doubles = (int)align_up(scr_col > scr_mo ? scr_col : scr_mo, 2);
     const int smem = (int)(((size_t)S.tables_doubles + S.per_warp_doubles + P.scr_doubles) * 8);
-    int occ = 0;
-    if (c->ts) occ = c->NT == 1 ? team_occupancy<1, true>(tw * 32, smem) : (c->NT == 2 ? team_occupancy<2, true>(tw * 32, smem) : team_occupancy<4, true>(tw * 32, smem));
-    else occ = c->NT == 1 ? team_occupancy<1, false>(tw * 32, smem) : (c->NT == 2 ? team_occupancy<2, false>(tw * 32, smem) : team_occupancy<4, false>(tw * 32, smem));
+    const int occ = S.nl_K ? lrdmc_k_team_occupancy_nl(c->NT, c->ts, tw * 32, smem) : lrdmc_k_team_occupancy_lat(c->NT, c->ts, tw * 32, smem);
     if (cudaGetLastError() != cudaSuccess || occ < 1) return;             // does not fit: stay with warp-per-walker
     c->team_tw = tw; c->team_smem = smem; c->team_ctas_per_sm = occ; c->team_grid_max = c->sm_count * occ;
 #endif
@@ -357,17 +344,17 @@ extern "C" int lrdmc_bind_walkers(lrdmc_ctx *c, void *dev_buf, size_t bytes, int
 
 // ---- launch helpers -----------------------------------------------------------------------------------------------
 static int grid_for(const lrdmc_ctx *c) { int g = (c->W.n_w + c->wpb - 1) / c->wpb; return g < c->grid_max ? g : c->grid_max; }
-#define LAUNCH_(KERNEL, NTV, TSV, grid, stream, ...) KERNEL<NTV, TSV><<<grid, c->wpb * 32, c->smem_bytes, stream>>>(__VA_ARGS__)
-#define DISPATCH_NT(KERNEL, grid, stream, ...)                                                                   \
+#define LAUNCH_(KERNEL, NTV, TSV, NLV, grid, stream, ...) KERNEL<NTV, TSV, NLV><<<grid, c->wpb * 32, c->smem_bytes, stream>>>(__VA_ARGS__)
+#define DISPATCH_NL_(KERNEL, NLV, grid, stream, ...)                                                             \
     do {                                                                                                         \
         if (c->ts) {                                                                                             \
-            if (c->NT == 1) LAUNCH_(KERNEL, 1, true, grid, stream, __VA_ARGS__);                                 \
-            else if (c->NT == 2) LAUNCH_(KERNEL, 2, true, grid, stream, __VA_ARGS__);                            \
-            else LAUNCH_(KERNEL, 4, true, grid, stream, __VA_ARGS__);                                            \
+            if (c->NT == 1) LAUNCH_(KERNEL, 1, true, NLV, grid, stream, __VA_ARGS__);                            \
+            else if (c->NT == 2) LAUNCH_(KERNEL, 2, true, NLV, grid, stream, __VA_ARGS__);                       \
+            else LAUNCH_(KERNEL, 4, true, NLV, grid, stream, __VA_ARGS__);                                       \
         } else {                                                                                                 \
-            if (c->NT == 1) LAUNCH_(KERNEL, 1, false, grid, stream, __VA_ARGS__);                                \
-            else if (c->NT == 2) LAUNCH_(KERNEL, 2, false, grid, stream, __VA_ARGS__);                           \
-            else LAUNCH_(KERNEL, 4, false, grid, stream, __VA_ARGS__);                                           \
+            if (c->NT == 1) LAUNCH_(KERNEL, 1, false, NLV, grid, stream, __VA_ARGS__);                           \
+            else if (c->NT == 2) LAUNCH_(KERNEL, 2, false, NLV, grid, stream, __VA_ARGS__);                      \
+            else LAUNCH_(KERNEL, 4, false, NLV, grid, stream, __VA_ARGS__);                                      \
         }                                                                                                        \
         ++c->launches;                                                                                           \
     } while (0)
@@ -375,7 +362,7 @@ static int grid_for(const lrdmc_ctx *c) { int g = (c->W.n_w + c->wpb - 1) / c->w
 static int rebuild(lrdmc_ctx *c, int do_invert /* bit 0: invert, bit 1: the MO cache is valid */, cudaStream_t st)
 {
     CK(cudaMemsetAsync(c->W.counter, 0, 64 * sizeof(int), st));
-    DISPATCH_NT(k_rebuild, grid_for(c), st, c->S, c->W, do_invert);
+    DISPATCH_NL_(k_rebuild, false, grid_for(c), st, c->S, c->W, do_invert);
     CK(cudaGetLastError());
     return LRDMC_OK;
 }
@@ -451,14 +438,13 @@ extern "C" int lrdmc_propagate(lrdmc_ctx *c, int mode, int n_moves, double tau, 
     const int grid = team ? (c->W.n_w < c->team_grid_max ? c->W.n_w : c->team_grid_max) : grid_for(c);
     CK(cudaEventRecord(c->ev[0], st));
     if (team) {
-#if LRDMC_BC_DMMA
-#define TEAM_(NTV, TSV) k_propagate_team<NTV, TSV><<<grid, c->team_tw * 32, c->team_smem, st>>>(c->S, c->W, c->team, mode, n_moves, tau, E0, (uint32_t)cycle)
-        if (c->ts) { if (c->NT == 1) TEAM_(1, true); else if (c->NT == 2) TEAM_(2, true); else TEAM_(4, true); }
-        else { if (c->NT == 1) TEAM_(1, false); else if (c->NT == 2) TEAM_(2, false); else TEAM_(4, false); }
-#undef TEAM_
-        ++c->launches;
-#endif
-    } else DISPATCH_NT(k_propagate, grid, st, c->S, c->W, mode, n_moves, tau, E0, (uint32_t)cycle);
+        if (c->S.nl_K) lrdmc_k_team_nl(c->NT, c->ts, grid, c->team_tw * 32, c->team_smem, st, c->S, c->W, c->team, mode, n_moves, tau, E0, (uint32_t)cycle);
+        else lrdmc_k_team_lat(c->NT, c->ts, grid, c->team_tw * 32, c->team_smem, st, c->S, c->W, c->team, mode, n_moves, tau, E0, (uint32_t)cycle);
+    } else {
+        if (c->S.nl_K) lrdmc_k_propagate_nl(c->NT, c->ts, grid, c->wpb * 32, c->smem_bytes, st, c->S, c->W, mode, n_moves, tau, E0, (uint32_t)cycle);
+        else lrdmc_k_propagate_lat(c->NT, c->ts, grid, c->wpb * 32, c->smem_bytes, st, c->S, c->W, mode, n_moves, tau, E0, (uint32_t)cycle);
+    }
+    ++c->launches;
     CK(cudaEventRecord(c->ev[1], st));
     CK(cudaGetLastError());
     k_reduce_obs<<<1, 1024, 0, st>>>(c->W, c->d_stats, team ? grid : grid * c->wpb); ++c->launches;
@@ -518,7 +504,9 @@ extern "C" int lrdmc_step_debug(lrdmc_ctx *c, double E0, uint64_t cycle, uint64_
     if (!c || !R_dev || !scal_dev || !jstar_dev || cycle > 0xFFFFFFFFull || step > 0xFFFFFFFFull) return LRDMC_EINVAL;
     if (!c->bound || !c->state_ok) return LRDMC_ESTATE;
     cudaStream_t st = (cudaStream_t)stream;
-    DISPATCH_NT(k_step_debug, grid_for(c), st, c->S, c->W, E0, (uint32_t)cycle, (uint32_t)step, R_dev, scal_dev, jstar_dev);
+    if (c->S.nl_K) lrdmc_k_step_debug_nl(c->NT, c->ts, grid_for(c), c->wpb * 32, c->smem_bytes, st, c->S, c->W, E0, (uint32_t)cycle, (uint32_t)step, R_dev, scal_dev, jstar_dev);
+    else lrdmc_k_step_debug_lat(c->NT, c->ts, grid_for(c), c->wpb * 32, c->smem_bytes, st, c->S, c->W, E0, (uint32_t)cycle, (uint32_t)step, R_dev, scal_dev, jstar_dev);
+    ++c->launches;
     CK(cudaGetLastError());
     return LRDMC_OK;
 }

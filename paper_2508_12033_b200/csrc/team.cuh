@@ -44,7 +44,7 @@ __device__ __forceinline__ void store_walker_team(const DevSys &S, const DevWalk
 
 // One evaluation by the team.  The result is valid in warp 0 only (it runs phase C); ws.R / ws.cum are complete for everyone
 // after the caller's next barrier.  s_vee: TW doubles of static shared memory.
-template <int NT, bool TS>
+template <int NT, bool TS, bool NL>
 __device__ __forceinline__ EvalOut evaluate_team(const DevSys &S, const TeamPlan &P, const WarpState &ws, const Tables &T, double *scr, double *s_vee, int *s_node)
 {
     const int N = S.N, n_nuc = S.n_nuc, TW = P.TW, NP = P.NP, tid = threadIdx.x, nthr = blockDim.x, lane = tid & 31, wt = tid >> 5;
@@ -95,8 +95,8 @@ __device__ __forceinline__ EvalOut evaluate_team(const DevSys &S, const TeamPlan
 
     // ---- phase B (rows a1-a5): work units (mesh, spin, 8-electron block, shell part); unit u -> warp u mod TW
     const int nb_mesh = P.nblk[0] + P.nblk[1];
-    for (int v = wt; v < P.n_units + P.n_units_nl; v += TW) {
-        if (v >= P.n_units) {            // non-local pseudopotential slots (row f1): unit = (spin, 8-slot block, shell part)
+    for (int v = wt; v < P.n_units + (NL ? P.n_units_nl : 0); v += TW) {
+        if (NL && v >= P.n_units) {            // non-local pseudopotential slots (row f1): unit = (spin, 8-slot block, shell part)
             const int u = v - P.n_units, part = u % NP, blk = u / NP, sp = blk >= P.nblk_nl[0] ? 1 : 0, s0 = 8 * (sp ? blk - P.nblk_nl[0] : blk);
             double acc[6], Jn[6], nuq[6]; bool valid, active; int i, slot;
             const bool any = nl_pass<NT, TS, true>(S, ws, T, sp, s0, lane, acc, Jn, nuq, valid, active, i, slot, &P, &P.col[part], part, NP);
@@ -171,7 +171,7 @@ __device__ __forceinline__ EvalOut evaluate_team(const DevSys &S, const TeamPlan
             for (int part = 0; part < NP; ++part) { A += q[part * 12 + d]; J += q[part * 12 + 6 + d]; }
             ws.R[p] = A * exp_tab(J - Jold[i], T.etab);
         }
-        for (int p = S.P_lat + tid; p < S.P; p += nthr) {          // non-local slots: R = -nu_q rho_q
+        if (NL) for (int p = S.P_lat + tid; p < S.P; p += nthr) {  // non-local slots: R = -nu_q rho_q
             const int o = p - S.P_lat, slot = o / 6, d = o - 6 * slot, i = slot / S.nl_K;
             const double *q = scr + P.o_nl + (size_t)slot * NP * 12, *qn = scr + P.o_nu + (size_t)slot * 7;
             double A = 0.0, J = 0.0;
@@ -187,19 +187,19 @@ __device__ __forceinline__ EvalOut evaluate_team(const DevSys &S, const TeamPlan
     if (wt == 0) {
         double Vee = 0.0;
         for (int w = 0; w < TW; ++w) Vee += s_vee[w];
-        o = phase_c(S, ws, lap_s, Vee, lane, *s_node);
+        o = phase_c<NL>(S, ws, lap_s, Vee, lane, NL ? *s_node : 0);
     }
     return o;
 }
 
 // Apply move j (row a10) by the team: warp w takes part P.mo[w] of the derivative pass of the mover (value, gradient, Laplacian
 // rows by DMMA), the partial rows meet in scr; Sherman-Morrison on Dinv_sigma over all threads.
-template <int NT, bool TS>
+template <int NT, bool TS, bool NL>
 __device__ __forceinline__ void apply_move_team(const DevSys &S, const TeamPlan &P, const WarpState &ws, const Tables &T, double *scr, int j)
 {
     const int N = S.N, TW = P.TW, tid = threadIdx.x, nthr = blockDim.x, lane = tid & 31, wt = tid >> 5;   // warp 0 holds the lightest shell part (s shells): it also refreshes the one-body cache
     int i; double px, py, pz;
-    move_target(S, ws, T.nuc, j, i, px, py, pz);
+    move_target<NL>(S, ws, T.nuc, j, i, px, py, pz);
     const int sp = spin_of(S, i), il = sp ? i - S.n_up : i, ns = sp ? S.n_dn : S.n_up;
     double *mc = ws.moc + (size_t)i * 5 * S.OS;
     const int rows = 5 * S.OS;
@@ -239,7 +239,7 @@ __device__ __forceinline__ void apply_move_team(const DevSys &S, const TeamPlan 
     __syncthreads();
 }
 
-template <int NT, bool TS>
+template <int NT, bool TS, bool NL>
 __global__ void __launch_bounds__(LRDMC_TEAM_MAX_WARPS * 32, 1) k_propagate_team(DevSys S, DevWalk W, TeamPlan P, int mode, int n_moves, double tau, double E0, uint32_t cycle)
 {
     extern __shared__ __align__(16) double smem[];
@@ -265,7 +265,7 @@ __global__ void __launch_bounds__(LRDMC_TEAM_MAX_WARPS * 32, 1) k_propagate_team
 #pragma unroll
                 for (int i = 0; i < 9; ++i) ws.U[i] = U[i]; }
             __syncthreads();
-            const EvalOut e = evaluate_team<NT, TS>(S, P, ws, T, scr, s_vee, &s_ctrl[3]);
+            const EvalOut e = evaluate_team<NT, TS, NL>(S, P, ws, T, scr, s_vee, &s_ctrl[3]);
             if (wt == 0) {                                       // the leader warp keeps the weight (same rules as k_propagate)
                 n_node += e.node;
                 bool last = false;
@@ -291,7 +291,7 @@ __global__ void __launch_bounds__(LRDMC_TEAM_MAX_WARPS * 32, 1) k_propagate_team
             __syncthreads();
             const bool last = s_ctrl[1] != 0; const int j = s_ctrl[2];
             if (last) break;
-            if (j >= 0) { apply_move_team<NT, TS>(S, P, ws, T, scr, j); ++moves; }
+            if (j >= 0) { apply_move_team<NT, TS, NL>(S, P, ws, T, scr, j); ++moves; }
             ++s;
         }
         store_walker_team(S, W, ws, k);

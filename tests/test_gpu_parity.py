@@ -282,6 +282,27 @@ def test_hydrogen_run_energy_matches_oracle_and_exact(B):
     g.close()
 
 
+def test_nonlocal_s_channel_energy_on_the_cuda_path(B):
+    """Scope row f1 through the CUDA path: one electron in -1/r plus an attractive non-local s channel.  The exact ground-state
+    energy comes from the radial eigen-solver of tests/test_oracle_nonlocal.py (independent of both implementations); LRDMC with the
+    non-local hops must reach it as a -> 0 in both modes, and the first generations must equal the oracle's to rounding."""
+    from paper_2508_12033_b200 import driver as drv
+    from test_oracle_nonlocal import _radial_ground_state
+    A0, B0, rc = -0.8, 1.5, 2.2
+    E_exact = _radial_ground_state(A0, B0, rc)
+    mk = lambda a: wl.with_nonlocal(wl.hydrogen(alpha=1.1, a=a), [[rc, A0, B0, 0, 1, 0, 1]])
+    out = drv.a_scan(mk, lambda s, n: wl.hydrogen_walkers(n, 3), [0.2, 0.3, 0.4], n_walkers=2048, cycles=150, moves=30, E0=-0.6)
+    for mode in ("balanced", "conventional"):
+        E0, s0, coef, chi2 = out[mode]
+        assert abs(E0 - E_exact) < 3 * s0 + 5e-4 and s0 < 1.5e-3, (mode, E0, s0, E_exact)
+    s = mk(0.3); x0 = wl.hydrogen_walkers(256, 3)
+    g = B.Lrdmc(s); g.lrdmc_set_positions(x0); o = ref.Ref(s); o.set_positions(x0)
+    recs = drv.run(g, B.BALANCED, 5, n_moves=18, E0=-0.6); outo = rdrv.run(o, ref.BALANCED, 5, n_moves=18, E0=-0.6)
+    for n in range(5):
+        assert abs(recs[n].num / recs[n].den - outo["e"][n]) < 1e-9 and abs(recs[n].wbar - outo["wbar"][n]) < 1e-9
+    g.close()
+
+
 def test_a_to_zero_scan_balanced_vs_conventional_table_shape(B):
     """SURVEY 8(f) f3, the shape of Table I (L254-L265): at every a the two modes agree within 3 combined sigma, and both
     E(a) extrapolate to the exact -1/2 Ha of the hydrogen atom (L23, L140) -- on the CUDA path, 2048 walkers."""
