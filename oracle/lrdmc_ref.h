@@ -38,6 +38,16 @@ int lrdmc_ref_create(lrdmc_ref_ctx **out, int n_nuc, const double *Z, const doub
 void lrdmc_ref_destroy(lrdmc_ref_ctx *);
 int lrdmc_ref_n_candidates(const lrdmc_ref_ctx *); /* P = 6 N n_mesh (+ 6 N K non-local slots) */
 
+/* Contracted shells and real solid-harmonic d shells (scope row f2; "cc-pVTZ basis sets ... The angular part of
+ * the basis functions was expressed using spherical (solid) harmonics", L285 "cartesian").  The shells passed to create are then
+ * PRIMITIVES; contracted shell cs is the run of consecutive primitive shells first[cs] .. first[cs+1]-1 (same centre, same type):
+ *   chi_cs,c(r) = sum_k coef[k] chi^prim_k,c(r)      (each primitive normalised to unit self-overlap, reading Q14)
+ * and for a d shell with sph[cs] != 0 the five real solid harmonics, each of unit self-overlap for a single primitive, in the order
+ *   z2 = zz - (xx + yy)/2,  xz,  yz,  x2-y2 = (sqrt(3)/2)(xx - yy),  xy      (xx.. = the normalised cartesian d primitives).
+ * n_ao and the MO matrices given to create refer to the CONTRACTED functions.  Call right after create. */
+int lrdmc_ref_set_contraction(lrdmc_ref_ctx *, int n_cshell, const int *first /*[n_cshell+1]*/, const double *coef /*[n_shell]*/,
+                              const int *sph /*[n_cshell]*/);
+
 /* Non-local (semi-local) pseudopotential, scope row f1 (L242 "DLA", L567 D1 "non-local pseudopotentials", L576 "DTM").
  * nl [n_nuc][7] = { r_c, A_0, B_0, A_1, B_1, A_2, B_2 }: channel l of nucleus I is v_l(r) = A_l exp(-B_l r^2) inside r < r_c
  * (synthetic Gaussian channels: the ccECP tables are not in the container); r_c <= 0: no non-local part on that nucleus.

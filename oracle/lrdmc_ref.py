@@ -63,6 +63,7 @@ def lib():
                                           C.c_double, C.c_double, C.c_double, C.c_void_p, C.c_void_p, C.c_double, C.c_double,
                                           C.c_uint64]
         _lib.lrdmc_ref_destroy.argtypes = [C.c_void_p]
+        _lib.lrdmc_ref_set_contraction.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]
         _lib.lrdmc_ref_set_nonlocal.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p]
         _lib.lrdmc_ref_nl_info.argtypes = [C.c_void_p] + [C.c_void_p] * 7
         _lib.lrdmc_ref_n_candidates.argtypes = [C.c_void_p]
@@ -118,6 +119,12 @@ class Ref:
         if rc:
             raise ValueError(f"lrdmc_ref_create failed: {rc}")
         self.h = h
+        if sysd.get("cs_first") is not None:                           # contracted / solid-harmonic shells (scope row f2)
+            cf = np.ascontiguousarray(sysd["cs_first"], dtype=np.int32); pc = np.ascontiguousarray(sysd["prim_coef"], dtype=np.float64)
+            sp = np.ascontiguousarray(sysd["cs_sph"], dtype=np.int32)
+            rc = L.lrdmc_ref_set_contraction(h, len(sp), cf.ctypes.data, pc.ctypes.data, sp.ctypes.data)
+            if rc:
+                raise ValueError(f"lrdmc_ref_set_contraction failed: {rc}")
         self.nl_slots = 0
         if sysd.get("nl") is not None and sysd.get("nl_K", 0) > 0:      # non-local pseudopotential channels (scope row f1)
             nl = np.ascontiguousarray(sysd["nl"], dtype=np.float64)

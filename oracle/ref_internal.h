@@ -15,6 +15,9 @@ struct lrdmc_ref_ctx {
     int n_up, n_dn, N;
     /* basis */
     int n_shell, n_ao; int *center, *type, *ao0; double *zeta;
+    /* contracted / spherical shells (scope row f2, L242 "cc-pVTZ ... spherical (solid) harmonics"): n_pao primitive AOs;
+     * contracted shell cs = primitive shells [cs_first[cs], cs_first[cs+1]) with coefficients prim_coef; cs_sph: 5 real solid d */
+    int n_pao, n_cshell, need_contraction; int *cs_first, *cs_sph; double *prim_coef;
     double *C_up, *C_dn;             /* [n_ao][n_up], [n_ao][n_dn] */
     /* Jastrow */
     double a_par, a_anti, b2; double *c1, *b1; /* c1 NULL: no one-body term */

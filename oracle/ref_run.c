@@ -28,7 +28,8 @@ int lrdmc_ref_create(lrdmc_ref_ctx **out, int n_nuc, const double *Z, const doub
         int t = type[s]; mu += (t == 0 || t == 10) ? 1 : (t == 1 ? 3 : (t == 2 ? 6 : -100000));
         if (center[s] < 0 || center[s] >= n_nuc || !(zeta[s] > 0.0)) mu = -100000;
     }
-    if (mu != n_ao) { lrdmc_ref_destroy(c); return LRDMC_REF_EINVAL; }
+    if (mu < 0) { lrdmc_ref_destroy(c); return LRDMC_REF_EINVAL; }
+    c->n_pao = mu; c->need_contraction = (mu != n_ao);      /* fewer functions than primitives: lrdmc_ref_set_contraction must follow */
     c->n_ao = n_ao; c->C_up = dupd(C_up, (size_t)n_ao * n_up); c->C_dn = dupd(C_dn, (size_t)n_ao * n_dn);
     c->a_par = a_par; c->a_anti = a_anti; c->b2 = b2; c->c1 = dupd(c1, n_nuc); c->b1 = c1 ? dupd(b1, n_nuc) : NULL;
     /* lattice: single mesh, or the double mesh of reading Q13: constant mixing g = 1/2 between a and a' */
@@ -58,10 +59,26 @@ void lrdmc_ref_destroy(lrdmc_ref_ctx *c)
     if (!c) return;
     free_walkers(c);
     free(c->Z); free(c->Rn); free(c->pp); free(c->center); free(c->type); free(c->zeta); free(c->ao0);
-    free(c->C_up); free(c->C_dn); free(c->c1); free(c->b1); free(c->nl); free(c);
+    free(c->C_up); free(c->C_dn); free(c->c1); free(c->b1); free(c->nl); free(c->cs_first); free(c->cs_sph); free(c->prim_coef); free(c);
 }
 
 int lrdmc_ref_n_candidates(const lrdmc_ref_ctx *c) { return c->P; }
+
+int lrdmc_ref_set_contraction(lrdmc_ref_ctx *c, int n_cshell, const int *first, const double *coef, const int *sph)
+{
+    if (!c || n_cshell < 1 || !first || !coef || !sph || first[0] != 0 || first[n_cshell] != c->n_shell || c->n_w) return LRDMC_REF_EINVAL;
+    int nao = 0;
+    for (int cs = 0; cs < n_cshell; ++cs) {
+        if (first[cs + 1] <= first[cs]) return LRDMC_REF_EINVAL;
+        int t = c->type[first[cs]], I = c->center[first[cs]];
+        for (int k = first[cs]; k < first[cs + 1]; ++k) if (c->type[k] != t || c->center[k] != I) return LRDMC_REF_EINVAL;
+        nao += (t == 1) ? 3 : (t == 2 ? (sph[cs] ? 5 : 6) : 1);
+    }
+    if (nao != c->n_ao) return LRDMC_REF_EINVAL;
+    c->n_cshell = n_cshell; c->cs_first = dupi(first, (size_t)n_cshell + 1); c->cs_sph = dupi(sph, n_cshell); c->prim_coef = dupd(coef, c->n_shell);
+    c->need_contraction = 0;
+    return LRDMC_REF_OK;
+}
 
 int lrdmc_ref_set_nonlocal(lrdmc_ref_ctx *c, int K, int dla, const double *nl)
 {
@@ -109,6 +126,7 @@ static int rebuild_all(lrdmc_ref_ctx *c)
 int lrdmc_ref_set_positions(lrdmc_ref_ctx *c, int n_w, const double *r)
 {
     if (!c || n_w < 1 || !r) return LRDMC_REF_EINVAL;
+    if (c->need_contraction) return LRDMC_REF_ESTATE;
     alloc_walkers(c, n_w);
     memcpy(c->r, r, sizeof(double) * (size_t)n_w * 3 * c->N);
     return rebuild_all(c);

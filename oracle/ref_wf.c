@@ -38,7 +38,8 @@ static void cart_gto(double zeta, const int lmn[3], const double d[3], double *v
     *lap = e * (f2[0] * f[1] * f[2] + f[0] * f2[1] * f[2] + f[0] * f[1] * f2[2]);
 }
 
-int lrdmc_ref_ao(const lrdmc_ref_ctx *c, const double r[3], double *val, double *grad, double *lap)
+/* the primitive functions, one after the other in shell order */
+static int ao_primitives(const lrdmc_ref_ctx *c, const double r[3], double *val, double *grad, double *lap)
 {
     for (int s = 0; s < c->n_shell; ++s) {
         const double *Rc = c->Rn + 3 * c->center[s];
@@ -63,6 +64,38 @@ int lrdmc_ref_ao(const lrdmc_ref_ctx *c, const double r[3], double *val, double 
         } else return LRDMC_REF_EINVAL;
     }
     return LRDMC_REF_OK;
+}
+
+/* AO values: the primitives themselves, or the contracted / solid-harmonic functions of lrdmc_ref_set_contraction */
+int lrdmc_ref_ao(const lrdmc_ref_ctx *c, const double r[3], double *val, double *grad, double *lap)
+{
+    if (c->need_contraction) return LRDMC_REF_ESTATE;
+    if (!c->n_cshell) return ao_primitives(c, r, val, grad, lap);
+    int np = c->n_pao;
+    double *pv = (double *)malloc(sizeof(double) * 5 * (size_t)np), *pg = pv + np, *pl = pv + 4 * np;
+    int rc = ao_primitives(c, r, pv, pg, pl);
+    const double h3 = sqrt(3.0) / 2.0;
+    int nu = 0;
+    for (int cs = 0; cs < c->n_cshell; ++cs) {
+        int t = c->type[c->cs_first[cs]], ncart = (t == 1) ? 3 : (t == 2 ? 6 : 1);
+        double cv[6] = { 0 }, cg[18] = { 0 }, cl[6] = { 0 };                 /* contracted cartesian components */
+        for (int k = c->cs_first[cs]; k < c->cs_first[cs + 1]; ++k)
+            for (int q = 0; q < ncart; ++q) {
+                int mu = c->ao0[k] + q; double d = c->prim_coef[k];
+                cv[q] += d * pv[mu]; cl[q] += d * pl[mu];
+                for (int ax = 0; ax < 3; ++ax) cg[3 * q + ax] += d * pg[3 * mu + ax];
+            }
+        if (t == 2 && c->cs_sph[cs]) {                                        /* xx xy xz yy yz zz -> z2, xz, yz, x2-y2, xy */
+            double w[5][6] = { { -0.5, 0, 0, -0.5, 0, 1.0 }, { 0, 0, 1, 0, 0, 0 }, { 0, 0, 0, 0, 1, 0 }, { h3, 0, 0, -h3, 0, 0 }, { 0, 1, 0, 0, 0, 0 } };
+            for (int m = 0; m < 5; ++m, ++nu) {
+                double v = 0, l = 0, g[3] = { 0, 0, 0 };
+                for (int q = 0; q < 6; ++q) { v += w[m][q] * cv[q]; l += w[m][q] * cl[q]; for (int ax = 0; ax < 3; ++ax) g[ax] += w[m][q] * cg[3 * q + ax]; }
+                val[nu] = v; lap[nu] = l; for (int ax = 0; ax < 3; ++ax) grad[3 * nu + ax] = g[ax];
+            }
+        } else for (int q = 0; q < ncart; ++q, ++nu) { val[nu] = cv[q]; lap[nu] = cl[q]; for (int ax = 0; ax < 3; ++ax) grad[3 * nu + ax] = cg[3 * q + ax]; }
+    }
+    free(pv);
+    return rc;
 }
 
 int lrdmc_ref_mo(const lrdmc_ref_ctx *c, int spin, const double r[3], double *val, double *grad, double *lap)

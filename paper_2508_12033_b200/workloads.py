@@ -27,8 +27,13 @@ def n_ao_of(types) -> int:
     return int(sum(_AO_PER_SHELL[int(t)] for t in types))
 
 
+def n_ao_contracted(types, first, sph) -> int:
+    """AO count of contracted shells: run cs of primitive shells first[cs]..first[cs+1]-1; a solid-harmonic d shell has 5 functions."""
+    return int(sum(5 if (int(types[first[cs]]) == SHELL_D and sph[cs]) else _AO_PER_SHELL[int(types[first[cs]])] for cs in range(len(sph))))
+
+
 def _system(name, Z, R, n_up, n_dn, center, stype, zeta, C_up, C_dn, jastrow, a, a2=0.0, pp=None,
-            n_walkers=0, cycles=0, moves=0, seed=PHILOX_RUN_SEED):
+            n_walkers=0, cycles=0, moves=0, seed=PHILOX_RUN_SEED, contraction=None):
     Z = np.ascontiguousarray(Z, dtype=np.float64)
     R = np.ascontiguousarray(R, dtype=np.float64).reshape(-1, 3)
     d = dict(
@@ -38,7 +43,11 @@ def _system(name, Z, R, n_up, n_dn, center, stype, zeta, C_up, C_dn, jastrow, a,
         shell_center=np.ascontiguousarray(center, dtype=np.int32),
         shell_type=np.ascontiguousarray(stype, dtype=np.int32),
         shell_zeta=np.ascontiguousarray(zeta, dtype=np.float64),
-        n_shell=int(len(center)), n_ao=n_ao_of(stype),
+        n_shell=int(len(center)), n_ao=n_ao_of(stype) if contraction is None else n_ao_contracted(stype, contraction[0], contraction[2]),
+        # contracted / solid-harmonic shells (scope row f2): the shells above are then primitives, the MOs refer to the contracted AOs
+        cs_first=None if contraction is None else np.ascontiguousarray(contraction[0], dtype=np.int32),
+        prim_coef=None if contraction is None else np.ascontiguousarray(contraction[1], dtype=np.float64),
+        cs_sph=None if contraction is None else np.ascontiguousarray(contraction[2], dtype=np.int32),
         C_up=np.ascontiguousarray(C_up, dtype=np.float64),
         C_dn=np.ascontiguousarray(C_dn, dtype=np.float64),
         a_par=float(jastrow.get("a_par", 0.0)), a_anti=float(jastrow.get("a_anti", 0.0)),
@@ -207,6 +216,32 @@ def tiny_molecule(n_up=2, n_dn=1, n_nuc=2, n_shell=6, seed=7, a=0.2, a2=0.0, wit
     jas = dict(a_par=0.25, a_anti=0.5, b2=0.8, c1=c1, b1=rng.uniform(0.5, 1.5, size=n_nuc))
     return _system(f"tiny-{n_up}u{n_dn}d", Z, R, n_up, n_dn, center, stype, zeta, C_up, C_dn, jas, a,
                    a2=a2, pp=pp)
+
+
+def contracted_molecule(n_up=3, n_dn=2, n_nuc=3, n_cshell=9, seed=31, a=0.2, spherical=True, with_pp=False):
+    """Scope row f2: a small molecule on CONTRACTED shells (1-3 primitives each, seeded coefficients) with real solid-harmonic d
+    shells -- the shape of the paper's cc-pVTZ / spherical-harmonics basis (L242); exponents and coefficients are synthetic."""
+    rng = np.random.default_rng(seed)
+    R = _separated_points(rng, n_nuc, lambda: rng.uniform(-1.5, 1.5, size=3), 1.0)
+    Z = rng.choice([1.0, 2.0, 3.0], size=n_nuc)
+    center, stype, zeta, coef, first, sph = [], [], [], [], [0], []
+    for cs in range(n_cshell):
+        t = (SHELL_S, SHELL_P, SHELL_D)[cs % 3]; nprim = int(rng.integers(1, 4))
+        z0 = np.exp(rng.uniform(np.log(0.2), np.log(1.0)))
+        for k in range(nprim):
+            center.append(cs % n_nuc); stype.append(t); zeta.append(z0 * 2.5 ** k); coef.append(rng.uniform(0.2, 1.0) * (1 if k % 2 == 0 else -0.5))
+        first.append(len(center)); sph.append(1 if (t == SHELL_D and spherical) else 0)
+    n_ao = n_ao_contracted(stype, first, sph)
+    C_up = _orthonormal_mos(rng, n_ao, n_up)
+    C_dn = _orthonormal_mos(rng, n_ao, n_dn) if n_dn else np.zeros((n_ao, 0))
+    pp = None; c1 = Z.copy()
+    if with_pp:
+        pp = np.stack([np.exp(rng.uniform(0.0, np.log(10.0), size=n_nuc)), np.exp(rng.uniform(0.0, np.log(10.0), size=n_nuc)),
+                       rng.uniform(0.0, 2.0 * Z), np.exp(rng.uniform(0.0, np.log(10.0), size=n_nuc))], axis=1)
+        c1 = np.full(n_nuc, 0.5)
+    jas = dict(a_par=0.25, a_anti=0.5, b2=0.8, c1=c1, b1=rng.uniform(0.5, 1.5, size=n_nuc))
+    return _system(f"contracted-{n_up}u{n_dn}d" + ("-sph" if spherical else "-cart"), Z, R, n_up, n_dn, center, stype, zeta, C_up, C_dn, jas, a,
+                   pp=pp, contraction=(first, coef, sph))
 
 
 def with_nonlocal(sysd, nl, dla=True):

@@ -155,6 +155,25 @@ def test_team_kernel_every_team_size(B, name, mode, tw, monkeypatch):
     g.close()
 
 
+@pytest.mark.parametrize("name", ["C3-water-methane-shaped", "tiny-3u2d-nlDLA-strong", "C5-cluster64-doublemesh"])
+def test_team_kernel_is_bitwise_reproducible(B, name, monkeypatch):
+    """compute-sanitizer is not available on the GPU pool; a shared-memory race between the warps of a team would show as
+    run-to-run differences.  Three runs of the same cycle from the same state must agree bit for bit (positions, inverses,
+    weights, local energies), for the largest team."""
+    monkeypatch.setenv("LRDMC_TEAM", "16")
+    s, x0 = SYSTEMS[name]()
+    outs = []
+    for rep in range(3):
+        g = B.Lrdmc(s); g.lrdmc_set_positions(x0)
+        g.lrdmc_propagate(B.BALANCED, 25, 0.0, -5.0, 3)
+        outs.append([np_(t).copy() for t in g.lrdmc_get_walkers()] + [np_(t).copy() for t in g.lrdmc_get_obs()])
+        assert g.launch_config()["block"] == 512
+        g.close()
+    for other in outs[1:]:
+        for a, b in zip(outs[0], other):
+            assert np.array_equal(a, b)
+
+
 def _whole_cycles(B, name, mode, n_cycles=2, keep=False):
     s, x0, o, g = _pair(B, name)
     N = s["n_up"] + s["n_dn"]; n_moves = 30

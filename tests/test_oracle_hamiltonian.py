@@ -64,6 +64,7 @@ SYSTEMS = {
     "tiny-2u2d-doublemesh": lambda: wl.tiny_molecule(2, 2, 2, 7, seed=9, a=0.15, a2=0.3),
     "C2": wl.synthetic10,
     "C3": lambda: wl.water_methane(n_walkers=4),
+    "contracted-sph": lambda: wl.contracted_molecule(3, 2, 3, 9, seed=31, spherical=True, with_pp=True),   # scope row f2
 }
 
 
@@ -93,7 +94,7 @@ def test_regularised_local_energy_equals_continuum_local_energy(name):
     assert checked >= 1     # random-MO trial functions have nodes everywhere: the D11 branch fires often on C3
 
 
-@pytest.mark.parametrize("name", ["tiny-2u1d", "tiny-3u3d-pp", "C2"])
+@pytest.mark.parametrize("name", ["tiny-2u1d", "tiny-3u3d-pp", "C2", "contracted-sph"])
 def test_continuum_laplacian_matches_finite_differences_of_logpsi(name):
     """lap_i Psi/Psi = lap_i log|Psi| + |grad_i log|Psi||^2, by 4th-order central differences of the brute-force log|Psi|."""
     s = SYSTEMS[name](); o = ref.Ref(s); x = wl.initial_walkers(s, 1, 33)[0]
@@ -111,7 +112,7 @@ def test_continuum_laplacian_matches_finite_differences_of_logpsi(name):
 
 
 # ----------------------------------------------------------------------------- ratios vs brute force (pin P3)
-@pytest.mark.parametrize("name", ["tiny-2u1d", "tiny-3u3d-pp", "tiny-2u2d-doublemesh", "C2"])
+@pytest.mark.parametrize("name", ["tiny-2u1d", "tiny-3u3d-pp", "tiny-2u2d-doublemesh", "C2", "contracted-sph"])
 def test_candidate_ratios_match_full_wavefunction_recomputation(name):
     s = SYSTEMS[name](); o = ref.Ref(s); rng = np.random.default_rng(6)
     x = wl.initial_walkers(s, 1, 44)[0]; U = _rand_frame(rng)

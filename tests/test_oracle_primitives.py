@@ -145,6 +145,66 @@ def test_ao_gradient_and_laplacian_match_finite_differences(stype):
     assert np.allclose(l, lap_fd, atol=2e-7)
 
 
+def _contracted_d(zetas, coefs, sph, centre=(0.1, -0.2, 0.3), extra_s=None):
+    """One contracted d shell (and optionally one s primitive as a second contracted shell) on one centre."""
+    n = len(zetas); types = [wl.SHELL_D] * n; z = list(zetas); co = list(coefs); first = [0, n]; sp = [1 if sph else 0]
+    if extra_s is not None:
+        types.append(wl.SHELL_S); z.append(extra_s); co.append(1.0); first.append(n + 1); sp.append(0)
+    nao = wl.n_ao_contracted(types, first, sp)
+    return wl._system("contracted-d", [1.0], [list(centre)], 1, 0, [0] * len(types), types, z, np.eye(nao)[:, :1], np.zeros((nao, 0)), {}, 0.2,
+                      contraction=(first, co, sp))
+
+
+def test_solid_harmonic_d_shell_is_orthonormal_and_has_no_s_component():
+    """Scope row f2 (L242 "spherical (solid) harmonics").  For one primitive the five functions z2, xz, yz, x2-y2, xy are
+    orthonormal and orthogonal to an s Gaussian on the same centre, while the cartesian xx + yy + zz overlaps it: 3-D
+    Gauss-Hermite quadrature, exact for these polynomials.  Their polynomial parts are harmonic and homogeneous of degree 2."""
+    zeta = 0.8; c = np.array([0.1, -0.2, 0.3])
+    t, wq = np.polynomial.hermite.hermgauss(14)
+
+    def overlap(ctx):
+        S = 0.0
+        for ix, x in enumerate(v):
+            for iy, y in enumerate(v):
+                for iz, z in enumerate(v):
+                    val, _, _ = ctx.ao(c + np.array([x, y, z]))
+                    S = S + wv[ix] * wv[iy] * wv[iz] * np.outer(val, val) * math.exp(2 * zq * (x * x + y * y + z * z))
+        return S
+    # the s function takes the same exponent, so that every product is polynomial x exp(-2 zeta r^2): the rule is then exact
+    o = ref.Ref(_contracted_d([zeta], [1.0], True, extra_s=zeta)); oc = ref.Ref(_contracted_d([zeta], [1.0], False, extra_s=zeta))
+    zq = zeta; v = t / math.sqrt(2 * zq); wv = wq / math.sqrt(2 * zq)
+    S = overlap(o)
+    assert S.shape == (6, 6) and np.allclose(S, np.eye(6), atol=1e-12)        # 5 solid harmonics + s: orthonormal, no s contaminant
+    Sc = overlap(oc)
+    assert abs(Sc[0, 6] - Sc[3, 6]) < 1e-12 and Sc[0, 6] > 0.5                # cartesian xx, yy, zz each overlap the s function
+    # harmonic and homogeneous of degree 2: strip the Gaussian, check f(2 d) = 4 f(d) and the values against the explicit polynomials
+    d = np.array([0.7, -0.4, 0.25]); val, _, _ = o.ao(c + d); val2, _, _ = o.ao(c + 2 * d)
+    r2 = d @ d
+    f = val[:5] * math.exp(zeta * r2); f2 = val2[:5] * math.exp(zeta * 4 * r2)
+    assert np.allclose(f2, 4 * f, rtol=1e-12)
+    poly = np.array([(2 * d[2]**2 - d[0]**2 - d[1]**2) / (2 * math.sqrt(3)), d[0] * d[2], d[1] * d[2], (d[0]**2 - d[1]**2) / 2, d[0] * d[1]])
+    assert np.allclose(f / f[4], poly / poly[4], rtol=1e-12)
+
+
+def test_contracted_shell_is_the_stated_sum_of_normalised_primitives_with_correct_derivatives():
+    """chi = sum_k d_k chi_k^prim: value against the closed form of the normalised primitives written out here; gradient and
+    Laplacian against 4th-order finite differences."""
+    zs = [0.4, 1.1, 3.0]; ds = [0.7, -0.35, 0.2]; c = np.array([0.1, -0.2, 0.3])
+    o = ref.Ref(_contracted_d(zs, ds, True)); r0 = c + np.array([0.45, 0.3, -0.35]); d = r0 - c
+    val, g, l = o.ao(r0)
+    N110 = lambda z: (2 * z / math.pi) ** 0.75 * (4 * z)            # norm of the xy-type d primitive (unit self-overlap)
+    want_xy = sum(dk * N110(z) * d[0] * d[1] * math.exp(-z * (d @ d)) for z, dk in zip(zs, ds))
+    want_z2 = sum(dk * N110(z) * (2 * d[2]**2 - d[0]**2 - d[1]**2) / (2 * math.sqrt(3)) * math.exp(-z * (d @ d)) for z, dk in zip(zs, ds))
+    assert abs(val[4] - want_xy) < 1e-14 and abs(val[0] - want_z2) < 1e-14
+    h = 1e-3; f = lambda r: o.ao(r)[0]; lap_fd = 0.0
+    for ax in range(3):
+        e = np.zeros(3); e[ax] = h
+        g_fd = (-f(r0 + 2 * e) + 8 * f(r0 + e) - 8 * f(r0 - e) + f(r0 - 2 * e)) / (12 * h)
+        assert np.allclose(g[:, ax], g_fd, atol=1e-9)
+        lap_fd = lap_fd + (-f(r0 + 2 * e) + 16 * f(r0 + e) - 30 * f(r0) + 16 * f(r0 - e) - f(r0 - 2 * e)) / (12 * h * h)
+    assert np.allclose(l, lap_fd, atol=2e-7)
+
+
 def test_mo_is_ao_times_coefficients():
     s = wl.synthetic10(); o = ref.Ref(s); r = np.array([0.3, -0.8, 0.5])
     av, ag, al = o.ao(r); mv, mg, ml = o.mo(0, r)
