@@ -62,6 +62,17 @@ typedef struct {
     const int *type;    /* [n_shell] LRDMC_SHELL_*: cartesian Gaussian primitives s (1 AO), p (x,y,z),
                            d (xx,xy,xz,yy,yz,zz), each normalised to unit self-overlap; or Slater s exp(-zeta r) */
     const double *zeta; /* [n_shell] > 0 */
+    /* Contracted shells and real solid-harmonic d shells ("cc-pVTZ ... spherical (solid) harmonics"; L285).
+     * n_cshell == 0 / cs_first == NULL: every shell above is a basis function set of its own.  Else the shells above are
+     * PRIMITIVES and contracted shell cs is the run cs_first[cs] .. cs_first[cs+1]-1 (same centre, same type):
+     * chi_cs,c = sum_k prim_coef[k] chi^prim_k,c; a d shell with cs_sph[cs] != 0 carries the five functions
+     * z2 = zz - (xx+yy)/2, xz, yz, x2-y2 = (sqrt(3)/2)(xx - yy), xy of the normalised cartesian primitives (unit self-overlap
+     * each for one primitive).  lrdmc_mo.n_ao and C_up / C_dn then refer to the CONTRACTED functions; lrdmc_init folds the
+     * contraction into the primitive coefficient tables (host, once), the kernels are unchanged. */
+    int n_cshell;
+    const int *cs_first;      /* [n_cshell + 1] */
+    const double *prim_coef;  /* [n_shell] */
+    const int *cs_sph;        /* [n_cshell] */
 } lrdmc_basis;
 typedef struct {
     int n_ao;                 /* must equal the AO count implied by the shells */

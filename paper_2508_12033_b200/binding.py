@@ -26,7 +26,8 @@ class System(C.Structure):
 
 
 class Basis(C.Structure):
-    _fields_ = [("n_shell", C.c_int), ("center", C.c_void_p), ("type", C.c_void_p), ("zeta", C.c_void_p)]
+    _fields_ = [("n_shell", C.c_int), ("center", C.c_void_p), ("type", C.c_void_p), ("zeta", C.c_void_p),
+                ("n_cshell", C.c_int), ("cs_first", C.c_void_p), ("prim_coef", C.c_void_p), ("cs_sph", C.c_void_p)]
 
 
 class Mo(C.Structure):
@@ -137,12 +138,13 @@ class Lrdmc:
         self.sysd = sysd
         self.N = sysd["n_up"] + sysd["n_dn"]; self.n_up = sysd["n_up"]; self.n_dn = sysd["n_dn"]
         k = {n: (None if sysd.get(n) is None else np.ascontiguousarray(sysd[n])) for n in
-             ("Z", "R", "pp", "shell_center", "shell_type", "shell_zeta", "C_up", "C_dn", "c1", "b1", "nl")}
+             ("Z", "R", "pp", "shell_center", "shell_type", "shell_zeta", "C_up", "C_dn", "c1", "b1", "nl", "cs_first", "prim_coef", "cs_sph")}
         self._keep = k
         p = lambda a: None if a is None else a.ctypes.data
         s = System(sysd["n_nuc"], p(k["Z"]), p(k["R"]), sysd["n_up"], sysd["n_dn"], p(k["pp"]),
                    p(k["nl"]), int(sysd.get("nl_K", 0) or 0), int(sysd.get("nl_dla", 1)))
-        b = Basis(sysd["n_shell"], p(k["shell_center"]), p(k["shell_type"]), p(k["shell_zeta"]))
+        b = Basis(sysd["n_shell"], p(k["shell_center"]), p(k["shell_type"]), p(k["shell_zeta"]),
+                  0 if k["cs_sph"] is None else len(k["cs_sph"]), p(k["cs_first"]), p(k["prim_coef"]), p(k["cs_sph"]))
         m = Mo(sysd["n_ao"], p(k["C_up"]), p(k["C_dn"]))
         j = Jastrow(sysd["a_par"], sysd["a_anti"], sysd["b2"], p(k["c1"]), p(k["b1"]))
         la = Lattice(sysd["a"], sysd["a2"], sysd["seed"])

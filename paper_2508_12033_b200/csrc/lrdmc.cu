@@ -68,7 +68,38 @@ extern "C" int lrdmc_init(lrdmc_ctx **out, const lrdmc_system *sys, const lrdmc_
         if (g < 0 || bas->center[s] < 0 || bas->center[s] >= sys->n_nuc || !(bas->zeta[s] > 0.0)) return LRDMC_EINVAL;
         group[s] = g; ao0[s] = n_ao; n_ao += ncomp[g];
     }
-    if (n_ao != mo->n_ao) return LRDMC_EINVAL;
+    // ---- contracted / solid-harmonic shells: fold the contraction into primitive coefficient matrices (include/lrdmc.h, lrdmc_basis)
+    std::vector<double> Cfold[2];
+    const double *Cup = mo->C_up, *Cdn = mo->C_dn;
+    if (bas->n_cshell > 0 && bas->cs_first) {
+        if (!bas->prim_coef || !bas->cs_sph || bas->cs_first[0] != 0 || bas->cs_first[bas->n_cshell] != bas->n_shell) return LRDMC_EINVAL;
+        static const double h3 = 0.86602540378443864676;           // sqrt(3)/2;  rows: z2, xz, yz, x2-y2, xy over xx xy xz yy yz zz
+        static const double SPH[5][6] = { { -0.5, 0, 0, -0.5, 0, 1.0 }, { 0, 0, 1, 0, 0, 0 }, { 0, 0, 0, 0, 1, 0 }, { h3, 0, 0, -h3, 0, 0 }, { 0, 1, 0, 0, 0, 0 } };
+        int nc = 0;
+        for (int cs = 0; cs < bas->n_cshell; ++cs) {
+            const int k0 = bas->cs_first[cs], k1 = bas->cs_first[cs + 1];
+            if (k1 <= k0) return LRDMC_EINVAL;
+            for (int k = k0; k < k1; ++k) if (bas->type[k] != bas->type[k0] || bas->center[k] != bas->center[k0]) return LRDMC_EINVAL;
+            nc += (group[k0] == 3 && bas->cs_sph[cs]) ? 5 : ncomp[group[k0]];
+        }
+        if (nc != mo->n_ao) return LRDMC_EINVAL;
+        for (int sp = 0; sp < 2; ++sp) {
+            const int ns = sp ? sys->n_dn : sys->n_up; const double *C = sp ? mo->C_dn : mo->C_up;
+            Cfold[sp].assign((size_t)n_ao * (ns > 0 ? ns : 1), 0.0);
+            int nu0 = 0;
+            for (int cs = 0; cs < bas->n_cshell; ++cs) {
+                const int k0 = bas->cs_first[cs], k1 = bas->cs_first[cs + 1], g = group[k0];
+                const bool sph = g == 3 && bas->cs_sph[cs];
+                const int nfun = sph ? 5 : ncomp[g];
+                for (int k = k0; k < k1; ++k) for (int q = 0; q < ncomp[g]; ++q) for (int f = 0; f < nfun; ++f) {
+                    const double w = bas->prim_coef[k] * (sph ? SPH[f][q] : (f == q ? 1.0 : 0.0));
+                    if (w != 0.0) for (int m = 0; m < ns; ++m) Cfold[sp][(size_t)(ao0[k] + q) * ns + m] += w * C[(size_t)(nu0 + f) * ns + m];
+                }
+                nu0 += nfun;
+            }
+        }
+        Cup = Cfold[0].data(); Cdn = Cfold[1].data();
+    } else if (n_ao != mo->n_ao) return LRDMC_EINVAL;
     lrdmc_ctx *c = (lrdmc_ctx *)calloc(1, sizeof(lrdmc_ctx));
     DevSys &S = c->S;
     S.N = sys->n_up + sys->n_dn; S.n_up = sys->n_up; S.n_dn = sys->n_dn; S.n_nuc = sys->n_nuc;
@@ -101,7 +132,7 @@ extern "C" int lrdmc_init(lrdmc_ctx **out, const lrdmc_system *sys, const lrdmc_
     int omax = sys->n_up > sys->n_dn ? sys->n_up : sys->n_dn, nt = (omax + 7) / 8;
     c->NT = nt <= 1 ? 1 : (nt == 2 ? 2 : 4);
     S.NT[0] = S.NT[1] = c->NT; S.OS = 8 * c->NT; S.dinv_rows[0] = S.dinv_rows[1] = 8 * c->NT;
-    S.same_C = (sys->n_dn == 0) || (sys->n_dn == sys->n_up && (mo->C_dn == mo->C_up || !memcmp(mo->C_up, mo->C_dn, sizeof(double) * (size_t)n_ao * sys->n_up)));
+    S.same_C = (sys->n_dn == 0) || (sys->n_dn == sys->n_up && (Cdn == Cup || !memcmp(Cup, Cdn, sizeof(double) * (size_t)n_ao * sys->n_up)));
     // ---- host images of the tables
     std::vector<double> h_sh((size_t)S.n_slots * 4), h_nuc((size_t)S.n_nuc * LRDMC_NUC_STRIDE, 0.0);
     for (int q = 0; q < S.n_slots; ++q) {
@@ -121,7 +152,7 @@ extern "C" int lrdmc_init(lrdmc_ctx **out, const lrdmc_system *sys, const lrdmc_
     std::vector<double> h_bf[2], h_et(256);
     for (int j = 0; j < 256; ++j) h_et[j] = exp2((double)j / 256.0);       // table of exp_tab
     for (int sp = 0; sp < (S.same_C ? 1 : 2); ++sp) {
-        const int ns = sp ? sys->n_dn : sys->n_up; const double *C = sp ? mo->C_dn : mo->C_up;
+        const int ns = sp ? sys->n_dn : sys->n_up; const double *C = sp ? Cdn : Cup;
         h_bf[sp].assign(bf_n, 0.0);
         int kstep = 0;
         for (int g = 0; g < 4; ++g) for (int it = 0; it < S.n_it[g]; ++it) for (int comp = 0; comp < ncomp[g]; ++comp, ++kstep)
@@ -142,7 +173,7 @@ extern "C" int lrdmc_init(lrdmc_ctx **out, const lrdmc_system *sys, const lrdmc_
     const size_t cf_n = LRDMC_BC_DMMA ? (size_t)S.n_kpairs * NA * 32 : 0;
     std::vector<double> h_cf[2];
     for (int sp = 0; sp < (S.same_C ? 1 : 2) && cf_n; ++sp) {
-        const int ns = sp ? sys->n_dn : sys->n_up; const double *C = sp ? mo->C_dn : mo->C_up;
+        const int ns = sp ? sys->n_dn : sys->n_up; const double *C = sp ? Cdn : Cup;
         h_cf[sp].assign(cf_n, 0.0);
         for (int g = 0; g < 4; ++g) for (int it = 0; it < S.n_it[g]; ++it) for (int comp = 0; comp < ncomp[g]; ++comp) {
             const int q = it * ncomp[g] + comp, pair = pair_base[g] + q / 2, par = q & 1;

@@ -54,6 +54,11 @@ SYSTEMS = {
     "ragged-9u4d-nlDLA": lambda: _with_walkers(wl.random_nonlocal(wl.tiny_molecule(9, 4, 4, 20, seed=11), 6, 1.2, 2, True), 13),
     "C3-water-methane-nlDLA": lambda: _with_walkers(wl.water_methane_nonlocal(n_walkers=100), 100),
     "C3-water-methane-nlTM": lambda: _with_walkers(wl.water_methane_nonlocal(n_walkers=50, dla=False), 50),
+    # scope row f2: contracted shells and real solid-harmonic d shells (the oracle evaluates the contracted functions themselves,
+    # lrdmc_init folds the contraction into its primitive coefficient tables)
+    "contracted-3u2d-sph-pp": lambda: _with_walkers(wl.contracted_molecule(3, 2, 3, 9, seed=31, spherical=True, with_pp=True), 37),
+    "contracted-9u7d-cart": lambda: _with_walkers(wl.contracted_molecule(9, 7, 4, 21, seed=32, spherical=False), 21),
+    "contracted-4u4d-sph-nlDLA": lambda: _with_walkers(wl.random_nonlocal(wl.contracted_molecule(4, 4, 3, 12, seed=33, spherical=True, with_pp=True), 9, 1.5, 2, True, scale=100.0), 29),
 }
 
 
@@ -145,7 +150,7 @@ def test_whole_cycle_trajectories_weights_and_branching(B, name, mode, kernel, m
                                        ("ragged-17u3d-NT4", "conventional"), ("he-triplet-slater", "balanced"), ("C3-water-methane-shaped", "balanced"),
                                        ("C3-water-methane-shaped", "conventional"), ("C5-cluster64-doublemesh", "balanced"),
                                        ("tiny-3u2d-nlDLA-strong", "balanced"), ("tiny-2u1d-nlTM-strong", "conventional"), ("C3-water-methane-nlDLA", "balanced"),
-                                       ("C3-water-methane-nlTM", "balanced")])
+                                       ("C3-water-methane-nlTM", "balanced"), ("contracted-4u4d-sph-nlDLA", "balanced")])
 def test_team_kernel_every_team_size(B, name, mode, tw, monkeypatch):
     """k_propagate_team with TW = 2, 4, 8, 16 warps per walker (work units = electron blocks x shell parts, partial sums
     in shared memory): same trajectories, weights and indices as the oracle."""
