@@ -127,6 +127,109 @@ __device__ __forceinline__ bool nl_pass(const DevSys &S, const WarpState &ws, co
     return true;
 }
 
+// Phase B of a system WITH non-local slots, by one warp: lattice blocks and slot blocks go through ONE loop with ONE ao_columns /
+// pade_six call site (a slot pass is a lattice pass about the centre R_I with step r_iI).  Two inlined copies of the shell sweep
+// doubled the hot instruction footprint: ncu showed 2.3 "no instruction" stall cycles per issue and the kernel at 35 % issue
+// utilisation.  Returns the node flag raised by the slots (rho_q < 0).
+template <int NT, bool TS>
+__device__ __forceinline__ int phase_b_with_nonlocal(const DevSys &S, const WarpState &ws, const Tables &T, const double *Jold, int lane)
+{
+    const int t = lane & 3, g = lane >> 2, N = S.N, K = S.nl_K, n_nuc = S.n_nuc;
+    const int nb0 = (S.n_up + 7) / 8, nbm = nb0 + (S.n_dn + 7) / 8, n_lat = S.n_mesh * nbm;
+    // Slots in range of a centre are few (about 2.5 of 16 at C3): list them first (lane per slot, ballot), then sweep 8 LISTED
+    // slots per pass.  With one coefficient table for both spins (same_C) a pass may mix spins (per-lane inverse, per-lane n_s);
+    // otherwise the list is cut at the first spin-down slot.  The list lives in the cumulative-sum array (free until phase C).
+    int *list = reinterpret_cast<int *>(ws.cum);
+    int n_act = 0, n_act_up = 0;
+    for (int s0 = 0; s0 < N * K; s0 += 32) {
+        const int sl = s0 + lane; const bool in = sl < N * K;
+        const int i = in ? sl / K : 0, kk = in ? sl - i * K : 0;
+        double r;
+        const bool act = in && nl_centre(S, T.nuc, ws.r[3 * i], ws.r[3 * i + 1], ws.r[3 * i + 2], kk, r) >= 0;
+        const unsigned m = __ballot_sync(0xffffffffu, act);
+        if (act) list[n_act + __popc(m & ((1u << lane) - 1u))] = sl;
+        if (in) { double *Ro = ws.R + S.P_lat + 6 * sl;
+#pragma unroll
+            for (int d = 0; d < 6; ++d) Ro[d] = 0.0; }
+        n_act_up += __popc(__ballot_sync(0xffffffffu, act && i < S.n_up));
+        n_act += __popc(m);
+    }
+    __syncwarp();
+    const int cut = S.same_C ? n_act : n_act_up;                    // passes never straddle `cut`
+    const int n_p0 = (cut + 7) / 8, n_nlp = n_p0 + (n_act - cut + 7) / 8;
+    int node_nl = 0;
+    for (int pass = 0; pass < n_lat + n_nlp; ++pass) {
+        const bool is_nl = pass >= n_lat;
+        int sp, il, kk = 0, mesh = 0, i; bool valid;
+        if (!is_nl) {
+            mesh = pass / nbm; const int rem = pass - mesh * nbm; sp = rem >= nb0 ? 1 : 0;
+            const int il0 = 8 * (sp ? rem - nb0 : rem), ns_ = sp ? S.n_dn : S.n_up;
+            valid = il0 + g < ns_; il = valid ? il0 + g : 0; i = (sp ? S.n_up : 0) + il;
+        } else {
+            const int b = pass - n_lat, lo = b < n_p0 ? 8 * b : cut + 8 * (b - n_p0), hi = b < n_p0 ? cut : n_act;
+            valid = lo + g < hi;
+            const int sl = list[valid ? lo + g : lo];               // an idle row repeats the pass's first slot (its result is dropped)
+            i = sl / K; kk = sl - i * K; sp = i < S.n_up ? 0 : 1; il = sp ? i - S.n_up : i;
+        }
+        const int ns = sp ? S.n_dn : S.n_up;
+        const double xi = ws.r[3 * i], yi = ws.r[3 * i + 1], zi = ws.r[3 * i + 2];
+        double x0 = xi, y0 = yi, z0 = zi, step = S.amesh[mesh], r = 0.0;
+        const double *nu = T.nuc;
+        if (is_nl) {
+            const int I = nl_centre(S, T.nuc, xi, yi, zi, kk, r);   // listed slots are in range: I >= 0
+            nu = T.nuc + I * LRDMC_NUC_STRIDE; x0 = nu[0]; y0 = nu[1]; z0 = nu[2]; step = r;
+        }
+        const double a2 = step * step;
+        double av[3][3];
+#pragma unroll
+        for (int k = 0; k < 3; ++k) { av[k][0] = step * ws.U[k]; av[k][1] = step * ws.U[3 + k]; av[k][2] = step * ws.U[6 + k]; }
+        double acc[6], Jn[6];
+        ao_columns<NT, TS>(S, T.shells, sp ? T.cf[1] : T.cf[0], T.etab, sp ? ws.dinv[1] : ws.dinv[0], ns, il, x0, y0, z0, av, a2, lane, acc);
+#pragma unroll
+        for (int d = 0; d < 6; ++d) Jn[d] = 0.0;
+        if (!is_nl || !S.nl_dla) {
+            if (S.has_j1) for (int I = t; I < n_nuc; I += 4) {
+                const double *np_ = T.nuc + I * LRDMC_NUC_STRIDE;
+                pade_six(x0 - np_[0], y0 - np_[1], z0 - np_[2], av, a2, -np_[4], np_[5], Jn);
+            }
+            for (int j = t; j < N; j += 4) {
+                const double c = (j == i) ? 0.0 : ((spin_of(S, j) == sp) ? S.a_par : S.a_anti);
+                pade_six(x0 - ws.r[3 * j], y0 - ws.r[3 * j + 1], z0 - ws.r[3 * j + 2], av, a2, c, S.b2, Jn);
+            }
+        }
+        const double Jo = Jold[i];
+        if (!is_nl) {
+            double Rv[6];
+#pragma unroll
+            for (int d = 0; d < 6; ++d) Rv[d] = quad_sum(acc[d]) * exp_tab(quad_sum(Jn[d]) - Jo, T.etab);
+            if (valid && t == 0) { double *Ro = ws.R + mesh * 6 * N + 6 * i;
+#pragma unroll
+                for (int d = 0; d < 6; ++d) Ro[d] = Rv[d]; }
+        } else {
+            double nuq[6];
+            {
+                const double ir = 1.0 / r, hx = (xi - nu[0]) * ir, hy = (yi - nu[1]) * ir, hz = (zi - nu[2]) * ir;   // rhat of the electron about the centre
+                const double r2 = r * r, *ch = nu + LRDMC_NL_OFF;
+                const double v0 = ch[1] * exp_nonpos(-ch[2] * r2), v1 = 3.0 * ch[3] * exp_nonpos(-ch[4] * r2), v2 = 5.0 * ch[5] * exp_nonpos(-ch[6] * r2);
+#pragma unroll
+                for (int k = 0; k < 3; ++k) {
+                    const double ct = ws.U[k] * hx + ws.U[3 + k] * hy + ws.U[6 + k] * hz, p2 = 0.5 * (3.0 * ct * ct - 1.0);
+                    nuq[2 * k] = (v0 + v1 * ct + v2 * p2) * (1.0 / 6.0);
+                    nuq[2 * k + 1] = (v0 - v1 * ct + v2 * p2) * (1.0 / 6.0);
+                }
+            }
+            double *Ro = ws.R + S.P_lat + 6 * (i * K + kk);
+#pragma unroll
+            for (int d = 0; d < 6; ++d) {
+                double rho = quad_sum(acc[d]);
+                if (!S.nl_dla) rho *= exp_tab(quad_sum(Jn[d]) - Jo, T.etab);
+                if (valid && t == 0) { Ro[d] = -nuq[d] * rho; if (rho < 0.0) node_nl = 1; }
+            }
+        }
+    }
+    return node_nl;
+}
+
 // Position an accepted move j puts its electron at: lattice hop r_i +- a e_k, or the quadrature point of a non-local slot.
 template <bool NL>
 __device__ __forceinline__ void move_target(const DevSys &S, const WarpState &ws, const double *nuc, int j, int &i, double &px, double &py, double &pz)
@@ -244,7 +347,7 @@ __device__ __forceinline__ EvalOut evaluate_walker(const DevSys &S, const WarpSt
 
     // ---- phase B (rows a1-a5): the 6 n_s candidates of each spin, 8 electrons (48 points) per warp pass in column form
 #ifndef LRDMC_CONTRACTION_MO
-    for (int mesh = 0; mesh < S.n_mesh; ++mesh) {
+    if (!NL) for (int mesh = 0; mesh < S.n_mesh; ++mesh) {
         const double am = S.amesh[mesh], a2 = am * am;
         double av[3][3];                                             // av[k] = a e_k, e_k = k-th column of U (Eq.D3-D4)
 #pragma unroll
@@ -342,29 +445,9 @@ __device__ __forceinline__ EvalOut evaluate_walker(const DevSys &S, const WarpSt
         }
     }
 #endif
-    // ---- non-local pseudopotential slots (row f1): 8 slots per warp pass, whole shell list
+    // ---- systems with non-local pseudopotential slots (row f1): lattice blocks and slot blocks in one loop
     int node_nl = 0;
-    if (NL) {
-        for (int sp = 0; sp < 2; ++sp) {
-            const int nslot = (sp ? S.n_dn : S.n_up) * S.nl_K;
-            for (int s0 = 0; s0 < nslot; s0 += 8) {
-                double acc[6], Jn[6], nuq[6]; bool valid, active; int i, slot;
-                const bool any = nl_pass<NT, TS, false>(S, ws, T, sp, s0, lane, acc, Jn, nuq, valid, active, i, slot);
-                double *Ro = ws.R + S.P_lat + 6 * slot;
-                if (!any) { if (valid && t == 0) {
-#pragma unroll
-                        for (int d = 0; d < 6; ++d) Ro[d] = 0.0; }
-                    continue; }
-                const double Jo = Jold[i];
-#pragma unroll
-                for (int d = 0; d < 6; ++d) {
-                    double rho = quad_sum(acc[d]);
-                    if (!S.nl_dla) rho *= exp_tab(quad_sum(Jn[d]) - Jo, T.etab);
-                    if (valid && t == 0) { Ro[d] = active ? -nuq[d] * rho : 0.0; if (active && rho < 0.0) node_nl = 1; }
-                }
-            }
-        }
-    }
+    if (NL) node_nl = phase_b_with_nonlocal<NT, TS>(S, ws, T, Jold, lane);
     __syncwarp();
 
     const EvalOut o = phase_c<NL>(S, ws, lap_s, Vee, lane, node_nl);
