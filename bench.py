@@ -113,7 +113,7 @@ def main():
     ap.add_argument("--impl", default="ours"); ap.add_argument("--nw", type=int, default=25600); ap.add_argument("--moves", type=int, default=100)
     ap.add_argument("--ref-nw", type=int, default=64); ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-conventional", action="store_true"); ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--workload", default="C4", choices=["C2", "C4", "C5", "C3nl"],
+    ap.add_argument("--workload", default="C4", choices=["C1", "C2", "C4", "C5", "C3nl"],
                     help="C4 (default) is the configuration the metric is quoted on; C2 / C5 are the other BASELINE.json systems, C3nl adds non-local pseudopotential channels (use with --nw/--moves)")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1")); local = int(os.environ.get("LOCAL_RANK", "0"))
@@ -134,6 +134,9 @@ def main():
     if args.workload == "C4":
         sysd = wl.water_methane(n_walkers=args.nw, moves=args.moves, seed=wl.PHILOX_RUN_SEED + rank, name="C4-water-methane-shaped")
         wname = "C4 water-methane-shaped: 16 e (8/8), 8 nuclei, 200 s/p/d GTOs, local PP, 1b+2b Jastrow, a=0.2 (BASELINE.json configs[3])"
+    elif args.workload == "C1":
+        sysd = wl.hydrogen(n_walkers=args.nw, moves=args.moves, seed=wl.PHILOX_RUN_SEED + rank)
+        wname = "C1 hydrogen atom: 1 e, psi = exp(-0.9 r), a=0.2 (BASELINE.json configs[0])"
     elif args.workload == "C2":
         sysd = wl.synthetic10(n_walkers=args.nw, moves=args.moves, seed=wl.PHILOX_RUN_SEED + rank)
         wname = "C2 synthetic 10-electron molecule: 5/5, 3 nuclei, 60 s/p/d GTOs, 1b+2b Jastrow, a=0.2 (BASELINE.json configs[1])"
@@ -143,7 +146,7 @@ def main():
     else:
         sysd = wl.cluster64(n_walkers=args.nw, moves=args.moves, seed=wl.PHILOX_RUN_SEED + rank)
         wname = "C5 64-electron cluster: 32/32, 24 nuclei, 600 s/p/d GTOs, 1b+2b Jastrow, double mesh a=0.2/a'=0.4 (BASELINE.json configs[4])"
-    x0 = wl.initial_walkers(sysd, args.nw, 5 + rank)
+    x0 = wl.hydrogen_walkers(args.nw, 1 + rank) if args.workload == "C1" else wl.initial_walkers(sysd, args.nw, 5 + rank)
     g = B.Lrdmc(sysd, device=dev)
     g.lrdmc_set_positions(x0, allow_singular=True)
     E0 = 0.0          # fixed Green's-function energy for the timing runs (W ~ 3N/a^2 = 1200 >> e_L; nonpos events are reported)
