@@ -73,62 +73,10 @@ __device__ __forceinline__ int nl_centre(const DevSys &S, const double *nuc, dou
     return -1;
 }
 
-// One pass over 8 non-local slots of spin sp (slot = (electron il, rank kk), lane = 4 g + t handles slot s0 + g): the six
-// quadrature points R_I +- r_iI e_k have exactly the +-(a e_k) structure of the lattice hops about the CENTRE R_I with step
-// r_iI, so the determinant ratios come from the same ao_columns (per-lane x0 = R_I, av = r_iI e_k, a2 = r_iI^2), and the
-// Jastrow ratios (nl_dla == 0) from the same pade_six.  nu_q = (1/6) sum_l (2l+1) v_l(r) P_l(+-e_k . rhat).
-// Output (lanes t == 0 of valid slots): acc6 = determinant-ratio share of this shell part, jn6 = Jastrow share, nu6.
-// Returns false (nothing computed) when no slot of the pass is active.
-template <int NT, bool TS, bool PART>
-__device__ __forceinline__ bool nl_pass(const DevSys &S, const WarpState &ws, const Tables &T, int sp, int s0, int lane,
-                                        double (&acc)[6], double (&Jn)[6], double (&nuq)[6], bool &valid, bool &active, int &i_out, int &slot_out,
-                                        const TeamPlan *tp = nullptr, const ShellPart *part = nullptr, int jpart = 0, int jparts = 1)
-{
-    const int t = lane & 3, g = lane >> 2, K = S.nl_K;
-    const int ns = sp ? S.n_dn : S.n_up, off = sp ? S.n_up : 0;
-    valid = s0 + g < ns * K;
-    const int sidx = valid ? s0 + g : 0, il = sidx / K, kk = sidx - il * K, i = off + il;
-    i_out = i; slot_out = i * K + kk;
-    const double xi = ws.r[3 * i], yi = ws.r[3 * i + 1], zi = ws.r[3 * i + 2];
-    double r;
-    const int I = valid ? nl_centre(S, T.nuc, xi, yi, zi, kk, r) : -1;
-    active = I >= 0;
-    if (!__any_sync(0xffffffffu, active)) return false;
-    const double *nu = T.nuc + (active ? I : 0) * LRDMC_NUC_STRIDE;
-    const double x0 = active ? nu[0] : xi, y0 = active ? nu[1] : yi, z0 = active ? nu[2] : zi;
-    const double rr = active ? r : 0.0, a2 = rr * rr;
-    double av[3][3];                                             // av[k] = r_iI e_k
-#pragma unroll
-    for (int k = 0; k < 3; ++k) { av[k][0] = rr * ws.U[k]; av[k][1] = rr * ws.U[3 + k]; av[k][2] = rr * ws.U[6 + k]; }
-    ao_columns<NT, TS, PART>(S, T.shells, sp ? T.cf[1] : T.cf[0], T.etab, sp ? ws.dinv[1] : ws.dinv[0], ns, il, x0, y0, z0, av, a2, lane, acc, tp, part);
-#pragma unroll
-    for (int d = 0; d < 6; ++d) { Jn[d] = 0.0; nuq[d] = 0.0; }
-    if (!S.nl_dla) {                                             // full ratio: Jastrow part at the quadrature points
-        if (S.has_j1) for (int Ip = t + 4 * jpart; Ip < S.n_nuc; Ip += 4 * jparts) {
-            const double *np_ = T.nuc + Ip * LRDMC_NUC_STRIDE;
-            pade_six(x0 - np_[0], y0 - np_[1], z0 - np_[2], av, a2, -np_[4], np_[5], Jn);
-        }
-        for (int j = t + 4 * jpart; j < S.N; j += 4 * jparts) {
-            const double c = (j == i) ? 0.0 : ((spin_of(S, j) == sp) ? S.a_par : S.a_anti);
-            pade_six(x0 - ws.r[3 * j], y0 - ws.r[3 * j + 1], z0 - ws.r[3 * j + 2], av, a2, c, S.b2, Jn);
-        }
-    }
-    if (active) {
-        const double ir = 1.0 / r, hx = (xi - nu[0]) * ir, hy = (yi - nu[1]) * ir, hz = (zi - nu[2]) * ir;   // rhat of the electron about the centre
-        const double r2 = r * r, *ch = nu + LRDMC_NL_OFF;
-        const double v0 = ch[1] * exp_nonpos(-ch[2] * r2), v1 = 3.0 * ch[3] * exp_nonpos(-ch[4] * r2), v2 = 5.0 * ch[5] * exp_nonpos(-ch[6] * r2);
-#pragma unroll
-        for (int k = 0; k < 3; ++k) {
-            const double ct = ws.U[k] * hx + ws.U[3 + k] * hy + ws.U[6 + k] * hz, p2 = 0.5 * (3.0 * ct * ct - 1.0);
-            nuq[2 * k] = (v0 + v1 * ct + v2 * p2) * (1.0 / 6.0);
-            nuq[2 * k + 1] = (v0 - v1 * ct + v2 * p2) * (1.0 / 6.0);
-        }
-    }
-    return true;
-}
-
 // Phase B of a system WITH non-local slots, by one warp: lattice blocks and slot blocks go through ONE loop with ONE ao_columns /
-// pade_six call site (a slot pass is a lattice pass about the centre R_I with step r_iI).  Two inlined copies of the shell sweep
+// pade_six call site.  The six quadrature points R_I +- r_iI e_k of a slot have exactly the +-(a e_k) structure of the lattice hops,
+// about the CENTRE R_I with step r_iI, so a slot pass is a lattice pass with per-lane arguments (x0 = R_I, av = r_iI e_k, the
+// Dinv column of the slot's electron); nu_q = (1/6) sum_l (2l+1) v_l(r) P_l(+-e_k . rhat).  Two inlined copies of the shell sweep
 // doubled the hot instruction footprint: ncu showed 2.3 "no instruction" stall cycles per issue and the kernel at 35 % issue
 // utilisation.  Returns the node flag raised by the slots (rho_q < 0).
 template <int NT, bool TS>

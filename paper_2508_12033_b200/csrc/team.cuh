@@ -91,74 +91,109 @@ __device__ __forceinline__ EvalOut evaluate_team(const DevSys &S, const TeamPlan
         vee_part = warp_sum(vee_part);
         if (lane == 0) s_vee[wt] = vee_part;
     }
+    if (NL && wt == TW - 1) {        // list the slots in range of a centre (ballot), clear the others; list in ws.cum (free until phase C)
+        int *lst = reinterpret_cast<int *>(ws.cum);
+        const int Kk = S.nl_K; int na = 0, nup = 0;
+        for (int s0 = 0; s0 < N * Kk; s0 += 32) {
+            const int sl = s0 + lane; const bool in = sl < N * Kk;
+            const int i = in ? sl / Kk : 0, kk = in ? sl - i * Kk : 0;
+            double r;
+            const bool act = in && nl_centre(S, T.nuc, ws.r[3 * i], ws.r[3 * i + 1], ws.r[3 * i + 2], kk, r) >= 0;
+            const unsigned m = __ballot_sync(0xffffffffu, act);
+            if (act) lst[na + __popc(m & ((1u << lane) - 1u))] = sl;
+            if (in) {
+                if (NP == 1) { double *Ro = ws.R + S.P_lat + 6 * sl;
+#pragma unroll
+                    for (int d = 0; d < 6; ++d) Ro[d] = 0.0; }
+                else scr[P.o_nu + (size_t)sl * 7 + 6] = 0.0;
+            }
+            nup += __popc(__ballot_sync(0xffffffffu, act && i < S.n_up));
+            na += __popc(m);
+        }
+        if (lane == 0) { s_node[1] = na; s_node[2] = S.same_C ? na : nup; }
+    }
     __syncthreads();
 
-    // ---- phase B (rows a1-a5): work units (mesh, spin, 8-electron block, shell part); unit u -> warp u mod TW
-    const int nb_mesh = P.nblk[0] + P.nblk[1];
-    for (int v = wt; v < P.n_units + (NL ? P.n_units_nl : 0); v += TW) {
-        if (NL && v >= P.n_units) {            // non-local pseudopotential slots (row f1): unit = (spin, 8-slot block, shell part)
-            const int u = v - P.n_units, part = u % NP, blk = u / NP, sp = blk >= P.nblk_nl[0] ? 1 : 0, s0 = 8 * (sp ? blk - P.nblk_nl[0] : blk);
-            double acc[6], Jn[6], nuq[6]; bool valid, active; int i, slot;
-            const bool any = nl_pass<NT, TS, true>(S, ws, T, sp, s0, lane, acc, Jn, nuq, valid, active, i, slot, &P, &P.col[part], part, NP);
-            if (NP == 1) {
-                double *Ro = ws.R + S.P_lat + 6 * slot;
-                const double Jo = Jold[i];
-#pragma unroll
-                for (int d = 0; d < 6; ++d) {
-                    double rho = any ? quad_sum(acc[d]) : 0.0;
-                    if (any && !S.nl_dla) rho *= exp_tab(quad_sum(Jn[d]) - Jo, T.etab);
-                    if (valid && t == 0) { Ro[d] = (any && active) ? -nuq[d] * rho : 0.0; if (any && active && rho < 0.0) atomicOr(s_node, 1); }
-                }
-            } else {
-                double *q = scr + P.o_nl + ((size_t)slot * NP + part) * 12, *qn = scr + P.o_nu + (size_t)slot * 7;
-#pragma unroll
-                for (int d = 0; d < 6; ++d) {
-                    const double A = any ? quad_sum(acc[d]) : 0.0, J = any ? quad_sum(Jn[d]) : 0.0;
-                    if (valid && t == 0) { q[d] = A; q[6 + d] = J; if (part == 0) qn[d] = (any && active) ? nuq[d] : 0.0; }
-                }
-                if (valid && t == 0 && part == 0) qn[6] = (any && active) ? 1.0 : 0.0;
-            }
-            continue;
+    // ---- phase B (rows a1-a5, f1): work units (mesh, spin, 8-electron block, shell part) and, with non-local slots, (pass of 8
+    //      LISTED slots, shell part); unit v -> warp v mod TW.  One loop, one ao_columns call site for both kinds.
+    const int nb_mesh = P.nblk[0] + P.nblk[1], K = S.nl_K;
+    const int *list = reinterpret_cast<const int *>(ws.cum);
+    const int n_act = NL ? s_node[1] : 0, cut = NL ? s_node[2] : 0, n_p0 = (cut + 7) / 8, n_nlp = n_p0 + (n_act - cut + 7) / 8;
+    for (int v = wt; v < P.n_units + n_nlp * NP; v += TW) {
+        const bool is_nl = NL && v >= P.n_units;
+        const int u = is_nl ? v - P.n_units : v, part = u % NP, blk = u / NP;
+        int sp, il, i, kk = 0, mesh = 0; bool valid;
+        if (!is_nl) {
+            mesh = blk / nb_mesh; const int rem = blk - mesh * nb_mesh; sp = rem >= P.nblk[0] ? 1 : 0;
+            const int il0 = 8 * (sp ? rem - P.nblk[0] : rem), ns_ = sp ? S.n_dn : S.n_up;
+            valid = il0 + g < ns_; il = valid ? il0 + g : 0; i = (sp ? S.n_up : 0) + il;
+        } else {
+            const int lo = blk < n_p0 ? 8 * blk : cut + 8 * (blk - n_p0), hi = blk < n_p0 ? cut : n_act;
+            valid = lo + g < hi;
+            const int sl = list[valid ? lo + g : lo];
+            i = sl / K; kk = sl - i * K; sp = i < S.n_up ? 0 : 1; il = sp ? i - S.n_up : i;
         }
-        const int u = v;
-        const int part = u % NP, blk = u / NP, mesh = blk / nb_mesh, rem = blk - mesh * nb_mesh;
-        const int sp = rem >= P.nblk[0] ? 1 : 0, il0 = 8 * (sp ? rem - P.nblk[0] : rem);
-        const int ns = sp ? S.n_dn : S.n_up, off = sp ? S.n_up : 0;
-        const double am = S.amesh[mesh], a2 = am * am;
+        const int ns = sp ? S.n_dn : S.n_up;
+        const double xi = ws.r[3 * i], yi = ws.r[3 * i + 1], zi = ws.r[3 * i + 2];
+        double x0 = xi, y0 = yi, z0 = zi, step = S.amesh[mesh], r = 0.0;
+        const double *nu = T.nuc;
+        if (is_nl) {
+            const int I = nl_centre(S, T.nuc, xi, yi, zi, kk, r);   // listed slots are in range
+            nu = T.nuc + I * LRDMC_NUC_STRIDE; x0 = nu[0]; y0 = nu[1]; z0 = nu[2]; step = r;
+        }
+        const double a2 = step * step;
         double av[3][3];
 #pragma unroll
-        for (int k = 0; k < 3; ++k) { av[k][0] = am * ws.U[k]; av[k][1] = am * ws.U[3 + k]; av[k][2] = am * ws.U[6 + k]; }
-        const bool valid = il0 + g < ns;
-        const int il = valid ? il0 + g : 0, i = off + il;
-        const double x0 = ws.r[3 * i], y0 = ws.r[3 * i + 1], z0 = ws.r[3 * i + 2];
+        for (int k = 0; k < 3; ++k) { av[k][0] = step * ws.U[k]; av[k][1] = step * ws.U[3 + k]; av[k][2] = step * ws.U[6 + k]; }
         double acc[6], Jn[6];
         ao_columns<NT, TS, true>(S, T.shells, sp ? T.cf[1] : T.cf[0], T.etab, sp ? ws.dinv[1] : ws.dinv[0], ns, il, x0, y0, z0, av, a2, lane, acc, &P, &P.col[part]);
 #pragma unroll
         for (int d = 0; d < 6; ++d) Jn[d] = 0.0;
-        if (S.has_j1) for (int I = t + 4 * part; I < n_nuc; I += 4 * NP) {
-            const double *nu = T.nuc + I * LRDMC_NUC_STRIDE;
-            pade_six(x0 - nu[0], y0 - nu[1], z0 - nu[2], av, a2, -nu[4], nu[5], Jn);
+        if (!is_nl || !S.nl_dla) {
+            if (S.has_j1) for (int I = t + 4 * part; I < n_nuc; I += 4 * NP) {
+                const double *np_ = T.nuc + I * LRDMC_NUC_STRIDE;
+                pade_six(x0 - np_[0], y0 - np_[1], z0 - np_[2], av, a2, -np_[4], np_[5], Jn);
+            }
+            for (int j = t + 4 * part; j < N; j += 4 * NP) {
+                const double c = (j == i) ? 0.0 : ((spin_of(S, j) == sp) ? S.a_par : S.a_anti);
+                pade_six(x0 - ws.r[3 * j], y0 - ws.r[3 * j + 1], z0 - ws.r[3 * j + 2], av, a2, c, S.b2, Jn);
+            }
         }
-        for (int j = t + 4 * part; j < N; j += 4 * NP) {
-            const double c = (j == i) ? 0.0 : ((spin_of(S, j) == sp) ? S.a_par : S.a_anti);
-            pade_six(x0 - ws.r[3 * j], y0 - ws.r[3 * j + 1], z0 - ws.r[3 * j + 2], av, a2, c, S.b2, Jn);
+        double nuq[6];
+#pragma unroll
+        for (int d = 0; d < 6; ++d) nuq[d] = 0.0;
+        if (is_nl && part == 0) {                                    // nu_q = (1/6) sum_l (2l+1) v_l(r) P_l(+-e_k . rhat)
+            const double ir = 1.0 / r, hx = (xi - nu[0]) * ir, hy = (yi - nu[1]) * ir, hz = (zi - nu[2]) * ir;
+            const double r2 = r * r, *ch = nu + LRDMC_NL_OFF;
+            const double v0 = ch[1] * exp_nonpos(-ch[2] * r2), v1 = 3.0 * ch[3] * exp_nonpos(-ch[4] * r2), v2 = 5.0 * ch[5] * exp_nonpos(-ch[6] * r2);
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                const double ct = ws.U[k] * hx + ws.U[3 + k] * hy + ws.U[6 + k] * hz, p2 = 0.5 * (3.0 * ct * ct - 1.0);
+                nuq[2 * k] = (v0 + v1 * ct + v2 * p2) * (1.0 / 6.0);
+                nuq[2 * k + 1] = (v0 - v1 * ct + v2 * p2) * (1.0 / 6.0);
+            }
         }
         if (NP == 1) {
             const double Jo = Jold[i];
-            double Rv[6];
+            double *Ro = is_nl ? ws.R + S.P_lat + 6 * (i * K + kk) : ws.R + mesh * 6 * N + 6 * i;
 #pragma unroll
-            for (int d = 0; d < 6; ++d) Rv[d] = quad_sum(acc[d]) * exp_tab(quad_sum(Jn[d]) - Jo, T.etab);
-            if (valid && t == 0) {
-                double *Ro = ws.R + mesh * 6 * N + 6 * i;
-#pragma unroll
-                for (int d = 0; d < 6; ++d) Ro[d] = Rv[d];
+            for (int d = 0; d < 6; ++d) {
+                double rho = quad_sum(acc[d]);
+                if (!is_nl || !S.nl_dla) rho *= exp_tab(quad_sum(Jn[d]) - Jo, T.etab);
+                if (valid && t == 0) { Ro[d] = is_nl ? -nuq[d] * rho : rho; if (is_nl && rho < 0.0) atomicOr(s_node, 1); }
             }
         } else {
-            double *q = scr + ((size_t)(mesh * N + i) * NP + part) * 12;
+            double *q = is_nl ? scr + P.o_nl + ((size_t)(i * K + kk) * NP + part) * 12 : scr + ((size_t)(mesh * N + i) * NP + part) * 12;
 #pragma unroll
             for (int d = 0; d < 6; ++d) {
                 const double A = quad_sum(acc[d]), J = quad_sum(Jn[d]);
                 if (valid && t == 0) { q[d] = A; q[6 + d] = J; }
+            }
+            if (is_nl && part == 0 && valid && t == 0) {
+                double *qn = scr + P.o_nu + (size_t)(i * K + kk) * 7;
+#pragma unroll
+                for (int d = 0; d < 6; ++d) qn[d] = nuq[d];
+                qn[6] = 1.0;
             }
         }
     }
@@ -174,12 +209,12 @@ __device__ __forceinline__ EvalOut evaluate_team(const DevSys &S, const TeamPlan
         if (NL) for (int p = S.P_lat + tid; p < S.P; p += nthr) {  // non-local slots: R = -nu_q rho_q
             const int o = p - S.P_lat, slot = o / 6, d = o - 6 * slot, i = slot / S.nl_K;
             const double *q = scr + P.o_nl + (size_t)slot * NP * 12, *qn = scr + P.o_nu + (size_t)slot * 7;
+            if (qn[6] == 0.0) { ws.R[p] = 0.0; continue; }          // slot not listed: no centre in range
             double A = 0.0, J = 0.0;
             for (int part = 0; part < NP; ++part) { A += q[part * 12 + d]; J += q[part * 12 + 6 + d]; }
-            const bool active = qn[6] != 0.0;
             const double rho = S.nl_dla ? A : A * exp_tab(J - Jold[i], T.etab);
-            ws.R[p] = active ? -qn[d] * rho : 0.0;
-            if (active && rho < 0.0) atomicOr(s_node, 1);
+            ws.R[p] = -qn[d] * rho;
+            if (rho < 0.0) atomicOr(s_node, 1);
         }
         __syncthreads();
     }
@@ -244,7 +279,7 @@ __global__ void __launch_bounds__(LRDMC_TEAM_MAX_WARPS * 32, 1) k_propagate_team
 {
     extern __shared__ __align__(16) double smem[];
     __shared__ double s_vee[LRDMC_TEAM_MAX_WARPS];
-    __shared__ int s_ctrl[4];
+    __shared__ int s_ctrl[8];      // [0] walker, [1] last, [2] selected move, [3] node flag of the slots, [4] listed slots, [5] spin cut of the list
     stage_tables(S, smem);
     const int tid = threadIdx.x, lane = tid & 31, wt = tid >> 5;
     const Tables T = table_pointers<TS>(S, smem);
