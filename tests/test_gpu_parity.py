@@ -384,6 +384,29 @@ def test_balanced_equals_conventional_on_the_synthetic_molecule(B):
     g.close()
 
 
+@pytest.mark.parametrize("dla", [True, False])
+def test_balanced_equals_conventional_with_nonlocal_slots(B, dla):
+    """Pin P12 with non-local hops in the Green's function (row f1; L244 / Table I shape: "both algorithms sample the same
+    fixed-node ground state"): helium-like atom, Slater orbital x Jastrow (so the determinant-locality and the full-ratio forms
+    differ), attractive s and repulsive p channel: about 1.5 % of the hops are non-local and a third of the non-local amplitudes
+    are sign-forbidden (they go to V_sf).  Error bars ~1e-3 Ha."""
+    from paper_2508_12033_b200 import driver as drv
+    rng = np.random.default_rng(0)
+    base = wl.slater_atom(2.0, [1.85], 1, 1, np.ones((1, 1)), np.ones((1, 1)), 0.25, jastrow=dict(a_anti=0.5, a_par=0.25, b2=0.5))
+    s = wl.with_nonlocal(base, [[2.0, -1.0, 1.2, 0.8, 0.9, 0.0, 1.0]], dla)
+    g = B.Lrdmc(s); g.lrdmc_set_positions(rng.normal(size=(4096, 2, 3)) * 0.7)
+    rb = drv.run(g, B.BALANCED, 300, n_moves=20, E0=-3.2)
+    Eb, sb = B.lrdmc_energy(rb, p=10, n_therm=60, n_blocks=10)
+    rc = drv.run(g, B.CONVENTIONAL, 300, tau=20 * 0.25**2 / 6, E0=-3.2, first_cycle=1000)
+    Ec, sc = B.lrdmc_energy(rc, p=10, n_therm=60, n_blocks=10)
+    R, scal, js = [np_(t) for t in g.lrdmc_step_debug(-3.2, 5000, 0)]
+    assert (js >= 12).sum() > 10 and (R[:, 12:] < 0).mean() > 0.1          # non-local hops are taken; forbidden ones exist
+    assert sum(r.n_nonfinite for r in rb + rc) == 0 and sc < 3e-3
+    assert abs(Eb - Ec) < 3 * np.hypot(sb, sc), (Eb, sb, Ec, sc)
+    assert Eb < -3.5                                                       # far below the channel-free helium energy (-2.90): the s channel binds
+    g.close()
+
+
 # ------------------------------------------------------------------------------------------ edge cases and error behaviour
 def test_edge_cases_and_errors(B):
     s = wl.tiny_molecule(2, 1, 2, 6, seed=7); g = B.Lrdmc(s)
