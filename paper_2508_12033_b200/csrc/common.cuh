@@ -22,6 +22,9 @@
 #ifndef LRDMC_BC_DMMA
 #define LRDMC_BC_DMMA 1         // Bc = C Dinv of the column form on the FP64 tensor pipe (0: DFMA chains over the mo_pass fragments)
 #endif
+#ifndef LRDMC_BC_STORE
+#define LRDMC_BC_STORE 1         // team kernel of the large systems: park the Bc entries (ao_columns BCS) instead of redoing the DMMAs
+#endif
 #define LRDMC_NUC_STRIDE 20  // doubles per nucleus row: Rx Ry Rz Z c1 b1 alpha beta gamma delta is_pp pad | r_c A0 B0 A1 B1 A2 B2 pad (non-local channels)
 #define LRDMC_NL_OFF 12      // first non-local entry of a nucleus row
 #define LRDMC_NL_MAX_K 4
@@ -70,6 +73,7 @@ struct TeamPlan {
     int it_base[4];       // first 4-shell iteration of each shell group
     int kstep_base[4];    // first mma k-step of each group in the `bf` fragment table
     int pair_base[4];     // first k-step pair of each group in the `cf` fragment table
+    int mesh_share;       // both meshes of a block are handled by the same warp: the second takes the first's parked Bc entries
     int o_scr, scr_doubles; // scratch (partial sums) behind the walker state, in doubles from the state base
     ShellPart col[LRDMC_TEAM_MAX_PARTS];     // parts of ao_columns (groups 0-2 start on even iterations: k-step pairs)
     ShellPart mo[LRDMC_TEAM_MAX_WARPS];      // parts of the derivative pass of the mover (one per warp)
@@ -94,6 +98,8 @@ struct DevWalk {
     unsigned long long *timing;      // [max_warps][2] globaltimer start/end per resident warp
     double *stats;        // device copy of the reduced numbers (see k_reduce_obs)
     int *counter;         // dynamic walker queue head; [1] = singular flag
+    double *bcs;          // per resident team CTA: parked Bc entries [block of a mesh][k-step pair][lane][2] (ao_columns BCS); NULL if unused
+    size_t bcs_stride;    // doubles per CTA
 };
 
 __device__ __forceinline__ double warp_sum(double v)

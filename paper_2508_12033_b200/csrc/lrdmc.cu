@@ -281,6 +281,15 @@ static size_t carve(const lrdmc_ctx *c, int n_w, char *base, DevWalk *W)
     TAKE(w, double, nw); TAKE(eL, double, nw); TAKE(W, double, nw); TAKE(omega, double, nw);
     TAKE(nmoves, long long, nw); TAKE(flags, int, nw * 3);
     TAKE(wq, unsigned long long, nw); TAKE(prefix, unsigned long long, nw); TAKE(parents, int, nw);
+    {   // parked Bc entries of the team kernel of the large systems (ao_columns BCS): [resident CTA][block of a mesh][k-step pair][lane][2]
+        const bool use = LRDMC_BC_STORE && LRDMC_BC_DMMA && !c->ts;
+        const size_t stride = (size_t)((S.n_up + 7) / 8 + (S.n_dn + 7) / 8) * S.n_kpairs * 64;
+        const size_t cta_bytes = ((size_t)S.tables_doubles + S.per_warp_doubles) * 8 + 1024;
+        size_t per_sm = 233472 / cta_bytes; if (per_sm > 32) per_sm = 32; if (per_sm < 1) per_sm = 1;      // resident team CTAs per SM, at most
+        if (W) W->bcs_stride = use ? stride : 0;
+        TAKE(bcs, double, use ? stride * per_sm * c->sm_count : 0);
+        if (W && !use) W->bcs = NULL;
+    }
     TAKE(timing, unsigned long long, 2 * (size_t)(c->grid_max * c->wpb > c->sm_count * 32 ? c->grid_max * c->wpb : c->sm_count * 32)); TAKE(counter, int, 64);
 #undef TAKE
     return o;
@@ -345,6 +354,7 @@ static void plan_team(lrdmc_ctx *c, int n_w)
     }
     int np = 1; while (nblk * np < tw && np < LRDMC_TEAM_MAX_PARTS && 2 * np <= (it_total + 1) / 2) np *= 2;
     P.NP = np; P.n_units = nblk * np;
+    P.mesh_share = S.n_mesh == 2 && ((P.nblk[0] + P.nblk[1]) * np) % tw == 0;
     int lpe = 32; while (lpe > 1 && (tw * 32) / lpe < S.N) lpe >>= 1;     // largest power of two with one pass over the electrons
     P.lpe = lpe;
     const double cost_col[4] = { 2.0, 1.0, 1.7, 2.9 }, cost_mo[4] = { 1.5, 1.0, 3.0, 6.0 };

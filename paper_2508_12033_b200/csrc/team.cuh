@@ -44,8 +44,12 @@ __device__ __forceinline__ void store_walker_team(const DevSys &S, const DevWalk
 
 // One evaluation by the team.  The result is valid in warp 0 only (it runs phase C); ws.R / ws.cum are complete for everyone
 // after the caller's next barrier.  s_vee: TW doubles of static shared memory.
-template <int NT, bool TS, bool NL>
-__device__ __forceinline__ EvalOut evaluate_team(const DevSys &S, const TeamPlan &P, const WarpState &ws, const Tables &T, double *scr, double *s_vee, int *s_node)
+// BCS: parked Bc entries (wavefunction.cuh, ao_columns): bcs_cta = this CTA's scratch [block of a mesh][k-step pair][lane];
+// reuse_spin = the spin that did not hop since the last evaluation (-1: none).  A unit's entries are parked and taken back by the
+// same warp: unit -> warp is a fixed map, and P.mesh_share says that both meshes of a block land on the same warp.
+template <int NT, bool TS, bool NL, bool BCS>
+__device__ __forceinline__ EvalOut evaluate_team(const DevSys &S, const TeamPlan &P, const WarpState &ws, const Tables &T, double *scr, double *s_vee, int *s_node,
+                                                 double2 *bcs_cta, int reuse_spin)
 {
     const int N = S.N, n_nuc = S.n_nuc, TW = P.TW, NP = P.NP, tid = threadIdx.x, nthr = blockDim.x, lane = tid & 31, wt = tid >> 5;
     const int t = lane & 3, g = lane >> 2;
@@ -122,9 +126,9 @@ __device__ __forceinline__ EvalOut evaluate_team(const DevSys &S, const TeamPlan
     for (int v = wt; v < P.n_units + n_nlp * NP; v += TW) {
         const bool is_nl = NL && v >= P.n_units;
         const int u = is_nl ? v - P.n_units : v, part = u % NP, blk = u / NP;
-        int sp, il, i, kk = 0, mesh = 0; bool valid;
+        int sp, il, i, kk = 0, mesh = 0, rem = 0; bool valid;
         if (!is_nl) {
-            mesh = blk / nb_mesh; const int rem = blk - mesh * nb_mesh; sp = rem >= P.nblk[0] ? 1 : 0;
+            mesh = blk / nb_mesh; rem = blk - mesh * nb_mesh; sp = rem >= P.nblk[0] ? 1 : 0;
             const int il0 = 8 * (sp ? rem - P.nblk[0] : rem), ns_ = sp ? S.n_dn : S.n_up;
             valid = il0 + g < ns_; il = valid ? il0 + g : 0; i = (sp ? S.n_up : 0) + il;
         } else {
@@ -146,6 +150,13 @@ __device__ __forceinline__ EvalOut evaluate_team(const DevSys &S, const TeamPlan
 #pragma unroll
         for (int k = 0; k < 3; ++k) { av[k][0] = step * ws.U[k]; av[k][1] = step * ws.U[3 + k]; av[k][2] = step * ws.U[6 + k]; }
         double acc[6], Jn[6];
+        if (BCS && !is_nl) {
+            double2 *bq = bcs_cta + (size_t)rem * S.n_kpairs * 32 + lane;
+            if ((mesh > 0 && P.mesh_share) || sp == reuse_spin)
+                ao_columns<NT, TS, true, 2>(S, T.shells, sp ? T.cf[1] : T.cf[0], T.etab, sp ? ws.dinv[1] : ws.dinv[0], ns, il, x0, y0, z0, av, a2, lane, acc, &P, &P.col[part], bq);
+            else
+                ao_columns<NT, TS, true, 1>(S, T.shells, sp ? T.cf[1] : T.cf[0], T.etab, sp ? ws.dinv[1] : ws.dinv[0], ns, il, x0, y0, z0, av, a2, lane, acc, &P, &P.col[part], bq);
+        } else
         ao_columns<NT, TS, true>(S, T.shells, sp ? T.cf[1] : T.cf[0], T.etab, sp ? ws.dinv[1] : ws.dinv[0], ns, il, x0, y0, z0, av, a2, lane, acc, &P, &P.col[part]);
 #pragma unroll
         for (int d = 0; d < 6; ++d) Jn[d] = 0.0;
@@ -285,6 +296,8 @@ __global__ void __launch_bounds__(LRDMC_TEAM_MAX_WARPS * 32, 1) k_propagate_team
     const Tables T = table_pointers<TS>(S, smem);
     WarpState ws = warp_views(S, smem, 0);
     double *scr = smem + S.tables_doubles + P.o_scr;
+    constexpr bool BCS = !TS && LRDMC_BC_STORE;                 // large systems: C Dinv is the largest share of the evaluation
+    double2 *bcs_cta = BCS ? reinterpret_cast<double2 *>(W.bcs + (size_t)blockIdx.x * W.bcs_stride) : nullptr;
     const unsigned long long t_start = globaltimer_ns();
     for (;;) {
         if (tid == 0) s_ctrl[0] = atomicAdd(W.counter, 1);
@@ -292,7 +305,7 @@ __global__ void __launch_bounds__(LRDMC_TEAM_MAX_WARPS * 32, 1) k_propagate_team
         const int k = s_ctrl[0];
         if (k >= W.n_w) break;
         load_walker_team(S, W, ws, T.nuc, k, P.TW);
-        uint32_t s = 0;
+        uint32_t s = 0; int reuse_spin = -1;
         double w = 1.0, tau_left = tau, omega = 0.0, eL_last = 0.0, W_last = 0.0; long long moves = 0; int n_node = 0, n_nonpos = 0;
         for (;;) {
             const StepDraws d = step_draws(S, (uint32_t)k, cycle, s, mode == LRDMC_CONVENTIONAL);
@@ -300,7 +313,7 @@ __global__ void __launch_bounds__(LRDMC_TEAM_MAX_WARPS * 32, 1) k_propagate_team
 #pragma unroll
                 for (int i = 0; i < 9; ++i) ws.U[i] = U[i]; }
             __syncthreads();
-            const EvalOut e = evaluate_team<NT, TS, NL>(S, P, ws, T, scr, s_vee, &s_ctrl[3]);
+            const EvalOut e = evaluate_team<NT, TS, NL, BCS>(S, P, ws, T, scr, s_vee, &s_ctrl[3], bcs_cta, reuse_spin);
             if (wt == 0) {                                       // the leader warp keeps the weight (same rules as k_propagate)
                 n_node += e.node;
                 bool last = false;
@@ -326,7 +339,11 @@ __global__ void __launch_bounds__(LRDMC_TEAM_MAX_WARPS * 32, 1) k_propagate_team
             __syncthreads();
             const bool last = s_ctrl[1] != 0; const int j = s_ctrl[2];
             if (last) break;
-            if (j >= 0) { apply_move_team<NT, TS, NL>(S, P, ws, T, scr, j); ++moves; }
+            if (j >= 0) {
+                apply_move_team<NT, TS, NL>(S, P, ws, T, scr, j); ++moves;
+                const int im = j < S.P_lat ? (j % (6 * S.N)) / 6 : (j - S.P_lat) / (6 * S.nl_K);   // the electron that hopped
+                reuse_spin = 1 - spin_of(S, im);
+            } else reuse_spin = -1;
             ++s;
         }
         store_walker_team(S, W, ws, k);

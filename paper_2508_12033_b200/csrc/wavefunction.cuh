@@ -197,10 +197,11 @@ __device__ __forceinline__ void mo_values(const DevSys &S, const double *__restr
 //   av[k] = a e_k (displacement of direction +k), a2 = a^2;  acc[d], d = 2k (+), 2k+1 (-): this lane's share (its
 //   shells) of the determinant ratio of candidate (i, d); the caller adds the four lanes of a quad.
 #if !LRDMC_BC_DMMA
-template <int NT, bool TS>
+template <int NT, bool TS, bool PART = false, int BCS = 0>
 __device__ __forceinline__ void ao_columns(const DevSys &S, const double *__restrict__ shells, const double *__restrict__ bf, const double *__restrict__ etab,
                                            const double *__restrict__ dinv, int ns, int il, double x0, double y0, double z0,
-                                           const double (&av)[3][3], double a2, int lane, double (&acc)[6])
+                                           const double (&av)[3][3], double a2, int lane, double (&acc)[6],
+                                           const TeamPlan * = nullptr, const ShellPart * = nullptr, double2 * = nullptr)
 {
     const int t = lane & 3;
     const double4 *sh4 = reinterpret_cast<const double4 *>(shells) + t;
@@ -292,29 +293,40 @@ __device__ __forceinline__ void ao_columns(const DevSys &S, const double *__rest
 // group is padded to an even number of k-steps; s and p iterations are taken two at a time with a one-iteration tail.
 // PART (team mode): only the iterations [part->lo[g], part->hi[g]) of each shell group (lo even in groups 0-2, so that a part
 // starts on a k-step pair); acc is then the part's share of the ratio.
-template <int NT, bool TS, bool PART = false>
+// BCS (team kernel of the large systems, where the C Dinv product is the largest share): the Bc entries of a block depend on the
+// inverse of ITS spin only, and not on the mesh.  BCS = 1: compute them (2 NT DMMA per k-step pair) and park them in a global
+// scratch `bcs0` [pair][lane] -- lane-private: the lane that parks an entry is the lane that takes it back; BCS = 2: take them from
+// there (blocks of the spin that did not hop since the last evaluation; the second mesh).  Results are bit-identical to BCS = 0.
+template <int NT, bool TS, bool PART = false, int BCS = 0>
 __device__ __forceinline__ void ao_columns(const DevSys &S, const double *__restrict__ shells, const double *__restrict__ cf, const double *__restrict__ etab,
                                            const double *__restrict__ dinv, int ns, int il, double x0, double y0, double z0,
                                            const double (&av)[3][3], double a2, int lane, double (&acc)[6],
-                                           const TeamPlan *tp = nullptr, const ShellPart *part = nullptr)
+                                           const TeamPlan *tp = nullptr, const ShellPart *part = nullptr, double2 *bcs0 = nullptr)
 {
+    double2 *bcs = bcs0;
 #define LRDMC_COL_RANGE(G, PAIRS)                                                               \
     const int n = PART ? part->hi[G] : S.n_it[G]; int it = PART ? part->lo[G] : 0;              \
-    if (PART) { sh4 = reinterpret_cast<const double4 *>(shells) + t + 4 * (tp->it_base[G] + it); b = cf + lane + (size_t)(tp->pair_base[G] + (PAIRS)) * NA * 32; }
+    if (PART) { sh4 = reinterpret_cast<const double4 *>(shells) + t + 4 * (tp->it_base[G] + it); b = cf + lane + (size_t)(tp->pair_base[G] + (PAIRS)) * NA * 32; \
+                if (BCS) bcs = bcs0 + (size_t)(tp->pair_base[G] + (PAIRS)) * 32; }
     const int t = lane & 3;
     const double4 *sh4 = reinterpret_cast<const double4 *>(shells) + t;
     const double *b = cf + lane;
     constexpr int NA = 2 * NT;
     double aop[NA];                                  // A fragments: Dinv[4 j + t][il] (rows >= n_s are zero padded)
 #pragma unroll
-    for (int j = 0; j < NA; ++j) aop[j] = dinv[(4 * j + t) * ns + il];
+    for (int j = 0; j < NA; ++j) aop[j] = (BCS == 2) ? 0.0 : dinv[(4 * j + t) * ns + il];
 #pragma unroll
     for (int d = 0; d < 6; ++d) acc[d] = 0.0;
 #define LRDMC_BPAIR(v0, v1)                                                                     \
     {                                                                                           \
-        v0 = 0.0; v1 = 0.0;                                                                     \
-        _Pragma("unroll") for (int j = 0; j < NA; ++j) dmma884(v0, v1, aop[j], ldt<TS>(b + j * 32));      \
-        b += NA * 32;                                                                           \
+        if (BCS == 2) { const double2 q_ = __ldcg(bcs); v0 = q_.x; v1 = q_.y; }                 \
+        else {                                                                                  \
+            v0 = 0.0; v1 = 0.0;                                                                 \
+            _Pragma("unroll") for (int j = 0; j < NA; ++j) dmma884(v0, v1, aop[j], ldt<TS>(b + j * 32));  \
+            if (BCS == 1) __stcg(bcs, make_double2(v0, v1));                                    \
+            b += NA * 32;                                                                       \
+        }                                                                                       \
+        if (BCS) bcs += 32;                                                                     \
     }
 #define LRDMC_GEOM                                                                              \
         const double4 s = *sh4; const double z = s.w;                                           \
