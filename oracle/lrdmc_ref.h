@@ -76,6 +76,9 @@ int lrdmc_ref_get_obs(const lrdmc_ref_ctx *, double *eL, double *W, double *omeg
 int lrdmc_ref_propagate(lrdmc_ref_ctx *, int mode, int n_moves, double tau, double E0, uint64_t cycle);
 int lrdmc_ref_reconfigure(lrdmc_ref_ctx *, uint64_t cycle, int32_t *parents_out /*nullable*/);
 int lrdmc_ref_estimators(const lrdmc_ref_ctx *, lrdmc_ref_stats *out);
+/* Walker k of this context draws from the random streams of slot `offset + k` (default 0): lets a test replay a few walkers
+ * taken from the middle of a large ensemble. */
+int lrdmc_ref_set_slot_offset(lrdmc_ref_ctx *, uint32_t offset);
 int lrdmc_ref_set_threads(int n); /* OpenMP threads over walkers; returns the count in effect */
 
 /* one evaluation + selection for every walker at (cycle, step), no state change.

@@ -63,6 +63,20 @@ def lib():
                                           C.c_double, C.c_double, C.c_double, C.c_void_p, C.c_void_p, C.c_double, C.c_double,
                                           C.c_uint64]
         _lib.lrdmc_ref_destroy.argtypes = [C.c_void_p]
+        vp = C.c_void_p      # every pointer argument is declared: a bare Python int would be passed as a 32-bit C int
+        _lib.lrdmc_ref_set_positions.argtypes = [vp, C.c_int, vp]
+        _lib.lrdmc_ref_get_state.argtypes = [vp, vp, vp, vp, vp]
+        _lib.lrdmc_ref_set_state.argtypes = [vp, C.c_int, vp, vp, vp, vp]
+        _lib.lrdmc_ref_get_obs.argtypes = [vp, vp, vp, vp, vp]
+        _lib.lrdmc_ref_estimators.argtypes = [vp, vp]
+        _lib.lrdmc_ref_ao.argtypes = [vp, vp, vp, vp, vp]
+        _lib.lrdmc_ref_mo.argtypes = [vp, C.c_int, vp, vp, vp, vp]
+        _lib.lrdmc_ref_logpsi.argtypes = [vp, vp, vp, vp]
+        _lib.lrdmc_ref_build_inverse.argtypes = [vp, vp, vp, vp]
+        _lib.lrdmc_ref_evaluate.argtypes = [vp] * 9
+        _lib.lrdmc_ref_philox4x32_10.argtypes = [vp, vp, vp]
+        _lib.lrdmc_ref_set_threads.argtypes = [C.c_int]
+        _lib.lrdmc_ref_set_slot_offset.argtypes = [vp, C.c_uint32]
         _lib.lrdmc_ref_set_contraction.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]
         _lib.lrdmc_ref_set_nonlocal.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p]
         _lib.lrdmc_ref_nl_info.argtypes = [C.c_void_p] + [C.c_void_p] * 7
@@ -142,6 +156,10 @@ class Ref:
             except Exception:       # interpreter shutdown
                 pass
             self.h = None
+
+    def set_slot_offset(self, offset):
+        """walker k draws from the random streams of slot offset + k"""
+        return lib().lrdmc_ref_set_slot_offset(self.h, offset)
 
     # ---- walkers ----
     def set_positions(self, r):

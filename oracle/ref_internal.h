@@ -34,6 +34,7 @@ struct lrdmc_ref_ctx {
     int n_w; double *r, *dinv_up, *dinv_dn, *w, *eL, *W, *omega; int64_t *nmoves;
     int *flag_node, *flag_nonpos, *flag_nonfinite; /* per-walker event counts of the last cycle */
     double wbar; int have_obs;
+    uint32_t slot0;                  /* random streams of walker k are keyed by slot slot0 + k (lrdmc_ref_set_slot_offset) */
 };
 
 static inline int ref_nocc(const lrdmc_ref_ctx *c, int spin) { return spin ? c->n_dn : c->n_up; }

@@ -90,6 +90,8 @@ int lrdmc_ref_set_nonlocal(lrdmc_ref_ctx *c, int K, int dla, const double *nl)
     return LRDMC_REF_OK;
 }
 
+int lrdmc_ref_set_slot_offset(lrdmc_ref_ctx *c, uint32_t offset) { if (!c) return LRDMC_REF_EINVAL; c->slot0 = offset; return LRDMC_REF_OK; }
+
 int lrdmc_ref_set_threads(int n)
 {
 #ifdef _OPENMP
@@ -187,7 +189,7 @@ static void propagate_walker(lrdmc_ref_ctx *c, int k, int mode, int n_moves, dou
     int64_t moves = 0; int nnode = 0, nnonpos = 0;
     int64_t cap = (mode == LRDMC_REF_BALANCED) ? n_moves : (n_moves > 0 ? n_moves : ((int64_t)1 << 30));
     for (uint64_t s = 0;; ++s) {
-        lrdmc_ref_draws(c, (uint32_t)k, cycle, s, u);
+        lrdmc_ref_draws(c, c->slot0 + (uint32_t)k, cycle, s, u);
         lrdmc_ref_frame(u[0], u[1], u[2], U);
         lrdmc_ref_evaluate(c, x, du, dd, U, R, scal, NULL, NULL);
         double bbar = scal[0], W = scal[2], eL = scal[3];
@@ -270,7 +272,7 @@ int lrdmc_ref_step_debug(const lrdmc_ref_ctx *c, double E0, uint64_t cycle, uint
     #pragma omp parallel for schedule(dynamic)
     for (int k = 0; k < c->n_w; ++k) {
         double u[5], U[9], s10[10], mg;
-        lrdmc_ref_draws(c, (uint32_t)k, cycle, step, u);
+        lrdmc_ref_draws(c, c->slot0 + (uint32_t)k, cycle, step, u);
         lrdmc_ref_frame(u[0], u[1], u[2], U);
         lrdmc_ref_evaluate(c, c->r + (size_t)k * 3 * c->N, c->dinv_up + (size_t)k * c->n_up * c->n_up,
                            c->dinv_dn + (size_t)k * c->n_dn * c->n_dn, U, R + (size_t)k * P, s10, NULL, NULL);

@@ -286,6 +286,36 @@ def test_full_size_c4_sampled_walkers_match_oracle(B):
     g.close()
 
 
+@pytest.mark.parametrize("cfg,mode", [("C4", "balanced"), ("C4", "conventional"), ("C5", "balanced"), ("C5", "conventional"), ("C3nl", "balanced")])
+def test_full_size_trajectories_of_sampled_walkers(B, cfg, mode):
+    """Whole branching intervals at the full BASELINE sizes in the launch configuration bench.py times (C4: 25600 walkers,
+    warp-per-walker; C5: 4096 walkers, team kernel with parked Bc entries; C3 + non-local slots: 25600): groups of walkers from
+    the start, the middle and the end of the ensemble are replayed by the oracle on their own random streams."""
+    s, n_w, n_moves, per = {"C4": (wl.water_methane(n_walkers=25600), 25600, 20, 6), "C5": (wl.cluster64(), 4096, 12, 2),
+                            "C3nl": (wl.water_methane_nonlocal(n_walkers=25600), 25600, 20, 6)}[cfg]
+    N = s["n_up"] + s["n_dn"]; x0 = wl.initial_walkers(s, n_w, 5)
+    g = B.Lrdmc(s); g.lrdmc_set_positions(x0, allow_singular=True)
+    cycle = 3
+    if mode == "balanced":
+        g.lrdmc_propagate(B.BALANCED, n_moves, 0.0, -5.0, cycle)
+    else:
+        tau = n_moves * s["a"]**2 / (3 * N) * (0.5 if s["a2"] > 0 else 1.0); g.lrdmc_propagate(B.CONVENTIONAL, 0, tau, -1.0, cycle)
+    gr, _, _, gw = [np_(t) for t in g.lrdmc_get_walkers()]; geL, gW, gom, gnm = [np_(t) for t in g.lrdmc_get_obs()]
+    for k0 in (0, n_w // 2 - 37, n_w - per):
+        o = ref.Ref(s); o.set_slot_offset(k0)
+        rc = o.set_positions(x0[k0:k0 + per]); assert rc in (0, -2)
+        if mode == "balanced":
+            assert o.propagate(ref.BALANCED, n_moves, 0.0, -5.0, cycle) == 0
+        else:
+            assert o.propagate(ref.CONVENTIONAL, 0, tau, -1.0, cycle) == 0
+        r, _, _, w = o.get_state(); eL, W, om, nm = o.get_obs()
+        sl = slice(k0, k0 + per); Kd = 3 * N / s["a"]**2
+        assert np.array_equal(gnm[sl], nm) and np.abs(gr[sl] - r).max() < 1e-11
+        assert relerr(gw[sl], w) < 1e-9 and relerr(gom[sl], om) < 1e-9
+        assert np.max(np.abs(geL[sl] - eL) / np.maximum(np.abs(eL), Kd)) < TOL
+    g.close()
+
+
 # ------------------------------------------------------------------------------------------ runs: energies within 3 sigma
 def test_hydrogen_run_energy_matches_oracle_and_exact(B):
     from paper_2508_12033_b200 import driver as drv
