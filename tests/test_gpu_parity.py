@@ -461,3 +461,28 @@ def test_edge_cases_and_errors(B):
     st = g.lrdmc_estimators(); so = o.estimators()
     assert st.n_nonpos_diag == so["n_nonpos_diag"] == 8 * 4 and st.wbar == 0.0 == so["wbar"]
     g.close()
+
+
+def test_malformed_nonlocal_and_contraction_inputs_are_rejected(B):
+    """lrdmc_init validates the f1 / f2 inputs: too many slots per electron, contracted shells that mix centres or types, ranges that
+    do not tile the primitive list, an MO matrix whose row count is not the contracted function count -> LRDMC_EINVAL."""
+    s = wl.random_nonlocal(wl.tiny_molecule(2, 1, 2, 6, seed=7), 8, 1.4, 1, True); s["nl_K"] = 5
+    with pytest.raises(B.LrdmcError) as e:
+        B.Lrdmc(s)
+    assert e.value.code == B.EINVAL
+    good = wl.contracted_molecule(3, 2, 3, 9, seed=31, spherical=True)
+    for breakit in ("first", "mixed", "nao"):
+        c = dict(good)
+        if breakit == "first":
+            f = good["cs_first"].copy(); f[-1] -= 1; c["cs_first"] = f                   # ranges do not end at n_shell
+        elif breakit == "mixed":
+            t = good["shell_type"].copy(); k = int(good["cs_first"][1]) - 1
+            if int(good["cs_first"][1]) - int(good["cs_first"][0]) < 2:
+                f = good["cs_first"].copy(); f[1] += 1; c["cs_first"] = f                # merge a p primitive into the first (s) shell
+            else:
+                t[k] = wl.SHELL_P; c["shell_type"] = t
+        else:
+            c["n_ao"] = good["n_ao"] + 1; c["C_up"] = np.vstack([good["C_up"], np.zeros((1, 3))]); c["C_dn"] = np.vstack([good["C_dn"], np.zeros((1, 2))])
+        with pytest.raises(B.LrdmcError) as e:
+            B.Lrdmc(c)
+        assert e.value.code == B.EINVAL, breakit
