@@ -7,9 +7,6 @@
 // __builtin_assume(__isShared(p)) made nvcc 12.9 delete the hop (apply_move) from k_propagate: measured, reverted.
 // Address spaces are inferred instead: with TS every per-warp pointer is "shared base + offset" with no global alternative.
 #define LRDMC_ASSUME_SHARED(p) ((void)0)
-#ifndef LRDMC_NB
-#define LRDMC_NB 2             // mma batches (of 8 candidate points) per warp pass
-#endif
 #ifndef LRDMC_WPB
 #define LRDMC_WPB 8            // warps (= walkers in flight) per CTA
 #endif
@@ -18,9 +15,6 @@
 #endif
 #ifndef LRDMC_LOCKSTEP
 #define LRDMC_LOCKSTEP 1        // balanced mode: the warps of a CTA step together (one barrier per step)
-#endif
-#ifndef LRDMC_BC_DMMA
-#define LRDMC_BC_DMMA 1         // Bc = C Dinv of the column form on the FP64 tensor pipe (0: DFMA chains over the mo_pass fragments)
 #endif
 #ifndef LRDMC_BC_STORE
 #define LRDMC_BC_STORE 1         // team kernel of the large systems: park the Bc entries (ao_columns BCS) instead of redoing the DMMAs

@@ -248,7 +248,7 @@ __device__ __forceinline__ EvalOut phase_c(const DevSys &S, const WarpState &ws,
     return o;
 }
 
-template <int NT, bool TS, int NB, bool NL = false>
+template <int NT, bool TS, bool NL = false>
 __device__ __forceinline__ EvalOut evaluate_walker(const DevSys &S, const WarpState &ws, const Tables &T, int lane)
 {
     const int N = S.N, n_nuc = S.n_nuc;
@@ -294,7 +294,6 @@ __device__ __forceinline__ EvalOut evaluate_walker(const DevSys &S, const WarpSt
     __syncwarp();
 
     // ---- phase B (rows a1-a5): the 6 n_s candidates of each spin, 8 electrons (48 points) per warp pass in column form
-#ifndef LRDMC_CONTRACTION_MO
     if (!NL) for (int mesh = 0; mesh < S.n_mesh; ++mesh) {
         const double am = S.amesh[mesh], a2 = am * am;
         double av[3][3];                                             // av[k] = a e_k, e_k = k-th column of U (Eq.D3-D4)
@@ -307,7 +306,7 @@ __device__ __forceinline__ EvalOut evaluate_walker(const DevSys &S, const WarpSt
                 const int il = valid ? il0 + g : 0, i = off + il;
                 const double x0 = ws.r[3 * i], y0 = ws.r[3 * i + 1], z0 = ws.r[3 * i + 2];
                 double acc[6], Jn[6];
-                ao_columns<NT, TS>(S, T.shells, LRDMC_BC_DMMA ? (sp ? T.cf[1] : T.cf[0]) : (sp ? T.bf[1] : T.bf[0]), T.etab, sp ? ws.dinv[1] : ws.dinv[0], ns, il, x0, y0, z0, av, a2, lane, acc);
+                ao_columns<NT, TS>(S, T.shells, sp ? T.cf[1] : T.cf[0], T.etab, sp ? ws.dinv[1] : ws.dinv[0], ns, il, x0, y0, z0, av, a2, lane, acc);
                 // Jastrow ratio (row a5): the 4 lanes of the quad split the partners; u = c r/(1 + b r) = c/(b + 1/r)
 #pragma unroll
                 for (int d = 0; d < 6; ++d) Jn[d] = 0.0;
@@ -331,68 +330,6 @@ __device__ __forceinline__ EvalOut evaluate_walker(const DevSys &S, const WarpSt
             }
         }
     }
-#else
-    // MO form: candidates, 8*NB points (NB mma batches of 8) per warp pass through the tensor-core MO pass
-    for (int mesh = 0; mesh < S.n_mesh; ++mesh) {
-        const double am = S.amesh[mesh];
-        for (int sp = 0; sp < 2; ++sp) {
-            const int ns = sp ? S.n_dn : S.n_up, off = sp ? S.n_up : 0, npts = 6 * ns;
-            if (ns == 0) continue;
-            const double *dinv = ws.dinv[sp];
-            for (int q0 = 0; q0 < npts; q0 += 8 * NB) {
-                bool valid[NB]; int ci[NB], cd[NB], cil[NB]; double pt[NB][3];
-#pragma unroll
-                for (int h = 0; h < NB; ++h) {
-                    valid[h] = q0 + 8 * h + g < npts;
-                    const int q = valid[h] ? q0 + 8 * h + g : 0, il = q / 6, d = q - 6 * il, i = off + il, k = d >> 1;
-                    const double step = (d & 1) ? -am : am;
-                    ci[h] = i; cd[h] = d; cil[h] = il;
-                    pt[h][0] = ws.r[3 * i] + step * ws.U[k]; pt[h][1] = ws.r[3 * i + 1] + step * ws.U[3 + k]; pt[h][2] = ws.r[3 * i + 2] + step * ws.U[6 + k];
-                }
-                double acc[NB][NT][2];
-                mo_values<NT, NB, TS>(S, T.shells, T.bf[sp], T.etab, pt, lane, acc);
-                // determinant ratio (row a4): sum_m phi_m(r') Dinv[m][il]; this lane holds m = 8 nt + 2t, +1 (rows beyond n_s are zero-padded)
-                double part[NB], Jn[NB];
-#pragma unroll
-                for (int h = 0; h < NB; ++h) { part[h] = 0.0; Jn[h] = 0.0; }
-#pragma unroll
-                for (int h = 0; h < NB; ++h)
-#pragma unroll
-                    for (int nt = 0; nt < NT; ++nt) {
-                        const int m = 8 * nt + 2 * t;
-                        part[h] += acc[h][nt][0] * dinv[m * ns + cil[h]] + acc[h][nt][1] * dinv[(m + 1) * ns + cil[h]];
-                    }
-                // Jastrow ratio (row a5): partners split over the 4 lanes of the quad; both points share each partner load
-                if (S.has_j1) for (int I = t; I < n_nuc; I += 4) {
-                    const double *nu = T.nuc + I * LRDMC_NUC_STRIDE;
-                    const double nx = nu[0], ny = nu[1], nz = nu[2], c1 = nu[4], b1 = nu[5];
-#pragma unroll
-                    for (int h = 0; h < NB; ++h) {
-                        const double dx = pt[h][0] - nx, dy = pt[h][1] - ny, dz = pt[h][2] - nz, r2 = dx * dx + dy * dy + dz * dz;
-                        const double r = r2 * fast_rsqrt(r2);
-                        Jn[h] -= c1 * r * fast_rcp(1.0 + b1 * r);
-                    }
-                }
-                for (int j = t; j < N; j += 4) {
-                    const double jx = ws.r[3 * j], jy = ws.r[3 * j + 1], jz = ws.r[3 * j + 2];
-                    const double cpar = (spin_of(S, j) == sp) ? S.a_par : S.a_anti;
-#pragma unroll
-                    for (int h = 0; h < NB; ++h) {
-                        const double dx = pt[h][0] - jx, dy = pt[h][1] - jy, dz = pt[h][2] - jz, r2 = dx * dx + dy * dy + dz * dz;
-                        const double r = r2 * fast_rsqrt(r2);
-                        const double u = cpar * r * fast_rcp(1.0 + S.b2 * r);
-                        if (j != ci[h]) Jn[h] += u;
-                    }
-                }
-#pragma unroll
-                for (int h = 0; h < NB; ++h) {
-                    const double dr = quad_sum(part[h]), dJ = quad_sum(Jn[h]) - Jold[ci[h]];
-                    if (valid[h] && t == 0) ws.R[mesh * 6 * N + 6 * ci[h] + cd[h]] = dr * exp(dJ);
-                }
-            }
-        }
-    }
-#endif
     // ---- systems with non-local pseudopotential slots (row f1): lattice blocks and slot blocks in one loop
     int node_nl = 0;
     if (NL) node_nl = phase_b_with_nonlocal<NT, TS>(S, ws, T, Jold, lane);

@@ -61,21 +61,17 @@ void KFN(lrdmc_k_step_debug)(int NT, int ts, int grid, int threads, int smem, cu
 int KFN(lrdmc_k_team_occupancy)(int NT, int ts, int threads, int smem)
 {
     int occ = 0;
-#if LRDMC_BC_DMMA
 #define STMT(NTV, TSV) cudaFuncSetAttribute(k_propagate_team<NTV, TSV, kNL>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); \
                        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_propagate_team<NTV, TSV, kNL>, threads, smem)
     PICK(NT, ts, STMT);
 #undef STMT
-#endif
     return occ;
 }
 void KFN(lrdmc_k_team)(int NT, int ts, int grid, int threads, int smem, cudaStream_t st, const DevSys &S, const DevWalk &W, const TeamPlan &P, int mode,
                        int n_moves, double tau, double E0, uint32_t cycle)
 {
-#if LRDMC_BC_DMMA
 #define STMT(NTV, TSV) k_propagate_team<NTV, TSV, kNL><<<grid, threads, smem, st>>>(S, W, P, mode, n_moves, tau, E0, cycle)
     PICK(NT, ts, STMT);
 #undef STMT
-#endif
 }
 #endif

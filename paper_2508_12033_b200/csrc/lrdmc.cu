@@ -170,7 +170,7 @@ extern "C" int lrdmc_init(lrdmc_ctx **out, const lrdmc_system *sys, const lrdmc_
     S.n_kpairs = pair_base[4];
     for (int g = 0; g < 5; ++g) c->pair_base[g] = pair_base[g];
     const int NA = 2 * c->NT;
-    const size_t cf_n = LRDMC_BC_DMMA ? (size_t)S.n_kpairs * NA * 32 : 0;
+    const size_t cf_n = (size_t)S.n_kpairs * NA * 32;
     std::vector<double> h_cf[2];
     for (int sp = 0; sp < (S.same_C ? 1 : 2) && cf_n; ++sp) {
         const int ns = sp ? sys->n_dn : sys->n_up; const double *C = sp ? Cdn : Cup;
@@ -282,7 +282,7 @@ static size_t carve(const lrdmc_ctx *c, int n_w, char *base, DevWalk *W)
     TAKE(nmoves, long long, nw); TAKE(flags, int, nw * 3);
     TAKE(wq, unsigned long long, nw); TAKE(prefix, unsigned long long, nw); TAKE(parents, int, nw);
     {   // parked Bc entries of the team kernel of the large systems (ao_columns BCS): [resident CTA][block of a mesh][k-step pair][lane][2]
-        const bool use = LRDMC_BC_STORE && LRDMC_BC_DMMA && !c->ts;
+        const bool use = LRDMC_BC_STORE && !c->ts;
         const size_t stride = (size_t)((S.n_up + 7) / 8 + (S.n_dn + 7) / 8) * S.n_kpairs * 64;
         const size_t cta_bytes = ((size_t)S.tables_doubles + S.per_warp_doubles) * 8 + 1024;
         size_t per_sm = 233472 / cta_bytes; if (per_sm > 32) per_sm = 32; if (per_sm < 1) per_sm = 1;      // resident team CTAs per SM, at most
@@ -332,7 +332,6 @@ static void plan_team(lrdmc_ctx *c, int n_w)
 {
     const DevSys &S = c->S; TeamPlan &P = c->team;
     c->team_tw = 1;
-#if LRDMC_BC_DMMA
     int tw = 1;
     const long slots = (long)c->grid_max * c->wpb;
     if (!c->ts) tw = 4;
@@ -369,7 +368,6 @@ static void plan_team(lrdmc_ctx *c, int n_w)
     const int occ = S.nl_K ? lrdmc_k_team_occupancy_nl(c->NT, c->ts, tw * 32, smem) : lrdmc_k_team_occupancy_lat(c->NT, c->ts, tw * 32, smem);
     if (cudaGetLastError() != cudaSuccess || occ < 1) return;             // does not fit: stay with warp-per-walker
     c->team_tw = tw; c->team_smem = smem; c->team_ctas_per_sm = occ; c->team_grid_max = c->sm_count * occ;
-#endif
 }
 
 extern "C" int lrdmc_bind_walkers(lrdmc_ctx *c, void *dev_buf, size_t bytes, int n_walkers)

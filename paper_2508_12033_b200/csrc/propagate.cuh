@@ -13,7 +13,7 @@ __device__ __forceinline__ void stage_tables(const DevSys &S, double *smem)
         const int nb = S.n_ksteps * S.NT[0] * 32;
         for (int i = threadIdx.x; i < nb; i += blockDim.x) smem[S.off_bf[0] + i] = S.bfrag[0][i];
         if (!S.same_C && S.n_dn > 0) for (int i = threadIdx.x; i < nb; i += blockDim.x) smem[S.off_bf[1] + i] = S.bfrag[1][i];
-        const int nc = LRDMC_BC_DMMA ? S.n_kpairs * 2 * S.NT[0] * 32 : 0;
+        const int nc = S.n_kpairs * 2 * S.NT[0] * 32;
         for (int i = threadIdx.x; i < nc; i += blockDim.x) smem[S.off_cf[0] + i] = S.cfrag[0][i];
         if (!S.same_C && S.n_dn > 0) for (int i = threadIdx.x; i < nc; i += blockDim.x) smem[S.off_cf[1] + i] = S.cfrag[1][i];
     }
@@ -119,7 +119,7 @@ __global__ void __launch_bounds__(LRDMC_WPB * 32, LRDMC_MINB) k_propagate(DevSys
         else if (!have) break;
         const StepDraws d = step_draws(S, (uint32_t)k, cycle, s, mode == LRDMC_CONVENTIONAL);
         publish_frame(ws, d, lane);
-        const EvalOut e = evaluate_walker<NT, TS, LRDMC_NB, NL>(S, ws, T, lane);
+        const EvalOut e = evaluate_walker<NT, TS, NL>(S, ws, T, lane);
         n_node += e.node;
         bool last = false; double omega = 0.0;
         if (mode == LRDMC_BALANCED) {
@@ -169,7 +169,7 @@ __global__ void __launch_bounds__(LRDMC_WPB * 32, LRDMC_MINB) k_step_debug(DevSy
         load_walker<TS>(S, W, ws, T.nuc, k, lane, true);
         const StepDraws d = step_draws(S, (uint32_t)k, cycle, step, true);
         publish_frame(ws, d, lane);
-        const EvalOut e = evaluate_walker<NT, TS, LRDMC_NB, NL>(S, ws, T, lane);
+        const EvalOut e = evaluate_walker<NT, TS, NL>(S, ws, T, lane);
         const int j = select_move(S, ws, d.u_sel, lane);
         for (int p = lane; p < S.P; p += 32) R_out[(size_t)k * S.P + p] = ws.R[p];
         if (lane == 0) {

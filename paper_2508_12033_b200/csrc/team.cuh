@@ -10,8 +10,6 @@
 #pragma once
 #include "propagate.cuh"
 
-#if LRDMC_BC_DMMA
-
 __device__ __forceinline__ void load_walker_team(const DevSys &S, const DevWalk &W, WarpState &ws, const double *nuc, int k, int TW)
 {
     const int N = S.N, tid = threadIdx.x, nthr = blockDim.x, lane = tid & 31, wt = tid >> 5;
@@ -359,4 +357,3 @@ __global__ void __launch_bounds__(LRDMC_TEAM_MAX_WARPS * 32, 1) k_propagate_team
     if (tid == 0) { W.timing[2 * blockIdx.x] = t_start; W.timing[2 * blockIdx.x + 1] = globaltimer_ns(); }
 }
 
-#endif  // LRDMC_BC_DMMA

@@ -113,77 +113,6 @@ __device__ __forceinline__ void mo_pass(const DevSys &S, const double *__restric
 #undef LRDMC_FEED
 }
 
-// Value-only pass over NB batches of 8 points at once (8*NB candidate points per warp pass): every shell row and every
-// B fragment is loaded once and used NB times, and the NB exponential chains of a lane are independent (ILP NB), which is
-// what the FP64 pipe needs with 4 warps per scheduler.  acc[h] = accumulators of batch h.
-template <int NT, int NB, bool TS>
-__device__ __forceinline__ void mo_values(const DevSys &S, const double *__restrict__ shells, const double *__restrict__ bf, const double *__restrict__ etab,
-                                          const double (&pt)[NB][3], int lane, double (&acc)[NB][NT][2])
-{
-    const int t = lane & 3;
-    const double4 *sh4 = reinterpret_cast<const double4 *>(shells) + t;
-    const double *b = bf + lane;
-#pragma unroll
-    for (int h = 0; h < NB; ++h)
-#pragma unroll
-        for (int nt = 0; nt < NT; ++nt) { acc[h][nt][0] = 0.0; acc[h][nt][1] = 0.0; }
-    double dx[NB], dy[NB], dz[NB], e[NB], a[NB];
-#ifdef LRDMC_SPLIT_ACC
-    double acc2[NB][NT][2];       // second accumulator set: consecutive k-steps of one batch do not wait for each other
-#pragma unroll
-    for (int h = 0; h < NB; ++h)
-#pragma unroll
-        for (int nt = 0; nt < NT; ++nt) { acc2[h][nt][0] = 0.0; acc2[h][nt][1] = 0.0; }
-#define LRDMC_ACC2 acc2
-#else
-#define LRDMC_ACC2 acc
-#endif
-#define LRDMC_FEED_(ACC)                                                                        \
-    {                                                                                           \
-        _Pragma("unroll") for (int nt = 0; nt < NT; ++nt) {                                     \
-            const double bv_ = ldt<TS>(b + nt * 32);                                                      \
-            _Pragma("unroll") for (int h = 0; h < NB; ++h) dmma884(ACC[h][nt][0], ACC[h][nt][1], a[h], bv_); \
-        }                                                                                       \
-        b += NT * 32;                                                                           \
-    }
-#define LRDMC_FEEDN LRDMC_FEED_(acc)
-#define LRDMC_FEEDM LRDMC_FEED_(LRDMC_ACC2)
-#define LRDMC_DISPN(SLATER)                                                                     \
-        const double4 s = *sh4; const double z = s.w;                                           \
-        _Pragma("unroll") for (int h = 0; h < NB; ++h) {                                        \
-            dx[h] = pt[h][0] - s.x; dy[h] = pt[h][1] - s.y; dz[h] = pt[h][2] - s.z;              \
-            const double q = dx[h] * dx[h] + dy[h] * dy[h] + dz[h] * dz[h];                      \
-            e[h] = exp_tab(exp_arg_floor(-z * (SLATER ? q * fast_rsqrt(q) : q)), etab);                         \
-        }
-#define LRDMC_SETA(expr) _Pragma("unroll") for (int h = 0; h < NB; ++h) a[h] = (expr);
-    for (int it = 0; it < S.n_it[0]; ++it, sh4 += 4) { LRDMC_DISPN(true) LRDMC_SETA(e[h]) LRDMC_FEEDN }      // Slater s
-    for (int it = 0; it < S.n_it[1]; ++it, sh4 += 4) { LRDMC_DISPN(false) LRDMC_SETA(e[h]) LRDMC_FEEDN }     // s
-    for (int it = 0; it < S.n_it[2]; ++it, sh4 += 4) {                                                        // p: x y z
-        LRDMC_DISPN(false)
-        LRDMC_SETA(dx[h] * e[h]) LRDMC_FEEDN LRDMC_SETA(dy[h] * e[h]) LRDMC_FEEDM LRDMC_SETA(dz[h] * e[h]) LRDMC_FEEDN
-    }
-    for (int it = 0; it < S.n_it[3]; ++it, sh4 += 4) {                                                        // d: xx xy xz yy yz zz
-        LRDMC_DISPN(false)
-        double xe[NB], ye[NB], ze[NB];
-#pragma unroll
-        for (int h = 0; h < NB; ++h) { xe[h] = dx[h] * e[h]; ye[h] = dy[h] * e[h]; ze[h] = dz[h] * e[h]; }
-        LRDMC_SETA(dx[h] * xe[h]) LRDMC_FEEDN LRDMC_SETA(dx[h] * ye[h]) LRDMC_FEEDM LRDMC_SETA(dx[h] * ze[h]) LRDMC_FEEDN
-        LRDMC_SETA(dy[h] * ye[h]) LRDMC_FEEDM LRDMC_SETA(dy[h] * ze[h]) LRDMC_FEEDN LRDMC_SETA(dz[h] * ze[h]) LRDMC_FEEDM
-    }
-#ifdef LRDMC_SPLIT_ACC
-#pragma unroll
-    for (int h = 0; h < NB; ++h)
-#pragma unroll
-        for (int nt = 0; nt < NT; ++nt) { acc[h][nt][0] += acc2[h][nt][0]; acc[h][nt][1] += acc2[h][nt][1]; }
-#endif
-#undef LRDMC_SETA
-#undef LRDMC_DISPN
-#undef LRDMC_FEEDN
-#undef LRDMC_FEEDM
-#undef LRDMC_FEED_
-#undef LRDMC_ACC2
-}
-
 // ---- candidate ratios in column form (rows a2-a4 fused) -----------------------------------------------------------
 // The determinant ratio of candidate p (electron i moved to r'_p) needs ONE linear combination of the MOs at r'_p:
 //     sum_m phi_m(r'_p) Dinv[m][i]  =  sum_mu chi_mu(r'_p) Bc[mu][i],      Bc = C Dinv   (A x n_s),
@@ -196,96 +125,6 @@ __device__ __forceinline__ void mo_values(const DevSys &S, const double *__restr
 // centre distance and three dot products between the six exponent arguments.
 //   av[k] = a e_k (displacement of direction +k), a2 = a^2;  acc[d], d = 2k (+), 2k+1 (-): this lane's share (its
 //   shells) of the determinant ratio of candidate (i, d); the caller adds the four lanes of a quad.
-#if !LRDMC_BC_DMMA
-template <int NT, bool TS, bool PART = false, int BCS = 0>
-__device__ __forceinline__ void ao_columns(const DevSys &S, const double *__restrict__ shells, const double *__restrict__ bf, const double *__restrict__ etab,
-                                           const double *__restrict__ dinv, int ns, int il, double x0, double y0, double z0,
-                                           const double (&av)[3][3], double a2, int lane, double (&acc)[6],
-                                           const TeamPlan * = nullptr, const ShellPart * = nullptr, double2 * = nullptr)
-{
-    const int t = lane & 3;
-    const double4 *sh4 = reinterpret_cast<const double4 *>(shells) + t;
-    const double *b = bf + t;                        // entry (k-step, MO m, shell slot t) sits at b[(kstep NT + m/8) 32 + (m%8) 4]
-    constexpr int NM = 8 * NT;
-    double dcol[NT <= 2 ? NM : 1];                   // column il of Dinv (rows >= n_s are zero padded)
-    if (NT <= 2) {
-#pragma unroll
-        for (int m = 0; m < (NT <= 2 ? NM : 1); ++m) dcol[m] = dinv[m * ns + il];
-    }
-#pragma unroll
-    for (int d = 0; d < 6; ++d) acc[d] = 0.0;
-#define LRDMC_DC(m) (NT <= 2 ? dcol[NT <= 2 ? (m) : 0] : dinv[(m) * ns + il])
-#define LRDMC_BCOL(dst)                                                                         \
-    {                                                                                           \
-        double s_ = 0.0;                                                                        \
-        _Pragma("unroll") for (int m = 0; m < NM; ++m) s_ = fma(ldt<TS>(b + (m >> 3) * 32 + (m & 7) * 4), LRDMC_DC(m), s_); \
-        dst = s_; b += NT * 32;                                                                 \
-    }
-    // exponent arguments of the six displaced points: -z (q0 +- 2 sk[k]),  q0 = |d0|^2 + a^2,  sk[k] = a e_k . d0
-#define LRDMC_GEOM                                                                              \
-        const double4 s = *sh4; const double z = s.w;                                           \
-        const double dx0 = x0 - s.x, dy0 = y0 - s.y, dz0 = z0 - s.z;                            \
-        const double q0 = fma(dx0, dx0, fma(dy0, dy0, fma(dz0, dz0, a2)));                      \
-        double sk[3];                                                                           \
-        _Pragma("unroll") for (int k = 0; k < 3; ++k) sk[k] = fma(av[k][0], dx0, fma(av[k][1], dy0, av[k][2] * dz0));
-#define LRDMC_EXPS                                                                              \
-        const double zq0 = -z * q0; const bool far_ = zq0 < 0.5 * LRDMC_EXP_XMIN;   /* |2 z sk| <= z q0: the six arguments lie in [2 zq, 0] */ \
-        const double zq = far_ ? 0.5 * LRDMC_EXP_XMIN : zq0, tz = far_ ? 0.0 : -2.0 * z;        \
-        double ex_[6], e[6];                                                                    \
-        _Pragma("unroll") for (int k = 0; k < 3; ++k) { ex_[2 * k] = fma(tz, sk[k], zq); ex_[2 * k + 1] = fma(-tz, sk[k], zq); } \
-        exp_tab_n<6>(ex_, e, etab);
-    for (int it = 0; it < S.n_it[0]; ++it, sh4 += 4) {            // Slater s: exp(-z r)
-        LRDMC_GEOM
-        double bc; LRDMC_BCOL(bc)
-#pragma unroll
-        for (int d = 0; d < 6; ++d) {
-            const double q = fma((d & 1) ? -2.0 : 2.0, sk[d >> 1], q0);
-            acc[d] = fma(exp_tab(exp_arg_floor(-z * (q * fast_rsqrt(q))), etab), bc, acc[d]);
-        }
-    }
-    for (int it = 0; it < S.n_it[1]; ++it, sh4 += 4) {            // s
-        LRDMC_GEOM
-        double bc; LRDMC_BCOL(bc)
-        LRDMC_EXPS
-#pragma unroll
-        for (int d = 0; d < 6; ++d) acc[d] = fma(e[d], bc, acc[d]);
-    }
-    for (int it = 0; it < S.n_it[2]; ++it, sh4 += 4) {            // p: x y z  ->  e (bc . d)
-        LRDMC_GEOM
-        double bc[3]; LRDMC_BCOL(bc[0]) LRDMC_BCOL(bc[1]) LRDMC_BCOL(bc[2])
-        LRDMC_EXPS
-        const double l0 = fma(bc[0], dx0, fma(bc[1], dy0, bc[2] * dz0));        // linear form at d0; the shift adds bc . (a e_k)
-#pragma unroll
-        for (int k = 0; k < 3; ++k) {
-            const double lk = fma(bc[0], av[k][0], fma(bc[1], av[k][1], bc[2] * av[k][2]));
-            acc[2 * k] = fma(e[2 * k], l0 + lk, acc[2 * k]);
-            acc[2 * k + 1] = fma(e[2 * k + 1], l0 - lk, acc[2 * k + 1]);
-        }
-    }
-    for (int it = 0; it < S.n_it[3]; ++it, sh4 += 4) {            // d: xx xy xz yy yz zz  ->  e Q(d),  Q(d0 +- v) = Q(d0) +- v.grad Q(d0) + Q(v)
-        LRDMC_GEOM
-        double bc[6]; LRDMC_BCOL(bc[0]) LRDMC_BCOL(bc[1]) LRDMC_BCOL(bc[2]) LRDMC_BCOL(bc[3]) LRDMC_BCOL(bc[4]) LRDMC_BCOL(bc[5])
-        LRDMC_EXPS
-        const double gx = fma(2.0 * bc[0], dx0, fma(bc[1], dy0, bc[2] * dz0));
-        const double gy = fma(bc[1], dx0, fma(2.0 * bc[3], dy0, bc[4] * dz0));
-        const double gz = fma(bc[2], dx0, fma(bc[4], dy0, 2.0 * bc[5] * dz0));
-        const double Q0 = 0.5 * fma(gx, dx0, fma(gy, dy0, gz * dz0));
-#pragma unroll
-        for (int k = 0; k < 3; ++k) {
-            const double vx = av[k][0], vy = av[k][1], vz = av[k][2];
-            const double lin = fma(gx, vx, fma(gy, vy, gz * vz));
-            const double Qv = fma(vx, fma(bc[0], vx, fma(bc[1], vy, bc[2] * vz)), fma(vy, fma(bc[3], vy, bc[4] * vz), bc[5] * vz * vz));
-            const double Qs = Q0 + Qv;
-            acc[2 * k] = fma(e[2 * k], Qs + lin, acc[2 * k]);
-            acc[2 * k + 1] = fma(e[2 * k + 1], Qs - lin, acc[2 * k + 1]);
-        }
-    }
-#undef LRDMC_EXPS
-#undef LRDMC_GEOM
-#undef LRDMC_BCOL
-#undef LRDMC_DC
-}
-#else
 // Bc on the FP64 tensor pipe: one mma.m8n8k4 row = electron g, k = 4 MOs, columns = (k-step parity, shell slot), so the
 // lane's two accumulators are exactly its own entries Bc[ao(slot t)][electron g] of two consecutive k-steps:
 // 2 NT DMMA + 2 NT LDS per pair of entries instead of 16 NT DFMA + 16 NT LDS (same FP64-pipe time, 1/8 of the issue slots).
@@ -406,7 +245,6 @@ __device__ __forceinline__ void ao_columns(const DevSys &S, const double *__rest
 #undef LRDMC_BPAIR
 #undef LRDMC_COL_RANGE
 }
-#endif
 
 // Refresh the cached MO rows (value, gradient, Laplacian) of electron i at position (px,py,pz): moc[i][comp][m].
 template <int NT, bool TS>
