@@ -51,6 +51,7 @@ SYSTEMS = {
     "tiny-3u2d-nlTM-K2": lambda: _with_walkers(wl.random_nonlocal(wl.tiny_molecule(3, 2, 3, 9, seed=21, with_pp=True), 5, 1.6, 2, False), 37),
     "tiny-3u2d-nlDLA-strong": lambda: _with_walkers(wl.random_nonlocal(wl.tiny_molecule(3, 2, 3, 9, seed=21, with_pp=True), 5, 1.6, 2, True, scale=200.0), 37),
     "tiny-2u1d-nlTM-strong": lambda: _with_walkers(wl.random_nonlocal(wl.tiny_molecule(2, 1, 2, 6, seed=7), 8, 1.4, 1, False, scale=600.0), 41),
+    "tiny-2u2d-doublemesh-nlTM": lambda: _with_walkers(wl.random_nonlocal(wl.tiny_molecule(2, 2, 2, 7, seed=9, a=0.15, a2=0.3), 4, 1.5, 2, False, scale=150.0), 33),
     "ragged-9u4d-nlDLA": lambda: _with_walkers(wl.random_nonlocal(wl.tiny_molecule(9, 4, 4, 20, seed=11), 6, 1.2, 2, True), 13),
     "C3-water-methane-nlDLA": lambda: _with_walkers(wl.water_methane_nonlocal(n_walkers=100), 100),
     "C3-water-methane-nlTM": lambda: _with_walkers(wl.water_methane_nonlocal(n_walkers=50, dla=False), 50),
@@ -150,7 +151,7 @@ def test_whole_cycle_trajectories_weights_and_branching(B, name, mode, kernel, m
                                        ("ragged-17u3d-NT4", "conventional"), ("he-triplet-slater", "balanced"), ("C3-water-methane-shaped", "balanced"),
                                        ("C3-water-methane-shaped", "conventional"), ("C5-cluster64-doublemesh", "balanced"),
                                        ("tiny-3u2d-nlDLA-strong", "balanced"), ("tiny-2u1d-nlTM-strong", "conventional"), ("C3-water-methane-nlDLA", "balanced"),
-                                       ("C3-water-methane-nlTM", "balanced"), ("contracted-4u4d-sph-nlDLA", "balanced")])
+                                       ("C3-water-methane-nlTM", "balanced"), ("contracted-4u4d-sph-nlDLA", "balanced"), ("tiny-2u2d-doublemesh-nlTM", "conventional")])
 def test_team_kernel_every_team_size(B, name, mode, tw, monkeypatch):
     """k_propagate_team with TW = 2, 4, 8, 16 warps per walker (work units = electron blocks x shell parts, partial sums
     in shared memory): same trajectories, weights and indices as the oracle."""
