@@ -326,8 +326,8 @@ static void partition_shells(const int n_it[4], const double cost[4], bool pairs
 }
 
 // Choose the team size for n_w walkers.  Warp-per-walker (team_tw = 1) when the walkers alone fill the resident warp slots;
-// otherwise the largest power of two 4 <= TW <= 16 with n_w TW <= slots (few walkers), or 4 for the large systems whose 36 KB
-// state leaves one warp per scheduler.  LRDMC_TEAM=<tw> forces a size (0/1: never).
+// otherwise 4 warps per walker: for few walkers (n_w up to 3/8 of the warp slots), and for the large systems whose 36 KB state
+// leaves one warp per scheduler.  LRDMC_TEAM=<tw> forces a size (0/1: never).
 static void plan_team(lrdmc_ctx *c, int n_w)
 {
     const DevSys &S = c->S; TeamPlan &P = c->team;
@@ -335,7 +335,8 @@ static void plan_team(lrdmc_ctx *c, int n_w)
     int tw = 1;
     const long slots = (long)c->grid_max * c->wpb;
     if (!c->ts) tw = 4;
-    else for (int cand = 4; cand <= LRDMC_TEAM_MAX_WARPS; cand *= 2) if ((long)n_w * cand <= slots) tw = cand;   // measured: 2 warps per walker do not pay
+    else if ((long)n_w * 8 <= 3 * slots) tw = 4;   // measured on C3/C4 (profiles/r1_team_kernel.md): 4 warps per walker beat 2, 8 and 16 at every N_w,
+                                                   // and beat warp-per-walker up to N_w of about 3/8 of the resident warp slots
     if (const char *e = getenv("LRDMC_TEAM")) { int v = atoi(e); tw = v < 1 ? 1 : v; }
     int p2 = 1; while (p2 * 2 <= tw && p2 * 2 <= LRDMC_TEAM_MAX_WARPS) p2 *= 2;
     tw = p2;
