@@ -384,6 +384,15 @@ extern "C" int lrdmc_bind_walkers(lrdmc_ctx *c, void *dev_buf, size_t bytes, int
 
 // ---- launch helpers -----------------------------------------------------------------------------------------------
 static int grid_for(const lrdmc_ctx *c) { int g = (c->W.n_w + c->wpb - 1) / c->wpb; return g < c->grid_max ? g : c->grid_max; }
+// Warp-per-walker launch of lrdmc_propagate: an SM's time grows with its resident warps (the kernel is dispatch-bound), so an
+// ensemble that does not fill the warp slots is spread over ALL resident CTAs with fewer warps each, instead of filling some SMs
+// with full CTAs (N_w = 1200 on C4: 150 CTAs x 8 warps put 16 walkers on two SMs -> 4.44 ms; 240 x 5 warps -> 10 per SM).
+static void propagate_shape(const lrdmc_ctx *c, int *grid, int *warps)
+{
+    int w = (c->W.n_w + c->grid_max - 1) / c->grid_max; if (w > c->wpb) w = c->wpb; if (w < 1) w = 1;
+    int g = (c->W.n_w + w - 1) / w; if (g > c->grid_max) g = c->grid_max;
+    *grid = g; *warps = w;
+}
 #define LAUNCH_(KERNEL, NTV, TSV, NLV, grid, stream, ...) KERNEL<NTV, TSV, NLV><<<grid, c->wpb * 32, c->smem_bytes, stream>>>(__VA_ARGS__)
 #define DISPATCH_NL_(KERNEL, NLV, grid, stream, ...)                                                             \
     do {                                                                                                         \
@@ -475,19 +484,20 @@ extern "C" int lrdmc_propagate(lrdmc_ctx *c, int mode, int n_moves, double tau, 
     cudaStream_t st = (cudaStream_t)stream;
     CK(cudaMemsetAsync(c->W.counter, 0, 64 * sizeof(int), st));
     const bool team = c->team_tw > 1;
-    const int grid = team ? (c->W.n_w < c->team_grid_max ? c->W.n_w : c->team_grid_max) : grid_for(c);
+    int grid = team ? (c->W.n_w < c->team_grid_max ? c->W.n_w : c->team_grid_max) : 0, warps = c->wpb;
+    if (!team) propagate_shape(c, &grid, &warps);
     CK(cudaEventRecord(c->ev[0], st));
     if (team) {
         if (c->S.nl_K) lrdmc_k_team_nl(c->NT, c->ts, grid, c->team_tw * 32, c->team_smem, st, c->S, c->W, c->team, mode, n_moves, tau, E0, (uint32_t)cycle);
         else lrdmc_k_team_lat(c->NT, c->ts, grid, c->team_tw * 32, c->team_smem, st, c->S, c->W, c->team, mode, n_moves, tau, E0, (uint32_t)cycle);
     } else {
-        if (c->S.nl_K) lrdmc_k_propagate_nl(c->NT, c->ts, grid, c->wpb * 32, c->smem_bytes, st, c->S, c->W, mode, n_moves, tau, E0, (uint32_t)cycle);
-        else lrdmc_k_propagate_lat(c->NT, c->ts, grid, c->wpb * 32, c->smem_bytes, st, c->S, c->W, mode, n_moves, tau, E0, (uint32_t)cycle);
+        if (c->S.nl_K) lrdmc_k_propagate_nl(c->NT, c->ts, grid, warps * 32, c->smem_bytes, st, c->S, c->W, mode, n_moves, tau, E0, (uint32_t)cycle);
+        else lrdmc_k_propagate_lat(c->NT, c->ts, grid, warps * 32, c->smem_bytes, st, c->S, c->W, mode, n_moves, tau, E0, (uint32_t)cycle);
     }
     ++c->launches;
     CK(cudaEventRecord(c->ev[1], st));
     CK(cudaGetLastError());
-    k_reduce_obs<<<1, 1024, 0, st>>>(c->W, c->d_stats, team ? grid : grid * c->wpb); ++c->launches;
+    k_reduce_obs<<<1, 1024, 0, st>>>(c->W, c->d_stats, team ? grid : grid * warps); ++c->launches;
     CK(cudaGetLastError());
     c->have_prop = 1; c->last_stream = st;
     return LRDMC_OK;
@@ -564,7 +574,8 @@ extern "C" int lrdmc_launch_config(const lrdmc_ctx *c, int *grid, int *block, in
         if (block) *block = c->team_tw * 32; if (smem_bytes) *smem_bytes = c->team_smem; if (ctas_per_sm) *ctas_per_sm = c->team_ctas_per_sm;
         return LRDMC_OK;
     }
-    if (grid) *grid = c->bound ? grid_for(c) : c->grid_max; if (block) *block = c->wpb * 32; if (smem_bytes) *smem_bytes = c->smem_bytes;
+    int pg = c->grid_max, pw = c->wpb; if (c->bound) propagate_shape(c, &pg, &pw);
+    if (grid) *grid = pg; if (block) *block = pw * 32; if (smem_bytes) *smem_bytes = c->smem_bytes;
     if (ctas_per_sm) *ctas_per_sm = c->ctas_per_sm;
     return LRDMC_OK;
 }
