@@ -34,10 +34,28 @@ static double dist(const double *p, const double *q)
     return sqrt(dx * dx + dy * dy + dz * dz);
 }
 
+/* chi_a(r) = exp(-zeta_a |r - R_a|^2) of the three-body Jastrow, optionally with gradient and Laplacian */
+static double j3_chi(const lrdmc_ref_ctx *c, int a, const double r[3], double g[3], double *lap)
+{
+    const double *Ra = c->Rn + 3 * c->j3_center[a]; double z = c->j3_zeta[a];
+    double d[3] = { r[0] - Ra[0], r[1] - Ra[1], r[2] - Ra[2] }, r2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2], v = exp(-z * r2);
+    if (g) for (int ax = 0; ax < 3; ++ax) g[ax] = -2.0 * z * d[ax] * v;
+    if (lap) *lap = (4.0 * z * z * r2 - 6.0 * z) * v;
+    return v;
+}
+/* V_a(i) = sum_{j != i} sum_b g_ab chi_b(r_j): the three-body field electron i feels through basis function a */
+static double j3_field(const lrdmc_ref_ctx *c, const double *x, int i, int a)
+{
+    double V = 0.0;
+    for (int j = 0; j < c->N; ++j) if (j != i) for (int b = 0; b < c->n_j3; ++b) V += c->j3_g[a * c->n_j3 + b] * j3_chi(c, b, x + 3 * j, NULL, NULL);
+    return V;
+}
+
 /* the part of J that involves electron i when it sits at ri (other electrons at x) */
 static double jastrow_of_electron(const lrdmc_ref_ctx *c, const double *x, int i, const double ri[3])
 {
     double J = 0.0;
+    for (int a = 0; a < c->n_j3; ++a) J += j3_chi(c, a, ri, NULL, NULL) * j3_field(c, x, i, a);   /* g symmetric: i<j and j<i pairs alike */
     if (c->c1) for (int I = 0; I < c->n_nuc; ++I) { double r = dist(ri, c->Rn + 3 * I); J -= c->c1[I] * r / (1.0 + c->b1[I] * r); }
     for (int j = 0; j < c->N; ++j) if (j != i) {
         double r = dist(ri, x + 3 * j), aij = ref_spin(c, i) == ref_spin(c, j) ? c->a_par : c->a_anti;
@@ -183,6 +201,12 @@ int lrdmc_ref_evaluate(const lrdmc_ref_ctx *c, const double *x, const double *di
             for (int ax = 0; ax < 3; ++ax) gJ[ax] += du * (ri[ax] - rj[ax]) / r;
             lJ += lu;
             if (j > i) Vee += 1.0 / r;
+        }
+        for (int a = 0; a < c->n_j3; ++a) {              /* three-body Jastrow: grad_i J3 = sum_a grad chi_a(r_i) V_a(i), same for the Laplacian */
+            double ga[3], la, V = j3_field(c, x, i, a);
+            j3_chi(c, a, ri, ga, &la);
+            for (int ax = 0; ax < 3; ++ax) gJ[ax] += ga[ax] * V;
+            lJ += la * V;
         }
         /* lap_i Psi / Psi for Psi = D exp(J) */
         double lap_i = Ld + 2.0 * (G[0] * gJ[0] + G[1] * gJ[1] + G[2] * gJ[2]) + lJ + (gJ[0] * gJ[0] + gJ[1] * gJ[1] + gJ[2] * gJ[2]);

@@ -190,6 +190,14 @@ int lrdmc_ref_logpsi(const lrdmc_ref_ctx *c, const double *x, double *logabs, in
             J += pade(aij, c->b2, sqrt(dx * dx + dy * dy + dz * dz));
         }
     }
+    /* three-body term, written as defined: sum_{i<j} sum_{ab} g_ab chi_a(r_i) chi_b(r_j) */
+    for (int i = 0; i < c->N; ++i) for (int j = i + 1; j < c->N; ++j)
+        for (int a = 0; a < c->n_j3; ++a) for (int b = 0; b < c->n_j3; ++b) {
+            const double *Ra = c->Rn + 3 * c->j3_center[a], *Rb = c->Rn + 3 * c->j3_center[b];
+            double da2 = 0.0, db2 = 0.0;
+            for (int ax = 0; ax < 3; ++ax) { double u = x[3 * i + ax] - Ra[ax], v = x[3 * j + ax] - Rb[ax]; da2 += u * u; db2 += v * v; }
+            J += c->j3_g[a * c->n_j3 + b] * exp(-c->j3_zeta[a] * da2) * exp(-c->j3_zeta[b] * db2);
+        }
     *logabs = la + J; *sign = sg;
     return LRDMC_REF_OK;
 }

@@ -57,6 +57,7 @@ def _system(name, Z, R, n_up, n_dn, center, stype, zeta, C_up, C_dn, jastrow, a,
         a=float(a), a2=float(a2), seed=int(seed),
         n_walkers=int(n_walkers), cycles=int(cycles), moves=int(moves),
         nl=None, nl_K=0, nl_dla=1,      # non-local pseudopotential channels (scope row f1): see with_nonlocal
+        j3_center=None, j3_zeta=None, j3_g=None,   # three-body Jastrow (scope row f2): see with_jastrow3
     )
     assert d["C_up"].shape == (d["n_ao"], d["n_up"])
     assert d["C_dn"].shape == (d["n_ao"], d["n_dn"])
@@ -242,6 +243,20 @@ def contracted_molecule(n_up=3, n_dn=2, n_nuc=3, n_cshell=9, seed=31, a=0.2, sph
     jas = dict(a_par=0.25, a_anti=0.5, b2=0.8, c1=c1, b1=rng.uniform(0.5, 1.5, size=n_nuc))
     return _system(f"contracted-{n_up}u{n_dn}d" + ("-sph" if spherical else "-cart"), Z, R, n_up, n_dn, center, stype, zeta, C_up, C_dn, jas, a,
                    pp=pp, contraction=(first, coef, sph))
+
+
+def with_jastrow3(sysd, seed, n_per_nucleus=1, strength=0.3):
+    """Attach a synthetic three-body Jastrow J3 = sum_{i<j} sum_ab g_ab chi_a(r_i) chi_b(r_j) on s-type Gaussians chi_a =
+    exp(-zeta_a |r - R_a|^2) centred on the nuclei (at most 8 functions): zeta log-uniform in [0.3, 2], g symmetric, uniform in
+    [-strength, strength].  The paper's runs use the TurboRVB 3-body Jastrow with optimised parameters (L242, L285): not in the container."""
+    rng = np.random.default_rng(seed)
+    centers = [I for I in range(sysd["n_nuc"]) for _ in range(n_per_nucleus)][:8]
+    n = len(centers)
+    zeta = np.exp(rng.uniform(np.log(0.3), np.log(2.0), size=n))
+    g = rng.uniform(-strength, strength, size=(n, n)); g = 0.5 * (g + g.T)
+    d = dict(sysd)
+    d.update(j3_center=np.ascontiguousarray(centers, dtype=np.int32), j3_zeta=zeta, j3_g=np.ascontiguousarray(g), name=sysd["name"] + "-J3")
+    return d
 
 
 def with_nonlocal(sysd, nl, dla=True):

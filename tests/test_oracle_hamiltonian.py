@@ -64,6 +64,7 @@ SYSTEMS = {
     "tiny-2u2d-doublemesh": lambda: wl.tiny_molecule(2, 2, 2, 7, seed=9, a=0.15, a2=0.3),
     "C2": wl.synthetic10,
     "C3": lambda: wl.water_methane(n_walkers=4),
+    "tiny-j3": lambda: wl.with_jastrow3(wl.tiny_molecule(3, 2, 3, 9, seed=21, with_pp=True), 4, 2),   # three-body Jastrow (scope row f2)
     "contracted-sph": lambda: wl.contracted_molecule(3, 2, 3, 9, seed=31, spherical=True, with_pp=True),   # scope row f2
 }
 
@@ -94,7 +95,7 @@ def test_regularised_local_energy_equals_continuum_local_energy(name):
     assert checked >= 1     # random-MO trial functions have nodes everywhere: the D11 branch fires often on C3
 
 
-@pytest.mark.parametrize("name", ["tiny-2u1d", "tiny-3u3d-pp", "C2", "contracted-sph"])
+@pytest.mark.parametrize("name", ["tiny-2u1d", "tiny-3u3d-pp", "C2", "contracted-sph", "tiny-j3"])
 def test_continuum_laplacian_matches_finite_differences_of_logpsi(name):
     """lap_i Psi/Psi = lap_i log|Psi| + |grad_i log|Psi||^2, by 4th-order central differences of the brute-force log|Psi|."""
     s = SYSTEMS[name](); o = ref.Ref(s); x = wl.initial_walkers(s, 1, 33)[0]
@@ -112,7 +113,7 @@ def test_continuum_laplacian_matches_finite_differences_of_logpsi(name):
 
 
 # ----------------------------------------------------------------------------- ratios vs brute force (pin P3)
-@pytest.mark.parametrize("name", ["tiny-2u1d", "tiny-3u3d-pp", "tiny-2u2d-doublemesh", "C2", "contracted-sph"])
+@pytest.mark.parametrize("name", ["tiny-2u1d", "tiny-3u3d-pp", "tiny-2u2d-doublemesh", "C2", "contracted-sph", "tiny-j3"])
 def test_candidate_ratios_match_full_wavefunction_recomputation(name):
     s = SYSTEMS[name](); o = ref.Ref(s); rng = np.random.default_rng(6)
     x = wl.initial_walkers(s, 1, 44)[0]; U = _rand_frame(rng)
@@ -140,6 +141,13 @@ def test_logpsi_matches_numpy_slogdet_and_explicit_jastrow():
             J += aij * r / (1 + s["b2"] * r)
     la, sg = o.logpsi(x)
     assert sg == int(su * sd) and abs(la - (lu + ld + J)) < 1e-11
+    # three-body Jastrow: J3 = sum_{i<j} sum_ab g_ab chi_a(r_i) chi_b(r_j), chi_a = exp(-zeta_a |r - R_a|^2), written out with numpy
+    s3 = wl.with_jastrow3(s, 4, 2); o3 = ref.Ref(s3)
+    chi = np.exp(-s3["j3_zeta"][None, :] * np.sum((x[:, None, :] - s["R"][s3["j3_center"]][None, :, :]) ** 2, axis=2))    # [electron][a]
+    M = chi @ s3["j3_g"] @ chi.T
+    J3 = np.sum(np.triu(M, 1))
+    la3, sg3 = o3.logpsi(x)
+    assert sg3 == sg and abs(la3 - (la + J3)) < 1e-12 and abs(J3) > 1e-3
 
 
 @pytest.mark.parametrize("name", ["tiny-2u1d", "tiny-3u3d-pp", "C2"])
