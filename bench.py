@@ -113,7 +113,7 @@ def main():
     ap.add_argument("--impl", default="ours"); ap.add_argument("--nw", type=int, default=25600); ap.add_argument("--moves", type=int, default=100)
     ap.add_argument("--ref-nw", type=int, default=64); ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-conventional", action="store_true"); ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--workload", default="C4", choices=["C1", "C2", "C4", "C5", "C3nl"],
+    ap.add_argument("--workload", default="C4", choices=["C1", "C2", "C4", "C5", "C3nl", "C3j3"],
                     help="C4 (default) is the configuration the metric is quoted on; C2 / C5 are the other BASELINE.json systems, C3nl adds non-local pseudopotential channels (use with --nw/--moves)")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1")); local = int(os.environ.get("LOCAL_RANK", "0"))
@@ -140,6 +140,9 @@ def main():
     elif args.workload == "C2":
         sysd = wl.synthetic10(n_walkers=args.nw, moves=args.moves, seed=wl.PHILOX_RUN_SEED + rank)
         wname = "C2 synthetic 10-electron molecule: 5/5, 3 nuclei, 60 s/p/d GTOs, 1b+2b Jastrow, a=0.2 (BASELINE.json configs[1])"
+    elif args.workload == "C3j3":
+        sysd = wl.with_jastrow3(wl.water_methane(n_walkers=args.nw, moves=args.moves, seed=wl.PHILOX_RUN_SEED + rank), 7, 1, strength=0.05)
+        wname = "C3/C4 water-methane-shaped system + synthetic three-body Jastrow (8 s Gaussians at the nuclei): scope row f2; flop count = without the J3 part"
     elif args.workload == "C3nl":
         sysd = wl.water_methane_nonlocal(n_walkers=args.nw, moves=args.moves, seed=wl.PHILOX_RUN_SEED + rank)
         wname = "C3/C4 water-methane-shaped system + synthetic non-local s/p/d pseudopotential channels (r_c = 0.8 bohr, DLA): scope row f1; flop count = lattice part only"

@@ -22,6 +22,7 @@
 #define LRDMC_NUC_STRIDE 20  // doubles per nucleus row: Rx Ry Rz Z c1 b1 alpha beta gamma delta is_pp pad | r_c A0 B0 A1 B1 A2 B2 pad (non-local channels)
 #define LRDMC_NL_OFF 12      // first non-local entry of a nucleus row
 #define LRDMC_NL_MAX_K 4
+#define LRDMC_J3_MAX 8
 #define LRDMC_EL_ARRAYS 4     // per-electron scratch arrays in shared memory: Jold, lap, s_k, old column
 
 // Everything a kernel needs to know about the system; passed by value (fits the 4 KB parameter space).
@@ -37,6 +38,8 @@ struct DevSys {
     int has_j1, has_pp;
     double amesh[2], gmesh[2], kappa[2], g_over_a2[2];
     double a_par, a_anti, b2, V_ii, Kdiag, a;
+    // three-body Jastrow J3 = sum_{i<j} sum_ab g_ab chi_a(r_i) chi_b(r_j), chi_a = exp(-zeta_a |r - R_a|^2) (extended kernels only)
+    int n_j3, j3_center[LRDMC_J3_MAX]; double j3_zeta[LRDMC_J3_MAX], j3_g[LRDMC_J3_MAX * LRDMC_J3_MAX];
     uint32_t key0, key1;
     // device tables (global memory copies; staged into shared memory when they fit)
     const double *shells;      // [n_slots][4] = cx cy cz zeta
@@ -48,7 +51,7 @@ struct DevSys {
     // shared-memory plan (units: doubles)
     int bf_in_smem, moc_in_smem;
     int off_shells, off_nuc, off_bf[2], off_etab, tables_doubles;
-    int o_r, o_dinv[2], o_moc, o_R, o_cum, o_el, o_ob, o_U, per_warp_doubles;
+    int o_r, o_dinv[2], o_moc, o_R, o_cum, o_el, o_ob, o_U, o_j3, per_warp_doubles;   // o_j3: chi3 [N][8], V3 [N][8], S3 [8] (systems with a J3)
     int dinv_rows[2];     // padded row count 8*NT
 };
 

@@ -8,6 +8,7 @@
 
 struct WarpState {            // per-warp views (shared memory; moc may live in global memory for large systems)
     double *r, *dinv[2], *moc, *R, *cum, *el, *ob, *U;
+    double *j3;               // three-body Jastrow (systems that have one): chi3 [N][8] = chi_a(r_j), then V3 [N][8], then S3 [8]
 };
 struct EvalOut { double bbar, Vsf, W, eL; int node; };
 
@@ -42,6 +43,20 @@ __device__ __forceinline__ void refresh_onebody(int n_nuc, int has_j1, double a_
     }
     J = warp_sum(J); gx = warp_sum(gx); gy = warp_sum(gy); gz = warp_sum(gz); lJ = warp_sum(lJ); vei = warp_sum(vei); vb = warp_sum(vb);
     if (lane == 0) { ob_i[0] = J; ob_i[1] = gx; ob_i[2] = gy; ob_i[3] = gz; ob_i[4] = lJ; ob_i[5] = vei; ob_i[6] = vb; }
+}
+
+// Three-body Jastrow (reading Q23): chi_a(r) = exp(-zeta_a |r - R_a|^2) of electron j, lanes a < 8 (zero beyond n_j3).
+__device__ __forceinline__ void refresh_j3_row(const DevSys &S, const double *nuc, double *chi3_j, double x, double y, double z, int lane)
+{
+    if (lane < LRDMC_J3_MAX) {
+        double v = 0.0;
+        if (lane < S.n_j3) {
+            const double *nu = nuc + S.j3_center[lane] * LRDMC_NUC_STRIDE;
+            const double dx = x - nu[0], dy = y - nu[1], dz = z - nu[2];
+            v = exp_nonpos(-S.j3_zeta[lane] * (dx * dx + dy * dy + dz * dz));
+        }
+        chi3_j[lane] = v;
+    }
 }
 
 // Pade term c r/(1 + b r) = c/(b + 1/r) of one partner at the six displaced points of an electron:
@@ -143,6 +158,23 @@ __device__ __forceinline__ int phase_b_with_nonlocal(const DevSys &S, const Warp
             for (int j = t; j < N; j += 4) {
                 const double c = (j == i) ? 0.0 : ((spin_of(S, j) == sp) ? S.a_par : S.a_anti);
                 pade_six(x0 - ws.r[3 * j], y0 - ws.r[3 * j + 1], z0 - ws.r[3 * j + 2], av, a2, c, S.b2, Jn);
+            }
+        }
+        if (S.n_j3 && (!is_nl || !S.nl_dla)) {                       // three-body Jastrow at the six displaced points: 6 exps per function
+            const double *V3 = ws.j3 + (N + i) * LRDMC_J3_MAX;
+            for (int a0 = 0; a0 < S.n_j3; a0 += 4) {                 // (uniform trip count: exp_tab_n synchronises the warp)
+                const bool on = a0 + t < S.n_j3; const int a = on ? a0 + t : 0;
+                const double *np_ = T.nuc + S.j3_center[a] * LRDMC_NUC_STRIDE, z = S.j3_zeta[a];
+                const double dx = x0 - np_[0], dy = y0 - np_[1], dz = z0 - np_[2], q0 = fma(dx, dx, fma(dy, dy, fma(dz, dz, a2)));
+                double ex_[6], e_[6];
+#pragma unroll
+                for (int k = 0; k < 3; ++k) {
+                    const double sk = fma(av[k][0], dx, fma(av[k][1], dy, av[k][2] * dz));
+                    ex_[2 * k] = exp_arg_floor(-z * fma(2.0, sk, q0)); ex_[2 * k + 1] = exp_arg_floor(-z * fma(-2.0, sk, q0));
+                }
+                exp_tab_n<6>(ex_, e_, T.etab);
+#pragma unroll
+                for (int d = 0; d < 6; ++d) Jn[d] = fma(e_[d], on ? V3[a] : 0.0, Jn[d]);
             }
         }
         const double Jo = Jold[i];
@@ -257,6 +289,19 @@ __device__ __forceinline__ EvalOut evaluate_walker(const DevSys &S, const WarpSt
 
     // ---- phase A (row a6): per-electron continuum pieces.  Two lanes per electron split the e-e partners; the
     //      one-body parts come from the cache.
+    if (NL && S.n_j3) {                // three-body fields V_a(i) = sum_b g_ab (S_b - chi_b(r_i)),  S_b = sum_j chi_b(r_j)
+        double *chi3 = ws.j3, *V3 = ws.j3 + N * LRDMC_J3_MAX, *S3 = V3 + N * LRDMC_J3_MAX;
+        if (lane < LRDMC_J3_MAX) { double sb = 0.0; for (int j = 0; j < N; ++j) sb += chi3[j * LRDMC_J3_MAX + lane]; S3[lane] = sb; }
+        __syncwarp();
+        for (int idx = lane; idx < N * LRDMC_J3_MAX; idx += 32) {
+            const int i = idx / LRDMC_J3_MAX, a = idx - i * LRDMC_J3_MAX;
+            double v = 0.0;
+#pragma unroll
+            for (int b = 0; b < LRDMC_J3_MAX; ++b) v += S.j3_g[a * LRDMC_J3_MAX + b] * (S3[b] - chi3[i * LRDMC_J3_MAX + b]);
+            V3[idx] = v;
+        }
+        __syncwarp();
+    }
     double vee_part = 0.0;
     for (int i0 = 0; i0 < N; i0 += 16) {
         const int i = i0 + (lane >> 1), sub = lane & 1;
@@ -286,6 +331,15 @@ __device__ __forceinline__ EvalOut evaluate_walker(const DevSys &S, const WarpSt
         if (act && sub == 0) {
             const double *ob = ws.ob + 8 * ii;
             gx += ob[1]; gy += ob[2]; gz += ob[3];
+            if (NL && S.n_j3) {        // J3 terms of electron i: sum_a chi_a V_a;  grad chi = -2 zeta d chi;  lap chi = (4 zeta^2 r^2 - 6 zeta) chi
+                const double *chi3 = ws.j3 + ii * LRDMC_J3_MAX, *V3 = ws.j3 + (N + ii) * LRDMC_J3_MAX;
+                for (int a = 0; a < S.n_j3; ++a) {
+                    const double *nu = T.nuc + S.j3_center[a] * LRDMC_NUC_STRIDE, z = S.j3_zeta[a];
+                    const double dx = xi - nu[0], dy = yi - nu[1], dz = zi - nu[2], cv = chi3[a] * V3[a], tz = -2.0 * z * cv;
+                    J += cv; gx += tz * dx; gy += tz * dy; gz += tz * dz;
+                    lJ += (4.0 * z * z * (dx * dx + dy * dy + dz * dz) - 6.0 * z) * cv;
+                }
+            }
             Jold[ii] = J + ob[0];
             lap_s[ii] = Ld + 2.0 * (Gx * gx + Gy * gy + Gz * gz) + (lJ + ob[4]) + (gx * gx + gy * gy + gz * gz);
         }
@@ -372,6 +426,7 @@ __device__ __forceinline__ void apply_move(const DevSys &S, const WarpState &ws,
     __syncwarp();
     refresh_mo_cache<NT, TS>(S, T.shells, sp ? T.bf[1] : T.bf[0], T.etab, mc, px, py, pz, lane);
     refresh_onebody(S.n_nuc, S.has_j1, S.a, T.nuc, ws.ob + 8 * i, px, py, pz, lane);
+    if (NL && S.n_j3) refresh_j3_row(S, T.nuc, ws.j3 + i * LRDMC_J3_MAX, px, py, pz, lane);
     if (lane == 0) { ws.r[3 * i] = px; ws.r[3 * i + 1] = py; ws.r[3 * i + 2] = pz; }
     __syncwarp();
     // s_k = sum_m phi_m Dinv[m][k];  rho = s_il;  Dinv'[m][il] = Dinv[m][il]/rho;  Dinv'[m][k] = Dinv[m][k] - Dinv[m][il] s_k / rho

@@ -114,6 +114,13 @@ extern "C" int lrdmc_init(lrdmc_ctx **out, const lrdmc_system *sys, const lrdmc_
     }
     for (int j = 0; j < S.P_lat; ++j) S.Kdiag += S.kappa[j / (6 * S.N)];      // K^a_{x,x} = sum_j kappa_j = 3N/a^2 (Eq.D5)
     S.a_par = jas->a_par; S.a_anti = jas->a_anti; S.b2 = jas->b2; S.has_j1 = jas->c1 != NULL; S.has_pp = sys->pp != NULL;
+    S.n_j3 = jas->n_j3 > 0 ? jas->n_j3 : 0;
+    if (S.n_j3 > LRDMC_J3_MAX || (S.n_j3 && (!jas->j3_center || !jas->j3_zeta || !jas->j3_g))) { free(c); return LRDMC_EINVAL; }
+    for (int a = 0; a < S.n_j3; ++a) {
+        if (jas->j3_center[a] < 0 || jas->j3_center[a] >= sys->n_nuc || !(jas->j3_zeta[a] > 0.0)) { free(c); return LRDMC_EINVAL; }
+        S.j3_center[a] = jas->j3_center[a]; S.j3_zeta[a] = jas->j3_zeta[a];
+        for (int b = 0; b < LRDMC_J3_MAX; ++b) S.j3_g[a * LRDMC_J3_MAX + b] = b < S.n_j3 ? jas->j3_g[a * S.n_j3 + b] : 0.0;
+    }
     S.key0 = (uint32_t)lat->seed; S.key1 = (uint32_t)(lat->seed >> 32);
     S.V_ii = 0.0;
     for (int I = 0; I < sys->n_nuc; ++I) for (int J = I + 1; J < sys->n_nuc; ++J) {
@@ -234,6 +241,7 @@ extern "C" int lrdmc_init(lrdmc_ctx **out, const lrdmc_system *sys, const lrdmc_
     S.o_el = (int)w; w += align_up((size_t)LRDMC_EL_ARRAYS * S.N, 2);
     S.o_U = (int)w; w += 10;                    // the step's lattice frame (9 doubles)
     S.o_ob = (int)w; w += 8 * (size_t)S.N;      // one-body cache: J1, grad J1, lap J1, v_ei, v^a_ei per electron
+    S.o_j3 = (int)w; if (S.n_j3) w += (size_t)S.N * 2 * LRDMC_J3_MAX + LRDMC_J3_MAX;   // three-body Jastrow: chi3, V3, S3
     S.per_warp_doubles = (int)w;
     const size_t per_sm = prop.sharedMemPerMultiprocessor, per_blk_max = prop.sharedMemPerBlockOptin, reserve = 1024;
     c->wpb = LRDMC_WPB;
@@ -250,8 +258,8 @@ extern "C" int lrdmc_init(lrdmc_ctx **out, const lrdmc_system *sys, const lrdmc_
 #undef SET_ALL
 #undef SET_SMEM
     c->ts = S.bf_in_smem && S.moc_in_smem;
-    if (S.nl_K) lrdmc_k_set_smem_nl(c->smem_bytes); else lrdmc_k_set_smem_lat(c->smem_bytes);
-    const int occ = S.nl_K ? lrdmc_k_occupancy_nl(c->NT, c->ts, c->wpb * 32, c->smem_bytes) : lrdmc_k_occupancy_lat(c->NT, c->ts, c->wpb * 32, c->smem_bytes);
+    if (S.nl_K || S.n_j3) lrdmc_k_set_smem_nl(c->smem_bytes); else lrdmc_k_set_smem_lat(c->smem_bytes);
+    const int occ = (S.nl_K || S.n_j3) ? lrdmc_k_occupancy_nl(c->NT, c->ts, c->wpb * 32, c->smem_bytes) : lrdmc_k_occupancy_lat(c->NT, c->ts, c->wpb * 32, c->smem_bytes);
     c->ctas_per_sm = occ > 0 ? occ : 1;
     c->grid_max = c->sm_count * c->ctas_per_sm;
     if (cudaGetLastError() != cudaSuccess) { /* attribute errors surface at launch */ }
@@ -332,6 +340,7 @@ static void plan_team(lrdmc_ctx *c, int n_w)
 {
     const DevSys &S = c->S; TeamPlan &P = c->team;
     c->team_tw = 1;
+    if (S.n_j3) return;                                  // systems with a three-body Jastrow run the warp-per-walker kernel
     int tw = 1;
     const long slots = (long)c->grid_max * c->wpb;
     if (!c->ts) tw = 4;
@@ -366,7 +375,7 @@ static void plan_team(lrdmc_ctx *c, int n_w)
     P.o_nl = (int)scr_lat; P.o_nu = (int)(scr_lat + scr_nl);
     P.o_scr = S.per_warp_doubles; P.scr_doubles = (int)align_up(scr_col > scr_mo ? scr_col : scr_mo, 2);
     const int smem = (int)(((size_t)S.tables_doubles + S.per_warp_doubles + P.scr_doubles) * 8);
-    const int occ = S.nl_K ? lrdmc_k_team_occupancy_nl(c->NT, c->ts, tw * 32, smem) : lrdmc_k_team_occupancy_lat(c->NT, c->ts, tw * 32, smem);
+    const int occ = (S.nl_K || S.n_j3) ? lrdmc_k_team_occupancy_nl(c->NT, c->ts, tw * 32, smem) : lrdmc_k_team_occupancy_lat(c->NT, c->ts, tw * 32, smem);
     if (cudaGetLastError() != cudaSuccess || occ < 1) return;             // does not fit: stay with warp-per-walker
     c->team_tw = tw; c->team_smem = smem; c->team_ctas_per_sm = occ; c->team_grid_max = c->sm_count * occ;
 }
@@ -488,10 +497,10 @@ extern "C" int lrdmc_propagate(lrdmc_ctx *c, int mode, int n_moves, double tau, 
     if (!team) propagate_shape(c, &grid, &warps);
     CK(cudaEventRecord(c->ev[0], st));
     if (team) {
-        if (c->S.nl_K) lrdmc_k_team_nl(c->NT, c->ts, grid, c->team_tw * 32, c->team_smem, st, c->S, c->W, c->team, mode, n_moves, tau, E0, (uint32_t)cycle);
+        if (c->S.nl_K || c->S.n_j3) lrdmc_k_team_nl(c->NT, c->ts, grid, c->team_tw * 32, c->team_smem, st, c->S, c->W, c->team, mode, n_moves, tau, E0, (uint32_t)cycle);
         else lrdmc_k_team_lat(c->NT, c->ts, grid, c->team_tw * 32, c->team_smem, st, c->S, c->W, c->team, mode, n_moves, tau, E0, (uint32_t)cycle);
     } else {
-        if (c->S.nl_K) lrdmc_k_propagate_nl(c->NT, c->ts, grid, warps * 32, c->smem_bytes, st, c->S, c->W, mode, n_moves, tau, E0, (uint32_t)cycle);
+        if (c->S.nl_K || c->S.n_j3) lrdmc_k_propagate_nl(c->NT, c->ts, grid, warps * 32, c->smem_bytes, st, c->S, c->W, mode, n_moves, tau, E0, (uint32_t)cycle);
         else lrdmc_k_propagate_lat(c->NT, c->ts, grid, warps * 32, c->smem_bytes, st, c->S, c->W, mode, n_moves, tau, E0, (uint32_t)cycle);
     }
     ++c->launches;
@@ -554,7 +563,7 @@ extern "C" int lrdmc_step_debug(lrdmc_ctx *c, double E0, uint64_t cycle, uint64_
     if (!c || !R_dev || !scal_dev || !jstar_dev || cycle > 0xFFFFFFFFull || step > 0xFFFFFFFFull) return LRDMC_EINVAL;
     if (!c->bound || !c->state_ok) return LRDMC_ESTATE;
     cudaStream_t st = (cudaStream_t)stream;
-    if (c->S.nl_K) lrdmc_k_step_debug_nl(c->NT, c->ts, grid_for(c), c->wpb * 32, c->smem_bytes, st, c->S, c->W, E0, (uint32_t)cycle, (uint32_t)step, R_dev, scal_dev, jstar_dev);
+    if (c->S.nl_K || c->S.n_j3) lrdmc_k_step_debug_nl(c->NT, c->ts, grid_for(c), c->wpb * 32, c->smem_bytes, st, c->S, c->W, E0, (uint32_t)cycle, (uint32_t)step, R_dev, scal_dev, jstar_dev);
     else lrdmc_k_step_debug_lat(c->NT, c->ts, grid_for(c), c->wpb * 32, c->smem_bytes, st, c->S, c->W, E0, (uint32_t)cycle, (uint32_t)step, R_dev, scal_dev, jstar_dev);
     ++c->launches;
     CK(cudaGetLastError());

@@ -43,7 +43,7 @@ __device__ __forceinline__ WarpState warp_views(const DevSys &S, double *smem, i
     double *base = smem + S.tables_doubles + (size_t)warp * S.per_warp_doubles;
     WarpState ws;
     ws.r = base + S.o_r; ws.dinv[0] = base + S.o_dinv[0]; ws.dinv[1] = base + S.o_dinv[1];
-    ws.moc = base + S.o_moc; ws.R = base + S.o_R; ws.cum = base + S.o_cum; ws.el = base + S.o_el; ws.ob = base + S.o_ob; ws.U = base + S.o_U;
+    ws.moc = base + S.o_moc; ws.R = base + S.o_R; ws.cum = base + S.o_cum; ws.el = base + S.o_el; ws.ob = base + S.o_ob; ws.U = base + S.o_U; ws.j3 = base + S.o_j3;
     return ws;
 }
 
@@ -71,6 +71,7 @@ __device__ __forceinline__ void load_walker(const DevSys &S, const DevWalk &W, W
     if (TS) { for (int i = lane; i < (int)mocn; i += 32) ws.moc[i] = W.moc[(size_t)k * mocn + i]; }
     else ws.moc = W.moc + (size_t)k * mocn;
     __syncwarp();
+    if (with_onebody && S.n_j3) for (int i = 0; i < N; ++i) refresh_j3_row(S, nuc, ws.j3 + i * LRDMC_J3_MAX, ws.r[3 * i], ws.r[3 * i + 1], ws.r[3 * i + 2], lane);
     if (with_onebody) for (int i = 0; i < N; ++i) refresh_onebody(S.n_nuc, S.has_j1, S.a, nuc, ws.ob + 8 * i, ws.r[3 * i], ws.r[3 * i + 1], ws.r[3 * i + 2], lane);
     __syncwarp();
 }

@@ -59,6 +59,11 @@ SYSTEMS = {
     # lrdmc_init folds the contraction into its primitive coefficient tables)
     "contracted-3u2d-sph-pp": lambda: _with_walkers(wl.contracted_molecule(3, 2, 3, 9, seed=31, spherical=True, with_pp=True), 37),
     "contracted-9u7d-cart": lambda: _with_walkers(wl.contracted_molecule(9, 7, 4, 21, seed=32, spherical=False), 21),
+    # scope row f2: three-body Jastrow (s Gaussians at the nuclei), alone, with non-local slots in the full-ratio form, on C3
+    "tiny-3u2d-pp-J3": lambda: _with_walkers(wl.with_jastrow3(wl.tiny_molecule(3, 2, 3, 9, seed=21, with_pp=True), 4, 2), 37),
+    "tiny-3u2d-J3-nlTM": lambda: _with_walkers(wl.with_jastrow3(wl.random_nonlocal(wl.tiny_molecule(3, 2, 3, 9, seed=21, with_pp=True), 5, 1.6, 2, False, scale=200.0), 4, 2), 37),
+    "ragged-9u4d-J3": lambda: _with_walkers(wl.with_jastrow3(wl.tiny_molecule(9, 4, 4, 20, seed=11), 6, 2, strength=0.1), 13),
+    "C3-water-methane-J3": lambda: _with_walkers(wl.with_jastrow3(wl.water_methane(n_walkers=100), 7, 1, strength=0.05), 100),
     "contracted-4u4d-sph-nlDLA": lambda: _with_walkers(wl.random_nonlocal(wl.contracted_molecule(4, 4, 3, 12, seed=33, spherical=True, with_pp=True), 9, 1.5, 2, True, scale=100.0), 29),
 }
 
