@@ -83,7 +83,7 @@ typedef struct {
     const double *c1, *b1;    /* [n_nuc] one-body Pade u1_I = -c1_I r/(1+b1_I r); c1 == NULL disables */
     /* Three-body (electron-electron-nucleus) Jastrow ("2+3-body Jastrow"; form = reading Q23):
      *   J3 = sum_{i<j} sum_{a,b} g_ab chi_a(r_i) chi_b(r_j),  chi_a(r) = exp(-zeta_a |r - R_{center_a}|^2),  g symmetric.
-     * n_j3 = 0 disables; at most 8 functions.  Systems with a J3 run the warp-per-walker kernel. */
+     * n_j3 = 0 disables; at most 8 functions. */
     int n_j3;
     const int *j3_center;     /* [n_j3] nucleus index */
     const double *j3_zeta;    /* [n_j3] > 0 */

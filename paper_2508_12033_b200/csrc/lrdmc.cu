@@ -340,7 +340,6 @@ static void plan_team(lrdmc_ctx *c, int n_w)
 {
     const DevSys &S = c->S; TeamPlan &P = c->team;
     c->team_tw = 1;
-    if (S.n_j3) return;                                  // systems with a three-body Jastrow run the warp-per-walker kernel
     int tw = 1;
     const long slots = (long)c->grid_max * c->wpb;
     if (!c->ts) tw = 4;

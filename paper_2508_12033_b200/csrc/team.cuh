@@ -23,7 +23,10 @@ __device__ __forceinline__ void load_walker_team(const DevSys &S, const DevWalk 
     if (S.moc_in_smem) { for (int i = tid; i < (int)mocn; i += nthr) ws.moc[i] = W.moc[(size_t)k * mocn + i]; }
     else ws.moc = W.moc + (size_t)k * mocn;
     __syncthreads();
-    for (int i = wt; i < N; i += TW) refresh_onebody(S.n_nuc, S.has_j1, S.a, nuc, ws.ob + 8 * i, ws.r[3 * i], ws.r[3 * i + 1], ws.r[3 * i + 2], lane);
+    for (int i = wt; i < N; i += TW) {
+        refresh_onebody(S.n_nuc, S.has_j1, S.a, nuc, ws.ob + 8 * i, ws.r[3 * i], ws.r[3 * i + 1], ws.r[3 * i + 2], lane);
+        if (S.n_j3) refresh_j3_row(S, nuc, ws.j3 + i * LRDMC_J3_MAX, ws.r[3 * i], ws.r[3 * i + 1], ws.r[3 * i + 2], lane);
+    }
     __syncthreads();
 }
 
@@ -53,6 +56,19 @@ __device__ __forceinline__ EvalOut evaluate_team(const DevSys &S, const TeamPlan
     const int t = lane & 3, g = lane >> 2;
     double *Jold = ws.el, *lap_s = ws.el + N;
 
+    if (NL && S.n_j3) {                // three-body fields V_a(i) = sum_b g_ab (S_b - chi_b(r_i)),  S_b = sum_j chi_b(r_j)   (evaluate.cuh)
+        double *chi3 = ws.j3, *V3 = ws.j3 + N * LRDMC_J3_MAX, *S3 = V3 + N * LRDMC_J3_MAX;
+        if (tid < LRDMC_J3_MAX) { double sb = 0.0; for (int j = 0; j < N; ++j) sb += chi3[j * LRDMC_J3_MAX + tid]; S3[tid] = sb; }
+        __syncthreads();
+        for (int idx = tid; idx < N * LRDMC_J3_MAX; idx += nthr) {
+            const int i = idx / LRDMC_J3_MAX, a = idx - i * LRDMC_J3_MAX;
+            double v = 0.0;
+#pragma unroll
+            for (int b = 0; b < LRDMC_J3_MAX; ++b) v += S.j3_g[a * LRDMC_J3_MAX + b] * (S3[b] - chi3[i * LRDMC_J3_MAX + b]);
+            V3[idx] = v;
+        }
+        __syncthreads();
+    }
     // ---- phase A (row a6): per-electron continuum pieces; P.lpe lanes of one warp per electron split the partners and the MOs
     {
         const int LPE = P.lpe, epp = nthr / LPE;
@@ -86,6 +102,15 @@ __device__ __forceinline__ EvalOut evaluate_team(const DevSys &S, const TeamPlan
             if (act && sub == 0) {
                 const double *ob = ws.ob + 8 * ii;
                 gx += ob[1]; gy += ob[2]; gz += ob[3];
+                if (NL && S.n_j3) {    // J3 terms of electron i (as in evaluate_walker)
+                    const double *chi3 = ws.j3 + ii * LRDMC_J3_MAX, *V3 = ws.j3 + (N + ii) * LRDMC_J3_MAX;
+                    for (int a = 0; a < S.n_j3; ++a) {
+                        const double *nu = T.nuc + S.j3_center[a] * LRDMC_NUC_STRIDE, z = S.j3_zeta[a];
+                        const double dx = xi - nu[0], dy = yi - nu[1], dz = zi - nu[2], cv = chi3[a] * V3[a], tz = -2.0 * z * cv;
+                        J += cv; gx += tz * dx; gy += tz * dy; gz += tz * dz;
+                        lJ += (4.0 * z * z * (dx * dx + dy * dy + dz * dz) - 6.0 * z) * cv;
+                    }
+                }
                 Jold[ii] = J + ob[0];
                 lap_s[ii] = Ld + 2.0 * (Gx * gx + Gy * gy + Gz * gz) + (lJ + ob[4]) + (gx * gx + gy * gy + gz * gz);
             }
@@ -166,6 +191,23 @@ __device__ __forceinline__ EvalOut evaluate_team(const DevSys &S, const TeamPlan
             for (int j = t + 4 * part; j < N; j += 4 * NP) {
                 const double c = (j == i) ? 0.0 : ((spin_of(S, j) == sp) ? S.a_par : S.a_anti);
                 pade_six(x0 - ws.r[3 * j], y0 - ws.r[3 * j + 1], z0 - ws.r[3 * j + 2], av, a2, c, S.b2, Jn);
+            }
+        }
+        if (NL && S.n_j3 && (!is_nl || !S.nl_dla)) {                 // three-body Jastrow: the functions are dealt over (part, quad lane)
+            const double *V3 = ws.j3 + (N + i) * LRDMC_J3_MAX;
+            for (int a0 = 4 * part; a0 < S.n_j3; a0 += 4 * NP) {     // (trip count uniform in the warp: exp_tab_n synchronises it)
+                const bool on = a0 + t < S.n_j3; const int a = on ? a0 + t : 0;
+                const double *np_ = T.nuc + S.j3_center[a] * LRDMC_NUC_STRIDE, z = S.j3_zeta[a];
+                const double dx = x0 - np_[0], dy = y0 - np_[1], dz = z0 - np_[2], q0 = fma(dx, dx, fma(dy, dy, fma(dz, dz, a2)));
+                double ex_[6], e_[6];
+#pragma unroll
+                for (int k = 0; k < 3; ++k) {
+                    const double sk = fma(av[k][0], dx, fma(av[k][1], dy, av[k][2] * dz));
+                    ex_[2 * k] = exp_arg_floor(-z * fma(2.0, sk, q0)); ex_[2 * k + 1] = exp_arg_floor(-z * fma(-2.0, sk, q0));
+                }
+                exp_tab_n<6>(ex_, e_, T.etab);
+#pragma unroll
+                for (int d = 0; d < 6; ++d) Jn[d] = fma(e_[d], on ? V3[a] : 0.0, Jn[d]);
             }
         }
         double nuq[6];
@@ -257,7 +299,7 @@ __device__ __forceinline__ void apply_move_team(const DevSys &S, const TeamPlan 
             for (int nt = 0; nt < NT; ++nt) { q[8 * nt + 2 * t] = acc[nt][0]; q[8 * nt + 2 * t + 1] = acc[nt][1]; }
         }
     }
-    if (wt == 0) refresh_onebody(S.n_nuc, S.has_j1, S.a, T.nuc, ws.ob + 8 * i, px, py, pz, lane);
+    if (wt == 0) { refresh_onebody(S.n_nuc, S.has_j1, S.a, T.nuc, ws.ob + 8 * i, px, py, pz, lane); if (NL && S.n_j3) refresh_j3_row(S, T.nuc, ws.j3 + i * LRDMC_J3_MAX, px, py, pz, lane); }
     __syncthreads();                                   // every thread has read the old position
     for (int idx = tid; idx < rows; idx += nthr) {
         double s = 0.0;

@@ -156,7 +156,8 @@ def test_whole_cycle_trajectories_weights_and_branching(B, name, mode, kernel, m
                                        ("ragged-17u3d-NT4", "conventional"), ("he-triplet-slater", "balanced"), ("C3-water-methane-shaped", "balanced"),
                                        ("C3-water-methane-shaped", "conventional"), ("C5-cluster64-doublemesh", "balanced"),
                                        ("tiny-3u2d-nlDLA-strong", "balanced"), ("tiny-2u1d-nlTM-strong", "conventional"), ("C3-water-methane-nlDLA", "balanced"),
-                                       ("C3-water-methane-nlTM", "balanced"), ("contracted-4u4d-sph-nlDLA", "balanced"), ("tiny-2u2d-doublemesh-nlTM", "conventional")])
+                                       ("C3-water-methane-nlTM", "balanced"), ("contracted-4u4d-sph-nlDLA", "balanced"), ("tiny-2u2d-doublemesh-nlTM", "conventional"),
+                                       ("tiny-3u2d-pp-J3", "balanced"), ("tiny-3u2d-J3-nlTM", "conventional"), ("C3-water-methane-J3", "balanced")])
 def test_team_kernel_every_team_size(B, name, mode, tw, monkeypatch):
     """k_propagate_team with TW = 2, 4, 8, 16 warps per walker (work units = electron blocks x shell parts, partial sums
     in shared memory): same trajectories, weights and indices as the oracle."""
