@@ -444,6 +444,29 @@ def test_balanced_equals_conventional_with_nonlocal_slots(B, dla):
     g.close()
 
 
+def test_helium_with_three_body_jastrow_still_reaches_the_exact_energy(B):
+    """Row f2 in whole runs: the nodeless He ground-state energy does not depend on the Jastrow factor, so with a three-body term
+    switched on E(a -> 0) must still be the textbook -2.903724 Ha, and the two modes must agree at fixed a (L234)."""
+    from paper_2508_12033_b200 import driver as drv
+    rng = np.random.default_rng(0); a = [0.15, 0.25, 0.35]; E = []; sg = []
+
+    def he(ai):
+        s = dict(wl.slater_atom(2.0, [1.85], 1, 1, np.ones((1, 1)), np.ones((1, 1)), ai, jastrow=dict(a_anti=0.5, a_par=0.25, b2=0.5)))
+        s.update(j3_center=np.array([0, 0], dtype=np.int32), j3_zeta=np.array([0.8, 2.0]), j3_g=np.array([[0.05, -0.03], [-0.03, 0.06]]), name="he-J3")
+        return s
+    for ai in a:
+        g = B.Lrdmc(he(ai)); g.lrdmc_set_positions(rng.normal(size=(4096, 2, 3)) * 0.7)
+        recs = drv.run(g, B.BALANCED, 300, n_moves=int(round(20 * (0.2 / ai) ** 2)), E0=-2.9)
+        e, sd = B.lrdmc_energy(recs, p=10, n_therm=60, n_blocks=10); E.append(e); sg.append(sd)
+        if ai == 0.25:
+            rc = drv.run(g, B.CONVENTIONAL, 300, tau=int(round(20 * (0.2 / ai) ** 2)) * ai**2 / 6, E0=-2.9, first_cycle=1000)
+            Ec, sc = B.lrdmc_energy(rc, p=10, n_therm=60, n_blocks=10)
+            assert abs(e - Ec) < 3 * np.hypot(sd, sc), (e, sd, Ec, sc)
+        g.close()
+    E0, s0, *_ = drv.fit_a_to_zero(a, E, sg)
+    assert abs(E0 + 2.903724) < 3 * s0 + 3e-4 and s0 < 3e-3, (E0, s0)
+
+
 # ------------------------------------------------------------------------------------------ edge cases and error behaviour
 def test_edge_cases_and_errors(B):
     s = wl.tiny_molecule(2, 1, 2, 6, seed=7); g = B.Lrdmc(s)
