@@ -140,3 +140,25 @@ def test_reference_arm_prints_one_json_line():
     line = json.loads(out.stdout.strip().splitlines()[-1])
     assert line["impl"] == "reference" and line["unit"] == "walker-moves/s" and line["value"] > 0 and line["cpu_baseline"]["kind"] == "oracle"
     assert line["e2e"]["h2d_bytes_per_step"] == 0 and line["higher_is_better"] is True
+
+
+def test_ctypes_structures_match_the_c_header(tmp_path):
+    """The binding's ctypes mirrors of lrdmc_system / lrdmc_basis / lrdmc_mo / lrdmc_jastrow / lrdmc_lattice / lrdmc_cycle_stats have
+    the sizes and field offsets gcc gives the structs of include/lrdmc.h (guards the f1 / f2 extensions of the problem statement)."""
+    import subprocess
+    names = {"lrdmc_system": B.System, "lrdmc_basis": B.Basis, "lrdmc_mo": B.Mo, "lrdmc_jastrow": B.Jastrow, "lrdmc_lattice": B.Lattice,
+             "lrdmc_cycle_stats": B.CycleStats}
+    lines = ['#include <stdio.h>', '#include <stddef.h>', '#include "lrdmc.h"', 'int main(void) {']
+    for cname, cls in names.items():
+        lines.append(f'printf("{cname} %zu\\n", sizeof({cname}));')
+        for fname, _ in cls._fields_:
+            lines.append(f'printf("{cname}.{fname} %zu\\n", offsetof({cname}, {fname}));')
+    lines += ['return 0; }']
+    src = tmp_path / "layout.c"; exe = tmp_path / "layout"
+    src.write_text("\n".join(lines))
+    subprocess.run(["gcc", "-I", os.path.join(ROOT, "include"), "-o", str(exe), str(src)], check=True)
+    out = dict(l.split() for l in subprocess.run([str(exe)], capture_output=True, text=True, check=True).stdout.splitlines())
+    for cname, cls in names.items():
+        assert int(out[cname]) == C.sizeof(cls), cname
+        for fname, _ in cls._fields_:
+            assert int(out[f"{cname}.{fname}"]) == getattr(cls, fname).offset, (cname, fname)
