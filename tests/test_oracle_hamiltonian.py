@@ -211,3 +211,66 @@ def test_local_pseudopotential_limits():
     x = (R0 + np.array([0.05, 0, 0]))[None, :]
     _, _, per, _ = o2.evaluate(x, np.eye(3))
     assert abs(per[0, 2] + Z / 0.05) < 1e-10 and abs(per[0, 4] + Z / 0.2) < 1e-12     # D10: -Z/max(r,a)
+
+
+def test_local_pseudopotential_mid_range_formula():
+    """The local-PP branch of v_ei at mid-range radii against the formula of include/lrdmc.h (lrdmc_system.pp, reading Q14)
+    written out here: v(r) = -(Z/r)(1 - e^{-alpha r^2}) + Z alpha r e^{-beta r^2} + gamma e^{-delta r^2}.  At r = 0.3 / 0.7 / 1.5 the
+    middle term is of order one: a wrong sign on it, a beta <-> delta swap or an alpha <-> beta swap fails this pin (each is
+    shown to change the value by far more than the tolerance), while the r -> 0 and r -> infinity limits would not notice."""
+    for seed in (3, 4):
+        s = wl.tiny_molecule(1, 0, 1, 1, seed=seed, with_pp=True); o = ref.Ref(s)
+        Z = float(s["Z"][0]); al, be, ga, de = (float(v) for v in s["pp"][0]); R0 = s["R"][0]
+        for r in (0.3, 0.7, 1.5):
+            want = -(Z / r) * (-math.expm1(-al * r * r)) + Z * al * r * math.exp(-be * r * r) + ga * math.exp(-de * r * r)
+            for direction in (np.array([1.0, 0, 0]), np.array([0.6, 0.0, -0.8])):
+                _, _, per, _ = o.evaluate((R0 + r * direction)[None, :], np.eye(3))
+                assert abs(per[0, 2] - want) < 1e-13 * max(1.0, abs(want)), (seed, r)
+                assert abs(per[0, 4] + Z / r) < 1e-13 * Z / r                     # L623: the bound of an ECP nucleus has no cutoff
+            # the pin has teeth: the plausible mistakes move the value well beyond the tolerance at these radii
+            wrong_sign = -(Z / r) * (-math.expm1(-al * r * r)) - Z * al * r * math.exp(-be * r * r) + ga * math.exp(-de * r * r)
+            swap_bd = -(Z / r) * (-math.expm1(-al * r * r)) + Z * al * r * math.exp(-de * r * r) + ga * math.exp(-be * r * r)
+            if r < 1.0:
+                assert abs(wrong_sign - want) > 1e-6 and abs(swap_bd - want) > 1e-9
+    # two PP nuclei: v_ei is the plain sum over nuclei of the same formula
+    s = wl.tiny_molecule(2, 1, 2, 6, seed=8, with_pp=True); o = ref.Ref(s)
+    x = wl.initial_walkers(s, 1, 3)[0]
+    _, _, per, _ = o.evaluate(x, np.eye(3))
+    for i in range(3):
+        want = 0.0
+        for I in range(2):
+            r = float(np.linalg.norm(x[i] - s["R"][I])); Z = float(s["Z"][I]); al, be, ga, de = (float(v) for v in s["pp"][I])
+            want += -(Z / r) * (-math.expm1(-al * r * r)) + Z * al * r * math.exp(-be * r * r) + ga * math.exp(-de * r * r)
+        assert abs(per[i, 2] - want) < 1e-12 * max(1.0, abs(want))
+
+
+def test_double_mesh_selection_weights_and_sums():
+    """Double mesh (reading Q13, g = 1/2): the heat-bath selection draws candidate j with probability kappa_j max(R_j, 0) / bbar,
+    kappa = (1/2)/(2 a^2) for the first 6N candidates (spacing a) and (1/2)/(2 a'^2) for the second 6N (spacing a').  Frequencies
+    over a 20 000-point u grid against those weights written out here; a kappa that ignored the mesh (or swapped a and a') is
+    shown to differ by far more than the grid resolution.  Also bbar, V_sf, K_diag and T_i re-assembled from R with the same kappas."""
+    s = wl.tiny_molecule(2, 2, 2, 7, seed=9, a=0.15, a2=0.3); o = ref.Ref(s); N = 4
+    rng = np.random.default_rng(17)
+    x = wl.initial_walkers(s, 1, 21)[0]; U = _rand_frame(rng)
+    R, sc, per, _ = o.evaluate(x, U)
+    assert len(R) == 12 * N
+    kap = np.concatenate([np.full(6 * N, 0.5 / (2 * 0.15**2)), np.full(6 * N, 0.5 / (2 * 0.3**2))])
+    q = kap * np.maximum(R, 0.0)
+    assert q[:6 * N].sum() > 0 and q[6 * N:].sum() > 0
+    assert abs(sc["bbar"] - q.sum()) < 1e-12 * q.sum()
+    assert abs(sc["V_sf"] - (kap * np.maximum(-R, 0.0)).sum()) < 1e-12 * max(1.0, sc["V_sf"])
+    assert abs(sc["K_diag"] - kap.sum()) < 1e-12 * kap.sum()
+    for i in range(N):          # T_i = g T_i(a) + (1-g) T_i(a'), T_i(a) = (sum_d R - 6)/a^2
+        T = 0.5 * (R[6 * i:6 * i + 6].sum() - 6) / 0.15**2 + 0.5 * (R[6 * N + 6 * i:6 * N + 6 * i + 6].sum() - 6) / 0.3**2
+        assert abs(per[i, 0] - T) < 1e-10 * max(1.0, abs(T))
+    M = 20000; counts = np.zeros(len(R))
+    for k in range(M):
+        j, _ = o.select(R, (k + 0.5) / M); counts[j] += 1
+    p = q / q.sum()
+    assert np.all(counts[R <= 0] == 0)
+    assert np.abs(counts / M - p).max() < 1.5 / M
+    p_flat = np.maximum(R, 0.0) / np.maximum(R, 0.0).sum()           # the mistakes this pin must catch
+    p_swap = kap[::-1] * np.maximum(R, 0.0); p_swap /= p_swap.sum()
+    assert np.abs(p_flat - p).max() > 20 / M and np.abs(p_swap - p).max() > 20 / M
+    # share of the coarse mesh among the selected moves = its share of bbar
+    assert abs(counts[6 * N:].sum() / M - q[6 * N:].sum() / q.sum()) < 12 * N * 1.5 / M
