@@ -107,6 +107,44 @@ def run_reference(args, rank, world):
     print(json.dumps(line), flush=True)
 
 
+def make_workload(args, rank, seed_shift=0):
+    seed = wl.PHILOX_RUN_SEED + rank + 1000 * seed_shift
+    if args.workload == "C4":
+        sysd = wl.water_methane(n_walkers=args.nw, moves=args.moves, seed=seed, name="C4-water-methane-shaped")
+        wname = "C4 water-methane-shaped: 16 e (8/8), 8 nuclei, 200 s/p/d GTOs, local PP, 1b+2b Jastrow, a=0.2 (BASELINE.json configs[3]; with --nw 100/400: configs[2])"
+    elif args.workload == "C1":
+        sysd = wl.hydrogen(n_walkers=args.nw, moves=args.moves, seed=seed)
+        wname = "C1 hydrogen atom: 1 e, psi = exp(-0.9 r), a=0.2 (BASELINE.json configs[0])"
+    elif args.workload == "C2":
+        sysd = wl.synthetic10(n_walkers=args.nw, moves=args.moves, seed=seed)
+        wname = "C2 synthetic 10-electron molecule: 5/5, 3 nuclei, 60 s/p/d GTOs, 1b+2b Jastrow, a=0.2 (BASELINE.json configs[1])"
+    elif args.workload == "C3j3":
+        sysd = wl.with_jastrow3(wl.water_methane(n_walkers=args.nw, moves=args.moves, seed=seed), 7, 1, strength=0.05)
+        wname = "C3/C4 water-methane-shaped system + synthetic three-body Jastrow (8 s Gaussians at the nuclei): scope row f2; flop count = without the J3 part"
+    elif args.workload == "C3nl":
+        sysd = wl.water_methane_nonlocal(n_walkers=args.nw, moves=args.moves, seed=seed)
+        wname = "C3/C4 water-methane-shaped system + synthetic non-local s/p/d pseudopotential channels (r_c = 0.8 bohr, DLA): scope row f1; flop count = lattice part only"
+    else:
+        sysd = wl.cluster64(n_walkers=args.nw, moves=args.moves, seed=seed)
+        wname = "C5 64-electron cluster: 32/32, 24 nuclei, 600 s/p/d GTOs, 1b+2b Jastrow, double mesh a=0.2/a'=0.4 (BASELINE.json configs[4])"
+    x0 = wl.hydrogen_walkers(args.nw, 1 + rank + 100 * seed_shift) if args.workload == "C1" else wl.initial_walkers(sysd, args.nw, 5 + rank + 100 * seed_shift)
+    return sysd, wname, x0
+
+
+def measured_traffic(workload, n_w, kernel):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the propagate kernel from an `ncu --set full` capture of THIS
+    workload (profiles/ncu_traffic_by_workload.md: one table row per captured workload); None if that workload was never captured."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "ncu_traffic_by_workload.md")) as f:
+            for ln in f:
+                c = [t.strip() for t in ln.strip().strip("|").split("|")]
+                if len(c) >= 5 and c[0] == workload and c[1] == str(n_w) and c[2] == kernel:
+                    return float(c[3])
+    except Exception:
+        pass
+    return None
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1); ap.add_argument("--steps", type=int, default=10); ap.add_argument("--warmup", type=int, default=3)
@@ -115,6 +153,10 @@ def main():
     ap.add_argument("--no-conventional", action="store_true"); ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--workload", default="C4", choices=["C1", "C2", "C4", "C5", "C3nl", "C3j3"],
                     help="C4 (default) is the configuration the metric is quoted on; C2 / C5 are the other BASELINE.json systems, C3nl adds non-local pseudopotential channels (use with --nw/--moves)")
+    ap.add_argument("--contexts", type=int, default=1,
+                    help="K independent ensembles of --nw walkers each (own context, own CUDA stream, own seed) in flight together: the paper's "
+                         "small-ensemble regime (100 walkers per GPU, L289) and the several-a batch of SURVEY 8(f) f3; value = aggregate over the K")
+    ap.add_argument("--team", type=int, default=0, help="lrdmc_set_option(LRDMC_OPT_TEAM_WARPS): 0 = automatic")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1")); local = int(os.environ.get("LOCAL_RANK", "0"))
     if args.impl == "reference":
@@ -131,56 +173,59 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
     dev = f"cuda:{local}"; torch.cuda.set_device(dev)
 
-    if args.workload == "C4":
-        sysd = wl.water_methane(n_walkers=args.nw, moves=args.moves, seed=wl.PHILOX_RUN_SEED + rank, name="C4-water-methane-shaped")
-        wname = "C4 water-methane-shaped: 16 e (8/8), 8 nuclei, 200 s/p/d GTOs, local PP, 1b+2b Jastrow, a=0.2 (BASELINE.json configs[3])"
-    elif args.workload == "C1":
-        sysd = wl.hydrogen(n_walkers=args.nw, moves=args.moves, seed=wl.PHILOX_RUN_SEED + rank)
-        wname = "C1 hydrogen atom: 1 e, psi = exp(-0.9 r), a=0.2 (BASELINE.json configs[0])"
-    elif args.workload == "C2":
-        sysd = wl.synthetic10(n_walkers=args.nw, moves=args.moves, seed=wl.PHILOX_RUN_SEED + rank)
-        wname = "C2 synthetic 10-electron molecule: 5/5, 3 nuclei, 60 s/p/d GTOs, 1b+2b Jastrow, a=0.2 (BASELINE.json configs[1])"
-    elif args.workload == "C3j3":
-        sysd = wl.with_jastrow3(wl.water_methane(n_walkers=args.nw, moves=args.moves, seed=wl.PHILOX_RUN_SEED + rank), 7, 1, strength=0.05)
-        wname = "C3/C4 water-methane-shaped system + synthetic three-body Jastrow (8 s Gaussians at the nuclei): scope row f2; flop count = without the J3 part"
-    elif args.workload == "C3nl":
-        sysd = wl.water_methane_nonlocal(n_walkers=args.nw, moves=args.moves, seed=wl.PHILOX_RUN_SEED + rank)
-        wname = "C3/C4 water-methane-shaped system + synthetic non-local s/p/d pseudopotential channels (r_c = 0.8 bohr, DLA): scope row f1; flop count = lattice part only"
-    else:
-        sysd = wl.cluster64(n_walkers=args.nw, moves=args.moves, seed=wl.PHILOX_RUN_SEED + rank)
-        wname = "C5 64-electron cluster: 32/32, 24 nuclei, 600 s/p/d GTOs, 1b+2b Jastrow, double mesh a=0.2/a'=0.4 (BASELINE.json configs[4])"
-    x0 = wl.hydrogen_walkers(args.nw, 1 + rank) if args.workload == "C1" else wl.initial_walkers(sysd, args.nw, 5 + rank)
-    g = B.Lrdmc(sysd, device=dev)
-    g.lrdmc_set_positions(x0, allow_singular=True)
-    E0 = 0.0          # fixed Green's-function energy for the timing runs (W ~ 3N/a^2 = 1200 >> e_L; nonpos events are reported)
+    K = max(1, args.contexts)
+    ctxs = []
+    for q in range(K):
+        sysd, wname, x0 = make_workload(args, rank, q)
+        g = B.Lrdmc(sysd, device=dev, options={B.OPT_TEAM_WARPS: args.team} if args.team else None)
+        g.stream = torch.cuda.Stream(device=dev) if K > 1 else torch.cuda.current_stream(dev)
+        with torch.cuda.stream(g.stream):
+            g.lrdmc_set_positions(x0, allow_singular=True)
+        ctxs.append((g, sysd, x0))
+    g, sysd, x0 = ctxs[0]
     N = sysd["n_up"] + sysd["n_dn"]
     tau = args.moves * sysd["a"] ** 2 / (3 * N)       # reading Q19 first guess; refined from a pilot below
+    E0 = [0.0] * K; esum = [0.0] * K; ecnt = [0] * K  # Green's-function energy per ensemble, fed back after each branching (L232)
 
     def barrier():
         if dist is not None:
             dist.barrier()
         torch.cuda.synchronize()
 
-    def timed(mode, steps, first_cycle, tau_):
-        """K steps bracketed by barrier+sync, CUDA events on the launching (current torch) stream."""
+    def timed(mode, steps, first_cycle, tau_, feedback=True):
+        """K steps bracketed by barrier+sync, CUDA events on the launching stream.  Per step: every ensemble's propagate + reconfigure
+        is enqueued on its own stream, then every ensemble's estimators are read (a step ends when all K results are on the host)."""
         barrier()
         e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
-        l0 = g.launch_count(); recs = []
-        e0.record()
-        for c in range(first_cycle, first_cycle + steps):
-            g.lrdmc_propagate(mode, args.moves if mode == B.BALANCED else 0, tau_, E0 if mode == B.BALANCED else 0.0, c)
-            g.lrdmc_reconfigure(c)
-            recs.append(g.lrdmc_estimators())
-        e1.record(); barrier()
-        return e0.elapsed_time(e1) * 1e-3, recs, g.launch_count() - l0
+        l0 = sum(c[0].launch_count() for c in ctxs); recs = [[] for _ in ctxs]
+        main_stream = torch.cuda.current_stream(dev)
+        e0.record(main_stream)
+        if K > 1:
+            for c in ctxs:
+                c[0].stream.wait_event(e0)
+        for cyc_ in range(first_cycle, first_cycle + steps):
+            for q, c in enumerate(ctxs):
+                with torch.cuda.stream(c[0].stream):
+                    c[0].lrdmc_propagate(mode, args.moves if mode == B.BALANCED else 0, tau_, E0[q] if mode == B.BALANCED else 0.0, cyc_)
+                    c[0].lrdmc_reconfigure(cyc_)
+            for q, c in enumerate(ctxs):
+                st = c[0].lrdmc_estimators(); recs[q].append(st)
+                if mode == B.BALANCED and feedback and st.den > 0:
+                    esum[q] += st.num / st.den; ecnt[q] += 1; E0[q] = esum[q] / ecnt[q]   # "Update E_0" (Alg.2 line 12 L418)
+        if K > 1:
+            for c in ctxs:
+                main_stream.wait_stream(c[0].stream)
+        e1.record(main_stream); barrier()
+        return e0.elapsed_time(e1) * 1e-3, recs, sum(c[0].launch_count() for c in ctxs) - l0
 
-    # ---- warm-up + pilot for tau (conventional mode with the same mean move count, L283-L285)
-    _, wrecs, _ = timed(B.BALANCED, args.warmup, 0, 0.0)
+    # ---- warm-up (it also seeds E_0) + timed balanced steps
+    timed(B.BALANCED, args.warmup, 0, 0.0)
     cyc = args.warmup
     with ClockSampler(local) as clk:
-        secs, recs, launches = timed(B.BALANCED, args.steps, cyc, 0.0)
+        secs, recs_all, launches = timed(B.BALANCED, args.steps, cyc, 0.0)
     cyc += args.steps
-    moves = sum(r.moves_sum for r in recs)
+    recs = recs_all[0]
+    moves = sum(r.moves_sum for rr in recs_all for r in rr)
     fmax = (lambda v: float(_allreduce(dist, torch, v, "max", dev))) if dist is not None else None
     fsum = (lambda v: float(_allreduce(dist, torch, v, "sum", dev))) if dist is not None else None
     value, tmax = aggregate_over_ranks(moves, secs, world, fmax, fsum)
@@ -188,57 +233,72 @@ def main():
     prop_ms = float(np.mean([r.propagate_ms for r in recs])); rec_ms = float(np.mean([r.reconfigure_ms for r in recs]))
     flop = drv.work_per_walker_move(sysd)
     peaks = B.lrdmc_measure_fp64_peaks()
-    achieved = flop["total"] * (moves / len(recs)) / (prop_ms * 1e-3) / 1e12
-    traffic = None
-    try:
-        with open(os.path.join(ROOT, "profiles", "ncu_propagate_traffic.txt")) as f:     # last ncu --set full capture (text)
-            for ln in f:
-                if ln.startswith("dram_bytes_per_launch"):
-                    traffic = float(ln.split()[1])
-    except Exception:
-        pass
-    roofline = {"bound": "alu", "kernel": "k_propagate", "achieved": achieved, "peak": peaks["dfma_tflops"], "unit": "TFLOP/s", "frac": achieved / peaks["dfma_tflops"],
-                "traffic": traffic, "peak_source": "measured live: lrdmc_measure_fp64_peaks (independent DFMA chains, all SMs)",
-                "dmma_peak": peaks["dmma_tflops"], "dfma_dmma_mixed": peaks["mixed_tflops"], "dfma_3reg_peak": peaks["dfma_3reg_tflops"], "dfma_with_2_alu_peak": peaks["dfma_alu_tflops"], "flop_per_walker_move": flop["total"],
+    cfg = g.launch_config()
+    per_launch_moves = sum(r.moves_sum for r in recs) / len(recs)
+    achieved = flop["total"] * per_launch_moves / (prop_ms * 1e-3) / 1e12
+    executed = flop["executed"] * per_launch_moves / (prop_ms * 1e-3) / 1e12
+    roofline = {"bound": "alu", "kernel": cfg["kernel"], "achieved": achieved, "peak": peaks["dfma_tflops"], "unit": "TFLOP/s", "frac": achieved / peaks["dfma_tflops"],
+                "traffic": measured_traffic(args.workload, args.nw, cfg["kernel"]),
+                "frac_note": "frac = ALGORITHMIC flop (SURVEY 8(d) count, every candidate through the MOs) / kernel time / peak: speed relative to the naive algorithm "
+                             "at peak, may exceed 1; frac_executed = flop the column-form kernel executes / kernel time / peak: FP64-pipe utilisation (compare ncu sm__pipe_fp64_cycles_active)",
+                "achieved_executed": executed, "frac_executed": executed / peaks["dfma_tflops"],
+                "flop_per_walker_move": flop["total"], "flop_executed_per_walker_move": flop["executed"],
+                "peak_source": "measured live: liblrdmc_probe lrdmc_measure_fp64_peaks (independent DFMA chains, all SMs)",
+                "dmma_peak": peaks["dmma_tflops"], "dfma_dmma_mixed": peaks["mixed_tflops"], "dfma_3reg_peak": peaks["dfma_3reg_tflops"], "dfma_with_2_alu_peak": peaks["dfma_alu_tflops"],
                 "kernel_ms": prop_ms, "kernel_share_of_step": prop_ms * len(recs) / (secs * 1e3),
                 "hbm_bytes_per_launch_algorithmic": 2 * drv.state_bytes_per_walker(sysd) * args.nw}
+    if K > 1:
+        roofline["note"] = f"{K} contexts in flight: kernel_ms is one launch of context 0 while the others run beside it; achieved/frac describe that launch, not the device"
 
+    evals = sum(r.moves_sum + args.nw for rr in recs_all for r in rr)
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tmax / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": wname,
-                       "n_walkers": args.nw, "moves_per_cycle": args.moves, "mode": "balanced", "parallelism": f"replicas x{world}",
-                       "l2": "inputs larger than L2: walker state %.0f MB per replica" % (drv.state_bytes_per_walker(sysd) * args.nw / 1e6),
-                       "launch": g.launch_config()},
+                       "n_walkers": args.nw, "contexts": K, "moves_per_cycle": args.moves, "mode": "balanced", "parallelism": f"replicas x{world}",
+                       "l2": "inputs larger than L2: walker state %.0f MB per replica" % (drv.state_bytes_per_walker(sysd) * args.nw * K / 1e6)
+                             if drv.state_bytes_per_walker(sysd) * args.nw * K > 126e6 else
+                             "walker state %.1f MB fits L2 (the path re-reads 2 x state per step from wherever it lives; HBM is not the bound)" % (drv.state_bytes_per_walker(sysd) * args.nw * K / 1e6),
+                       "launch": cfg},
             "roofline": roofline, "gpu_launches": launches, "reconfigure_ms": rec_ms,
+            "result_check": {"E0_feedback": True, "e_mean_last_step": float(np.mean([rr[-1].num / rr[-1].den for rr in recs_all])),
+                             "E0_last": float(np.mean(E0)), "n_nonpos_diag": int(sum(r.n_nonpos_diag for rr in recs_all for r in rr)),
+                             "n_nonfinite": int(sum(r.n_nonfinite for rr in recs_all for r in rr)),
+                             "node_flag_share_of_evaluations": float(sum(r.n_node_flag for rr in recs_all for r in rr)) / max(1, evals),
+                             "wbar_last_step": float(np.mean([rr[-1].wbar for rr in recs_all]))},
             "branch_idle": {"balanced_device": float(np.mean([r.barrier_idle_frac for r in recs])), "balanced_lockstep": float(np.mean([r.lockstep_idle_frac for r in recs]))}}
 
     # ---- conventional mode at equal N_w and equal mean move count
     if not args.no_conventional:
         _, pil, _ = timed(B.CONVENTIONAL, 1, cyc, tau); cyc += 1
-        mean_moves = pil[0].moves_sum / args.nw
+        mean_moves = pil[0][0].moves_sum / args.nw
         tau *= args.moves / max(1.0, mean_moves)
         timed(B.CONVENTIONAL, 1, cyc, tau); cyc += 1
-        csecs, crecs, _ = timed(B.CONVENTIONAL, args.steps, cyc, tau); cyc += args.steps
-        cmoves = sum(r.moves_sum for r in crecs)
+        csecs, crecs_all, _ = timed(B.CONVENTIONAL, args.steps, cyc, tau); cyc += args.steps
+        crecs = crecs_all[0]
+        cmoves = sum(r.moves_sum for rr in crecs_all for r in rr)
         cval, _ = aggregate_over_ranks(cmoves, csecs, world, fmax, fsum)
-        line["conventional"] = {"value": cval, "unit": UNIT, "tau": tau, "mean_moves_per_cycle": cmoves / len(crecs) / args.nw,
+        line["conventional"] = {"value": cval, "unit": UNIT, "tau": tau, "mean_moves_per_cycle": cmoves / len(crecs) / args.nw / K,
                                 "moves_max": int(max(r.moves_max for r in crecs)), "ms_per_step": 1e3 * csecs / args.steps,
-                                "balanced_over_conventional": value / cval}
+                                "balanced_over_conventional": value / cval, "n_nonfinite": int(sum(r.n_nonfinite for rr in crecs_all for r in rr))}
         line["branch_idle"]["conventional_device"] = float(np.mean([r.barrier_idle_frac for r in crecs]))
         line["branch_idle"]["conventional_lockstep"] = float(np.mean([r.lockstep_idle_frac for r in crecs]))
 
     # ---- end to end through the host-buffer C-ABI call (H2D of the positions, D2H of positions + stats inside the timed region)
     if not args.no_e2e:
-        xin = torch.from_numpy(x0).pin_memory()
-        g.lrdmc_run_host(xin, B.BALANCED, args.moves, 0.0, E0, cyc, 1); cyc += 1
+        xin = [torch.from_numpy(c[2]).pin_memory() for c in ctxs]
+        for q, c in enumerate(ctxs):
+            c[0].lrdmc_run_host(xin[q], B.BALANCED, args.moves, 0.0, E0[q], cyc, 1)
+        cyc += 1
         barrier(); t0 = time.perf_counter(); emoves = 0
-        for s in range(args.steps):
-            st, xout = g.lrdmc_run_host(xin, B.BALANCED, args.moves, 0.0, E0, cyc, 1); cyc += 1
-            emoves += st[0].moves_sum
+        for s_ in range(args.steps):
+            for q, c in enumerate(ctxs):        # the host-buffer call is synchronous: with K contexts they run one after the other
+                st, xout = c[0].lrdmc_run_host(xin[q], B.BALANCED, args.moves, 0.0, E0[q], cyc, 1)
+                emoves += st[0].moves_sum
+            cyc += 1
         barrier(); esecs = time.perf_counter() - t0
         eval_, _ = aggregate_over_ranks(emoves, esecs, world, fmax, fsum)
-        nbytes = int(x0.nbytes)
-        line["e2e"] = {"value": eval_, "unit": UNIT, "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes + 104,
+        nbytes = int(x0.nbytes) * K
+        line["e2e"] = {"value": eval_, "unit": UNIT, "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes + 104 * K,
                        "note": "lrdmc_run_host: pinned host positions in, set_positions (inverse rebuild), propagate, reconfigure, estimators, host positions out"}
     line["clocks"] = clk.summary()
 
@@ -249,7 +309,8 @@ def main():
                                 "sample": f"same {args.workload} system, N_w={args.ref_nw} walkers x {n // (args.ref_nw * args.moves)} cycles x {args.moves} moves ({n} walker-moves, {dt:.1f} s), balanced, incl. reconfiguration"}
     if rank == 0:
         print(json.dumps(line), flush=True)
-    g.close()
+    for c in ctxs:
+        c[0].close()
     if dist is not None:
         dist.destroy_process_group()
 

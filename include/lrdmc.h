@@ -6,6 +6,9 @@
  *
  * Conventions
  *   - Every function returns int: 0 = LRDMC_OK, < 0 = hard error (nothing modified unless stated).
+ *   - No process-global state: everything lives in the ctx (no environment variables are read; the text of a CUDA error is
+ *     kept per ctx, see lrdmc_last_error).  Calls on DIFFERENT contexts may run concurrently from different threads and on
+ *     different streams; calls on one ctx must be serialised by the caller.
  *   - "host"   pointer: ordinary CPU memory, read or written synchronously inside the call.
  *   - "device" pointer: CUDA device memory of the current device; used asynchronously on `stream`
  *     (a cudaStream_t passed as void*, NULL = legacy default stream).  The caller keeps such buffers alive
@@ -101,8 +104,21 @@ typedef struct {
 int lrdmc_init(lrdmc_ctx **out, const lrdmc_system *, const lrdmc_basis *, const lrdmc_mo *, const lrdmc_jastrow *,
                const lrdmc_lattice *);
 void lrdmc_free(lrdmc_ctx *);
-const char *lrdmc_strerror(int code);
+const char *lrdmc_strerror(int code);      /* static text per error code */
+/* Text of the last LRDMC_ECUDA of this ctx (cudaGetErrorString + source line; "" if none).  ctx == NULL: the text of the last
+ * failed lrdmc_init of the CALLING THREAD (thread-local, like errno: a failed init leaves no ctx to ask). */
+const char *lrdmc_last_error(const lrdmc_ctx *);
 int lrdmc_n_candidates(const lrdmc_ctx *); /* P = 6 N n_mesh + 6 N nl_K */
+
+/* Explicit tuning / test knobs (no environment variables).  Call BEFORE lrdmc_walker_bytes / lrdmc_bind_walkers (ESTATE once
+ * walkers are bound: the buffer was carved for the old plan).
+ *   LRDMC_OPT_TEAM_WARPS    value 0 = automatic (default), 1 = one warp per walker, 2/4/8/16 = a CTA of that
+ *                           many warps per walker (north_star "one CTA or warp group per walker"); other values are rounded down to
+ *                           a power of two.  The parity tests run every size.
+ *   LRDMC_OPT_GLOBAL_TABLES value != 0: keep the MO-coefficient fragment tables and the MO cache in global memory even when
+ *                           they fit shared memory (the code path of the 64-electron configuration, forced on small systems by tests). */
+enum { LRDMC_OPT_TEAM_WARPS = 1, LRDMC_OPT_GLOBAL_TABLES = 2 };
+int lrdmc_set_option(lrdmc_ctx *, int option, int value);
 
 /* ---- walker storage: structure of arrays in ONE caller-owned device buffer ---------------------------
  * positions (double-buffered for the branching gather), inverse Slater matrices per spin, cached MO
@@ -111,7 +127,8 @@ size_t lrdmc_walker_bytes(const lrdmc_ctx *, int n_walkers);
 int lrdmc_bind_walkers(lrdmc_ctx *, void *dev_buf /*device*/, size_t bytes, int n_walkers); /* EINVAL if too small */
 
 /* Upload positions r [n_w][N][3] (device), build Dinv_sigma = D_sigma^{-1} by pivoted elimination and the MO
- * caches (row a13), weights <- 1.  Synchronises `stream`; returns ESINGULAR if any Slater matrix had a zero pivot. */
+ * caches (row a13), weights <- 1.  Synchronises `stream`; returns ESINGULAR if any Slater matrix was singular (a pivot
+ * <= 2^-44 max|D_ij|, reading Q24): the state IS set all the same, the singular walkers are dead (see n_singular below). */
 int lrdmc_set_positions(lrdmc_ctx *, const double *r_dev, void *stream);
 
 /* One branching interval for every walker (weights reset to 1 on entry, Alg.2 line 4 L401 / Alg.1 line 4 L350):
@@ -136,6 +153,10 @@ typedef struct {
     int64_t n_node_flag;    /* evaluations that saw at least one R_j < 0 */
     int64_t n_nonpos_diag;  /* evaluations with W(x)-E0 <= 0 (balanced; walker weight set to 0, reading Q16) */
     int64_t n_nonfinite;    /* walkers whose weight left the finite range (set to 0) */
+    int64_t n_singular;     /* walkers whose Slater matrix was singular at the last (re)build -- after lrdmc_reconfigure: the
+                               rebuild of that branching; before: set_positions / set_state.  Reading Q24: such a walker is DEAD
+                               (zero inverses, never evaluated): the next propagate gives it w = omega = 0, the next branching
+                               replaces it */
     double lockstep_idle_frac; /* 1 - sum n_k/(N_w max n_k): idle share of a lock-step batch (L168, App. C) */
     double barrier_idle_frac;  /* measured: 1 - sum_warps busy time / (resident warps x kernel span) */
     float propagate_ms, reconfigure_ms; /* CUDA-event durations of the last calls on their stream */
@@ -162,23 +183,26 @@ int lrdmc_set_state(lrdmc_ctx *, const double *r_dev, const double *dinv_up_dev,
 /* Per-walker observables of the last propagate (device, nullable): e_L, W, omega [n_w] doubles; n_moves [n_w] int64 */
 int lrdmc_get_obs(lrdmc_ctx *, double *eL_dev, double *W_dev, double *omega_dev, int64_t *n_moves_dev, void *stream);
 
-/* End-to-end convenience with HOST buffers: H2D of r_in [n_w][N][3], set_positions, n_cycles x (propagate,
- * reconfigure, estimators -> stats_out[c], E0 feedback as running mean of e_n when mode is balanced), D2H of the
- * final positions into r_out (nullable).  Walkers must be bound.  Synchronous. */
+/* End-to-end convenience with HOST buffers (Alg.2 lines 2-13 L398-L420 / Alg.1): H2D of r_in [n_w][N][3], set_positions,
+ * n_cycles x (propagate, reconfigure, estimators -> stats_out[c] (nullable, [n_cycles])), D2H of the final positions into r_out
+ * (nullable).  Balanced mode feeds E0 back after each branching ("Update E_0", L232 / L418; reading Q8a): E0 <- running mean of
+ * e_n = num_n/den_n over the generations so far, the mean restarting once at generation n_therm (0: never) so that the
+ * equilibration transient does not stay in it; conventional mode keeps E0 (the constant shift of Q8b).  Walkers must be bound.
+ * Synchronous.  Errors: EINVAL, ESTATE (no walkers bound), ESINGULAR (a Slater matrix of r_in had a zero pivot; nothing was
+ * propagated, r_out untouched), ECUDA. */
 int lrdmc_run_host(lrdmc_ctx *, const double *r_in_host, double *r_out_host, int mode, int n_moves, double tau, double E0,
-                   uint64_t first_cycle, int n_cycles, lrdmc_cycle_stats *stats_out_host, void *stream);
-
-/* Roofline denominators measured on this device ("measure DFMA and DMMA peaks on the box"):
- * TFLOP/s of independent FP64 FMA chains, of mma.sync m8n8k4 f64 chains, and of both issued together. Host outputs. */
-int lrdmc_measure_fp64_peaks(double *dfma_tflops, double *dmma_tflops, double *mixed_tflops);
-/* Same, for the two instruction forms that set the real ceiling of the path (dispatch model):
- * dfma_3reg_tflops -- FMAs whose three source operands are three different registers (3 dispatch cycles instead of 2);
- * dfma_alu_tflops  -- two-register FMAs each followed by two independent integer ALU instructions of the same warp
- *                     (FP64 flop only; 1/2 of dfma_tflops when nothing overlaps).  Host outputs; the second may be NULL. */
-int lrdmc_measure_fp64_operand_peak(double *dfma_3reg_tflops, double *dfma_alu_tflops);
+                   uint64_t first_cycle, int n_cycles, int n_therm, lrdmc_cycle_stats *stats_out_host, void *stream);
 
 /* Test hook for pin P11: fills out_dev [n][4] (uint32) with Philox4x32-10 blocks for counters ctr_dev [n][4], key[2]. */
 int lrdmc_debug_philox(const uint32_t *ctr_dev, uint32_t key0, uint32_t key1, uint32_t *out_dev, int n, void *stream);
+/* Test hook for row a0: out_dev [n][14] (device) = u1, u2, u3, u_sel, u_tau and the frame U[9] (row-major, versors = columns) that
+ * walker slots 0..n-1 draw at (cycle, step) -- the same device functions the walker kernels call. */
+int lrdmc_debug_draws(const lrdmc_ctx *, uint64_t cycle, uint64_t step, double *out_dev, int n, void *stream);
+/* Diagnostics for bench.py: kernels launched by this ctx so far; and the launch shape lrdmc_propagate uses for the bound
+ * walkers (grid, threads per CTA, dynamic shared memory, resident CTAs per SM; any pointer may be NULL), with
+ * *team_warps = warps per walker: 1 = kernel k_propagate (warp per walker), > 1 = kernel k_propagate_team. */
+int lrdmc_launch_count(const lrdmc_ctx *);
+int lrdmc_launch_config(const lrdmc_ctx *, int *grid, int *block, int *smem_bytes, int *ctas_per_sm, int *team_warps);
 
 #ifdef __cplusplus
 }

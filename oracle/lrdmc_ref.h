@@ -25,6 +25,7 @@ typedef struct {
     int64_t moves_min, moves_max, moves_sum;
     int64_t n_node_flag, n_nonpos_diag, n_nonfinite;
     double lockstep_idle_frac; /* 1 - sum_k n_k / (N_w max_k n_k): what a lock-step batch would idle */
+    int64_t n_singular;        /* walkers whose Slater matrix was singular at the last (re)build (reading Q24) */
 } lrdmc_ref_stats;
 
 /* System description (all arrays copied).  pp == NULL: all-electron; else [n_nuc][4] local
@@ -71,7 +72,10 @@ int lrdmc_ref_set_nonlocal(lrdmc_ref_ctx *, int K, int dla, const double *nl);
 int lrdmc_ref_nl_info(const lrdmc_ref_ctx *, const double *x, const double *dinv_up, const double *dinv_dn, const double U[9],
                       double *nu, double *rho, double *cand);
 
-/* walkers */
+/* walkers.  Reading Q24 (the paper is silent; SURVEY row a13 "LRDMC_ESINGULAR if |D| = 0"): a walker whose Slater matrix has a
+ * pivot <= 2^-44 max|D| at a (re)build is DEAD: its inverses are set to zero, it is never evaluated, the next propagate gives it
+ * w = omega = 0 (e_L = W = 0, no moves), so the next branching replaces it.  set_positions returns ESINGULAR if there is any
+ * (the state is set all the same); reconfigure reports them in the stats (n_singular). */
 int lrdmc_ref_set_positions(lrdmc_ref_ctx *, int n_w, const double *r /*[n_w][N][3]*/);
 int lrdmc_ref_get_state(const lrdmc_ref_ctx *, double *r, double *dinv_up, double *dinv_dn, double *w);
 int lrdmc_ref_set_state(lrdmc_ref_ctx *, int n_w, const double *r, const double *dinv_up, const double *dinv_dn,

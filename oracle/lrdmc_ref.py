@@ -35,7 +35,7 @@ class Stats(C.Structure):
     _fields_ = [("wbar", C.c_double), ("num", C.c_double), ("den", C.c_double),
                 ("moves_min", C.c_int64), ("moves_max", C.c_int64), ("moves_sum", C.c_int64),
                 ("n_node_flag", C.c_int64), ("n_nonpos_diag", C.c_int64), ("n_nonfinite", C.c_int64),
-                ("lockstep_idle_frac", C.c_double)]
+                ("lockstep_idle_frac", C.c_double), ("n_singular", C.c_int64)]
 
     def asdict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}

@@ -43,12 +43,13 @@ def energy(wbar, num, den, p=10, n_therm=0, n_blocks=20):
     return E, sigma
 
 
-def run(o: "ref.Ref", mode, cycles, n_moves=0, tau=0.0, E0=None, E_ref=None, first_cycle=0, feedback=True):
+def run(o: "ref.Ref", mode, cycles, n_moves=0, tau=0.0, E0=None, E_ref=None, first_cycle=0, feedback=True, n_therm=0):
     """Alg.2 (balanced) / Alg.1 (conventional) outer loop on an oracle context whose walkers are set.
 
     Returns a dict of per-generation arrays (wbar, num, den, e, moves_*, flags).  `E0`: initial guess
     for the balanced Green's function (Eq.28); updated after each branching (L232) as the running mean
-    of e_n when `feedback`.  Conventional mode passes the fixed shift E_ref (Q8b)."""
+    of e_n when `feedback`; the mean restarts once at generation `n_therm` (reading Q8a: "after n_therm: restart the mean").
+    Conventional mode passes the fixed shift E_ref (Q8b)."""
     rec = {k: [] for k in ("wbar", "num", "den", "moves_min", "moves_max", "moves_sum", "n_node_flag",
                            "n_nonpos_diag", "n_nonfinite", "lockstep_idle_frac", "E0_used")}
     e_hist = []
@@ -62,8 +63,9 @@ def run(o: "ref.Ref", mode, cycles, n_moves=0, tau=0.0, E0=None, E_ref=None, fir
                 rec[k].append(s[k])
         rec["E0_used"].append(shift)
         e_hist.append(s["num"] / s["den"])
-        if mode == ref.BALANCED and feedback:
-            E0 = float(np.mean(e_hist))          # "Update E_0" (Alg.2 line 12, L418; reading Q8a)
+        if mode == ref.BALANCED and feedback:    # "Update E_0" (Alg.2 line 12, L418; reading Q8a)
+            i = len(e_hist) - 1
+            E0 = float(np.mean(e_hist[n_therm:] if (n_therm > 0 and i >= n_therm) else e_hist))
     out = {k: np.array(v) for k, v in rec.items()}
     out["e"] = np.array(e_hist)
     return out

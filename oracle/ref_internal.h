@@ -36,6 +36,8 @@ struct lrdmc_ref_ctx {
     /* walkers */
     int n_w; double *r, *dinv_up, *dinv_dn, *w, *eL, *W, *omega; int64_t *nmoves;
     int *flag_node, *flag_nonpos, *flag_nonfinite; /* per-walker event counts of the last cycle */
+    int *dead;                       /* walker whose Slater matrix was singular at the last (re)build (reading Q24): weight 0, never evaluated */
+    int64_t n_singular;              /* number of such walkers */
     double wbar; int have_obs;
     uint32_t slot0;                  /* random streams of walker k are keyed by slot slot0 + k (lrdmc_ref_set_slot_offset) */
 };

@@ -49,7 +49,7 @@ int lrdmc_ref_create(lrdmc_ref_ctx **out, int n_nuc, const double *Z, const doub
 static void free_walkers(lrdmc_ref_ctx *c)
 {
     free(c->r); free(c->dinv_up); free(c->dinv_dn); free(c->w); free(c->eL); free(c->W); free(c->omega); free(c->nmoves);
-    free(c->flag_node); free(c->flag_nonpos); free(c->flag_nonfinite);
+    free(c->flag_node); free(c->flag_nonpos); free(c->flag_nonfinite); free(c->dead); c->dead = NULL; c->n_singular = 0;
     c->r = c->dinv_up = c->dinv_dn = c->w = c->eL = c->W = c->omega = NULL; c->nmoves = NULL;
     c->flag_node = c->flag_nonpos = c->flag_nonfinite = NULL; c->n_w = 0; c->have_obs = 0;
 }
@@ -125,15 +125,20 @@ static void alloc_walkers(lrdmc_ref_ctx *c, int n_w)
     c->W = (double *)calloc(nw, sizeof(double)); c->omega = (double *)calloc(nw, sizeof(double));
     c->nmoves = (int64_t *)calloc(nw, sizeof(int64_t));
     c->flag_node = (int *)calloc(nw, sizeof(int)); c->flag_nonpos = (int *)calloc(nw, sizeof(int)); c->flag_nonfinite = (int *)calloc(nw, sizeof(int));
+    c->dead = (int *)calloc(nw, sizeof(int));
     for (int k = 0; k < n_w; ++k) c->w[k] = 1.0;
 }
 
+/* inverses of every walker from its positions (row a13); singular walkers are marked dead, their inverses zeroed (reading Q24) */
 static int rebuild_all(lrdmc_ref_ctx *c)
 {
-    size_t ou = (size_t)c->n_up * c->n_up, od = (size_t)c->n_dn * c->n_dn; int bad = 0;
-    #pragma omp parallel for schedule(dynamic) reduction(|:bad)
-    for (int k = 0; k < c->n_w; ++k)
-        if (lrdmc_ref_build_inverse(c, c->r + (size_t)k * 3 * c->N, c->dinv_up + k * ou, c->dinv_dn + k * od)) bad |= 1;
+    size_t ou = (size_t)c->n_up * c->n_up, od = (size_t)c->n_dn * c->n_dn; int64_t bad = 0;
+    #pragma omp parallel for schedule(dynamic) reduction(+:bad)
+    for (int k = 0; k < c->n_w; ++k) {
+        c->dead[k] = lrdmc_ref_build_inverse(c, c->r + (size_t)k * 3 * c->N, c->dinv_up + k * ou, c->dinv_dn + k * od) != 0;
+        if (c->dead[k]) { memset(c->dinv_up + k * ou, 0, sizeof(double) * ou); memset(c->dinv_dn + k * od, 0, sizeof(double) * od); ++bad; }
+    }
+    c->n_singular = bad;
     return bad ? LRDMC_REF_ESINGULAR : LRDMC_REF_OK;
 }
 
@@ -166,7 +171,7 @@ int lrdmc_ref_set_state(lrdmc_ref_ctx *c, int n_w, const double *r, const double
     if (dinv_up) {
         memcpy(c->dinv_up, dinv_up, sizeof(double) * nw * c->n_up * c->n_up);
         if (c->n_dn) memcpy(c->dinv_dn, dinv_dn, sizeof(double) * nw * c->n_dn * c->n_dn);
-    } else { int rc = rebuild_all(c); if (rc) return rc; }
+    } else rebuild_all(c);                     /* dead walkers are marked, not an error here (reading Q24) */
     if (w) memcpy(c->w, w, sizeof(double) * nw);
     return LRDMC_REF_OK;
 }
@@ -194,6 +199,10 @@ static void cand_pos(const lrdmc_ref_ctx *c, const double *x, const double U[9],
 static void propagate_walker(lrdmc_ref_ctx *c, int k, int mode, int n_moves, double tau, double E0, uint64_t cycle)
 {
     int N = c->N, P = c->P;
+    if (c->dead[k]) {                                   /* singular at the last (re)build: dies at the next branching (reading Q24) */
+        c->w[k] = 0.0; c->omega[k] = 0.0; c->eL[k] = 0.0; c->W[k] = 0.0; c->nmoves[k] = 0; c->flag_node[k] = 0; c->flag_nonpos[k] = 0;
+        return;
+    }
     double *x = c->r + (size_t)k * 3 * N;
     double *du = c->dinv_up + (size_t)k * c->n_up * c->n_up, *dd = c->dinv_dn + (size_t)k * c->n_dn * c->n_dn;
     double *R = (double *)malloc(sizeof(double) * (size_t)P), scal[10], u[5], U[9], rp[3];
@@ -248,7 +257,7 @@ int lrdmc_ref_estimators(const lrdmc_ref_ctx *c, lrdmc_ref_stats *out)
 {
     if (!c->have_obs) return LRDMC_REF_ESTATE;
     memset(out, 0, sizeof(*out));
-    out->wbar = c->wbar; out->moves_min = INT64_MAX;
+    out->wbar = c->wbar; out->moves_min = INT64_MAX; out->n_singular = c->n_singular;
     for (int k = 0; k < c->n_w; ++k) {
         out->num += c->omega[k] * c->eL[k]; out->den += c->omega[k];   /* Eq.34 (L227) / Eq.20 (L135) */
         if (c->nmoves[k] < out->moves_min) out->moves_min = c->nmoves[k];
@@ -274,7 +283,8 @@ int lrdmc_ref_reconfigure(lrdmc_ref_ctx *c, uint64_t cycle, int32_t *parents_out
     for (int k = 0; k < n_w; ++k) c->w[k] = 1.0;
     if (parents_out) memcpy(parents_out, par, sizeof(int32_t) * (size_t)n_w);
     free(rn); free(par);
-    return rebuild_all(c);
+    rebuild_all(c);                             /* singular walkers: marked dead and counted in the stats (reading Q24), not an error */
+    return LRDMC_REF_OK;
 }
 
 int lrdmc_ref_step_debug(const lrdmc_ref_ctx *c, double E0, uint64_t cycle, uint64_t step, double *R, double *scal, int32_t *jstar)

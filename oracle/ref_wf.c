@@ -117,17 +117,23 @@ int lrdmc_ref_mo(const lrdmc_ref_ctx *c, int spin, const double r[3], double *va
     return rc;
 }
 
-/* Gauss-Jordan inverse with partial (row) pivoting; also log|det| and its sign.  ESINGULAR on a zero pivot. */
+/* Gauss-Jordan inverse with partial (row) pivoting; also log|det| and its sign.
+ * ESINGULAR when a pivot is not above 2^-44 max|A_ij| (reading Q24 of DESIGN.md: "|D| = 0" in FP64.  Two identical rows -- two
+ * same-spin electrons at one point -- leave a pivot of rounding size ~2^-52 max|A|, not an exact zero; a matrix whose pivots fall
+ * below 2^-44 has lost all but 8 bits of its inverse anyway). */
 int ref_invert(int n, const double *A, double *Ainv, double *logabs, int *sign)
 {
     double la = 0.0; int sg = 1;
     if (n == 0) { if (logabs) *logabs = 0.0; if (sign) *sign = 1; return LRDMC_REF_OK; }
+    double amax = 0.0;
+    for (int i = 0; i < n * n; ++i) if (fabs(A[i]) > amax) amax = fabs(A[i]);
+    const double tiny = ldexp(amax, -44);
     double *M = (double *)malloc(sizeof(double) * 2 * (size_t)n * n);
     for (int i = 0; i < n; ++i) for (int j = 0; j < n; ++j) { M[i * 2 * n + j] = A[i * n + j]; M[i * 2 * n + n + j] = (i == j); }
     for (int col = 0; col < n; ++col) {
         int piv = col; double best = fabs(M[col * 2 * n + col]);
         for (int i = col + 1; i < n; ++i) if (fabs(M[i * 2 * n + col]) > best) { best = fabs(M[i * 2 * n + col]); piv = i; }
-        if (!(best > 0.0) || !isfinite(best)) { free(M); return LRDMC_REF_ESINGULAR; }
+        if (!(best > tiny) || !isfinite(best)) { free(M); return LRDMC_REF_ESINGULAR; }
         if (piv != col) { for (int j = 0; j < 2 * n; ++j) { double t = M[col * 2 * n + j]; M[col * 2 * n + j] = M[piv * 2 * n + j]; M[piv * 2 * n + j] = t; } sg = -sg; }
         double p = M[col * 2 * n + col];
         la += log(fabs(p)); if (p < 0) sg = -sg;

@@ -15,9 +15,15 @@ LIB_PATH = os.environ.get("LRDMC_LIB", os.path.join(_HERE, "liblrdmc.so"))    # 
 BALANCED, CONVENTIONAL = 0, 1
 OK, EINVAL, ESINGULAR, ESTATE, ECUDA, ENOMEM = 0, -1, -2, -3, -4, -5
 
-EXPORTS = ["lrdmc_init", "lrdmc_free", "lrdmc_strerror", "lrdmc_n_candidates", "lrdmc_walker_bytes", "lrdmc_bind_walkers",
-           "lrdmc_set_positions", "lrdmc_propagate", "lrdmc_reconfigure", "lrdmc_estimators", "lrdmc_energy", "lrdmc_step_debug",
-           "lrdmc_get_walkers", "lrdmc_set_state", "lrdmc_get_obs", "lrdmc_run_host", "lrdmc_measure_fp64_peaks", "lrdmc_measure_fp64_operand_peak", "lrdmc_debug_philox"]
+PROBE_LIB_PATH = os.path.join(_HERE, "liblrdmc_probe.so")                     # include/lrdmc_probe.h (bench.py's roofline denominators)
+OPT_TEAM_WARPS, OPT_GLOBAL_TABLES = 1, 2
+
+# every symbol this module touches; tests check that include/lrdmc.h (resp. lrdmc_probe.h) declares each and the libraries export each
+EXPORTS = ["lrdmc_init", "lrdmc_free", "lrdmc_strerror", "lrdmc_last_error", "lrdmc_set_option", "lrdmc_n_candidates", "lrdmc_walker_bytes",
+           "lrdmc_bind_walkers", "lrdmc_set_positions", "lrdmc_propagate", "lrdmc_reconfigure", "lrdmc_estimators", "lrdmc_energy",
+           "lrdmc_step_debug", "lrdmc_get_walkers", "lrdmc_set_state", "lrdmc_get_obs", "lrdmc_run_host", "lrdmc_debug_philox",
+           "lrdmc_debug_draws", "lrdmc_launch_count", "lrdmc_launch_config"]
+PROBE_EXPORTS = ["lrdmc_measure_fp64_peaks", "lrdmc_measure_fp64_operand_peak"]
 
 
 class System(C.Structure):
@@ -46,7 +52,7 @@ class Lattice(C.Structure):
 class CycleStats(C.Structure):
     _fields_ = [("wbar", C.c_double), ("num", C.c_double), ("den", C.c_double),
                 ("moves_min", C.c_int64), ("moves_max", C.c_int64), ("moves_sum", C.c_int64),
-                ("n_node_flag", C.c_int64), ("n_nonpos_diag", C.c_int64), ("n_nonfinite", C.c_int64),
+                ("n_node_flag", C.c_int64), ("n_nonpos_diag", C.c_int64), ("n_nonfinite", C.c_int64), ("n_singular", C.c_int64),
                 ("lockstep_idle_frac", C.c_double), ("barrier_idle_frac", C.c_double),
                 ("propagate_ms", C.c_float), ("reconfigure_ms", C.c_float)]
 
@@ -81,26 +87,29 @@ def load_library():
         L.lrdmc_get_walkers.argtypes = [vp, vp, vp, vp, vp, vp]
         L.lrdmc_set_state.argtypes = [vp, vp, vp, vp, vp, vp]
         L.lrdmc_get_obs.argtypes = [vp, vp, vp, vp, vp, vp]
-        L.lrdmc_run_host.argtypes = [vp, vp, vp, i32, i32, dbl, dbl, u64, i32, C.POINTER(CycleStats), vp]
-        L.lrdmc_measure_fp64_peaks.argtypes = [C.POINTER(dbl), C.POINTER(dbl), C.POINTER(dbl)]
-        L.lrdmc_measure_fp64_operand_peak.argtypes = [C.POINTER(dbl), C.POINTER(dbl)]
+        L.lrdmc_run_host.argtypes = [vp, vp, vp, i32, i32, dbl, dbl, u64, i32, i32, C.POINTER(CycleStats), vp]
+        L.lrdmc_last_error.argtypes = [vp]; L.lrdmc_last_error.restype = C.c_char_p
+        L.lrdmc_set_option.argtypes = [vp, i32, i32]
         L.lrdmc_debug_philox.argtypes = [vp, C.c_uint32, C.c_uint32, vp, i32, vp]
         L.lrdmc_debug_draws.argtypes = [vp, u64, u64, vp, i32, vp]
         L.lrdmc_launch_count.argtypes = [vp]
-        L.lrdmc_launch_config.argtypes = [vp, C.POINTER(i32), C.POINTER(i32), C.POINTER(i32), C.POINTER(i32)]
+        L.lrdmc_launch_config.argtypes = [vp, C.POINTER(i32), C.POINTER(i32), C.POINTER(i32), C.POINTER(i32), C.POINTER(i32)]
         _lib = L
     return _lib
 
 
 class LrdmcError(RuntimeError):
-    def __init__(self, code, where):
+    def __init__(self, code, where, ctx=None):
         self.code = code
-        super().__init__(f"{where}: {load_library().lrdmc_strerror(code).decode()} ({code})")
+        L = load_library(); text = L.lrdmc_strerror(code).decode()
+        if code == ECUDA:
+            text += ": " + L.lrdmc_last_error(ctx).decode()
+        super().__init__(f"{where}: {text} ({code})")
 
 
-def _check(rc, where, allow=()):
+def _check(rc, where, allow=(), ctx=None):
     if rc != 0 and rc not in allow:
-        raise LrdmcError(rc, where)
+        raise LrdmcError(rc, where, ctx)
     return rc
 
 
@@ -116,18 +125,29 @@ def lrdmc_energy(records, p=10, n_therm=0, n_blocks=20):
     return E.value, sg.value
 
 
+_probe = None
+
+
 def lrdmc_measure_fp64_peaks():
-    a, b, m = C.c_double(), C.c_double(), C.c_double()
-    _check(load_library().lrdmc_measure_fp64_peaks(C.byref(a), C.byref(b), C.byref(m)), "lrdmc_measure_fp64_peaks")
-    t, u = C.c_double(), C.c_double()
-    _check(load_library().lrdmc_measure_fp64_operand_peak(C.byref(t), C.byref(u)), "lrdmc_measure_fp64_operand_peak")
+    """include/lrdmc_probe.h: FP64 peaks measured on the current device (liblrdmc_probe.so, not the product library)."""
+    global _probe
+    if _probe is None:
+        if not os.path.exists(PROBE_LIB_PATH):
+            raise RuntimeError(f"{PROBE_LIB_PATH} is missing: run `python -m paper_2508_12033_b200.build`")
+        _probe = C.CDLL(PROBE_LIB_PATH)
+        dp = C.POINTER(C.c_double)
+        _probe.lrdmc_measure_fp64_peaks.argtypes = [dp, dp, dp]; _probe.lrdmc_measure_fp64_operand_peak.argtypes = [dp, dp]
+    a, b, m, t, u = (C.c_double() for _ in range(5))
+    if _probe.lrdmc_measure_fp64_peaks(C.byref(a), C.byref(b), C.byref(m)) or _probe.lrdmc_measure_fp64_operand_peak(C.byref(t), C.byref(u)):
+        raise RuntimeError("FP64 peak probe failed (CUDA error)")
     return dict(dfma_tflops=a.value, dmma_tflops=b.value, mixed_tflops=m.value, dfma_3reg_tflops=t.value, dfma_alu_tflops=u.value)
 
 
 class Lrdmc:
     """One context = one system on the current CUDA device; walkers live in a torch uint8 tensor owned by this object."""
 
-    def __init__(self, sysd, device="cuda:0"):
+    def __init__(self, sysd, device="cuda:0", options=None):
+        """options: {OPT_TEAM_WARPS: tw, OPT_GLOBAL_TABLES: 0/1} applied with lrdmc_set_option before any walker is bound."""
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("liblrdmc needs a CUDA device (B200, sm_100a); there is no CPU fallback")
@@ -153,6 +173,8 @@ class Lrdmc:
         h = C.c_void_p()
         _check(L.lrdmc_init(C.byref(h), C.byref(s), C.byref(b), C.byref(m), C.byref(j), C.byref(la)), "lrdmc_init")
         self.h = h
+        for opt, val in (options or {}).items():
+            self.lrdmc_set_option(opt, val)
         self.P = L.lrdmc_n_candidates(h)
         self.n_w = 0
         self.buf = None
@@ -176,6 +198,12 @@ class Lrdmc:
             return a.to(self.device).contiguous()
         return t.from_numpy(np.ascontiguousarray(a, dtype=dtype)).to(self.device)
 
+    def lrdmc_set_option(self, option, value):
+        _check(self.L.lrdmc_set_option(self.h, int(option), int(value)), "lrdmc_set_option", ctx=self.h)
+
+    def lrdmc_last_error(self):
+        return self.L.lrdmc_last_error(self.h).decode()
+
     # ---- storage ----
     def lrdmc_walker_bytes(self, n_w):
         return int(self.L.lrdmc_walker_bytes(self.h, n_w))
@@ -183,7 +211,7 @@ class Lrdmc:
     def lrdmc_bind_walkers(self, n_w):
         nbytes = self.lrdmc_walker_bytes(n_w)
         self.buf = self.torch.zeros(nbytes, dtype=self.torch.uint8, device=self.device)
-        _check(self.L.lrdmc_bind_walkers(self.h, _ptr(self.buf), nbytes, n_w), "lrdmc_bind_walkers")
+        _check(self.L.lrdmc_bind_walkers(self.h, _ptr(self.buf), nbytes, n_w), "lrdmc_bind_walkers", ctx=self.h)
         self.n_w = n_w
 
     # ---- the path ----
@@ -192,20 +220,20 @@ class Lrdmc:
         if self.n_w != r.shape[0]:
             self.lrdmc_bind_walkers(int(r.shape[0]))
         assert tuple(r.shape) == (self.n_w, self.N, 3)
-        return _check(self.L.lrdmc_set_positions(self.h, _ptr(r), self._stream()), "lrdmc_set_positions",
+        return _check(self.L.lrdmc_set_positions(self.h, _ptr(r), self._stream()), "lrdmc_set_positions", ctx=self.h,
                       allow=(ESINGULAR,) if allow_singular else ())
 
     def lrdmc_propagate(self, mode, n_moves, tau, E0, cycle):
-        _check(self.L.lrdmc_propagate(self.h, mode, n_moves, tau, E0, cycle, self._stream()), "lrdmc_propagate")
+        _check(self.L.lrdmc_propagate(self.h, mode, n_moves, tau, E0, cycle, self._stream()), "lrdmc_propagate", ctx=self.h)
 
     def lrdmc_reconfigure(self, cycle, want_parents=False):
         par = self.torch.empty(self.n_w, dtype=self.torch.int32, device=self.device) if want_parents else None
-        _check(self.L.lrdmc_reconfigure(self.h, cycle, _ptr(par), self._stream()), "lrdmc_reconfigure")
+        _check(self.L.lrdmc_reconfigure(self.h, cycle, _ptr(par), self._stream()), "lrdmc_reconfigure", ctx=self.h)
         return par
 
     def lrdmc_estimators(self):
         s = CycleStats()
-        _check(self.L.lrdmc_estimators(self.h, C.byref(s)), "lrdmc_estimators")
+        _check(self.L.lrdmc_estimators(self.h, C.byref(s)), "lrdmc_estimators", ctx=self.h)
         return s
 
     def lrdmc_step_debug(self, E0, cycle, step):
@@ -213,14 +241,14 @@ class Lrdmc:
         R = t.empty((self.n_w, self.P), dtype=t.float64, device=self.device)
         scal = t.empty((self.n_w, 8), dtype=t.float64, device=self.device)
         js = t.empty(self.n_w, dtype=t.int32, device=self.device)
-        _check(self.L.lrdmc_step_debug(self.h, E0, cycle, step, _ptr(R), _ptr(scal), _ptr(js), self._stream()), "lrdmc_step_debug")
+        _check(self.L.lrdmc_step_debug(self.h, E0, cycle, step, _ptr(R), _ptr(scal), _ptr(js), self._stream()), "lrdmc_step_debug", ctx=self.h)
         return R, scal, js
 
     def lrdmc_get_walkers(self):
         t = self.torch; f = dict(dtype=t.float64, device=self.device)
         r = t.empty((self.n_w, self.N, 3), **f); du = t.empty((self.n_w, self.n_up, self.n_up), **f)
         dd = t.empty((self.n_w, self.n_dn, self.n_dn), **f); w = t.empty(self.n_w, **f)
-        _check(self.L.lrdmc_get_walkers(self.h, _ptr(r), _ptr(du), _ptr(dd) if self.n_dn else None, _ptr(w), self._stream()), "lrdmc_get_walkers")
+        _check(self.L.lrdmc_get_walkers(self.h, _ptr(r), _ptr(du), _ptr(dd) if self.n_dn else None, _ptr(w), self._stream()), "lrdmc_get_walkers", ctx=self.h)
         return r, du, dd, w
 
     def lrdmc_set_state(self, r, du=None, dd=None, w=None):
@@ -229,17 +257,17 @@ class Lrdmc:
             self.lrdmc_bind_walkers(int(r.shape[0]))
         du = None if du is None else self._dev(du, np.float64); dd = None if dd is None or self.n_dn == 0 else self._dev(dd, np.float64)
         w = None if w is None else self._dev(w, np.float64)
-        _check(self.L.lrdmc_set_state(self.h, _ptr(r), _ptr(du), _ptr(dd), _ptr(w), self._stream()), "lrdmc_set_state")
+        _check(self.L.lrdmc_set_state(self.h, _ptr(r), _ptr(du), _ptr(dd), _ptr(w), self._stream()), "lrdmc_set_state", ctx=self.h)
         self._hold = (r, du, dd, w)
 
     def lrdmc_get_obs(self):
         t = self.torch; f = dict(dtype=t.float64, device=self.device)
         eL = t.empty(self.n_w, **f); W = t.empty(self.n_w, **f); om = t.empty(self.n_w, **f)
         nm = t.empty(self.n_w, dtype=t.int64, device=self.device)
-        _check(self.L.lrdmc_get_obs(self.h, _ptr(eL), _ptr(W), _ptr(om), _ptr(nm), self._stream()), "lrdmc_get_obs")
+        _check(self.L.lrdmc_get_obs(self.h, _ptr(eL), _ptr(W), _ptr(om), _ptr(nm), self._stream()), "lrdmc_get_obs", ctx=self.h)
         return eL, W, om, nm
 
-    def lrdmc_run_host(self, r_host, mode, n_moves, tau, E0, first_cycle, n_cycles, want_positions=True):
+    def lrdmc_run_host(self, r_host, mode, n_moves, tau, E0, first_cycle, n_cycles, want_positions=True, n_therm=0):
         """HOST buffers in and out (numpy / pinned torch CPU tensors): copies are inside the call."""
         r_in = np.ascontiguousarray(r_host, dtype=np.float64) if not isinstance(r_host, self.torch.Tensor) else r_host
         n_w = int(r_in.shape[0])
@@ -253,7 +281,7 @@ class Lrdmc:
         stats = (CycleStats * max(1, n_cycles))()
         pin = r_in.data_ptr() if isinstance(r_in, self.torch.Tensor) else r_in.ctypes.data
         _check(self.L.lrdmc_run_host(self.h, pin, None if r_out is None else r_out.data_ptr(), mode, n_moves, tau, E0, first_cycle, n_cycles,
-                                     stats, self._stream()), "lrdmc_run_host")
+                                     n_therm, stats, self._stream()), "lrdmc_run_host", ctx=self.h)
         return [stats[i] for i in range(n_cycles)], r_out
 
     # ---- diagnostics ----
@@ -261,13 +289,14 @@ class Lrdmc:
         return int(self.L.lrdmc_launch_count(self.h))
 
     def launch_config(self):
-        g, b, s, c = C.c_int(), C.c_int(), C.c_int(), C.c_int()
-        self.L.lrdmc_launch_config(self.h, C.byref(g), C.byref(b), C.byref(s), C.byref(c))
-        return dict(grid=g.value, block=b.value, smem_bytes=s.value, ctas_per_sm=c.value)
+        g, b, s, c, t = C.c_int(), C.c_int(), C.c_int(), C.c_int(), C.c_int()
+        self.L.lrdmc_launch_config(self.h, C.byref(g), C.byref(b), C.byref(s), C.byref(c), C.byref(t))
+        return dict(grid=g.value, block=b.value, smem_bytes=s.value, ctas_per_sm=c.value, team_warps=t.value,
+                    kernel="k_propagate" if t.value <= 1 else "k_propagate_team")
 
     def debug_draws(self, cycle, step, n):
         out = self.torch.empty((n, 14), dtype=self.torch.float64, device=self.device)
-        _check(self.L.lrdmc_debug_draws(self.h, cycle, step, _ptr(out), n, self._stream()), "lrdmc_debug_draws")
+        _check(self.L.lrdmc_debug_draws(self.h, cycle, step, _ptr(out), n, self._stream()), "lrdmc_debug_draws", ctx=self.h)
         return out
 
     def debug_philox(self, ctr, key):

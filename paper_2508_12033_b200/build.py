@@ -3,7 +3,7 @@
     python -m paper_2508_12033_b200.build [--force] [-v]
 
 Translation units (compiled in parallel, then linked): lrdmc.cu (C-ABI, host logic, rebuild / reconfigure / reduction kernels),
-lrdmc_aux.cu (estimators over generations, host-buffer driver, peak probes) and kernels.cu four times -- the walker kernels
+lrdmc_aux.cu (estimators over generations, host-buffer driver, test hooks) and kernels.cu four times -- the walker kernels
 {lattice-only, with non-local pseudopotential slots} x {warp-per-walker, team}.
 """
 from __future__ import annotations
@@ -15,6 +15,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "liblrdmc.so")
+PROBE_LIB = os.path.join(HERE, "liblrdmc_probe.so")      # include/lrdmc_probe.h: FP64 peak micro-benchmarks (bench.py only)
 OBJDIR = os.path.join(HERE, "build")
 # (source, object name, extra defines)
 UNITS = [("lrdmc.cu", "lrdmc.o", []), ("lrdmc_aux.cu", "lrdmc_aux.o", []),
@@ -47,6 +48,9 @@ def build(force: bool = False, verbose: bool = False) -> str:
         if failed:
             raise subprocess.CalledProcessError(1, failed[0])
         subprocess.run([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", LIB] + [os.path.join(OBJDIR, o) for _, o, _ in UNITS], check=True)
+    probe_src = os.path.join(CSRC, "probe.cu")
+    if force or not os.path.exists(PROBE_LIB) or any(os.path.getmtime(d) > os.path.getmtime(PROBE_LIB) for d in (probe_src, os.path.join(CSRC, "peaks.cuh"))):
+        subprocess.run([os.environ.get("NVCC", "nvcc")] + NVCC_FLAGS + ["-shared", "-o", PROBE_LIB, probe_src], check=True)
     return LIB
 
 

@@ -90,6 +90,8 @@ struct DevWalk {
     double *w, *eL, *W, *omega;
     long long *nmoves;
     int *flags;           // [n_w][3] node / nonpos / nonfinite counts of the last propagate
+    int *dead;            // [n_w] 1: Slater matrix singular at the last (re)build (reading Q24): weight 0, never evaluated
+    long long *n_sing;    // device counter of such walkers (lives in the ctx's DevStats)
     unsigned long long *wq, *prefix; // comb workspace
     int *parents;
     unsigned long long *timing;      // [max_warps][2] globaltimer start/end per resident warp
@@ -97,6 +99,7 @@ struct DevWalk {
     int *counter;         // dynamic walker queue head; [1] = singular flag
     double *bcs;          // per resident team CTA: parked Bc entries [block of a mesh][k-step pair][lane][2] (ao_columns BCS); NULL if unused
     size_t bcs_stride;    // doubles per CTA
+    int bcs_ctas;         // CTAs the scratch was sized for
 };
 
 __device__ __forceinline__ double warp_sum(double v)

@@ -14,19 +14,23 @@
 #include "propagate.cuh"
 #include "kernels.h"
 #include "reconfigure.cuh"
-#include "peaks.cuh"
 #include "api_internal.h"
 
-#define CK(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) { snprintf(g_cuda_msg, sizeof g_cuda_msg, "%s at %s:%d", cudaGetErrorString(e_), __FILE__, __LINE__); return LRDMC_ECUDA; } } while (0)
-static char g_cuda_msg[256] = "";
+// CUDA errors: the text goes into the context (lrdmc_last_error); every function that uses CK has a ctx pointer named `c`.
+#define CK(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) { snprintf(c->msg, sizeof c->msg, "%s at %s:%d", cudaGetErrorString(e_), __FILE__, __LINE__); return LRDMC_ECUDA; } } while (0)
+// lrdmc_init has no context to hand back when it fails: its text is kept per calling thread (like errno), read with lrdmc_last_error(NULL).
+static thread_local char t_init_msg[256] = "";
 
 struct lrdmc_ctx {
     DevSys S; DevWalk W;
-    void *d_tables; DevStats *d_stats;
-    int NT, ts, wpb, ctas_per_sm, sm_count, smem_bytes, grid_max;
+    void *d_tables; DevStats *d_stats, *h_stats;   // h_stats: pinned staging of the per-generation sums (read back on the ctx's own stream)
+    int NT, ts, wpb, ctas_per_sm, sm_count, smem_bytes, grid_max; size_t smem_per_sm;
     int bound, have_prop, have_reconf, state_ok;
     cudaEvent_t ev[4]; cudaStream_t last_stream;
     int launches;   // kernels launched so far (bench.py reports it)
+    char msg[256];  // text of the last CUDA error of this context (lrdmc_last_error)
+    int opt_team, opt_global_tables;            // lrdmc_set_option
+    size_t n_sh, n_nuc_d, bf_n, cf_n;           // table sizes in doubles (shared-memory plan)
     // team mode (team.cuh): chosen at lrdmc_bind_walkers from N_w and the footprint; team_tw == 1 -> warp-per-walker kernel
     TeamPlan team; int team_tw, team_smem, team_ctas_per_sm, team_grid_max, pair_base[5];
 };
@@ -38,7 +42,7 @@ extern "C" const char *lrdmc_strerror(int code)
     case LRDMC_EINVAL: return "invalid argument";
     case LRDMC_ESINGULAR: return "singular Slater matrix";
     case LRDMC_ESTATE: return "call order: walkers not bound / positions not set / nothing propagated";
-    case LRDMC_ECUDA: return g_cuda_msg[0] ? g_cuda_msg : "CUDA error";
+    case LRDMC_ECUDA: return "CUDA error (text: lrdmc_last_error)";
     case LRDMC_ENOMEM: return "system does not fit the shared-memory plan";
     default: return "unknown error";
     }
@@ -51,13 +55,95 @@ static double gto_norm(double z, int l, int m, int n)
 }
 static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
+// ---- shared-memory plan: either every table and the MO cache sit in shared memory (TS kernels), or the fragment tables and
+// the cache are read from global memory (large systems; LRDMC_OPT_GLOBAL_TABLES forces this path for tests).  No mixed case: a
+// fragment pointer that may be shared OR global makes nvcc 12.9 infer "shared" for it (cvta.to.shared + ld.shared on a global
+// address).  Re-run by lrdmc_set_option; the device tables themselves do not depend on it.
+static int plan_smem(lrdmc_ctx *c)
+{
+    DevSys &S = c->S;
+    cudaDeviceProp prop; int dev = 0; CK(cudaGetDevice(&dev)); CK(cudaGetDeviceProperties(&prop, dev));
+    c->sm_count = prop.multiProcessorCount; c->smem_per_sm = prop.sharedMemPerMultiprocessor;
+    const size_t bf_n = c->bf_n, cf_n = c->cf_n;
+    const size_t bf_doubles = (bf_n + cf_n) * (S.same_C ? 1 : 2);
+    const size_t moc_doubles = (size_t)S.N * 5 * S.OS;
+    const bool fits = bf_doubles * 8 <= 64 * 1024 && moc_doubles * 8 <= 12 * 1024 && !c->opt_global_tables;
+    S.bf_in_smem = fits; S.moc_in_smem = fits;
+    size_t o = 0;
+    S.off_etab = (int)o; o += 256;              // always first: exp_tab addresses it as (dynamic smem base) + 8 j
+    S.off_shells = (int)o; o += align_up(c->n_sh, 2);
+    S.off_nuc = (int)o; o += align_up(c->n_nuc_d, 2);
+    S.off_bf[0] = (int)o; if (S.bf_in_smem) o += bf_n;
+    S.off_bf[1] = (int)o; if (S.bf_in_smem && !S.same_C) o += bf_n;
+    S.off_cf[0] = (int)o; if (S.bf_in_smem) o += cf_n;
+    S.off_cf[1] = (int)o; if (S.bf_in_smem && !S.same_C) o += cf_n;
+    S.tables_doubles = (int)align_up(o, 2);
+    size_t w = 0;
+    S.o_r = (int)w; w += align_up(3 * (size_t)S.N, 2);
+    S.o_dinv[0] = (int)w; w += align_up((size_t)S.dinv_rows[0] * S.n_up, 2);
+    S.o_dinv[1] = (int)w; w += align_up((size_t)S.dinv_rows[1] * S.n_dn, 2);
+    S.o_moc = (int)w; if (S.moc_in_smem) w += align_up(moc_doubles, 2);
+    S.o_R = (int)w; w += align_up((size_t)S.P, 2);
+    S.o_cum = (int)w; w += align_up((size_t)S.P, 2);
+    S.o_el = (int)w; w += align_up((size_t)LRDMC_EL_ARRAYS * S.N, 2);
+    S.o_U = (int)w; w += 10;                    // the step's lattice frame (9 doubles)
+    S.o_ob = (int)w; w += 8 * (size_t)S.N;      // one-body cache: J1, grad J1, lap J1, v_ei, v^a_ei per electron
+    S.o_j3 = (int)w; if (S.n_j3) w += (size_t)S.N * 2 * LRDMC_J3_MAX + LRDMC_J3_MAX;   // three-body Jastrow: chi3, V3, S3
+    S.per_warp_doubles = (int)w;
+    const size_t per_sm = prop.sharedMemPerMultiprocessor, per_blk_max = prop.sharedMemPerBlockOptin, reserve = 1024;
+    c->wpb = LRDMC_WPB;
+    for (;;) {
+        size_t need = ((size_t)S.tables_doubles + (size_t)c->wpb * S.per_warp_doubles) * 8;
+        if ((need + reserve) * LRDMC_MINB <= per_sm || c->wpb == 1) { c->smem_bytes = (int)need; break; }
+        --c->wpb;
+    }
+    if ((size_t)c->smem_bytes > per_blk_max) return LRDMC_ENOMEM;
+#define SET_SMEM(K) CK(cudaFuncSetAttribute(K, cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem_bytes))
+#define SET_ALL(NTV, TSV) SET_SMEM((k_rebuild<NTV, TSV, false>))
+    SET_ALL(1, true); SET_ALL(2, true); SET_ALL(4, true); SET_ALL(1, false); SET_ALL(2, false); SET_ALL(4, false);
+#undef SET_ALL
+#undef SET_SMEM
+    c->ts = S.bf_in_smem && S.moc_in_smem;
+    if (S.nl_K || S.n_j3) lrdmc_k_set_smem_nl(c->smem_bytes); else lrdmc_k_set_smem_lat(c->smem_bytes);
+    const int occ = (S.nl_K || S.n_j3) ? lrdmc_k_occupancy_nl(c->NT, c->ts, c->wpb * 32, c->smem_bytes) : lrdmc_k_occupancy_lat(c->NT, c->ts, c->wpb * 32, c->smem_bytes);
+    CK(cudaGetLastError());
+    c->ctas_per_sm = occ > 0 ? occ : 1;
+    c->grid_max = c->sm_count * c->ctas_per_sm;
+    return LRDMC_OK;
+}
+
+static int init_device(lrdmc_ctx *c, const std::vector<double> &h_sh, const std::vector<double> &h_nuc, const std::vector<double> &h_et,
+                       const std::vector<double> (&h_bf)[2], const std::vector<double> (&h_cf)[2])
+{
+    DevSys &S = c->S;
+    int ndev = 0; CK(cudaGetDeviceCount(&ndev));
+    const size_t bf_n = c->bf_n, cf_n = c->cf_n;
+    const size_t bytes = (h_sh.size() + h_nuc.size() + h_et.size() + (bf_n + cf_n) * (S.same_C ? 1 : 2)) * sizeof(double);
+    CK(cudaMalloc(&c->d_tables, bytes));
+    double *d = (double *)c->d_tables;
+    CK(cudaMemcpy(d, h_sh.data(), h_sh.size() * 8, cudaMemcpyHostToDevice)); S.shells = d; d += h_sh.size();
+    CK(cudaMemcpy(d, h_nuc.data(), h_nuc.size() * 8, cudaMemcpyHostToDevice)); S.nuc = d; d += h_nuc.size();
+    CK(cudaMemcpy(d, h_et.data(), h_et.size() * 8, cudaMemcpyHostToDevice)); S.etab = d; d += h_et.size();
+    CK(cudaMemcpy(d, h_bf[0].data(), bf_n * 8, cudaMemcpyHostToDevice)); S.bfrag[0] = d; d += bf_n;
+    if (!S.same_C) { CK(cudaMemcpy(d, h_bf[1].data(), bf_n * 8, cudaMemcpyHostToDevice)); S.bfrag[1] = d; d += bf_n; } else S.bfrag[1] = S.bfrag[0];
+    S.cfrag[0] = S.cfrag[1] = d;
+    if (cf_n) {
+        CK(cudaMemcpy(d, h_cf[0].data(), cf_n * 8, cudaMemcpyHostToDevice)); d += cf_n;
+        if (!S.same_C) { CK(cudaMemcpy(d, h_cf[1].data(), cf_n * 8, cudaMemcpyHostToDevice)); S.cfrag[1] = d; }
+    }
+    CK(cudaMalloc((void **)&c->d_stats, sizeof(DevStats)));
+    CK(cudaMemset(c->d_stats, 0, sizeof(DevStats)));
+    CK(cudaMallocHost((void **)&c->h_stats, sizeof(DevStats)));
+    for (int i = 0; i < 4; ++i) CK(cudaEventCreate(&c->ev[i]));
+    return plan_smem(c);
+}
+
 extern "C" int lrdmc_init(lrdmc_ctx **out, const lrdmc_system *sys, const lrdmc_basis *bas, const lrdmc_mo *mo, const lrdmc_jastrow *jas,
                           const lrdmc_lattice *lat)
 {
     if (!out || !sys || !bas || !mo || !jas || !lat) return LRDMC_EINVAL;
     if (sys->n_nuc < 1 || sys->n_up < 1 || sys->n_dn < 0 || sys->n_up > LRDMC_MAX_OCC || sys->n_dn > LRDMC_MAX_OCC) return LRDMC_EINVAL;
     if (bas->n_shell < 1 || !(lat->a > 0.0) || lat->a2 < 0.0 || !sys->Z || !sys->R || !mo->C_up || (sys->n_dn && !mo->C_dn)) return LRDMC_EINVAL;
-    int ndev = 0; CK(cudaGetDeviceCount(&ndev));
     // ---- shells: sort by group (Slater s, s, p, d), pad each group to a multiple of 4
     static const int ncomp[4] = { 1, 1, 3, 6 };
     static const int lmn[4][6][3] = { { {0,0,0} }, { {0,0,0} }, { {1,0,0}, {0,1,0}, {0,0,1} }, { {2,0,0}, {1,1,0}, {1,0,1}, {0,2,0}, {0,1,1}, {0,0,2} } };
@@ -101,6 +187,7 @@ extern "C" int lrdmc_init(lrdmc_ctx **out, const lrdmc_system *sys, const lrdmc_
         Cup = Cfold[0].data(); Cdn = Cfold[1].data();
     } else if (n_ao != mo->n_ao) return LRDMC_EINVAL;
     lrdmc_ctx *c = (lrdmc_ctx *)calloc(1, sizeof(lrdmc_ctx));
+    if (!c) return LRDMC_ENOMEM;
     DevSys &S = c->S;
     S.N = sys->n_up + sys->n_dn; S.n_up = sys->n_up; S.n_dn = sys->n_dn; S.n_nuc = sys->n_nuc;
     S.n_mesh = lat->a2 > 0.0 ? 2 : 1; S.P_lat = 6 * S.N * S.n_mesh; S.a = lat->a;
@@ -195,74 +282,10 @@ extern "C" int lrdmc_init(lrdmc_ctx **out, const lrdmc_system *sys, const lrdmc_
             }
         }
     }
-    // ---- device copies
-    size_t bytes = (h_sh.size() + h_nuc.size() + h_et.size() + (bf_n + cf_n) * (S.same_C ? 1 : 2)) * sizeof(double);
-    cudaError_t ce = cudaMalloc(&c->d_tables, bytes);
-    if (ce != cudaSuccess) { snprintf(g_cuda_msg, sizeof g_cuda_msg, "%s (cudaMalloc tables)", cudaGetErrorString(ce)); free(c); return LRDMC_ECUDA; }
-    double *d = (double *)c->d_tables;
-    cudaMemcpy(d, h_sh.data(), h_sh.size() * 8, cudaMemcpyHostToDevice); S.shells = d; d += h_sh.size();
-    cudaMemcpy(d, h_nuc.data(), h_nuc.size() * 8, cudaMemcpyHostToDevice); S.nuc = d; d += h_nuc.size();
-    cudaMemcpy(d, h_et.data(), h_et.size() * 8, cudaMemcpyHostToDevice); S.etab = d; d += h_et.size();
-    cudaMemcpy(d, h_bf[0].data(), bf_n * 8, cudaMemcpyHostToDevice); S.bfrag[0] = d; d += bf_n;
-    if (!S.same_C) { cudaMemcpy(d, h_bf[1].data(), bf_n * 8, cudaMemcpyHostToDevice); S.bfrag[1] = d; d += bf_n; } else S.bfrag[1] = S.bfrag[0];
-    S.cfrag[0] = S.cfrag[1] = d;
-    if (cf_n) {
-        cudaMemcpy(d, h_cf[0].data(), cf_n * 8, cudaMemcpyHostToDevice); d += cf_n;
-        if (!S.same_C) { cudaMemcpy(d, h_cf[1].data(), cf_n * 8, cudaMemcpyHostToDevice); S.cfrag[1] = d; }
-    }
-    if (cudaMalloc((void **)&c->d_stats, sizeof(DevStats)) != cudaSuccess) { cudaFree(c->d_tables); free(c); return LRDMC_ECUDA; }
-    cudaMemset(c->d_stats, 0, sizeof(DevStats));
-    // ---- shared-memory plan
-    cudaDeviceProp prop; int dev = 0; cudaGetDevice(&dev); cudaGetDeviceProperties(&prop, dev);
-    c->sm_count = prop.multiProcessorCount;
-    const size_t bf_doubles = (bf_n + cf_n) * (S.same_C ? 1 : 2);
-    const size_t moc_doubles = (size_t)S.N * 5 * S.OS;
-    // Either every table and the MO cache sit in shared memory (TS kernels), or the fragment tables and the cache are read
-    // from global memory (large systems; LRDMC_GLOBAL_TABLES forces this path for tests).  No mixed case: a fragment pointer
-    // that may be shared OR global makes nvcc 12.9 infer "shared" for it (cvta.to.shared + ld.shared on a global address).
-    const bool fits = bf_doubles * 8 <= 64 * 1024 && moc_doubles * 8 <= 12 * 1024 && !getenv("LRDMC_GLOBAL_TABLES");
-    S.bf_in_smem = fits; S.moc_in_smem = fits;
-    size_t o = 0;
-    S.off_etab = (int)o; o += 256;              // always first: exp_tab addresses it as (dynamic smem base) + 8 j
-    S.off_shells = (int)o; o += align_up(h_sh.size(), 2);
-    S.off_nuc = (int)o; o += align_up(h_nuc.size(), 2);
-    S.off_bf[0] = (int)o; if (S.bf_in_smem) o += bf_n;
-    S.off_bf[1] = (int)o; if (S.bf_in_smem && !S.same_C) o += bf_n;
-    S.off_cf[0] = (int)o; if (S.bf_in_smem) o += cf_n;
-    S.off_cf[1] = (int)o; if (S.bf_in_smem && !S.same_C) o += cf_n;
-    S.tables_doubles = (int)align_up(o, 2);
-    size_t w = 0;
-    S.o_r = (int)w; w += align_up(3 * (size_t)S.N, 2);
-    S.o_dinv[0] = (int)w; w += align_up((size_t)S.dinv_rows[0] * S.n_up, 2);
-    S.o_dinv[1] = (int)w; w += align_up((size_t)S.dinv_rows[1] * S.n_dn, 2);
-    S.o_moc = (int)w; if (S.moc_in_smem) w += align_up(moc_doubles, 2);
-    S.o_R = (int)w; w += align_up((size_t)S.P, 2);
-    S.o_cum = (int)w; w += align_up((size_t)S.P, 2);
-    S.o_el = (int)w; w += align_up((size_t)LRDMC_EL_ARRAYS * S.N, 2);
-    S.o_U = (int)w; w += 10;                    // the step's lattice frame (9 doubles)
-    S.o_ob = (int)w; w += 8 * (size_t)S.N;      // one-body cache: J1, grad J1, lap J1, v_ei, v^a_ei per electron
-    S.o_j3 = (int)w; if (S.n_j3) w += (size_t)S.N * 2 * LRDMC_J3_MAX + LRDMC_J3_MAX;   // three-body Jastrow: chi3, V3, S3
-    S.per_warp_doubles = (int)w;
-    const size_t per_sm = prop.sharedMemPerMultiprocessor, per_blk_max = prop.sharedMemPerBlockOptin, reserve = 1024;
-    c->wpb = LRDMC_WPB;
-    for (;;) {
-        size_t need = ((size_t)S.tables_doubles + (size_t)c->wpb * S.per_warp_doubles) * 8;
-        if ((need + reserve) * LRDMC_MINB <= per_sm || c->wpb == 1) { c->smem_bytes = (int)need; break; }
-        --c->wpb;
-    }
-    if ((size_t)c->smem_bytes > per_blk_max) { lrdmc_free(c); return LRDMC_ENOMEM; }
-    for (int i = 0; i < 4; ++i) cudaEventCreate(&c->ev[i]);
-#define SET_SMEM(K) cudaFuncSetAttribute(K, cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem_bytes)
-#define SET_ALL(NTV, TSV) SET_SMEM((k_rebuild<NTV, TSV, false>))
-    SET_ALL(1, true); SET_ALL(2, true); SET_ALL(4, true); SET_ALL(1, false); SET_ALL(2, false); SET_ALL(4, false);
-#undef SET_ALL
-#undef SET_SMEM
-    c->ts = S.bf_in_smem && S.moc_in_smem;
-    if (S.nl_K || S.n_j3) lrdmc_k_set_smem_nl(c->smem_bytes); else lrdmc_k_set_smem_lat(c->smem_bytes);
-    const int occ = (S.nl_K || S.n_j3) ? lrdmc_k_occupancy_nl(c->NT, c->ts, c->wpb * 32, c->smem_bytes) : lrdmc_k_occupancy_lat(c->NT, c->ts, c->wpb * 32, c->smem_bytes);
-    c->ctas_per_sm = occ > 0 ? occ : 1;
-    c->grid_max = c->sm_count * c->ctas_per_sm;
-    if (cudaGetLastError() != cudaSuccess) { /* attribute errors surface at launch */ }
+    // ---- device copies (every CUDA call checked; on failure the text moves to the calling thread's slot and the ctx is freed)
+    c->n_sh = h_sh.size(); c->n_nuc_d = h_nuc.size(); c->bf_n = bf_n; c->cf_n = cf_n;
+    const int rc = init_device(c, h_sh, h_nuc, h_et, h_bf, h_cf);
+    if (rc != LRDMC_OK) { snprintf(t_init_msg, sizeof t_init_msg, "%s", c->msg); lrdmc_free(c); return rc; }
     *out = c;
     return LRDMC_OK;
 }
@@ -272,11 +295,28 @@ extern "C" void lrdmc_free(lrdmc_ctx *c)
     if (!c) return;
     if (c->d_tables) cudaFree(c->d_tables);
     if (c->d_stats) cudaFree(c->d_stats);
+    if (c->h_stats) cudaFreeHost(c->h_stats);
     for (int i = 0; i < 4; ++i) if (c->ev[i]) cudaEventDestroy(c->ev[i]);
     free(c);
 }
 
 extern "C" int lrdmc_n_candidates(const lrdmc_ctx *c) { return c ? c->S.P : LRDMC_EINVAL; }
+
+extern "C" const char *lrdmc_last_error(const lrdmc_ctx *c) { return c ? c->msg : t_init_msg; }
+
+extern "C" int lrdmc_set_option(lrdmc_ctx *c, int option, int value)
+{
+    if (!c) return LRDMC_EINVAL;
+    if (c->bound) return LRDMC_ESTATE;            // the walker buffer was carved with the old plan
+    switch (option) {
+    case LRDMC_OPT_TEAM_WARPS:
+        if (value < 0 || value > LRDMC_TEAM_MAX_WARPS) return LRDMC_EINVAL;
+        c->opt_team = value; return LRDMC_OK;
+    case LRDMC_OPT_GLOBAL_TABLES:
+        c->opt_global_tables = value != 0; return plan_smem(c);
+    default: return LRDMC_EINVAL;
+    }
+}
 
 // ---- walker buffer carving -------------------------------------------------------------------------------------
 static size_t carve(const lrdmc_ctx *c, int n_w, char *base, DevWalk *W)
@@ -287,14 +327,14 @@ static size_t carve(const lrdmc_ctx *c, int n_w, char *base, DevWalk *W)
     TAKE(dinv[0], double, nw * S.n_up * S.n_up); TAKE(dinv[1], double, nw * S.n_dn * S.n_dn + 1);
     TAKE(moc, double, nw * S.N * 5 * S.OS); TAKE(moc_alt, double, nw * S.N * 5 * S.OS);
     TAKE(w, double, nw); TAKE(eL, double, nw); TAKE(W, double, nw); TAKE(omega, double, nw);
-    TAKE(nmoves, long long, nw); TAKE(flags, int, nw * 3);
+    TAKE(nmoves, long long, nw); TAKE(flags, int, nw * 3); TAKE(dead, int, nw);
     TAKE(wq, unsigned long long, nw); TAKE(prefix, unsigned long long, nw); TAKE(parents, int, nw);
     {   // parked Bc entries of the team kernel of the large systems (ao_columns BCS): [resident CTA][block of a mesh][k-step pair][lane][2]
         const bool use = LRDMC_BC_STORE && !c->ts;
         const size_t stride = (size_t)((S.n_up + 7) / 8 + (S.n_dn + 7) / 8) * S.n_kpairs * 64;
         const size_t cta_bytes = ((size_t)S.tables_doubles + S.per_warp_doubles) * 8 + 1024;
-        size_t per_sm = 233472 / cta_bytes; if (per_sm > 32) per_sm = 32; if (per_sm < 1) per_sm = 1;      // resident team CTAs per SM, at most
-        if (W) W->bcs_stride = use ? stride : 0;
+        size_t per_sm = c->smem_per_sm / cta_bytes; if (per_sm > 32) per_sm = 32; if (per_sm < 1) per_sm = 1;   // resident team CTAs per SM, at most
+        if (W) { W->bcs_stride = use ? stride : 0; W->bcs_ctas = use ? (int)(per_sm * c->sm_count) : 0; }     // plan_team clamps the grid to this
         TAKE(bcs, double, use ? stride * per_sm * c->sm_count : 0);
         if (W && !use) W->bcs = NULL;
     }
@@ -335,7 +375,7 @@ static void partition_shells(const int n_it[4], const double cost[4], bool pairs
 
 // Choose the team size for n_w walkers.  Warp-per-walker (team_tw = 1) when the walkers alone fill the resident warp slots;
 // otherwise 4 warps per walker: for few walkers (n_w up to 3/8 of the warp slots), and for the large systems whose 36 KB state
-// leaves one warp per scheduler.  LRDMC_TEAM=<tw> forces a size (0/1: never).
+// leaves one warp per scheduler.  lrdmc_set_option(LRDMC_OPT_TEAM_WARPS, tw) forces a size (1: warp-per-walker).
 static void plan_team(lrdmc_ctx *c, int n_w)
 {
     const DevSys &S = c->S; TeamPlan &P = c->team;
@@ -345,7 +385,7 @@ static void plan_team(lrdmc_ctx *c, int n_w)
     if (!c->ts) tw = 4;
     else if ((long)n_w * 8 <= 3 * slots) tw = 4;   // measured on C3/C4 (profiles/r1_team_kernel.md): 4 warps per walker beat 2, 8 and 16 at every N_w,
                                                    // and beat warp-per-walker up to N_w of about 3/8 of the resident warp slots
-    if (const char *e = getenv("LRDMC_TEAM")) { int v = atoi(e); tw = v < 1 ? 1 : v; }
+    if (c->opt_team > 0) tw = c->opt_team;        // LRDMC_OPT_TEAM_WARPS (tests force 1, 2, 4, 8, 16)
     int p2 = 1; while (p2 * 2 <= tw && p2 * 2 <= LRDMC_TEAM_MAX_WARPS) p2 *= 2;
     tw = p2;
     if (tw <= 1) return;
@@ -377,6 +417,7 @@ static void plan_team(lrdmc_ctx *c, int n_w)
     const int occ = (S.nl_K || S.n_j3) ? lrdmc_k_team_occupancy_nl(c->NT, c->ts, tw * 32, smem) : lrdmc_k_team_occupancy_lat(c->NT, c->ts, tw * 32, smem);
     if (cudaGetLastError() != cudaSuccess || occ < 1) return;             // does not fit: stay with warp-per-walker
     c->team_tw = tw; c->team_smem = smem; c->team_ctas_per_sm = occ; c->team_grid_max = c->sm_count * occ;
+    if (c->W.bcs && c->team_grid_max > c->W.bcs_ctas) c->team_grid_max = c->W.bcs_ctas;   // the parked-entry scratch is indexed by blockIdx.x
 }
 
 extern "C" int lrdmc_bind_walkers(lrdmc_ctx *c, void *dev_buf, size_t bytes, int n_walkers)
@@ -385,6 +426,7 @@ extern "C" int lrdmc_bind_walkers(lrdmc_ctx *c, void *dev_buf, size_t bytes, int
     char *base = (char *)align_up((size_t)dev_buf, 256);
     if (carve(c, n_walkers, NULL, NULL) + (size_t)(base - (char *)dev_buf) > bytes) return LRDMC_EINVAL;
     carve(c, n_walkers, base, &c->W);
+    c->W.n_sing = &c->d_stats->n_singular;
     plan_team(c, n_walkers);
     c->W.n_w = n_walkers; c->bound = 1; c->state_ok = 0; c->have_prop = c->have_reconf = 0;
     return LRDMC_OK;
@@ -419,6 +461,8 @@ static void propagate_shape(const lrdmc_ctx *c, int *grid, int *warps)
 static int rebuild(lrdmc_ctx *c, int do_invert /* bit 0: invert, bit 1: the MO cache is valid */, cudaStream_t st)
 {
     CK(cudaMemsetAsync(c->W.counter, 0, 64 * sizeof(int), st));
+    if (do_invert & 1) CK(cudaMemsetAsync(c->W.n_sing, 0, sizeof(long long), st));
+    else CK(cudaMemsetAsync(c->W.dead, 0, sizeof(int) * (size_t)c->W.n_w, st));     // inverses supplied by the caller: nobody is dead
     DISPATCH_NL_(k_rebuild, false, grid_for(c), st, c->S, c->W, do_invert);
     CK(cudaGetLastError());
     return LRDMC_OK;
@@ -543,12 +587,14 @@ extern "C" int lrdmc_estimators(lrdmc_ctx *c, lrdmc_cycle_stats *out)
 {
     if (!c || !out) return LRDMC_EINVAL;
     if (!c->have_prop) return LRDMC_ESTATE;
+    // read back on the stream of the last call and wait for that stream only: other contexts' streams keep running
+    CK(cudaMemcpyAsync(c->h_stats, c->d_stats, sizeof(DevStats), cudaMemcpyDeviceToHost, c->last_stream));
     CK(cudaStreamSynchronize(c->last_stream));
-    DevStats h; CK(cudaMemcpy(&h, c->d_stats, sizeof h, cudaMemcpyDeviceToHost));
+    const DevStats h = *c->h_stats;
     memset(out, 0, sizeof *out);
     out->wbar = c->have_reconf ? h.wbar : 0.0; out->num = h.num; out->den = h.den;
     out->moves_min = h.moves_min; out->moves_max = h.moves_max; out->moves_sum = h.moves_sum;
-    out->n_node_flag = h.n_node; out->n_nonpos_diag = h.n_nonpos; out->n_nonfinite = h.n_nonfinite;
+    out->n_node_flag = h.n_node; out->n_nonpos_diag = h.n_nonpos; out->n_nonfinite = h.n_nonfinite; out->n_singular = h.n_singular;
     out->lockstep_idle_frac = h.moves_max > 0 ? 1.0 - (double)h.moves_sum / ((double)c->W.n_w * (double)h.moves_max) : 0.0;
     out->barrier_idle_frac = (h.span_ns > 0.0 && h.n_warps > 0) ? 1.0 - h.busy_ns / (h.span_ns * h.n_warps) : 0.0;
     cudaEventElapsedTime(&out->propagate_ms, c->ev[0], c->ev[1]);
@@ -574,16 +620,17 @@ extern "C" int lrdmc_bound_walkers(const lrdmc_ctx *c) { return (c && c->bound) 
 extern "C" int lrdmc_n_electrons(const lrdmc_ctx *c) { return c ? c->S.N : 0; }
 extern "C" const DevSys *lrdmc_devsys(const lrdmc_ctx *c) { return &c->S; }
 extern "C" double *lrdmc_positions_ptr(const lrdmc_ctx *c, int which) { return which ? c->W.r_alt : c->W.r; }
-extern "C" int lrdmc_launch_config(const lrdmc_ctx *c, int *grid, int *block, int *smem_bytes, int *ctas_per_sm)
+extern "C" int lrdmc_launch_config(const lrdmc_ctx *c, int *grid, int *block, int *smem_bytes, int *ctas_per_sm, int *team_warps)
 {
     if (!c) return LRDMC_EINVAL;
     if (c->bound && c->team_tw > 1) {            // team mode: one CTA of team_tw warps per walker
         if (grid) *grid = c->W.n_w < c->team_grid_max ? c->W.n_w : c->team_grid_max;
         if (block) *block = c->team_tw * 32; if (smem_bytes) *smem_bytes = c->team_smem; if (ctas_per_sm) *ctas_per_sm = c->team_ctas_per_sm;
+        if (team_warps) *team_warps = c->team_tw;
         return LRDMC_OK;
     }
     int pg = c->grid_max, pw = c->wpb; if (c->bound) propagate_shape(c, &pg, &pw);
     if (grid) *grid = pg; if (block) *block = pw * 32; if (smem_bytes) *smem_bytes = c->smem_bytes;
-    if (ctas_per_sm) *ctas_per_sm = c->ctas_per_sm;
+    if (ctas_per_sm) *ctas_per_sm = c->ctas_per_sm; if (team_warps) *team_warps = 1;
     return LRDMC_OK;
 }

@@ -108,13 +108,19 @@ __global__ void __launch_bounds__(LRDMC_WPB * 32, LRDMC_MINB) k_propagate(DevSys
     bool have = false; int k = 0; uint32_t s = 0;
     double w = 1.0, tau_left = tau; long long moves = 0; int n_node = 0, n_nonpos = 0;
     for (;;) {
-        if (!have) {
+        while (!have) {
             if (lane == 0) k = atomicAdd(W.counter, 1);
             k = __shfl_sync(0xffffffffu, k, 0);
-            if (k < W.n_w) {
-                load_walker<TS>(S, W, ws, T.nuc, k, lane, true);
-                have = true; s = 0; w = 1.0; tau_left = tau; moves = 0; n_node = 0; n_nonpos = 0;
+            if (k >= W.n_w) break;
+            if (W.dead[k]) {                                   // singular at the last (re)build (reading Q24): weight 0, not evaluated
+                if (lane == 0) {
+                    W.w[k] = 0.0; W.eL[k] = 0.0; W.W[k] = 0.0; W.omega[k] = 0.0; W.nmoves[k] = 0;
+                    W.flags[3 * k] = 0; W.flags[3 * k + 1] = 0; W.flags[3 * k + 2] = 0;
+                }
+                continue;
             }
+            load_walker<TS>(S, W, ws, T.nuc, k, lane, true);
+            have = true; s = 0; w = 1.0; tau_left = tau; moves = 0; n_node = 0; n_nonpos = 0;
         }
         if (LRDMC_LOCKSTEP) { if (!__syncthreads_or(have)) break; if (!have) continue; }
         else if (!have) break;
@@ -202,15 +208,21 @@ __global__ void __launch_bounds__(LRDMC_WPB * 32) k_rebuild(DevSys S, DevWalk W,
         }
         __syncwarp();
         if (do_invert & 1) {
+            bool ok = true;
             for (int sp = 0; sp < 2; ++sp) {
                 const int ns = sp ? S.n_dn : S.n_up, off = sp ? S.n_up : 0;
                 if (!ns) continue;
                 double *A = ws.dinv[sp];
                 for (int idx = lane; idx < ns * ns; idx += 32) { int i = idx / ns, m = idx - i * ns; A[idx] = ws.moc[(size_t)(off + i) * 5 * S.OS + m]; }
                 __syncwarp();
-                if (!warp_invert(A, ns, ns, reinterpret_cast<int *>(ws.cum), lane) && lane == 0) atomicOr(W.counter + 1, 1);
+                if (!warp_invert(A, ns, ns, reinterpret_cast<int *>(ws.cum), lane)) ok = false;
                 __syncwarp();
             }
+            if (!ok) {       // reading Q24: a singular walker is dead (zero inverses, weight 0 in the next propagate) and counted
+                for (int sp = 0; sp < 2; ++sp) { const int ns = sp ? S.n_dn : S.n_up; for (int idx = lane; idx < ns * ns; idx += 32) ws.dinv[sp][idx] = 0.0; }
+                if (lane == 0) { atomicOr(W.counter + 1, 1); atomicAdd(reinterpret_cast<unsigned long long *>(W.n_sing), 1ull); }
+            }
+            if (lane == 0) W.dead[k] = ok ? 0 : 1;
         }
         store_walker(S, W, ws, k, lane);
         if (!S.moc_in_smem) ws = warp_views(S, smem, warp);

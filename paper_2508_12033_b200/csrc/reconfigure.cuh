@@ -10,6 +10,7 @@
 struct DevStats {
     double wbar, num, den, busy_ns, span_ns;
     long long moves_min, moves_max, moves_sum, n_node, n_nonpos, n_nonfinite;
+    long long n_singular;          // walkers found singular by the last k_rebuild (reading Q24)
     int n_warps, comb_degenerate;
 };
 

@@ -344,6 +344,14 @@ __global__ void __launch_bounds__(LRDMC_TEAM_MAX_WARPS * 32, 1) k_propagate_team
         __syncthreads();
         const int k = s_ctrl[0];
         if (k >= W.n_w) break;
+        if (W.dead[k]) {                                        // singular at the last (re)build (reading Q24): weight 0, not evaluated
+            if (tid == 0) {
+                W.w[k] = 0.0; W.eL[k] = 0.0; W.W[k] = 0.0; W.omega[k] = 0.0; W.nmoves[k] = 0;
+                W.flags[3 * k] = 0; W.flags[3 * k + 1] = 0; W.flags[3 * k + 2] = 0;
+            }
+            __syncthreads();                                    // everyone has read s_ctrl[0]
+            continue;
+        }
         load_walker_team(S, W, ws, T.nuc, k, P.TW);
         uint32_t s = 0; int reuse_spin = -1;
         double w = 1.0, tau_left = tau, omega = 0.0, eL_last = 0.0, W_last = 0.0; long long moves = 0; int n_node = 0, n_nonpos = 0;

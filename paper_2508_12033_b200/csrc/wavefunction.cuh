@@ -264,10 +264,16 @@ __device__ __forceinline__ void refresh_mo_cache(const DevSys &S, const double *
 }
 
 // In-place Gauss-Jordan inversion with partial (row) pivoting of the n x n matrix A (row stride ld) by one warp.
-// On entry A[i][m] = D[i][m]; on exit A[m][i] = Dinv[m][i] (sum_m D[i][m] Dinv[m][k] = delta_ik).  Returns false on a zero pivot.
+// On entry A[i][m] = D[i][m]; on exit A[m][i] = Dinv[m][i] (sum_m D[i][m] Dinv[m][k] = delta_ik).  Returns false when a pivot
+// is not above 2^-44 max|A_ij| (reading Q24: "|D| = 0" in FP64 -- two identical rows leave a pivot of rounding size, not a zero).
 __device__ __forceinline__ bool warp_invert(double *A, int n, int ld, int *perm, int lane)
 {
     bool ok = true;
+    double amax = 0.0;
+    for (int idx = lane; idx < n * n; idx += 32) amax = fmax(amax, fabs(A[(idx / n) * ld + idx % n]));
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) amax = fmax(amax, __shfl_xor_sync(0xffffffffu, amax, o));
+    const double tiny = ldexp(amax, -44);
     for (int c = 0; c < n; ++c) {
         // pivot search over rows i >= c
         double best = -1.0; int bi = c;
@@ -277,7 +283,7 @@ __device__ __forceinline__ bool warp_invert(double *A, int n, int ld, int *perm,
             double ob = __shfl_xor_sync(0xffffffffu, best, o); int oi = __shfl_xor_sync(0xffffffffu, bi, o);
             if (ob > best || (ob == best && oi < bi)) { best = ob; bi = oi; }
         }
-        if (!(best > 0.0) || isinf(best)) { ok = false; break; }
+        if (!(best > tiny) || isinf(best)) { ok = false; break; }
         if (lane == 0) perm[c] = bi;
         if (bi != c) for (int j = lane; j < n; j += 32) { double tmp = A[c * ld + j]; A[c * ld + j] = A[bi * ld + j]; A[bi * ld + j] = tmp; }
         __syncwarp();

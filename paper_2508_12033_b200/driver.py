@@ -10,13 +10,21 @@ from . import binding as B
 
 
 def work_per_walker_move(sysd):
-    """Algorithmic FP64 flop per walker-move (SURVEY.md 8(d) count; exp = 25 flop):
-    2PAO + P(8S+2A) + 25PS + 12P(N-1+M) + 2PO + [8S+10A+10AO] + 4O^2."""
+    """FP64 flop per walker-move, two counts.
+
+    `total` -- the ALGORITHMIC count of SURVEY.md 8(d) (every candidate through the MOs; exp = 25 flop):
+        2PAO + P(8S+2A) + 25PS + 12P(N-1+M) + 2PO + [8S+10A+10AO] + 4O^2.
+    `executed` -- what the kernels actually run (DESIGN.md section 4, column form): the candidates never go through the MOs;
+        per evaluation Bc = C Dinv costs sum_spin 2 A O n_spin = 2AON and every AO value meets ONE number (2PA), so the terms
+        2PAO + 2PO become 2PA + 2AON; everything else is counted as in `total`.  `total / executed` is the algorithmic saving of
+        the column form; `executed / time` is what the FP64 pipe really delivers (compare ncu sm__pipe_fp64_cycles_active)."""
     N = sysd["n_up"] + sysd["n_dn"]; M = sysd["n_nuc"]; A = sysd["n_ao"]; S = sysd["n_shell"]
     O = max(sysd["n_up"], sysd["n_dn"]); P = 6 * N * (2 if sysd["a2"] > 0 else 1)
     parts = dict(gemm=2 * P * A * O, ao_poly=P * (8 * S + 2 * A), exps=25 * P * S, jastrow=12 * P * (N - 1 + M),
                  ratios=2 * P * O, refresh=8 * S + 10 * A + 10 * A * O, sherman_morrison=4 * O * O)
     parts["total"] = sum(parts.values())
+    parts["column_form"] = 2 * P * A + 2 * A * O * N
+    parts["executed"] = parts["total"] - parts["gemm"] - parts["ratios"] + parts["column_form"]
     return parts
 
 
@@ -26,18 +34,22 @@ def state_bytes_per_walker(sysd):
     return 8 * (3 * N + sysd["n_up"] ** 2 + sysd["n_dn"] ** 2 + N * 5 * OS)
 
 
-def run(g: "B.Lrdmc", mode, cycles, n_moves=0, tau=0.0, E0=0.0, first_cycle=0, feedback=True):
+def run(g: "B.Lrdmc", mode, cycles, n_moves=0, tau=0.0, E0=0.0, first_cycle=0, feedback=True, n_therm=0):
     """Returns the list of per-generation CycleStats.  Balanced: E0 is the Green's-function energy of Eq.28,
-    updated to the running mean of e_n (reading Q8a).  Conventional: E0 is the fixed reference shift (Q8b)."""
-    recs = []; esum = 0.0
-    for c in range(first_cycle, first_cycle + cycles):
+    updated after each branching (L232, Alg.2 line 12 L418) to the running mean of e_n; the mean restarts once, when
+    generation n_therm is reached, so that the equilibration transient does not stay in it (reading Q8a).
+    Conventional: E0 is the fixed reference shift (Q8b)."""
+    recs = []; esum = 0.0; ecnt = 0
+    for i, c in enumerate(range(first_cycle, first_cycle + cycles)):
         g.lrdmc_propagate(mode, n_moves, tau, E0, c)
         g.lrdmc_reconfigure(c)
         s = g.lrdmc_estimators()
         recs.append(s)
-        esum += s.num / s.den
+        if i == n_therm and n_therm > 0:
+            esum = 0.0; ecnt = 0
+        esum += s.num / s.den; ecnt += 1
         if mode == B.BALANCED and feedback:
-            E0 = esum / len(recs)
+            E0 = esum / ecnt
     return recs
 
 

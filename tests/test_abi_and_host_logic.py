@@ -23,14 +23,33 @@ def lib():
     return B.load_library()
 
 
-def test_library_exports_every_declared_symbol(lib):
-    hdr = open(os.path.join(ROOT, "include", "lrdmc.h")).read()
+def _declared(header):
+    hdr = open(os.path.join(ROOT, "include", header)).read()
     hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
-    names = set(re.findall(r"\b(lrdmc_[a-z0-9_]+)\s*\(", hdr))
-    assert {"lrdmc_init", "lrdmc_propagate", "lrdmc_reconfigure", "lrdmc_estimators"} <= names and len(names) >= 18
+    return set(re.findall(r"\b(lrdmc_[a-z0-9_]+)\s*\(", hdr))
+
+
+def test_library_exports_every_declared_symbol(lib):
+    names = _declared("lrdmc.h")
+    assert {"lrdmc_init", "lrdmc_propagate", "lrdmc_reconfigure", "lrdmc_estimators", "lrdmc_set_option", "lrdmc_last_error"} <= names and len(names) >= 20
     for n in sorted(names):
         assert hasattr(lib, n), n
-    assert set(B.EXPORTS) <= names
+    assert set(B.EXPORTS) == names               # the binding's list IS the header's list
+    # every library symbol binding.py touches (L.lrdmc_x / self.L.lrdmc_x / load_library().lrdmc_x) is declared in the header
+    src = open(os.path.join(ROOT, "paper_2508_12033_b200", "binding.py")).read()
+    used = set(re.findall(r"(?:\bL|self\.L|load_library\(\))\.(lrdmc_[a-z0-9_]+)", src))
+    assert used and used <= names, used - names
+    probe_names = _declared("lrdmc_probe.h")
+    assert probe_names == set(B.PROBE_EXPORTS) and not (probe_names & names)
+    assert set(re.findall(r"_probe\.(lrdmc_[a-z0-9_]+)", src)) <= probe_names
+    probe = C.CDLL(B.PROBE_LIB_PATH)
+    for n in probe_names:
+        assert hasattr(probe, n), n
+        assert not hasattr(lib, n), n            # the product library carries no measurement probes
+    # no environment variable steers the product library
+    csrc = os.path.join(ROOT, "paper_2508_12033_b200", "csrc")
+    for f in os.listdir(csrc):
+        assert "getenv" not in open(os.path.join(csrc, f)).read(), f
 
 
 def test_header_declares_only_c_types():
@@ -42,7 +61,9 @@ def test_header_declares_only_c_types():
 
 def test_strerror_and_struct_layout(lib):
     assert lib.lrdmc_strerror(0) == b"ok" and b"singular" in lib.lrdmc_strerror(-2)
-    assert C.sizeof(B.CycleStats) == 96          # 3 doubles, 6 int64, 2 doubles, 2 floats
+    assert lib.lrdmc_last_error(None) is not None      # per-thread slot of a failed lrdmc_init; "" or the CUDA text
+    assert lib.lrdmc_set_option(None, 1, 4) == B.EINVAL
+    assert C.sizeof(B.CycleStats) == 104         # 3 doubles, 7 int64, 2 doubles, 2 floats
 
 
 def test_no_cpu_fallback():

@@ -72,10 +72,10 @@ def _with_walkers(s, n):
     return s, wl.initial_walkers(s, n, 5)
 
 
-def _pair(B, name):
+def _pair(B, name, options=None):
     s, x0 = SYSTEMS[name]()
     o = ref.Ref(s); rc = o.set_positions(x0); assert rc == 0, rc
-    g = B.Lrdmc(s); g.lrdmc_set_positions(x0)
+    g = B.Lrdmc(s, options=options); g.lrdmc_set_positions(x0)
     return s, x0, o, g
 
 
@@ -143,12 +143,13 @@ def test_one_evaluation_and_selection_from_the_oracle_state(B, name):
 @pytest.mark.parametrize("name", list(SYSTEMS))
 @pytest.mark.parametrize("mode", ["balanced", "conventional"])
 @pytest.mark.parametrize("kernel", ["warp-per-walker", "auto"])
-def test_whole_cycle_trajectories_weights_and_branching(B, name, mode, kernel, monkeypatch):
-    """kernel = warp-per-walker forces k_propagate; auto lets lrdmc_bind_walkers pick the team size (k_propagate_team for
-    these small ensembles and for the 64-electron system), as bench.py and a user get it."""
+def test_whole_cycle_trajectories_weights_and_branching(B, name, mode, kernel):
+    """kernel = warp-per-walker forces k_propagate (lrdmc_set_option LRDMC_OPT_TEAM_WARPS = 1); auto lets lrdmc_bind_walkers pick
+    the team size (k_propagate_team for these small ensembles and for the 64-electron system), as bench.py and a user get it."""
+    g = _whole_cycles(B, name, mode, keep=True, options={B.OPT_TEAM_WARPS: 1} if kernel == "warp-per-walker" else None)
     if kernel == "warp-per-walker":
-        monkeypatch.setenv("LRDMC_TEAM", "1")
-    _whole_cycles(B, name, mode)
+        assert g.launch_config()["kernel"] == "k_propagate"
+    g.close()
 
 
 @pytest.mark.parametrize("tw", [2, 4, 8, 16])
@@ -158,25 +159,24 @@ def test_whole_cycle_trajectories_weights_and_branching(B, name, mode, kernel, m
                                        ("tiny-3u2d-nlDLA-strong", "balanced"), ("tiny-2u1d-nlTM-strong", "conventional"), ("C3-water-methane-nlDLA", "balanced"),
                                        ("C3-water-methane-nlTM", "balanced"), ("contracted-4u4d-sph-nlDLA", "balanced"), ("tiny-2u2d-doublemesh-nlTM", "conventional"),
                                        ("tiny-3u2d-pp-J3", "balanced"), ("tiny-3u2d-J3-nlTM", "conventional"), ("C3-water-methane-J3", "balanced")])
-def test_team_kernel_every_team_size(B, name, mode, tw, monkeypatch):
+def test_team_kernel_every_team_size(B, name, mode, tw):
     """k_propagate_team with TW = 2, 4, 8, 16 warps per walker (work units = electron blocks x shell parts, partial sums
     in shared memory): same trajectories, weights and indices as the oracle."""
-    monkeypatch.setenv("LRDMC_TEAM", str(tw))
-    g = _whole_cycles(B, name, mode, n_cycles=1, keep=True)
-    assert g.launch_config()["block"] == 32 * tw
+    g = _whole_cycles(B, name, mode, n_cycles=1, keep=True, options={B.OPT_TEAM_WARPS: tw})
+    cfg = g.launch_config()
+    assert cfg["block"] == 32 * tw and cfg["team_warps"] == tw and cfg["kernel"] == "k_propagate_team"
     g.close()
 
 
 @pytest.mark.parametrize("name", ["C3-water-methane-shaped", "tiny-3u2d-nlDLA-strong", "C5-cluster64-doublemesh"])
-def test_team_kernel_is_bitwise_reproducible(B, name, monkeypatch):
+def test_team_kernel_is_bitwise_reproducible(B, name):
     """compute-sanitizer is not available on the GPU pool; a shared-memory race between the warps of a team would show as
     run-to-run differences.  Three runs of the same cycle from the same state must agree bit for bit (positions, inverses,
     weights, local energies), for the largest team."""
-    monkeypatch.setenv("LRDMC_TEAM", "16")
     s, x0 = SYSTEMS[name]()
     outs = []
     for rep in range(3):
-        g = B.Lrdmc(s); g.lrdmc_set_positions(x0)
+        g = B.Lrdmc(s, options={B.OPT_TEAM_WARPS: 16}); g.lrdmc_set_positions(x0)
         g.lrdmc_propagate(B.BALANCED, 25, 0.0, -5.0, 3)
         outs.append([np_(t).copy() for t in g.lrdmc_get_walkers()] + [np_(t).copy() for t in g.lrdmc_get_obs()])
         assert g.launch_config()["block"] == 512
@@ -186,8 +186,8 @@ def test_team_kernel_is_bitwise_reproducible(B, name, monkeypatch):
             assert np.array_equal(a, b)
 
 
-def _whole_cycles(B, name, mode, n_cycles=2, keep=False):
-    s, x0, o, g = _pair(B, name)
+def _whole_cycles(B, name, mode, n_cycles=2, keep=False, options=None):
+    s, x0, o, g = _pair(B, name, options)
     N = s["n_up"] + s["n_dn"]; n_moves = 30
     for cycle in range(n_cycles):
         if mode == "balanced":
@@ -220,11 +220,10 @@ def _whole_cycles(B, name, mode, n_cycles=2, keep=False):
 
 
 @pytest.mark.parametrize("name", ["C1-hydrogen", "tiny-3u3d-pp", "C3-water-methane-shaped"])
-def test_large_system_path_tables_in_global_memory(B, name, monkeypatch):
+def test_large_system_path_tables_in_global_memory(B, name):
     """The kernels of systems whose tables do not fit shared memory (C5) read fragments and MO cache from global memory;
-    LRDMC_GLOBAL_TABLES forces that path on small systems so that it is compared with the oracle on every run."""
-    monkeypatch.setenv("LRDMC_GLOBAL_TABLES", "1")
-    s, x0, o, g = _pair(B, name)
+    lrdmc_set_option(LRDMC_OPT_GLOBAL_TABLES) forces that path on small systems so that it is compared with the oracle on every run."""
+    s, x0, o, g = _pair(B, name, {B.OPT_GLOBAL_TABLES: 1})
     N = s["n_up"] + s["n_dn"]; Kd = 3 * N / s["a"]**2
     r, du, dd, w = o.get_state(); g.lrdmc_set_state(r, du, dd, w)
     R, scal, js = o.step_debug(-3.0, 2, 1)
@@ -340,6 +339,33 @@ def test_hydrogen_run_energy_matches_oracle_and_exact(B):
     recs_c = drv.run(g, B.CONVENTIONAL, 200, tau=40 * 0.04 / 3, E0=-0.5, first_cycle=1000)
     Ec, sc = B.lrdmc_energy(recs_c, p=10, n_therm=40, n_blocks=10)
     assert abs(Ec - Eg) < 3 * np.hypot(sc, sg) + 1e-3                                     # balanced == conventional (L244)
+    g.close()
+
+
+def test_c2_full_run_energy_matches_the_oracle_run(B):
+    """north_star: "mean energies over full runs within 3 combined standard errors".  BASELINE configs[1] at its full size (C2:
+    1024 walkers x 100 branchings x 50 moves, Alg.2 with the E_0 feedback of L232 / L418), the whole run on the CUDA path and the
+    whole run through the oracle (5.1 M walker-moves on the host cores): the first generations agree to rounding (same seeds, same
+    streams), the run energies within 3 combined sigma."""
+    from paper_2508_12033_b200 import driver as drv
+    s = wl.synthetic10(); x0 = wl.initial_walkers(s, 1024, 5); Kd = 3 * 10 / s["a"]**2
+    g = B.Lrdmc(s); g.lrdmc_set_positions(x0)
+    recs = drv.run(g, B.BALANCED, 100, n_moves=50, E0=0.0, n_therm=20)
+    Eg, sg = B.lrdmc_energy(recs, p=5, n_therm=20, n_blocks=10)
+    ref.set_threads(0)
+    o = ref.Ref(s); assert o.set_positions(x0) == 0
+    out = rdrv.run(o, ref.BALANCED, 100, n_moves=50, E0=0.0, n_therm=20)
+    Eo, so = rdrv.energy(out["wbar"], out["num"], out["den"], p=5, n_therm=20, n_blocks=10)
+    for n in range(5):
+        assert abs(recs[n].num / recs[n].den - out["e"][n]) < 1e-9 * Kd and abs(recs[n].wbar - out["wbar"][n]) < 1e-9 * out["wbar"][n], n
+        assert recs[n].moves_sum == out["moves_sum"][n]
+    assert sum(r.n_nonfinite + r.n_nonpos_diag + r.n_singular for r in recs) == 0 and out["n_nonfinite"].sum() == 0
+    assert abs(Eg - Eo) < 3 * np.hypot(sg, so), (Eg, sg, Eo, so)
+    # how long the two runs stay on one trajectory (reported, not asserted: the first near-tie or 1e-16 difference in a weight separates them)
+    same = 0
+    while same < 100 and abs(recs[same].num / recs[same].den - out["e"][same]) < 1e-6 * Kd:
+        same += 1
+    print(f"C2 full run: GPU {Eg:.5f} +- {sg:.5f}, oracle {Eo:.5f} +- {so:.5f}, generations on one trajectory: {same}")
     g.close()
 
 
@@ -467,6 +493,87 @@ def test_helium_with_three_body_jastrow_still_reaches_the_exact_energy(B):
     assert abs(E0 + 2.903724) < 3 * s0 + 3e-4 and s0 < 3e-3, (E0, s0)
 
 
+# ------------------------------------------------------------------------------------------ the host-buffer entry point (bench.py's e2e number)
+@pytest.mark.parametrize("n_therm", [0, 2])
+def test_run_host_end_to_end_matches_the_oracle_driver(B, n_therm):
+    """lrdmc_run_host (HOST positions in, Alg.2 lines 2-13 with the E_0 feedback of L232 / L418 inside the library, HOST positions
+    out) on C3 with 100 walkers against oracle.ref_driver.run: every generation's num/den and wbar to 1e-9 (a wrong feedback rule --
+    no update, or a mean that does not restart at n_therm -- changes the weights of the following generation), the positions handed
+    back equal lrdmc_get_walkers() bit for bit, the hop counts are exact."""
+    s = wl.water_methane(n_walkers=100); x0 = wl.initial_walkers(s, 100, 5); n_cyc = 4; Kd = 3 * 16 / s["a"]**2
+    g = B.Lrdmc(s)
+    stats, r_out = g.lrdmc_run_host(x0, B.BALANCED, 20, 0.0, 3.0, 11, n_cyc, n_therm=n_therm)
+    o = ref.Ref(s); assert o.set_positions(x0) == 0
+    out = rdrv.run(o, ref.BALANCED, n_cyc, n_moves=20, E0=3.0, first_cycle=11, n_therm=n_therm)
+    assert len(stats) == n_cyc
+    for n in range(n_cyc):
+        assert abs(stats[n].num / stats[n].den - out["e"][n]) < 1e-9 * Kd, n
+        assert abs(stats[n].wbar - out["wbar"][n]) < 1e-9 * out["wbar"][n], n
+        assert abs(stats[n].den - out["den"][n]) < 1e-9 * out["den"][n], n
+        assert stats[n].moves_sum == out["moves_sum"][n] == 20 * 100 and stats[n].n_singular == 0
+    # the feedback really changed E_0 between generations (otherwise the comparison above would not test it)
+    assert len(set(np.round(out["E0_used"], 9))) == n_cyc
+    if n_therm:
+        assert abs(out["E0_used"][3] - out["e"][2]) < 1e-12         # generation 2 restarted the mean
+    gr = np_(g.lrdmc_get_walkers()[0])
+    assert np.array_equal(r_out.numpy(), gr) and np.abs(gr - o.get_state()[0]).max() < 1e-11
+    # conventional mode keeps the shift (Q8b)
+    stats_c, _ = g.lrdmc_run_host(x0, B.CONVENTIONAL, 0, 20 * s["a"]**2 / 48, 5.0, 40, 2)
+    o.set_positions(x0); out_c = rdrv.run(o, ref.CONVENTIONAL, 2, tau=20 * s["a"]**2 / 48, E_ref=5.0, first_cycle=40)
+    for n in range(2):
+        assert abs(stats_c[n].num / stats_c[n].den - out_c["e"][n]) < 1e-9 * Kd and stats_c[n].moves_sum == out_c["moves_sum"][n]
+    g.close()
+
+
+def test_run_host_errors(B):
+    s = wl.tiny_molecule(2, 1, 2, 6, seed=7); g = B.Lrdmc(s)
+    xs = wl.initial_walkers(s, 4, 3)
+    L = g.L; import ctypes as C
+    st = (B.CycleStats * 2)()
+    assert L.lrdmc_run_host(g.h, xs.ctypes.data, None, B.BALANCED, 5, 0.0, 0.0, 0, 2, 0, st, None) == B.ESTATE      # nothing bound
+    g.lrdmc_bind_walkers(4)
+    assert L.lrdmc_run_host(g.h, None, None, B.BALANCED, 5, 0.0, 0.0, 0, 2, 0, st, None) == B.EINVAL
+    assert L.lrdmc_run_host(g.h, xs.ctypes.data, None, B.BALANCED, 5, 0.0, 0.0, 0, 2, -1, st, None) == B.EINVAL
+    bad = xs.copy(); bad[2, 1] = bad[2, 0]                                                # coincident same-spin electrons
+    out = np.full_like(bad, 7.0)
+    assert L.lrdmc_run_host(g.h, bad.ctypes.data, out.ctypes.data, B.BALANCED, 5, 0.0, 0.0, 0, 2, 0, st, None) == B.ESINGULAR
+    assert np.all(out == 7.0)                                                             # nothing propagated, r_out untouched
+    assert L.lrdmc_run_host(g.h, xs.ctypes.data, out.ctypes.data, B.BALANCED, 5, 0.0, -5.0, 0, 2, 0, st, None) == 0
+    assert st[1].moves_sum == 20 and np.array_equal(out, np_(g.lrdmc_get_walkers()[0]))
+    g.close()
+
+
+@pytest.mark.parametrize("tw", [1, 4])
+def test_singular_walkers_are_dead_until_the_next_branching(B, tw):
+    """Reading Q24 on the CUDA path, both kernels, against the oracle: walkers with coincident same-spin electrons are reported
+    (ESINGULAR, n_singular), get zero inverses, leave propagate with w = omega = 0 and no moves, are never parents, and the live
+    walkers beside them follow the oracle's trajectories."""
+    s = wl.tiny_molecule(2, 1, 2, 6, seed=7)
+    x = wl.initial_walkers(s, 70, 3); deadk = [2, 4, 33, 69]
+    for k in deadk:
+        x[k, 1] = x[k, 0]
+    g = B.Lrdmc(s, options={B.OPT_TEAM_WARPS: tw}); o = ref.Ref(s)
+    assert g.lrdmc_set_positions(x, allow_singular=True) == B.ESINGULAR and o.set_positions(x) == -2
+    gr, gdu, gdd, gw = [np_(t) for t in g.lrdmc_get_walkers()]; r, du, dd, w = o.get_state()
+    assert np.all(gdu[deadk] == 0.0) and np.all(gdd[deadk] == 0.0)
+    live = np.setdiff1d(np.arange(70), deadk)
+    assert np.max(np.abs(gdu[live] - du[live]) / np.abs(du[live]).max(axis=(1, 2), keepdims=True)) < 1e-8
+    g.lrdmc_propagate(B.BALANCED, 9, 0.0, -5.0, 0); assert o.propagate(ref.BALANCED, 9, 0.0, -5.0, 0) == 0
+    gr, _, _, gw = [np_(t) for t in g.lrdmc_get_walkers()]; r, _, _, w = o.get_state()
+    geL, gW, gom, gnm = [np_(t) for t in g.lrdmc_get_obs()]; eL, W, om, nm = o.get_obs()
+    assert np.all(gw[deadk] == 0.0) and np.all(gom[deadk] == 0.0) and np.all(gnm[deadk] == 0) and np.array_equal(gnm, nm)
+    assert np.abs(gr - r).max() < 1e-11 and relerr(gw, w) < 1e-9 and relerr(gom, om) < 1e-9
+    par = np_(g.lrdmc_reconfigure(0, want_parents=True)); rc, opar = o.reconfigure(0)
+    assert np.array_equal(par, opar) and not set(deadk) & set(par.tolist())
+    st = g.lrdmc_estimators(); so = o.estimators()
+    assert st.n_singular == so["n_singular"] == 0 and st.moves_sum == so["moves_sum"] == 9 * 66
+    assert abs(st.wbar - so["wbar"]) < 1e-9 * so["wbar"]
+    # before the branching the count of the last rebuild (set_positions) is what the stats carry
+    g.lrdmc_set_positions(x, allow_singular=True); g.lrdmc_propagate(B.BALANCED, 1, 0.0, -5.0, 1)
+    assert g.lrdmc_estimators().n_singular == 4
+    g.close()
+
+
 # ------------------------------------------------------------------------------------------ edge cases and error behaviour
 def test_edge_cases_and_errors(B):
     s = wl.tiny_molecule(2, 1, 2, 6, seed=7); g = B.Lrdmc(s)
@@ -482,8 +589,10 @@ def test_edge_cases_and_errors(B):
             g.lrdmc_propagate(bad["mode"], bad["n_moves"], bad["tau"], 0.0, 0)
         assert e.value.code == B.EINVAL
     xs = wl.initial_walkers(s, 4, 3); xs[2, 1] = xs[2, 0]                                 # coincident same-spin electrons
-    rc = g.lrdmc_set_positions(xs, allow_singular=True)
-    assert rc in (0, B.ESINGULAR)
+    assert g.lrdmc_set_positions(xs, allow_singular=True) == B.ESINGULAR                 # reading Q24: pivot <= 2^-44 max|D|
+    with pytest.raises(B.LrdmcError) as e:
+        g.lrdmc_set_option(B.OPT_TEAM_WARPS, 4)                                          # options come before the walkers are bound
+    assert e.value.code == B.ESTATE
     # W - E0 <= 0 is counted and kills the weight (reading Q16)
     g.lrdmc_set_positions(wl.initial_walkers(s, 8, 3)); o.set_positions(wl.initial_walkers(s, 8, 3))
     g.lrdmc_propagate(B.BALANCED, 3, 0.0, 1e6, 0); o.propagate(ref.BALANCED, 3, 0.0, 1e6, 0)

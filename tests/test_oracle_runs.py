@@ -131,3 +131,36 @@ def test_population_factor_and_energy_estimator():
     assert abs(E - 3.0) < 1e-14
     E, sg = drv.energy(wbar, -0.5 * np.ones(5), den, p=3)
     assert E == -0.5 and sg < 1e-15
+
+
+def test_singular_walkers_are_dead_until_the_next_branching():
+    """Reading Q24: a walker whose Slater matrix is singular (here: two same-spin electrons at one point, and a matrix with a pivot
+    of rounding size) is reported by set_positions (ESINGULAR), gets zero inverses, is never evaluated, leaves propagate with
+    w = omega = 0 and no moves, is never chosen as a parent, and is gone after the branching."""
+    s = wl.tiny_molecule(2, 1, 2, 6, seed=7); o = ref.Ref(s)
+    x = wl.initial_walkers(s, 6, 3); x[2, 1] = x[2, 0]; x[4, 1] = x[4, 0]        # coincident same-spin pairs in walkers 2 and 4
+    assert o.set_positions(x) == -2
+    r, du, dd, w = o.get_state()
+    assert np.all(du[[2, 4]] == 0.0) and np.all(dd[[2, 4]] == 0.0) and np.abs(du[0]).max() > 0
+    rc, du1, dd1 = o.build_inverse(x[2]); assert rc == -2
+    # the live walkers are untouched by their dead neighbours: same trajectories as in an ensemble without them
+    o2 = ref.Ref(s); keep = [0, 1, 3, 5]
+    assert o.propagate(ref.BALANCED, 7, 0.0, -5.0, 0) == 0
+    eL, W, om, nm = o.get_obs(); r1, _, _, w1 = o.get_state()
+    assert np.all(w1[[2, 4]] == 0.0) and np.all(om[[2, 4]] == 0.0) and np.all(nm[[2, 4]] == 0) and np.all(nm[keep] == 7)
+    assert np.array_equal(r1[[2, 4]], x[[2, 4]])
+    for k in keep:
+        o2.set_slot_offset(k); assert o2.set_positions(x[k:k + 1]) == 0
+        assert o2.propagate(ref.BALANCED, 7, 0.0, -5.0, 0) == 0
+        assert np.array_equal(o2.get_state()[0][0], r1[k]) and o2.get_state()[3][0] == w1[k]
+    st = o.estimators(); assert st["n_singular"] == 2 and st["moves_sum"] == 28
+    rc, par = o.reconfigure(0); assert rc == 0
+    assert 2 not in par and 4 not in par
+    assert o.estimators()["n_singular"] == 0 and abs(o.estimators()["wbar"] - w1.sum() / 6) < 1e-12
+    # a matrix with two rows equal up to rounding noise is singular by the 2^-44 rule, a well-conditioned one is not
+    A = np.random.default_rng(0).normal(size=(5, 5)); B_ = A.copy(); B_[3] = A[1] * (1 + 2e-16)
+    import ctypes as C
+    inv = np.zeros((5, 5))
+    f = ref.lib().ref_invert; f.argtypes = [C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+    assert f(5, A.ctypes.data, inv.ctypes.data, None, None) == 0 and np.allclose(inv @ A, np.eye(5), atol=1e-12)
+    assert f(5, B_.ctypes.data, inv.ctypes.data, None, None) == -2
