@@ -69,3 +69,42 @@ def run(o: "ref.Ref", mode, cycles, n_moves=0, tau=0.0, E0=None, E_ref=None, fir
     out = {k: np.array(v) for k, v in rec.items()}
     out["e"] = np.array(e_hist)
     return out
+
+
+def fit_even_powers(a_list, energies, sigmas, n_terms=2):
+    """E(a) = E_0 + c_2 a^2 (+ c_4 a^4): the lattice bias is even in a and vanishes as a -> 0 (L23, L140).  Weighted least squares
+    through the normal equations, written out; returns (E_0, sigma(E_0))."""
+    a = np.asarray(a_list, float); E = np.asarray(energies, float); w = 1.0 / np.asarray(sigmas, float) ** 2
+    M = np.zeros((n_terms, n_terms)); v = np.zeros(n_terms)
+    for k in range(n_terms):
+        for l in range(n_terms):
+            M[k, l] = np.sum(w * a ** (2 * k) * a ** (2 * l))
+        v[k] = np.sum(w * a ** (2 * k) * E)
+    cov = np.linalg.inv(M)
+    return float((cov @ v)[0]), float(np.sqrt(cov[0, 0]))
+
+
+def a_scan(make_system, make_walkers, a_list, n_walkers, cycles, moves, modes=("balanced", "conventional"), E0=0.0, n_therm=None,
+           p=10, n_blocks=10):
+    """The a -> 0 validation in the shape of Table I (L254-L265): one run per lattice spacing and algorithm, one after the other;
+    E(a) per row, then the a -> 0 fit per algorithm (L140).  Run number q (a-major, mode-minor) uses the Philox key
+    seed + 1000003 (q + 1): independent points.  Conventional runs take tau = moves a^2 / (3N) (same mean move count, Q19)."""
+    rows = []
+    for ia, a in enumerate(a_list):
+        row = {"a": a}
+        for im, mode in enumerate(modes):
+            q = ia * len(modes) + im
+            s = dict(make_system(a)); s["seed"] = int(s["seed"]) + 1000003 * (q + 1)
+            N = s["n_up"] + s["n_dn"]
+            o = ref.Ref(s); rc = o.set_positions(make_walkers(s, n_walkers)); assert rc == 0, rc
+            if mode == "balanced":
+                out = run(o, ref.BALANCED, cycles, n_moves=moves, E0=E0)
+            else:
+                out = run(o, ref.CONVENTIONAL, cycles, tau=moves * a * a / (3 * N), E_ref=E0)
+            row[mode] = energy(out["wbar"], out["num"], out["den"], p=p, n_therm=cycles // 5 if n_therm is None else n_therm, n_blocks=n_blocks)
+            row[mode + "_first_e"] = out["e"][:3].copy()
+        rows.append(row)
+    res = {"rows": rows}
+    for mode in modes:
+        res[mode] = fit_even_powers([r["a"] for r in rows], [r[mode][0] for r in rows], [r[mode][1] for r in rows])
+    return res

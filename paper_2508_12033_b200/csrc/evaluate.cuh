@@ -72,6 +72,28 @@ __device__ __forceinline__ void pade_six(double dx, double dy, double dz, const 
     }
 }
 
+// Three-body Jastrow at the six displaced points x0 +- av[k] of one electron (reading Q23): Jn[d] += sum_a chi_a(point d) V_a,
+// the functions dealt over the `stride` lanes that share the electron (t = this lane's index among them, a = a0 + t): six table
+// exponentials per function in the same +- form as the AOs.  The trip count is uniform in the warp (exp_tab_n synchronises it).
+__device__ __forceinline__ void j3_six(const DevSys &S, const Tables &T, const double *V3, double x0, double y0, double z0, const double (&av)[3][3],
+                                       double a2, int t, double (&Jn)[6], int a_first = 0, int a_stride = 4)
+{
+    for (int a0 = a_first; a0 < S.n_j3; a0 += a_stride) {
+        const bool on = a0 + t < S.n_j3; const int a = on ? a0 + t : 0;
+        const double *np_ = T.nuc + S.j3_center[a] * LRDMC_NUC_STRIDE, z = S.j3_zeta[a];
+        const double dx = x0 - np_[0], dy = y0 - np_[1], dz = z0 - np_[2], q0 = fma(dx, dx, fma(dy, dy, fma(dz, dz, a2)));
+        double ex_[6], e_[6];
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            const double sk = fma(av[k][0], dx, fma(av[k][1], dy, av[k][2] * dz));
+            ex_[2 * k] = exp_arg_floor(-z * fma(2.0, sk, q0)); ex_[2 * k + 1] = exp_arg_floor(-z * fma(-2.0, sk, q0));
+        }
+        exp_tab_n<6>(ex_, e_, T.etab);
+#pragma unroll
+        for (int d = 0; d < 6; ++d) Jn[d] = fma(e_[d], on ? V3[a] : 0.0, Jn[d]);
+    }
+}
+
 // ---- non-local pseudopotential candidates (scope row f1; include/lrdmc.h lrdmc_system.nl) ------------------------------
 // The kk-th centre in range of the point (x,y,z): nuclei with r_c > 0 and |r - R_I| < r_c in ascending order.  Returns its index
 // (-1: fewer than kk+1 in range) and the distance.  Every lane runs the same loop on the same data (uniform result).
@@ -94,7 +116,7 @@ __device__ __forceinline__ int nl_centre(const DevSys &S, const double *nuc, dou
 // Dinv column of the slot's electron); nu_q = (1/6) sum_l (2l+1) v_l(r) P_l(+-e_k . rhat).  Two inlined copies of the shell sweep
 // doubled the hot instruction footprint: ncu showed 2.3 "no instruction" stall cycles per issue and the kernel at 35 % issue
 // utilisation.  Returns the node flag raised by the slots (rho_q < 0).
-template <int NT, bool TS>
+template <int NT, bool TS, bool J3>
 __device__ __forceinline__ int phase_b_with_nonlocal(const DevSys &S, const WarpState &ws, const Tables &T, const double *Jold, int lane)
 {
     const int t = lane & 3, g = lane >> 2, N = S.N, K = S.nl_K, n_nuc = S.n_nuc;
@@ -160,23 +182,7 @@ __device__ __forceinline__ int phase_b_with_nonlocal(const DevSys &S, const Warp
                 pade_six(x0 - ws.r[3 * j], y0 - ws.r[3 * j + 1], z0 - ws.r[3 * j + 2], av, a2, c, S.b2, Jn);
             }
         }
-        if (S.n_j3 && (!is_nl || !S.nl_dla)) {                       // three-body Jastrow at the six displaced points: 6 exps per function
-            const double *V3 = ws.j3 + (N + i) * LRDMC_J3_MAX;
-            for (int a0 = 0; a0 < S.n_j3; a0 += 4) {                 // (uniform trip count: exp_tab_n synchronises the warp)
-                const bool on = a0 + t < S.n_j3; const int a = on ? a0 + t : 0;
-                const double *np_ = T.nuc + S.j3_center[a] * LRDMC_NUC_STRIDE, z = S.j3_zeta[a];
-                const double dx = x0 - np_[0], dy = y0 - np_[1], dz = z0 - np_[2], q0 = fma(dx, dx, fma(dy, dy, fma(dz, dz, a2)));
-                double ex_[6], e_[6];
-#pragma unroll
-                for (int k = 0; k < 3; ++k) {
-                    const double sk = fma(av[k][0], dx, fma(av[k][1], dy, av[k][2] * dz));
-                    ex_[2 * k] = exp_arg_floor(-z * fma(2.0, sk, q0)); ex_[2 * k + 1] = exp_arg_floor(-z * fma(-2.0, sk, q0));
-                }
-                exp_tab_n<6>(ex_, e_, T.etab);
-#pragma unroll
-                for (int d = 0; d < 6; ++d) Jn[d] = fma(e_[d], on ? V3[a] : 0.0, Jn[d]);
-            }
-        }
+        if (J3 && (!is_nl || !S.nl_dla)) j3_six(S, T, ws.j3 + (N + i) * LRDMC_J3_MAX, x0, y0, z0, av, a2, t, Jn);
         const double Jo = Jold[i];
         if (!is_nl) {
             double Rv[6];
@@ -211,11 +217,11 @@ __device__ __forceinline__ int phase_b_with_nonlocal(const DevSys &S, const Warp
 }
 
 // Position an accepted move j puts its electron at: lattice hop r_i +- a e_k, or the quadrature point of a non-local slot.
-template <bool NL>
+template <bool SLOTS>
 __device__ __forceinline__ void move_target(const DevSys &S, const WarpState &ws, const double *nuc, int j, int &i, double &px, double &py, double &pz)
 {
     const int N = S.N;
-    if (!NL || j < S.P_lat) {
+    if (!SLOTS || j < S.P_lat) {
         const int mesh = j / (6 * N), jj = j - mesh * 6 * N, d = jj - 6 * (jj / 6), k = d >> 1;
         i = jj / 6;
         const double step = (d & 1) ? -S.amesh[mesh] : S.amesh[mesh];
@@ -232,7 +238,7 @@ __device__ __forceinline__ void move_target(const DevSys &S, const WarpState &ws
 
 // Phase C (row a7) of one evaluation, by one warp on the candidate ratios R[P] left in shared memory.
 // node0: node flag already raised by the non-local candidates (rho_q < 0), any lane.
-template <bool NL = false>
+template <bool SLOTS = false>
 __device__ __forceinline__ EvalOut phase_c(const DevSys &S, const WarpState &ws, const double *lap_s, double Vee, int lane, int node0 = 0)
 {
     const int N = S.N;
@@ -245,10 +251,10 @@ __device__ __forceinline__ EvalOut phase_c(const DevSys &S, const WarpState &ws,
         const int j = j0 + e;
         if (j < P) {
             const double Rj = ws.R[j];
-            const double kap = NL ? (j < 6 * N ? S.kappa[0] : (j < S.P_lat ? S.kappa[1] : 1.0))   // non-local slots hold -nu_q rho_q itself
+            const double kap = SLOTS ? (j < 6 * N ? S.kappa[0] : (j < S.P_lat ? S.kappa[1] : 1.0))   // non-local slots hold -nu_q rho_q itself
                                   : S.kappa[j >= 6 * N ? 1 : 0];
             if (Rj > 0.0) loc += kap * Rj;
-            else if (Rj < 0.0) { vsf_part -= kap * Rj; if (!NL || j < S.P_lat) node = 1; }
+            else if (Rj < 0.0) { vsf_part -= kap * Rj; if (!SLOTS || j < S.P_lat) node = 1; }
             ws.cum[j] = loc;
         }
     }
@@ -280,16 +286,19 @@ __device__ __forceinline__ EvalOut phase_c(const DevSys &S, const WarpState &ws,
     return o;
 }
 
-template <int NT, bool TS, bool NL = false>
+// EXT (extended kernels, separate instantiations so that each system pays only for what it has): bit 0 = non-local
+// pseudopotential slots (row f1), bit 1 = three-body Jastrow (row f2).
+template <int NT, bool TS, int EXT = 0>
 __device__ __forceinline__ EvalOut evaluate_walker(const DevSys &S, const WarpState &ws, const Tables &T, int lane)
 {
+    constexpr bool SLOTS = (EXT & 1) != 0, J3 = (EXT & 2) != 0;
     const int N = S.N, n_nuc = S.n_nuc;
     const int t = lane & 3, g = lane >> 2;
     double *Jold = ws.el, *lap_s = ws.el + N;
 
     // ---- phase A (row a6): per-electron continuum pieces.  Two lanes per electron split the e-e partners; the
     //      one-body parts come from the cache.
-    if (NL && S.n_j3) {                // three-body fields V_a(i) = sum_b g_ab (S_b - chi_b(r_i)),  S_b = sum_j chi_b(r_j)
+    if (J3) {                          // three-body fields V_a(i) = sum_b g_ab (S_b - chi_b(r_i)),  S_b = sum_j chi_b(r_j)
         double *chi3 = ws.j3, *V3 = ws.j3 + N * LRDMC_J3_MAX, *S3 = V3 + N * LRDMC_J3_MAX;
         if (lane < LRDMC_J3_MAX) { double sb = 0.0; for (int j = 0; j < N; ++j) sb += chi3[j * LRDMC_J3_MAX + lane]; S3[lane] = sb; }
         __syncwarp();
@@ -331,7 +340,7 @@ __device__ __forceinline__ EvalOut evaluate_walker(const DevSys &S, const WarpSt
         if (act && sub == 0) {
             const double *ob = ws.ob + 8 * ii;
             gx += ob[1]; gy += ob[2]; gz += ob[3];
-            if (NL && S.n_j3) {        // J3 terms of electron i: sum_a chi_a V_a;  grad chi = -2 zeta d chi;  lap chi = (4 zeta^2 r^2 - 6 zeta) chi
+            if (J3) {                  // J3 terms of electron i: sum_a chi_a V_a;  grad chi = -2 zeta d chi;  lap chi = (4 zeta^2 r^2 - 6 zeta) chi
                 const double *chi3 = ws.j3 + ii * LRDMC_J3_MAX, *V3 = ws.j3 + (N + ii) * LRDMC_J3_MAX;
                 for (int a = 0; a < S.n_j3; ++a) {
                     const double *nu = T.nuc + S.j3_center[a] * LRDMC_NUC_STRIDE, z = S.j3_zeta[a];
@@ -348,7 +357,7 @@ __device__ __forceinline__ EvalOut evaluate_walker(const DevSys &S, const WarpSt
     __syncwarp();
 
     // ---- phase B (rows a1-a5): the 6 n_s candidates of each spin, 8 electrons (48 points) per warp pass in column form
-    if (!NL) for (int mesh = 0; mesh < S.n_mesh; ++mesh) {
+    if (!SLOTS) for (int mesh = 0; mesh < S.n_mesh; ++mesh) {
         const double am = S.amesh[mesh], a2 = am * am;
         double av[3][3];                                             // av[k] = a e_k, e_k = k-th column of U (Eq.D3-D4)
 #pragma unroll
@@ -372,6 +381,7 @@ __device__ __forceinline__ EvalOut evaluate_walker(const DevSys &S, const WarpSt
                     const double c = (j == i) ? 0.0 : ((spin_of(S, j) == sp) ? S.a_par : S.a_anti);
                     pade_six(x0 - ws.r[3 * j], y0 - ws.r[3 * j + 1], z0 - ws.r[3 * j + 2], av, a2, c, S.b2, Jn);
                 }
+                if (J3) j3_six(S, T, ws.j3 + (N + i) * LRDMC_J3_MAX, x0, y0, z0, av, a2, t, Jn);
                 const double Jo = Jold[i];
                 double Rv[6];
 #pragma unroll
@@ -386,10 +396,10 @@ __device__ __forceinline__ EvalOut evaluate_walker(const DevSys &S, const WarpSt
     }
     // ---- systems with non-local pseudopotential slots (row f1): lattice blocks and slot blocks in one loop
     int node_nl = 0;
-    if (NL) node_nl = phase_b_with_nonlocal<NT, TS>(S, ws, T, Jold, lane);
+    if (SLOTS) node_nl = phase_b_with_nonlocal<NT, TS, J3>(S, ws, T, Jold, lane);
     __syncwarp();
 
-    const EvalOut o = phase_c<NL>(S, ws, lap_s, Vee, lane, node_nl);
+    const EvalOut o = phase_c<SLOTS>(S, ws, lap_s, Vee, lane, node_nl);
     __syncwarp();
     return o;
 }
@@ -416,17 +426,17 @@ __device__ __forceinline__ int select_move(const DevSys &S, const WarpState &ws,
 }
 
 // Apply move j (row a10): r_i <- r'_j, refresh the cached MO rows and the one-body cache of electron i, Sherman-Morrison on Dinv_sigma.
-template <int NT, bool TS, bool NL = false>
+template <int NT, bool TS, int EXT = 0>
 __device__ __forceinline__ void apply_move(const DevSys &S, const WarpState &ws, const Tables &T, int j, int lane)
 {
     const int N = S.N; int i; double px, py, pz;
-    move_target<NL>(S, ws, T.nuc, j, i, px, py, pz);
+    move_target<(EXT & 1) != 0>(S, ws, T.nuc, j, i, px, py, pz);
     const int sp = spin_of(S, i), il = sp ? i - S.n_up : i, ns = sp ? S.n_dn : S.n_up;
     double *mc = ws.moc + (size_t)i * 5 * S.OS;
     __syncwarp();
     refresh_mo_cache<NT, TS>(S, T.shells, sp ? T.bf[1] : T.bf[0], T.etab, mc, px, py, pz, lane);
     refresh_onebody(S.n_nuc, S.has_j1, S.a, T.nuc, ws.ob + 8 * i, px, py, pz, lane);
-    if (NL && S.n_j3) refresh_j3_row(S, T.nuc, ws.j3 + i * LRDMC_J3_MAX, px, py, pz, lane);
+    if (EXT & 2) refresh_j3_row(S, T.nuc, ws.j3 + i * LRDMC_J3_MAX, px, py, pz, lane);
     if (lane == 0) { ws.r[3 * i] = px; ws.r[3 * i + 1] = py; ws.r[3 * i + 2] = pz; }
     __syncwarp();
     // s_k = sum_m phi_m Dinv[m][k];  rho = s_il;  Dinv'[m][il] = Dinv[m][il]/rho;  Dinv'[m][k] = Dinv[m][k] - Dinv[m][il] s_k / rho

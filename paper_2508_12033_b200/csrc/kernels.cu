@@ -1,6 +1,7 @@
-// kernels.cu -- the walker kernels' launchers.  This one source is compiled FOUR times (build.py: -DLRDMC_NL=0|1 x
-// -DLRDMC_TEAM_TU=0|1, in parallel): NL = with / without the non-local pseudopotential slots (separate code, so that lattice-only
-// systems keep their register allocation: inlined into one kernel the slots cost 284 B of spills and 9 % of the C4 throughput),
+// kernels.cu -- the walker kernels' launchers.  This one source is compiled EIGHT times (build.py: -DLRDMC_EXT=0|1|2|3 x
+// -DLRDMC_TEAM_TU=0|1, in parallel): EXT bit 0 = non-local pseudopotential slots, bit 1 = three-body Jastrow (separate code, so
+// that every system keeps the register allocation of what it actually has: inlined behind runtime flags the slots cost the
+// lattice-only kernel 284 B of spills and 9 % of the C4 throughput; slots and J3 in one instantiation spilled 196 B),
 // TEAM_TU = the team kernel / the warp-per-walker kernels.  lrdmc.cu (host logic) calls them through kernels.h.
 #include "common.cuh"
 #include "philox.cuh"
@@ -10,15 +11,19 @@
 #include "team.cuh"
 #include "kernels.h"
 
-#ifndef LRDMC_NL
-#error "compile with -DLRDMC_NL=0 or 1"
+#ifndef LRDMC_EXT
+#error "compile with -DLRDMC_EXT=0, 1, 2 or 3"
 #endif
-#if LRDMC_NL
-#define KFN(name) name##_nl
+#if LRDMC_EXT == 0
+#define KFN(name) name##_e0
+#elif LRDMC_EXT == 1
+#define KFN(name) name##_e1
+#elif LRDMC_EXT == 2
+#define KFN(name) name##_e2
 #else
-#define KFN(name) name##_lat
+#define KFN(name) name##_e3
 #endif
-static constexpr bool kNL = LRDMC_NL != 0;
+static constexpr int kNL = LRDMC_EXT;
 
 #define FOR_EACH_NT_TS(X) X(1, true) X(2, true) X(4, true) X(1, false) X(2, false) X(4, false)
 #define PICK(NT_, TS_, STMT)                                                                   \

@@ -1,4 +1,5 @@
-// kernels.h -- launchers of the walker kernels (kernels.cu, compiled once per {lattice-only, non-local} x {warp-per-walker, team});
+// kernels.h -- launchers of the walker kernels (kernels.cu, compiled once per EXT in {0: lattice only, 1: non-local slots, 2: three-body
+// Jastrow, 3: both} x {warp-per-walker, team});
 // internal to liblrdmc, not part of the C-ABI.
 #pragma once
 #include "common.cuh"
@@ -13,6 +14,10 @@
     int lrdmc_k_team_occupancy_##sfx(int NT, int ts, int threads, int smem);                                                                  \
     void lrdmc_k_team_##sfx(int NT, int ts, int grid, int threads, int smem, cudaStream_t st, const DevSys &S, const DevWalk &W,               \
                             const TeamPlan &P, int mode, int n_moves, double tau, double E0, uint32_t cycle);
-LRDMC_K_DECL(lat)
-LRDMC_K_DECL(nl)
+LRDMC_K_DECL(e0)
+LRDMC_K_DECL(e1)
+LRDMC_K_DECL(e2)
+LRDMC_K_DECL(e3)
 #undef LRDMC_K_DECL
+// dispatch on the run-time EXT value of a system
+#define LRDMC_K_CALL(ext, name, ...) ((ext) == 0 ? name##_e0(__VA_ARGS__) : (ext) == 1 ? name##_e1(__VA_ARGS__) : (ext) == 2 ? name##_e2(__VA_ARGS__) : name##_e3(__VA_ARGS__))

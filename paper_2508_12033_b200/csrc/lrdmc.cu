@@ -24,6 +24,7 @@ static thread_local char t_init_msg[256] = "";
 struct lrdmc_ctx {
     DevSys S; DevWalk W;
     void *d_tables; DevStats *d_stats, *h_stats;   // h_stats: pinned staging of the per-generation sums (read back on the ctx's own stream)
+    int ext;        // 0 lattice only, bit 0: non-local slots, bit 1: three-body Jastrow
     int NT, ts, wpb, ctas_per_sm, sm_count, smem_bytes, grid_max; size_t smem_per_sm;
     int bound, have_prop, have_reconf, state_ok;
     cudaEvent_t ev[4]; cudaStream_t last_stream;
@@ -104,8 +105,9 @@ static int plan_smem(lrdmc_ctx *c)
 #undef SET_ALL
 #undef SET_SMEM
     c->ts = S.bf_in_smem && S.moc_in_smem;
-    if (S.nl_K || S.n_j3) lrdmc_k_set_smem_nl(c->smem_bytes); else lrdmc_k_set_smem_lat(c->smem_bytes);
-    const int occ = (S.nl_K || S.n_j3) ? lrdmc_k_occupancy_nl(c->NT, c->ts, c->wpb * 32, c->smem_bytes) : lrdmc_k_occupancy_lat(c->NT, c->ts, c->wpb * 32, c->smem_bytes);
+    c->ext = (S.nl_K ? 1 : 0) | (S.n_j3 ? 2 : 0);     // which instantiation of the walker kernels this system runs (kernels.cu)
+    LRDMC_K_CALL(c->ext, lrdmc_k_set_smem, c->smem_bytes);
+    const int occ = LRDMC_K_CALL(c->ext, lrdmc_k_occupancy, c->NT, c->ts, c->wpb * 32, c->smem_bytes);
     CK(cudaGetLastError());
     c->ctas_per_sm = occ > 0 ? occ : 1;
     c->grid_max = c->sm_count * c->ctas_per_sm;
@@ -414,7 +416,7 @@ static void plan_team(lrdmc_ctx *c, int n_w)
     P.o_nl = (int)scr_lat; P.o_nu = (int)(scr_lat + scr_nl);
     P.o_scr = S.per_warp_doubles; P.scr_doubles = (int)align_up(scr_col > scr_mo ? scr_col : scr_mo, 2);
     const int smem = (int)(((size_t)S.tables_doubles + S.per_warp_doubles + P.scr_doubles) * 8);
-    const int occ = (S.nl_K || S.n_j3) ? lrdmc_k_team_occupancy_nl(c->NT, c->ts, tw * 32, smem) : lrdmc_k_team_occupancy_lat(c->NT, c->ts, tw * 32, smem);
+    const int occ = LRDMC_K_CALL(c->ext, lrdmc_k_team_occupancy, c->NT, c->ts, tw * 32, smem);
     if (cudaGetLastError() != cudaSuccess || occ < 1) return;             // does not fit: stay with warp-per-walker
     c->team_tw = tw; c->team_smem = smem; c->team_ctas_per_sm = occ; c->team_grid_max = c->sm_count * occ;
     if (c->W.bcs && c->team_grid_max > c->W.bcs_ctas) c->team_grid_max = c->W.bcs_ctas;   // the parked-entry scratch is indexed by blockIdx.x
@@ -539,13 +541,8 @@ extern "C" int lrdmc_propagate(lrdmc_ctx *c, int mode, int n_moves, double tau, 
     int grid = team ? (c->W.n_w < c->team_grid_max ? c->W.n_w : c->team_grid_max) : 0, warps = c->wpb;
     if (!team) propagate_shape(c, &grid, &warps);
     CK(cudaEventRecord(c->ev[0], st));
-    if (team) {
-        if (c->S.nl_K || c->S.n_j3) lrdmc_k_team_nl(c->NT, c->ts, grid, c->team_tw * 32, c->team_smem, st, c->S, c->W, c->team, mode, n_moves, tau, E0, (uint32_t)cycle);
-        else lrdmc_k_team_lat(c->NT, c->ts, grid, c->team_tw * 32, c->team_smem, st, c->S, c->W, c->team, mode, n_moves, tau, E0, (uint32_t)cycle);
-    } else {
-        if (c->S.nl_K || c->S.n_j3) lrdmc_k_propagate_nl(c->NT, c->ts, grid, warps * 32, c->smem_bytes, st, c->S, c->W, mode, n_moves, tau, E0, (uint32_t)cycle);
-        else lrdmc_k_propagate_lat(c->NT, c->ts, grid, warps * 32, c->smem_bytes, st, c->S, c->W, mode, n_moves, tau, E0, (uint32_t)cycle);
-    }
+    if (team) LRDMC_K_CALL(c->ext, lrdmc_k_team, c->NT, c->ts, grid, c->team_tw * 32, c->team_smem, st, c->S, c->W, c->team, mode, n_moves, tau, E0, (uint32_t)cycle);
+    else LRDMC_K_CALL(c->ext, lrdmc_k_propagate, c->NT, c->ts, grid, warps * 32, c->smem_bytes, st, c->S, c->W, mode, n_moves, tau, E0, (uint32_t)cycle);
     ++c->launches;
     CK(cudaEventRecord(c->ev[1], st));
     CK(cudaGetLastError());
@@ -608,8 +605,7 @@ extern "C" int lrdmc_step_debug(lrdmc_ctx *c, double E0, uint64_t cycle, uint64_
     if (!c || !R_dev || !scal_dev || !jstar_dev || cycle > 0xFFFFFFFFull || step > 0xFFFFFFFFull) return LRDMC_EINVAL;
     if (!c->bound || !c->state_ok) return LRDMC_ESTATE;
     cudaStream_t st = (cudaStream_t)stream;
-    if (c->S.nl_K || c->S.n_j3) lrdmc_k_step_debug_nl(c->NT, c->ts, grid_for(c), c->wpb * 32, c->smem_bytes, st, c->S, c->W, E0, (uint32_t)cycle, (uint32_t)step, R_dev, scal_dev, jstar_dev);
-    else lrdmc_k_step_debug_lat(c->NT, c->ts, grid_for(c), c->wpb * 32, c->smem_bytes, st, c->S, c->W, E0, (uint32_t)cycle, (uint32_t)step, R_dev, scal_dev, jstar_dev);
+    LRDMC_K_CALL(c->ext, lrdmc_k_step_debug, c->NT, c->ts, grid_for(c), c->wpb * 32, c->smem_bytes, st, c->S, c->W, E0, (uint32_t)cycle, (uint32_t)step, R_dev, scal_dev, jstar_dev);
     ++c->launches;
     CK(cudaGetLastError());
     return LRDMC_OK;

@@ -92,7 +92,7 @@ __device__ __forceinline__ void store_walker(const DevSys &S, const DevWalk &W, 
 }
 
 // ---- the projection kernel (Alg.2 lines 4-8 L401-L410 / Alg.1 lines 4-16 L350-L374) ----------------------------
-template <int NT, bool TS, bool NL>
+template <int NT, bool TS, int EXT>
 __global__ void __launch_bounds__(LRDMC_WPB * 32, LRDMC_MINB) k_propagate(DevSys S, DevWalk W, int mode, int n_moves, double tau, double E0, uint32_t cycle)
 {
     extern __shared__ __align__(16) double smem[];
@@ -126,7 +126,7 @@ __global__ void __launch_bounds__(LRDMC_WPB * 32, LRDMC_MINB) k_propagate(DevSys
         else if (!have) break;
         const StepDraws d = step_draws(S, (uint32_t)k, cycle, s, mode == LRDMC_CONVENTIONAL);
         publish_frame(ws, d, lane);
-        const EvalOut e = evaluate_walker<NT, TS, NL>(S, ws, T, lane);
+        const EvalOut e = evaluate_walker<NT, TS, EXT>(S, ws, T, lane);
         n_node += e.node;
         bool last = false; double omega = 0.0;
         if (mode == LRDMC_BALANCED) {
@@ -145,7 +145,7 @@ __global__ void __launch_bounds__(LRDMC_WPB * 32, LRDMC_MINB) k_propagate(DevSys
         }
         if (!last) {
             const int j = select_move(S, ws, d.u_sel, lane);   // Alg.2 line 7 (L408)
-            if (j >= 0) { apply_move<NT, TS, NL>(S, ws, T, j, lane); ++moves; }
+            if (j >= 0) { apply_move<NT, TS, EXT>(S, ws, T, j, lane); ++moves; }
             ++s;
             continue;
         }
@@ -163,7 +163,7 @@ __global__ void __launch_bounds__(LRDMC_WPB * 32, LRDMC_MINB) k_propagate(DevSys
 }
 
 // ---- parity hook: one evaluation + selection, no state change ---------------------------------------------------
-template <int NT, bool TS, bool NL>
+template <int NT, bool TS, int EXT>
 __global__ void __launch_bounds__(LRDMC_WPB * 32, LRDMC_MINB) k_step_debug(DevSys S, DevWalk W, double E0, uint32_t cycle, uint32_t step, double *R_out,
                                                     double *scal_out, int *jstar_out)
 {
@@ -176,7 +176,7 @@ __global__ void __launch_bounds__(LRDMC_WPB * 32, LRDMC_MINB) k_step_debug(DevSy
         load_walker<TS>(S, W, ws, T.nuc, k, lane, true);
         const StepDraws d = step_draws(S, (uint32_t)k, cycle, step, true);
         publish_frame(ws, d, lane);
-        const EvalOut e = evaluate_walker<NT, TS, NL>(S, ws, T, lane);
+        const EvalOut e = evaluate_walker<NT, TS, EXT>(S, ws, T, lane);
         const int j = select_move(S, ws, d.u_sel, lane);
         for (int p = lane; p < S.P; p += 32) R_out[(size_t)k * S.P + p] = ws.R[p];
         if (lane == 0) {

@@ -48,15 +48,16 @@ __device__ __forceinline__ void store_walker_team(const DevSys &S, const DevWalk
 // BCS: parked Bc entries (wavefunction.cuh, ao_columns): bcs_cta = this CTA's scratch [block of a mesh][k-step pair][lane];
 // reuse_spin = the spin that did not hop since the last evaluation (-1: none).  A unit's entries are parked and taken back by the
 // same warp: unit -> warp is a fixed map, and P.mesh_share says that both meshes of a block land on the same warp.
-template <int NT, bool TS, bool NL, bool BCS>
+template <int NT, bool TS, int EXT, bool BCS>
 __device__ __forceinline__ EvalOut evaluate_team(const DevSys &S, const TeamPlan &P, const WarpState &ws, const Tables &T, double *scr, double *s_vee, int *s_node,
                                                  double2 *bcs_cta, int reuse_spin)
 {
     const int N = S.N, n_nuc = S.n_nuc, TW = P.TW, NP = P.NP, tid = threadIdx.x, nthr = blockDim.x, lane = tid & 31, wt = tid >> 5;
     const int t = lane & 3, g = lane >> 2;
+    constexpr bool NL = (EXT & 1) != 0, J3 = (EXT & 2) != 0;      // non-local slots / three-body Jastrow (separate instantiations)
     double *Jold = ws.el, *lap_s = ws.el + N;
 
-    if (NL && S.n_j3) {                // three-body fields V_a(i) = sum_b g_ab (S_b - chi_b(r_i)),  S_b = sum_j chi_b(r_j)   (evaluate.cuh)
+    if (J3) {                          // three-body fields V_a(i) = sum_b g_ab (S_b - chi_b(r_i)),  S_b = sum_j chi_b(r_j)   (evaluate.cuh)
         double *chi3 = ws.j3, *V3 = ws.j3 + N * LRDMC_J3_MAX, *S3 = V3 + N * LRDMC_J3_MAX;
         if (tid < LRDMC_J3_MAX) { double sb = 0.0; for (int j = 0; j < N; ++j) sb += chi3[j * LRDMC_J3_MAX + tid]; S3[tid] = sb; }
         __syncthreads();
@@ -102,7 +103,7 @@ __device__ __forceinline__ EvalOut evaluate_team(const DevSys &S, const TeamPlan
             if (act && sub == 0) {
                 const double *ob = ws.ob + 8 * ii;
                 gx += ob[1]; gy += ob[2]; gz += ob[3];
-                if (NL && S.n_j3) {    // J3 terms of electron i (as in evaluate_walker)
+                if (J3) {              // J3 terms of electron i (as in evaluate_walker)
                     const double *chi3 = ws.j3 + ii * LRDMC_J3_MAX, *V3 = ws.j3 + (N + ii) * LRDMC_J3_MAX;
                     for (int a = 0; a < S.n_j3; ++a) {
                         const double *nu = T.nuc + S.j3_center[a] * LRDMC_NUC_STRIDE, z = S.j3_zeta[a];
@@ -193,23 +194,8 @@ __device__ __forceinline__ EvalOut evaluate_team(const DevSys &S, const TeamPlan
                 pade_six(x0 - ws.r[3 * j], y0 - ws.r[3 * j + 1], z0 - ws.r[3 * j + 2], av, a2, c, S.b2, Jn);
             }
         }
-        if (NL && S.n_j3 && (!is_nl || !S.nl_dla)) {                 // three-body Jastrow: the functions are dealt over (part, quad lane)
-            const double *V3 = ws.j3 + (N + i) * LRDMC_J3_MAX;
-            for (int a0 = 4 * part; a0 < S.n_j3; a0 += 4 * NP) {     // (trip count uniform in the warp: exp_tab_n synchronises it)
-                const bool on = a0 + t < S.n_j3; const int a = on ? a0 + t : 0;
-                const double *np_ = T.nuc + S.j3_center[a] * LRDMC_NUC_STRIDE, z = S.j3_zeta[a];
-                const double dx = x0 - np_[0], dy = y0 - np_[1], dz = z0 - np_[2], q0 = fma(dx, dx, fma(dy, dy, fma(dz, dz, a2)));
-                double ex_[6], e_[6];
-#pragma unroll
-                for (int k = 0; k < 3; ++k) {
-                    const double sk = fma(av[k][0], dx, fma(av[k][1], dy, av[k][2] * dz));
-                    ex_[2 * k] = exp_arg_floor(-z * fma(2.0, sk, q0)); ex_[2 * k + 1] = exp_arg_floor(-z * fma(-2.0, sk, q0));
-                }
-                exp_tab_n<6>(ex_, e_, T.etab);
-#pragma unroll
-                for (int d = 0; d < 6; ++d) Jn[d] = fma(e_[d], on ? V3[a] : 0.0, Jn[d]);
-            }
-        }
+        if (J3 && (!is_nl || !S.nl_dla))                             // three-body Jastrow: the functions are dealt over (part, quad lane)
+            j3_six(S, T, ws.j3 + (N + i) * LRDMC_J3_MAX, x0, y0, z0, av, a2, t, Jn, 4 * part, 4 * NP);
         double nuq[6];
 #pragma unroll
         for (int d = 0; d < 6; ++d) nuq[d] = 0.0;
@@ -280,12 +266,12 @@ __device__ __forceinline__ EvalOut evaluate_team(const DevSys &S, const TeamPlan
 
 // Apply move j (row a10) by the team: warp w takes part P.mo[w] of the derivative pass of the mover (value, gradient, Laplacian
 // rows by DMMA), the partial rows meet in scr; Sherman-Morrison on Dinv_sigma over all threads.
-template <int NT, bool TS, bool NL>
+template <int NT, bool TS, int EXT>
 __device__ __forceinline__ void apply_move_team(const DevSys &S, const TeamPlan &P, const WarpState &ws, const Tables &T, double *scr, int j)
 {
     const int N = S.N, TW = P.TW, tid = threadIdx.x, nthr = blockDim.x, lane = tid & 31, wt = tid >> 5;   // warp 0 holds the lightest shell part (s shells): it also refreshes the one-body cache
     int i; double px, py, pz;
-    move_target<NL>(S, ws, T.nuc, j, i, px, py, pz);
+    move_target<(EXT & 1) != 0>(S, ws, T.nuc, j, i, px, py, pz);
     const int sp = spin_of(S, i), il = sp ? i - S.n_up : i, ns = sp ? S.n_dn : S.n_up;
     double *mc = ws.moc + (size_t)i * 5 * S.OS;
     const int rows = 5 * S.OS;
@@ -299,7 +285,7 @@ __device__ __forceinline__ void apply_move_team(const DevSys &S, const TeamPlan 
             for (int nt = 0; nt < NT; ++nt) { q[8 * nt + 2 * t] = acc[nt][0]; q[8 * nt + 2 * t + 1] = acc[nt][1]; }
         }
     }
-    if (wt == 0) { refresh_onebody(S.n_nuc, S.has_j1, S.a, T.nuc, ws.ob + 8 * i, px, py, pz, lane); if (NL && S.n_j3) refresh_j3_row(S, T.nuc, ws.j3 + i * LRDMC_J3_MAX, px, py, pz, lane); }
+    if (wt == 0) { refresh_onebody(S.n_nuc, S.has_j1, S.a, T.nuc, ws.ob + 8 * i, px, py, pz, lane); if (EXT & 2) refresh_j3_row(S, T.nuc, ws.j3 + i * LRDMC_J3_MAX, px, py, pz, lane); }
     __syncthreads();                                   // every thread has read the old position
     for (int idx = tid; idx < rows; idx += nthr) {
         double s = 0.0;
@@ -325,7 +311,7 @@ __device__ __forceinline__ void apply_move_team(const DevSys &S, const TeamPlan 
     __syncthreads();
 }
 
-template <int NT, bool TS, bool NL>
+template <int NT, bool TS, int EXT>
 __global__ void __launch_bounds__(LRDMC_TEAM_MAX_WARPS * 32, 1) k_propagate_team(DevSys S, DevWalk W, TeamPlan P, int mode, int n_moves, double tau, double E0, uint32_t cycle)
 {
     extern __shared__ __align__(16) double smem[];
@@ -361,7 +347,7 @@ __global__ void __launch_bounds__(LRDMC_TEAM_MAX_WARPS * 32, 1) k_propagate_team
 #pragma unroll
                 for (int i = 0; i < 9; ++i) ws.U[i] = U[i]; }
             __syncthreads();
-            const EvalOut e = evaluate_team<NT, TS, NL, BCS>(S, P, ws, T, scr, s_vee, &s_ctrl[3], bcs_cta, reuse_spin);
+            const EvalOut e = evaluate_team<NT, TS, EXT, BCS>(S, P, ws, T, scr, s_vee, &s_ctrl[3], bcs_cta, reuse_spin);
             if (wt == 0) {                                       // the leader warp keeps the weight (same rules as k_propagate)
                 n_node += e.node;
                 bool last = false;
@@ -388,7 +374,7 @@ __global__ void __launch_bounds__(LRDMC_TEAM_MAX_WARPS * 32, 1) k_propagate_team
             const bool last = s_ctrl[1] != 0; const int j = s_ctrl[2];
             if (last) break;
             if (j >= 0) {
-                apply_move_team<NT, TS, NL>(S, P, ws, T, scr, j); ++moves;
+                apply_move_team<NT, TS, EXT>(S, P, ws, T, scr, j); ++moves;
                 const int im = j < S.P_lat ? (j % (6 * S.N)) / 6 : (j - S.P_lat) / (6 * S.nl_K);   // the electron that hopped
                 reuse_spin = 1 - spin_of(S, im);
             } else reuse_spin = -1;

@@ -69,24 +69,58 @@ def fit_a_to_zero(a_list, energies, sigmas, n_terms=2):
 
 
 def a_scan(make_system, make_walkers, a_list, n_walkers, cycles, moves, modes=("balanced", "conventional"), E0=0.0, n_therm=None,
-           p=10, n_blocks=10, device="cuda:0"):
-    """One LRDMC run per lattice spacing and mode on the CUDA path; rows shaped like Table I (a, E_balanced, E_conventional).
-    make_system(a) -> system dict; make_walkers(system, n_walkers) -> positions.  Conventional mode uses the projection time with
-    the same mean move count, tau = moves a^2 / (3N) (reading Q19)."""
+           p=10, n_blocks=10, device="cuda:0", concurrent=True, feedback_therm=0):
+    """SURVEY 8(f) f3 "several a in one batch": one LRDMC run per (lattice spacing, mode), ALL of them in flight together on the CUDA
+    path -- every run is a context of its own on a CUDA stream of its own; per generation the propagate + reconfigure of every run
+    is enqueued first, then every run's estimators are read and its E_0 updated, so the small ensembles of an a-scan share the
+    device instead of leaving most SMs idle one after the other (`concurrent=False`: one run after the other, same numbers).
+    Rows shaped like Table I (a, E_balanced, E_conventional; L254-L265), then the E(a) = E_0 + c a^2 fits (L140).
+    make_system(a) -> system dict; make_walkers(system, n_walkers) -> positions.  Run number q (a-major, mode-minor) draws from its
+    own random streams: Philox key = the system's seed + 1000003 (q + 1), so the points of the fit are statistically independent.
+    Conventional mode uses the projection time with the same mean move count, tau = moves a^2 / (3N) (reading Q19)."""
+    import torch
+    runs = []
+    for ia, a in enumerate(a_list):
+        for im, mode in enumerate(modes):
+            q = ia * len(modes) + im
+            sysd = dict(make_system(a)); sysd["seed"] = int(sysd["seed"]) + 1000003 * (q + 1)
+            N = sysd["n_up"] + sysd["n_dn"]
+            g = B.Lrdmc(sysd, device=device)
+            st = torch.cuda.Stream(device=device) if concurrent else torch.cuda.current_stream(device)
+            with torch.cuda.stream(st):
+                g.lrdmc_set_positions(make_walkers(sysd, n_walkers))
+            runs.append(dict(a=a, mode=mode, g=g, stream=st, E0=E0, esum=0.0, ecnt=0, recs=[],
+                             kind=B.BALANCED if mode == "balanced" else B.CONVENTIONAL,
+                             n_moves=moves if mode == "balanced" else 0, tau=0.0 if mode == "balanced" else moves * a * a / (3 * N)))
+
+    def step(batch, c):
+        for r in batch:                                            # enqueue: nothing here waits for the device
+            with torch.cuda.stream(r["stream"]):
+                r["g"].lrdmc_propagate(r["kind"], r["n_moves"], r["tau"], r["E0"], c)
+                r["g"].lrdmc_reconfigure(c)
+        for r in batch:                                            # read back: each call waits for its own stream only
+            s = r["g"].lrdmc_estimators(); r["recs"].append(s)
+            if len(r["recs"]) - 1 == feedback_therm and feedback_therm > 0:
+                r["esum"] = 0.0; r["ecnt"] = 0
+            r["esum"] += s.num / s.den; r["ecnt"] += 1
+            if r["kind"] == B.BALANCED:
+                r["E0"] = r["esum"] / r["ecnt"]                    # "Update E_0" (Alg.2 line 12 L418; reading Q8a)
+    if concurrent:
+        for c in range(cycles):
+            step(runs, c)
+    else:
+        for r in runs:
+            for c in range(cycles):
+                step([r], c)
     rows = []
     for a in a_list:
-        sysd = make_system(a); N = sysd["n_up"] + sysd["n_dn"]
         row = {"a": a}
-        for mode in modes:
-            g = B.Lrdmc(sysd, device=device)
-            g.lrdmc_set_positions(make_walkers(sysd, n_walkers))
-            if mode == "balanced":
-                recs = run(g, B.BALANCED, cycles, n_moves=moves, E0=E0)
-            else:
-                recs = run(g, B.CONVENTIONAL, cycles, tau=moves * a * a / (3 * N), E0=E0)
-            row[mode] = B.lrdmc_energy(recs, p=p, n_therm=cycles // 5 if n_therm is None else n_therm, n_blocks=n_blocks)
-            g.close()
+        for r in runs:
+            if r["a"] == a:
+                row[r["mode"]] = B.lrdmc_energy(r["recs"], p=p, n_therm=cycles // 5 if n_therm is None else n_therm, n_blocks=n_blocks)
         rows.append(row)
+    for r in runs:
+        r["g"].close()
     out = {"rows": rows}
     for mode in modes:
         out[mode] = fit_a_to_zero([r["a"] for r in rows], [r[mode][0] for r in rows], [r[mode][1] for r in rows])

@@ -391,11 +391,13 @@ def test_nonlocal_s_channel_energy_on_the_cuda_path(B):
 
 
 def test_a_to_zero_scan_balanced_vs_conventional_table_shape(B):
-    """SURVEY 8(f) f3, the shape of Table I (L254-L265): at every a the two modes agree within 3 combined sigma, and both
-    E(a) extrapolate to the exact -1/2 Ha of the hydrogen atom (L23, L140) -- on the CUDA path, 2048 walkers."""
+    """SURVEY 8(f) f3, the shape of Table I (L254-L265): several a and both algorithms in ONE batch (8 contexts on 8 streams in
+    flight together).  At every a the two modes agree within 3 combined sigma, both E(a) extrapolate to the exact -1/2 Ha of the
+    hydrogen atom (L23, L140), and the batch equals the same runs made one after the other bit for bit (the runs are independent:
+    concurrency changes nothing but the wall time)."""
     from paper_2508_12033_b200 import driver as drv
-    out = drv.a_scan(lambda a: wl.hydrogen(alpha=0.9, a=a), lambda s, n: wl.hydrogen_walkers(n, 1), [0.15, 0.25, 0.35, 0.45],
-                     n_walkers=2048, cycles=150, moves=30, E0=-0.5)
+    mk = lambda a: wl.hydrogen(alpha=0.9, a=a); mw = lambda s, n: wl.hydrogen_walkers(n, 1); a_list = [0.15, 0.25, 0.35, 0.45]
+    out = drv.a_scan(mk, mw, a_list, n_walkers=2048, cycles=150, moves=30, E0=-0.5)
     for r in out["rows"]:
         (Eb, sb), (Ec, sc) = r["balanced"], r["conventional"]
         assert abs(Eb - Ec) < 3 * np.hypot(sb, sc) + 2e-4, r
@@ -403,6 +405,36 @@ def test_a_to_zero_scan_balanced_vs_conventional_table_shape(B):
     for mode in ("balanced", "conventional"):
         E0, s0, coef, chi2 = out[mode]
         assert abs(E0 + 0.5) < 3 * s0 + 2e-4 and s0 < 1e-3, (mode, E0, s0)
+    seq = drv.a_scan(mk, mw, a_list[:2], n_walkers=2048, cycles=40, moves=30, E0=-0.5, concurrent=False)
+    con = drv.a_scan(mk, mw, a_list[:2], n_walkers=2048, cycles=40, moves=30, E0=-0.5, concurrent=True)
+    for rs, rc in zip(seq["rows"], con["rows"]):
+        assert rs["balanced"] == rc["balanced"] and rs["conventional"] == rc["conventional"]
+
+
+def test_a_to_zero_scan_matches_the_oracle_scan_row_by_row(B):
+    """f3 against the oracle: the same a-scan (same systems, same per-run Philox keys) through oracle.ref_driver.a_scan; every row
+    and both extrapolations within 3 combined sigma, and the first generations of every run equal to rounding."""
+    from paper_2508_12033_b200 import driver as drv
+    mk = lambda a: wl.hydrogen(alpha=0.9, a=a); mw = lambda s, n: wl.hydrogen_walkers(n, 1); a_list = [0.2, 0.3, 0.4]
+    kw = dict(n_walkers=1024, cycles=120, moves=30, E0=-0.5, n_therm=24, p=10, n_blocks=10)
+    ref.set_threads(0)
+    oo = rdrv.a_scan(mk, mw, a_list, **kw)
+    gg = drv.a_scan(mk, mw, a_list, **kw)
+    for ro, rg in zip(oo["rows"], gg["rows"]):
+        for mode in ("balanced", "conventional"):
+            (Eo, so), (Eg, sg) = ro[mode], rg[mode]
+            assert abs(Eo - Eg) < 3 * np.hypot(so, sg) + 1e-12, (ro["a"], mode, Eo, so, Eg, sg)
+            assert 0.3 < sg / so < 3.0                                                    # same statistics, same error bars
+    for mode in ("balanced", "conventional"):
+        assert abs(oo[mode][0] - gg[mode][0]) < 3 * np.hypot(oo[mode][1], gg[mode][1])
+        assert abs(oo[mode][1] - gg[mode][1]) < 0.5 * oo[mode][1]
+    # first generations of one run of the batch against the oracle's run with the same key (q = 3: a = 0.3, conventional)
+    s = dict(mk(0.3)); s["seed"] += 1000003 * 4
+    g = B.Lrdmc(s); g.lrdmc_set_positions(mw(s, 1024))
+    recs = drv.run(g, B.CONVENTIONAL, 3, tau=30 * 0.09 / 3, E0=-0.5)
+    for n in range(3):
+        assert abs(recs[n].num / recs[n].den - oo["rows"][1]["conventional_first_e"][n]) < 1e-9
+    g.close()
 
 
 def test_helium_energies_on_the_cuda_path(B):

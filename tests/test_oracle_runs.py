@@ -164,3 +164,31 @@ def test_singular_walkers_are_dead_until_the_next_branching():
     f = ref.lib().ref_invert; f.argtypes = [C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
     assert f(5, A.ctypes.data, inv.ctypes.data, None, None) == 0 and np.allclose(inv @ A, np.eye(5), atol=1e-12)
     assert f(5, B_.ctypes.data, inv.ctypes.data, None, None) == -2
+
+
+def test_a_scan_fit_closed_forms_and_independent_runs():
+    """oracle.ref_driver.a_scan / fit_even_powers (the oracle side of scope row f3).  The fit against closed forms: exact data
+    E = E_0 + c a^2 are reproduced; for equal error bars sigma(E_0) equals the textbook intercept error of a straight line in
+    a^2; a four-point, three-term fit of exact quartic data returns its intercept.  The scan: every (a, mode) run has its own
+    Philox key (first generations differ between runs that share a and the walkers), rows carry (E, sigma) per mode."""
+    a = np.array([0.1, 0.2, 0.3, 0.4]); x = a**2; sg = np.full(4, 2e-3)
+    E0, s0 = drv.fit_even_powers(a, -0.5 + 0.3 * x, sg)
+    assert abs(E0 + 0.5) < 1e-13
+    assert abs(s0 - 2e-3 * np.sqrt(np.sum(x**2) / (4 * np.sum(x**2) - np.sum(x)**2))) < 1e-15
+    E0, _ = drv.fit_even_powers(a, 1.25 - 2 * x + 7 * x**2, sg, n_terms=3)
+    assert abs(E0 - 1.25) < 1e-11
+    # a point with a tiny error bar pins the curve
+    E0, _ = drv.fit_even_powers([0.0, 0.2, 0.4], [3.0, 9.0, -4.0], [1e-9, 1.0, 1.0])
+    assert abs(E0 - 3.0) < 1e-8
+    mk = lambda a_: wl.hydrogen(alpha=0.9, a=a_); mw = lambda s, n: wl.hydrogen_walkers(n, 1)
+    out = drv.a_scan(mk, mw, [0.2, 0.4], n_walkers=48, cycles=12, moves=8, E0=-0.5, n_blocks=4)
+    assert [r["a"] for r in out["rows"]] == [0.2, 0.4]
+    for r in out["rows"]:
+        for mode in ("balanced", "conventional"):
+            E, s = r[mode]; assert -0.8 < E < -0.3 and s > 0
+    # run q = 0 is what ref_driver.run gives with key seed + 1000003, and differs from a run with the unshifted key
+    s = dict(mk(0.2)); s["seed"] += 1000003
+    o = ref.Ref(s); o.set_positions(mw(s, 48)); e_shift = drv.run(o, ref.BALANCED, 3, n_moves=8, E0=-0.5)["e"]
+    o = ref.Ref(mk(0.2)); o.set_positions(mw(s, 48)); e_plain = drv.run(o, ref.BALANCED, 3, n_moves=8, E0=-0.5)["e"]
+    assert np.array_equal(out["rows"][0]["balanced_first_e"], e_shift) and not np.array_equal(e_shift, e_plain)
+    assert len(out["balanced"]) == 2 and out["balanced"][1] > 0
