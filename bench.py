@@ -121,6 +121,9 @@ def make_workload(args, rank, seed_shift=0):
     elif args.workload == "C3j3":
         sysd = wl.with_jastrow3(wl.water_methane(n_walkers=args.nw, moves=args.moves, seed=seed), 7, 1, strength=0.05)
         wname = "C3/C4 water-methane-shaped system + synthetic three-body Jastrow (8 s Gaussians at the nuclei): scope row f2; flop count = without the J3 part"
+    elif args.workload == "C3j3spd":
+        sysd = wl.with_jastrow3(wl.water_methane(n_walkers=args.nw, moves=args.moves, seed=seed), 8, 3, strength=0.03, n_max=24, poly=True)
+        wname = "C3/C4 water-methane-shaped system + synthetic three-body Jastrow (24 s/p/d Gaussians at the nuclei): scope row f2; flop count = without the J3 part"
     elif args.workload == "C3nl":
         sysd = wl.water_methane_nonlocal(n_walkers=args.nw, moves=args.moves, seed=seed)
         wname = "C3/C4 water-methane-shaped system + synthetic non-local s/p/d pseudopotential channels (r_c = 0.8 bohr, DLA): scope row f1; flop count = lattice part only"
@@ -131,14 +134,14 @@ def make_workload(args, rank, seed_shift=0):
     return sysd, wname, x0
 
 
-def measured_traffic(workload, n_w, kernel):
+def measured_traffic(workload, n_w, kernel, moves):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of the propagate kernel from an `ncu --set full` capture of THIS
     workload (profiles/ncu_traffic_by_workload.md: one table row per captured workload); None if that workload was never captured."""
     try:
         with open(os.path.join(ROOT, "profiles", "ncu_traffic_by_workload.md")) as f:
             for ln in f:
                 c = [t.strip() for t in ln.strip().strip("|").split("|")]
-                if len(c) >= 5 and c[0] == workload and c[1] == str(n_w) and c[2] == kernel:
+                if len(c) >= 5 and c[0] == workload and c[1] == str(n_w) and c[2] == kernel and c[4] == str(moves):
                     return float(c[3])
     except Exception:
         pass
@@ -151,7 +154,7 @@ def main():
     ap.add_argument("--impl", default="ours"); ap.add_argument("--nw", type=int, default=25600); ap.add_argument("--moves", type=int, default=100)
     ap.add_argument("--ref-nw", type=int, default=64); ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-conventional", action="store_true"); ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--workload", default="C4", choices=["C1", "C2", "C4", "C5", "C3nl", "C3j3"],
+    ap.add_argument("--workload", default="C4", choices=["C1", "C2", "C4", "C5", "C3nl", "C3j3", "C3j3spd"],
                     help="C4 (default) is the configuration the metric is quoted on; C2 / C5 are the other BASELINE.json systems, C3nl adds non-local pseudopotential channels (use with --nw/--moves)")
     ap.add_argument("--contexts", type=int, default=1,
                     help="K independent ensembles of --nw walkers each (own context, own CUDA stream, own seed) in flight together: the paper's "
@@ -238,7 +241,7 @@ def main():
     achieved = flop["total"] * per_launch_moves / (prop_ms * 1e-3) / 1e12
     executed = flop["executed"] * per_launch_moves / (prop_ms * 1e-3) / 1e12
     roofline = {"bound": "alu", "kernel": cfg["kernel"], "achieved": achieved, "peak": peaks["dfma_tflops"], "unit": "TFLOP/s", "frac": achieved / peaks["dfma_tflops"],
-                "traffic": measured_traffic(args.workload, args.nw, cfg["kernel"]),
+                "traffic": measured_traffic(args.workload, args.nw, cfg["kernel"], args.moves) if K == 1 else None,
                 "frac_note": "frac = ALGORITHMIC flop (SURVEY 8(d) count, every candidate through the MOs) / kernel time / peak: speed relative to the naive algorithm "
                              "at peak, may exceed 1; frac_executed = flop the column-form kernel executes / kernel time / peak: FP64-pipe utilisation (compare ncu sm__pipe_fp64_cycles_active)",
                 "achieved_executed": executed, "frac_executed": executed / peaks["dfma_tflops"],

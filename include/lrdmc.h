@@ -85,12 +85,14 @@ typedef struct {
     double a_par, a_anti, b2; /* two-body Pade u2 = a r/(1+b2 r), a by spin pair; a = 0 disables */
     const double *c1, *b1;    /* [n_nuc] one-body Pade u1_I = -c1_I r/(1+b1_I r); c1 == NULL disables */
     /* Three-body (electron-electron-nucleus) Jastrow ("2+3-body Jastrow"; form = reading Q23):
-     *   J3 = sum_{i<j} sum_{a,b} g_ab chi_a(r_i) chi_b(r_j),  chi_a(r) = exp(-zeta_a |r - R_{center_a}|^2),  g symmetric.
-     * n_j3 = 0 disables; at most 8 functions. */
+     *   J3 = sum_{i<j} sum_{a,b} g_ab chi_a(r_i) chi_b(r_j),  chi_a(r) = dx^l dy^m dz^n exp(-zeta_a |d|^2),  d = r - R_{center_a},
+     * g symmetric; s, p and cartesian d Gaussians (l + m + n <= 2, unnormalised: a norm is a factor of g).
+     * n_j3 = 0 disables; at most 32 functions (LRDMC_EINVAL beyond). */
     int n_j3;
     const int *j3_center;     /* [n_j3] nucleus index */
     const double *j3_zeta;    /* [n_j3] > 0 */
     const double *j3_g;       /* [n_j3][n_j3] */
+    const int *j3_lmn;        /* [n_j3][3] monomial exponents (l, m, n) of each function; NULL: all s functions */
 } lrdmc_jastrow;
 typedef struct {
     double a;      /* lattice spacing (Eq.D3) */

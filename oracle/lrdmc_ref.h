@@ -50,10 +50,11 @@ int lrdmc_ref_set_contraction(lrdmc_ref_ctx *, int n_cshell, const int *first /*
                               const int *sph /*[n_cshell]*/);
 
 /* Three-body Jastrow (scope row f2; "the Jastrow factor used ... in the TurboRVB calculations", L285 "2+3-body Jastrow"):
- *   J3(x) = sum_{i<j} sum_{a,b} g_ab chi_a(r_i) chi_b(r_j),   chi_a(r) = exp(-zeta_a |r - R_{center_a}|^2)   (s-type Gaussians on nuclei),
+ *   J3(x) = sum_{i<j} sum_{a,b} g_ab chi_a(r_i) chi_b(r_j),   chi_a(r) = dx^l dy^m dz^n exp(-zeta_a |d|^2),  d = r - R_{center_a},
+ * s, p and cartesian d Gaussians on the nuclei: (l, m, n) = lmn[a], l + m + n <= 2, unnormalised (a norm is a factor of g); lmn NULL = all s.
  * g symmetric [n][n] (electron-electron-nucleus terms for a, b on one nucleus, e-e-n-n terms otherwise); added to J of Psi_G = D exp(J).
- * The functional form is named by the paper only: this is reading Q23 of DESIGN.md.  Call right after create. */
-int lrdmc_ref_set_jastrow3(lrdmc_ref_ctx *, int n, const int *center, const double *zeta, const double *g);
+ * Any number of functions.  The functional form is named by the paper only: this is reading Q23 of DESIGN.md.  Call right after create. */
+int lrdmc_ref_set_jastrow3(lrdmc_ref_ctx *, int n, const int *center, const double *zeta, const double *g, const int *lmn /*[n][3] or NULL*/);
 
 /* Non-local (semi-local) pseudopotential, scope row f1 (L242 "DLA", L567 D1 "non-local pseudopotentials", L576 "DTM").
  * nl [n_nuc][7] = { r_c, A_0, B_0, A_1, B_1, A_2, B_2 }: channel l of nucleus I is v_l(r) = A_l exp(-B_l r^2) inside r < r_c

@@ -78,7 +78,7 @@ def lib():
         _lib.lrdmc_ref_set_threads.argtypes = [C.c_int]
         _lib.lrdmc_ref_set_slot_offset.argtypes = [vp, C.c_uint32]
         _lib.lrdmc_ref_set_contraction.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]
-        _lib.lrdmc_ref_set_jastrow3.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]
+        _lib.lrdmc_ref_set_jastrow3.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         _lib.lrdmc_ref_set_nonlocal.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p]
         _lib.lrdmc_ref_nl_info.argtypes = [C.c_void_p] + [C.c_void_p] * 7
         _lib.lrdmc_ref_n_candidates.argtypes = [C.c_void_p]
@@ -143,7 +143,8 @@ class Ref:
         if sysd.get("j3_zeta") is not None:                            # three-body Jastrow (scope row f2)
             jc = np.ascontiguousarray(sysd["j3_center"], dtype=np.int32); jz = np.ascontiguousarray(sysd["j3_zeta"], dtype=np.float64)
             jg = np.ascontiguousarray(sysd["j3_g"], dtype=np.float64)
-            rc = L.lrdmc_ref_set_jastrow3(h, len(jz), jc.ctypes.data, jz.ctypes.data, jg.ctypes.data)
+            jl = None if sysd.get("j3_lmn") is None else np.ascontiguousarray(sysd["j3_lmn"], dtype=np.int32)
+            rc = L.lrdmc_ref_set_jastrow3(h, len(jz), jc.ctypes.data, jz.ctypes.data, jg.ctypes.data, None if jl is None else jl.ctypes.data)
             if rc:
                 raise ValueError(f"lrdmc_ref_set_jastrow3 failed: {rc}")
         self.nl_slots = 0

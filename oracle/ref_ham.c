@@ -34,14 +34,23 @@ static double dist(const double *p, const double *q)
     return sqrt(dx * dx + dy * dy + dz * dz);
 }
 
-/* chi_a(r) = exp(-zeta_a |r - R_a|^2) of the three-body Jastrow, optionally with gradient and Laplacian */
+/* chi_a(r) = dx^l dy^m dz^n exp(-zeta_a |d|^2), d = r - R_a, of the three-body Jastrow (l = m = n = 0 without j3_lmn), optionally
+ * with gradient and Laplacian.  Per axis, u(v) = v^k exp(-zeta v^2):  u' = (k v^(k-1) - 2 zeta v^(k+1)) e,
+ * u'' = (k (k-1) v^(k-2) - 2 zeta (2k+1) v^k + 4 zeta^2 v^(k+2)) e; chi is the product of the three axis functions. */
+static double ipow(double v, int k) { double p = 1.0; for (int q = 0; q < k; ++q) p *= v; return k < 0 ? 0.0 : p; }
 static double j3_chi(const lrdmc_ref_ctx *c, int a, const double r[3], double g[3], double *lap)
 {
     const double *Ra = c->Rn + 3 * c->j3_center[a]; double z = c->j3_zeta[a];
-    double d[3] = { r[0] - Ra[0], r[1] - Ra[1], r[2] - Ra[2] }, r2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2], v = exp(-z * r2);
-    if (g) for (int ax = 0; ax < 3; ++ax) g[ax] = -2.0 * z * d[ax] * v;
-    if (lap) *lap = (4.0 * z * z * r2 - 6.0 * z) * v;
-    return v;
+    double u[3], u1[3], u2[3];
+    for (int ax = 0; ax < 3; ++ax) {
+        int k = c->j3_lmn ? c->j3_lmn[3 * a + ax] : 0; double v = r[ax] - Ra[ax], e = exp(-z * v * v);
+        u[ax] = ipow(v, k) * e;
+        u1[ax] = (k * ipow(v, k - 1) - 2.0 * z * ipow(v, k + 1)) * e;
+        u2[ax] = (k * (k - 1) * ipow(v, k - 2) - 2.0 * z * (2 * k + 1) * ipow(v, k) + 4.0 * z * z * ipow(v, k + 2)) * e;
+    }
+    if (g) { g[0] = u1[0] * u[1] * u[2]; g[1] = u[0] * u1[1] * u[2]; g[2] = u[0] * u[1] * u1[2]; }
+    if (lap) *lap = u2[0] * u[1] * u[2] + u[0] * u2[1] * u[2] + u[0] * u[1] * u2[2];
+    return u[0] * u[1] * u[2];
 }
 /* V_a(i) = sum_{j != i} sum_b g_ab chi_b(r_j): the three-body field electron i feels through basis function a */
 static double j3_field(const lrdmc_ref_ctx *c, const double *x, int i, int a)

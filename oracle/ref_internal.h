@@ -22,8 +22,8 @@ struct lrdmc_ref_ctx {
     /* Jastrow */
     double a_par, a_anti, b2; double *c1, *b1; /* c1 NULL: no one-body term */
     /* three-body (electron-electron-nucleus) Jastrow, scope row f2: J3 = sum_{i<j} sum_{ab} g_ab chi_a(r_i) chi_b(r_j),
-     * chi_a(r) = exp(-zeta_a |r - R_{c_a}|^2), g symmetric [n_j3][n_j3] */
-    int n_j3; int *j3_center; double *j3_zeta, *j3_g;
+     * chi_a(r) = dx^l dy^m dz^n exp(-zeta_a |d|^2), d = r - R_{c_a}, (l,m,n) = j3_lmn[a] (NULL: s functions), g symmetric [n_j3][n_j3] */
+    int n_j3; int *j3_center, *j3_lmn; double *j3_zeta, *j3_g;
     /* lattice */
     double a, a2; int n_mesh; double amesh[2], gmesh[2], kappa[2]; /* kappa_m = g_m / (2 a_m^2) */
     int P;                           /* all candidates: P_lat lattice hops + 6 N nl_K non-local slots */

@@ -59,7 +59,7 @@ void lrdmc_ref_destroy(lrdmc_ref_ctx *c)
     if (!c) return;
     free_walkers(c);
     free(c->Z); free(c->Rn); free(c->pp); free(c->center); free(c->type); free(c->zeta); free(c->ao0);
-    free(c->C_up); free(c->C_dn); free(c->c1); free(c->b1); free(c->nl); free(c->j3_center); free(c->j3_zeta); free(c->j3_g); free(c->cs_first); free(c->cs_sph); free(c->prim_coef); free(c);
+    free(c->C_up); free(c->C_dn); free(c->c1); free(c->b1); free(c->nl); free(c->j3_center); free(c->j3_zeta); free(c->j3_g); free(c->j3_lmn); free(c->cs_first); free(c->cs_sph); free(c->prim_coef); free(c);
 }
 
 int lrdmc_ref_n_candidates(const lrdmc_ref_ctx *c) { return c->P; }
@@ -80,15 +80,17 @@ int lrdmc_ref_set_contraction(lrdmc_ref_ctx *c, int n_cshell, const int *first, 
     return LRDMC_REF_OK;
 }
 
-int lrdmc_ref_set_jastrow3(lrdmc_ref_ctx *c, int n, const int *center, const double *zeta, const double *g)
+int lrdmc_ref_set_jastrow3(lrdmc_ref_ctx *c, int n, const int *center, const double *zeta, const double *g, const int *lmn)
 {
     if (!c || n < 0 || (n > 0 && (!center || !zeta || !g)) || c->n_w) return LRDMC_REF_EINVAL;
     for (int a = 0; a < n; ++a) {
         if (center[a] < 0 || center[a] >= c->n_nuc || !(zeta[a] > 0.0)) return LRDMC_REF_EINVAL;
+        if (lmn && (lmn[3 * a] < 0 || lmn[3 * a + 1] < 0 || lmn[3 * a + 2] < 0 || lmn[3 * a] + lmn[3 * a + 1] + lmn[3 * a + 2] > 2)) return LRDMC_REF_EINVAL;
         for (int b = 0; b < n; ++b) if (g[a * n + b] != g[b * n + a]) return LRDMC_REF_EINVAL;
     }
-    free(c->j3_center); free(c->j3_zeta); free(c->j3_g);
+    free(c->j3_center); free(c->j3_zeta); free(c->j3_g); free(c->j3_lmn);
     c->n_j3 = n; c->j3_center = n ? dupi(center, n) : NULL; c->j3_zeta = dupd(n ? zeta : NULL, n); c->j3_g = dupd(n ? g : NULL, (size_t)n * n);
+    c->j3_lmn = (n && lmn) ? dupi(lmn, 3 * n) : NULL;
     return LRDMC_REF_OK;
 }
 

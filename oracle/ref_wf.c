@@ -196,13 +196,16 @@ int lrdmc_ref_logpsi(const lrdmc_ref_ctx *c, const double *x, double *logabs, in
             J += pade(aij, c->b2, sqrt(dx * dx + dy * dy + dz * dz));
         }
     }
-    /* three-body term, written as defined: sum_{i<j} sum_{ab} g_ab chi_a(r_i) chi_b(r_j) */
+    /* three-body term, written as defined: sum_{i<j} sum_{ab} g_ab chi_a(r_i) chi_b(r_j), chi = monomial (j3_lmn, 1 without) x Gaussian */
     for (int i = 0; i < c->N; ++i) for (int j = i + 1; j < c->N; ++j)
         for (int a = 0; a < c->n_j3; ++a) for (int b = 0; b < c->n_j3; ++b) {
             const double *Ra = c->Rn + 3 * c->j3_center[a], *Rb = c->Rn + 3 * c->j3_center[b];
-            double da2 = 0.0, db2 = 0.0;
-            for (int ax = 0; ax < 3; ++ax) { double u = x[3 * i + ax] - Ra[ax], v = x[3 * j + ax] - Rb[ax]; da2 += u * u; db2 += v * v; }
-            J += c->j3_g[a * c->n_j3 + b] * exp(-c->j3_zeta[a] * da2) * exp(-c->j3_zeta[b] * db2);
+            double da2 = 0.0, db2 = 0.0, pa = 1.0, pb = 1.0;
+            for (int ax = 0; ax < 3; ++ax) {
+                double u = x[3 * i + ax] - Ra[ax], v = x[3 * j + ax] - Rb[ax]; da2 += u * u; db2 += v * v;
+                if (c->j3_lmn) { pa *= pow(u, c->j3_lmn[3 * a + ax]); pb *= pow(v, c->j3_lmn[3 * b + ax]); }
+            }
+            J += c->j3_g[a * c->n_j3 + b] * pa * exp(-c->j3_zeta[a] * da2) * pb * exp(-c->j3_zeta[b] * db2);
         }
     *logabs = la + J; *sign = sg;
     return LRDMC_REF_OK;

@@ -42,7 +42,7 @@ class Mo(C.Structure):
 
 class Jastrow(C.Structure):
     _fields_ = [("a_par", C.c_double), ("a_anti", C.c_double), ("b2", C.c_double), ("c1", C.c_void_p), ("b1", C.c_void_p),
-                ("n_j3", C.c_int), ("j3_center", C.c_void_p), ("j3_zeta", C.c_void_p), ("j3_g", C.c_void_p)]
+                ("n_j3", C.c_int), ("j3_center", C.c_void_p), ("j3_zeta", C.c_void_p), ("j3_g", C.c_void_p), ("j3_lmn", C.c_void_p)]
 
 
 class Lattice(C.Structure):
@@ -159,7 +159,7 @@ class Lrdmc:
         self.sysd = sysd
         self.N = sysd["n_up"] + sysd["n_dn"]; self.n_up = sysd["n_up"]; self.n_dn = sysd["n_dn"]
         k = {n: (None if sysd.get(n) is None else np.ascontiguousarray(sysd[n])) for n in
-             ("Z", "R", "pp", "shell_center", "shell_type", "shell_zeta", "C_up", "C_dn", "c1", "b1", "nl", "cs_first", "prim_coef", "cs_sph", "j3_center", "j3_zeta", "j3_g")}
+             ("Z", "R", "pp", "shell_center", "shell_type", "shell_zeta", "C_up", "C_dn", "c1", "b1", "nl", "cs_first", "prim_coef", "cs_sph", "j3_center", "j3_zeta", "j3_g", "j3_lmn")}
         self._keep = k
         p = lambda a: None if a is None else a.ctypes.data
         s = System(sysd["n_nuc"], p(k["Z"]), p(k["R"]), sysd["n_up"], sysd["n_dn"], p(k["pp"]),
@@ -168,7 +168,7 @@ class Lrdmc:
                   0 if k["cs_sph"] is None else len(k["cs_sph"]), p(k["cs_first"]), p(k["prim_coef"]), p(k["cs_sph"]))
         m = Mo(sysd["n_ao"], p(k["C_up"]), p(k["C_dn"]))
         j = Jastrow(sysd["a_par"], sysd["a_anti"], sysd["b2"], p(k["c1"]), p(k["b1"]),
-                    0 if k["j3_zeta"] is None else len(k["j3_zeta"]), p(k["j3_center"]), p(k["j3_zeta"]), p(k["j3_g"]))
+                    0 if k["j3_zeta"] is None else len(k["j3_zeta"]), p(k["j3_center"]), p(k["j3_zeta"]), p(k["j3_g"]), p(k["j3_lmn"]))
         la = Lattice(sysd["a"], sysd["a2"], sysd["seed"])
         h = C.c_void_p()
         _check(L.lrdmc_init(C.byref(h), C.byref(s), C.byref(b), C.byref(m), C.byref(j), C.byref(la)), "lrdmc_init")

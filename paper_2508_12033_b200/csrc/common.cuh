@@ -22,8 +22,13 @@
 #define LRDMC_NUC_STRIDE 20  // doubles per nucleus row: Rx Ry Rz Z c1 b1 alpha beta gamma delta is_pp pad | r_c A0 B0 A1 B1 A2 B2 pad (non-local channels)
 #define LRDMC_NL_OFF 12      // first non-local entry of a nucleus row
 #define LRDMC_NL_MAX_K 4
-#define LRDMC_J3_MAX 8
+#define LRDMC_J3_MAX 32       // three-body Jastrow functions, at most (lane per function in the row refresh)
 #define LRDMC_EL_ARRAYS 4     // per-electron scratch arrays in shared memory: Jold, lap, s_k, old column
+#define LRDMC_MAX_LG 8        // list groups of the listed candidate sweep: (shell type, chunk of at most 64 sorted shell slots)
+// Screening of the listed candidate sweep: a shell is listed for a row of six displaced points
+// x0 +- step e_k when |x0 - R_shell| < step + srad, srad = sqrt(LRDMC_LIST_THR / zeta) (Gaussians) or LRDMC_LIST_THR / zeta (Slater):
+// every exponent of an unlisted shell is below -LRDMC_LIST_THR in ANY frame (|x0 +- step e - R| >= |x0 - R| - step).
+#define LRDMC_LIST_THR 52.0
 
 // Everything a kernel needs to know about the system; passed by value (fits the 4 KB parameter space).
 struct DevSys {
@@ -38,8 +43,11 @@ struct DevSys {
     int has_j1, has_pp;
     double amesh[2], gmesh[2], kappa[2], g_over_a2[2];
     double a_par, a_anti, b2, V_ii, Kdiag, a;
-    // three-body Jastrow J3 = sum_{i<j} sum_ab g_ab chi_a(r_i) chi_b(r_j), chi_a = exp(-zeta_a |r - R_a|^2) (extended kernels only)
-    int n_j3, j3_center[LRDMC_J3_MAX]; double j3_zeta[LRDMC_J3_MAX], j3_g[LRDMC_J3_MAX * LRDMC_J3_MAX];
+    // three-body Jastrow J3 = sum_{i<j} sum_ab g_ab chi_a(r_i) chi_b(r_j), chi_a = dx^l dy^m dz^n exp(-zeta_a |r - R_a|^2) (extended kernels only)
+    int n_j3, j3s;             // functions; j3s = row stride of the per-walker arrays and of g = n_j3 rounded up to a multiple of 4
+    int j3_poly;               // some function has a monomial factor (p / d functions): l | m << 2 | n << 4 in j3_lmn
+    int j3_center[LRDMC_J3_MAX], j3_lmn[LRDMC_J3_MAX]; double j3_zeta[LRDMC_J3_MAX];
+    const double *j3g; int off_j3g;   // g [j3s][j3s] (zero padded): global copy, staged into the shared tables at off_j3g
     uint32_t key0, key1;
     // device tables (global memory copies; staged into shared memory when they fit)
     const double *shells;      // [n_slots][4] = cx cy cz zeta
@@ -48,10 +56,16 @@ struct DevSys {
     const double *etab;        // [256] 2^(j/256) for exp_tab
     const double *cfrag[2];    // [n_kpairs][2 NT][32] FP64 mma B fragments of the Bc = C Dinv product (ao_columns), norms folded in
     int n_kpairs, off_cf[2];   // pairs of k-steps (each shell group padded to an even number of k-steps)
+    // listed candidate sweep (team kernel of the large systems): sorted slots in list groups of one type and at most 64 slots
+    int n_lg, lg_type[LRDMC_MAX_LG], lg_slot0[LRDMC_MAX_LG], lg_n[LRDMC_MAX_LG], lg_ao0[LRDMC_MAX_LG];
+    int n_aop;                 // AO count of the sorted, padded shell list (slot-major: components of a shell are consecutive)
+    int off_srad, o_am;        // shared memory: srad [n_slots] in the tables; per walker: listed-shell masks [N][n_lg] (64 bit each)
+    const double *srad;        // [n_slots] screening radii (LRDMC_LIST_THR); padded slots: -1e300 (never listed)
+    const double *cn[2];       // [n_aop][OS] MO coefficients with the AO norms folded in, slot-major (Bc = C Dinv by rows)
     // shared-memory plan (units: doubles)
     int bf_in_smem, moc_in_smem;
     int off_shells, off_nuc, off_bf[2], off_etab, tables_doubles;
-    int o_r, o_dinv[2], o_moc, o_R, o_cum, o_el, o_ob, o_U, o_j3, per_warp_doubles;   // o_j3: chi3 [N][8], V3 [N][8], S3 [8] (systems with a J3)
+    int o_r, o_dinv[2], o_moc, o_R, o_cum, o_el, o_ob, o_U, o_j3, per_warp_doubles;   // o_j3: chi3 [N][j3s], V3 [N][j3s], S3 [j3s] (systems with a J3)
     int dinv_rows[2];     // padded row count 8*NT
 };
 
@@ -72,12 +86,14 @@ struct TeamPlan {
     int pair_base[4];     // first k-step pair of each group in the `cf` fragment table
     int mesh_share;       // both meshes of a block are handled by the same warp: the second takes the first's parked Bc entries
     int o_scr, scr_doubles; // scratch (partial sums) behind the walker state, in doubles from the state base
+    int listed;           // the candidate pass is the listed sweep (large systems without slots / J3): rows of RB (mesh, electron) pairs per warp batch
+    int RB;
     ShellPart col[LRDMC_TEAM_MAX_PARTS];     // parts of ao_columns (groups 0-2 start on even iterations: k-step pairs)
     ShellPart mo[LRDMC_TEAM_MAX_WARPS];      // parts of the derivative pass of the mover (one per warp)
 };
 
 // Table pointers as a kernel sees them (shared memory, or global memory for the fragments of the largest systems)
-struct Tables { const double *shells, *nuc, *bf[2], *cf[2], *etab; };
+struct Tables { const double *shells, *nuc, *bf[2], *cf[2], *etab, *srad, *j3g; };
 
 // Walker storage (views into the caller's buffer)
 struct DevWalk {
@@ -97,7 +113,8 @@ struct DevWalk {
     unsigned long long *timing;      // [max_warps][2] globaltimer start/end per resident warp
     double *stats;        // device copy of the reduced numbers (see k_reduce_obs)
     int *counter;         // dynamic walker queue head; [1] = singular flag
-    double *bcs;          // per resident team CTA: parked Bc entries [block of a mesh][k-step pair][lane][2] (ao_columns BCS); NULL if unused
+    double *bcs;          // per resident team CTA: Bc = C Dinv of its walker, [electron][n_aop] (listed sweep, updated rank-1 with the inverse),
+                          // or the parked Bc entries [block of a mesh][k-step pair][lane][2] of ao_columns BCS; NULL if unused
     size_t bcs_stride;    // doubles per CTA
     int bcs_ctas;         // CTAs the scratch was sized for
 };

@@ -8,7 +8,8 @@
 
 struct WarpState {            // per-warp views (shared memory; moc may live in global memory for large systems)
     double *r, *dinv[2], *moc, *R, *cum, *el, *ob, *U;
-    double *j3;               // three-body Jastrow (systems that have one): chi3 [N][8] = chi_a(r_j), then V3 [N][8], then S3 [8]
+    double *j3;               // three-body Jastrow (systems that have one): chi3 [N][j3s] = chi_a(r_j), then V3 [N][j3s], then S3 [j3s]
+    unsigned long long *am;   // listed sweep (large systems): listed-shell masks [N][n_lg]
 };
 struct EvalOut { double bbar, Vsf, W, eL; int node; };
 
@@ -45,17 +46,71 @@ __device__ __forceinline__ void refresh_onebody(int n_nuc, int has_j1, double a_
     if (lane == 0) { ob_i[0] = J; ob_i[1] = gx; ob_i[2] = gy; ob_i[3] = gz; ob_i[4] = lJ; ob_i[5] = vei; ob_i[6] = vb; }
 }
 
-// Three-body Jastrow (reading Q23): chi_a(r) = exp(-zeta_a |r - R_a|^2) of electron j, lanes a < 8 (zero beyond n_j3).
+// Three-body Jastrow (reading Q23): chi_a(r) = dx^l dy^m dz^n exp(-zeta_a |r - R_a|^2) of electron j, lane per function (zero beyond n_j3).
+__device__ __forceinline__ double mono_pow(double v, int k) { return k == 0 ? 1.0 : (k == 1 ? v : v * v); }     // v^k, k = 0, 1, 2
 __device__ __forceinline__ void refresh_j3_row(const DevSys &S, const double *nuc, double *chi3_j, double x, double y, double z, int lane)
 {
-    if (lane < LRDMC_J3_MAX) {
+    if (lane < S.j3s) {
         double v = 0.0;
         if (lane < S.n_j3) {
             const double *nu = nuc + S.j3_center[lane] * LRDMC_NUC_STRIDE;
             const double dx = x - nu[0], dy = y - nu[1], dz = z - nu[2];
             v = exp_nonpos(-S.j3_zeta[lane] * (dx * dx + dy * dy + dz * dz));
+            if (S.j3_poly) { const int q = S.j3_lmn[lane]; v *= mono_pow(dx, q & 3) * mono_pow(dy, (q >> 2) & 3) * mono_pow(dz, (q >> 4) & 3); }
         }
         chi3_j[lane] = v;
+    }
+}
+
+// The fields V_a(i) = sum_b g_ab (S_b - chi_b(r_i)), S_b = sum_j chi_b(r_j), of all electrons (start of every evaluation) by the threads
+// tid = 0 .. nthr-1 of a warp (SYNC = __syncwarp) or of a CTA (__syncthreads): j3 = chi3 [N][j3s], V3 [N][j3s], S3 [j3s]; g staged in the tables.
+template <typename SYNC>
+__device__ __forceinline__ void j3_fields(const DevSys &S, const double *__restrict__ g3, double *j3, int tid, int nthr, SYNC sync)
+{
+    const int N = S.N, J = S.j3s;
+    double *chi3 = j3, *V3 = j3 + N * J, *S3 = V3 + N * J;
+    for (int b = tid; b < J; b += nthr) { double sb = 0.0; for (int j = 0; j < N; ++j) sb += chi3[j * J + b]; S3[b] = sb; }
+    sync();
+    for (int idx = tid; idx < N * J; idx += nthr) {
+        const int i = idx / J, a = idx - i * J;
+        double v = 0.0;
+        for (int b = 0; b < J; b += 4) {
+#pragma unroll
+            for (int q = 0; q < 4; ++q) v += g3[a * J + b + q] * (S3[b + q] - chi3[i * J + b + q]);
+        }
+        V3[idx] = v;
+    }
+    sync();
+}
+
+// J3 terms of electron i in the continuum pieces (phase A): J += sum_a chi_a V_a, grad and Laplacian alike.  s functions:
+// grad chi = -2 zeta d chi, lap chi = (4 zeta^2 r^2 - 6 zeta) chi.  With monomials, per axis u(v) = v^k e^{-zeta v^2}:
+// u' = (k v^(k-1) - 2 zeta v^(k+1)) e, u'' = (k (k-1) v^(k-2) - 2 zeta (2k+1) v^k + 4 zeta^2 v^(k+2)) e, chi = product of the three axes.
+__device__ __forceinline__ void j3_axis(double v, int k, double z, double &f, double &f1, double &f2)
+{
+    const double v2 = v * v, tz = 2.0 * z, fz2 = 4.0 * z * z;
+    f = mono_pow(v, k);
+    f1 = k == 0 ? -tz * v : (k == 1 ? 1.0 - tz * v2 : (2.0 - tz * v2) * v);
+    f2 = k == 0 ? fz2 * v2 - tz : (k == 1 ? (fz2 * v2 - 3.0 * tz) * v : 2.0 + (fz2 * v2 - 5.0 * tz) * v2);
+}
+__device__ __forceinline__ void j3_electron_terms(const DevSys &S, const double *nuc, const double *chi3_i, const double *V3_i, double xi, double yi, double zi,
+                                                  double &J, double &gx, double &gy, double &gz, double &lJ)
+{
+    for (int a = 0; a < S.n_j3; ++a) {
+        const double *nu = nuc + S.j3_center[a] * LRDMC_NUC_STRIDE, z = S.j3_zeta[a];
+        const double dx = xi - nu[0], dy = yi - nu[1], dz = zi - nu[2], V = V3_i[a];
+        const int q = S.j3_poly ? S.j3_lmn[a] : 0;
+        if (q == 0) {
+            const double cv = chi3_i[a] * V, tz = -2.0 * z * cv;
+            J += cv; gx += tz * dx; gy += tz * dy; gz += tz * dz;
+            lJ += (4.0 * z * z * (dx * dx + dy * dy + dz * dz) - 6.0 * z) * cv;
+        } else {
+            const double eV = exp_nonpos(-z * (dx * dx + dy * dy + dz * dz)) * V;
+            double fx, fx1, fx2, fy, fy1, fy2, fz, fz1, fz2;
+            j3_axis(dx, q & 3, z, fx, fx1, fx2); j3_axis(dy, (q >> 2) & 3, z, fy, fy1, fy2); j3_axis(dz, (q >> 4) & 3, z, fz, fz1, fz2);
+            J += chi3_i[a] * V; gx += fx1 * fy * fz * eV; gy += fx * fy1 * fz * eV; gz += fx * fy * fz1 * eV;
+            lJ += (fx2 * fy * fz + fx * fy2 * fz + fx * fy * fz2) * eV;
+        }
     }
 }
 
@@ -89,8 +144,19 @@ __device__ __forceinline__ void j3_six(const DevSys &S, const Tables &T, const d
             ex_[2 * k] = exp_arg_floor(-z * fma(2.0, sk, q0)); ex_[2 * k + 1] = exp_arg_floor(-z * fma(-2.0, sk, q0));
         }
         exp_tab_n<6>(ex_, e_, T.etab);
+        const double Va = on ? V3[a] : 0.0;
+        if (S.j3_poly) {               // monomial factor at the displaced points d0 +- av[k] (uniform branch: a property of the system)
+            const int q = S.j3_lmn[a], kx = q & 3, ky = (q >> 2) & 3, kz = (q >> 4) & 3;
 #pragma unroll
-        for (int d = 0; d < 6; ++d) Jn[d] = fma(e_[d], on ? V3[a] : 0.0, Jn[d]);
+            for (int k = 0; k < 3; ++k) {
+                const double pp = mono_pow(dx + av[k][0], kx) * mono_pow(dy + av[k][1], ky) * mono_pow(dz + av[k][2], kz);
+                const double pm = mono_pow(dx - av[k][0], kx) * mono_pow(dy - av[k][1], ky) * mono_pow(dz - av[k][2], kz);
+                Jn[2 * k] = fma(e_[2 * k] * pp, Va, Jn[2 * k]); Jn[2 * k + 1] = fma(e_[2 * k + 1] * pm, Va, Jn[2 * k + 1]);
+            }
+        } else {
+#pragma unroll
+            for (int d = 0; d < 6; ++d) Jn[d] = fma(e_[d], Va, Jn[d]);
+        }
     }
 }
 
@@ -182,7 +248,7 @@ __device__ __forceinline__ int phase_b_with_nonlocal(const DevSys &S, const Warp
                 pade_six(x0 - ws.r[3 * j], y0 - ws.r[3 * j + 1], z0 - ws.r[3 * j + 2], av, a2, c, S.b2, Jn);
             }
         }
-        if (J3 && (!is_nl || !S.nl_dla)) j3_six(S, T, ws.j3 + (N + i) * LRDMC_J3_MAX, x0, y0, z0, av, a2, t, Jn);
+        if (J3 && (!is_nl || !S.nl_dla)) j3_six(S, T, ws.j3 + (N + i) * S.j3s, x0, y0, z0, av, a2, t, Jn);
         const double Jo = Jold[i];
         if (!is_nl) {
             double Rv[6];
@@ -298,19 +364,7 @@ __device__ __forceinline__ EvalOut evaluate_walker(const DevSys &S, const WarpSt
 
     // ---- phase A (row a6): per-electron continuum pieces.  Two lanes per electron split the e-e partners; the
     //      one-body parts come from the cache.
-    if (J3) {                          // three-body fields V_a(i) = sum_b g_ab (S_b - chi_b(r_i)),  S_b = sum_j chi_b(r_j)
-        double *chi3 = ws.j3, *V3 = ws.j3 + N * LRDMC_J3_MAX, *S3 = V3 + N * LRDMC_J3_MAX;
-        if (lane < LRDMC_J3_MAX) { double sb = 0.0; for (int j = 0; j < N; ++j) sb += chi3[j * LRDMC_J3_MAX + lane]; S3[lane] = sb; }
-        __syncwarp();
-        for (int idx = lane; idx < N * LRDMC_J3_MAX; idx += 32) {
-            const int i = idx / LRDMC_J3_MAX, a = idx - i * LRDMC_J3_MAX;
-            double v = 0.0;
-#pragma unroll
-            for (int b = 0; b < LRDMC_J3_MAX; ++b) v += S.j3_g[a * LRDMC_J3_MAX + b] * (S3[b] - chi3[i * LRDMC_J3_MAX + b]);
-            V3[idx] = v;
-        }
-        __syncwarp();
-    }
+    if (J3) j3_fields(S, T.j3g, ws.j3, lane, 32, [] { __syncwarp(); });     // three-body fields V_a(i) of this evaluation
     double vee_part = 0.0;
     for (int i0 = 0; i0 < N; i0 += 16) {
         const int i = i0 + (lane >> 1), sub = lane & 1;
@@ -340,15 +394,7 @@ __device__ __forceinline__ EvalOut evaluate_walker(const DevSys &S, const WarpSt
         if (act && sub == 0) {
             const double *ob = ws.ob + 8 * ii;
             gx += ob[1]; gy += ob[2]; gz += ob[3];
-            if (J3) {                  // J3 terms of electron i: sum_a chi_a V_a;  grad chi = -2 zeta d chi;  lap chi = (4 zeta^2 r^2 - 6 zeta) chi
-                const double *chi3 = ws.j3 + ii * LRDMC_J3_MAX, *V3 = ws.j3 + (N + ii) * LRDMC_J3_MAX;
-                for (int a = 0; a < S.n_j3; ++a) {
-                    const double *nu = T.nuc + S.j3_center[a] * LRDMC_NUC_STRIDE, z = S.j3_zeta[a];
-                    const double dx = xi - nu[0], dy = yi - nu[1], dz = zi - nu[2], cv = chi3[a] * V3[a], tz = -2.0 * z * cv;
-                    J += cv; gx += tz * dx; gy += tz * dy; gz += tz * dz;
-                    lJ += (4.0 * z * z * (dx * dx + dy * dy + dz * dz) - 6.0 * z) * cv;
-                }
-            }
+            if (J3) j3_electron_terms(S, T.nuc, ws.j3 + ii * S.j3s, ws.j3 + (N + ii) * S.j3s, xi, yi, zi, J, gx, gy, gz, lJ);
             Jold[ii] = J + ob[0];
             lap_s[ii] = Ld + 2.0 * (Gx * gx + Gy * gy + Gz * gz) + (lJ + ob[4]) + (gx * gx + gy * gy + gz * gz);
         }
@@ -381,7 +427,7 @@ __device__ __forceinline__ EvalOut evaluate_walker(const DevSys &S, const WarpSt
                     const double c = (j == i) ? 0.0 : ((spin_of(S, j) == sp) ? S.a_par : S.a_anti);
                     pade_six(x0 - ws.r[3 * j], y0 - ws.r[3 * j + 1], z0 - ws.r[3 * j + 2], av, a2, c, S.b2, Jn);
                 }
-                if (J3) j3_six(S, T, ws.j3 + (N + i) * LRDMC_J3_MAX, x0, y0, z0, av, a2, t, Jn);
+                if (J3) j3_six(S, T, ws.j3 + (N + i) * S.j3s, x0, y0, z0, av, a2, t, Jn);
                 const double Jo = Jold[i];
                 double Rv[6];
 #pragma unroll
@@ -436,7 +482,7 @@ __device__ __forceinline__ void apply_move(const DevSys &S, const WarpState &ws,
     __syncwarp();
     refresh_mo_cache<NT, TS>(S, T.shells, sp ? T.bf[1] : T.bf[0], T.etab, mc, px, py, pz, lane);
     refresh_onebody(S.n_nuc, S.has_j1, S.a, T.nuc, ws.ob + 8 * i, px, py, pz, lane);
-    if (EXT & 2) refresh_j3_row(S, T.nuc, ws.j3 + i * LRDMC_J3_MAX, px, py, pz, lane);
+    if (EXT & 2) refresh_j3_row(S, T.nuc, ws.j3 + i * S.j3s, px, py, pz, lane);
     if (lane == 0) { ws.r[3 * i] = px; ws.r[3 * i + 1] = py; ws.r[3 * i + 2] = pz; }
     __syncwarp();
     // s_k = sum_m phi_m Dinv[m][k];  rho = s_il;  Dinv'[m][il] = Dinv[m][il]/rho;  Dinv'[m][k] = Dinv[m][k] - Dinv[m][il] s_k / rho

@@ -74,6 +74,8 @@ static int plan_smem(lrdmc_ctx *c)
     S.off_etab = (int)o; o += 256;              // always first: exp_tab addresses it as (dynamic smem base) + 8 j
     S.off_shells = (int)o; o += align_up(c->n_sh, 2);
     S.off_nuc = (int)o; o += align_up(c->n_nuc_d, 2);
+    S.off_srad = (int)o; o += align_up((size_t)S.n_slots, 2);
+    S.off_j3g = (int)o; o += (size_t)S.j3s * S.j3s;
     S.off_bf[0] = (int)o; if (S.bf_in_smem) o += bf_n;
     S.off_bf[1] = (int)o; if (S.bf_in_smem && !S.same_C) o += bf_n;
     S.off_cf[0] = (int)o; if (S.bf_in_smem) o += cf_n;
@@ -89,7 +91,8 @@ static int plan_smem(lrdmc_ctx *c)
     S.o_el = (int)w; w += align_up((size_t)LRDMC_EL_ARRAYS * S.N, 2);
     S.o_U = (int)w; w += 10;                    // the step's lattice frame (9 doubles)
     S.o_ob = (int)w; w += 8 * (size_t)S.N;      // one-body cache: J1, grad J1, lap J1, v_ei, v^a_ei per electron
-    S.o_j3 = (int)w; if (S.n_j3) w += (size_t)S.N * 2 * LRDMC_J3_MAX + LRDMC_J3_MAX;   // three-body Jastrow: chi3, V3, S3
+    S.o_j3 = (int)w; if (S.n_j3) w += (size_t)S.N * 2 * S.j3s + S.j3s;   // three-body Jastrow: chi3, V3, S3
+    S.o_am = (int)w; if (!fits && !S.nl_K && !S.n_j3) w += (size_t)S.N * S.n_lg;       // listed-shell masks (listed sweep of the large systems)
     S.per_warp_doubles = (int)w;
     const size_t per_sm = prop.sharedMemPerMultiprocessor, per_blk_max = prop.sharedMemPerBlockOptin, reserve = 1024;
     c->wpb = LRDMC_WPB;
@@ -115,12 +118,14 @@ static int plan_smem(lrdmc_ctx *c)
 }
 
 static int init_device(lrdmc_ctx *c, const std::vector<double> &h_sh, const std::vector<double> &h_nuc, const std::vector<double> &h_et,
-                       const std::vector<double> (&h_bf)[2], const std::vector<double> (&h_cf)[2])
+                       const std::vector<double> (&h_bf)[2], const std::vector<double> (&h_cf)[2], const std::vector<double> &h_srad, const std::vector<double> &h_j3g,
+                       const std::vector<double> (&h_cn)[2])
 {
     DevSys &S = c->S;
     int ndev = 0; CK(cudaGetDeviceCount(&ndev));
     const size_t bf_n = c->bf_n, cf_n = c->cf_n;
-    const size_t bytes = (h_sh.size() + h_nuc.size() + h_et.size() + (bf_n + cf_n) * (S.same_C ? 1 : 2)) * sizeof(double);
+    const size_t cn_n = h_cn[0].size();
+    const size_t bytes = (h_sh.size() + h_nuc.size() + h_et.size() + h_srad.size() + h_j3g.size() + (bf_n + cf_n + cn_n) * (S.same_C ? 1 : 2)) * sizeof(double);
     CK(cudaMalloc(&c->d_tables, bytes));
     double *d = (double *)c->d_tables;
     CK(cudaMemcpy(d, h_sh.data(), h_sh.size() * 8, cudaMemcpyHostToDevice)); S.shells = d; d += h_sh.size();
@@ -131,8 +136,12 @@ static int init_device(lrdmc_ctx *c, const std::vector<double> &h_sh, const std:
     S.cfrag[0] = S.cfrag[1] = d;
     if (cf_n) {
         CK(cudaMemcpy(d, h_cf[0].data(), cf_n * 8, cudaMemcpyHostToDevice)); d += cf_n;
-        if (!S.same_C) { CK(cudaMemcpy(d, h_cf[1].data(), cf_n * 8, cudaMemcpyHostToDevice)); S.cfrag[1] = d; }
+        if (!S.same_C) { CK(cudaMemcpy(d, h_cf[1].data(), cf_n * 8, cudaMemcpyHostToDevice)); S.cfrag[1] = d; d += cf_n; }
     }
+    CK(cudaMemcpy(d, h_srad.data(), h_srad.size() * 8, cudaMemcpyHostToDevice)); S.srad = d; d += h_srad.size();
+    S.j3g = d; if (h_j3g.size()) { CK(cudaMemcpy(d, h_j3g.data(), h_j3g.size() * 8, cudaMemcpyHostToDevice)); d += h_j3g.size(); }
+    CK(cudaMemcpy(d, h_cn[0].data(), cn_n * 8, cudaMemcpyHostToDevice)); S.cn[0] = S.cn[1] = d; d += cn_n;
+    if (!S.same_C) { CK(cudaMemcpy(d, h_cn[1].data(), cn_n * 8, cudaMemcpyHostToDevice)); S.cn[1] = d; d += cn_n; }
     CK(cudaMalloc((void **)&c->d_stats, sizeof(DevStats)));
     CK(cudaMemset(c->d_stats, 0, sizeof(DevStats)));
     CK(cudaMallocHost((void **)&c->h_stats, sizeof(DevStats)));
@@ -203,12 +212,16 @@ extern "C" int lrdmc_init(lrdmc_ctx **out, const lrdmc_system *sys, const lrdmc_
     }
     for (int j = 0; j < S.P_lat; ++j) S.Kdiag += S.kappa[j / (6 * S.N)];      // K^a_{x,x} = sum_j kappa_j = 3N/a^2 (Eq.D5)
     S.a_par = jas->a_par; S.a_anti = jas->a_anti; S.b2 = jas->b2; S.has_j1 = jas->c1 != NULL; S.has_pp = sys->pp != NULL;
-    S.n_j3 = jas->n_j3 > 0 ? jas->n_j3 : 0;
+    S.n_j3 = jas->n_j3 > 0 ? jas->n_j3 : 0; S.j3s = (S.n_j3 + 3) & ~3; S.j3_poly = 0;
     if (S.n_j3 > LRDMC_J3_MAX || (S.n_j3 && (!jas->j3_center || !jas->j3_zeta || !jas->j3_g))) { free(c); return LRDMC_EINVAL; }
     for (int a = 0; a < S.n_j3; ++a) {
         if (jas->j3_center[a] < 0 || jas->j3_center[a] >= sys->n_nuc || !(jas->j3_zeta[a] > 0.0)) { free(c); return LRDMC_EINVAL; }
-        S.j3_center[a] = jas->j3_center[a]; S.j3_zeta[a] = jas->j3_zeta[a];
-        for (int b = 0; b < LRDMC_J3_MAX; ++b) S.j3_g[a * LRDMC_J3_MAX + b] = b < S.n_j3 ? jas->j3_g[a * S.n_j3 + b] : 0.0;
+        S.j3_center[a] = jas->j3_center[a]; S.j3_zeta[a] = jas->j3_zeta[a]; S.j3_lmn[a] = 0;
+        if (jas->j3_lmn) {
+            const int *q = jas->j3_lmn + 3 * a;
+            if (q[0] < 0 || q[1] < 0 || q[2] < 0 || q[0] + q[1] + q[2] > 2) { free(c); return LRDMC_EINVAL; }
+            S.j3_lmn[a] = q[0] | (q[1] << 2) | (q[2] << 4); if (S.j3_lmn[a]) S.j3_poly = 1;
+        }
     }
     S.key0 = (uint32_t)lat->seed; S.key1 = (uint32_t)(lat->seed >> 32);
     S.V_ii = 0.0;
@@ -284,9 +297,44 @@ extern "C" int lrdmc_init(lrdmc_ctx **out, const lrdmc_system *sys, const lrdmc_
             }
         }
     }
+    // ---- listed candidate sweep: list groups (one shell type, at most 64 slots each), slot-major coefficient rows, screening radii
+    {
+        S.n_lg = 0; S.n_aop = 0;
+        int ao_run = 0;
+        for (int g = 0; g < 4; ++g) {
+            const int nsl = 4 * S.n_it[g];
+            for (int s0 = 0; s0 < nsl; s0 += 64) {
+                if (S.n_lg == LRDMC_MAX_LG) { free(c); return LRDMC_ENOMEM; }
+                S.lg_type[S.n_lg] = g; S.lg_slot0[S.n_lg] = base[g] + s0; S.lg_n[S.n_lg] = nsl - s0 < 64 ? nsl - s0 : 64;
+                S.lg_ao0[S.n_lg] = ao_run + s0 * ncomp[g]; ++S.n_lg;
+            }
+            ao_run += nsl * ncomp[g];
+        }
+        S.n_aop = ao_run;
+    }
+    std::vector<double> h_srad(S.n_slots), h_cn[2];
+    {
+        double amax = lat->a > lat->a2 ? lat->a : lat->a2; (void)amax;
+        for (int q = 0; q < S.n_slots; ++q) {
+            const int s = slot_shell[q];
+            h_srad[q] = s < 0 ? -1e300 : (group[s] == 0 ? LRDMC_LIST_THR / bas->zeta[s] : sqrt(LRDMC_LIST_THR / bas->zeta[s]));
+        }
+        for (int sp = 0; sp < (S.same_C ? 1 : 2); ++sp) {
+            const int ns = sp ? sys->n_dn : sys->n_up; const double *C = sp ? Cdn : Cup;
+            h_cn[sp].assign((size_t)S.n_aop * S.OS, 0.0);
+            int row = 0;
+            for (int g = 0; g < 4; ++g) for (int q = base[g]; q < base[g] + 4 * S.n_it[g]; ++q) for (int comp = 0; comp < ncomp[g]; ++comp, ++row) {
+                const int s = slot_shell[q]; if (s < 0) continue;
+                const double nrm = g == 0 ? 1.0 : gto_norm(bas->zeta[s], lmn[g][comp][0], lmn[g][comp][1], lmn[g][comp][2]);
+                for (int m = 0; m < ns; ++m) h_cn[sp][(size_t)row * S.OS + m] = nrm * C[(size_t)(ao0[s] + comp) * ns + m];
+            }
+        }
+    }
     // ---- device copies (every CUDA call checked; on failure the text moves to the calling thread's slot and the ctx is freed)
     c->n_sh = h_sh.size(); c->n_nuc_d = h_nuc.size(); c->bf_n = bf_n; c->cf_n = cf_n;
-    const int rc = init_device(c, h_sh, h_nuc, h_et, h_bf, h_cf);
+    std::vector<double> h_j3g((size_t)S.j3s * S.j3s, 0.0);          // three-body couplings g [j3s][j3s], zero padded
+    for (int a = 0; a < S.n_j3; ++a) for (int b = 0; b < S.n_j3; ++b) h_j3g[(size_t)a * S.j3s + b] = jas->j3_g[a * S.n_j3 + b];
+    const int rc = init_device(c, h_sh, h_nuc, h_et, h_bf, h_cf, h_srad, h_j3g, h_cn);
     if (rc != LRDMC_OK) { snprintf(t_init_msg, sizeof t_init_msg, "%s", c->msg); lrdmc_free(c); return rc; }
     *out = c;
     return LRDMC_OK;
@@ -333,7 +381,8 @@ static size_t carve(const lrdmc_ctx *c, int n_w, char *base, DevWalk *W)
     TAKE(wq, unsigned long long, nw); TAKE(prefix, unsigned long long, nw); TAKE(parents, int, nw);
     {   // parked Bc entries of the team kernel of the large systems (ao_columns BCS): [resident CTA][block of a mesh][k-step pair][lane][2]
         const bool use = LRDMC_BC_STORE && !c->ts;
-        const size_t stride = (size_t)((S.n_up + 7) / 8 + (S.n_dn + 7) / 8) * S.n_kpairs * 64;
+        size_t stride = (size_t)((S.n_up + 7) / 8 + (S.n_dn + 7) / 8) * S.n_kpairs * 64;
+        if (c->ext == 0 && stride < (size_t)S.N * S.n_aop) stride = (size_t)S.N * S.n_aop;       // listed sweep: Bc [electron][n_aop]
         const size_t cta_bytes = ((size_t)S.tables_doubles + S.per_warp_doubles) * 8 + 1024;
         size_t per_sm = c->smem_per_sm / cta_bytes; if (per_sm > 32) per_sm = 32; if (per_sm < 1) per_sm = 1;   // resident team CTAs per SM, at most
         if (W) { W->bcs_stride = use ? stride : 0; W->bcs_ctas = use ? (int)(per_sm * c->sm_count) : 0; }     // plan_team clamps the grid to this
@@ -384,7 +433,7 @@ static void plan_team(lrdmc_ctx *c, int n_w)
     c->team_tw = 1;
     int tw = 1;
     const long slots = (long)c->grid_max * c->wpb;
-    if (!c->ts) tw = 4;
+    if (!c->ts) tw = (c->ext == 0 && LRDMC_BC_STORE) ? 8 : 4;   // listed sweep (listed.cuh): measured at C5 N_w = 4096, TW = 4 / 8 / 16: 2.27 / 2.82 / 2.64 M walker-moves/s
     else if ((long)n_w * 8 <= 3 * slots) tw = 4;   // measured on C3/C4 (profiles/r1_team_kernel.md): 4 warps per walker beat 2, 8 and 16 at every N_w,
                                                    // and beat warp-per-walker up to N_w of about 3/8 of the resident warp slots
     if (c->opt_team > 0) tw = c->opt_team;        // LRDMC_OPT_TEAM_WARPS (tests force 1, 2, 4, 8, 16)
@@ -418,6 +467,8 @@ static void plan_team(lrdmc_ctx *c, int n_w)
     const int smem = (int)(((size_t)S.tables_doubles + S.per_warp_doubles + P.scr_doubles) * 8);
     const int occ = LRDMC_K_CALL(c->ext, lrdmc_k_team_occupancy, c->NT, c->ts, tw * 32, smem);
     if (cudaGetLastError() != cudaSuccess || occ < 1) return;             // does not fit: stay with warp-per-walker
+    P.listed = !c->ts && c->ext == 0 && LRDMC_BC_STORE;
+    { const int rows = S.n_mesh * S.N; int rb = (rows + tw - 1) / tw; P.RB = rb > 16 ? 16 : (rb < 1 ? 1 : rb); }
     c->team_tw = tw; c->team_smem = smem; c->team_ctas_per_sm = occ; c->team_grid_max = c->sm_count * occ;
     if (c->W.bcs && c->team_grid_max > c->W.bcs_ctas) c->team_grid_max = c->W.bcs_ctas;   // the parked-entry scratch is indexed by blockIdx.x
 }

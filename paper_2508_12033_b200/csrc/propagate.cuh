@@ -9,6 +9,8 @@ __device__ __forceinline__ void stage_tables(const DevSys &S, double *smem)
 {
     for (int i = threadIdx.x; i < S.n_slots * 4; i += blockDim.x) smem[S.off_shells + i] = S.shells[i];
     for (int i = threadIdx.x; i < S.n_nuc * LRDMC_NUC_STRIDE; i += blockDim.x) smem[S.off_nuc + i] = S.nuc[i];
+    for (int i = threadIdx.x; i < S.n_slots; i += blockDim.x) smem[S.off_srad + i] = S.srad[i];
+    for (int i = threadIdx.x; i < S.j3s * S.j3s; i += blockDim.x) smem[S.off_j3g + i] = S.j3g[i];
     if (S.bf_in_smem) {
         const int nb = S.n_ksteps * S.NT[0] * 32;
         for (int i = threadIdx.x; i < nb; i += blockDim.x) smem[S.off_bf[0] + i] = S.bfrag[0][i];
@@ -27,7 +29,7 @@ template <bool TS>
 __device__ __forceinline__ Tables table_pointers(const DevSys &S, const double *smem)
 {
     Tables T;
-    T.shells = smem + S.off_shells; T.nuc = smem + S.off_nuc; T.etab = smem;
+    T.shells = smem + S.off_shells; T.nuc = smem + S.off_nuc; T.etab = smem; T.srad = smem + S.off_srad; T.j3g = smem + S.off_j3g;
     if (TS) {
         T.bf[0] = smem + S.off_bf[0]; T.bf[1] = smem + (S.same_C ? S.off_bf[0] : S.off_bf[1]);
         T.cf[0] = smem + S.off_cf[0]; T.cf[1] = smem + (S.same_C ? S.off_cf[0] : S.off_cf[1]);
@@ -44,6 +46,7 @@ __device__ __forceinline__ WarpState warp_views(const DevSys &S, double *smem, i
     WarpState ws;
     ws.r = base + S.o_r; ws.dinv[0] = base + S.o_dinv[0]; ws.dinv[1] = base + S.o_dinv[1];
     ws.moc = base + S.o_moc; ws.R = base + S.o_R; ws.cum = base + S.o_cum; ws.el = base + S.o_el; ws.ob = base + S.o_ob; ws.U = base + S.o_U; ws.j3 = base + S.o_j3;
+    ws.am = reinterpret_cast<unsigned long long *>(base + S.o_am);
     return ws;
 }
 
@@ -71,7 +74,7 @@ __device__ __forceinline__ void load_walker(const DevSys &S, const DevWalk &W, W
     if (TS) { for (int i = lane; i < (int)mocn; i += 32) ws.moc[i] = W.moc[(size_t)k * mocn + i]; }
     else ws.moc = W.moc + (size_t)k * mocn;
     __syncwarp();
-    if (with_onebody && S.n_j3) for (int i = 0; i < N; ++i) refresh_j3_row(S, nuc, ws.j3 + i * LRDMC_J3_MAX, ws.r[3 * i], ws.r[3 * i + 1], ws.r[3 * i + 2], lane);
+    if (with_onebody && S.n_j3) for (int i = 0; i < N; ++i) refresh_j3_row(S, nuc, ws.j3 + i * S.j3s, ws.r[3 * i], ws.r[3 * i + 1], ws.r[3 * i + 2], lane);
     if (with_onebody) for (int i = 0; i < N; ++i) refresh_onebody(S.n_nuc, S.has_j1, S.a, nuc, ws.ob + 8 * i, ws.r[3 * i], ws.r[3 * i + 1], ws.r[3 * i + 2], lane);
     __syncwarp();
 }

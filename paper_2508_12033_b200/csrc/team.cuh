@@ -9,6 +9,34 @@
 // The walker queue, the weight rules (Alg.2 lines 4-8 L401-L410 / Alg.1) and the HBM layout are those of k_propagate.
 #pragma once
 #include "propagate.cuh"
+#include "listed.cuh"
+
+// ---- listed sweep of the large systems (listed.cuh): the CTA's Bc = C Dinv of its walker, [electron][n_aop] in global scratch ----
+// Built when the walker is loaded: thread = one AO row of C (slot-major, norms folded in), eight inverse columns at a time.
+__device__ __forceinline__ void team_build_bc(const DevSys &S, const WarpState &ws, double *__restrict__ bc)
+{
+    const int tid = threadIdx.x, nthr = blockDim.x, A = S.n_aop, OS = S.OS;
+    for (int sp = 0; sp < 2; ++sp) {
+        const int ns = sp ? S.n_dn : S.n_up, off = sp ? S.n_up : 0;
+        if (!ns) continue;
+        const double *__restrict__ cn = S.cn[sp], *dinv = ws.dinv[sp];
+        for (int ao = tid; ao < A; ao += nthr) {
+            const double *crow = cn + (size_t)ao * OS;
+            for (int il0 = 0; il0 < ns; il0 += 8) {
+                double acc[8];
+#pragma unroll
+                for (int j = 0; j < 8; ++j) acc[j] = 0.0;
+                for (int m = 0; m < ns; ++m) {
+                    const double cv = __ldg(crow + m); const double *dr = dinv + m * ns + il0;   // columns beyond n_s read padding, never stored
+#pragma unroll
+                    for (int j = 0; j < 8; ++j) acc[j] = fma(cv, dr[j], acc[j]);
+                }
+#pragma unroll
+                for (int j = 0; j < 8; ++j) if (il0 + j < ns) bc[(size_t)(off + il0 + j) * A + ao] = acc[j];
+            }
+        }
+    }
+}
 
 __device__ __forceinline__ void load_walker_team(const DevSys &S, const DevWalk &W, WarpState &ws, const double *nuc, int k, int TW)
 {
@@ -25,7 +53,7 @@ __device__ __forceinline__ void load_walker_team(const DevSys &S, const DevWalk 
     __syncthreads();
     for (int i = wt; i < N; i += TW) {
         refresh_onebody(S.n_nuc, S.has_j1, S.a, nuc, ws.ob + 8 * i, ws.r[3 * i], ws.r[3 * i + 1], ws.r[3 * i + 2], lane);
-        if (S.n_j3) refresh_j3_row(S, nuc, ws.j3 + i * LRDMC_J3_MAX, ws.r[3 * i], ws.r[3 * i + 1], ws.r[3 * i + 2], lane);
+        if (S.n_j3) refresh_j3_row(S, nuc, ws.j3 + i * S.j3s, ws.r[3 * i], ws.r[3 * i + 1], ws.r[3 * i + 2], lane);
     }
     __syncthreads();
 }
@@ -52,24 +80,13 @@ template <int NT, bool TS, int EXT, bool BCS>
 __device__ __forceinline__ EvalOut evaluate_team(const DevSys &S, const TeamPlan &P, const WarpState &ws, const Tables &T, double *scr, double *s_vee, int *s_node,
                                                  double2 *bcs_cta, int reuse_spin)
 {
+    constexpr bool LISTED = BCS && EXT == 0;       // large systems without slots / J3: listed sweep on the CTA's rank-1-updated Bc (listed.cuh)
     const int N = S.N, n_nuc = S.n_nuc, TW = P.TW, NP = P.NP, tid = threadIdx.x, nthr = blockDim.x, lane = tid & 31, wt = tid >> 5;
     const int t = lane & 3, g = lane >> 2;
     constexpr bool NL = (EXT & 1) != 0, J3 = (EXT & 2) != 0;      // non-local slots / three-body Jastrow (separate instantiations)
     double *Jold = ws.el, *lap_s = ws.el + N;
 
-    if (J3) {                          // three-body fields V_a(i) = sum_b g_ab (S_b - chi_b(r_i)),  S_b = sum_j chi_b(r_j)   (evaluate.cuh)
-        double *chi3 = ws.j3, *V3 = ws.j3 + N * LRDMC_J3_MAX, *S3 = V3 + N * LRDMC_J3_MAX;
-        if (tid < LRDMC_J3_MAX) { double sb = 0.0; for (int j = 0; j < N; ++j) sb += chi3[j * LRDMC_J3_MAX + tid]; S3[tid] = sb; }
-        __syncthreads();
-        for (int idx = tid; idx < N * LRDMC_J3_MAX; idx += nthr) {
-            const int i = idx / LRDMC_J3_MAX, a = idx - i * LRDMC_J3_MAX;
-            double v = 0.0;
-#pragma unroll
-            for (int b = 0; b < LRDMC_J3_MAX; ++b) v += S.j3_g[a * LRDMC_J3_MAX + b] * (S3[b] - chi3[i * LRDMC_J3_MAX + b]);
-            V3[idx] = v;
-        }
-        __syncthreads();
-    }
+    if (J3) j3_fields(S, T.j3g, ws.j3, tid, nthr, [] { __syncthreads(); });     // three-body fields V_a(i) of this evaluation (evaluate.cuh)
     // ---- phase A (row a6): per-electron continuum pieces; P.lpe lanes of one warp per electron split the partners and the MOs
     {
         const int LPE = P.lpe, epp = nthr / LPE;
@@ -103,15 +120,7 @@ __device__ __forceinline__ EvalOut evaluate_team(const DevSys &S, const TeamPlan
             if (act && sub == 0) {
                 const double *ob = ws.ob + 8 * ii;
                 gx += ob[1]; gy += ob[2]; gz += ob[3];
-                if (J3) {              // J3 terms of electron i (as in evaluate_walker)
-                    const double *chi3 = ws.j3 + ii * LRDMC_J3_MAX, *V3 = ws.j3 + (N + ii) * LRDMC_J3_MAX;
-                    for (int a = 0; a < S.n_j3; ++a) {
-                        const double *nu = T.nuc + S.j3_center[a] * LRDMC_NUC_STRIDE, z = S.j3_zeta[a];
-                        const double dx = xi - nu[0], dy = yi - nu[1], dz = zi - nu[2], cv = chi3[a] * V3[a], tz = -2.0 * z * cv;
-                        J += cv; gx += tz * dx; gy += tz * dy; gz += tz * dz;
-                        lJ += (4.0 * z * z * (dx * dx + dy * dy + dz * dz) - 6.0 * z) * cv;
-                    }
-                }
+                if (J3) j3_electron_terms(S, T.nuc, ws.j3 + ii * S.j3s, ws.j3 + (N + ii) * S.j3s, xi, yi, zi, J, gx, gy, gz, lJ);
                 Jold[ii] = J + ob[0];
                 lap_s[ii] = Ld + 2.0 * (Gx * gx + Gy * gy + Gz * gz) + (lJ + ob[4]) + (gx * gx + gy * gy + gz * gz);
             }
@@ -141,6 +150,54 @@ __device__ __forceinline__ EvalOut evaluate_team(const DevSys &S, const TeamPlan
         if (lane == 0) { s_node[1] = na; s_node[2] = S.same_C ? na : nup; }
     }
     __syncthreads();
+
+    if (LISTED) {
+        // ---- phase B of the large systems (rows a1-a5): batches of RB rows (mesh, electron) per warp; the listed sweep leaves the
+        //      determinant ratios in R, the Jastrow ratios of the same rows follow in the same warp (quad per row)
+        const int n_rows = S.n_mesh * N, RB = P.RB;
+        const double *bc = reinterpret_cast<const double *>(bcs_cta);
+        for (int b0 = wt * RB; b0 < n_rows; b0 += TW * RB) {
+            const int nr = min(RB, n_rows - b0);
+            ao_listed_warp(S, T.shells, T.etab, ws.r, ws.U, ws.am, bc, b0, nr, ws.R, lane);
+            for (int r0 = 0; r0 < nr; r0 += 8) {
+                const bool valid = r0 + g < nr;
+                const int rho = b0 + (valid ? r0 + g : 0), mesh = rho / N, i = rho - mesh * N, sp = spin_of(S, i);
+                const double x0 = ws.r[3 * i], y0 = ws.r[3 * i + 1], z0 = ws.r[3 * i + 2], am_ = S.amesh[mesh], a2 = am_ * am_;
+                double av[3][3], Jn[6];
+#pragma unroll
+                for (int k = 0; k < 3; ++k) { av[k][0] = am_ * ws.U[k]; av[k][1] = am_ * ws.U[3 + k]; av[k][2] = am_ * ws.U[6 + k]; }
+#pragma unroll
+                for (int d = 0; d < 6; ++d) Jn[d] = 0.0;
+                if (S.has_j1) for (int I = t; I < n_nuc; I += 4) {
+                    const double *np_ = T.nuc + I * LRDMC_NUC_STRIDE;
+                    pade_six(x0 - np_[0], y0 - np_[1], z0 - np_[2], av, a2, -np_[4], np_[5], Jn);
+                }
+                for (int j = t; j < N; j += 4) {
+                    const double c = (j == i) ? 0.0 : ((spin_of(S, j) == sp) ? S.a_par : S.a_anti);
+                    pade_six(x0 - ws.r[3 * j], y0 - ws.r[3 * j + 1], z0 - ws.r[3 * j + 2], av, a2, c, S.b2, Jn);
+                }
+                const double Jo = Jold[i];
+                double *Ro = ws.R + mesh * 6 * N + 6 * i;
+                double Rv[6];
+#pragma unroll
+                for (int d = 0; d < 6; ++d) Rv[d] = Ro[d] * exp_tab(quad_sum(Jn[d]) - Jo, T.etab);
+                __syncwarp();
+                if (valid && t == 0) {
+#pragma unroll
+                    for (int d = 0; d < 6; ++d) Ro[d] = Rv[d];
+                }
+            }
+            __syncwarp();
+        }
+        __syncthreads();
+        EvalOut o; o.bbar = 0.0; o.Vsf = 0.0; o.W = 0.0; o.eL = 0.0; o.node = 0;
+        if (wt == 0) {
+            double Vee = 0.0;
+            for (int w = 0; w < TW; ++w) Vee += s_vee[w];
+            o = phase_c<false>(S, ws, lap_s, Vee, lane, 0);
+        }
+        return o;
+    }
 
     // ---- phase B (rows a1-a5, f1): work units (mesh, spin, 8-electron block, shell part) and, with non-local slots, (pass of 8
     //      LISTED slots, shell part); unit v -> warp v mod TW.  One loop, one ao_columns call site for both kinds.
@@ -174,7 +231,7 @@ __device__ __forceinline__ EvalOut evaluate_team(const DevSys &S, const TeamPlan
 #pragma unroll
         for (int k = 0; k < 3; ++k) { av[k][0] = step * ws.U[k]; av[k][1] = step * ws.U[3 + k]; av[k][2] = step * ws.U[6 + k]; }
         double acc[6], Jn[6];
-        if (BCS && !is_nl) {
+        if (BCS && !LISTED && !is_nl) {
             double2 *bq = bcs_cta + (size_t)rem * S.n_kpairs * 32 + lane;
             if ((mesh > 0 && P.mesh_share) || sp == reuse_spin)
                 ao_columns<NT, TS, true, 2>(S, T.shells, sp ? T.cf[1] : T.cf[0], T.etab, sp ? ws.dinv[1] : ws.dinv[0], ns, il, x0, y0, z0, av, a2, lane, acc, &P, &P.col[part], bq);
@@ -195,7 +252,7 @@ __device__ __forceinline__ EvalOut evaluate_team(const DevSys &S, const TeamPlan
             }
         }
         if (J3 && (!is_nl || !S.nl_dla))                             // three-body Jastrow: the functions are dealt over (part, quad lane)
-            j3_six(S, T, ws.j3 + (N + i) * LRDMC_J3_MAX, x0, y0, z0, av, a2, t, Jn, 4 * part, 4 * NP);
+            j3_six(S, T, ws.j3 + (N + i) * S.j3s, x0, y0, z0, av, a2, t, Jn, 4 * part, 4 * NP);
         double nuq[6];
 #pragma unroll
         for (int d = 0; d < 6; ++d) nuq[d] = 0.0;
@@ -267,8 +324,9 @@ __device__ __forceinline__ EvalOut evaluate_team(const DevSys &S, const TeamPlan
 // Apply move j (row a10) by the team: warp w takes part P.mo[w] of the derivative pass of the mover (value, gradient, Laplacian
 // rows by DMMA), the partial rows meet in scr; Sherman-Morrison on Dinv_sigma over all threads.
 template <int NT, bool TS, int EXT>
-__device__ __forceinline__ void apply_move_team(const DevSys &S, const TeamPlan &P, const WarpState &ws, const Tables &T, double *scr, int j)
+__device__ __forceinline__ void apply_move_team(const DevSys &S, const TeamPlan &P, const WarpState &ws, const Tables &T, double *scr, int j, double *bc = nullptr)
 {
+    constexpr bool LISTED = !TS && LRDMC_BC_STORE && EXT == 0;
     const int N = S.N, TW = P.TW, tid = threadIdx.x, nthr = blockDim.x, lane = tid & 31, wt = tid >> 5;   // warp 0 holds the lightest shell part (s shells): it also refreshes the one-body cache
     int i; double px, py, pz;
     move_target<(EXT & 1) != 0>(S, ws, T.nuc, j, i, px, py, pz);
@@ -285,7 +343,9 @@ __device__ __forceinline__ void apply_move_team(const DevSys &S, const TeamPlan 
             for (int nt = 0; nt < NT; ++nt) { q[8 * nt + 2 * t] = acc[nt][0]; q[8 * nt + 2 * t + 1] = acc[nt][1]; }
         }
     }
-    if (wt == 0) { refresh_onebody(S.n_nuc, S.has_j1, S.a, T.nuc, ws.ob + 8 * i, px, py, pz, lane); if (EXT & 2) refresh_j3_row(S, T.nuc, ws.j3 + i * LRDMC_J3_MAX, px, py, pz, lane); }
+    if (wt == 0) { refresh_onebody(S.n_nuc, S.has_j1, S.a, T.nuc, ws.ob + 8 * i, px, py, pz, lane); if (EXT & 2) refresh_j3_row(S, T.nuc, ws.j3 + i * S.j3s, px, py, pz, lane); }
+    if (LISTED && wt == TW - 1)            // the mover's listed-shell masks at its new position
+        list_masks(S, T.shells, T.srad, ws.am + i * S.n_lg, px, py, pz, fmax(S.amesh[0], S.amesh[1]), lane, 0, 1);
     __syncthreads();                                   // every thread has read the old position
     for (int idx = tid; idx < rows; idx += nthr) {
         double s = 0.0;
@@ -307,6 +367,23 @@ __device__ __forceinline__ void apply_move_team(const DevSys &S, const TeamPlan 
         const int m = idx / ns, kk = idx - m * ns;
         const double ci = col[m] * irho;
         dinv[idx] = (kk == il) ? ci : dinv[idx] - ci * sk[kk];
+    }
+    if (LISTED) {      // Bc = C Dinv follows the inverse by the same rank-1 formula: Bc'[:,k] = Bc[:,k] - Bc[:,il] s_k / rho, Bc'[:,il] = Bc[:,il] / rho
+        // item = (AO, chunk of 8 columns): eight independent loads in flight per thread, consecutive threads on consecutive AOs (coalesced);
+        // column il itself is rescaled in a second sweep (every item of the first reads its OLD entries)
+        const int A = S.n_aop, off = sp ? S.n_up : 0, nch = (ns + 7) >> 3;
+        const double *bi = bc + (size_t)i * A;
+        for (int it = tid; it < A * nch; it += nthr) {
+            const int ch = it / A, ao = it - ch * A, k0 = 8 * ch;
+            const double f = bi[ao] * irho;
+            double v[8];
+#pragma unroll
+            for (int q = 0; q < 8; ++q) v[q] = (k0 + q < ns) ? __ldcg(bc + (size_t)(off + k0 + q) * A + ao) : 0.0;
+#pragma unroll
+            for (int q = 0; q < 8; ++q) if (k0 + q < ns && k0 + q != il) __stcg(bc + (size_t)(off + k0 + q) * A + ao, fma(-f, sk[k0 + q], v[q]));
+        }
+        __syncthreads();
+        for (int ao = tid; ao < A; ao += nthr) bc[(size_t)i * A + ao] = bi[ao] * irho;
     }
     __syncthreads();
 }
@@ -339,6 +416,12 @@ __global__ void __launch_bounds__(LRDMC_TEAM_MAX_WARPS * 32, 1) k_propagate_team
             continue;
         }
         load_walker_team(S, W, ws, T.nuc, k, P.TW);
+        if (BCS && EXT == 0) {                                  // listed sweep: masks of every electron, Bc of this walker
+            for (int i = wt; i < S.N; i += P.TW)
+                list_masks(S, T.shells, T.srad, ws.am + i * S.n_lg, ws.r[3 * i], ws.r[3 * i + 1], ws.r[3 * i + 2], fmax(S.amesh[0], S.amesh[1]), lane, 0, 1);
+            team_build_bc(S, ws, reinterpret_cast<double *>(bcs_cta));
+            __syncthreads();
+        }
         uint32_t s = 0; int reuse_spin = -1;
         double w = 1.0, tau_left = tau, omega = 0.0, eL_last = 0.0, W_last = 0.0; long long moves = 0; int n_node = 0, n_nonpos = 0;
         for (;;) {
@@ -374,7 +457,7 @@ __global__ void __launch_bounds__(LRDMC_TEAM_MAX_WARPS * 32, 1) k_propagate_team
             const bool last = s_ctrl[1] != 0; const int j = s_ctrl[2];
             if (last) break;
             if (j >= 0) {
-                apply_move_team<NT, TS, EXT>(S, P, ws, T, scr, j); ++moves;
+                apply_move_team<NT, TS, EXT>(S, P, ws, T, scr, j, reinterpret_cast<double *>(bcs_cta)); ++moves;
                 const int im = j < S.P_lat ? (j % (6 * S.N)) / 6 : (j - S.P_lat) / (6 * S.nl_K);   // the electron that hopped
                 reuse_spin = 1 - spin_of(S, im);
             } else reuse_spin = -1;

@@ -57,7 +57,7 @@ def _system(name, Z, R, n_up, n_dn, center, stype, zeta, C_up, C_dn, jastrow, a,
         a=float(a), a2=float(a2), seed=int(seed),
         n_walkers=int(n_walkers), cycles=int(cycles), moves=int(moves),
         nl=None, nl_K=0, nl_dla=1,      # non-local pseudopotential channels (scope row f1): see with_nonlocal
-        j3_center=None, j3_zeta=None, j3_g=None,   # three-body Jastrow (scope row f2): see with_jastrow3
+        j3_center=None, j3_zeta=None, j3_g=None, j3_lmn=None,   # three-body Jastrow (scope row f2): see with_jastrow3
     )
     assert d["C_up"].shape == (d["n_ao"], d["n_up"])
     assert d["C_dn"].shape == (d["n_ao"], d["n_dn"])
@@ -245,17 +245,40 @@ def contracted_molecule(n_up=3, n_dn=2, n_nuc=3, n_cshell=9, seed=31, a=0.2, sph
                    pp=pp, contraction=(first, coef, sph))
 
 
-def with_jastrow3(sysd, seed, n_per_nucleus=1, strength=0.3):
-    """Attach a synthetic three-body Jastrow J3 = sum_{i<j} sum_ab g_ab chi_a(r_i) chi_b(r_j) on s-type Gaussians chi_a =
-    exp(-zeta_a |r - R_a|^2) centred on the nuclei (at most 8 functions): zeta log-uniform in [0.3, 2], g symmetric, uniform in
-    [-strength, strength].  The paper's runs use the TurboRVB 3-body Jastrow with optimised parameters (L242, L285): not in the container."""
+def contracted_slater_molecule(a=0.2, with_gaussians=True):
+    """Scope row f2: CONTRACTED SLATER shells (L242 names the Slater-type basis of the TurboRVB runs): a two-centre, four-electron
+    (2/2) molecule whose s functions are fixed sums of 2-3 Slater primitives exp(-zeta r), optionally next to Gaussian p/d shells
+    (one contracted p, one solid-harmonic d) so that all shell groups of the kernels meet in one system.  Seeded, synthetic."""
+    rng = np.random.default_rng(41)
+    R = np.array([[0.0, 0.0, -0.7], [0.1, 0.0, 0.75]]); Z = np.array([2.0, 2.0])
+    center = [0, 0, 0, 1, 1, 0, 1]; stype = [SHELL_SLATER_S] * 7; zeta = [2.6, 1.4, 0.9, 3.1, 1.1, 0.7, 0.8]
+    coef = [0.5, 0.4, 0.2, 0.7, -0.3, 1.0, 1.0]; first = [0, 3, 5, 6, 7]; sph = [0, 0, 0, 0]
+    if with_gaussians:
+        center += [0, 0, 1]; stype += [SHELL_P, SHELL_P, SHELL_D]; zeta += [1.3, 0.5, 0.9]; coef += [0.6, 0.5, 1.0]
+        first += [9, 10]; sph += [0, 1]
+    n_ao = n_ao_contracted(stype, first, sph)
+    C_up = _orthonormal_mos(rng, n_ao, 2); C_dn = _orthonormal_mos(rng, n_ao, 2)
+    jas = dict(a_par=0.25, a_anti=0.5, b2=0.8, c1=Z.copy(), b1=np.array([1.1, 0.9]))
+    return _system("contracted-slater-2u2d" + ("-spd" if with_gaussians else ""), Z, R, 2, 2, center, stype, zeta, C_up, C_dn, jas, a,
+                   contraction=(first, coef, sph))
+
+
+def with_jastrow3(sysd, seed, n_per_nucleus=1, strength=0.3, n_max=8, poly=False):
+    """Attach a synthetic three-body Jastrow J3 = sum_{i<j} sum_ab g_ab chi_a(r_i) chi_b(r_j) on Gaussians centred on the nuclei,
+    chi_a = dx^l dy^m dz^n exp(-zeta_a |r - R_a|^2) (at most n_max functions): zeta log-uniform in [0.3, 2], g symmetric, uniform in
+    [-strength, strength].  poly = False: s functions only (j3_lmn None); poly = True: the monomials cycle through s, the three p and
+    the six cartesian d functions.  The paper's runs use the TurboRVB 3-body Jastrow with optimised parameters (L242, L285): not in
+    the container."""
     rng = np.random.default_rng(seed)
-    centers = [I for I in range(sysd["n_nuc"]) for _ in range(n_per_nucleus)][:8]
+    centers = [I for I in range(sysd["n_nuc"]) for _ in range(n_per_nucleus)][:n_max]
     n = len(centers)
     zeta = np.exp(rng.uniform(np.log(0.3), np.log(2.0), size=n))
     g = rng.uniform(-strength, strength, size=(n, n)); g = 0.5 * (g + g.T)
     d = dict(sysd)
     d.update(j3_center=np.ascontiguousarray(centers, dtype=np.int32), j3_zeta=zeta, j3_g=np.ascontiguousarray(g), name=sysd["name"] + "-J3")
+    if poly:
+        mono = [(0, 0, 0), (1, 0, 0), (0, 1, 0), (0, 0, 1), (2, 0, 0), (1, 1, 0), (1, 0, 1), (0, 2, 0), (0, 1, 1), (0, 0, 2)]
+        d.update(j3_lmn=np.ascontiguousarray([mono[(3 * k + seed) % 10] for k in range(n)], dtype=np.int32), name=sysd["name"] + "-J3spd")
     return d
 
 

@@ -59,10 +59,16 @@ SYSTEMS = {
     # lrdmc_init folds the contraction into its primitive coefficient tables)
     "contracted-3u2d-sph-pp": lambda: _with_walkers(wl.contracted_molecule(3, 2, 3, 9, seed=31, spherical=True, with_pp=True), 37),
     "contracted-9u7d-cart": lambda: _with_walkers(wl.contracted_molecule(9, 7, 4, 21, seed=32, spherical=False), 21),
+    "contracted-slater-spd": lambda: _with_walkers(wl.contracted_slater_molecule(), 45),                # contracted Slater shells + Gaussian p / solid-harmonic d
+    "contracted-slater-only": lambda: _with_walkers(wl.contracted_slater_molecule(with_gaussians=False), 33),
     # scope row f2: three-body Jastrow (s Gaussians at the nuclei), alone, with non-local slots in the full-ratio form, on C3
     "tiny-3u2d-pp-J3": lambda: _with_walkers(wl.with_jastrow3(wl.tiny_molecule(3, 2, 3, 9, seed=21, with_pp=True), 4, 2), 37),
     "tiny-3u2d-J3-nlTM": lambda: _with_walkers(wl.with_jastrow3(wl.random_nonlocal(wl.tiny_molecule(3, 2, 3, 9, seed=21, with_pp=True), 5, 1.6, 2, False, scale=200.0), 4, 2), 37),
     "ragged-9u4d-J3": lambda: _with_walkers(wl.with_jastrow3(wl.tiny_molecule(9, 4, 4, 20, seed=11), 6, 2, strength=0.1), 13),
+    # scope row f2 (remainder): p and cartesian d functions in the three-body Jastrow, more than 8 functions (12, 12, 24)
+    "tiny-3u2d-pp-J3spd": lambda: _with_walkers(wl.with_jastrow3(wl.tiny_molecule(3, 2, 3, 9, seed=21, with_pp=True), 5, 4, n_max=12, poly=True), 37),
+    "ragged-9u4d-J3spd-nlTM": lambda: _with_walkers(wl.with_jastrow3(wl.random_nonlocal(wl.tiny_molecule(9, 4, 4, 20, seed=11), 5, 1.6, 2, False, scale=50.0), 6, 3, strength=0.1, n_max=12, poly=True), 13),
+    "C3-water-methane-J3spd": lambda: _with_walkers(wl.with_jastrow3(wl.water_methane(n_walkers=100), 8, 3, strength=0.03, n_max=24, poly=True), 100),
     "C3-water-methane-J3": lambda: _with_walkers(wl.with_jastrow3(wl.water_methane(n_walkers=100), 7, 1, strength=0.05), 100),
     "contracted-4u4d-sph-nlDLA": lambda: _with_walkers(wl.random_nonlocal(wl.contracted_molecule(4, 4, 3, 12, seed=33, spherical=True, with_pp=True), 9, 1.5, 2, True, scale=100.0), 29),
 }
@@ -158,7 +164,8 @@ def test_whole_cycle_trajectories_weights_and_branching(B, name, mode, kernel):
                                        ("C3-water-methane-shaped", "conventional"), ("C5-cluster64-doublemesh", "balanced"),
                                        ("tiny-3u2d-nlDLA-strong", "balanced"), ("tiny-2u1d-nlTM-strong", "conventional"), ("C3-water-methane-nlDLA", "balanced"),
                                        ("C3-water-methane-nlTM", "balanced"), ("contracted-4u4d-sph-nlDLA", "balanced"), ("tiny-2u2d-doublemesh-nlTM", "conventional"),
-                                       ("tiny-3u2d-pp-J3", "balanced"), ("tiny-3u2d-J3-nlTM", "conventional"), ("C3-water-methane-J3", "balanced")])
+                                       ("tiny-3u2d-pp-J3", "balanced"), ("tiny-3u2d-J3-nlTM", "conventional"), ("C3-water-methane-J3", "balanced"),
+                                       ("tiny-3u2d-pp-J3spd", "balanced"), ("ragged-9u4d-J3spd-nlTM", "conventional"), ("C3-water-methane-J3spd", "balanced")])
 def test_team_kernel_every_team_size(B, name, mode, tw):
     """k_propagate_team with TW = 2, 4, 8, 16 warps per walker (work units = electron blocks x shell parts, partial sums
     in shared memory): same trajectories, weights and indices as the oracle."""

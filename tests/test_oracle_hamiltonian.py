@@ -65,7 +65,9 @@ SYSTEMS = {
     "C2": wl.synthetic10,
     "C3": lambda: wl.water_methane(n_walkers=4),
     "tiny-j3": lambda: wl.with_jastrow3(wl.tiny_molecule(3, 2, 3, 9, seed=21, with_pp=True), 4, 2),   # three-body Jastrow (scope row f2)
+    "tiny-j3-spd": lambda: wl.with_jastrow3(wl.tiny_molecule(3, 2, 3, 9, seed=21, with_pp=True), 5, 4, n_max=12, poly=True),   # s/p/d functions, 12 of them
     "contracted-sph": lambda: wl.contracted_molecule(3, 2, 3, 9, seed=31, spherical=True, with_pp=True),   # scope row f2
+    "contracted-slater": wl.contracted_slater_molecule,                                                      # scope row f2: contracted Slater shells
 }
 
 
@@ -95,7 +97,7 @@ def test_regularised_local_energy_equals_continuum_local_energy(name):
     assert checked >= 1     # random-MO trial functions have nodes everywhere: the D11 branch fires often on C3
 
 
-@pytest.mark.parametrize("name", ["tiny-2u1d", "tiny-3u3d-pp", "C2", "contracted-sph", "tiny-j3"])
+@pytest.mark.parametrize("name", ["tiny-2u1d", "tiny-3u3d-pp", "C2", "contracted-sph", "tiny-j3", "tiny-j3-spd", "contracted-slater"])
 def test_continuum_laplacian_matches_finite_differences_of_logpsi(name):
     """lap_i Psi/Psi = lap_i log|Psi| + |grad_i log|Psi||^2, by 4th-order central differences of the brute-force log|Psi|."""
     s = SYSTEMS[name](); o = ref.Ref(s); x = wl.initial_walkers(s, 1, 33)[0]
@@ -113,7 +115,7 @@ def test_continuum_laplacian_matches_finite_differences_of_logpsi(name):
 
 
 # ----------------------------------------------------------------------------- ratios vs brute force (pin P3)
-@pytest.mark.parametrize("name", ["tiny-2u1d", "tiny-3u3d-pp", "tiny-2u2d-doublemesh", "C2", "contracted-sph", "tiny-j3"])
+@pytest.mark.parametrize("name", ["tiny-2u1d", "tiny-3u3d-pp", "tiny-2u2d-doublemesh", "C2", "contracted-sph", "tiny-j3", "tiny-j3-spd", "contracted-slater"])
 def test_candidate_ratios_match_full_wavefunction_recomputation(name):
     s = SYSTEMS[name](); o = ref.Ref(s); rng = np.random.default_rng(6)
     x = wl.initial_walkers(s, 1, 44)[0]; U = _rand_frame(rng)
@@ -148,6 +150,14 @@ def test_logpsi_matches_numpy_slogdet_and_explicit_jastrow():
     J3 = np.sum(np.triu(M, 1))
     la3, sg3 = o3.logpsi(x)
     assert sg3 == sg and abs(la3 - (la + J3)) < 1e-12 and abs(J3) > 1e-3
+    # the same with p and cartesian d functions and more than 8 of them: chi_a = dx^l dy^m dz^n exp(-zeta_a |d|^2), d = r - R_a
+    sp = wl.with_jastrow3(s, 5, 6, n_max=12, poly=True); op = ref.Ref(sp)
+    assert len(sp["j3_zeta"]) == 12 and set(map(int, sp["j3_lmn"].sum(axis=1))) == {0, 1, 2}
+    d = x[:, None, :] - s["R"][sp["j3_center"]][None, :, :]                                                              # [electron][a][3]
+    chi = np.prod(d ** sp["j3_lmn"][None, :, :], axis=2) * np.exp(-sp["j3_zeta"][None, :] * np.sum(d * d, axis=2))
+    J3p = np.sum(np.triu(chi @ sp["j3_g"] @ chi.T, 1))
+    lap_, sgp = op.logpsi(x)
+    assert sgp == sg and abs(lap_ - (la + J3p)) < 1e-12 and abs(J3p) > 1e-3
 
 
 @pytest.mark.parametrize("name", ["tiny-2u1d", "tiny-3u3d-pp", "C2"])

@@ -205,6 +205,32 @@ def test_contracted_shell_is_the_stated_sum_of_normalised_primitives_with_correc
     assert np.allclose(l, lap_fd, atol=2e-7)
 
 
+def test_contracted_slater_shell_is_the_stated_sum_with_correct_derivatives():
+    """Scope row f2, contracted Slater shells: chi = sum_k d_k exp(-zeta_k |r - R|) written out; gradient and Laplacian against
+    the closed forms grad = -sum d_k zeta_k e^{-zeta_k r} rhat, lap = sum d_k e^{-zeta_k r} (zeta_k^2 - 2 zeta_k / r) and against finite
+    differences; the Gaussian p / solid-harmonic d shells beside them keep their own pins (same code path as before)."""
+    s = wl.contracted_slater_molecule(); o = ref.Ref(s)
+    assert s["n_ao"] == 4 + 3 + 5 and s["n_shell"] == 10
+    rng = np.random.default_rng(2)
+    prim = [(0, [(2.6, 0.5), (1.4, 0.4), (0.9, 0.2)]), (1, [(3.1, 0.7), (1.1, -0.3)]), (0, [(0.7, 1.0)]), (1, [(0.8, 1.0)])]
+    for _ in range(5):
+        r = rng.normal(size=3) * 1.2; v, g, l = o.ao(r)
+        for mu, (I, terms) in enumerate(prim):
+            d = r - s["R"][I]; rr = np.linalg.norm(d)
+            val = sum(c * math.exp(-z * rr) for z, c in terms)
+            grad = -sum(c * z * math.exp(-z * rr) for z, c in terms) * d / rr
+            lap = sum(c * math.exp(-z * rr) * (z * z - 2 * z / rr) for z, c in terms)
+            assert abs(v[mu] - val) < 1e-15 and np.abs(g[mu] - grad).max() < 1e-14 and abs(l[mu] - lap) < 1e-13
+        h = 1e-3                                          # 4th-order finite differences of every function (incl. the p and d shells)
+        lap_fd = np.zeros(s["n_ao"])
+        for ax in range(3):
+            e = np.zeros(3); e[ax] = h
+            fp, fm, fpp, fmm = o.ao(r + e)[0], o.ao(r - e)[0], o.ao(r + 2 * e)[0], o.ao(r - 2 * e)[0]
+            assert np.abs(g[:, ax] - (-fpp + 8 * fp - 8 * fm + fmm) / (12 * h)).max() < 1e-9
+            lap_fd += (-fpp + 16 * fp - 30 * v + 16 * fm - fmm) / (12 * h * h)
+        assert np.abs(l - lap_fd).max() < 2e-6
+
+
 def test_mo_is_ao_times_coefficients():
     s = wl.synthetic10(); o = ref.Ref(s); r = np.array([0.3, -0.8, 0.5])
     av, ag, al = o.ao(r); mv, mg, ml = o.mo(0, r)
