@@ -130,8 +130,9 @@ __device__ __forceinline__ void pade_six(double dx, double dy, double dz, const 
 // Three-body Jastrow at the six displaced points x0 +- av[k] of one electron (reading Q23): Jn[d] += sum_a chi_a(point d) V_a,
 // the functions dealt over the `stride` lanes that share the electron (t = this lane's index among them, a = a0 + t): six table
 // exponentials per function in the same +- form as the AOs.  The trip count is uniform in the warp (exp_tab_n synchronises it).
-__device__ __forceinline__ void j3_six(const DevSys &S, const Tables &T, const double *V3, double x0, double y0, double z0, const double (&av)[3][3],
-                                       double a2, int t, double (&Jn)[6], int a_first = 0, int a_stride = 4)
+template <bool POLY>
+__device__ __forceinline__ void j3_six_loop(const DevSys &S, const Tables &T, const double *V3, double x0, double y0, double z0, const double (&av)[3][3],
+                                            double a2, int t, double (&Jn)[6], int a_first, int a_stride)
 {
     for (int a0 = a_first; a0 < S.n_j3; a0 += a_stride) {
         const bool on = a0 + t < S.n_j3; const int a = on ? a0 + t : 0;
@@ -145,7 +146,7 @@ __device__ __forceinline__ void j3_six(const DevSys &S, const Tables &T, const d
         }
         exp_tab_n<6>(ex_, e_, T.etab);
         const double Va = on ? V3[a] : 0.0;
-        if (S.j3_poly) {               // monomial factor at the displaced points d0 +- av[k] (uniform branch: a property of the system)
+        if (POLY) {                    // monomial factor at the displaced points d0 +- av[k]
             const int q = S.j3_lmn[a], kx = q & 3, ky = (q >> 2) & 3, kz = (q >> 4) & 3;
 #pragma unroll
             for (int k = 0; k < 3; ++k) {
@@ -158,6 +159,12 @@ __device__ __forceinline__ void j3_six(const DevSys &S, const Tables &T, const d
             for (int d = 0; d < 6; ++d) Jn[d] = fma(e_[d], Va, Jn[d]);
         }
     }
+}
+__device__ __forceinline__ void j3_six(const DevSys &S, const Tables &T, const double *V3, double x0, double y0, double z0, const double (&av)[3][3],
+                                       double a2, int t, double (&Jn)[6], int a_first = 0, int a_stride = 4)
+{
+    if (S.j3_poly) j3_six_loop<true>(S, T, V3, x0, y0, z0, av, a2, t, Jn, a_first, a_stride);      // uniform: a property of the system
+    else j3_six_loop<false>(S, T, V3, x0, y0, z0, av, a2, t, Jn, a_first, a_stride);
 }
 
 // ---- non-local pseudopotential candidates (scope row f1; include/lrdmc.h lrdmc_system.nl) ------------------------------

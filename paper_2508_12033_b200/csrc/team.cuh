@@ -71,6 +71,18 @@ __device__ __forceinline__ void store_walker_team(const DevSys &S, const DevWalk
     if (S.moc_in_smem) for (int i = tid; i < (int)mocn; i += nthr) W.moc[(size_t)k * mocn + i] = ws.moc[i];
 }
 
+// The draws of step `step` of walker `slot` (row a0) by one warp: frame U in out[0..8], u_sel in out[10], u_tau in out[11].
+__device__ __forceinline__ void team_step_frame(const DevSys &S, double *out, uint32_t slot, uint32_t cycle, uint32_t step, bool need_tau, int lane)
+{
+    const StepDraws d = step_draws(S, slot, cycle, step, need_tau);
+    if (lane == 0) {
+        double U[9]; lattice_frame(d.u1, d.u2, d.u3, U);
+#pragma unroll
+        for (int i = 0; i < 9; ++i) out[i] = U[i];
+        out[10] = d.u_sel; out[11] = d.u_tau;
+    }
+}
+
 // One evaluation by the team.  The result is valid in warp 0 only (it runs phase C); ws.R / ws.cum are complete for everyone
 // after the caller's next barrier.  s_vee: TW doubles of static shared memory.
 // BCS: parked Bc entries (wavefunction.cuh, ao_columns): bcs_cta = this CTA's scratch [block of a mesh][k-step pair][lane];
@@ -393,6 +405,7 @@ __global__ void __launch_bounds__(LRDMC_TEAM_MAX_WARPS * 32, 1) k_propagate_team
 {
     extern __shared__ __align__(16) double smem[];
     __shared__ double s_vee[LRDMC_TEAM_MAX_WARPS];
+    __shared__ double s_frame[2][12];   // per step parity: lattice frame U [9], pad, u_sel, u_tau (team_step_frame)
     __shared__ int s_ctrl[8];      // [0] walker, [1] last, [2] selected move, [3] node flag of the slots, [4] listed slots, [5] spin cut of the list
     stage_tables(S, smem);
     const int tid = threadIdx.x, lane = tid & 31, wt = tid >> 5;
@@ -424,14 +437,19 @@ __global__ void __launch_bounds__(LRDMC_TEAM_MAX_WARPS * 32, 1) k_propagate_team
         }
         uint32_t s = 0; int reuse_spin = -1;
         double w = 1.0, tau_left = tau, omega = 0.0, eL_last = 0.0, W_last = 0.0; long long moves = 0; int n_node = 0, n_nonpos = 0;
+        // The draws and the frame of step s depend on (walker, cycle, s) alone: the last warp prepares those of step s + 1 in the
+        // other half of s_frame while the leader warp runs phase C and the selection of step s -- off the critical path of the step.
+        if (wt == P.TW - 1) team_step_frame(S, s_frame[0], (uint32_t)k, cycle, 0u, mode == LRDMC_CONVENTIONAL, lane);
+        if (tid == 0) s_ctrl[3] = 0;
+        __syncthreads();
         for (;;) {
-            const StepDraws d = step_draws(S, (uint32_t)k, cycle, s, mode == LRDMC_CONVENTIONAL);
-            if (tid == 0) { s_ctrl[3] = 0; double U[9]; lattice_frame(d.u1, d.u2, d.u3, U);
-#pragma unroll
-                for (int i = 0; i < 9; ++i) ws.U[i] = U[i]; }
-            __syncthreads();
+            double *fr = s_frame[s & 1];
+            ws.U = fr;
             const EvalOut e = evaluate_team<NT, TS, EXT, BCS>(S, P, ws, T, scr, s_vee, &s_ctrl[3], bcs_cta, reuse_spin);
+            if (wt == P.TW - 1) team_step_frame(S, s_frame[(s + 1) & 1], (uint32_t)k, cycle, s + 1, mode == LRDMC_CONVENTIONAL, lane);
             if (wt == 0) {                                       // the leader warp keeps the weight (same rules as k_propagate)
+                StepDraws d; d.u_sel = fr[10]; d.u_tau = fr[11];
+                if (lane == 0) s_ctrl[3] = 0;                    // node flag of the slots: consumed by phase C, clear for the next evaluation
                 n_node += e.node;
                 bool last = false;
                 if (mode == LRDMC_BALANCED) {
