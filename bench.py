@@ -160,6 +160,7 @@ def main():
                     help="K independent ensembles of --nw walkers each (own context, own CUDA stream, own seed) in flight together: the paper's "
                          "small-ensemble regime (100 walkers per GPU, L289) and the several-a batch of SURVEY 8(f) f3; value = aggregate over the K")
     ap.add_argument("--team", type=int, default=0, help="lrdmc_set_option(LRDMC_OPT_TEAM_WARPS): 0 = automatic")
+    ap.add_argument("--listed", type=int, default=-1, help="lrdmc_set_option(LRDMC_OPT_LISTED): -1 = automatic, 0 = dense candidate sweep, 1 = listed sweep on stored Bc")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1")); local = int(os.environ.get("LOCAL_RANK", "0"))
     if args.impl == "reference":
@@ -180,7 +181,10 @@ def main():
     ctxs = []
     for q in range(K):
         sysd, wname, x0 = make_workload(args, rank, q)
-        g = B.Lrdmc(sysd, device=dev, options={B.OPT_TEAM_WARPS: args.team} if args.team else None)
+        opts = {}
+        if args.team: opts[B.OPT_TEAM_WARPS] = args.team
+        if args.listed >= 0: opts[B.OPT_LISTED] = args.listed
+        g = B.Lrdmc(sysd, device=dev, options=opts or None)
         g.stream = torch.cuda.Stream(device=dev) if K > 1 else torch.cuda.current_stream(dev)
         with torch.cuda.stream(g.stream):
             g.lrdmc_set_positions(x0, allow_singular=True)

@@ -118,8 +118,12 @@ int lrdmc_n_candidates(const lrdmc_ctx *); /* P = 6 N n_mesh + 6 N nl_K */
  *                           many warps per walker (north_star "one CTA or warp group per walker"); other values are rounded down to
  *                           a power of two.  The parity tests run every size.
  *   LRDMC_OPT_GLOBAL_TABLES value != 0: keep the MO-coefficient fragment tables and the MO cache in global memory even when
- *                           they fit shared memory (the code path of the 64-electron configuration, forced on small systems by tests). */
-enum { LRDMC_OPT_TEAM_WARPS = 1, LRDMC_OPT_GLOBAL_TABLES = 2 };
+ *                           they fit shared memory (the code path of the 64-electron configuration, forced on small systems by tests).
+ *   LRDMC_OPT_LISTED        candidate pass of lattice-only systems (no non-local slots, no three-body Jastrow) as a LISTED sweep: per-electron
+ *                           lists of the shells within reach (every dropped exponent < -52) and Bc = C Dinv kept as rank-1-updated walker
+ *                           state instead of recomputed.  value -1 = automatic (default), 0 = dense sweep, 1 = listed.
+ *                           Ignored (dense) for systems with slots or a three-body Jastrow. */
+enum { LRDMC_OPT_TEAM_WARPS = 1, LRDMC_OPT_GLOBAL_TABLES = 2, LRDMC_OPT_LISTED = 3 };
 int lrdmc_set_option(lrdmc_ctx *, int option, int value);
 
 /* ---- walker storage: structure of arrays in ONE caller-owned device buffer ---------------------------

@@ -16,7 +16,7 @@ BALANCED, CONVENTIONAL = 0, 1
 OK, EINVAL, ESINGULAR, ESTATE, ECUDA, ENOMEM = 0, -1, -2, -3, -4, -5
 
 PROBE_LIB_PATH = os.path.join(_HERE, "liblrdmc_probe.so")                     # include/lrdmc_probe.h (bench.py's roofline denominators)
-OPT_TEAM_WARPS, OPT_GLOBAL_TABLES = 1, 2
+OPT_TEAM_WARPS, OPT_GLOBAL_TABLES, OPT_LISTED = 1, 2, 3
 
 # every symbol this module touches; tests check that include/lrdmc.h (resp. lrdmc_probe.h) declares each and the libraries export each
 EXPORTS = ["lrdmc_init", "lrdmc_free", "lrdmc_strerror", "lrdmc_last_error", "lrdmc_set_option", "lrdmc_n_candidates", "lrdmc_walker_bytes",

@@ -3,8 +3,8 @@
     python -m paper_2508_12033_b200.build [--force] [-v]
 
 Translation units (compiled in parallel, then linked): lrdmc.cu (C-ABI, host logic, rebuild / reconfigure / reduction kernels),
-lrdmc_aux.cu (estimators over generations, host-buffer driver, test hooks) and kernels.cu eight times -- the walker kernels
-{lattice only, + non-local pseudopotential slots, + three-body Jastrow, + both} x {warp-per-walker, team}.
+lrdmc_aux.cu (estimators over generations, host-buffer driver, test hooks) and kernels.cu ten times -- the walker kernels
+{lattice only, + non-local pseudopotential slots, + three-body Jastrow, + both, lattice only as a listed sweep} x {warp-per-walker, team}.
 """
 from __future__ import annotations
 
@@ -20,7 +20,7 @@ OBJDIR = os.path.join(HERE, "build")
 # (source, object name, extra defines)
 UNITS = [("lrdmc.cu", "lrdmc.o", []), ("lrdmc_aux.cu", "lrdmc_aux.o", [])] + [
     ("kernels.cu", f"kernels_e{ext}_{'team' if team else 'warp'}.o", [f"-DLRDMC_EXT={ext}", f"-DLRDMC_TEAM_TU={team}"])
-    for ext in (0, 1, 2, 3) for team in (0, 1)]
+    for ext in (0, 1, 2, 3, 4) for team in (0, 1)]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC"]
 
 

@@ -58,12 +58,13 @@ struct DevSys {
     int n_kpairs, off_cf[2];   // pairs of k-steps (each shell group padded to an even number of k-steps)
     // listed candidate sweep (team kernel of the large systems): sorted slots in list groups of one type and at most 64 slots
     int n_lg, lg_type[LRDMC_MAX_LG], lg_slot0[LRDMC_MAX_LG], lg_n[LRDMC_MAX_LG], lg_ao0[LRDMC_MAX_LG];
+    int lg_off[LRDMC_MAX_LG], lt;   // byte offset of a list group inside an electron's list row; lt = bytes per electron (sum of lg_n, multiple of 4)
     int n_aop;                 // AO count of the sorted, padded shell list (slot-major: components of a shell are consecutive)
-    int off_srad, o_am;        // shared memory: srad [n_slots] in the tables; per walker: listed-shell masks [N][n_lg] (64 bit each)
+    int off_srad, o_am;        // shared memory: srad [n_slots] in the tables; per walker: the listed-shell lists (listed.cuh), (N (lt + n_lg) + 7) / 8 doubles
     const double *srad;        // [n_slots] screening radii (LRDMC_LIST_THR); padded slots: -1e300 (never listed)
     const double *cn[2];       // [n_aop][OS] MO coefficients with the AO norms folded in, slot-major (Bc = C Dinv by rows)
     // shared-memory plan (units: doubles)
-    int bf_in_smem, moc_in_smem;
+    int bf_in_smem, moc_in_smem, cf_in_smem;   // cf_in_smem: the pair table of ao_columns is staged too (not with the listed sweep)
     int off_shells, off_nuc, off_bf[2], off_etab, tables_doubles;
     int o_r, o_dinv[2], o_moc, o_R, o_cum, o_el, o_ob, o_U, o_j3, per_warp_doubles;   // o_j3: chi3 [N][j3s], V3 [N][j3s], S3 [j3s] (systems with a J3)
     int dinv_rows[2];     // padded row count 8*NT
@@ -86,8 +87,7 @@ struct TeamPlan {
     int pair_base[4];     // first k-step pair of each group in the `cf` fragment table
     int mesh_share;       // both meshes of a block are handled by the same warp: the second takes the first's parked Bc entries
     int o_scr, scr_doubles; // scratch (partial sums) behind the walker state, in doubles from the state base
-    int listed;           // the candidate pass is the listed sweep (large systems without slots / J3): rows of RB (mesh, electron) pairs per warp batch
-    int RB;
+    int listed;           // the candidate pass is the listed sweep (listed.cuh): 8-row batches (mesh, electron) dealt to the warps
     ShellPart col[LRDMC_TEAM_MAX_PARTS];     // parts of ao_columns (groups 0-2 start on even iterations: k-step pairs)
     ShellPart mo[LRDMC_TEAM_MAX_WARPS];      // parts of the derivative pass of the mover (one per warp)
 };

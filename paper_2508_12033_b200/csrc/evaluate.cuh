@@ -5,11 +5,13 @@
 #include "fastmath.cuh"
 #include "philox.cuh"
 #include "wavefunction.cuh"
+#include "listed.cuh"
 
 struct WarpState {            // per-warp views (shared memory; moc may live in global memory for large systems)
     double *r, *dinv[2], *moc, *R, *cum, *el, *ob, *U;
     double *j3;               // three-body Jastrow (systems that have one): chi3 [N][j3s] = chi_a(r_j), then V3 [N][j3s], then S3 [j3s]
-    unsigned long long *am;   // listed sweep (large systems): listed-shell masks [N][n_lg]
+    unsigned char *lw;        // listed sweep: this walker's listed-shell lists (listed.cuh: counts [n_lg][N], slots [N][lt])
+    double *bc;               // listed sweep: this walker's Bc = C Dinv [N][n_aop] (global scratch of the resident warp / CTA, rank-1 updated)
 };
 struct EvalOut { double bbar, Vsf, W, eL; int node; };
 
@@ -359,12 +361,48 @@ __device__ __forceinline__ EvalOut phase_c(const DevSys &S, const WarpState &ws,
     return o;
 }
 
+// Phase B as a LISTED sweep (listed.cuh; EXT bit 2) of the 8-row batches first, first + stride, ... of the rows (mesh, electron) by one warp:
+// quad per row, the determinant ratios from the walker's stored Bc over the electron's own shell lists, the Jastrow ratios of the same
+// rows from the same geometry, R_j = ratio * exp(J' - J).  Rows are independent, so a warp finishes its batches without meeting the others.
+__device__ __forceinline__ void listed_phase_b(const DevSys &S, const WarpState &ws, const Tables &T, const double *Jold, int first, int stride, int lane)
+{
+    const int N = S.N, n_nuc = S.n_nuc, t = lane & 3, g = lane >> 2, n_rows = S.n_mesh * N;
+    for (int r0 = 8 * first; r0 < n_rows; r0 += 8 * stride) {
+        const bool valid = r0 + g < n_rows;
+        const int rho = valid ? r0 + g : r0, mesh = rho / N, i = rho - mesh * N, sp = spin_of(S, i);
+        const double x0 = ws.r[3 * i], y0 = ws.r[3 * i + 1], z0 = ws.r[3 * i + 2], am_ = S.amesh[mesh], a2 = am_ * am_;
+        double av[3][3], acc[6], Jn[6];
+#pragma unroll
+        for (int k = 0; k < 3; ++k) { av[k][0] = am_ * ws.U[k]; av[k][1] = am_ * ws.U[3 + k]; av[k][2] = am_ * ws.U[6 + k]; }
+        ao_listed_quad(S, T.shells, T.etab, ws.lw, ws.bc, i, valid, x0, y0, z0, av, a2, lane, acc);
+#pragma unroll
+        for (int d = 0; d < 6; ++d) Jn[d] = 0.0;
+        if (S.has_j1) for (int I = t; I < n_nuc; I += 4) {
+            const double *np_ = T.nuc + I * LRDMC_NUC_STRIDE;
+            pade_six(x0 - np_[0], y0 - np_[1], z0 - np_[2], av, a2, -np_[4], np_[5], Jn);
+        }
+        for (int j = t; j < N; j += 4) {
+            const double c = (j == i) ? 0.0 : ((spin_of(S, j) == sp) ? S.a_par : S.a_anti);
+            pade_six(x0 - ws.r[3 * j], y0 - ws.r[3 * j + 1], z0 - ws.r[3 * j + 2], av, a2, c, S.b2, Jn);
+        }
+        const double Jo = Jold[i];
+        double Rv[6];
+#pragma unroll
+        for (int d = 0; d < 6; ++d) Rv[d] = quad_sum(acc[d]) * exp_tab(quad_sum(Jn[d]) - Jo, T.etab);
+        if (valid && t == 0) {
+            double *Ro = ws.R + mesh * 6 * N + 6 * i;
+#pragma unroll
+            for (int d = 0; d < 6; ++d) Ro[d] = Rv[d];
+        }
+    }
+}
+
 // EXT (extended kernels, separate instantiations so that each system pays only for what it has): bit 0 = non-local
-// pseudopotential slots (row f1), bit 1 = three-body Jastrow (row f2).
+// pseudopotential slots (row f1), bit 1 = three-body Jastrow (row f2), bit 2 = listed candidate sweep on stored Bc (listed.cuh; lattice-only systems).
 template <int NT, bool TS, int EXT = 0>
 __device__ __forceinline__ EvalOut evaluate_walker(const DevSys &S, const WarpState &ws, const Tables &T, int lane)
 {
-    constexpr bool SLOTS = (EXT & 1) != 0, J3 = (EXT & 2) != 0;
+    constexpr bool SLOTS = (EXT & 1) != 0, J3 = (EXT & 2) != 0, LISTED = (EXT & 4) != 0;
     const int N = S.N, n_nuc = S.n_nuc;
     const int t = lane & 3, g = lane >> 2;
     double *Jold = ws.el, *lap_s = ws.el + N;
@@ -410,7 +448,8 @@ __device__ __forceinline__ EvalOut evaluate_walker(const DevSys &S, const WarpSt
     __syncwarp();
 
     // ---- phase B (rows a1-a5): the 6 n_s candidates of each spin, 8 electrons (48 points) per warp pass in column form
-    if (!SLOTS) for (int mesh = 0; mesh < S.n_mesh; ++mesh) {
+    if (LISTED) listed_phase_b(S, ws, T, Jold, 0, 1, lane);
+    if (!SLOTS && !LISTED) for (int mesh = 0; mesh < S.n_mesh; ++mesh) {
         const double am = S.amesh[mesh], a2 = am * am;
         double av[3][3];                                             // av[k] = a e_k, e_k = k-th column of U (Eq.D3-D4)
 #pragma unroll
@@ -490,6 +529,7 @@ __device__ __forceinline__ void apply_move(const DevSys &S, const WarpState &ws,
     refresh_mo_cache<NT, TS>(S, T.shells, sp ? T.bf[1] : T.bf[0], T.etab, mc, px, py, pz, lane);
     refresh_onebody(S.n_nuc, S.has_j1, S.a, T.nuc, ws.ob + 8 * i, px, py, pz, lane);
     if (EXT & 2) refresh_j3_row(S, T.nuc, ws.j3 + i * S.j3s, px, py, pz, lane);
+    if (EXT & 4) list_build(S, T.shells, T.srad, ws.lw, i, px, py, pz, fmax(S.amesh[0], S.amesh[1]), lane);   // the mover's listed shells at its new position
     if (lane == 0) { ws.r[3 * i] = px; ws.r[3 * i + 1] = py; ws.r[3 * i + 2] = pz; }
     __syncwarp();
     // s_k = sum_m phi_m Dinv[m][k];  rho = s_il;  Dinv'[m][il] = Dinv[m][il]/rho;  Dinv'[m][k] = Dinv[m][k] - Dinv[m][il] s_k / rho
@@ -506,5 +546,6 @@ __device__ __forceinline__ void apply_move(const DevSys &S, const WarpState &ws,
         const double ci = col[m] * irho;
         dinv[idx] = (kk == il) ? ci : dinv[idx] - ci * sk[kk];
     }
+    if (EXT & 4) bc_rank1_update(S, ws.bc, sp, il, ns, sk, irho, lane, 32);
     __syncwarp();
 }

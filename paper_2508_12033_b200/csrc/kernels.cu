@@ -1,5 +1,5 @@
-// kernels.cu -- the walker kernels' launchers.  This one source is compiled EIGHT times (build.py: -DLRDMC_EXT=0|1|2|3 x
-// -DLRDMC_TEAM_TU=0|1, in parallel): EXT bit 0 = non-local pseudopotential slots, bit 1 = three-body Jastrow (separate code, so
+// kernels.cu -- the walker kernels' launchers.  This one source is compiled TEN times (build.py: -DLRDMC_EXT=0|1|2|3|4 x
+// -DLRDMC_TEAM_TU=0|1, in parallel): EXT bit 0 = non-local pseudopotential slots, bit 1 = three-body Jastrow, 4 = listed candidate sweep on stored Bc (lattice-only systems; listed.cuh) (separate code, so
 // that every system keeps the register allocation of what it actually has: inlined behind runtime flags the slots cost the
 // lattice-only kernel 284 B of spills and 9 % of the C4 throughput; slots and J3 in one instantiation spilled 196 B),
 // TEAM_TU = the team kernel / the warp-per-walker kernels.  lrdmc.cu (host logic) calls them through kernels.h.
@@ -12,7 +12,7 @@
 #include "kernels.h"
 
 #ifndef LRDMC_EXT
-#error "compile with -DLRDMC_EXT=0, 1, 2 or 3"
+#error "compile with -DLRDMC_EXT=0, 1, 2, 3 or 4"
 #endif
 #if LRDMC_EXT == 0
 #define KFN(name) name##_e0
@@ -20,8 +20,10 @@
 #define KFN(name) name##_e1
 #elif LRDMC_EXT == 2
 #define KFN(name) name##_e2
-#else
+#elif LRDMC_EXT == 3
 #define KFN(name) name##_e3
+#else
+#define KFN(name) name##_e4
 #endif
 static constexpr int kNL = LRDMC_EXT;
 

@@ -1,5 +1,5 @@
 // kernels.h -- launchers of the walker kernels (kernels.cu, compiled once per EXT in {0: lattice only, 1: non-local slots, 2: three-body
-// Jastrow, 3: both} x {warp-per-walker, team});
+// Jastrow, 3: both, 4: lattice only as a listed sweep on stored Bc} x {warp-per-walker, team});
 // internal to liblrdmc, not part of the C-ABI.
 #pragma once
 #include "common.cuh"
@@ -18,6 +18,7 @@ LRDMC_K_DECL(e0)
 LRDMC_K_DECL(e1)
 LRDMC_K_DECL(e2)
 LRDMC_K_DECL(e3)
+LRDMC_K_DECL(e4)
 #undef LRDMC_K_DECL
 // dispatch on the run-time EXT value of a system
-#define LRDMC_K_CALL(ext, name, ...) ((ext) == 0 ? name##_e0(__VA_ARGS__) : (ext) == 1 ? name##_e1(__VA_ARGS__) : (ext) == 2 ? name##_e2(__VA_ARGS__) : name##_e3(__VA_ARGS__))
+#define LRDMC_K_CALL(ext, name, ...) ((ext) == 0 ? name##_e0(__VA_ARGS__) : (ext) == 1 ? name##_e1(__VA_ARGS__) : (ext) == 2 ? name##_e2(__VA_ARGS__) : (ext) == 3 ? name##_e3(__VA_ARGS__) : name##_e4(__VA_ARGS__))

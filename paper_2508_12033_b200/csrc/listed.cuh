@@ -18,27 +18,15 @@
 #include "common.cuh"
 #include "fastmath.cuh"
 
-__device__ __forceinline__ int warp_sum_int(int v)
+// Per-walker lists (shared memory, bytes): cnt [n_lg][N] listed-shell counts, then lst [N][lt] slot numbers (relative to the list group's first
+// slot), the groups of an electron at lg_off[lg].  A shell is listed for electron i when |r_i - R_shell| < step_max + srad: the test depends on the
+// position only, so the lists are kept with the walker state and rebuilt for the electron that hopped.
+__device__ __forceinline__ int list_doubles(const DevSys &S) { return (S.N * (S.lt + S.n_lg) + 7) >> 3; }
+__device__ __forceinline__ void list_build(const DevSys &S, const double *shells, const double *srad, unsigned char *lw, int i, double x, double y, double z,
+                                           double step_max, int lane)
 {
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-    return v;
-}
-
-// position of the n-th (0-based) set bit of a 64-bit mask (n < popcount)
-__device__ __forceinline__ int nth_set_bit64(unsigned long long m, int n)
-{
-    const unsigned lo = (unsigned)m, hi = (unsigned)(m >> 32);
-    const int pl = __popc(lo);
-    return n < pl ? (int)__fns(lo, 0, n + 1) : 32 + (int)__fns(hi, 0, n - pl + 1);
-}
-
-// Listed-shell masks of one point for the list groups lg = first, first + stride, ...: bit q of group lg = slot lg_slot0 + q is within
-// step_max + srad of (x, y, z).  One warp; lane 0 writes am_i[lg].
-__device__ __forceinline__ void list_masks(const DevSys &S, const double *shells, const double *srad, unsigned long long *am_i, double x, double y,
-                                           double z, double step_max, int lane, int first, int stride)
-{
-    for (int lg = first; lg < S.n_lg; lg += stride) {
+    unsigned char *cnt = lw, *lrow = lw + S.n_lg * S.N + i * S.lt;
+    for (int lg = 0; lg < S.n_lg; ++lg) {
         unsigned w[2];
 #pragma unroll
         for (int h = 0; h < 2; ++h) {
@@ -48,7 +36,58 @@ __device__ __forceinline__ void list_masks(const DevSys &S, const double *shells
             const double dx = x - sh.x, dy = y - sh.y, dz = z - sh.z, rad = step_max + srad[q];
             w[h] = __ballot_sync(0xffffffffu, in && rad > 0.0 && dx * dx + dy * dy + dz * dz < rad * rad);
         }
-        if (lane == 0) am_i[lg] = ((unsigned long long)w[1] << 32) | w[0];
+        unsigned char *l = lrow + S.lg_off[lg];
+        const unsigned below = (1u << lane) - 1u; const int n0 = __popc(w[0]);
+        if ((w[0] >> lane) & 1u) l[__popc(w[0] & below)] = (unsigned char)lane;
+        if ((w[1] >> lane) & 1u) l[n0 + __popc(w[1] & below)] = (unsigned char)(lane + 32);
+        if (lane == 0) cnt[lg * S.N + i] = (unsigned char)(n0 + __popc(w[1]));
+    }
+}
+
+// Bc = C Dinv of one walker, [electron][n_aop], by the threads tid = 0 .. nthr-1 (a warp or a CTA): thread = one AO row of C (slot-major, norms
+// folded in), eight inverse columns at a time.  Built when the walker is loaded (reading Q15: the state is rebuilt wherever the inverse is).
+__device__ __forceinline__ void build_bc(const DevSys &S, const double *dinv0, const double *dinv1, double *__restrict__ bc, int tid, int nthr)
+{
+    const int A = S.n_aop, OS = S.OS;
+    for (int sp = 0; sp < 2; ++sp) {
+        const int ns = sp ? S.n_dn : S.n_up, off = sp ? S.n_up : 0;
+        if (!ns) continue;
+        const double *__restrict__ cn = S.cn[sp], *dinv = sp ? dinv1 : dinv0;
+        for (int ao = tid; ao < A; ao += nthr) {
+            const double *crow = cn + (size_t)ao * OS;
+            for (int il0 = 0; il0 < ns; il0 += 8) {
+                double acc[8];
+#pragma unroll
+                for (int j = 0; j < 8; ++j) acc[j] = 0.0;
+                for (int m = 0; m < ns; ++m) {
+                    const double cv = __ldg(crow + m); const double *dr = dinv + m * ns + il0;   // columns beyond n_s read padding, never stored
+#pragma unroll
+                    for (int j = 0; j < 8; ++j) acc[j] = fma(cv, dr[j], acc[j]);
+                }
+#pragma unroll
+                for (int j = 0; j < 8; ++j) if (il0 + j < ns) bc[(size_t)(off + il0 + j) * A + ao] = acc[j];
+            }
+        }
+    }
+}
+
+// Bc follows the inverse by the same rank-1 formula after electron i (spin sp, column il) hopped: Bc'[:,k] = Bc[:,k] - Bc[:,il] s_k / rho,
+// Bc'[:,il] = Bc[:,il] / rho.  Thread = one AO (consecutive threads on consecutive AOs: coalesced), eight columns in flight at a time; a thread
+// touches the entries of its own AOs only, so no barrier is needed inside.
+__device__ __forceinline__ void bc_rank1_update(const DevSys &S, double *bc, int sp, int il, int ns, const double *sk, double irho, int tid, int nthr)
+{
+    const size_t A = (size_t)S.n_aop;
+    double *b0 = bc + (size_t)(sp ? S.n_up : 0) * A;
+    for (int ao = tid; ao < (int)A; ao += nthr) {
+        double *p = b0 + ao;
+        const double f = __ldcg(p + (size_t)il * A) * irho;
+        for (int k0 = 0; k0 < ns; k0 += 8, p += 8 * A) {
+            double v[8];
+#pragma unroll
+            for (int q = 0; q < 8; ++q) v[q] = (k0 + q < ns) ? __ldcg(p + q * A) : 0.0;
+#pragma unroll
+            for (int q = 0; q < 8; ++q) if (k0 + q < ns) __stcg(p + q * A, (k0 + q == il) ? f : fma(-f, sk[k0 + q], v[q]));
+        }
     }
 }
 
@@ -71,58 +110,30 @@ __device__ __forceinline__ SixGeom six_gaussians(const double4 s, double x0, dou
     return G;
 }
 
-// The listed sweep of the rows rho0 .. rho0 + nrows - 1 (row = mesh N + electron; nrows <= 32, best <= 16) by ONE warp:
-// R[mesh 6N + 6 i + d] <- sum over the listed shells of chi(x_i +- a_mesh e_k) . Bc[i][.]   (the determinant ratio of candidate (i, d)).
-//   r_el [N][3] positions, U the step's frame, am [N][n_lg] listed-shell masks, bc [N][n_aop] this walker's Bc.
-__device__ __forceinline__ void ao_listed_warp(const DevSys &S, const double *__restrict__ shells, const double *__restrict__ etab,
-                                               const double *__restrict__ r_el, const double *__restrict__ U, const unsigned long long *__restrict__ am,
-                                               const double *__restrict__ bc, int rho0, int nrows, double *__restrict__ R, int lane)
+// The listed sweep of ONE row per quad (lane = 4 g + t: row g of the batch, t = which of four listed shells taken together): the share of lane t in
+//     sum over the listed shells of chi(x0 +- av[k]) . Bc[i][.]        (the determinant ratios of the six candidates of electron i on this mesh);
+// the caller adds the four lanes of a quad.  Every quad walks ITS electron's lists; a list group takes ceil(max over the 8 rows of n / 4) iterations.
+//   lw this walker's lists, bc its Bc [N][n_aop], valid = the quad holds a row (idle quads run with coefficient 0).
+__device__ __forceinline__ void ao_listed_quad(const DevSys &S, const double *__restrict__ shells, const double *__restrict__ etab, const unsigned char *lw,
+                                               const double *__restrict__ bc, int i, bool valid, double x0, double y0, double z0, const double (&av)[3][3], double a2,
+                                               int lane, double (&acc)[6])
 {
-    const int N = S.N, A = S.n_aop;
-    const bool inr = lane < nrows;
-    const int my_rho = rho0 + (inr ? lane : 0), my_mesh = my_rho / N, my_i = my_rho - my_mesh * N;
-    if (inr) { double *Ro = R + my_mesh * 6 * N + 6 * my_i;
+    const int t = lane & 3, N = S.N;
+    const unsigned char *cnt = lw + i, *lrow = lw + S.n_lg * N + i * S.lt;
+    const double *bci = bc + (size_t)i * S.n_aop;
 #pragma unroll
-        for (int d = 0; d < 6; ++d) Ro[d] = 0.0; }
-    __syncwarp();
+    for (int d = 0; d < 6; ++d) acc[d] = 0.0;
     for (int lg = 0; lg < S.n_lg; ++lg) {
-        const unsigned long long mk = inr ? am[my_i * S.n_lg + lg] : 0ull;
-        const int n_r = __popcll(mk);
-        const int total = warp_sum_int(n_r);
-        if (total == 0) continue;                                        // (uniform)
-        int c = (total + 31) >> 5;
-        for (;;) { if (warp_sum_int((n_r + c - 1) / c) <= 32) break; ++c; }
-        const int m_r = (n_r + c - 1) / c;                                // lanes of this row
-        int incl = m_r;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += v; }
-        const int start = incl - m_r, used = __shfl_sync(0xffffffffu, incl, 31);
-        int mmax = m_r;
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) mmax = max(mmax, __shfl_xor_sync(0xffffffffu, mmax, o));
-        int row = 0;
-        for (int r = 1; r < nrows; ++r) { const int s = __shfl_sync(0xffffffffu, start, r); if (lane >= s) row = r; }
-        const bool has = lane < used;
-        const int rstart = __shfl_sync(0xffffffffu, start, row), rend = rstart + __shfl_sync(0xffffffffu, m_r, row);   // lanes [rstart, rend) share the row
-        unsigned long long m = __shfl_sync(0xffffffffu, mk, row);
-        const int piece = lane - rstart;
-        if (has && piece > 0) m &= ~0ull << nth_set_bit64(m, piece * c);  // this lane's piece starts at listed shell number piece * c
-        if (!has) m = 0ull;
-        const int rho = rho0 + row, mesh = rho / N, i = rho - mesh * N;
-        const double x0 = r_el[3 * i], y0 = r_el[3 * i + 1], z0 = r_el[3 * i + 2], am_ = S.amesh[mesh], a2 = am_ * am_;
-        double av[3][3];
-#pragma unroll
-        for (int k = 0; k < 3; ++k) { av[k][0] = am_ * U[k]; av[k][1] = am_ * U[3 + k]; av[k][2] = am_ * U[6 + k]; }
-        const double *bcr = bc + (size_t)i * A + S.lg_ao0[lg];
+        const int n = valid ? cnt[lg * N] : 0;
+        const int nmax = __reduce_max_sync(0xffffffffu, n);
+        const unsigned char *l = lrow + S.lg_off[lg];
+        const double *bcr = bci + S.lg_ao0[lg];
         const double4 *sh4 = reinterpret_cast<const double4 *>(shells) + S.lg_slot0[lg];
         const int type = S.lg_type[lg];
-        double acc[6];
-#pragma unroll
-        for (int d = 0; d < 6; ++d) acc[d] = 0.0;
         if (type == 0) {                                                  // Slater s: exp(-z r)
-            for (int k = 0; k < c; ++k) {
-                const bool valid = m != 0ull; const int q = valid ? __ffsll((long long)m) - 1 : 0; m &= m - 1ull;
-                const double b = valid ? bcr[q] : 0.0;
+            for (int k0 = 0; k0 < nmax; k0 += 4) {
+                const bool ok = k0 + t < n; const int q = ok ? l[k0 + t] : 0;
+                const double b = ok ? bcr[q] : 0.0;
                 const double4 s = sh4[q]; const double dx0 = x0 - s.x, dy0 = y0 - s.y, dz0 = z0 - s.z;
                 const double q0 = fma(dx0, dx0, fma(dy0, dy0, fma(dz0, dz0, a2)));
 #pragma unroll
@@ -134,18 +145,18 @@ __device__ __forceinline__ void ao_listed_warp(const DevSys &S, const double *__
                 }
             }
         } else if (type == 1) {                                           // s Gaussians
-            for (int k = 0; k < c; ++k) {
-                const bool valid = m != 0ull; const int q = valid ? __ffsll((long long)m) - 1 : 0; m &= m - 1ull;
-                const double b = valid ? bcr[q] : 0.0;
+            for (int k0 = 0; k0 < nmax; k0 += 4) {
+                const bool ok = k0 + t < n; const int q = ok ? l[k0 + t] : 0;
+                const double b = ok ? bcr[q] : 0.0;
                 const SixGeom G = six_gaussians(sh4[q], x0, y0, z0, av, a2, etab);
 #pragma unroll
                 for (int d = 0; d < 6; ++d) acc[d] = fma(G.e[d], b, acc[d]);
             }
         } else if (type == 2) {                                           // p Gaussians: e (bc . (d0 +- a e_k))
-            for (int k = 0; k < c; ++k) {
-                const bool valid = m != 0ull; const int q = valid ? __ffsll((long long)m) - 1 : 0; m &= m - 1ull;
+            for (int k0 = 0; k0 < nmax; k0 += 4) {
+                const bool ok = k0 + t < n; const int q = ok ? l[k0 + t] : 0;
                 const double *bp = bcr + 3 * q;
-                const double bx = valid ? bp[0] : 0.0, by = valid ? bp[1] : 0.0, bz = valid ? bp[2] : 0.0;
+                const double bx = ok ? bp[0] : 0.0, by = ok ? bp[1] : 0.0, bz = ok ? bp[2] : 0.0;
                 const SixGeom G = six_gaussians(sh4[q], x0, y0, z0, av, a2, etab);
                 const double l0 = fma(bx, G.dx0, fma(by, G.dy0, bz * G.dz0));
 #pragma unroll
@@ -156,12 +167,12 @@ __device__ __forceinline__ void ao_listed_warp(const DevSys &S, const double *__
                 }
             }
         } else {                                                          // d Gaussians: e Q(d), Q(d0 +- v) = Q(d0) +- v.grad Q(d0) + Q(v)
-            for (int k = 0; k < c; ++k) {
-                const bool valid = m != 0ull; const int q = valid ? __ffsll((long long)m) - 1 : 0; m &= m - 1ull;
+            for (int k0 = 0; k0 < nmax; k0 += 4) {
+                const bool ok = k0 + t < n; const int q = ok ? l[k0 + t] : 0;
                 const double *bp = bcr + 6 * q;
                 double b[6];
 #pragma unroll
-                for (int j = 0; j < 6; ++j) b[j] = valid ? bp[j] : 0.0;
+                for (int j = 0; j < 6; ++j) b[j] = ok ? bp[j] : 0.0;
                 const SixGeom G = six_gaussians(sh4[q], x0, y0, z0, av, a2, etab);
                 const double gx = fma(2.0 * b[0], G.dx0, fma(b[1], G.dy0, b[2] * G.dz0));
                 const double gy = fma(b[1], G.dx0, fma(2.0 * b[3], G.dy0, b[4] * G.dz0));
@@ -178,14 +189,5 @@ __device__ __forceinline__ void ao_listed_warp(const DevSys &S, const double *__
                 }
             }
         }
-        // the lanes of a row add up (suffix sums inside [rstart, rend)); the row's first lane adds the group's share to R
-        for (int o = 1; o < mmax; o <<= 1) {
-#pragma unroll
-            for (int d = 0; d < 6; ++d) { const double v = __shfl_down_sync(0xffffffffu, acc[d], o); if (lane + o < rend) acc[d] += v; }
-        }
-        if (has && piece == 0) { double *Ro = R + mesh * 6 * N + 6 * i;
-#pragma unroll
-            for (int d = 0; d < 6; ++d) Ro[d] += acc[d]; }
-        __syncwarp();
     }
 }

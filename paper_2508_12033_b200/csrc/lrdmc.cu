@@ -30,7 +30,8 @@ struct lrdmc_ctx {
     cudaEvent_t ev[4]; cudaStream_t last_stream;
     int launches;   // kernels launched so far (bench.py reports it)
     char msg[256];  // text of the last CUDA error of this context (lrdmc_last_error)
-    int opt_team, opt_global_tables;            // lrdmc_set_option
+    int opt_team, opt_global_tables, opt_listed; // lrdmc_set_option (opt_listed: -1 automatic, 0 dense, 1 listed)
+    int listed;                                 // the candidate pass of this system is the listed sweep (EXT = 4)
     size_t n_sh, n_nuc_d, bf_n, cf_n;           // table sizes in doubles (shared-memory plan)
     // team mode (team.cuh): chosen at lrdmc_bind_walkers from N_w and the footprint; team_tw == 1 -> warp-per-walker kernel
     TeamPlan team; int team_tw, team_smem, team_ctas_per_sm, team_grid_max, pair_base[5];
@@ -76,10 +77,13 @@ static int plan_smem(lrdmc_ctx *c)
     S.off_nuc = (int)o; o += align_up(c->n_nuc_d, 2);
     S.off_srad = (int)o; o += align_up((size_t)S.n_slots, 2);
     S.off_j3g = (int)o; o += (size_t)S.j3s * S.j3s;
+    // listed sweep (EXT = 4): lattice-only systems; automatic = the systems whose tables live in global memory (64 electrons, 600 AOs)
+    c->listed = !S.nl_K && !S.n_j3 && LRDMC_BC_STORE && (c->opt_listed < 0 ? !fits : c->opt_listed != 0);
     S.off_bf[0] = (int)o; if (S.bf_in_smem) o += bf_n;
     S.off_bf[1] = (int)o; if (S.bf_in_smem && !S.same_C) o += bf_n;
-    S.off_cf[0] = (int)o; if (S.bf_in_smem) o += cf_n;
-    S.off_cf[1] = (int)o; if (S.bf_in_smem && !S.same_C) o += cf_n;
+    S.cf_in_smem = S.bf_in_smem && !c->listed;
+    S.off_cf[0] = (int)o; if (S.bf_in_smem && !c->listed) o += cf_n;            // the pair table of ao_columns is not used by the listed sweep
+    S.off_cf[1] = (int)o; if (S.bf_in_smem && !S.same_C && !c->listed) o += cf_n;
     S.tables_doubles = (int)align_up(o, 2);
     size_t w = 0;
     S.o_r = (int)w; w += align_up(3 * (size_t)S.N, 2);
@@ -92,7 +96,7 @@ static int plan_smem(lrdmc_ctx *c)
     S.o_U = (int)w; w += 10;                    // the step's lattice frame (9 doubles)
     S.o_ob = (int)w; w += 8 * (size_t)S.N;      // one-body cache: J1, grad J1, lap J1, v_ei, v^a_ei per electron
     S.o_j3 = (int)w; if (S.n_j3) w += (size_t)S.N * 2 * S.j3s + S.j3s;   // three-body Jastrow: chi3, V3, S3
-    S.o_am = (int)w; if (!fits && !S.nl_K && !S.n_j3) w += (size_t)S.N * S.n_lg;       // listed-shell masks (listed sweep of the large systems)
+    S.o_am = (int)w; if (c->listed) w += ((size_t)S.N * (S.lt + S.n_lg) + 7) / 8;       // listed-shell lists (listed.cuh)
     S.per_warp_doubles = (int)w;
     const size_t per_sm = prop.sharedMemPerMultiprocessor, per_blk_max = prop.sharedMemPerBlockOptin, reserve = 1024;
     c->wpb = LRDMC_WPB;
@@ -108,7 +112,7 @@ static int plan_smem(lrdmc_ctx *c)
 #undef SET_ALL
 #undef SET_SMEM
     c->ts = S.bf_in_smem && S.moc_in_smem;
-    c->ext = (S.nl_K ? 1 : 0) | (S.n_j3 ? 2 : 0);     // which instantiation of the walker kernels this system runs (kernels.cu)
+    c->ext = c->listed ? 4 : (S.nl_K ? 1 : 0) | (S.n_j3 ? 2 : 0);     // which instantiation of the walker kernels this system runs (kernels.cu)
     LRDMC_K_CALL(c->ext, lrdmc_k_set_smem, c->smem_bytes);
     const int occ = LRDMC_K_CALL(c->ext, lrdmc_k_occupancy, c->NT, c->ts, c->wpb * 32, c->smem_bytes);
     CK(cudaGetLastError());
@@ -199,6 +203,7 @@ extern "C" int lrdmc_init(lrdmc_ctx **out, const lrdmc_system *sys, const lrdmc_
     } else if (n_ao != mo->n_ao) return LRDMC_EINVAL;
     lrdmc_ctx *c = (lrdmc_ctx *)calloc(1, sizeof(lrdmc_ctx));
     if (!c) return LRDMC_ENOMEM;
+    c->opt_listed = -1;
     DevSys &S = c->S;
     S.N = sys->n_up + sys->n_dn; S.n_up = sys->n_up; S.n_dn = sys->n_dn; S.n_nuc = sys->n_nuc;
     S.n_mesh = lat->a2 > 0.0 ? 2 : 1; S.P_lat = 6 * S.N * S.n_mesh; S.a = lat->a;
@@ -299,14 +304,14 @@ extern "C" int lrdmc_init(lrdmc_ctx **out, const lrdmc_system *sys, const lrdmc_
     }
     // ---- listed candidate sweep: list groups (one shell type, at most 64 slots each), slot-major coefficient rows, screening radii
     {
-        S.n_lg = 0; S.n_aop = 0;
+        S.n_lg = 0; S.n_aop = 0; S.lt = 0;
         int ao_run = 0;
         for (int g = 0; g < 4; ++g) {
             const int nsl = 4 * S.n_it[g];
             for (int s0 = 0; s0 < nsl; s0 += 64) {
                 if (S.n_lg == LRDMC_MAX_LG) { free(c); return LRDMC_ENOMEM; }
                 S.lg_type[S.n_lg] = g; S.lg_slot0[S.n_lg] = base[g] + s0; S.lg_n[S.n_lg] = nsl - s0 < 64 ? nsl - s0 : 64;
-                S.lg_ao0[S.n_lg] = ao_run + s0 * ncomp[g]; ++S.n_lg;
+                S.lg_ao0[S.n_lg] = ao_run + s0 * ncomp[g]; S.lg_off[S.n_lg] = S.lt; S.lt += S.lg_n[S.n_lg]; ++S.n_lg;
             }
             ao_run += nsl * ncomp[g];
         }
@@ -364,6 +369,9 @@ extern "C" int lrdmc_set_option(lrdmc_ctx *c, int option, int value)
         c->opt_team = value; return LRDMC_OK;
     case LRDMC_OPT_GLOBAL_TABLES:
         c->opt_global_tables = value != 0; return plan_smem(c);
+    case LRDMC_OPT_LISTED:
+        if (value < -1 || value > 1) return LRDMC_EINVAL;
+        c->opt_listed = value; return plan_smem(c);
     default: return LRDMC_EINVAL;
     }
 }
@@ -380,13 +388,18 @@ static size_t carve(const lrdmc_ctx *c, int n_w, char *base, DevWalk *W)
     TAKE(nmoves, long long, nw); TAKE(flags, int, nw * 3); TAKE(dead, int, nw);
     TAKE(wq, unsigned long long, nw); TAKE(prefix, unsigned long long, nw); TAKE(parents, int, nw);
     {   // parked Bc entries of the team kernel of the large systems (ao_columns BCS): [resident CTA][block of a mesh][k-step pair][lane][2]
-        const bool use = LRDMC_BC_STORE && !c->ts;
+        const bool use = LRDMC_BC_STORE && (!c->ts || c->listed);
         size_t stride = (size_t)((S.n_up + 7) / 8 + (S.n_dn + 7) / 8) * S.n_kpairs * 64;
-        if (c->ext == 0 && stride < (size_t)S.N * S.n_aop) stride = (size_t)S.N * S.n_aop;       // listed sweep: Bc [electron][n_aop]
+        if (c->listed) stride = (size_t)S.N * S.n_aop;       // listed sweep: Bc [electron][n_aop] per resident walker
         const size_t cta_bytes = ((size_t)S.tables_doubles + S.per_warp_doubles) * 8 + 1024;
         size_t per_sm = c->smem_per_sm / cta_bytes; if (per_sm > 32) per_sm = 32; if (per_sm < 1) per_sm = 1;   // resident team CTAs per SM, at most
-        if (W) { W->bcs_stride = use ? stride : 0; W->bcs_ctas = use ? (int)(per_sm * c->sm_count) : 0; }     // plan_team clamps the grid to this
-        TAKE(bcs, double, use ? stride * per_sm * c->sm_count : 0);
+        size_t n_res = per_sm * c->sm_count;                  // team CTAs (plan_team clamps the grid to this) ...
+        if (c->listed) {                                      // ... or the resident warps of the warp-per-walker kernel; never more than the walkers
+            if ((size_t)c->grid_max * c->wpb > n_res) n_res = (size_t)c->grid_max * c->wpb;
+            if (n_res > nw + LRDMC_WPB) n_res = nw + LRDMC_WPB;
+        }
+        if (W) { W->bcs_stride = use ? stride : 0; W->bcs_ctas = use ? (int)n_res : 0; }
+        TAKE(bcs, double, use ? stride * n_res : 0);
         if (W && !use) W->bcs = NULL;
     }
     TAKE(timing, unsigned long long, 2 * (size_t)(c->grid_max * c->wpb > c->sm_count * 32 ? c->grid_max * c->wpb : c->sm_count * 32)); TAKE(counter, int, 64);
@@ -433,7 +446,7 @@ static void plan_team(lrdmc_ctx *c, int n_w)
     c->team_tw = 1;
     int tw = 1;
     const long slots = (long)c->grid_max * c->wpb;
-    if (!c->ts) tw = (c->ext == 0 && LRDMC_BC_STORE) ? 8 : 4;   // listed sweep (listed.cuh): measured at C5 N_w = 4096, TW = 4 / 8 / 16: 2.27 / 2.82 / 2.64 M walker-moves/s
+    if (!c->ts) tw = c->listed ? 8 : 4;   // listed sweep (listed.cuh): measured at C5 N_w = 4096, TW = 4 / 8 / 16: 2.27 / 2.82 / 2.64 M walker-moves/s
     else if ((long)n_w * 8 <= 3 * slots) tw = 4;   // measured on C3/C4 (profiles/r1_team_kernel.md): 4 warps per walker beat 2, 8 and 16 at every N_w,
                                                    // and beat warp-per-walker up to N_w of about 3/8 of the resident warp slots
     if (c->opt_team > 0) tw = c->opt_team;        // LRDMC_OPT_TEAM_WARPS (tests force 1, 2, 4, 8, 16)
@@ -467,8 +480,7 @@ static void plan_team(lrdmc_ctx *c, int n_w)
     const int smem = (int)(((size_t)S.tables_doubles + S.per_warp_doubles + P.scr_doubles) * 8);
     const int occ = LRDMC_K_CALL(c->ext, lrdmc_k_team_occupancy, c->NT, c->ts, tw * 32, smem);
     if (cudaGetLastError() != cudaSuccess || occ < 1) return;             // does not fit: stay with warp-per-walker
-    P.listed = !c->ts && c->ext == 0 && LRDMC_BC_STORE;
-    { const int rows = S.n_mesh * S.N; int rb = (rows + tw - 1) / tw; P.RB = rb > 16 ? 16 : (rb < 1 ? 1 : rb); }
+    P.listed = c->listed;
     c->team_tw = tw; c->team_smem = smem; c->team_ctas_per_sm = occ; c->team_grid_max = c->sm_count * occ;
     if (c->W.bcs && c->team_grid_max > c->W.bcs_ctas) c->team_grid_max = c->W.bcs_ctas;   // the parked-entry scratch is indexed by blockIdx.x
 }

@@ -15,7 +15,7 @@ __device__ __forceinline__ void stage_tables(const DevSys &S, double *smem)
         const int nb = S.n_ksteps * S.NT[0] * 32;
         for (int i = threadIdx.x; i < nb; i += blockDim.x) smem[S.off_bf[0] + i] = S.bfrag[0][i];
         if (!S.same_C && S.n_dn > 0) for (int i = threadIdx.x; i < nb; i += blockDim.x) smem[S.off_bf[1] + i] = S.bfrag[1][i];
-        const int nc = S.n_kpairs * 2 * S.NT[0] * 32;
+        const int nc = S.cf_in_smem ? S.n_kpairs * 2 * S.NT[0] * 32 : 0;
         for (int i = threadIdx.x; i < nc; i += blockDim.x) smem[S.off_cf[0] + i] = S.cfrag[0][i];
         if (!S.same_C && S.n_dn > 0) for (int i = threadIdx.x; i < nc; i += blockDim.x) smem[S.off_cf[1] + i] = S.cfrag[1][i];
     }
@@ -46,7 +46,7 @@ __device__ __forceinline__ WarpState warp_views(const DevSys &S, double *smem, i
     WarpState ws;
     ws.r = base + S.o_r; ws.dinv[0] = base + S.o_dinv[0]; ws.dinv[1] = base + S.o_dinv[1];
     ws.moc = base + S.o_moc; ws.R = base + S.o_R; ws.cum = base + S.o_cum; ws.el = base + S.o_el; ws.ob = base + S.o_ob; ws.U = base + S.o_U; ws.j3 = base + S.o_j3;
-    ws.am = reinterpret_cast<unsigned long long *>(base + S.o_am);
+    ws.lw = reinterpret_cast<unsigned char *>(base + S.o_am); ws.bc = nullptr;
     return ws;
 }
 
@@ -60,8 +60,9 @@ __device__ __forceinline__ void publish_frame(const WarpState &ws, const StepDra
     __syncwarp();
 }
 
-template <bool TS>
-__device__ __forceinline__ void load_walker(const DevSys &S, const DevWalk &W, WarpState &ws, const double *nuc, int k, int lane, bool with_dinv, bool with_onebody = true)
+// LISTED (EXT bit 2): also the listed-shell masks of every electron and Bc = C Dinv of this walker in the warp's global scratch ws.bc.
+template <bool TS, bool LISTED = false>
+__device__ __forceinline__ void load_walker(const DevSys &S, const DevWalk &W, WarpState &ws, const Tables &T, int k, int lane, bool with_dinv, bool with_onebody = true)
 {
     const int N = S.N;
     for (int i = lane; i < 3 * N; i += 32) ws.r[i] = W.r[(size_t)k * 3 * N + i];
@@ -74,8 +75,13 @@ __device__ __forceinline__ void load_walker(const DevSys &S, const DevWalk &W, W
     if (TS) { for (int i = lane; i < (int)mocn; i += 32) ws.moc[i] = W.moc[(size_t)k * mocn + i]; }
     else ws.moc = W.moc + (size_t)k * mocn;
     __syncwarp();
+    const double *nuc = T.nuc;
     if (with_onebody && S.n_j3) for (int i = 0; i < N; ++i) refresh_j3_row(S, nuc, ws.j3 + i * S.j3s, ws.r[3 * i], ws.r[3 * i + 1], ws.r[3 * i + 2], lane);
     if (with_onebody) for (int i = 0; i < N; ++i) refresh_onebody(S.n_nuc, S.has_j1, S.a, nuc, ws.ob + 8 * i, ws.r[3 * i], ws.r[3 * i + 1], ws.r[3 * i + 2], lane);
+    if (LISTED) {
+        for (int i = 0; i < N; ++i) list_build(S, T.shells, T.srad, ws.lw, i, ws.r[3 * i], ws.r[3 * i + 1], ws.r[3 * i + 2], fmax(S.amesh[0], S.amesh[1]), lane);
+        build_bc(S, ws.dinv[0], ws.dinv[1], ws.bc, lane, 32);
+    }
     __syncwarp();
 }
 
@@ -103,6 +109,7 @@ __global__ void __launch_bounds__(LRDMC_WPB * 32, LRDMC_MINB) k_propagate(DevSys
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, gwarp = blockIdx.x * (blockDim.x >> 5) + warp;
     const Tables T = table_pointers<TS>(S, smem);
     WarpState ws = warp_views(S, smem, warp);
+    if (EXT & 4) ws.bc = W.bcs + (size_t)gwarp * W.bcs_stride;
     const unsigned long long t_start = globaltimer_ns();
     // The warps of a CTA meet at a barrier once per step, whatever walker and step index each of them is at: they then run
     // the same code region at the same time and share the small instruction caches (L0 6 KB, L1.5 32 KB against 140 KB of
@@ -122,7 +129,7 @@ __global__ void __launch_bounds__(LRDMC_WPB * 32, LRDMC_MINB) k_propagate(DevSys
                 }
                 continue;
             }
-            load_walker<TS>(S, W, ws, T.nuc, k, lane, true);
+            load_walker<TS, (EXT & 4) != 0>(S, W, ws, T, k, lane, true);
             have = true; s = 0; w = 1.0; tau_left = tau; moves = 0; n_node = 0; n_nonpos = 0;
         }
         if (LRDMC_LOCKSTEP) { if (!__syncthreads_or(have)) break; if (!have) continue; }
@@ -159,7 +166,7 @@ __global__ void __launch_bounds__(LRDMC_WPB * 32, LRDMC_MINB) k_propagate(DevSys
             W.w[k] = w; W.eL[k] = e.eL; W.W[k] = e.W; W.omega[k] = omega; W.nmoves[k] = moves;
             W.flags[3 * k] = n_node; W.flags[3 * k + 1] = n_nonpos; W.flags[3 * k + 2] = nonfinite;
         }
-        if (!TS) ws = warp_views(S, smem, warp);               // load_walker pointed ws.moc at the walker's global rows
+        if (!TS) { ws = warp_views(S, smem, warp); if (EXT & 4) ws.bc = W.bcs + (size_t)gwarp * W.bcs_stride; }   // load_walker pointed ws.moc at the walker's global rows
         have = false;
     }
     if (lane == 0) { W.timing[2 * gwarp] = t_start; W.timing[2 * gwarp + 1] = globaltimer_ns(); }
@@ -176,7 +183,8 @@ __global__ void __launch_bounds__(LRDMC_WPB * 32, LRDMC_MINB) k_step_debug(DevSy
     const Tables T = table_pointers<TS>(S, smem);
     WarpState ws = warp_views(S, smem, warp);
     for (int k = blockIdx.x * wpb + warp; k < W.n_w; k += gridDim.x * wpb) {
-        load_walker<TS>(S, W, ws, T.nuc, k, lane, true);
+        if (EXT & 4) ws.bc = W.bcs + (size_t)(blockIdx.x * wpb + warp) * W.bcs_stride;
+        load_walker<TS, (EXT & 4) != 0>(S, W, ws, T, k, lane, true);
         const StepDraws d = step_draws(S, (uint32_t)k, cycle, step, true);
         publish_frame(ws, d, lane);
         const EvalOut e = evaluate_walker<NT, TS, EXT>(S, ws, T, lane);
@@ -204,7 +212,7 @@ __global__ void __launch_bounds__(LRDMC_WPB * 32) k_rebuild(DevSys S, DevWalk W,
     WarpState ws = warp_views(S, smem, warp);
     const int N = S.N;
     for (int k = blockIdx.x * wpb + warp; k < W.n_w; k += gridDim.x * wpb) {
-        load_walker<TS>(S, W, ws, T.nuc, k, lane, !(do_invert & 1), false);
+        load_walker<TS>(S, W, ws, T, k, lane, !(do_invert & 1), false);
         if (!(do_invert & 2)) for (int i = 0; i < N; ++i) {
             const int sp = spin_of(S, i);
             refresh_mo_cache<NT, TS>(S, T.shells, T.bf[sp], T.etab, ws.moc + (size_t)i * 5 * S.OS, ws.r[3 * i], ws.r[3 * i + 1], ws.r[3 * i + 2], lane);

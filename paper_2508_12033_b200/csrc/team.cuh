@@ -11,33 +11,6 @@
 #include "propagate.cuh"
 #include "listed.cuh"
 
-// ---- listed sweep of the large systems (listed.cuh): the CTA's Bc = C Dinv of its walker, [electron][n_aop] in global scratch ----
-// Built when the walker is loaded: thread = one AO row of C (slot-major, norms folded in), eight inverse columns at a time.
-__device__ __forceinline__ void team_build_bc(const DevSys &S, const WarpState &ws, double *__restrict__ bc)
-{
-    const int tid = threadIdx.x, nthr = blockDim.x, A = S.n_aop, OS = S.OS;
-    for (int sp = 0; sp < 2; ++sp) {
-        const int ns = sp ? S.n_dn : S.n_up, off = sp ? S.n_up : 0;
-        if (!ns) continue;
-        const double *__restrict__ cn = S.cn[sp], *dinv = ws.dinv[sp];
-        for (int ao = tid; ao < A; ao += nthr) {
-            const double *crow = cn + (size_t)ao * OS;
-            for (int il0 = 0; il0 < ns; il0 += 8) {
-                double acc[8];
-#pragma unroll
-                for (int j = 0; j < 8; ++j) acc[j] = 0.0;
-                for (int m = 0; m < ns; ++m) {
-                    const double cv = __ldg(crow + m); const double *dr = dinv + m * ns + il0;   // columns beyond n_s read padding, never stored
-#pragma unroll
-                    for (int j = 0; j < 8; ++j) acc[j] = fma(cv, dr[j], acc[j]);
-                }
-#pragma unroll
-                for (int j = 0; j < 8; ++j) if (il0 + j < ns) bc[(size_t)(off + il0 + j) * A + ao] = acc[j];
-            }
-        }
-    }
-}
-
 __device__ __forceinline__ void load_walker_team(const DevSys &S, const DevWalk &W, WarpState &ws, const double *nuc, int k, int TW)
 {
     const int N = S.N, tid = threadIdx.x, nthr = blockDim.x, lane = tid & 31, wt = tid >> 5;
@@ -92,7 +65,7 @@ template <int NT, bool TS, int EXT, bool BCS>
 __device__ __forceinline__ EvalOut evaluate_team(const DevSys &S, const TeamPlan &P, const WarpState &ws, const Tables &T, double *scr, double *s_vee, int *s_node,
                                                  double2 *bcs_cta, int reuse_spin)
 {
-    constexpr bool LISTED = BCS && EXT == 0;       // large systems without slots / J3: listed sweep on the CTA's rank-1-updated Bc (listed.cuh)
+    constexpr bool LISTED = (EXT & 4) != 0;        // listed sweep on the CTA's rank-1-updated Bc (listed.cuh); BCS: parked Bc entries of the dense sweep
     const int N = S.N, n_nuc = S.n_nuc, TW = P.TW, NP = P.NP, tid = threadIdx.x, nthr = blockDim.x, lane = tid & 31, wt = tid >> 5;
     const int t = lane & 3, g = lane >> 2;
     constexpr bool NL = (EXT & 1) != 0, J3 = (EXT & 2) != 0;      // non-local slots / three-body Jastrow (separate instantiations)
@@ -164,43 +137,9 @@ __device__ __forceinline__ EvalOut evaluate_team(const DevSys &S, const TeamPlan
     __syncthreads();
 
     if (LISTED) {
-        // ---- phase B of the large systems (rows a1-a5): batches of RB rows (mesh, electron) per warp; the listed sweep leaves the
+        // ---- phase B as a listed sweep (rows a1-a5): 8-row batches (mesh, electron) per warp; the listed sweep leaves the
         //      determinant ratios in R, the Jastrow ratios of the same rows follow in the same warp (quad per row)
-        const int n_rows = S.n_mesh * N, RB = P.RB;
-        const double *bc = reinterpret_cast<const double *>(bcs_cta);
-        for (int b0 = wt * RB; b0 < n_rows; b0 += TW * RB) {
-            const int nr = min(RB, n_rows - b0);
-            ao_listed_warp(S, T.shells, T.etab, ws.r, ws.U, ws.am, bc, b0, nr, ws.R, lane);
-            for (int r0 = 0; r0 < nr; r0 += 8) {
-                const bool valid = r0 + g < nr;
-                const int rho = b0 + (valid ? r0 + g : 0), mesh = rho / N, i = rho - mesh * N, sp = spin_of(S, i);
-                const double x0 = ws.r[3 * i], y0 = ws.r[3 * i + 1], z0 = ws.r[3 * i + 2], am_ = S.amesh[mesh], a2 = am_ * am_;
-                double av[3][3], Jn[6];
-#pragma unroll
-                for (int k = 0; k < 3; ++k) { av[k][0] = am_ * ws.U[k]; av[k][1] = am_ * ws.U[3 + k]; av[k][2] = am_ * ws.U[6 + k]; }
-#pragma unroll
-                for (int d = 0; d < 6; ++d) Jn[d] = 0.0;
-                if (S.has_j1) for (int I = t; I < n_nuc; I += 4) {
-                    const double *np_ = T.nuc + I * LRDMC_NUC_STRIDE;
-                    pade_six(x0 - np_[0], y0 - np_[1], z0 - np_[2], av, a2, -np_[4], np_[5], Jn);
-                }
-                for (int j = t; j < N; j += 4) {
-                    const double c = (j == i) ? 0.0 : ((spin_of(S, j) == sp) ? S.a_par : S.a_anti);
-                    pade_six(x0 - ws.r[3 * j], y0 - ws.r[3 * j + 1], z0 - ws.r[3 * j + 2], av, a2, c, S.b2, Jn);
-                }
-                const double Jo = Jold[i];
-                double *Ro = ws.R + mesh * 6 * N + 6 * i;
-                double Rv[6];
-#pragma unroll
-                for (int d = 0; d < 6; ++d) Rv[d] = Ro[d] * exp_tab(quad_sum(Jn[d]) - Jo, T.etab);
-                __syncwarp();
-                if (valid && t == 0) {
-#pragma unroll
-                    for (int d = 0; d < 6; ++d) Ro[d] = Rv[d];
-                }
-            }
-            __syncwarp();
-        }
+        listed_phase_b(S, ws, T, Jold, wt, TW, lane);        // 8-row batches wt, wt + TW, ...; ws.bc = this CTA's Bc (set by the kernel)
         __syncthreads();
         EvalOut o; o.bbar = 0.0; o.Vsf = 0.0; o.W = 0.0; o.eL = 0.0; o.node = 0;
         if (wt == 0) {
@@ -243,7 +182,7 @@ __device__ __forceinline__ EvalOut evaluate_team(const DevSys &S, const TeamPlan
 #pragma unroll
         for (int k = 0; k < 3; ++k) { av[k][0] = step * ws.U[k]; av[k][1] = step * ws.U[3 + k]; av[k][2] = step * ws.U[6 + k]; }
         double acc[6], Jn[6];
-        if (BCS && !LISTED && !is_nl) {
+        if (BCS && !is_nl) {
             double2 *bq = bcs_cta + (size_t)rem * S.n_kpairs * 32 + lane;
             if ((mesh > 0 && P.mesh_share) || sp == reuse_spin)
                 ao_columns<NT, TS, true, 2>(S, T.shells, sp ? T.cf[1] : T.cf[0], T.etab, sp ? ws.dinv[1] : ws.dinv[0], ns, il, x0, y0, z0, av, a2, lane, acc, &P, &P.col[part], bq);
@@ -338,7 +277,7 @@ __device__ __forceinline__ EvalOut evaluate_team(const DevSys &S, const TeamPlan
 template <int NT, bool TS, int EXT>
 __device__ __forceinline__ void apply_move_team(const DevSys &S, const TeamPlan &P, const WarpState &ws, const Tables &T, double *scr, int j, double *bc = nullptr)
 {
-    constexpr bool LISTED = !TS && LRDMC_BC_STORE && EXT == 0;
+    constexpr bool LISTED = (EXT & 4) != 0;
     const int N = S.N, TW = P.TW, tid = threadIdx.x, nthr = blockDim.x, lane = tid & 31, wt = tid >> 5;   // warp 0 holds the lightest shell part (s shells): it also refreshes the one-body cache
     int i; double px, py, pz;
     move_target<(EXT & 1) != 0>(S, ws, T.nuc, j, i, px, py, pz);
@@ -357,7 +296,7 @@ __device__ __forceinline__ void apply_move_team(const DevSys &S, const TeamPlan 
     }
     if (wt == 0) { refresh_onebody(S.n_nuc, S.has_j1, S.a, T.nuc, ws.ob + 8 * i, px, py, pz, lane); if (EXT & 2) refresh_j3_row(S, T.nuc, ws.j3 + i * S.j3s, px, py, pz, lane); }
     if (LISTED && wt == TW - 1)            // the mover's listed-shell masks at its new position
-        list_masks(S, T.shells, T.srad, ws.am + i * S.n_lg, px, py, pz, fmax(S.amesh[0], S.amesh[1]), lane, 0, 1);
+        list_build(S, T.shells, T.srad, ws.lw, i, px, py, pz, fmax(S.amesh[0], S.amesh[1]), lane);
     __syncthreads();                                   // every thread has read the old position
     for (int idx = tid; idx < rows; idx += nthr) {
         double s = 0.0;
@@ -380,23 +319,7 @@ __device__ __forceinline__ void apply_move_team(const DevSys &S, const TeamPlan 
         const double ci = col[m] * irho;
         dinv[idx] = (kk == il) ? ci : dinv[idx] - ci * sk[kk];
     }
-    if (LISTED) {      // Bc = C Dinv follows the inverse by the same rank-1 formula: Bc'[:,k] = Bc[:,k] - Bc[:,il] s_k / rho, Bc'[:,il] = Bc[:,il] / rho
-        // item = (AO, chunk of 8 columns): eight independent loads in flight per thread, consecutive threads on consecutive AOs (coalesced);
-        // column il itself is rescaled in a second sweep (every item of the first reads its OLD entries)
-        const int A = S.n_aop, off = sp ? S.n_up : 0, nch = (ns + 7) >> 3;
-        const double *bi = bc + (size_t)i * A;
-        for (int it = tid; it < A * nch; it += nthr) {
-            const int ch = it / A, ao = it - ch * A, k0 = 8 * ch;
-            const double f = bi[ao] * irho;
-            double v[8];
-#pragma unroll
-            for (int q = 0; q < 8; ++q) v[q] = (k0 + q < ns) ? __ldcg(bc + (size_t)(off + k0 + q) * A + ao) : 0.0;
-#pragma unroll
-            for (int q = 0; q < 8; ++q) if (k0 + q < ns && k0 + q != il) __stcg(bc + (size_t)(off + k0 + q) * A + ao, fma(-f, sk[k0 + q], v[q]));
-        }
-        __syncthreads();
-        for (int ao = tid; ao < A; ao += nthr) bc[(size_t)i * A + ao] = bi[ao] * irho;
-    }
+    if (LISTED) bc_rank1_update(S, bc, sp, il, ns, sk, irho, tid, nthr);   // Bc = C Dinv follows the inverse (listed.cuh)
     __syncthreads();
 }
 
@@ -412,8 +335,10 @@ __global__ void __launch_bounds__(LRDMC_TEAM_MAX_WARPS * 32, 1) k_propagate_team
     const Tables T = table_pointers<TS>(S, smem);
     WarpState ws = warp_views(S, smem, 0);
     double *scr = smem + S.tables_doubles + P.o_scr;
-    constexpr bool BCS = !TS && LRDMC_BC_STORE;                 // large systems: C Dinv is the largest share of the evaluation
-    double2 *bcs_cta = BCS ? reinterpret_cast<double2 *>(W.bcs + (size_t)blockIdx.x * W.bcs_stride) : nullptr;
+    constexpr bool LISTED = (EXT & 4) != 0;                     // listed sweep on stored, rank-1-updated Bc
+    constexpr bool BCS = !TS && LRDMC_BC_STORE && !LISTED;      // large systems, dense sweep: parked Bc entries
+    double2 *bcs_cta = (BCS || LISTED) ? reinterpret_cast<double2 *>(W.bcs + (size_t)blockIdx.x * W.bcs_stride) : nullptr;
+    if (LISTED) ws.bc = W.bcs + (size_t)blockIdx.x * W.bcs_stride;
     const unsigned long long t_start = globaltimer_ns();
     for (;;) {
         if (tid == 0) s_ctrl[0] = atomicAdd(W.counter, 1);
@@ -429,10 +354,10 @@ __global__ void __launch_bounds__(LRDMC_TEAM_MAX_WARPS * 32, 1) k_propagate_team
             continue;
         }
         load_walker_team(S, W, ws, T.nuc, k, P.TW);
-        if (BCS && EXT == 0) {                                  // listed sweep: masks of every electron, Bc of this walker
+        if (LISTED) {                                           // listed sweep: masks of every electron, Bc of this walker
             for (int i = wt; i < S.N; i += P.TW)
-                list_masks(S, T.shells, T.srad, ws.am + i * S.n_lg, ws.r[3 * i], ws.r[3 * i + 1], ws.r[3 * i + 2], fmax(S.amesh[0], S.amesh[1]), lane, 0, 1);
-            team_build_bc(S, ws, reinterpret_cast<double *>(bcs_cta));
+                list_build(S, T.shells, T.srad, ws.lw, i, ws.r[3 * i], ws.r[3 * i + 1], ws.r[3 * i + 2], fmax(S.amesh[0], S.amesh[1]), lane);
+            build_bc(S, ws.dinv[0], ws.dinv[1], reinterpret_cast<double *>(bcs_cta), tid, blockDim.x);
             __syncthreads();
         }
         uint32_t s = 0; int reuse_spin = -1;
@@ -488,7 +413,7 @@ __global__ void __launch_bounds__(LRDMC_TEAM_MAX_WARPS * 32, 1) k_propagate_team
             W.w[k] = w; W.eL[k] = eL_last; W.W[k] = W_last; W.omega[k] = omega; W.nmoves[k] = moves;
             W.flags[3 * k] = n_node; W.flags[3 * k + 1] = n_nonpos; W.flags[3 * k + 2] = nonfinite;
         }
-        if (!S.moc_in_smem) ws = warp_views(S, smem, 0);
+        if (!S.moc_in_smem) { ws = warp_views(S, smem, 0); if (LISTED) ws.bc = W.bcs + (size_t)blockIdx.x * W.bcs_stride; }
         __syncthreads();                                        // the state and s_ctrl are free for the next walker
     }
     if (tid == 0) { W.timing[2 * blockIdx.x] = t_start; W.timing[2 * blockIdx.x + 1] = globaltimer_ns(); }

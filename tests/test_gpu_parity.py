@@ -226,6 +226,30 @@ def _whole_cycles(B, name, mode, n_cycles=2, keep=False, options=None):
     g.close()
 
 
+LATTICE_ONLY = ["C1-hydrogen", "tiny-2u1d", "tiny-3u3d-pp", "tiny-2u2d-doublemesh", "ragged-5u2d", "ragged-9u4d-NT2", "ragged-17u3d-NT4", "he-triplet-slater",
+                "C2-synthetic10", "C3-water-methane-shaped", "contracted-3u2d-sph-pp", "contracted-9u7d-cart", "contracted-slater-spd"]
+
+
+@pytest.mark.parametrize("name", LATTICE_ONLY)
+@pytest.mark.parametrize("mode", ["balanced", "conventional"])
+@pytest.mark.parametrize("tw", [1, 4])
+def test_listed_sweep_forced_on_small_systems(B, name, mode, tw):
+    """lrdmc_set_option(LRDMC_OPT_LISTED, 1): per-electron shell lists + Bc = C Dinv as rank-1-updated state (the candidate pass of the 64-electron
+    configuration) forced on every lattice-only system, with tables in shared memory, in the warp-per-walker and the team kernel: one evaluation and
+    whole cycles against the oracle (which never screens)."""
+    s, x0, o, g = _pair(B, name, {B.OPT_LISTED: 1, B.OPT_TEAM_WARPS: tw})
+    N = s["n_up"] + s["n_dn"]; Kd = 3 * N / s["a"]**2
+    r, du, dd, w = o.get_state(); g.lrdmc_set_state(r, du, dd, w)
+    R, scal, js = o.step_debug(-3.0, 2, 1)
+    gR, gscal, gjs = [np_(t) for t in g.lrdmc_step_debug(-3.0, 2, 1)]
+    assert relerr(gR, R, 1.0) < TOL and np.array_equal(gjs, js)
+    assert np.max(np.abs(gscal[:, :4] - scal[:, :4]) / np.maximum(np.abs(scal[:, :4]), Kd)) < TOL
+    g.close()
+    g = _whole_cycles(B, name, mode, keep=True, options={B.OPT_LISTED: 1, B.OPT_TEAM_WARPS: tw})
+    assert g.launch_config()["kernel"] == ("k_propagate" if tw == 1 else "k_propagate_team")
+    g.close()
+
+
 @pytest.mark.parametrize("name", ["C1-hydrogen", "tiny-3u3d-pp", "C3-water-methane-shaped"])
 def test_large_system_path_tables_in_global_memory(B, name):
     """The kernels of systems whose tables do not fit shared memory (C5) read fragments and MO cache from global memory;
