@@ -632,7 +632,7 @@ extern "C" int lrdmc_reconfigure(lrdmc_ctx *c, uint64_t cycle, int32_t *parents_
     k_comb<<<1, COMB_THREADS, 0, st>>>(c->W, ctr[0], c->d_stats, parents_dev); ++c->launches;
     CK(cudaGetLastError());
     const int rec = 3 * c->S.N;
-    size_t total = (size_t)c->W.n_w * (rec + c->S.N * 5 * c->S.OS / 2); int gb = (int)((total + 255) / 256); if (gb > 148 * 16) gb = 148 * 16;
+    size_t total = (size_t)c->W.n_w * (rec + c->S.N * 5 * c->S.OS / 2); int gb = (int)((total + 255) / 256); if (gb > c->sm_count * 16) gb = c->sm_count * 16;
     k_gather<<<gb, 256, 0, st>>>(c->W, rec, c->S.N * 5 * c->S.OS); ++c->launches;
     CK(cudaGetLastError());
     double *tmp = c->W.r; c->W.r = c->W.r_alt; c->W.r_alt = tmp;
