@@ -129,6 +129,20 @@ __device__ __forceinline__ void pade_six(double dx, double dy, double dz, const 
     }
 }
 
+// R_j = (determinant ratio) * exp(J' - J) of the six candidates of a quad's row, from the lanes' shares: after the quad sums every lane holds the six
+// sums; lane t finishes candidates d = t and (t < 2) d = 4 + t and stores them itself -- two exponentials per lane instead of six inlined copies
+// (the extended kernels' hot loop has to fit the instruction cache), same arithmetic per candidate.
+__device__ __forceinline__ void finish_ratios(const double (&acc)[6], const double (&Jn)[6], double Jo, const double *etab, int t, bool valid, double *Ro)
+{
+    double A[6], J[6];
+#pragma unroll
+    for (int d = 0; d < 6; ++d) { A[d] = quad_sum(acc[d]); J[d] = quad_sum(Jn[d]); }
+    const double a0 = t == 0 ? A[0] : (t == 1 ? A[1] : (t == 2 ? A[2] : A[3])), j0 = t == 0 ? J[0] : (t == 1 ? J[1] : (t == 2 ? J[2] : J[3]));
+    const double a1 = t == 0 ? A[4] : A[5], j1 = t == 0 ? J[4] : J[5];
+    const double r0 = a0 * exp_tab(j0 - Jo, etab), r1 = a1 * exp_tab(j1 - Jo, etab);
+    if (valid) { Ro[t] = r0; if (t < 2) Ro[4 + t] = r1; }
+}
+
 // Three-body Jastrow at the six displaced points x0 +- av[k] of one electron (reading Q23): Jn[d] += sum_a chi_a(point d) V_a,
 // the functions dealt over the `stride` lanes that share the electron (t = this lane's index among them, a = a0 + t): six table
 // exponentials per function in the same +- form as the AOs.  The trip count is uniform in the warp (exp_tab_n synchronises it).
@@ -260,12 +274,7 @@ __device__ __forceinline__ int phase_b_with_nonlocal(const DevSys &S, const Warp
         if (J3 && (!is_nl || !S.nl_dla)) j3_six(S, T, ws.j3 + (N + i) * S.j3s, x0, y0, z0, av, a2, t, Jn);
         const double Jo = Jold[i];
         if (!is_nl) {
-            double Rv[6];
-#pragma unroll
-            for (int d = 0; d < 6; ++d) Rv[d] = quad_sum(acc[d]) * exp_tab(quad_sum(Jn[d]) - Jo, T.etab);
-            if (valid && t == 0) { double *Ro = ws.R + mesh * 6 * N + 6 * i;
-#pragma unroll
-                for (int d = 0; d < 6; ++d) Ro[d] = Rv[d]; }
+            finish_ratios(acc, Jn, Jo, T.etab, t, valid, ws.R + mesh * 6 * N + 6 * i);
         } else {
             double nuq[6];
             {
@@ -386,14 +395,7 @@ __device__ __forceinline__ void listed_phase_b(const DevSys &S, const WarpState 
             pade_six(x0 - ws.r[3 * j], y0 - ws.r[3 * j + 1], z0 - ws.r[3 * j + 2], av, a2, c, S.b2, Jn);
         }
         const double Jo = Jold[i];
-        double Rv[6];
-#pragma unroll
-        for (int d = 0; d < 6; ++d) Rv[d] = quad_sum(acc[d]) * exp_tab(quad_sum(Jn[d]) - Jo, T.etab);
-        if (valid && t == 0) {
-            double *Ro = ws.R + mesh * 6 * N + 6 * i;
-#pragma unroll
-            for (int d = 0; d < 6; ++d) Ro[d] = Rv[d];
-        }
+        finish_ratios(acc, Jn, Jo, T.etab, t, valid, ws.R + mesh * 6 * N + 6 * i);
     }
 }
 
@@ -475,14 +477,7 @@ __device__ __forceinline__ EvalOut evaluate_walker(const DevSys &S, const WarpSt
                 }
                 if (J3) j3_six(S, T, ws.j3 + (N + i) * S.j3s, x0, y0, z0, av, a2, t, Jn);
                 const double Jo = Jold[i];
-                double Rv[6];
-#pragma unroll
-                for (int d = 0; d < 6; ++d) Rv[d] = quad_sum(acc[d]) * exp_tab(quad_sum(Jn[d]) - Jo, T.etab);
-                if (valid && t == 0) {
-                    double *Ro = ws.R + mesh * 6 * N + 6 * i;
-#pragma unroll
-                    for (int d = 0; d < 6; ++d) Ro[d] = Rv[d];
-                }
+                finish_ratios(acc, Jn, Jo, T.etab, t, valid, ws.R + mesh * 6 * N + 6 * i);
             }
         }
     }

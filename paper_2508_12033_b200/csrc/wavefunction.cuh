@@ -10,6 +10,13 @@
 #pragma once
 #include "common.cuh"
 #include "fastmath.cuh"
+#ifndef LRDMC_COMPACT_COLUMNS
+#if defined(LRDMC_EXT) && (LRDMC_EXT == 1 || LRDMC_EXT == 2 || LRDMC_EXT == 3)
+#define LRDMC_COMPACT_COLUMNS 1
+#else
+#define LRDMC_COMPACT_COLUMNS 0
+#endif
+#endif
 
 // Table element load with an explicit address space.  TS: the tables sit in shared memory (plain load, inferred LDS).
 // !TS: global memory -- spelled as ld.global.nc, because nvcc 12.9 otherwise infers "shared" for the fragment pointer of the
@@ -207,6 +214,26 @@ __device__ __forceinline__ void ao_columns(const DevSys &S, const double *__rest
         }
         sh4 += 4;
     };
+    // LRDMC_COMPACT_COLUMNS (extended kernels): ONE copy of each shell body (the second iteration of a k-step pair goes round a two-trip loop) instead of
+    // three (pair loop + tail): the extended kernels' hot loop did not fit the instruction cache (ncu: `no_instruction` 0.9 - 1.2 stall cycles per issue
+    // at 11.4 k - 11.8 k SASS instructions against 0.06 for the lattice-only kernel's 10.0 k).
+#if LRDMC_COMPACT_COLUMNS
+    {
+        LRDMC_COL_RANGE(0, it / 2) double b0, sv = 0.0;
+        for (const int i0 = it; it < n; ++it) { if (!((it - i0) & 1)) { LRDMC_BPAIR(b0, sv) } else b0 = sv; slater_body(b0); }
+    }
+    {
+        LRDMC_COL_RANGE(1, it / 2) double b0, sv = 0.0;
+        for (const int i0 = it; it < n; ++it) { if (!((it - i0) & 1)) { LRDMC_BPAIR(b0, sv) } else b0 = sv; s_body(b0); }
+    }
+    {
+        LRDMC_COL_RANGE(2, 3 * it / 2) double b0, b1, b2, sv = 0.0;        // k-steps of two iterations: (0 1 2)(3 4 5) = pairs (0 1)(2 3)(4 5)
+        for (const int i0 = it; it < n; ++it) {
+            if (!((it - i0) & 1)) { LRDMC_BPAIR(b0, b1) LRDMC_BPAIR(b2, sv) } else { b0 = sv; LRDMC_BPAIR(b1, b2) }
+            p_body(b0, b1, b2);
+        }
+    }
+#else
     {
         LRDMC_COL_RANGE(0, it / 2) double b0, b1;
         for (; it + 1 < n; it += 2) { LRDMC_BPAIR(b0, b1) slater_body(b0); slater_body(b1); }
@@ -222,6 +249,7 @@ __device__ __forceinline__ void ao_columns(const DevSys &S, const double *__rest
         for (; it + 1 < n; it += 2) { LRDMC_BPAIR(b0, b1) LRDMC_BPAIR(b2, b3) LRDMC_BPAIR(b4, b5) p_body(b0, b1, b2); p_body(b3, b4, b5); }
         if (it < n) { LRDMC_BPAIR(b0, b1) LRDMC_BPAIR(b2, b3) p_body(b0, b1, b2); }
     }
+#endif
     { LRDMC_COL_RANGE(3, 3 * it) for (; it < n; ++it, sh4 += 4) {   // d: xx xy xz yy yz zz  ->  e Q(d),  Q(d0 +- v) = Q(d0) +- v.grad Q(d0) + Q(v)
         double bc[6]; LRDMC_BPAIR(bc[0], bc[1]) LRDMC_BPAIR(bc[2], bc[3]) LRDMC_BPAIR(bc[4], bc[5])
         LRDMC_GEOM
