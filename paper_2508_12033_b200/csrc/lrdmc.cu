@@ -629,8 +629,10 @@ extern "C" int lrdmc_reconfigure(lrdmc_ctx *c, uint64_t cycle, int32_t *parents_
         ctr[0] = n0; ctr[1] = n1; ctr[2] = n2; ctr[3] = n3; k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
     }
     CK(cudaEventRecord(c->ev[2], st));
-    k_comb<<<1, COMB_THREADS, 0, st>>>(c->W, ctr[0], c->d_stats, parents_dev); ++c->launches;
+    const int split = c->W.n_w > 8192;        // large ensembles: the search (one 128-bit binary search per slot) runs on the whole device
+    k_comb<<<1, COMB_THREADS, 0, st>>>(c->W, ctr[0], c->d_stats, parents_dev, !split); ++c->launches;
     CK(cudaGetLastError());
+    if (split) { k_comb_search<<<(c->W.n_w + 255) / 256, 256, 0, st>>>(c->W, ctr[0], c->d_stats, parents_dev); ++c->launches; CK(cudaGetLastError()); }
     const int rec = 3 * c->S.N;
     size_t total = (size_t)c->W.n_w * (rec + c->S.N * 5 * c->S.OS / 2); int gb = (int)((total + 255) / 256); if (gb > c->sm_count * 16) gb = c->sm_count * 16;
     k_gather<<<gb, 256, 0, st>>>(c->W, rec, c->S.N * 5 * c->S.OS); ++c->launches;

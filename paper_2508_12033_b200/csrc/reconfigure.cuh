@@ -12,11 +12,26 @@ struct DevStats {
     long long moves_min, moves_max, moves_sum, n_node, n_nonpos, n_nonfinite;
     long long n_singular;          // walkers found singular by the last k_rebuild (reading Q24)
     int n_warps, comb_degenerate;
+    unsigned long long comb_T;     // total of the quantised weights (k_comb -> k_comb_search)
 };
 
 #define COMB_THREADS 1024
 
-__global__ void __launch_bounds__(COMB_THREADS) k_comb(DevWalk W, uint32_t r32, DevStats *st, int *parents_user)
+// parent[k] = smallest beta with prefix[beta] * (N_w 2^32) > (r32 + k 2^32) * T, in 128-bit integers (Eq.17 against the cumulative weights, L121)
+__device__ __forceinline__ int comb_parent(const unsigned long long *prefix, int n_w, uint32_t r32, unsigned long long T, int k)
+{
+    const unsigned __int128 scale = (unsigned __int128)(unsigned long long)n_w << 32;
+    const unsigned __int128 rhs = ((unsigned __int128)r32 + ((unsigned __int128)(unsigned long long)k << 32)) * T;
+    int lo = 0, hi = n_w - 1;
+    while (lo < hi) {
+        int mid = (lo + hi) >> 1;
+        if ((unsigned __int128)prefix[mid] * scale > rhs) hi = mid; else lo = mid + 1;
+    }
+    return lo;
+}
+
+// `search_here`: the comb search runs in this CTA (small ensembles: one launch); otherwise k_comb_search does it on the whole device.
+__global__ void __launch_bounds__(COMB_THREADS) k_comb(DevWalk W, uint32_t r32, DevStats *st, int *parents_user, int search_here)
 {
     __shared__ double s_max[32];
     __shared__ unsigned long long s_part[COMB_THREADS];
@@ -58,18 +73,23 @@ __global__ void __launch_bounds__(COMB_THREADS) k_comb(DevWalk W, uint32_t r32, 
     for (int k = k0; k < k1; ++k) { run += W.wq[k]; W.prefix[k] = run; }
     __syncthreads();
     const unsigned long long T = s_part[COMB_THREADS - 1];
-    // 4. comb search: smallest beta with prefix[beta] * (N_w 2^32) > (r32 + k 2^32) * T
-    const unsigned __int128 scale = (unsigned __int128)(unsigned long long)n_w << 32;
-    for (int k = tid; k < n_w; k += COMB_THREADS) {
-        const unsigned __int128 rhs = ((unsigned __int128)r32 + ((unsigned __int128)(unsigned long long)k << 32)) * T;
-        int lo = 0, hi = n_w - 1;
-        while (lo < hi) {
-            int mid = (lo + hi) >> 1;
-            if ((unsigned __int128)W.prefix[mid] * scale > rhs) hi = mid; else lo = mid + 1;
-        }
-        W.parents[k] = lo; if (parents_user) parents_user[k] = lo;
+    // 4. comb search
+    if (search_here) for (int k = tid; k < n_w; k += COMB_THREADS) {
+        const int b = comb_parent(W.prefix, n_w, r32, T, k);
+        W.parents[k] = b; if (parents_user) parents_user[k] = b;
     }
-    if (tid == 0) { st->wbar = ldexp((double)T, -sh) / (double)n_w; st->comb_degenerate = 0; }   // Eq.16
+    if (tid == 0) { st->wbar = ldexp((double)T, -sh) / (double)n_w; st->comb_degenerate = 0; st->comb_T = T; }   // Eq.16
+}
+
+// The comb search of large ensembles, one thread per new slot on the whole device (k_comb left prefix, T and the degenerate flag).
+__global__ void k_comb_search(DevWalk W, uint32_t r32, const DevStats *st, int *parents_user)
+{
+    if (st->comb_degenerate) return;                 // k_comb wrote the identity
+    const int n_w = W.n_w; const unsigned long long T = st->comb_T;
+    for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < n_w; k += gridDim.x * blockDim.x) {
+        const int b = comb_parent(W.prefix, n_w, r32, T, k);
+        W.parents[k] = b; if (parents_user) parents_user[k] = b;
+    }
 }
 
 // new slot k <- positions of parent[k]; weights <- 1 (L129).  Inverses and caches are rebuilt afterwards (reading Q15),

@@ -271,7 +271,7 @@ def test_large_system_path_tables_in_global_memory(B, name):
 
 
 # ------------------------------------------------------------------------------------------ a12: reconfiguration alone
-@pytest.mark.parametrize("n_w", [1, 2, 5, 33, 1024, 1025, 4099])
+@pytest.mark.parametrize("n_w", [1, 2, 5, 33, 1024, 1025, 4099, 8192, 8193, 70001])      # above 8192 the comb search is a kernel of its own (k_comb_search)
 def test_reconfigure_indices_bit_exact_for_adversarial_weights(B, n_w):
     s = wl.hydrogen(); g = B.Lrdmc(s); o = ref.Ref(s); rng = np.random.default_rng(n_w)
     x0 = wl.hydrogen_walkers(n_w, 2)
