@@ -200,8 +200,8 @@ def main():
         torch.cuda.synchronize()
 
     def timed(mode, steps, first_cycle, tau_, feedback=True):
-        """K steps bracketed by barrier+sync, CUDA events on the launching stream.  Per step: every ensemble's propagate + reconfigure
-        is enqueued on its own stream, then every ensemble's estimators are read (a step ends when all K results are on the host)."""
+        """K steps bracketed by barrier+sync, CUDA events on the launching stream.  Per step and ensemble: read the estimators of its last
+        interval (E_0 feedback), enqueue propagate + reconfigure on its own stream; the region ends when all results are on the host."""
         barrier()
         e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
         l0 = sum(c[0].launch_count() for c in ctxs); recs = [[] for _ in ctxs]
@@ -210,15 +210,20 @@ def main():
         if K > 1:
             for c in ctxs:
                 c[0].stream.wait_event(e0)
+        def collect(q, c):
+            st = c[0].lrdmc_estimators(); recs[q].append(st)
+            if mode == B.BALANCED and feedback and st.den > 0:
+                esum[q] += st.num / st.den; ecnt[q] += 1; E0[q] = esum[q] / ecnt[q]   # "Update E_0" (Alg.2 line 12 L418)
+        # pipelined over the ensembles (driver.a_scan does the same): ensemble q's next interval is enqueued as soon as ITS last one has been read
         for cyc_ in range(first_cycle, first_cycle + steps):
             for q, c in enumerate(ctxs):
+                if cyc_ > first_cycle:
+                    collect(q, c)
                 with torch.cuda.stream(c[0].stream):
                     c[0].lrdmc_propagate(mode, args.moves if mode == B.BALANCED else 0, tau_, E0[q] if mode == B.BALANCED else 0.0, cyc_)
                     c[0].lrdmc_reconfigure(cyc_)
-            for q, c in enumerate(ctxs):
-                st = c[0].lrdmc_estimators(); recs[q].append(st)
-                if mode == B.BALANCED and feedback and st.den > 0:
-                    esum[q] += st.num / st.den; ecnt[q] += 1; E0[q] = esum[q] / ecnt[q]   # "Update E_0" (Alg.2 line 12 L418)
+        for q, c in enumerate(ctxs):
+            collect(q, c)
         if K > 1:
             for c in ctxs:
                 main_stream.wait_stream(c[0].stream)

@@ -71,8 +71,8 @@ def fit_a_to_zero(a_list, energies, sigmas, n_terms=2):
 def a_scan(make_system, make_walkers, a_list, n_walkers, cycles, moves, modes=("balanced", "conventional"), E0=0.0, n_therm=None,
            p=10, n_blocks=10, device="cuda:0", concurrent=True, feedback_therm=0):
     """SURVEY 8(f) f3 "several a in one batch": one LRDMC run per (lattice spacing, mode), ALL of them in flight together on the CUDA
-    path -- every run is a context of its own on a CUDA stream of its own; per generation the propagate + reconfigure of every run
-    is enqueued first, then every run's estimators are read and its E_0 updated, so the small ensembles of an a-scan share the
+    path -- every run is a context of its own on a CUDA stream of its own; each run's next generation is enqueued as soon as its own
+    estimators have been read and its E_0 updated (pipelined, no barrier across the runs), so the small ensembles of an a-scan share the
     device instead of leaving most SMs idle one after the other (`concurrent=False`: one run after the other, same numbers).
     Rows shaped like Table I (a, E_balanced, E_conventional; L254-L265), then the E(a) = E_0 + c a^2 fits (L140).
     make_system(a) -> system dict; make_walkers(system, n_walkers) -> positions.  Run number q (a-major, mode-minor) draws from its
@@ -93,25 +93,33 @@ def a_scan(make_system, make_walkers, a_list, n_walkers, cycles, moves, modes=("
                              kind=B.BALANCED if mode == "balanced" else B.CONVENTIONAL,
                              n_moves=moves if mode == "balanced" else 0, tau=0.0 if mode == "balanced" else moves * a * a / (3 * N)))
 
-    def step(batch, c):
-        for r in batch:                                            # enqueue: nothing here waits for the device
-            with torch.cuda.stream(r["stream"]):
-                r["g"].lrdmc_propagate(r["kind"], r["n_moves"], r["tau"], r["E0"], c)
-                r["g"].lrdmc_reconfigure(c)
-        for r in batch:                                            # read back: each call waits for its own stream only
-            s = r["g"].lrdmc_estimators(); r["recs"].append(s)
-            if len(r["recs"]) - 1 == feedback_therm and feedback_therm > 0:
-                r["esum"] = 0.0; r["ecnt"] = 0
-            r["esum"] += s.num / s.den; r["ecnt"] += 1
-            if r["kind"] == B.BALANCED:
-                r["E0"] = r["esum"] / r["ecnt"]                    # "Update E_0" (Alg.2 line 12 L418; reading Q8a)
+    def enqueue(r, c):                                             # nothing here waits for the device
+        with torch.cuda.stream(r["stream"]):
+            r["g"].lrdmc_propagate(r["kind"], r["n_moves"], r["tau"], r["E0"], c)
+            r["g"].lrdmc_reconfigure(c)
+
+    def collect(r):                                                # waits for the run's own stream only
+        s = r["g"].lrdmc_estimators(); r["recs"].append(s)
+        if len(r["recs"]) - 1 == feedback_therm and feedback_therm > 0:
+            r["esum"] = 0.0; r["ecnt"] = 0
+        r["esum"] += s.num / s.den; r["ecnt"] += 1
+        if r["kind"] == B.BALANCED:
+            r["E0"] = r["esum"] / r["ecnt"]                        # "Update E_0" (Alg.2 line 12 L418; reading Q8a)
     if concurrent:
+        # Pipelined: a run's generation c is enqueued as soon as ITS generation c - 1 has been read (E_0 feedback), while the other runs'
+        # kernels are still queued or running -- no barrier across the runs between generations, so the device always has every run's
+        # CTAs to fill its SMs with (a generation of all runs together does not fit the resident slots: lock-stepped generations ran in two waves).
         for c in range(cycles):
-            step(runs, c)
+            for r in runs:
+                if c > 0:
+                    collect(r)
+                enqueue(r, c)
+        for r in runs:
+            collect(r)
     else:
         for r in runs:
             for c in range(cycles):
-                step([r], c)
+                enqueue(r, c); collect(r)
     rows = []
     for a in a_list:
         row = {"a": a}
