@@ -259,6 +259,9 @@ def main():
                 "dmma_peak": peaks["dmma_tflops"], "dfma_dmma_mixed": peaks["mixed_tflops"], "dfma_3reg_peak": peaks["dfma_3reg_tflops"], "dfma_with_2_alu_peak": peaks["dfma_alu_tflops"],
                 "kernel_ms": prop_ms, "kernel_share_of_step": prop_ms * len(recs) / (secs * 1e3),
                 "hbm_bytes_per_launch_algorithmic": 2 * drv.state_bytes_per_walker(sysd) * args.nw}
+    if cfg.get("listed_sweep"):      # the executed count assumes the dense sweep; the listed sweep skips the unlisted (electron, shell) pairs and keeps Bc as state
+        roofline["frac_executed"] = None; roofline["achieved_executed"] = None
+        roofline["frac_executed_note"] = "listed sweep: the flop executed depend on the walkers' shell lists (DESIGN.md section 4: 58 % of the pairs are skipped at C5, 41 % at C4); the dense column-form count would give %.3f" % (executed / peaks["dfma_tflops"])
     if K > 1:
         roofline["note"] = f"{K} contexts in flight: kernel_ms is one launch of context 0 while the others run beside it; achieved/frac describe that launch, not the device"
 

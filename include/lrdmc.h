@@ -209,6 +209,8 @@ int lrdmc_debug_draws(const lrdmc_ctx *, uint64_t cycle, uint64_t step, double *
  * *team_warps = warps per walker: 1 = kernel k_propagate (warp per walker), > 1 = kernel k_propagate_team. */
 int lrdmc_launch_count(const lrdmc_ctx *);
 int lrdmc_launch_config(const lrdmc_ctx *, int *grid, int *block, int *smem_bytes, int *ctas_per_sm, int *team_warps);
+/* 1 if the candidate pass of this ctx is the listed sweep (LRDMC_OPT_LISTED, or automatic for global-table systems), else 0 */
+int lrdmc_listed_sweep(const lrdmc_ctx *);
 
 #ifdef __cplusplus
 }

@@ -22,7 +22,7 @@ OPT_TEAM_WARPS, OPT_GLOBAL_TABLES, OPT_LISTED = 1, 2, 3
 EXPORTS = ["lrdmc_init", "lrdmc_free", "lrdmc_strerror", "lrdmc_last_error", "lrdmc_set_option", "lrdmc_n_candidates", "lrdmc_walker_bytes",
            "lrdmc_bind_walkers", "lrdmc_set_positions", "lrdmc_propagate", "lrdmc_reconfigure", "lrdmc_estimators", "lrdmc_energy",
            "lrdmc_step_debug", "lrdmc_get_walkers", "lrdmc_set_state", "lrdmc_get_obs", "lrdmc_run_host", "lrdmc_debug_philox",
-           "lrdmc_debug_draws", "lrdmc_launch_count", "lrdmc_launch_config"]
+           "lrdmc_debug_draws", "lrdmc_launch_count", "lrdmc_launch_config", "lrdmc_listed_sweep"]
 PROBE_EXPORTS = ["lrdmc_measure_fp64_peaks", "lrdmc_measure_fp64_operand_peak"]
 
 
@@ -94,6 +94,7 @@ def load_library():
         L.lrdmc_debug_draws.argtypes = [vp, u64, u64, vp, i32, vp]
         L.lrdmc_launch_count.argtypes = [vp]
         L.lrdmc_launch_config.argtypes = [vp, C.POINTER(i32), C.POINTER(i32), C.POINTER(i32), C.POINTER(i32), C.POINTER(i32)]
+        L.lrdmc_listed_sweep.argtypes = [vp]
         _lib = L
     return _lib
 
@@ -292,7 +293,7 @@ class Lrdmc:
         g, b, s, c, t = C.c_int(), C.c_int(), C.c_int(), C.c_int(), C.c_int()
         self.L.lrdmc_launch_config(self.h, C.byref(g), C.byref(b), C.byref(s), C.byref(c), C.byref(t))
         return dict(grid=g.value, block=b.value, smem_bytes=s.value, ctas_per_sm=c.value, team_warps=t.value,
-                    kernel="k_propagate" if t.value <= 1 else "k_propagate_team")
+                    kernel="k_propagate" if t.value <= 1 else "k_propagate_team", listed_sweep=bool(self.L.lrdmc_listed_sweep(self.h)))
 
     def debug_draws(self, cycle, step, n):
         out = self.torch.empty((n, 14), dtype=self.torch.float64, device=self.device)

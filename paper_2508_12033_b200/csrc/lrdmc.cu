@@ -677,6 +677,7 @@ extern "C" int lrdmc_step_debug(lrdmc_ctx *c, double E0, uint64_t cycle, uint64_
 }
 
 extern "C" int lrdmc_launch_count(const lrdmc_ctx *c) { return c ? c->launches : 0; }
+extern "C" int lrdmc_listed_sweep(const lrdmc_ctx *c) { return c ? c->listed : 0; }
 extern "C" int lrdmc_bound_walkers(const lrdmc_ctx *c) { return (c && c->bound) ? c->W.n_w : 0; }
 extern "C" int lrdmc_n_electrons(const lrdmc_ctx *c) { return c ? c->S.N : 0; }
 extern "C" const DevSys *lrdmc_devsys(const lrdmc_ctx *c) { return &c->S; }
