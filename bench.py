@@ -261,7 +261,8 @@ def main():
                 "hbm_bytes_per_launch_algorithmic": 2 * drv.state_bytes_per_walker(sysd) * args.nw}
     if cfg.get("listed_sweep"):      # the executed count assumes the dense sweep; the listed sweep skips the unlisted (electron, shell) pairs and keeps Bc as state
         roofline["frac_executed"] = None; roofline["achieved_executed"] = None
-        roofline["frac_executed_note"] = "listed sweep: the flop executed depend on the walkers' shell lists (DESIGN.md section 4: 58 % of the pairs are skipped at C5, 41 % at C4); the dense column-form count would give %.3f" % (executed / peaks["dfma_tflops"])
+        roofline["frac_executed_note"] = ("listed sweep: the flop executed depend on the walkers' shell lists (DESIGN.md section 4: 58 percent of the pairs are skipped at C5, 41 percent at C4); "
+                                          f"the dense column-form count would give {executed / peaks['dfma_tflops']:.3f}")
     if K > 1:
         roofline["note"] = f"{K} contexts in flight: kernel_ms is one launch of context 0 while the others run beside it; achieved/frac describe that launch, not the device"
 
