@@ -256,7 +256,7 @@ def main():
                 "achieved_executed": executed, "frac_executed": executed / peaks["dfma_tflops"],
                 "flop_per_walker_move": flop["total"], "flop_executed_per_walker_move": flop["executed"],
                 "peak_source": "measured live: liblrdmc_probe lrdmc_measure_fp64_peaks (independent DFMA chains, all SMs)",
-                "dmma_peak": peaks["dmma_tflops"], "dfma_dmma_mixed": peaks["mixed_tflops"], "dfma_3reg_peak": peaks["dfma_3reg_tflops"], "dfma_with_2_alu_peak": peaks["dfma_alu_tflops"],
+                "dmma_peak": peaks["dmma_tflops"], "dfma_dmma_mixed": peaks["mixed_tflops"], "dfma_3reg_peak": peaks["dfma_3reg_tflops"], "dfma_1shared_peak": peaks["dfma_shared1_tflops"], "dfma_with_2_alu_peak": peaks["dfma_alu_tflops"],
                 "kernel_ms": prop_ms, "kernel_share_of_step": prop_ms * len(recs) / (secs * 1e3),
                 "hbm_bytes_per_launch_algorithmic": 2 * drv.state_bytes_per_walker(sysd) * args.nw}
     if cfg.get("listed_sweep"):      # the executed count assumes the dense sweep; the listed sweep skips the unlisted (electron, shell) pairs and keeps Bc as state

@@ -16,6 +16,8 @@ int lrdmc_measure_fp64_peaks(double *dfma_tflops, double *dmma_tflops, double *m
  * dfma_alu_tflops  -- two-register FMAs each followed by two independent integer ALU instructions of the same warp
  *                     (FP64 flop only).  The second pointer may be NULL. */
 int lrdmc_measure_fp64_operand_peak(double *dfma_3reg_tflops, double *dfma_alu_tflops);
+/* FMAs with ONE source register shared with the neighbouring FMAs (acc[i] += g[i] * b; operand-reuse cache): between the 2- and the 3-register forms */
+int lrdmc_measure_fp64_shared_operand_peak(double *dfma_shared1_tflops);
 #ifdef __cplusplus
 }
 #endif

@@ -23,7 +23,7 @@ EXPORTS = ["lrdmc_init", "lrdmc_free", "lrdmc_strerror", "lrdmc_last_error", "lr
            "lrdmc_bind_walkers", "lrdmc_set_positions", "lrdmc_propagate", "lrdmc_reconfigure", "lrdmc_estimators", "lrdmc_energy",
            "lrdmc_step_debug", "lrdmc_get_walkers", "lrdmc_set_state", "lrdmc_get_obs", "lrdmc_run_host", "lrdmc_debug_philox",
            "lrdmc_debug_draws", "lrdmc_launch_count", "lrdmc_launch_config", "lrdmc_listed_sweep"]
-PROBE_EXPORTS = ["lrdmc_measure_fp64_peaks", "lrdmc_measure_fp64_operand_peak"]
+PROBE_EXPORTS = ["lrdmc_measure_fp64_peaks", "lrdmc_measure_fp64_operand_peak", "lrdmc_measure_fp64_shared_operand_peak"]
 
 
 class System(C.Structure):
@@ -137,11 +137,12 @@ def lrdmc_measure_fp64_peaks():
             raise RuntimeError(f"{PROBE_LIB_PATH} is missing: run `python -m paper_2508_12033_b200.build`")
         _probe = C.CDLL(PROBE_LIB_PATH)
         dp = C.POINTER(C.c_double)
-        _probe.lrdmc_measure_fp64_peaks.argtypes = [dp, dp, dp]; _probe.lrdmc_measure_fp64_operand_peak.argtypes = [dp, dp]
-    a, b, m, t, u = (C.c_double() for _ in range(5))
-    if _probe.lrdmc_measure_fp64_peaks(C.byref(a), C.byref(b), C.byref(m)) or _probe.lrdmc_measure_fp64_operand_peak(C.byref(t), C.byref(u)):
+        _probe.lrdmc_measure_fp64_peaks.argtypes = [dp, dp, dp]; _probe.lrdmc_measure_fp64_operand_peak.argtypes = [dp, dp]; _probe.lrdmc_measure_fp64_shared_operand_peak.argtypes = [dp]
+    a, b, m, t, u, v = (C.c_double() for _ in range(6))
+    if (_probe.lrdmc_measure_fp64_peaks(C.byref(a), C.byref(b), C.byref(m)) or _probe.lrdmc_measure_fp64_operand_peak(C.byref(t), C.byref(u))
+            or _probe.lrdmc_measure_fp64_shared_operand_peak(C.byref(v))):
         raise RuntimeError("FP64 peak probe failed (CUDA error)")
-    return dict(dfma_tflops=a.value, dmma_tflops=b.value, mixed_tflops=m.value, dfma_3reg_tflops=t.value, dfma_alu_tflops=u.value)
+    return dict(dfma_tflops=a.value, dmma_tflops=b.value, mixed_tflops=m.value, dfma_3reg_tflops=t.value, dfma_alu_tflops=u.value, dfma_shared1_tflops=v.value)
 
 
 class Lrdmc:

@@ -42,6 +42,24 @@ static __global__ void __launch_bounds__(256) k_fp64_peak_3reg(double *out, int 
     if (s == 123.456) out[blockIdx.x * blockDim.x + threadIdx.x] = s;
 }
 
+// DFMA with ONE source operand shared with the neighbouring DFMAs (acc[i] += g[i] * b: the form of the candidate pass's accumulations, where the
+// operand-reuse cache can hold b): between the two cases above -- 2.56 dispatch cycles on B200 against 2.18 (two shared) and 3.11 (none).
+static __global__ void __launch_bounds__(256) k_fp64_peak_shared1(double *out, int iters, double seed)
+{
+    double f[8], g[8];
+    const double b = 1.0 - 1e-7 * (1 + threadIdx.x);
+#pragma unroll
+    for (int i = 0; i < 8; ++i) { f[i] = seed * (i + 1); g[i] = 1e-7 * (i + 1 + threadIdx.x); }
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int i = 0; i < 8; ++i) f[i] = fma(g[i], b, f[i]);
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) s += f[i];
+    if (s == 123.456) out[blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
 // DFMA (two register operands + a constant: 2 dispatch cycles) interleaved with independent integer ALU work of the same
 // warp (an and and an add per DFMA with run-time operands, which the compiler cannot fold): does the other work hide in the FP64 instruction's
 // second cycle?  On B200 it does not: the time is the SUM of the dispatch cycles (2 + 1 + 1), see DESIGN.md section 4.

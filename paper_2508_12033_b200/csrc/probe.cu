@@ -34,20 +34,21 @@ extern "C" int lrdmc_measure_fp64_peaks(double *dfma, double *dmma, double *mixe
     return 0;
 }
 
-extern "C" int lrdmc_measure_fp64_operand_peak(double *dfma3, double *dfma_alu)
+static int operand_peaks(double *dfma3, double *dfma_alu, double *dfma_shared1)
 {
     int dev = 0; cudaDeviceProp prop;
     if (!dfma3 || cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return -4;
     const int blocks = prop.multiProcessorCount * 8, threads = 256, iters = 8192;
     double *d_out = NULL; if (cudaMalloc((void **)&d_out, sizeof(double) * blocks * threads) != cudaSuccess) return -4;
     cudaEvent_t e0, e1; cudaEventCreate(&e0); cudaEventCreate(&e1);
-    double res[2] = { 0, 0 };
-    for (int mode = 0; mode < 2; ++mode) {
+    double res[3] = { 0, 0, 0 };
+    for (int mode = 0; mode < 3; ++mode) {
         float best = 1e30f;
         for (int rep = 0; rep < 5; ++rep) {
             cudaEventRecord(e0);
             if (mode == 0) k_fp64_peak_3reg<<<blocks, threads>>>(d_out, iters, 1.000001);
-            else k_fp64_peak_alu<<<blocks, threads>>>(d_out, iters, 1.000001);
+            else if (mode == 1) k_fp64_peak_alu<<<blocks, threads>>>(d_out, iters, 1.000001);
+            else k_fp64_peak_shared1<<<blocks, threads>>>(d_out, iters, 1.000001);
             cudaEventRecord(e1); cudaEventSynchronize(e1);
             float ms = 0; cudaEventElapsedTime(&ms, e0, e1);
             if (rep > 0 && ms < best) best = ms;
@@ -56,7 +57,9 @@ extern "C" int lrdmc_measure_fp64_operand_peak(double *dfma3, double *dfma_alu)
     }
     cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d_out);
     if (cudaGetLastError() != cudaSuccess) return -4;
-    *dfma3 = res[0]; if (dfma_alu) *dfma_alu = res[1];
+    *dfma3 = res[0]; if (dfma_alu) *dfma_alu = res[1]; if (dfma_shared1) *dfma_shared1 = res[2];
     return 0;
 }
+extern "C" int lrdmc_measure_fp64_operand_peak(double *dfma3, double *dfma_alu) { return operand_peaks(dfma3, dfma_alu, NULL); }
+extern "C" int lrdmc_measure_fp64_shared_operand_peak(double *dfma_shared1) { double t; return operand_peaks(&t, NULL, dfma_shared1); }
 
