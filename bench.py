@@ -71,11 +71,11 @@ class ClockSampler:
                 "reasons": reasons, "samples": len(self.rows)}
 
 
-def oracle_sample(sysd, n_w, cycles, moves, seed=5, min_seconds=0.0):
+def oracle_sample(sysd, n_w, cycles, moves, seed=5, min_seconds=0.0, threads=0):
     """The oracle as it stands, timed on the host cores on a bounded sample of the same workload."""
     from oracle import lrdmc_ref as ref
     o = ref.Ref(sysd)
-    cores = ref.set_threads(0)
+    cores = ref.set_threads(threads)           # 0 = all host cores (OpenMP over walkers)
     x0 = wl.initial_walkers(sysd, n_w, seed)
     rc = o.set_positions(x0)
     if rc not in (0, -2):
@@ -249,7 +249,7 @@ def main():
     per_launch_moves = sum(r.moves_sum for r in recs) / len(recs)
     achieved = flop["total"] * per_launch_moves / (prop_ms * 1e-3) / 1e12
     executed = flop["executed"] * per_launch_moves / (prop_ms * 1e-3) / 1e12
-    roofline = {"bound": "alu", "kernel": cfg["kernel"], "achieved": achieved, "peak": peaks["dfma_tflops"], "unit": "TFLOP/s", "frac": achieved / peaks["dfma_tflops"],
+    roofline = {"bound": "alu", "kernel": cfg["kernel"], "achieved": achieved, "peak": peaks["dfma_tflops"], "unit": "TFLOP/s", "frac": achieved / peaks["dfma_tflops"], "frac_vs_dmma_peak": achieved / peaks["dmma_tflops"],
                 "traffic": measured_traffic(args.workload, args.nw, cfg["kernel"], args.moves) if K == 1 else None,
                 "frac_note": "frac = ALGORITHMIC flop (SURVEY 8(d) count, every candidate through the MOs) / kernel time / peak: speed relative to the naive algorithm "
                              "at peak, may exceed 1; frac_executed = flop the column-form kernel executes / kernel time / peak: FP64-pipe utilisation (compare ncu sm__pipe_fp64_cycles_active)",
@@ -321,7 +321,10 @@ def main():
     if rank == 0 and not args.no_cpu_baseline and world == 1:
         ref_sys = sysd if args.workload != "C4" else wl.water_methane(n_walkers=args.ref_nw)
         v, cores, dt, n = oracle_sample(ref_sys, args.ref_nw, 2, args.moves, min_seconds=12.0)
-        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
+        # also on ONE core (after the all-core sample: the oracle's thread count stays at what was set last)
+        v1, _, dt1, n1 = oracle_sample(ref_sys, 8, 1, args.moves, min_seconds=3.0, threads=1)
+        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "value_1core": v1,
+                                "sample_1core": f"N_w=8 walkers x {n1 // (8 * args.moves)} cycles x {args.moves} moves, 1 thread ({dt1:.1f} s)",
                                 "sample": f"same {args.workload} system, N_w={args.ref_nw} walkers x {n // (args.ref_nw * args.moves)} cycles x {args.moves} moves ({n} walker-moves, {dt:.1f} s), balanced, incl. reconfiguration"}
     if rank == 0:
         print(json.dumps(line), flush=True)
