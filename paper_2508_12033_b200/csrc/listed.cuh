@@ -1,19 +1,20 @@
-// listed.cuh -- the candidate pass of the LARGE systems (tables in global memory: 64 electrons, 600 AOs) as a LISTED sweep.
+// listed.cuh -- the candidate pass as a LISTED sweep (template bit EXT = 4 of the walker kernels): chosen automatically for the systems whose tables
+// live in global memory (64 electrons, 600 AOs), available on any lattice-only system through LRDMC_OPT_LISTED.
 //
 // Rows a1-a4 of the scope table in column form (wavefunction.cuh: sum_m phi_m(r') Dinv[m][i] = sum_mu chi_mu(r') Bc[mu][i], Bc = C Dinv),
 // with two changes against the dense sweep of ao_columns:
-//   (1) Gaussian sparsity.  In a 12-bohr cluster most (electron, shell) pairs contribute nothing: a shell is LISTED for a row of six
-//       displaced points x0 +- step e_k only when |x0 - R_shell| < step + srad(zeta) (common.cuh LRDMC_LIST_THR: every exponent of an
-//       unlisted shell is below -52 in any frame, its terms below 1e-22 of the norm).  Counted on thermalised configurations: 58 % of
-//       the pairs of the 64-electron configuration are unlisted.  The test depends on positions only, so the
-//       lists are 64-bit masks per (electron, list group) kept with the walker state and refreshed for the electron that hopped.
-//   (2) Bc is STATE, not recomputed: the CTA keeps Bc [electron][n_aop] of its walker in global scratch, builds it when the walker
-//       is loaded and updates it with the same rank-1 formula as the inverse after every hop
+//   (1) Gaussian sparsity.  Most (electron, shell) pairs of an extended system contribute nothing: a shell is LISTED for the six displaced
+//       points x0 +- step e_k of an electron only when |x0 - R_shell| < step + srad(zeta) (common.cuh LRDMC_LIST_THR: every exponent of an
+//       unlisted shell is below -52 in any frame, its terms below 1e-22 of the norm).  Counted on thermalised configurations: 58 % of the
+//       pairs of the 64-electron configuration and 41 % of the water-methane-shaped one are unlisted.  The test
+//       depends on the positions only, so the lists (bytes, per electron and list group) are kept with the walker state in shared memory
+//       and rebuilt for the electron that hopped.
+//   (2) Bc is STATE, not recomputed: Bc [electron][n_aop] of the walker lives in a global scratch of the resident CTA / warp, is built when
+//       the walker is loaded and follows the inverse by the same rank-1 formula after every hop
 //       (Bc'[:,k] = Bc[:,k] - Bc[:,i] s_k / rho, Bc'[:,i] = Bc[:,i] / rho: 2 A n_s flop instead of 2 A O n_s on the tensor pipe).
-// Work is dealt by ROWS (mesh, electron), a batch of at most 16 rows per warp: the lanes of the warp split every row's list of a
-// type group into pieces of c consecutive listed shells (c minimal with sum_rows ceil(n_row / c) <= 32), sweep c pairs each, and add
-// their shares by a segmented shuffle reduction.  The Jastrow ratios of the same rows follow in the same warp, so a warp finishes
-// R_j of its rows without meeting the others.
+// The sweep keeps the lane map of the dense pass -- a quad per row (mesh, electron), lane t takes every fourth entry of ITS electron's
+// list -- so the four shares meet in a quad shuffle and the Jastrow ratios of the same 8 rows reuse the geometry (evaluate.cuh,
+// listed_phase_b); 8-row batches are independent, a team deals them to its warps.  The oracle never screens.
 #pragma once
 #include "common.cuh"
 #include "fastmath.cuh"
@@ -21,7 +22,6 @@
 // Per-walker lists (shared memory, bytes): cnt [n_lg][N] listed-shell counts, then lst [N][lt] slot numbers (relative to the list group's first
 // slot), the groups of an electron at lg_off[lg].  A shell is listed for electron i when |r_i - R_shell| < step_max + srad: the test depends on the
 // position only, so the lists are kept with the walker state and rebuilt for the electron that hopped.
-__device__ __forceinline__ int list_doubles(const DevSys &S) { return (S.N * (S.lt + S.n_lg) + 7) >> 3; }
 __device__ __forceinline__ void list_build(const DevSys &S, const double *shells, const double *srad, unsigned char *lw, int i, double x, double y, double z,
                                            double step_max, int lane)
 {
