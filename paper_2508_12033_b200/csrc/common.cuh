@@ -17,7 +17,7 @@
 #define LRDMC_LOCKSTEP 1        // balanced mode: the warps of a CTA step together (one barrier per step)
 #endif
 #ifndef LRDMC_BC_STORE
-#define LRDMC_BC_STORE 1         // team kernel of the large systems: park the Bc entries (ao_columns BCS) instead of redoing the DMMAs
+#define LRDMC_BC_STORE 1         // Bc kept between evaluations: listed sweep (listed.cuh), or parked entries of the dense sweep of the large systems (ao_columns BCS)
 #endif
 #define LRDMC_NUC_STRIDE 20  // doubles per nucleus row: Rx Ry Rz Z c1 b1 alpha beta gamma delta is_pp pad | r_c A0 B0 A1 B1 A2 B2 pad (non-local channels)
 #define LRDMC_NL_OFF 12      // first non-local entry of a nucleus row
@@ -113,7 +113,7 @@ struct DevWalk {
     unsigned long long *timing;      // [max_warps][2] globaltimer start/end per resident warp
     double *stats;        // device copy of the reduced numbers (see k_reduce_obs)
     int *counter;         // dynamic walker queue head; [1] = singular flag
-    double *bcs;          // per resident team CTA: Bc = C Dinv of its walker, [electron][n_aop] (listed sweep, updated rank-1 with the inverse),
+    double *bcs;          // per resident team CTA / warp of the warp-per-walker kernel: Bc = C Dinv of its walker, [electron][n_aop] (listed sweep, updated rank-1 with the inverse),
                           // or the parked Bc entries [block of a mesh][k-step pair][lane][2] of ao_columns BCS; NULL if unused
     size_t bcs_stride;    // doubles per CTA
     int bcs_ctas;         // CTAs the scratch was sized for

@@ -60,7 +60,7 @@ __device__ __forceinline__ void publish_frame(const WarpState &ws, const StepDra
     __syncwarp();
 }
 
-// LISTED (EXT bit 2): also the listed-shell masks of every electron and Bc = C Dinv of this walker in the warp's global scratch ws.bc.
+// LISTED (EXT bit 2): also the shell lists of every electron and Bc = C Dinv of this walker in the warp's global scratch ws.bc.
 template <bool TS, bool LISTED = false>
 __device__ __forceinline__ void load_walker(const DevSys &S, const DevWalk &W, WarpState &ws, const Tables &T, int k, int lane, bool with_dinv, bool with_onebody = true)
 {

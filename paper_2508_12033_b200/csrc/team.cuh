@@ -295,7 +295,7 @@ __device__ __forceinline__ void apply_move_team(const DevSys &S, const TeamPlan 
         }
     }
     if (wt == 0) { refresh_onebody(S.n_nuc, S.has_j1, S.a, T.nuc, ws.ob + 8 * i, px, py, pz, lane); if (EXT & 2) refresh_j3_row(S, T.nuc, ws.j3 + i * S.j3s, px, py, pz, lane); }
-    if (LISTED && wt == TW - 1)            // the mover's listed-shell masks at its new position
+    if (LISTED && wt == TW - 1)            // the mover's shell lists at its new position
         list_build(S, T.shells, T.srad, ws.lw, i, px, py, pz, fmax(S.amesh[0], S.amesh[1]), lane);
     __syncthreads();                                   // every thread has read the old position
     for (int idx = tid; idx < rows; idx += nthr) {
@@ -354,7 +354,7 @@ __global__ void __launch_bounds__(LRDMC_TEAM_MAX_WARPS * 32, 1) k_propagate_team
             continue;
         }
         load_walker_team(S, W, ws, T.nuc, k, P.TW);
-        if (LISTED) {                                           // listed sweep: masks of every electron, Bc of this walker
+        if (LISTED) {                                           // listed sweep: shell lists of every electron, Bc of this walker
             for (int i = wt; i < S.N; i += P.TW)
                 list_build(S, T.shells, T.srad, ws.lw, i, ws.r[3 * i], ws.r[3 * i + 1], ws.r[3 * i + 2], fmax(S.amesh[0], S.amesh[1]), lane);
             build_bc(S, ws.dinv[0], ws.dinv[1], reinterpret_cast<double *>(bcs_cta), tid, blockDim.x);
