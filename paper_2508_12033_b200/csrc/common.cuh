@@ -10,6 +10,9 @@
 #ifndef LRDMC_WPB
 #define LRDMC_WPB 8            // warps (= walkers in flight) per CTA
 #endif
+#ifndef LRDMC_WPB_EXT
+#define LRDMC_WPB_EXT 6        // the same for the extended kernels (non-local slots / three-body Jastrow): their state leaves room for 7, which two
+#endif                         // CTAs cannot spread evenly over the 4 schedulers (lrdmc.cu plan_smem); 192 threads also lift the register cap to 168
 #ifndef LRDMC_MINB
 #define LRDMC_MINB 2           // CTAs per SM the register allocation must allow
 #endif

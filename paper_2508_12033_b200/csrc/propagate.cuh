@@ -102,7 +102,7 @@ __device__ __forceinline__ void store_walker(const DevSys &S, const DevWalk &W, 
 
 // ---- the projection kernel (Alg.2 lines 4-8 L401-L410 / Alg.1 lines 4-16 L350-L374) ----------------------------
 template <int NT, bool TS, int EXT>
-__global__ void __launch_bounds__(LRDMC_WPB * 32, LRDMC_MINB) k_propagate(DevSys S, DevWalk W, int mode, int n_moves, double tau, double E0, uint32_t cycle)
+__global__ void __launch_bounds__(((EXT & 3) ? LRDMC_WPB_EXT : LRDMC_WPB) * 32, LRDMC_MINB) k_propagate(DevSys S, DevWalk W, int mode, int n_moves, double tau, double E0, uint32_t cycle)
 {
     extern __shared__ __align__(16) double smem[];
     stage_tables(S, smem);
@@ -174,7 +174,7 @@ __global__ void __launch_bounds__(LRDMC_WPB * 32, LRDMC_MINB) k_propagate(DevSys
 
 // ---- parity hook: one evaluation + selection, no state change ---------------------------------------------------
 template <int NT, bool TS, int EXT>
-__global__ void __launch_bounds__(LRDMC_WPB * 32, LRDMC_MINB) k_step_debug(DevSys S, DevWalk W, double E0, uint32_t cycle, uint32_t step, double *R_out,
+__global__ void __launch_bounds__(((EXT & 3) ? LRDMC_WPB_EXT : LRDMC_WPB) * 32, LRDMC_MINB) k_step_debug(DevSys S, DevWalk W, double E0, uint32_t cycle, uint32_t step, double *R_out,
                                                     double *scal_out, int *jstar_out)
 {
     extern __shared__ __align__(16) double smem[];
