@@ -11,8 +11,8 @@
 #define LRDMC_WPB 8            // warps (= walkers in flight) per CTA
 #endif
 #ifndef LRDMC_WPB_EXT
-#define LRDMC_WPB_EXT 6        // the same for the extended kernels (non-local slots / three-body Jastrow): their state leaves room for 7, which two
-#endif                         // CTAs cannot spread evenly over the 4 schedulers (lrdmc.cu plan_smem); 192 threads also lift the register cap to 168
+#define LRDMC_WPB_EXT 6        // second instantiation of the extended kernels (non-local slots / three-body Jastrow) for systems whose state leaves room
+#endif                         // for 6 or 7 warps only: 7 cannot be spread evenly over the 4 schedulers (lrdmc.cu plan_smem), and 192 threads lift the register cap to 168
 #ifndef LRDMC_MINB
 #define LRDMC_MINB 2           // CTAs per SM the register allocation must allow
 #endif
@@ -69,7 +69,7 @@ struct DevSys {
     // shared-memory plan (units: doubles)
     int bf_in_smem, moc_in_smem, cf_in_smem;   // cf_in_smem: the pair table of ao_columns is staged too (not with the listed sweep)
     int off_shells, off_nuc, off_bf[2], off_etab, tables_doubles;
-    int o_r, o_dinv[2], o_moc, o_R, o_cum, o_el, o_ob, o_U, o_j3, per_warp_doubles;   // o_j3: chi3 [N][j3s], V3 [N][j3s], S3 [j3s] (systems with a J3)
+    int o_r, o_dinv[2], o_moc, o_R, o_el, o_ob, o_U, o_j3, per_warp_doubles;   // o_j3: chi3 [N][j3s], V3 [N][j3s], S3 [j3s] (systems with a J3)
     int dinv_rows[2];     // padded row count 8*NT
 };
 

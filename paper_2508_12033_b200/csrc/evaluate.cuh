@@ -8,12 +8,13 @@
 #include "listed.cuh"
 
 struct WarpState {            // per-warp views (shared memory; moc may live in global memory for large systems)
-    double *r, *dinv[2], *moc, *R, *cum, *el, *ob, *U;
+    double *r, *dinv[2], *moc, *R, *el, *ob, *U;
     double *j3;               // three-body Jastrow (systems that have one): chi3 [N][j3s] = chi_a(r_j), then V3 [N][j3s], then S3 [j3s]
     unsigned char *lw;        // listed sweep: this walker's listed-shell lists (listed.cuh: counts [n_lg][N], slots [N][lt])
     double *bc;               // listed sweep: this walker's Bc = C Dinv [N][n_aop] (global scratch of the resident warp / CTA, rank-1 updated)
 };
-struct EvalOut { double bbar, Vsf, W, eL; int node; };
+struct EvalOut { double bbar, Vsf, W, eL; int node;
+                 double c_loc, c_excl; };   // per LANE: sum of the allowed amplitudes of the lane's candidate chunk, and of the chunks before it (select_move)
 
 __device__ __forceinline__ int spin_of(const DevSys &S, int i) { return i < S.n_up ? 0 : 1; }
 
@@ -212,8 +213,8 @@ __device__ __forceinline__ int phase_b_with_nonlocal(const DevSys &S, const Warp
     const int nb0 = (S.n_up + 7) / 8, nbm = nb0 + (S.n_dn + 7) / 8, n_lat = S.n_mesh * nbm;
     // Slots in range of a centre are few (about 2.5 of 16 at C3): list them first (lane per slot, ballot), then sweep 8 LISTED
     // slots per pass.  With one coefficient table for both spins (same_C) a pass may mix spins (per-lane inverse, per-lane n_s);
-    // otherwise the list is cut at the first spin-down slot.  The list lives in the cumulative-sum array (free until phase C).
-    int *list = reinterpret_cast<int *>(ws.cum);
+    // otherwise the list is cut at the first spin-down slot.  The list (N K <= 4 N ints) lives in the s_k / old-column scratch of the hop (free during an evaluation).
+    int *list = reinterpret_cast<int *>(ws.el + 2 * N);
     int n_act = 0, n_act_up = 0;
     for (int s0 = 0; s0 < N * K; s0 += 32) {
         const int sl = s0 + lane; const bool in = sl < N * K;
@@ -320,6 +321,15 @@ __device__ __forceinline__ void move_target(const DevSys &S, const WarpState &ws
     }
 }
 
+// One term of the cumulative sums: the product kappa_j R_j is rounded before the add (reading Q12), in phase_c and in select_move alike.
+__device__ __forceinline__ double amp_add(double run, double kap, double Rj) { return __dadd_rn(run, __dmul_rn(kap, Rj)); }
+template <bool SLOTS>
+__device__ __forceinline__ double kappa_of(const DevSys &S, int j)
+{
+    return SLOTS ? (j < 6 * S.N ? S.kappa[0] : (j < S.P_lat ? S.kappa[1] : 1.0))   // non-local slots hold -nu_q rho_q itself
+                 : S.kappa[j >= 6 * S.N ? 1 : 0];
+}
+
 // Phase C (row a7) of one evaluation, by one warp on the candidate ratios R[P] left in shared memory.
 // node0: node flag already raised by the non-local candidates (rho_q < 0), any lane.
 template <bool SLOTS = false>
@@ -329,24 +339,23 @@ __device__ __forceinline__ EvalOut phase_c(const DevSys &S, const WarpState &ws,
     // ---- phase C (row a7): fixed-node split (Eq.D1) and the cumulative sums C_j of the allowed amplitudes in candidate
     //      order (row a9 searches them).  Each lane owns a contiguous chunk; chunk totals are scanned across the warp
     //      (reading Q12: the summation order is free, a draw closer than 1e-9 to a bin edge is a reported near-tie).
+    //      C_j = (sum over the lane's chunk up to j) + (sum of the chunks before): only the two per-lane numbers are kept
+    //      (EvalOut.c_loc / c_excl); select_move re-walks the one chunk that holds the selected move -- no C_j array.
     const int P = S.P, chunk = (P + 31) >> 5, j0 = lane * chunk;
     double vsf_part = 0.0, loc = 0.0; int node = node0;
     for (int e = 0; e < chunk; ++e) {
         const int j = j0 + e;
         if (j < P) {
             const double Rj = ws.R[j];
-            const double kap = SLOTS ? (j < 6 * N ? S.kappa[0] : (j < S.P_lat ? S.kappa[1] : 1.0))   // non-local slots hold -nu_q rho_q itself
-                                  : S.kappa[j >= 6 * N ? 1 : 0];
-            if (Rj > 0.0) loc += kap * Rj;
+            const double kap = kappa_of<SLOTS>(S, j);
+            if (Rj > 0.0) loc = amp_add(loc, kap, Rj);
             else if (Rj < 0.0) { vsf_part -= kap * Rj; if (!SLOTS || j < S.P_lat) node = 1; }
-            ws.cum[j] = loc;
         }
     }
     double inc = loc;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) { const double v = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += v; }
     double excl = __shfl_up_sync(0xffffffffu, inc, 1); if (lane == 0) excl = 0.0;
-    for (int e = 0; e < chunk; ++e) { const int j = j0 + e; if (j < P) ws.cum[j] += excl; }
     const double bbar = __shfl_sync(0xffffffffu, inc, 31);
     const double Vsf = warp_sum(vsf_part);
     node = __any_sync(0xffffffffu, node);
@@ -367,6 +376,7 @@ __device__ __forceinline__ EvalOut phase_c(const DevSys &S, const WarpState &ws,
     o.bbar = bbar; o.Vsf = Vsf; o.node = node;
     o.W = S.Kdiag + vsum + Vee + S.V_ii + Vsf;                        // L628 + kinetic diagonal of Eq.D5 (reading Q3)
     o.eL = o.W - bbar;                                                // L223
+    o.c_loc = loc; o.c_excl = excl;
     return o;
 }
 
@@ -491,19 +501,28 @@ __device__ __forceinline__ EvalOut evaluate_walker(const DevSys &S, const WarpSt
     return o;
 }
 
-// Heat-bath selection (Eq.29): j* = min{ j : C_j > u C_{P-1} } on the sequential cumulative sums left in ws.cum;
+// Heat-bath selection (Eq.29): j* = min{ j : C_j > u C_{P-1} } with C_j as phase_c defines them (e = the EvalOut of THIS warp's phase_c);
 // fallback = last allowed move; -1 if none is allowed.  All lanes return the same j*.
-__device__ __forceinline__ int select_move(const DevSys &S, const WarpState &ws, double u_sel, int lane)
+template <bool SLOTS = false>
+__device__ __forceinline__ int select_move(const DevSys &S, const WarpState &ws, const EvalOut &e, double u_sel, int lane)
 {
-    LRDMC_ASSUME_SHARED(ws.cum); LRDMC_ASSUME_SHARED(ws.R);
-    const int P = S.P;
-    const double tot = ws.cum[P - 1];
+    LRDMC_ASSUME_SHARED(ws.R);
+    const int P = S.P, chunk = (P + 31) >> 5, j0 = lane * chunk;
+    const double mine = e.c_loc + e.c_excl;                            // C_j of the last candidate of this lane's chunk
+    const double tot = __shfl_sync(0xffffffffu, mine, (P - 1) / chunk);  // C_{P-1}
     if (!(tot > 0.0)) return -1;
     const double thr = __dmul_rn(u_sel, tot);
-    for (int j0 = 0; j0 < P; j0 += 32) {
-        int j = j0 + lane;
-        unsigned hit = __ballot_sync(0xffffffffu, j < P && ws.cum[j] > thr);
-        if (hit) return j0 + __ffs(hit) - 1;
+    const unsigned hit = __ballot_sync(0xffffffffu, j0 < P && e.c_loc > 0.0 && mine > thr);   // (a chunk without an allowed move cannot hold j*)
+    if (hit) {                                                         // the first chunk whose last C_j passes holds j*: its lane walks it again
+        const int L = __ffs(hit) - 1; int js = -1;
+        if (lane == L) {
+            double run = 0.0;
+            for (int q = 0; q < chunk && js < 0; ++q) {
+                const int j = j0 + q;
+                if (j < P) { const double Rj = ws.R[j]; if (Rj > 0.0) { run = amp_add(run, kappa_of<SLOTS>(S, j), Rj); if (run + e.c_excl > thr) js = j; } }
+            }
+        }
+        return __shfl_sync(0xffffffffu, js, L);
     }
     int last = -1;                                                     // rounding left no C_j > thr: last j with q_j > 0
     for (int j = lane; j < P; j += 32) if (ws.R[j] > 0.0) last = j;

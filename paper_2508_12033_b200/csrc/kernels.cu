@@ -26,6 +26,16 @@
 #define KFN(name) name##_e4
 #endif
 static constexpr int kNL = LRDMC_EXT;
+// The extended warp-per-walker kernels exist twice: compiled for LRDMC_WPB warps per CTA (128 registers) and for LRDMC_WPB_EXT (168 registers, no spills);
+// a launch of at most LRDMC_WPB_EXT warps takes the second (systems whose per-walker state leaves room for 6 warps per CTA only).
+#if LRDMC_EXT >= 1 && LRDMC_EXT <= 3
+#define kWs LRDMC_WPB_EXT
+#define KSEL(threads, BIG, SMALL) do { if ((threads) <= 32 * LRDMC_WPB_EXT) { SMALL; } else { BIG; } } while (0)
+#define KBOTH(BIG, SMALL) do { BIG; SMALL; } while (0)
+#else
+#define KSEL(threads, BIG, SMALL) do { BIG; } while (0)
+#define KBOTH(BIG, SMALL) do { BIG; } while (0)
+#endif
 
 #define FOR_EACH_NT_TS(X) X(1, true) X(2, true) X(4, true) X(1, false) X(2, false) X(4, false)
 #define PICK(NT_, TS_, STMT)                                                                   \
@@ -37,15 +47,18 @@ static constexpr int kNL = LRDMC_EXT;
 #if !LRDMC_TEAM_TU
 void KFN(lrdmc_k_set_smem)(int smem)
 {
-#define X(NTV, TSV) cudaFuncSetAttribute(k_propagate<NTV, TSV, kNL>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); \
-                    cudaFuncSetAttribute(k_step_debug<NTV, TSV, kNL>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+#define X(NTV, TSV) KBOTH(cudaFuncSetAttribute(k_propagate<NTV, TSV, kNL>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); \
+                          cudaFuncSetAttribute(k_step_debug<NTV, TSV, kNL>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem), \
+                          cudaFuncSetAttribute(k_propagate<NTV, TSV, kNL, kWs>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); \
+                          cudaFuncSetAttribute(k_step_debug<NTV, TSV, kNL, kWs>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     FOR_EACH_NT_TS(X)
 #undef X
 }
 int KFN(lrdmc_k_occupancy)(int NT, int ts, int threads, int smem)
 {
     int occ = 0;
-#define STMT(NTV, TSV) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_propagate<NTV, TSV, kNL>, threads, smem)
+#define STMT(NTV, TSV) KSEL(threads, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_propagate<NTV, TSV, kNL>, threads, smem), \
+                            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_propagate<NTV, TSV, kNL, kWs>, threads, smem))
     PICK(NT, ts, STMT);
 #undef STMT
     return occ;
@@ -53,14 +66,16 @@ int KFN(lrdmc_k_occupancy)(int NT, int ts, int threads, int smem)
 void KFN(lrdmc_k_propagate)(int NT, int ts, int grid, int threads, int smem, cudaStream_t st, const DevSys &S, const DevWalk &W, int mode, int n_moves,
                             double tau, double E0, uint32_t cycle)
 {
-#define STMT(NTV, TSV) k_propagate<NTV, TSV, kNL><<<grid, threads, smem, st>>>(S, W, mode, n_moves, tau, E0, cycle)
+#define STMT(NTV, TSV) KSEL(threads, (k_propagate<NTV, TSV, kNL><<<grid, threads, smem, st>>>(S, W, mode, n_moves, tau, E0, cycle)), \
+                            (k_propagate<NTV, TSV, kNL, kWs><<<grid, threads, smem, st>>>(S, W, mode, n_moves, tau, E0, cycle)))
     PICK(NT, ts, STMT);
 #undef STMT
 }
 void KFN(lrdmc_k_step_debug)(int NT, int ts, int grid, int threads, int smem, cudaStream_t st, const DevSys &S, const DevWalk &W, double E0, uint32_t cycle,
                              uint32_t step, double *R_out, double *scal_out, int *jstar_out)
 {
-#define STMT(NTV, TSV) k_step_debug<NTV, TSV, kNL><<<grid, threads, smem, st>>>(S, W, E0, cycle, step, R_out, scal_out, jstar_out)
+#define STMT(NTV, TSV) KSEL(threads, (k_step_debug<NTV, TSV, kNL><<<grid, threads, smem, st>>>(S, W, E0, cycle, step, R_out, scal_out, jstar_out)), \
+                            (k_step_debug<NTV, TSV, kNL, kWs><<<grid, threads, smem, st>>>(S, W, E0, cycle, step, R_out, scal_out, jstar_out)))
     PICK(NT, ts, STMT);
 #undef STMT
 }

@@ -91,7 +91,6 @@ static int plan_smem(lrdmc_ctx *c)
     S.o_dinv[1] = (int)w; w += align_up((size_t)S.dinv_rows[1] * S.n_dn, 2);
     S.o_moc = (int)w; if (S.moc_in_smem) w += align_up(moc_doubles, 2);
     S.o_R = (int)w; w += align_up((size_t)S.P, 2);
-    S.o_cum = (int)w; w += align_up((size_t)S.P, 2);
     S.o_el = (int)w; w += align_up((size_t)LRDMC_EL_ARRAYS * S.N, 2);
     S.o_U = (int)w; w += 10;                    // the step's lattice frame (9 doubles)
     S.o_ob = (int)w; w += 8 * (size_t)S.N;      // one-body cache: J1, grad J1, lap J1, v_ei, v^a_ei per electron
@@ -99,7 +98,7 @@ static int plan_smem(lrdmc_ctx *c)
     S.o_am = (int)w; if (c->listed) w += ((size_t)S.N * (S.lt + S.n_lg) + 7) / 8;       // listed-shell lists (listed.cuh)
     S.per_warp_doubles = (int)w;
     const size_t per_sm = prop.sharedMemPerMultiprocessor, per_blk_max = prop.sharedMemPerBlockOptin, reserve = 1024;
-    c->wpb = (S.nl_K || S.n_j3) ? LRDMC_WPB_EXT : LRDMC_WPB;      // the extended kernels are compiled for LRDMC_WPB_EXT warps (propagate.cuh)
+    c->wpb = LRDMC_WPB;
     for (;;) {
         size_t need = ((size_t)S.tables_doubles + (size_t)c->wpb * S.per_warp_doubles) * 8;
         if ((need + reserve) * LRDMC_MINB <= per_sm || c->wpb == 1) { c->smem_bytes = (int)need; break; }

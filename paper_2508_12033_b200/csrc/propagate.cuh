@@ -45,7 +45,7 @@ __device__ __forceinline__ WarpState warp_views(const DevSys &S, double *smem, i
     double *base = smem + S.tables_doubles + (size_t)warp * S.per_warp_doubles;
     WarpState ws;
     ws.r = base + S.o_r; ws.dinv[0] = base + S.o_dinv[0]; ws.dinv[1] = base + S.o_dinv[1];
-    ws.moc = base + S.o_moc; ws.R = base + S.o_R; ws.cum = base + S.o_cum; ws.el = base + S.o_el; ws.ob = base + S.o_ob; ws.U = base + S.o_U; ws.j3 = base + S.o_j3;
+    ws.moc = base + S.o_moc; ws.R = base + S.o_R; ws.el = base + S.o_el; ws.ob = base + S.o_ob; ws.U = base + S.o_U; ws.j3 = base + S.o_j3;
     ws.lw = reinterpret_cast<unsigned char *>(base + S.o_am); ws.bc = nullptr;
     return ws;
 }
@@ -101,8 +101,9 @@ __device__ __forceinline__ void store_walker(const DevSys &S, const DevWalk &W, 
 }
 
 // ---- the projection kernel (Alg.2 lines 4-8 L401-L410 / Alg.1 lines 4-16 L350-L374) ----------------------------
-template <int NT, bool TS, int EXT>
-__global__ void __launch_bounds__(((EXT & 3) ? LRDMC_WPB_EXT : LRDMC_WPB) * 32, LRDMC_MINB) k_propagate(DevSys S, DevWalk W, int mode, int n_moves, double tau, double E0, uint32_t cycle)
+// WPBK: the warps per CTA the kernel is compiled for (launch bound; registers per thread = 65536 / (LRDMC_MINB 32 WPBK)).
+template <int NT, bool TS, int EXT, int WPBK = LRDMC_WPB>
+__global__ void __launch_bounds__(WPBK * 32, LRDMC_MINB) k_propagate(DevSys S, DevWalk W, int mode, int n_moves, double tau, double E0, uint32_t cycle)
 {
     extern __shared__ __align__(16) double smem[];
     stage_tables(S, smem);
@@ -154,7 +155,7 @@ __global__ void __launch_bounds__(((EXT & 3) ? LRDMC_WPB_EXT : LRDMC_WPB) * 32, 
             if (last) omega = w;
         }
         if (!last) {
-            const int j = select_move(S, ws, d.u_sel, lane);   // Alg.2 line 7 (L408)
+            const int j = select_move<(EXT & 1) != 0>(S, ws, e, d.u_sel, lane);   // Alg.2 line 7 (L408)
             if (j >= 0) { apply_move<NT, TS, EXT>(S, ws, T, j, lane); ++moves; }
             ++s;
             continue;
@@ -173,8 +174,8 @@ __global__ void __launch_bounds__(((EXT & 3) ? LRDMC_WPB_EXT : LRDMC_WPB) * 32, 
 }
 
 // ---- parity hook: one evaluation + selection, no state change ---------------------------------------------------
-template <int NT, bool TS, int EXT>
-__global__ void __launch_bounds__(((EXT & 3) ? LRDMC_WPB_EXT : LRDMC_WPB) * 32, LRDMC_MINB) k_step_debug(DevSys S, DevWalk W, double E0, uint32_t cycle, uint32_t step, double *R_out,
+template <int NT, bool TS, int EXT, int WPBK = LRDMC_WPB>
+__global__ void __launch_bounds__(WPBK * 32, LRDMC_MINB) k_step_debug(DevSys S, DevWalk W, double E0, uint32_t cycle, uint32_t step, double *R_out,
                                                     double *scal_out, int *jstar_out)
 {
     extern __shared__ __align__(16) double smem[];
@@ -188,7 +189,7 @@ __global__ void __launch_bounds__(((EXT & 3) ? LRDMC_WPB_EXT : LRDMC_WPB) * 32, 
         const StepDraws d = step_draws(S, (uint32_t)k, cycle, step, true);
         publish_frame(ws, d, lane);
         const EvalOut e = evaluate_walker<NT, TS, EXT>(S, ws, T, lane);
-        const int j = select_move(S, ws, d.u_sel, lane);
+        const int j = select_move<(EXT & 1) != 0>(S, ws, e, d.u_sel, lane);
         for (int p = lane; p < S.P; p += 32) R_out[(size_t)k * S.P + p] = ws.R[p];
         if (lane == 0) {
             double *o = scal_out + 8 * (size_t)k;
@@ -226,7 +227,7 @@ __global__ void __launch_bounds__(LRDMC_WPB * 32) k_rebuild(DevSys S, DevWalk W,
                 double *A = ws.dinv[sp];
                 for (int idx = lane; idx < ns * ns; idx += 32) { int i = idx / ns, m = idx - i * ns; A[idx] = ws.moc[(size_t)(off + i) * 5 * S.OS + m]; }
                 __syncwarp();
-                if (!warp_invert(A, ns, ns, reinterpret_cast<int *>(ws.cum), lane)) ok = false;
+                if (!warp_invert(A, ns, ns, reinterpret_cast<int *>(ws.el), lane)) ok = false;      // row permutation: n_s ints in the per-electron scratch (4 N doubles)
                 __syncwarp();
             }
             if (!ok) {       // reading Q24: a singular walker is dead (zero inverses, weight 0 in the next propagate) and counted

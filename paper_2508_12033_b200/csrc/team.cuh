@@ -56,7 +56,7 @@ __device__ __forceinline__ void team_step_frame(const DevSys &S, double *out, ui
     }
 }
 
-// One evaluation by the team.  The result is valid in warp 0 only (it runs phase C); ws.R / ws.cum are complete for everyone
+// One evaluation by the team.  The result is valid in warp 0 only (it runs phase C); ws.R is complete for everyone
 // after the caller's next barrier.  s_vee: TW doubles of static shared memory.
 // BCS: parked Bc entries (wavefunction.cuh, ao_columns): bcs_cta = this CTA's scratch [block of a mesh][k-step pair][lane];
 // reuse_spin = the spin that did not hop since the last evaluation (-1: none).  A unit's entries are parked and taken back by the
@@ -113,8 +113,8 @@ __device__ __forceinline__ EvalOut evaluate_team(const DevSys &S, const TeamPlan
         vee_part = warp_sum(vee_part);
         if (lane == 0) s_vee[wt] = vee_part;
     }
-    if (NL && wt == TW - 1) {        // list the slots in range of a centre (ballot), clear the others; list in ws.cum (free until phase C)
-        int *lst = reinterpret_cast<int *>(ws.cum);
+    if (NL && wt == TW - 1) {        // list the slots in range of a centre (ballot), clear the others; list in the hop's s_k / old-column scratch (free during an evaluation)
+        int *lst = reinterpret_cast<int *>(ws.el + 2 * N);
         const int Kk = S.nl_K; int na = 0, nup = 0;
         for (int s0 = 0; s0 < N * Kk; s0 += 32) {
             const int sl = s0 + lane; const bool in = sl < N * Kk;
@@ -153,7 +153,7 @@ __device__ __forceinline__ EvalOut evaluate_team(const DevSys &S, const TeamPlan
     // ---- phase B (rows a1-a5, f1): work units (mesh, spin, 8-electron block, shell part) and, with non-local slots, (pass of 8
     //      LISTED slots, shell part); unit v -> warp v mod TW.  One loop, one ao_columns call site for both kinds.
     const int nb_mesh = P.nblk[0] + P.nblk[1], K = S.nl_K;
-    const int *list = reinterpret_cast<const int *>(ws.cum);
+    const int *list = reinterpret_cast<const int *>(ws.el + 2 * N);
     const int n_act = NL ? s_node[1] : 0, cut = NL ? s_node[2] : 0, n_p0 = (cut + 7) / 8, n_nlp = n_p0 + (n_act - cut + 7) / 8;
     for (int v = wt; v < P.n_units + n_nlp * NP; v += TW) {
         const bool is_nl = NL && v >= P.n_units;
@@ -392,7 +392,7 @@ __global__ void __launch_bounds__(LRDMC_TEAM_MAX_WARPS * 32, 1) k_propagate_team
                     if (last) omega = w;
                 }
                 int j = -1;
-                if (!last) j = select_move(S, ws, d.u_sel, lane);      // Alg.2 line 7 (L408)
+                if (!last) j = select_move<(EXT & 1) != 0>(S, ws, e, d.u_sel, lane);      // Alg.2 line 7 (L408)
                 else { eL_last = e.eL; W_last = e.W; }
                 if (lane == 0) { s_ctrl[1] = last ? 1 : 0; s_ctrl[2] = j; }
             }
