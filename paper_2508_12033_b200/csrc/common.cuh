@@ -22,6 +22,9 @@
 #ifndef LRDMC_BC_STORE
 #define LRDMC_BC_STORE 1         // Bc kept between evaluations: listed sweep (listed.cuh), or parked entries of the dense sweep of the large systems (ao_columns BCS)
 #endif
+// Systems with a three-body Jastrow keep the fragment table `bf` of the mover's derivative pass (12.8 KB at 200 AOs, read once per move, the same for every
+// walker: L1-resident) in global memory, so that their larger per-walker state still leaves room for 8 warps per CTA.  EXT is the kernels' feature mask.
+#define LRDMC_BF_SMEM(TS, EXT) ((TS) && !((EXT) & 2))
 #define LRDMC_NUC_STRIDE 20  // doubles per nucleus row: Rx Ry Rz Z c1 b1 alpha beta gamma delta is_pp pad | r_c A0 B0 A1 B1 A2 B2 pad (non-local channels)
 #define LRDMC_NL_OFF 12      // first non-local entry of a nucleus row
 #define LRDMC_NL_MAX_K 4
@@ -68,6 +71,7 @@ struct DevSys {
     const double *cn[2];       // [n_aop][OS] MO coefficients with the AO norms folded in, slot-major (Bc = C Dinv by rows)
     // shared-memory plan (units: doubles)
     int bf_in_smem, moc_in_smem, cf_in_smem;   // cf_in_smem: the pair table of ao_columns is staged too (not with the listed sweep)
+    int bfm_in_smem;                           // the fragment table `bf` of the mover's derivative pass is staged too (LRDMC_BF_SMEM: not with a three-body Jastrow)
     int off_shells, off_nuc, off_bf[2], off_etab, tables_doubles;
     int o_r, o_dinv[2], o_moc, o_R, o_el, o_ob, o_U, o_j3, per_warp_doubles;   // o_j3: chi3 [N][j3s], V3 [N][j3s], S3 [j3s] (systems with a J3)
     int dinv_rows[2];     // padded row count 8*NT

@@ -540,7 +540,7 @@ __device__ __forceinline__ void apply_move(const DevSys &S, const WarpState &ws,
     const int sp = spin_of(S, i), il = sp ? i - S.n_up : i, ns = sp ? S.n_dn : S.n_up;
     double *mc = ws.moc + (size_t)i * 5 * S.OS;
     __syncwarp();
-    refresh_mo_cache<NT, TS>(S, T.shells, sp ? T.bf[1] : T.bf[0], T.etab, mc, px, py, pz, lane);
+    refresh_mo_cache<NT, LRDMC_BF_SMEM(TS, EXT)>(S, T.shells, sp ? T.bf[1] : T.bf[0], T.etab, mc, px, py, pz, lane);
     refresh_onebody(S.n_nuc, S.has_j1, S.a, T.nuc, ws.ob + 8 * i, px, py, pz, lane);
     if (EXT & 2) refresh_j3_row(S, T.nuc, ws.j3 + i * S.j3s, px, py, pz, lane);
     if (EXT & 4) list_build(S, T.shells, T.srad, ws.lw, i, px, py, pz, fmax(S.amesh[0], S.amesh[1]), lane);   // the mover's listed shells at its new position

@@ -70,7 +70,7 @@ static int plan_smem(lrdmc_ctx *c)
     const size_t bf_doubles = (bf_n + cf_n) * (S.same_C ? 1 : 2);
     const size_t moc_doubles = (size_t)S.N * 5 * S.OS;
     const bool fits = bf_doubles * 8 <= 64 * 1024 && moc_doubles * 8 <= 12 * 1024 && !c->opt_global_tables;
-    S.bf_in_smem = fits; S.moc_in_smem = fits;
+    S.bf_in_smem = fits; S.moc_in_smem = fits; S.bfm_in_smem = fits && !S.n_j3;     // LRDMC_BF_SMEM (common.cuh)
     size_t o = 0;
     S.off_etab = (int)o; o += 256;              // always first: exp_tab addresses it as (dynamic smem base) + 8 j
     S.off_shells = (int)o; o += align_up(c->n_sh, 2);
@@ -79,8 +79,8 @@ static int plan_smem(lrdmc_ctx *c)
     S.off_j3g = (int)o; o += (size_t)S.j3s * S.j3s;
     // listed sweep (EXT = 4): lattice-only systems; automatic = the systems whose tables live in global memory (64 electrons, 600 AOs)
     c->listed = !S.nl_K && !S.n_j3 && LRDMC_BC_STORE && (c->opt_listed < 0 ? !fits : c->opt_listed != 0);
-    S.off_bf[0] = (int)o; if (S.bf_in_smem) o += bf_n;
-    S.off_bf[1] = (int)o; if (S.bf_in_smem && !S.same_C) o += bf_n;
+    S.off_bf[0] = (int)o; if (S.bfm_in_smem) o += bf_n;
+    S.off_bf[1] = (int)o; if (S.bfm_in_smem && !S.same_C) o += bf_n;
     S.cf_in_smem = S.bf_in_smem && !c->listed;
     S.off_cf[0] = (int)o; if (S.bf_in_smem && !c->listed) o += cf_n;            // the pair table of ao_columns is not used by the listed sweep
     S.off_cf[1] = (int)o; if (S.bf_in_smem && !S.same_C && !c->listed) o += cf_n;
@@ -109,8 +109,9 @@ static int plan_smem(lrdmc_ctx *c)
     if (c->wpb == 7 || c->wpb == 5) { --c->wpb; c->smem_bytes = (int)(((size_t)S.tables_doubles + (size_t)c->wpb * S.per_warp_doubles) * 8); }
     if ((size_t)c->smem_bytes > per_blk_max) return LRDMC_ENOMEM;
 #define SET_SMEM(K) CK(cudaFuncSetAttribute(K, cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem_bytes))
-#define SET_ALL(NTV, TSV) SET_SMEM((k_rebuild<NTV, TSV, false>))
-    SET_ALL(1, true); SET_ALL(2, true); SET_ALL(4, true); SET_ALL(1, false); SET_ALL(2, false); SET_ALL(4, false);
+#define SET_ALL(NTV, TSV, BFV) SET_SMEM((k_rebuild<NTV, TSV, BFV>))
+    SET_ALL(1, true, true); SET_ALL(2, true, true); SET_ALL(4, true, true); SET_ALL(1, true, false); SET_ALL(2, true, false); SET_ALL(4, true, false);
+    SET_ALL(1, false, false); SET_ALL(2, false, false); SET_ALL(4, false, false);
 #undef SET_ALL
 #undef SET_SMEM
     c->ts = S.bf_in_smem && S.moc_in_smem;
@@ -530,7 +531,8 @@ static int rebuild(lrdmc_ctx *c, int do_invert /* bit 0: invert, bit 1: the MO c
     CK(cudaMemsetAsync(c->W.counter, 0, 64 * sizeof(int), st));
     if (do_invert & 1) CK(cudaMemsetAsync(c->W.n_sing, 0, sizeof(long long), st));
     else CK(cudaMemsetAsync(c->W.dead, 0, sizeof(int) * (size_t)c->W.n_w, st));     // inverses supplied by the caller: nobody is dead
-    DISPATCH_NL_(k_rebuild, false, grid_for(c), st, c->S, c->W, do_invert);
+    if (c->S.bfm_in_smem) DISPATCH_NL_(k_rebuild, true, grid_for(c), st, c->S, c->W, do_invert);      // third argument: LRDMC_BF_SMEM
+    else DISPATCH_NL_(k_rebuild, false, grid_for(c), st, c->S, c->W, do_invert);
     CK(cudaGetLastError());
     return LRDMC_OK;
 }

@@ -12,7 +12,7 @@ __device__ __forceinline__ void stage_tables(const DevSys &S, double *smem)
     for (int i = threadIdx.x; i < S.n_slots; i += blockDim.x) smem[S.off_srad + i] = S.srad[i];
     for (int i = threadIdx.x; i < S.j3s * S.j3s; i += blockDim.x) smem[S.off_j3g + i] = S.j3g[i];
     if (S.bf_in_smem) {
-        const int nb = S.n_ksteps * S.NT[0] * 32;
+        const int nb = S.bfm_in_smem ? S.n_ksteps * S.NT[0] * 32 : 0;
         for (int i = threadIdx.x; i < nb; i += blockDim.x) smem[S.off_bf[0] + i] = S.bfrag[0][i];
         if (!S.same_C && S.n_dn > 0) for (int i = threadIdx.x; i < nb; i += blockDim.x) smem[S.off_bf[1] + i] = S.bfrag[1][i];
         const int nc = S.cf_in_smem ? S.n_kpairs * 2 * S.NT[0] * 32 : 0;
@@ -25,18 +25,16 @@ __device__ __forceinline__ void stage_tables(const DevSys &S, double *smem)
 
 // TS (tables + MO cache in shared memory): every pointer below is "shared base + offset" with no global alternative, so the
 // compiler's address-space inference emits LDS/STS.  !TS (64-electron config): fragments / cache stay in global memory.
-template <bool TS>
+// BFS: the derivative-pass fragments `bf` are in shared memory (LRDMC_BF_SMEM), else global.
+template <bool TS, bool BFS = TS>
 __device__ __forceinline__ Tables table_pointers(const DevSys &S, const double *smem)
 {
     Tables T;
     T.shells = smem + S.off_shells; T.nuc = smem + S.off_nuc; T.etab = smem; T.srad = smem + S.off_srad; T.j3g = smem + S.off_j3g;
-    if (TS) {
-        T.bf[0] = smem + S.off_bf[0]; T.bf[1] = smem + (S.same_C ? S.off_bf[0] : S.off_bf[1]);
-        T.cf[0] = smem + S.off_cf[0]; T.cf[1] = smem + (S.same_C ? S.off_cf[0] : S.off_cf[1]);
-    } else {                                       // global memory only: a single provenance per pointer (see lrdmc_init)
-        T.bf[0] = S.bfrag[0]; T.bf[1] = S.bfrag[1];
-        T.cf[0] = S.cfrag[0]; T.cf[1] = S.cfrag[1];
-    }
+    if (BFS) { T.bf[0] = smem + S.off_bf[0]; T.bf[1] = smem + (S.same_C ? S.off_bf[0] : S.off_bf[1]); }
+    else { T.bf[0] = S.bfrag[0]; T.bf[1] = S.bfrag[1]; }        // global memory only: a single provenance per pointer (see lrdmc_init)
+    if (TS) { T.cf[0] = smem + S.off_cf[0]; T.cf[1] = smem + (S.same_C ? S.off_cf[0] : S.off_cf[1]); }
+    else { T.cf[0] = S.cfrag[0]; T.cf[1] = S.cfrag[1]; }
     return T;
 }
 
@@ -108,7 +106,7 @@ __global__ void __launch_bounds__(WPBK * 32, LRDMC_MINB) k_propagate(DevSys S, D
     extern __shared__ __align__(16) double smem[];
     stage_tables(S, smem);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, gwarp = blockIdx.x * (blockDim.x >> 5) + warp;
-    const Tables T = table_pointers<TS>(S, smem);
+    const Tables T = table_pointers<TS, LRDMC_BF_SMEM(TS, EXT)>(S, smem);
     WarpState ws = warp_views(S, smem, warp);
     if (EXT & 4) ws.bc = W.bcs + (size_t)gwarp * W.bcs_stride;
     const unsigned long long t_start = globaltimer_ns();
@@ -181,7 +179,7 @@ __global__ void __launch_bounds__(WPBK * 32, LRDMC_MINB) k_step_debug(DevSys S, 
     extern __shared__ __align__(16) double smem[];
     stage_tables(S, smem);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, wpb = blockDim.x >> 5;
-    const Tables T = table_pointers<TS>(S, smem);
+    const Tables T = table_pointers<TS, LRDMC_BF_SMEM(TS, EXT)>(S, smem);
     WarpState ws = warp_views(S, smem, warp);
     for (int k = blockIdx.x * wpb + warp; k < W.n_w; k += gridDim.x * wpb) {
         if (EXT & 4) ws.bc = W.bcs + (size_t)(blockIdx.x * wpb + warp) * W.bcs_stride;
@@ -203,20 +201,20 @@ __global__ void __launch_bounds__(WPBK * 32, LRDMC_MINB) k_step_debug(DevSys S, 
 }
 
 // ---- (re)build of the inverses and MO caches from the positions (row a13) ---------------------------------------
-template <int NT, bool TS, bool NL_UNUSED>
+template <int NT, bool TS, bool BFS>
 __global__ void __launch_bounds__(LRDMC_WPB * 32) k_rebuild(DevSys S, DevWalk W, int do_invert)
 {
     extern __shared__ __align__(16) double smem[];
     stage_tables(S, smem);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, wpb = blockDim.x >> 5;
-    const Tables T = table_pointers<TS>(S, smem);
+    const Tables T = table_pointers<TS, BFS>(S, smem);
     WarpState ws = warp_views(S, smem, warp);
     const int N = S.N;
     for (int k = blockIdx.x * wpb + warp; k < W.n_w; k += gridDim.x * wpb) {
         load_walker<TS>(S, W, ws, T, k, lane, !(do_invert & 1), false);
         if (!(do_invert & 2)) for (int i = 0; i < N; ++i) {
             const int sp = spin_of(S, i);
-            refresh_mo_cache<NT, TS>(S, T.shells, T.bf[sp], T.etab, ws.moc + (size_t)i * 5 * S.OS, ws.r[3 * i], ws.r[3 * i + 1], ws.r[3 * i + 2], lane);
+            refresh_mo_cache<NT, BFS>(S, T.shells, T.bf[sp], T.etab, ws.moc + (size_t)i * 5 * S.OS, ws.r[3 * i], ws.r[3 * i + 1], ws.r[3 * i + 2], lane);
         }
         __syncwarp();
         if (do_invert & 1) {

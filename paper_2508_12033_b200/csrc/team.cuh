@@ -286,7 +286,7 @@ __device__ __forceinline__ void apply_move_team(const DevSys &S, const TeamPlan 
     const int rows = 5 * S.OS;
     {
         double acc[NT][2];
-        mo_pass<NT, true, TS, true>(S, T.shells, sp ? T.bf[1] : T.bf[0], T.etab, px, py, pz, lane, acc, &P, &P.mo[wt]);
+        mo_pass<NT, true, LRDMC_BF_SMEM(TS, EXT), true>(S, T.shells, sp ? T.bf[1] : T.bf[0], T.etab, px, py, pz, lane, acc, &P, &P.mo[wt]);
         const int t = lane & 3, g = lane >> 2;
         if (g < 5) {
             double *q = scr + (size_t)wt * rows + g * S.OS;
@@ -332,7 +332,7 @@ __global__ void __launch_bounds__(LRDMC_TEAM_MAX_WARPS * 32, 1) k_propagate_team
     __shared__ int s_ctrl[8];      // [0] walker, [1] last, [2] selected move, [3] node flag of the slots, [4] listed slots, [5] spin cut of the list
     stage_tables(S, smem);
     const int tid = threadIdx.x, lane = tid & 31, wt = tid >> 5;
-    const Tables T = table_pointers<TS>(S, smem);
+    const Tables T = table_pointers<TS, LRDMC_BF_SMEM(TS, EXT)>(S, smem);
     WarpState ws = warp_views(S, smem, 0);
     double *scr = smem + S.tables_doubles + P.o_scr;
     constexpr bool LISTED = (EXT & 4) != 0;                     // listed sweep on stored, rank-1-updated Bc
