@@ -28,26 +28,31 @@ __device__ __forceinline__ void dmma884(double &c0, double &c1, double a, double
     asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
 }
 
-// per-axis monomial v^k and its first / second derivative including the Gaussian factor's contribution:
-//   d/dv [v^k e^{-z v^2}] = (k v^{k-1} - 2 z v^{k+1}) e ,  d2/dv2 = (k(k-1) v^{k-2} - 2 z (2k+1) v^k + 4 z^2 v^{k+2}) e
-struct AxisPoly { double f[3], f1[3], f2[3]; };
-__device__ __forceinline__ AxisPoly axis_poly(double v, double z)
+// Derivative pass: the 8 mma rows of a lane group g = lane / 4 are 8 COMPONENTS of the cartesian primitive x^l y^m z^n e^{-z r^2} at ONE point:
+//   g = 0 value, 1..3 d/dx, d/dy, d/dz, 4..6 d2/dx2, d2/dy2, d2/dz2 (their sum is the Laplacian: mo_pass adds rows 5 and 6 to row 4 at the end), 7 zero.
+// Every row is ONE product of per-axis factors: the plain monomial v^k on two axes and, on the lane's SPECIAL axis, its first or second
+// derivative with the Gaussian's contribution,
+//   d/dv [v^k e^{-z v^2}] = (k v^{k-1} - 2 z v^{k+1}) e ,  d2/dv2 = (k(k-1) v^{k-2} - 2 z (2k+1) v^k + 4 z^2 v^{k+2}) e .
+// So a lane selects its three factor arrays once per shell and spends two multiplications per AO component -- no per-component selects, and the
+// three second derivatives are formed by the otherwise idle rows 4-6 instead of by every lane (round 2: 1.58 k -> 1.0 k instructions per move).
+struct DerivSel { int axis, fam; double on; };      // special axis (0 x, 1 y, 2 z; -1 none), family 1 / 2 (first / second derivative), 0 for the zero row
+__device__ __forceinline__ DerivSel deriv_sel(int g)
 {
-    AxisPoly p; double v2 = v * v, tz = 2.0 * z, fz2 = 4.0 * z * z;
-    p.f[0] = 1.0; p.f[1] = v; p.f[2] = v2;
-    p.f1[0] = -tz * v;            p.f1[1] = 1.0 - tz * v2;              p.f1[2] = 2.0 * v - tz * v2 * v;
-    p.f2[0] = -tz + fz2 * v2;     p.f2[1] = (-3.0 * tz + fz2 * v2) * v; p.f2[2] = 2.0 - 5.0 * tz * v2 + fz2 * v2 * v2;
-    return p;
+    DerivSel d; d.axis = (g >= 1 && g <= 6) ? (g - 1) % 3 : -1; d.fam = g <= 3 ? 1 : 2; d.on = g == 7 ? 0.0 : 1.0;
+    return d;
 }
-// component g of the cartesian primitive x^l y^m z^n e:  g = 0 value, 1..3 gradient, 4 Laplacian, >4 zero
-template <int L, int M, int N>
-__device__ __forceinline__ double gto_component(int g, const AxisPoly &X, const AxisPoly &Y, const AxisPoly &Z, double e)
+template <int KMAX>
+__device__ __forceinline__ void deriv_axes(const DerivSel &q, double dx, double dy, double dz, double z, double (&ax)[KMAX + 1], double (&ay)[KMAX + 1],
+                                           double (&az)[KMAX + 1])
 {
-    double fx = (g == 1) ? X.f1[L] : X.f[L], fy = (g == 2) ? Y.f1[M] : Y.f[M], fz = (g == 3) ? Z.f1[N] : Z.f[N];
-    double v = fx * fy * fz;
-    double lap = X.f2[L] * Y.f[M] * Z.f[N] + X.f[L] * Y.f2[M] * Z.f[N] + X.f[L] * Y.f[M] * Z.f2[N];
-    v = (g == 4) ? lap : v;
-    return (g > 4) ? 0.0 : v * e;
+    const double u = q.axis == 1 ? dy : (q.axis == 2 ? dz : dx), u2 = u * u, tz = 2.0 * z, fz2 = tz * tz;
+    double sp[KMAX + 1], fx[KMAX + 1], fy[KMAX + 1], fz[KMAX + 1];
+    sp[0] = q.fam == 1 ? -tz * u : fma(fz2, u2, -tz);
+    fx[0] = 1.0; fy[0] = 1.0; fz[0] = 1.0;
+    if (KMAX >= 1) { sp[1] = q.fam == 1 ? fma(-tz, u2, 1.0) : fma(fz2, u2, -3.0 * tz) * u; fx[1] = dx; fy[1] = dy; fz[1] = dz; }
+    if (KMAX >= 2) { sp[2] = q.fam == 1 ? u * fma(-tz, u2, 2.0) : fma(u2, fma(fz2, u2, -5.0 * tz), 2.0); fx[2] = dx * dx; fy[2] = dy * dy; fz[2] = dz * dz; }
+#pragma unroll
+    for (int k = 0; k <= KMAX; ++k) { ax[k] = q.axis == 0 ? sp[k] : fx[k]; ay[k] = q.axis == 1 ? sp[k] : fy[k]; az[k] = q.axis == 2 ? sp[k] : fz[k]; }
 }
 
 // One pass over the whole (sorted, padded) shell list for the 8 points held by the warp.
@@ -63,6 +68,7 @@ __device__ __forceinline__ void mo_pass(const DevSys &S, const double *__restric
     const int n_ = PART ? part->hi[G] : S.n_it[G]; int it = PART ? part->lo[G] : 0;             \
     if (PART) { sh4 = reinterpret_cast<const double4 *>(shells) + t + 4 * (tp->it_base[G] + it); b = bf + lane + (size_t)(tp->kstep_base[G] + NC * it) * NT * 32; }
     const int t = lane & 3, g = lane >> 2;
+    const DerivSel dq = deriv_sel(g);
     const double4 *sh4 = reinterpret_cast<const double4 *>(shells) + t;
     const double *b = bf + lane;
 #pragma unroll
@@ -89,7 +95,7 @@ __device__ __forceinline__ void mo_pass(const DevSys &S, const double *__restric
         double4 s = *sh4; double dx = px - s.x, dy = py - s.y, dz = pz - s.z, z = s.w;
         double e = exp_tab(exp_arg_floor(-z * (dx * dx + dy * dy + dz * dz)), etab);
         if (!DERIV) { LRDMC_FEED(e); }
-        else { AxisPoly X = axis_poly(dx, z), Y = axis_poly(dy, z), Z = axis_poly(dz, z); LRDMC_FEED((gto_component<0, 0, 0>(g, X, Y, Z, e))); }
+        else { double ax[1], ay[1], az[1]; deriv_axes<0>(dq, dx, dy, dz, z, ax, ay, az); LRDMC_FEED(ax[0] * ay[0] * (az[0] * (e * dq.on))); }
     } }
     // ---- group 2: p Gaussians (x, y, z)
     { LRDMC_MO_RANGE(2, 3) for (; it < n_; ++it, sh4 += 4) {
@@ -97,9 +103,9 @@ __device__ __forceinline__ void mo_pass(const DevSys &S, const double *__restric
         double e = exp_tab(exp_arg_floor(-z * (dx * dx + dy * dy + dz * dz)), etab);
         if (!DERIV) { LRDMC_FEED(dx * e); LRDMC_FEED(dy * e); LRDMC_FEED(dz * e); }
         else {
-            AxisPoly X = axis_poly(dx, z), Y = axis_poly(dy, z), Z = axis_poly(dz, z);
-            LRDMC_FEED((gto_component<1, 0, 0>(g, X, Y, Z, e))); LRDMC_FEED((gto_component<0, 1, 0>(g, X, Y, Z, e)));
-            LRDMC_FEED((gto_component<0, 0, 1>(g, X, Y, Z, e)));
+            double ax[2], ay[2], az[2]; deriv_axes<1>(dq, dx, dy, dz, z, ax, ay, az);
+            const double eo = e * dq.on, yz = ay[0] * az[0] * eo;
+            LRDMC_FEED(ax[1] * yz); LRDMC_FEED(ax[0] * (ay[1] * (az[0] * eo))); LRDMC_FEED(ax[0] * (ay[0] * (az[1] * eo)));
         }
     } }
     // ---- group 3: d Gaussians (xx, xy, xz, yy, yz, zz)
@@ -110,12 +116,22 @@ __device__ __forceinline__ void mo_pass(const DevSys &S, const double *__restric
             double xe = dx * e, ye = dy * e, ze = dz * e;
             LRDMC_FEED(dx * xe); LRDMC_FEED(dx * ye); LRDMC_FEED(dx * ze); LRDMC_FEED(dy * ye); LRDMC_FEED(dy * ze); LRDMC_FEED(dz * ze);
         } else {
-            AxisPoly X = axis_poly(dx, z), Y = axis_poly(dy, z), Z = axis_poly(dz, z);
-            LRDMC_FEED((gto_component<2, 0, 0>(g, X, Y, Z, e))); LRDMC_FEED((gto_component<1, 1, 0>(g, X, Y, Z, e)));
-            LRDMC_FEED((gto_component<1, 0, 1>(g, X, Y, Z, e))); LRDMC_FEED((gto_component<0, 2, 0>(g, X, Y, Z, e)));
-            LRDMC_FEED((gto_component<0, 1, 1>(g, X, Y, Z, e))); LRDMC_FEED((gto_component<0, 0, 2>(g, X, Y, Z, e)));
+            double ax[3], ay[3], az[3]; deriv_axes<2>(dq, dx, dy, dz, z, ax, ay, az);
+            const double eo = e * dq.on, x0 = ax[0] * eo, x1 = ax[1] * eo;
+            LRDMC_FEED(ax[2] * eo * (ay[0] * az[0])); LRDMC_FEED(x1 * (ay[1] * az[0])); LRDMC_FEED(x1 * (ay[0] * az[1]));
+            LRDMC_FEED(x0 * (ay[2] * az[0])); LRDMC_FEED(x0 * (ay[1] * az[1])); LRDMC_FEED(x0 * (ay[0] * az[2]));
         }
     } }
+    if (DERIV) {                          // rows 4, 5, 6 hold the three second derivatives: their sum, the Laplacian, goes to row 4
+#pragma unroll
+        for (int nt = 0; nt < NT; ++nt) {
+#pragma unroll
+            for (int c = 0; c < 2; ++c) {
+                const double s2 = __shfl_down_sync(0xffffffffu, acc[nt][c], 4) + __shfl_down_sync(0xffffffffu, acc[nt][c], 8);
+                if (g == 4) acc[nt][c] += s2;
+            }
+        }
+    }
 #undef LRDMC_MO_RANGE
 #undef LRDMC_FEED
 }
