@@ -92,7 +92,7 @@ static int plan_smem(lrdmc_ctx *c)
     S.o_moc = (int)w; if (S.moc_in_smem) w += align_up(moc_doubles, 2);
     S.o_R = (int)w; w += align_up((size_t)S.P, 2);
     S.o_el = (int)w; w += align_up((size_t)LRDMC_EL_ARRAYS * S.N, 2);
-    S.o_U = (int)w; w += 10;                    // the step's lattice frame (9 doubles)
+    S.o_U = (int)w; w += LRDMC_FRAME_BATCH * LRDMC_FRAME_STRIDE;   // prepared draws + lattice frames of LRDMC_FRAME_BATCH steps (propagate.cuh)
     S.o_ob = (int)w; w += 8 * (size_t)S.N;      // one-body cache: J1, grad J1, lap J1, v_ei, v^a_ei per electron
     S.o_j3 = (int)w; if (S.n_j3) w += (size_t)S.N * 2 * S.j3s + S.j3s;   // three-body Jastrow: chi3, V3, S3
     S.o_am = (int)w; if (c->listed) w += ((size_t)S.N * (S.lt + S.n_lg) + 7) / 8;       // listed-shell lists (listed.cuh)

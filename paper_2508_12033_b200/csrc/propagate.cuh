@@ -58,6 +58,23 @@ __device__ __forceinline__ void publish_frame(const WarpState &ws, const StepDra
     __syncwarp();
 }
 
+// The draws and frames of the steps s0 .. s0 + LRDMC_FRAME_BATCH - 1 of walker `slot`, one LANE per step (they depend on (slot, cycle, step) alone): the
+// Philox rounds and the frame's sincos / sqrt sequences are warp instructions whichever lanes need them, so preparing four steps costs what one did.
+// fr = the warp's frame buffer [LRDMC_FRAME_BATCH][LRDMC_FRAME_STRIDE].
+__device__ __forceinline__ void prepare_frames(const DevSys &S, double *fr, uint32_t slot, uint32_t cycle, uint32_t s0, bool need_tau, int lane)
+{
+    __syncwarp();
+    const StepDraws d = step_draws(S, slot, cycle, s0 + (lane < LRDMC_FRAME_BATCH ? lane : 0), need_tau);
+    if (lane < LRDMC_FRAME_BATCH) {
+        double U[9]; lattice_frame(d.u1, d.u2, d.u3, U);
+        double *o = fr + lane * LRDMC_FRAME_STRIDE;
+#pragma unroll
+        for (int i = 0; i < 9; ++i) o[i] = U[i];
+        o[10] = d.u_sel; o[11] = d.u_tau;
+    }
+    __syncwarp();
+}
+
 // LISTED (EXT bit 2): also the shell lists of every electron and Bc = C Dinv of this walker in the warp's global scratch ws.bc.
 template <bool TS, bool LISTED = false>
 __device__ __forceinline__ void load_walker(const DevSys &S, const DevWalk &W, WarpState &ws, const Tables &T, int k, int lane, bool with_dinv, bool with_onebody = true)
@@ -109,6 +126,7 @@ __global__ void __launch_bounds__(WPBK * 32, LRDMC_MINB) k_propagate(DevSys S, D
     const Tables T = table_pointers<TS, LRDMC_BF_SMEM(TS, EXT)>(S, smem);
     WarpState ws = warp_views(S, smem, warp);
     if (EXT & 4) ws.bc = W.bcs + (size_t)gwarp * W.bcs_stride;
+    double *const frames = ws.U;             // [LRDMC_FRAME_BATCH][LRDMC_FRAME_STRIDE]; ws.U points at the current step's frame
     const unsigned long long t_start = globaltimer_ns();
     // The warps of a CTA meet at a barrier once per step, whatever walker and step index each of them is at: they then run
     // the same code region at the same time and share the small instruction caches (L0 6 KB, L1.5 32 KB against 140 KB of
@@ -133,8 +151,9 @@ __global__ void __launch_bounds__(WPBK * 32, LRDMC_MINB) k_propagate(DevSys S, D
         }
         if (LRDMC_LOCKSTEP) { if (!__syncthreads_or(have)) break; if (!have) continue; }
         else if (!have) break;
-        const StepDraws d = step_draws(S, (uint32_t)k, cycle, s, mode == LRDMC_CONVENTIONAL);
-        publish_frame(ws, d, lane);
+        if ((s & (LRDMC_FRAME_BATCH - 1)) == 0) prepare_frames(S, frames, (uint32_t)k, cycle, s, mode == LRDMC_CONVENTIONAL, lane);
+        ws.U = frames + (s & (LRDMC_FRAME_BATCH - 1)) * LRDMC_FRAME_STRIDE;
+        StepDraws d; d.u_sel = ws.U[10]; d.u_tau = ws.U[11];
         const EvalOut e = evaluate_walker<NT, TS, EXT>(S, ws, T, lane);
         n_node += e.node;
         bool last = false; double omega = 0.0;
