@@ -25,7 +25,8 @@
 // Systems with a three-body Jastrow keep the fragment table `bf` of the mover's derivative pass (12.8 KB at 200 AOs, read once per move, the same for every
 // walker: L1-resident) in global memory, so that their larger per-walker state still leaves room for 8 warps per CTA.  EXT is the kernels' feature mask.
 #define LRDMC_BF_SMEM(TS, EXT) ((TS) && !((EXT) & 2))
-#define LRDMC_FRAME_BATCH 4    // warp-per-walker kernel: the draws and lattice frames of this many consecutive steps are prepared at once, one lane per step
+#define LRDMC_FRAME_BATCH 4    // warp-per-walker kernel: the draws and lattice frames of up to this many consecutive steps are prepared at once, one lane per step
+                               // (DevSys.frame_batch = 4, 2 or 1: the largest that costs no warp of occupancy, lrdmc.cu plan_smem)
 #define LRDMC_FRAME_STRIDE 12  // doubles per prepared step: U [9], pad, u_sel, u_tau
 #define LRDMC_NUC_STRIDE 20  // doubles per nucleus row: Rx Ry Rz Z c1 b1 alpha beta gamma delta is_pp pad | r_c A0 B0 A1 B1 A2 B2 pad (non-local channels)
 #define LRDMC_NL_OFF 12      // first non-local entry of a nucleus row
@@ -72,6 +73,7 @@ struct DevSys {
     const double *srad;        // [n_slots] screening radii (LRDMC_LIST_THR); padded slots: -1e300 (never listed)
     const double *cn[2];       // [n_aop][OS] MO coefficients with the AO norms folded in, slot-major (Bc = C Dinv by rows)
     // shared-memory plan (units: doubles)
+    int frame_batch;                           // steps per prepared batch of draws / frames (power of two <= LRDMC_FRAME_BATCH)
     int bf_in_smem, moc_in_smem, cf_in_smem;   // cf_in_smem: the pair table of ao_columns is staged too (not with the listed sweep)
     int bfm_in_smem;                           // the fragment table `bf` of the mover's derivative pass is staged too (LRDMC_BF_SMEM: not with a three-body Jastrow)
     int off_shells, off_nuc, off_bf[2], off_etab, tables_doubles;

@@ -92,21 +92,25 @@ static int plan_smem(lrdmc_ctx *c)
     S.o_moc = (int)w; if (S.moc_in_smem) w += align_up(moc_doubles, 2);
     S.o_R = (int)w; w += align_up((size_t)S.P, 2);
     S.o_el = (int)w; w += align_up((size_t)LRDMC_EL_ARRAYS * S.N, 2);
-    S.o_U = (int)w; w += LRDMC_FRAME_BATCH * LRDMC_FRAME_STRIDE;   // prepared draws + lattice frames of LRDMC_FRAME_BATCH steps (propagate.cuh)
     S.o_ob = (int)w; w += 8 * (size_t)S.N;      // one-body cache: J1, grad J1, lap J1, v_ei, v^a_ei per electron
     S.o_j3 = (int)w; if (S.n_j3) w += (size_t)S.N * 2 * S.j3s + S.j3s;   // three-body Jastrow: chi3, V3, S3
     S.o_am = (int)w; if (c->listed) w += ((size_t)S.N * (S.lt + S.n_lg) + 7) / 8;       // listed-shell lists (listed.cuh)
-    S.per_warp_doubles = (int)w;
+    S.o_U = (int)w;                             // last: prepared draws + lattice frames of S.frame_batch steps (propagate.cuh prepare_frames)
     const size_t per_sm = prop.sharedMemPerMultiprocessor, per_blk_max = prop.sharedMemPerBlockOptin, reserve = 1024;
-    c->wpb = LRDMC_WPB;
-    for (;;) {
-        size_t need = ((size_t)S.tables_doubles + (size_t)c->wpb * S.per_warp_doubles) * 8;
-        if ((need + reserve) * LRDMC_MINB <= per_sm || c->wpb == 1) { c->smem_bytes = (int)need; break; }
-        --c->wpb;
-    }
-    // Warp w of a CTA issues from scheduler w mod 4, and the warps of a CTA meet at a barrier every step: with 7 (5) warps per CTA the fullest
-    // scheduler sets the pace of all -- 2 x 7 warps run at the pace of 16.  Measured (C3nl / C3j3, 7 -> 6 warps): 75.6 -> 71.7 ms, 61.4 -> 58.2 ms.
-    if (c->wpb == 7 || c->wpb == 5) { --c->wpb; c->smem_bytes = (int)(((size_t)S.tables_doubles + (size_t)c->wpb * S.per_warp_doubles) * 8); }
+    // warps per CTA that LRDMC_MINB CTAs of `pw` doubles per warp leave room for.  The hardware deals the warps of the resident CTAs round-robin over the
+    // 4 schedulers and the warps of a CTA meet at a barrier every step: with 7 (5) warps per CTA the fullest scheduler sets the pace of all -- 2 x 7 warps
+    // run at the pace of 16 -- so 7 and 5 are never chosen.  Measured (C3nl / C3j3, 7 -> 6 warps): 75.6 -> 71.7 ms, 61.4 -> 58.2 ms.
+    auto warps_for = [&](size_t pw) {
+        int n = LRDMC_WPB;
+        while (n > 1 && (((size_t)S.tables_doubles + (size_t)n * pw) * 8 + reserve) * LRDMC_MINB > per_sm) --n;
+        return (n == 7 || n == 5) ? n - 1 : n;
+    };
+    S.frame_batch = 1;                          // the largest batch of prepared frames that costs no warp of occupancy
+    c->wpb = warps_for(w + LRDMC_FRAME_STRIDE);
+    for (int fb = LRDMC_FRAME_BATCH; fb > 1; fb >>= 1) if (warps_for(w + (size_t)fb * LRDMC_FRAME_STRIDE) == c->wpb) { S.frame_batch = fb; break; }
+    w += (size_t)S.frame_batch * LRDMC_FRAME_STRIDE;
+    S.per_warp_doubles = (int)w;
+    c->smem_bytes = (int)(((size_t)S.tables_doubles + (size_t)c->wpb * S.per_warp_doubles) * 8);
     if ((size_t)c->smem_bytes > per_blk_max) return LRDMC_ENOMEM;
 #define SET_SMEM(K) CK(cudaFuncSetAttribute(K, cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem_bytes))
 #define SET_ALL(NTV, TSV, BFV) SET_SMEM((k_rebuild<NTV, TSV, BFV>))

@@ -60,12 +60,12 @@ __device__ __forceinline__ void publish_frame(const WarpState &ws, const StepDra
 
 // The draws and frames of the steps s0 .. s0 + LRDMC_FRAME_BATCH - 1 of walker `slot`, one LANE per step (they depend on (slot, cycle, step) alone): the
 // Philox rounds and the frame's sincos / sqrt sequences are warp instructions whichever lanes need them, so preparing four steps costs what one did.
-// fr = the warp's frame buffer [LRDMC_FRAME_BATCH][LRDMC_FRAME_STRIDE].
+// fr = the warp's frame buffer [S.frame_batch][LRDMC_FRAME_STRIDE].
 __device__ __forceinline__ void prepare_frames(const DevSys &S, double *fr, uint32_t slot, uint32_t cycle, uint32_t s0, bool need_tau, int lane)
 {
     __syncwarp();
-    const StepDraws d = step_draws(S, slot, cycle, s0 + (lane < LRDMC_FRAME_BATCH ? lane : 0), need_tau);
-    if (lane < LRDMC_FRAME_BATCH) {
+    const StepDraws d = step_draws(S, slot, cycle, s0 + (lane < S.frame_batch ? lane : 0), need_tau);
+    if (lane < S.frame_batch) {
         double U[9]; lattice_frame(d.u1, d.u2, d.u3, U);
         double *o = fr + lane * LRDMC_FRAME_STRIDE;
 #pragma unroll
@@ -151,8 +151,8 @@ __global__ void __launch_bounds__(WPBK * 32, LRDMC_MINB) k_propagate(DevSys S, D
         }
         if (LRDMC_LOCKSTEP) { if (!__syncthreads_or(have)) break; if (!have) continue; }
         else if (!have) break;
-        if ((s & (LRDMC_FRAME_BATCH - 1)) == 0) prepare_frames(S, frames, (uint32_t)k, cycle, s, mode == LRDMC_CONVENTIONAL, lane);
-        ws.U = frames + (s & (LRDMC_FRAME_BATCH - 1)) * LRDMC_FRAME_STRIDE;
+        if ((s & (S.frame_batch - 1)) == 0) prepare_frames(S, frames, (uint32_t)k, cycle, s, mode == LRDMC_CONVENTIONAL, lane);
+        ws.U = frames + (s & (S.frame_batch - 1)) * LRDMC_FRAME_STRIDE;
         StepDraws d; d.u_sel = ws.U[10]; d.u_tau = ws.U[11];
         const EvalOut e = evaluate_walker<NT, TS, EXT>(S, ws, T, lane);
         n_node += e.node;
