@@ -423,7 +423,8 @@ extern "C" size_t lrdmc_walker_bytes(const lrdmc_ctx *c, int n_walkers)
 // ---- team mode planning (team.cuh) ----------------------------------------------------------------------------------
 // Cut the sorted shell list into K parts of about equal cost.  Unit = two 4-shell iterations in groups 0-2 when `pairs`
 // (a part of ao_columns must start on a k-step pair), else one iteration; units go to parts by their cumulative cost.
-static void partition_shells(const int n_it[4], const double cost[4], bool pairs, int K, ShellPart *out)
+// `lead` is work part 0 has besides its shells, in the same cost units (the team's warp 0 also refreshes the one-body cache).
+static void partition_shells(const int n_it[4], const double cost[4], bool pairs, int K, ShellPart *out, double lead = 0.0)
 {
     struct Unit { int g, lo, hi; double c; };
     std::vector<Unit> units; double total = 0.0;
@@ -435,7 +436,7 @@ static void partition_shells(const int n_it[4], const double cost[4], bool pairs
         }
     }
     for (int k = 0; k < K; ++k) for (int g = 0; g < 4; ++g) out[k].lo[g] = out[k].hi[g] = 0;
-    double cum = 0.0;
+    double cum = lead; total += lead;
     for (const Unit &u : units) {
         int k = total > 0.0 ? (int)((cum + 0.5 * u.c) / total * K) : 0;
         if (k > K - 1) k = K - 1;
@@ -476,9 +477,11 @@ static void plan_team(lrdmc_ctx *c, int n_w)
     P.mesh_share = S.n_mesh == 2 && ((P.nblk[0] + P.nblk[1]) * np) % tw == 0;
     int lpe = 32; while (lpe > 1 && (tw * 32) / lpe < S.N) lpe >>= 1;     // largest power of two with one pass over the electrons
     P.lpe = lpe;
-    const double cost_col[4] = { 2.0, 1.0, 1.7, 2.9 }, cost_mo[4] = { 1.5, 1.0, 3.0, 6.0 };
+    // relative cost of a 4-shell iteration by group (s with one exponent per row, contracted s, p, d): measured on C3, N_w = 100 / 400, against
+    // the derivative pass of wavefunction.cuh (one product per row): 9.61 -> 10.33 and 27.65 -> 28.96 M walker-moves/s over the former { 1.5, 1, 3, 6 }
+    const double cost_col[4] = { 2.0, 1.0, 1.45, 2.1 }, cost_mo[4] = { 1.3, 1.0, 1.5, 2.2 };
     partition_shells(S.n_it, cost_col, true, np, P.col);
-    partition_shells(S.n_it, cost_mo, false, tw, P.mo);
+    partition_shells(S.n_it, cost_mo, false, tw, P.mo, 3.0);
     P.nblk_nl[0] = (S.n_up * S.nl_K + 7) / 8; P.nblk_nl[1] = (S.n_dn * S.nl_K + 7) / 8; P.n_units_nl = (P.nblk_nl[0] + P.nblk_nl[1]) * np;
     const size_t scr_lat = np > 1 ? (size_t)S.n_mesh * S.N * np * 12 : 0, scr_nl = np > 1 ? (size_t)S.N * S.nl_K * np * 12 : 0,
                  scr_nu = np > 1 ? (size_t)S.N * S.nl_K * 7 : 0, scr_col = scr_lat + scr_nl + scr_nu, scr_mo = (size_t)tw * 5 * S.OS;
