@@ -212,6 +212,28 @@ int lrdmc_launch_config(const lrdmc_ctx *, int *grid, int *block, int *smem_byte
 /* 1 if the candidate pass of this ctx is the listed sweep (LRDMC_OPT_LISTED, or automatic for global-table systems), else 0 */
 int lrdmc_listed_sweep(const lrdmc_ctx *);
 
+/* ---- allocation-free entry point (csrc/comb_static.cu) -------------------------------------------------------------------------
+ * The integer comb of the branching step alone (Eq.15-17, reading Q21: the arithmetic of lrdmc_reconfigure, bit for bit), for
+ * callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid it): no ctx, no walker
+ * buffer, and NO cudaMalloc / cudaFree / allocating library routine inside.  Its workspace (quantised weights and their prefix sums) is a
+ * static device array of LRDMC_COMB_STATIC_MAX_WALKERS x 16 bytes = 1 MiB that every GPU loading the library holds until exit.
+ *   w_dev       (device, in)  raw weights w [n_walkers]
+ *   seed, cycle the run seed (lrdmc_lattice.seed) and the cycle label (< 2^32): the comb offset xi is the same Philox draw
+ *               lrdmc_reconfigure(ctx, cycle) takes
+ *   parents_dev (device, out) parent[k] [n_walkers] int32; identity if a weight is negative / non-finite or all are zero
+ *   wbar_dev    (device, out, nullable) Eq.16 mean raw weight (0 in the degenerate case)
+ * Asynchronous on `stream`.  ALL calls share the one scratch array: calls that overlap on the GPU (different streams or host threads)
+ * race -- order them.  The array keeps the last call's contents; nothing in it has to be cleared (every call writes the entries it reads).
+ * Errors: LRDMC_EINVAL for NULL pointers, n_walkers < 1, cycle >= 2^32 and for n_walkers > LRDMC_COMB_STATIC_MAX_WALKERS (nothing is
+ * launched; use lrdmc_reconfigure for larger ensembles); LRDMC_ECUDA.  lrdmc_comb_static_error() returns the text of the calling thread's
+ * last failure ("" if the last call succeeded).  lrdmc_comb_static_setup() resolves the array's device address for the current device
+ * ahead of time (cudaGetSymbolAddress, once per device; lrdmc_comb_static does it on its first call otherwise). */
+#define LRDMC_COMB_STATIC_MAX_WALKERS 65536
+int lrdmc_comb_static(const double *w_dev, int n_walkers, uint64_t seed, uint64_t cycle, int32_t *parents_dev, double *wbar_dev,
+                      void *stream);
+int lrdmc_comb_static_setup(void);
+const char *lrdmc_comb_static_error(void);
+
 #ifdef __cplusplus
 }
 #endif

@@ -17,12 +17,14 @@ OK, EINVAL, ESINGULAR, ESTATE, ECUDA, ENOMEM = 0, -1, -2, -3, -4, -5
 
 PROBE_LIB_PATH = os.path.join(_HERE, "liblrdmc_probe.so")                     # include/lrdmc_probe.h (bench.py's roofline denominators)
 OPT_TEAM_WARPS, OPT_GLOBAL_TABLES, OPT_LISTED = 1, 2, 3
+COMB_STATIC_MAX_WALKERS = 65536                                               # LRDMC_COMB_STATIC_MAX_WALKERS
 
 # every symbol this module touches; tests check that include/lrdmc.h (resp. lrdmc_probe.h) declares each and the libraries export each
 EXPORTS = ["lrdmc_init", "lrdmc_free", "lrdmc_strerror", "lrdmc_last_error", "lrdmc_set_option", "lrdmc_n_candidates", "lrdmc_walker_bytes",
            "lrdmc_bind_walkers", "lrdmc_set_positions", "lrdmc_propagate", "lrdmc_reconfigure", "lrdmc_estimators", "lrdmc_energy",
            "lrdmc_step_debug", "lrdmc_get_walkers", "lrdmc_set_state", "lrdmc_get_obs", "lrdmc_run_host", "lrdmc_debug_philox",
-           "lrdmc_debug_draws", "lrdmc_launch_count", "lrdmc_launch_config", "lrdmc_listed_sweep"]
+           "lrdmc_debug_draws", "lrdmc_launch_count", "lrdmc_launch_config", "lrdmc_listed_sweep",
+           "lrdmc_comb_static", "lrdmc_comb_static_setup", "lrdmc_comb_static_error"]
 PROBE_EXPORTS = ["lrdmc_measure_fp64_peaks", "lrdmc_measure_fp64_operand_peak", "lrdmc_measure_fp64_shared_operand_peak"]
 
 
@@ -95,6 +97,9 @@ def load_library():
         L.lrdmc_launch_count.argtypes = [vp]
         L.lrdmc_launch_config.argtypes = [vp, C.POINTER(i32), C.POINTER(i32), C.POINTER(i32), C.POINTER(i32), C.POINTER(i32)]
         L.lrdmc_listed_sweep.argtypes = [vp]
+        L.lrdmc_comb_static.argtypes = [vp, i32, u64, u64, vp, vp, vp]
+        L.lrdmc_comb_static_setup.argtypes = []
+        L.lrdmc_comb_static_error.argtypes = []; L.lrdmc_comb_static_error.restype = C.c_char_p
         _lib = L
     return _lib
 
@@ -124,6 +129,24 @@ def lrdmc_energy(records, p=10, n_therm=0, n_blocks=20):
     E, sg = C.c_double(), C.c_double()
     _check(load_library().lrdmc_energy(arr, len(records), p, n_therm, n_blocks, C.byref(E), C.byref(sg)), "lrdmc_energy")
     return E.value, sg.value
+
+
+def lrdmc_comb_static(w, seed, cycle, want_wbar=True):
+    """include/lrdmc.h lrdmc_comb_static: the comb of the branching step with NO allocation inside the library (static device scratch,
+    at most COMB_STATIC_MAX_WALKERS walkers).  `w`: float64 CUDA tensor [n_w]; the two outputs are allocated HERE, by the caller's side.
+    Returns (parents int32 [n_w], wbar float64 [1] or None), both on w's device, asynchronous on torch's current stream."""
+    import torch
+    L = load_library()
+    if not (isinstance(w, torch.Tensor) and w.is_cuda and w.dtype == torch.float64 and w.dim() == 1 and w.is_contiguous()):
+        raise ValueError("lrdmc_comb_static: w must be a contiguous 1-d float64 CUDA tensor")
+    with torch.cuda.device(w.device):
+        par = torch.empty(w.shape[0], dtype=torch.int32, device=w.device)
+        wbar = torch.empty(1, dtype=torch.float64, device=w.device) if want_wbar else None
+        rc = L.lrdmc_comb_static(_ptr(w), int(w.shape[0]), int(seed), int(cycle), _ptr(par), _ptr(wbar),
+                                 C.c_void_p(torch.cuda.current_stream(w.device).cuda_stream))
+    if rc != 0:
+        raise RuntimeError(f"{L.lrdmc_comb_static_error().decode()} ({rc})")
+    return par, wbar
 
 
 _probe = None

@@ -3,7 +3,7 @@
     python -m paper_2508_12033_b200.build [--force] [-v]
 
 Translation units (compiled in parallel, then linked): lrdmc.cu (C-ABI, host logic, rebuild / reconfigure / reduction kernels),
-lrdmc_aux.cu (estimators over generations, host-buffer driver, test hooks) and kernels.cu ten times -- the walker kernels
+lrdmc_aux.cu (estimators over generations, host-buffer driver, test hooks), comb_static.cu (the allocation-free comb) and kernels.cu ten times -- the walker kernels
 {lattice only, + non-local pseudopotential slots, + three-body Jastrow, + both, lattice only as a listed sweep} x {warp-per-walker, team}.
 """
 from __future__ import annotations
@@ -18,7 +18,7 @@ LIB = os.path.join(HERE, "liblrdmc.so")
 PROBE_LIB = os.path.join(HERE, "liblrdmc_probe.so")      # include/lrdmc_probe.h: FP64 peak micro-benchmarks (bench.py only)
 OBJDIR = os.path.join(HERE, "build")
 # (source, object name, extra defines)
-UNITS = [("lrdmc.cu", "lrdmc.o", []), ("lrdmc_aux.cu", "lrdmc_aux.o", [])] + [
+UNITS = [("lrdmc.cu", "lrdmc.o", []), ("lrdmc_aux.cu", "lrdmc_aux.o", []), ("comb_static.cu", "comb_static.o", [])] + [
     ("kernels.cu", f"kernels_e{ext}_{'team' if team else 'warp'}.o", [f"-DLRDMC_EXT={ext}", f"-DLRDMC_TEAM_TU={team}"])
     for ext in (0, 1, 2, 3, 4) for team in (0, 1)]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC"]
