@@ -688,3 +688,73 @@ def test_malformed_nonlocal_and_contraction_inputs_are_rejected(B):
         with pytest.raises(B.LrdmcError) as e:
             B.Lrdmc(c)
         assert e.value.code == B.EINVAL, breakit
+
+
+# ------------------------------------------------------------------------------------------ random shapes x random options
+def _random_case(case):
+    """A seeded random system (electron counts 1..19 / 0..n_up, 1..6 nuclei, 3..39 shells; primitive or contracted basis; optionally a
+    second mesh, a local pseudopotential, non-local slots, a three-body Jastrow) with a random kernel choice (team size, global tables,
+    listed sweep), mode and ensemble size.  A sweep of 1000 such cases ran green on the B200 before these 24 were fixed as tests."""
+    rng = np.random.default_rng([2026, case])
+    while True:
+        n_up = int(rng.integers(1, 20)); n_dn = int(rng.integers(0, n_up + 1)); n_nuc = int(rng.integers(1, 7))
+        n_shell = int(rng.integers(max(3, (n_up + 3) // 2), 40)); seed = int(rng.integers(1, 10**6)); a2 = 0.0 if rng.random() < 0.7 else 0.3
+        try:
+            if rng.random() < 0.6:
+                s = wl.tiny_molecule(n_up, n_dn, n_nuc, n_shell, seed=seed, a=0.15 if a2 else 0.2, a2=a2, with_pp=bool(rng.integers(0, 2)))
+            else:
+                s = wl.contracted_molecule(n_up, n_dn, n_nuc, max(n_shell // 2, (n_up + 1) // 2 + 2), seed=seed, spherical=bool(rng.integers(0, 2)), with_pp=bool(rng.integers(0, 2)))
+        except Exception:
+            continue                                    # fewer basis functions than orbitals: draw again
+        break
+    ext = int(rng.integers(0, 4))
+    if ext & 1:
+        args = (int(rng.integers(2, 9)), int(rng.integers(1, 3)), bool(rng.integers(0, 2))); scale = float(rng.choice([1.0, 50.0, 200.0]))
+        s1 = wl.random_nonlocal(s, args[0], float(rng.uniform(0.5, 1.0)), args[1], args[2], scale=scale)
+        s = s1 if s1["nl_K"] <= 4 else wl.random_nonlocal(s, args[0], 0.5, args[1], args[2], scale=scale)      # disjoint spheres: one slot per electron
+    if ext & 2:
+        s = wl.with_jastrow3(s, int(rng.integers(2, 9)), int(rng.integers(1, 4)), strength=0.1, n_max=int(rng.choice([8, 12, 24])), poly=bool(rng.integers(0, 2)))
+    n_w = int(rng.integers(1, 60)); x0 = wl.initial_walkers(s, n_w, int(rng.integers(1, 100)))
+    opts = {}; tw = int(rng.choice([0, 1, 2, 4, 8, 16]))
+    if tw:
+        opts["OPT_TEAM_WARPS"] = tw
+    if rng.random() < 0.3:
+        opts["OPT_GLOBAL_TABLES"] = 1
+    if ext == 0 and rng.random() < 0.5:
+        opts["OPT_LISTED"] = 1
+    return s, x0, opts, ("balanced" if rng.random() < 0.5 else "conventional")
+
+
+@pytest.mark.parametrize("case", range(24))
+def test_random_shapes_and_options(B, case):
+    """One evaluation from the oracle's state and two whole cycles, as the fixed systems above.  Ratios are sums of phi x Dinv products, so their
+    scale is max(1, max|Dinv|) of the walker (random orbitals give near-singular Slater matrices now and then: conditioning, not arithmetic)."""
+    s, x0, opts, mode = _random_case(case)
+    N = s["n_up"] + s["n_dn"]; Kd = 3 * N * ((1 / s["a"]**2) if s["a2"] == 0 else (0.5 / s["a"]**2 + 0.5 / s["a2"]**2))
+    o = ref.Ref(s)
+    if o.set_positions(x0) != 0:
+        pytest.skip("a singular Slater matrix among the random walkers")
+    g = B.Lrdmc(s, options={getattr(B, k): v for k, v in opts.items()}); g.lrdmc_set_positions(x0)
+    r, du, dd, w = o.get_state(); g.lrdmc_set_state(r, du, dd, w)
+    cond = np.maximum(1.0, np.maximum(np.abs(du).max(axis=(1, 2)), np.abs(dd).max(axis=(1, 2)) if dd.size else 0.0))[:, None]
+    R, scal, js = o.step_debug(-3.0, 2, 1); gR, gscal, gjs = [np_(t) for t in g.lrdmc_step_debug(-3.0, 2, 1)]
+    assert np.max(np.abs(gR - R) / np.maximum(np.abs(R), cond)) < TOL
+    near_tie = scal[:, 7] < 1e-9
+    assert np.array_equal(gjs[~near_tie], js[~near_tie])
+    assert np.max(np.abs(gscal[:, :4] - scal[:, :4]) / np.maximum(np.abs(scal[:, :4]), Kd * cond)) < TOL
+    for cycle in range(2):
+        if mode == "balanced":
+            assert o.propagate(ref.BALANCED, 20, 0.0, -5.0, cycle) == 0; g.lrdmc_propagate(B.BALANCED, 20, 0.0, -5.0, cycle)
+        else:
+            tau = 20 * s["a"]**2 / (3 * N)
+            assert o.propagate(ref.CONVENTIONAL, 0, tau, -1.0, cycle) == 0; g.lrdmc_propagate(B.CONVENTIONAL, 0, tau, -1.0, cycle)
+        gr, gdu, gdd, gw = [np_(t) for t in g.lrdmc_get_walkers()]; geL, gW, gom, gnm = [np_(t) for t in g.lrdmc_get_obs()]
+        r, du, dd, w = o.get_state(); eL, W, om, nm = o.get_obs()
+        assert np.array_equal(gnm, nm) and np.abs(gr - r).max() < 1e-11
+        assert relerr(gw, w) < 1e-9 and relerr(gom, om) < 1e-9
+        rc, par = o.reconfigure(cycle); gpar = np_(g.lrdmc_reconfigure(cycle, want_parents=True))
+        assert np.array_equal(gpar, par)
+        so, sg = o.estimators(), g.lrdmc_estimators()
+        assert abs(sg.wbar - so["wbar"]) <= 1e-9 * so["wbar"]
+        assert (sg.n_node_flag, sg.n_nonpos_diag, sg.n_nonfinite) == (so["n_node_flag"], so["n_nonpos_diag"], so["n_nonfinite"])
+    g.close()
